@@ -1,0 +1,344 @@
+"""Pins of the float64 oracle (oracle/lcf_oracle.c) to things other than itself.
+
+The paper prints no reproducible worked example (its figure values need its private data), so the
+oracle is pinned to what the mathematics fixes: LAPACK (numpy eigh/svd/matmul, float64), closed
+forms, identities that follow from Eqs. 1-5, 9, 11-13, and a
+literal brute-force implementation of the paper's own data flow (form C_w = W C explicitly, as the
+paper does) on tiny inputs.  A dropped term, wrong sign, transposed or
+un-conjugated operand in any oracle step fails at least one test here.
+"""
+import numpy as np
+import pytest
+
+from paper_2405_11105_b200 import synth
+
+
+def cn(rng, shape):
+    return (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)) / np.sqrt(2)
+
+
+def casorati(iq):
+    """[N][Nx][Nz] -> C [P][N], row p = z + Nz*x."""
+    N = iq.shape[0]
+    return iq.reshape(N, -1).T.astype(np.complex128)
+
+
+def rand_herm(rng, n, cond=1e6):
+    q, _ = np.linalg.qr(cn(rng, (n, n)))
+    lam = np.logspace(0, -np.log10(cond), n)
+    return (q * lam) @ q.conj().T, lam, q
+
+
+# ---------------------------------------------------------------- windows (Eq. 11)
+def test_windows_support_lengths_config2(oracle):
+    # centres 15.5 + 32 k, |d| <= 72 on a 256 axis: supports counted by hand
+    g = oracle.axis_windows(256, 8, 24.0, 3.0)
+    assert [(row != 0).sum() for row in g] == [88, 120, 144, 144, 144, 144, 120, 88]
+    # peak of an interior window: nearest pixels are 0.5 px from the centre
+    assert np.isclose(g[3].max(), np.exp(-0.25 / (2 * 24.0 ** 2)), rtol=1e-15)
+
+
+def test_windows_symmetry_and_special_cases(oracle):
+    for n, K, s, t in [(64, 3, 16.0, 3.0), (100, 4, 10.0, 0.0), (37, 5, 3.0, 2.0)]:
+        g = oracle.axis_windows(n, K, s, t)
+        assert np.allclose(g, g[::-1, ::-1], rtol=1e-12, atol=0)          # grid is mirror symmetric
+        assert np.array_equal(g != 0, (g != 0)[::-1, ::-1])
+        assert g.max() <= 1.0 and g.min() >= 0.0
+        if t <= 0:
+            assert (g > 0).all()
+    assert np.array_equal(oracle.axis_windows(17, 1, 0.0, 0.0), np.ones((1, 17)))     # all-ones
+    # one pixel, centred exactly: c = 0.5*1/1 - 0.5 = 0 -> weight exp(0) = 1
+    assert oracle.axis_windows(1, 1, 5.0, 3.0)[0, 0] == 1.0
+    # centre of a 2-window grid on 8 px: c = 1.5, 5.5; value at i=0 of window 0 = exp(-1.5^2/(2*4))
+    g = oracle.axis_windows(8, 2, 2.0, 0.0)
+    assert np.isclose(g[0, 0], np.exp(-2.25 / 8.0), rtol=1e-15)
+    assert np.isclose(g[1, 7], np.exp(-2.25 / 8.0), rtol=1e-15)
+    # truncation is inclusive: |d| = 1.5 <= trunc*sigma = 1.5 kept, 2.5 dropped
+    g = oracle.axis_windows(8, 2, 1.5, 1.0)
+    assert g[0, 0] > 0 and g[0, 3] > 0 and g[0, 4] == 0
+
+
+# ---------------------------------------------------------------- Gram (Eqs. 1, 12)
+def test_gram_matches_blas_and_identities(oracle):
+    rng = np.random.default_rng(1)
+    N, Nx, Nz = 7, 9, 11
+    iq = cn(rng, (N, Nx, Nz)).astype(np.complex64)
+    gz = oracle.axis_windows(Nz, 2, 3.0, 2.0)
+    gx = oracle.axis_windows(Nx, 3, 2.0, 0.0)
+    Cm = casorati(iq)
+    Rsum = 0
+    for kz in range(2):
+        for kx in range(3):
+            w = (gx[kx][:, None] * gz[kz][None, :]).reshape(-1)
+            R = oracle.gram(iq, gz[kz], gx[kx])
+            ref = (Cm.conj().T * w ** 2) @ Cm                       # C^H diag(w^2) C
+            assert np.abs(R - ref).max() <= 1e-13 * np.abs(ref).max()
+            assert np.abs(R - R.conj().T).max() == 0.0               # exactly Hermitian
+            # trace(R) = sum_p w_p^2 ||s_p||^2
+            assert np.isclose(np.trace(R).real, (w ** 2 * (np.abs(Cm) ** 2).sum(1)).sum(), rtol=1e-13)
+            assert np.linalg.eigvalsh(R).min() >= -1e-12 * np.trace(R).real
+            Rsum = Rsum + R
+    wtot = sum(np.outer(gx[kx], gz[kz]).reshape(-1) ** 2 for kz in range(2) for kx in range(3))
+    assert np.abs(Rsum - (Cm.conj().T * wtot) @ Cm).max() <= 1e-12 * np.abs(Rsum).max()
+
+
+def test_gram_conjugation_convention(oracle):
+    # R[i][j] = sum conj(S_i) S_j : for one pixel with s = (1, i) -> R[0][1] = conj(1)*i = +i
+    iq = np.zeros((2, 1, 1), dtype=np.complex64)
+    iq[0, 0, 0] = 1.0
+    iq[1, 0, 0] = 1j
+    R = oracle.gram(iq, np.ones(1), np.ones(1))
+    assert R[0, 1] == 1j and R[1, 0] == -1j and R[0, 0] == 1 and R[1, 1] == 1
+
+
+# ---------------------------------------------------------------- EVD (Eqs. 2, 3)
+@pytest.mark.parametrize("n,cond", [(1, 1.0), (2, 10.0), (5, 1e3), (32, 1e7), (64, 1e10)])
+def test_jacobi_vs_lapack(oracle, n, cond):
+    rng = np.random.default_rng(n)
+    A, lam_true, _ = rand_herm(rng, n, cond)
+    A = (A + A.conj().T) / 2
+    lam, V, sweeps = oracle.jacobi(A)
+    w = np.linalg.eigvalsh(A)[::-1]
+    assert np.abs(lam - w).max() <= 1e-13 * abs(w).max()
+    assert (np.diff(lam) <= 0).all()                                   # sorted descending
+    assert np.abs(V.conj().T @ V - np.eye(n)).max() <= 1e-13           # unitary
+    assert np.linalg.norm(A @ V - V * lam) <= 1e-12 * np.linalg.norm(A)
+    if n >= 5:
+        # leading well-separated invariant subspace agrees with LAPACK's
+        _, U = np.linalg.eigh(A)
+        U = U[:, ::-1]
+        k = 3
+        assert np.linalg.norm(V[:, :k] @ V[:, :k].conj().T - U[:, :k] @ U[:, :k].conj().T) <= 1e-9
+
+
+def test_jacobi_2x2_closed_form(oracle):
+    a, b, al = 2.0, -1.0, 0.7 - 1.9j
+    A = np.array([[a, al], [np.conj(al), b]])
+    lam, V, _ = oracle.jacobi(A)
+    r = np.sqrt(((a - b) / 2) ** 2 + abs(al) ** 2)
+    assert np.allclose(lam, [(a + b) / 2 + r, (a + b) / 2 - r], rtol=1e-15, atol=1e-15)
+    assert np.linalg.norm(A @ V - V * lam) < 1e-14
+
+
+def test_jacobi_degenerate_inputs(oracle):
+    lam, V, sweeps = oracle.jacobi(np.zeros((4, 4), dtype=complex))
+    assert (lam == 0).all() and np.array_equal(V, np.eye(4)) and sweeps == 0
+    lam, V, _ = oracle.jacobi(np.diag([1.0, 3.0, 2.0]).astype(complex))
+    assert np.array_equal(lam, [3.0, 2.0, 1.0])
+    assert np.array_equal(np.abs(V), np.eye(3)[:, [1, 2, 0]])
+    # repeated eigenvalues: any orthonormal basis is right -> check residual only
+    q, _ = np.linalg.qr(cn(np.random.default_rng(0), (6, 6)))
+    A = (q * np.array([5, 5, 5, 1, 1, 0.0])) @ q.conj().T
+    lam, V, _ = oracle.jacobi((A + A.conj().T) / 2)
+    assert np.allclose(lam, [5, 5, 5, 1, 1, 0], atol=1e-13)
+    assert np.linalg.norm(A @ V - V * lam) < 1e-13
+
+
+def test_eigenvalues_are_squared_singular_values(oracle):
+    # Eq. 3: all-ones window -> lambda_i = sigma_i(C)^2
+    rng = np.random.default_rng(3)
+    iq = (cn(rng, (12, 6, 10)) * np.logspace(0, -3, 12)[:, None, None]).astype(np.complex64)
+    R = oracle.gram(iq, np.ones(10), np.ones(6))
+    lam, V, _ = oracle.jacobi(R)
+    sv = np.linalg.svd(casorati(iq), compute_uv=False)
+    assert np.abs(lam - sv ** 2).max() <= 1e-13 * sv[0] ** 2
+    # right singular vectors = eigenvectors (up to phase): compare rank-1 projectors of the top ones
+    _, _, Vh = np.linalg.svd(casorati(iq), full_matrices=False)
+    for i in range(4):
+        v = Vh[i].conj()
+        assert np.linalg.norm(np.outer(v, v.conj()) - np.outer(V[:, i], V[:, i].conj())) < 1e-8
+
+
+def test_unitary_temporal_mixing_leaves_spectrum(oracle):
+    rng = np.random.default_rng(4)
+    iq = cn(rng, (8, 5, 7)).astype(np.complex64)
+    Q, _ = np.linalg.qr(cn(rng, (8, 8)))
+    Cm = casorati(iq)
+    gz, gx = oracle.axis_windows(7, 1, 2.0, 0.0)[0], oracle.axis_windows(5, 1, 2.0, 0.0)[0]
+    w2 = np.outer(gx, gz).reshape(-1) ** 2
+    R1 = (Cm.conj().T * w2) @ Cm
+    C2 = Cm @ Q
+    R2 = (C2.conj().T * w2) @ C2
+    assert np.abs(oracle.gram(iq, gz, gx) - R1).max() < 1e-12
+    l1, _, _ = oracle.jacobi(R1)
+    l2, _, _ = oracle.jacobi((R2 + R2.conj().T) / 2)
+    assert np.abs(l1 - l2).max() <= 1e-12 * l1[0]
+
+
+# ---------------------------------------------------------------- cut-off and weights
+def test_energy_cutoff_bruteforce(oracle):
+    # hand-made spectra, rule: smallest 1-based m with cumulative energy > frac * total
+    assert oracle.cutoff_energy(np.array([90.0, 9.0, 0.9, 0.1]), 0.995) == 3      # 99.9 > 99.5
+    assert oracle.cutoff_energy(np.array([90.0, 9.0, 0.9, 0.1]), 0.90) == 2       # 90 is not > 90
+    assert oracle.cutoff_energy(np.array([90.0, 9.0, 0.9, 0.1]), 0.89) == 1
+    assert oracle.cutoff_energy(np.array([1.0, 1.0, 1.0, 1.0]), 0.5) == 3         # 2 is not > 2
+    assert oracle.cutoff_energy(np.array([1.0, 1.0, 1.0, 1.0]), 1.0) == 4         # never exceeds
+    assert oracle.cutoff_energy(np.array([10.0, 1.0, -5.0]), 0.95) == 2           # negatives clamp to 0
+    rng = np.random.default_rng(5)
+    for _ in range(50):
+        lam = np.sort(rng.random(9) ** 4)[::-1]
+        frac = rng.uniform(0.3, 0.999)
+        cum = [lam[:m].sum() for m in range(1, 10)]
+        want = next((m + 1 for m in range(9) if cum[m] > frac * lam.sum()), 9)
+        assert oracle.cutoff_energy(lam, frac) == want
+
+
+def test_weights_closed_forms(oracle):
+    assert np.array_equal(oracle.weights(6, False, 2, 0.5), [0, 0, 1, 1, 1, 1])
+    assert np.array_equal(oracle.weights(3, False, 0, 0.5), [1, 1, 1])
+    assert np.array_equal(oracle.weights(3, False, 3, 0.5), [0, 0, 0])
+    wt = oracle.weights(8, True, 3, np.log(3.0))                                      # Eq. 9
+    assert np.isclose(wt[2], 0.5, rtol=1e-15)            # i = k  -> 1/2
+    assert np.isclose(wt[3], 0.75, rtol=1e-15)           # i = k+1, e^-beta = 1/3 -> 3/4
+    assert np.isclose(wt[1], 0.25, rtol=1e-15)           # i = k-1 -> 1/4
+    assert np.isclose(wt[4], 0.9, rtol=1e-15)            # i = k+2, e^-2beta = 1/9 -> 9/10
+    assert (np.diff(wt) > 0).all()
+    assert np.allclose(wt[:5] + wt[:5][::-1], 1.0)     # sigmoid is odd about i = k
+    # beta -> infinity reproduces the hard weights except wt_k = 1/2
+    big = oracle.weights(6, True, 2, 1e3)
+    assert np.allclose(big, [0, 0.5, 1, 1, 1, 1], atol=1e-300)
+
+
+# ---------------------------------------------------------------- filter matrix (Eqs. 4, 5)
+def test_filter_projector_properties(oracle):
+    rng = np.random.default_rng(6)
+    n, c = 10, 3
+    A, _, _ = rand_herm(rng, n, 1e4)
+    lam, V, _ = oracle.jacobi((A + A.conj().T) / 2)
+    F = oracle.filter_matrix(V, oracle.weights(n, False, c, 0.5))
+    assert np.abs(F - F.conj().T).max() < 1e-14                       # Hermitian
+    assert np.abs(F @ F - F).max() < 1e-13                            # idempotent
+    assert np.isclose(np.trace(F).real, n - c, atol=1e-12)            # rank N - c
+    Pi_c = V[:, :c] @ V[:, :c].conj().T
+    assert np.abs(F - (np.eye(n) - Pi_c)).max() < 1e-13               # Eq. 4 == Eq. 5
+    # against LAPACK's invariant subspace: F kills the c dominant eigenvectors of A
+    _, U = np.linalg.eigh(A)
+    assert np.abs(U[:, -c:].conj().T @ F).max() < 1e-9
+    assert np.abs(oracle.filter_matrix(V, np.ones(n)) - np.eye(n)).max() < 1e-13      # keep all -> I
+    wt = rng.random(n)
+    assert np.abs(oracle.filter_matrix(V, wt) - (V * wt) @ V.conj().T).max() < 1e-14
+
+
+# ---------------------------------------------------------------- projection + PD
+def test_projection_allpass_and_trace_identity(oracle):
+    rng = np.random.default_rng(7)
+    N, Nx, Nz = 6, 8, 9
+    iq = cn(rng, (N, Nx, Nz)).astype(np.complex64)
+    gz, gx = oracle.axis_windows(Nz, 2, 3.0, 1.5)[1], oracle.axis_windows(Nx, 2, 2.5, 0.0)[0]
+    w2 = np.outer(gx, gz) ** 2
+    energy = (np.abs(iq.astype(np.complex128)) ** 2).sum(0)             # [Nx][Nz]
+    PD = oracle.project_pd(iq, gz, gx, np.eye(N, dtype=complex))
+    assert np.allclose(PD, w2 * energy, rtol=1e-13, atol=0)             # all components kept
+    assert (PD[w2 == 0] == 0).all() and (w2 == 0).any()
+    R = oracle.gram(iq, gz, gx)
+    lam, V, _ = oracle.jacobi(R)
+    for soft, c in [(False, 2), (True, 3)]:
+        wt = oracle.weights(N, soft, c, 0.8)
+        PD = oracle.project_pd(iq, gz, gx, oracle.filter_matrix(V, wt))
+        # sum_p PD_k(p) = trace(F^H R F) = sum_i wt_i^2 lambda_i
+        assert np.isclose(PD.sum(), (wt ** 2 * lam).sum(), rtol=1e-12)
+
+
+def test_rank_r_clutter_is_removed(oracle):
+    # exact rank-r clutter, zero blood: removing r components leaves round-off.  Fails if the Gram
+    # and the projection disagree on which operand is conjugated (R-bar has conjugate eigenvectors).
+    r, N = 3, 8
+    iq = synth.rank_r_clutter(10, 7, N, r, seed=11)
+    gz, gx = oracle.axis_windows(10, 1, 4.0, 0.0)[0], oracle.axis_windows(7, 1, 3.0, 0.0)[0]
+    res = oracle.window(iq, gz, gx, oracle.HARD_FIXED, k_fixed=r)
+    total = oracle.project_pd(iq, gz, gx, np.eye(N, dtype=complex)).sum()
+    # complex64 storage of S = A B^H leaves a rank-deficiency error of ~1e-7 relative amplitude
+    assert res["PDk"].sum() <= 1e-12 * total
+    res2 = oracle.window(iq, gz, gx, oracle.HARD_FIXED, k_fixed=r - 1)
+    assert res2["PDk"].sum() > 1e-4 * total                     # one clutter component left
+
+
+def test_dc_removal_textbook_case(oracle):
+    # constant-in-time tissue on half the pixels, a pure slow-time tone (integer cycles, so orthogonal
+    # to DC) on the other half: R = |T|^2 11^H + |b|^2 u u^H exactly, v1 = 1/sqrt(N), and removing c = 1
+    # component is the classical DC-removal (mean-subtraction) clutter filter.
+    rng = np.random.default_rng(8)
+    N, Nx, Nz = 16, 6, 6
+    tissue = cn(rng, (1, Nx, Nz)) * 100.0
+    tissue[:, :, 3:] = 0
+    blood = cn(rng, (1, Nx, Nz))
+    blood[:, :, :3] = 0
+    tone = np.exp(2j * np.pi * 3 * np.arange(N) / N)[:, None, None]
+    iq = (tissue + blood * tone).astype(np.complex64)
+    res = oracle.window(iq, np.ones(Nz), np.ones(Nx), oracle.HARD_FIXED, k_fixed=1)
+    s = iq.astype(np.complex128)
+    ref = (np.abs(s - s.mean(0, keepdims=True)) ** 2).sum(0)
+    assert np.allclose(res["PDk"], ref, rtol=1e-5, atol=1e-9 * ref.max())
+    assert np.allclose(res["PDk"][:, 3:], N * np.abs(blood[0, :, 3:]) ** 2, rtol=1e-5)
+    assert np.allclose(np.abs(res["V"][:, 0]), 1 / np.sqrt(N), rtol=1e-6)
+
+
+def _bruteforce_window(iq, w, soft, c, beta):
+    """The paper's own data flow, literally: C_w = W C (Eq. 11), R = C_w^H C_w (Eq. 12), EVD (Eq. 2,
+    LAPACK), C^ = C_w V L^ V^H (Eq. 4), PD = sum_t |C^|^2."""
+    Cm = casorati(iq)
+    Cw = w.reshape(-1, 1) * Cm
+    R = Cw.conj().T @ Cw
+    lam, V = np.linalg.eigh(R)
+    lam, V = lam[::-1], V[:, ::-1]
+    i = np.arange(1, len(lam) + 1)
+    wt = 1 / (1 + np.exp(-beta * (i - c))) if soft else (i > c).astype(float)
+    Chat = Cw @ (V * wt) @ V.conj().T
+    return (np.abs(Chat) ** 2).sum(1).reshape(iq.shape[1:]), lam
+
+
+def test_bruteforce_tiny_localized(oracle):
+    # 3 x 2 px, N = 3, K = 2 windows (and a slightly larger case), whole path vs the literal version
+    for (Nz, Nx, N, Kz, Kx, sg, tr, soft, c, seed) in [(3, 2, 3, 2, 1, 1.0, 0.0, False, 1, 0),
+                                                        (6, 5, 4, 2, 2, 2.0, 1.2, True, 2, 1),
+                                                        (6, 5, 4, 2, 2, 2.0, 1.2, False, 2, 2)]:
+        iq = synth.random_cube(Nz, Nx, N, seed)
+        iq = (iq * np.array([30.0, 5.0, 1.0, 0.2])[:N, None, None]).astype(np.complex64)
+        mode = oracle.SOFT_FIXED if soft else oracle.HARD_FIXED
+        out = oracle.run(iq, Kz, Kx, sg, sg, tr, mode, k_fixed=c, beta=0.7)
+        gz, gx = oracle.axis_windows(Nz, Kz, sg, tr), oracle.axis_windows(Nx, Kx, sg, tr)
+        PD = np.zeros((Nx, Nz))
+        for kx in range(Kx):
+            for kz in range(Kz):
+                pdk, lam = _bruteforce_window(iq, np.outer(gx[kx], gz[kz]), soft, c, 0.7)
+                assert np.allclose(out["lam"][kx * Kz + kz], lam, rtol=0, atol=1e-12 * lam[0])
+                PD += pdk / pdk.mean()
+        assert np.allclose(out["PD"], PD, rtol=1e-9)
+
+
+# ---------------------------------------------------------------- combination (Eq. 13)
+def test_combine_properties(oracle):
+    rng = np.random.default_rng(9)
+    pk = rng.random((4, 5, 6))
+    pk[2] = 0.0                                            # a window with zero flow power -> alpha = 0
+    PD, alpha = oracle.combine(pk)
+    assert alpha[2] == 0.0
+    assert np.allclose(alpha[[0, 1, 3]], 1.0 / pk[[0, 1, 3]].mean(axis=(1, 2)))
+    assert np.isclose(PD.sum(), 30 * 3)                    # each alpha_k PD_k has unit mean
+    PD2, _ = oracle.combine(pk * np.array([3.0, 0.1, 7.0, 100.0])[:, None, None])
+    assert np.allclose(PD, PD2)                            # per-window amplitude scaling cancels
+    PD3, _ = oracle.combine(np.stack([pk[0]] * 3))
+    assert np.allclose(PD3, 3 * pk[0] / pk[0].mean())      # K identical windows -> K x single
+
+
+def test_run_invariances_and_composition(oracle):
+    cfg = synth.scaled_config(synth.baseline_configs()[0], Nz=24, Nx=20, N=8, n_frames=8)
+    iq = synth.generate(cfg)
+    f = cfg.filt
+    a = oracle.run(iq, 2, 2, 6.0, 5.0, 2.0, oracle.SOFT_ENERGY, frac=0.9, beta=0.5)
+    b = oracle.run((iq * (0.3 - 2.0j)).astype(np.complex64), 2, 2, 6.0, 5.0, 2.0, oracle.SOFT_ENERGY, frac=0.9, beta=0.5)
+    assert np.allclose(a["PD"], b["PD"], rtol=1e-5)                  # S -> cS leaves PD_final unchanged
+    assert np.isclose(a["PD"].sum(), 4 * iq.shape[1] * iq.shape[2], rtol=1e-12)
+    # run() == per-step functions composed by hand
+    gz, gx = oracle.axis_windows(24, 2, 6.0, 2.0), oracle.axis_windows(20, 2, 5.0, 2.0)
+    pks = []
+    for kx in range(2):
+        for kz in range(2):
+            R = oracle.gram(iq, gz[kz], gx[kx])
+            lam, V, _ = oracle.jacobi(R)
+            c = oracle.cutoff_energy(lam, 0.9)
+            assert c == a["c"][kx * 2 + kz]
+            F = oracle.filter_matrix(V, oracle.weights(8, True, c, 0.5))
+            pks.append(oracle.project_pd(iq, gz[kz], gx[kx], F))
+    PD, _ = oracle.combine(np.stack(pks))
+    assert np.allclose(PD, a["PD"], rtol=1e-12)
