@@ -1,0 +1,129 @@
+/*
+ * lcf.h -- C ABI of liblcf.so: the B200 (sm_100a) localized spatiotemporal EVD clutter filter.
+ *
+ * One call of lcf_filter() runs, for one slow-time ensemble, the whole hot path of
+ * arXiv 2405.11105 (Huang et al.), cited below as PAPER.md:<line> of the extracted text:
+ *
+ *   a1  window-weighted temporal covariances   R_k = S^H diag(w_k^2) S        Eqs. 1, 11, 12
+ *                                                                              PAPER.md:41-46, 138-152
+ *   a2  batched Hermitian eigendecomposition   R_k = V_k Lambda_k V_k^H       Eq. 2
+ *   a3  eigen-weights and projector factor     wt (hard cut / sigmoid), B_k = V_k diag(wt)
+ *                                                                              PAPER.md:57-59, Eq. 9 :111-118
+ *   a4  projection + power Doppler             PD_k(p) = w_k(p)^2 sum_t |(s_p V_k diag(wt) V_k^H)_t|^2
+ *                                                                              Eq. 4
+ *   a5  recombination                          PD = sum_k PD_k / mean_p(PD_k)  Eq. 13
+ *
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback.  All functions return an
+ * lcf_status; none throws, aborts or prints.  Pointers are marked HOST or DEVICE.
+ *
+ * Data layout (the Casorati matrix of an Ny x Nx x Nt MATLAB cube, z fastest):
+ *   iq  DEVICE, complex64 interleaved (re, im), C order [N][Nx][Nz]: frame t, lateral x, axial z.
+ *       Casorati row p = z + Nz*x, column = frame.  16-byte aligned.  Read only.
+ *   pd  DEVICE, float32 [Nx][Nz].  Overwritten.
+ *   Window index k = kx*Kz + kz.
+ */
+#ifndef LCF_H_
+#define LCF_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lcf_plan lcf_plan; /* opaque; owns window tables and all device workspace */
+
+typedef enum {
+    LCF_OK = 0,
+    LCF_ERR_INVALID_ARG = 1,   /* NULL pointer, non-positive size, bad mode/parameter            */
+    LCF_ERR_UNSUPPORTED = 2,   /* N beyond what the EVD kernel holds in shared memory            */
+    LCF_ERR_ALLOC = 3,         /* device or host allocation failed                                */
+    LCF_ERR_CUDA = 4,          /* a CUDA call or launch failed (sticky per plan)                  */
+    LCF_ERR_NOT_CONVERGED = 5  /* some window's Jacobi iteration hit the sweep cap unconverged    */
+} lcf_status;
+
+/* Gaussian window grid (Eq. 11; centre/SD formulas are not given in the paper,
+ * DESIGN.md "Readings"): per axis, centre c_k = (k + 1/2) n / K - 1/2 (0-based
+ * pixels), g(i) = exp(-(i - c_k)^2 / (2 sigma^2)) for |i - c_k| <= trunc_sigmas * sigma, else 0;
+ * w_k(z, x) = g_z(z) g_x(x).  sigma <= 0 on an axis: g = 1 on that axis (all-ones window).
+ * trunc_sigmas <= 0: no truncation.  Evaluated in double precision. */
+typedef struct {
+    int Kz, Kx;
+    float sigma_z, sigma_x;
+    float trunc_sigmas;
+} lcf_windows;
+
+typedef enum {
+    LCF_HARD_FIXED = 0,  /* wt_i = 0 for i <= k_fixed, 1 above (i is 1-based)          */
+    LCF_HARD_ENERGY = 1, /* hard, c = min{m : sum_{i<=m} max(l_i,0) > energy_frac * sum_i max(l_i,0)}*/
+    LCF_SOFT_FIXED = 2,  /* wt_i = 1 / (1 + exp(-beta (i - k_fixed)))  (Eq. 9)     */
+    LCF_SOFT_ENERGY = 3  /* sigmoid centred on the energy-rule c                                     */
+} lcf_thresh_mode;
+
+typedef struct {
+    int mode;           /* lcf_thresh_mode                                                      */
+    int k_fixed;        /* 0 <= k_fixed <= N (FIXED modes)                                      */
+    double energy_frac; /* in (0, 1) (ENERGY modes)                                             */
+    double beta;        /* > 0 (SOFT modes)                                                     */
+    int precision;      /* 0: fp32 Gram + fp32 EVD.  1: exact-product fp64 Gram + fp64 EVD
+                           (single precision can hamper the EVD).  The projection
+                           is fp32 in both.                                                     */
+} lcf_thresh;
+
+/* Builds window tables, the work decomposition and all device workspace on the current CUDA device.
+ * Nz, Nx, N >= 1 (N >= 2).  *out is set to NULL on failure.  Synchronous (allocates, copies). */
+lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, const lcf_windows* win,
+                           const lcf_thresh* thr);
+
+/* Enqueues the whole path on `stream` (a cudaStream_t passed as void*; NULL = default stream) and
+ * returns without synchronising; no allocation, no host<->device copy.  One call in flight per plan
+ * (the workspace is shared): use one plan per stream to pipeline.  iq_dev and pd_dev must not
+ * alias.  Returns LCF_ERR_CUDA if a launch failed. */
+lcf_status lcf_filter(lcf_plan* plan, const void* iq_dev, float* pd_dev, void* stream);
+
+/* Same path with HOST buffers (pinned or pageable): copies iq_host -> plan-owned device staging,
+ * filters, copies the image back and synchronises `stream`.  The staging buffers are allocated on
+ * first use (LCF_ERR_ALLOC on failure). */
+lcf_status lcf_filter_host(lcf_plan* plan, const void* iq_host, float* pd_host, void* stream);
+
+/* Frees everything.  lcf_plan_destroy(NULL) is a no-op returning LCF_OK. */
+lcf_status lcf_plan_destroy(lcf_plan* plan);
+
+/* ---- diagnostics for the parity harness.  Each synchronises the plan's last stream, copies
+ * device -> HOST and describes the most recent lcf_filter call.  They return
+ * LCF_ERR_NOT_CONVERGED (after filling the output) if any window's EVD did not converge. ---- */
+int lcf_num_windows(const lcf_plan* plan);                         /* K = Kz*Kx (0 if plan NULL) */
+lcf_status lcf_get_eigenvalues(lcf_plan* plan, double* lam /* HOST [K][N], descending */);
+lcf_status lcf_get_cutoffs(lcf_plan* plan, int* c /* HOST [K]: rejected components per window */);
+lcf_status lcf_get_sweeps(lcf_plan* plan, int* sweeps /* HOST [K]: Jacobi sweeps used */);
+lcf_status lcf_get_gram(lcf_plan* plan, double* R /* HOST [K][N][N][2], R[i][j] as in Eq. 12 */);
+/* V[a][i] = component a of the eigenvector of the i-th largest eigenvalue */
+lcf_status lcf_get_eigenvectors(lcf_plan* plan, double* V /* HOST [K][N][N][2] */);
+/* wt[i] = weight of the i-th largest eigenvalue (0-based storage of the paper's 1-based i) */
+lcf_status lcf_get_weights(lcf_plan* plan, double* wt /* HOST [K][N] */);
+/* F_k = V diag(wt) V^H (Eq. 4), built on the device from V and wt */
+lcf_status lcf_get_filters(lcf_plan* plan, double* F /* HOST [K][N][N][2] */);
+/* m_k = mean over the full field of view of PD_k (Eq. 13's 1/alpha_k) */
+lcf_status lcf_get_window_means(lcf_plan* plan, double* m /* HOST [K] */);
+
+/* ---- measurement helpers ---- */
+/* Device time in ms of each stage of the most recent lcf_filter call when the plan has timing
+ * enabled: [gram, evd, weights_projector, projection, combine].  Enabling timing records CUDA
+ * events on the caller's stream between the launches (no synchronisation in lcf_filter). */
+lcf_status lcf_set_timing(lcf_plan* plan, int enabled);
+lcf_status lcf_get_stage_ms(lcf_plan* plan, float ms[5] /* HOST */);
+/* Algorithmic work of one lcf_filter call: Hermitian-half Gram flops,
+ * projection flops, compulsory HBM bytes, sum_k P_k, kernel launches per call. */
+typedef struct {
+    double gram_flops, proj_flops, hbm_bytes, sum_Pk;
+    int launches;
+} lcf_work;
+lcf_status lcf_get_work(const lcf_plan* plan, lcf_work* out /* HOST */);
+/* Arithmetic-pipe microbenchmark on the current device: kind 0 = FP32 FFMA, 1 = FP32 packed
+ * FFMA2 (fma.rn.f32x2), 2 = FP64 DFMA.  Writes achieved TFLOP/s (2 flops per FMA lane). */
+lcf_status lcf_measure_peak(int kind, double* tflops /* HOST */);
+
+const char* lcf_status_string(lcf_status s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LCF_H_ */

@@ -1,0 +1,123 @@
+// lcf_internal.h -- plan layout and kernel launchers shared by the liblcf.so translation units.
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstddef>
+#include <cstdint>
+#include <vector>
+
+#include "../../include/lcf.h"
+
+namespace lcf {
+
+// ---- window geometry (Eq. 11; truncation/centres: DESIGN.md "Readings") ----
+struct WinBox {      // support box of window k = kx*Kz + kz, and where its PD tile lives
+    int z0, Lz;      // axial support [z0, z0+Lz)
+    int x0, Lx;      // lateral support [x0, x0+Lx)
+    int kz, kx;
+    int Pk;          // Lz*Lx
+    int pad_;
+    long long tile_off;  // offset (floats) of this window's PD_k tile [Lx][Lz] in the tile buffer
+};
+
+// One Gram CTA: window k, flattened box pixels q in [q0, q1) (q = (x-x0)*Lz + (z-z0)), tile batch.
+struct GramItem {
+    int k, q0, q1, batch, pslot;
+};
+// One projection CTA: window k, box pixels [q0, q1) with q1-q0 <= PROJ_TPIX.
+struct ProjItem {
+    int k, q0, q1;
+};
+
+constexpr int GRAM_TP = 32;        // pixels per shared-memory tile of the Gram kernel
+constexpr int GRAM_THREADS = 160;  // max thread tiles per Gram CTA (136 upper tiles at N=128)
+constexpr int PROJ_TPIX = 64;      // pixels per projection CTA
+constexpr int PROJ_KT = 16;        // frames per pipeline stage of the projection kernel
+constexpr int PROJ_STAGES = 3;
+constexpr int VB_WARPS = 8;        // warps per CTA of the weights/projector kernel
+constexpr int VB_ROWS = 2;         // rows of V per warp
+
+struct StageTimer {
+    cudaEvent_t ev[6];
+    bool have = false;
+};
+
+}  // namespace lcf
+
+struct lcf_plan {
+    int Nz = 0, Nx = 0, N = 0, Kz = 0, Kx = 0, K = 0;
+    long long P = 0;
+    lcf_windows win{};
+    lcf_thresh thr{};
+    int prec = 0;            // 0 fp32, 1 fp64 (Gram, Jacobi, V)
+    int NP = 0, Ns = 0;      // rotation pairs per Jacobi step, slots (= 2*NP >= N)
+    int max_sweeps = 0;
+    size_t esz = 4;          // sizeof(real) of the Gram/EVD precision
+
+    // host copies
+    std::vector<double> gz_h, gx_h;      // [Kz][Nz], [Kx][Nx]
+    std::vector<lcf::WinBox> box_h;      // [K]
+    std::vector<int> pfirst_h;           // [K+1] first projection item of window k
+    std::vector<int> gfirst_h;           // [K+1] first Gram partial slot of window k
+    long long sumPk = 0;
+
+    // device: tables
+    double *gz_d = nullptr, *gx_d = nullptr;
+    lcf::WinBox* box_d = nullptr;
+    int *kzlo_d = nullptr, *kzhi_d = nullptr, *kxlo_d = nullptr, *kxhi_d = nullptr;  // per pixel coord
+    // Gram
+    lcf::GramItem* gitems_d = nullptr;
+    int n_gitems = 0, n_gslots = 0, gram_Tn = 0, gram_TM = 0, gram_tiles_per_batch = 0, gram_batches = 0;
+    int* gfirst_d = nullptr;
+    void* gpart_d = nullptr;   // [n_gslots][N][N] complex real
+    void* R_d = nullptr;       // [K][N][N] complex real (full Hermitian)
+    // EVD
+    void* rotlog_d = nullptr;  // [K][max_sweeps*(Ns-1)][3][NP] real
+    double* lam_d = nullptr;   // [K][N] descending
+    int* order_d = nullptr;    // [K][N] slot of the i-th largest eigenvalue
+    int* cut_d = nullptr;      // [K]
+    int* sweeps_d = nullptr;   // [K]
+    int* conv_d = nullptr;     // [K] 1 = converged
+    float* wslot_d = nullptr;  // [K][Ns] weight of the eigenvector sitting in slot s
+    double* wslot_dd_d = nullptr;  // [K][Ns] same, double (diagnostic filter build)
+    double* wt_d = nullptr;    // [K][N] weight by rank
+    void* V_d = nullptr;       // [K][N][Ns] complex real, slot order
+    float2* B_d = nullptr;     // [K][N][Ns] complex float: V diag(wslot)
+    // projection / combine
+    lcf::ProjItem* pitems_d = nullptr;
+    int n_pitems = 0;
+    int* pfirst_d = nullptr;
+    float* tiles_d = nullptr;  // [sumPk]
+    float* tsum_d = nullptr;   // [n_pitems]
+    double* mean_d = nullptr;  // [K]
+    float* alpha_d = nullptr;  // [K]
+    double* F_d = nullptr;     // [K][N][N][2] (diagnostic, allocated on demand)
+    // host staging for lcf_filter_host
+    void* iq_stage_d = nullptr;
+    float* pd_stage_d = nullptr;
+
+    cudaStream_t last_stream = nullptr;
+    bool ran = false;
+    bool cuda_failed = false;
+    bool timing = false;
+    lcf::StageTimer timer;
+    int smem_optin = 0;
+    int num_sms = 0;
+    // launch geometry decided at create
+    int jac_threads = 0, jac_bpt = 0;
+    size_t jac_smem = 0, gram_smem = 0, proj_smem = 0;
+    int proj_threads = 0, proj_nct = 0;
+};
+
+namespace lcf {
+// each returns the cudaError_t of configuring/launching; kernels are asynchronous on `st`
+cudaError_t launch_gram(lcf_plan* p, const float2* iq, cudaStream_t st);
+cudaError_t launch_jacobi(lcf_plan* p, cudaStream_t st);
+cudaError_t launch_vbuild(lcf_plan* p, cudaStream_t st);
+cudaError_t launch_project(lcf_plan* p, const float2* iq, cudaStream_t st);
+cudaError_t launch_combine(lcf_plan* p, float* pd, cudaStream_t st);
+cudaError_t launch_build_filters(lcf_plan* p, cudaStream_t st);
+cudaError_t configure_gram(lcf_plan* p);     // each: opt-in shared memory size, launch geometry
+cudaError_t configure_evd(lcf_plan* p);
+cudaError_t configure_project(lcf_plan* p);
+}  // namespace lcf

@@ -1,0 +1,424 @@
+// lcf_plan.cu -- the C ABI of liblcf.so (include/lcf.h): plan construction (window tables of
+// Eq. 11, work decomposition, workspace), lcf_filter (enqueues the kernels of
+// steps a1..a5), diagnostics getters.  Host code only builds tables and moves bytes; every step of
+// the path runs in the kernels of lcf_gram.cu / lcf_evd.cu / lcf_project.cu.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "lcf_internal.h"
+
+using namespace lcf;
+
+namespace {
+
+template <typename T>
+bool dev_alloc(T** p, size_t count) {
+    *p = nullptr;
+    if (count == 0) count = 1;
+    return cudaMalloc(reinterpret_cast<void**>(p), count * sizeof(T)) == cudaSuccess;
+}
+template <typename T>
+bool dev_upload(T** p, const std::vector<T>& h) {
+    if (!dev_alloc(p, h.size())) return false;
+    if (h.empty()) return true;
+    return cudaMemcpy(*p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice) == cudaSuccess;
+}
+
+// One axis of the window grid (Eq. 11; centres at cell centres, inclusive box truncation).
+void axis_windows(int n, int K, double sigma, double trunc, std::vector<double>& g, std::vector<int>& lo,
+                  std::vector<int>& hi) {
+    g.assign((size_t)K * n, 0.0);
+    lo.assign(K, 0);
+    hi.assign(K, -1);
+    for (int k = 0; k < K; ++k) {
+        const double c = (k + 0.5) * (double)n / (double)K - 0.5;
+        int l = n, h = -1;
+        for (int i = 0; i < n; ++i) {
+            double v;
+            if (sigma <= 0.0) v = 1.0;
+            else {
+                const double d = (double)i - c;
+                if (trunc > 0.0 && std::fabs(d) > trunc * sigma) v = 0.0;
+                else v = std::exp(-(d * d) / (2.0 * sigma * sigma));
+            }
+            g[(size_t)k * n + i] = v;
+            if (v != 0.0) { if (i < l) l = i; if (i > h) h = i; }
+        }
+        // a Gaussian that underflows to 0 inside its box leaves holes; the box [l, h] still covers it
+        lo[k] = l; hi[k] = h;
+    }
+}
+
+void free_plan_device(lcf_plan* p) {
+    cudaFree(p->gz_d); cudaFree(p->gx_d); cudaFree(p->box_d);
+    cudaFree(p->kzlo_d); cudaFree(p->kzhi_d); cudaFree(p->kxlo_d); cudaFree(p->kxhi_d);
+    cudaFree(p->gitems_d); cudaFree(p->gfirst_d); cudaFree(p->gpart_d); cudaFree(p->R_d);
+    cudaFree(p->rotlog_d); cudaFree(p->lam_d); cudaFree(p->order_d); cudaFree(p->cut_d);
+    cudaFree(p->sweeps_d); cudaFree(p->conv_d); cudaFree(p->wslot_d); cudaFree(p->wslot_dd_d); cudaFree(p->wt_d);
+    cudaFree(p->V_d); cudaFree(p->B_d); cudaFree(p->pitems_d); cudaFree(p->pfirst_d);
+    cudaFree(p->tiles_d); cudaFree(p->tsum_d); cudaFree(p->mean_d); cudaFree(p->alpha_d);
+    cudaFree(p->F_d); cudaFree(p->iq_stage_d); cudaFree(p->pd_stage_d);
+    if (p->timer.have)
+        for (auto& e : p->timer.ev) cudaEventDestroy(e);
+}
+
+lcf_status sync_plan(lcf_plan* p) {
+    if (!p) return LCF_ERR_INVALID_ARG;
+    if (!p->ran) return LCF_ERR_INVALID_ARG;
+    if (cudaStreamSynchronize(p->last_stream) != cudaSuccess) { p->cuda_failed = true; return LCF_ERR_CUDA; }
+    return LCF_OK;
+}
+
+lcf_status conv_status(lcf_plan* p) {
+    std::vector<int> cv(p->K);
+    if (cudaMemcpy(cv.data(), p->conv_d, sizeof(int) * p->K, cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    for (int v : cv)
+        if (!v) return LCF_ERR_NOT_CONVERGED;
+    return LCF_OK;
+}
+
+}  // namespace
+
+extern "C" const char* lcf_status_string(lcf_status s) {
+    switch (s) {
+        case LCF_OK: return "ok";
+        case LCF_ERR_INVALID_ARG: return "invalid argument";
+        case LCF_ERR_UNSUPPORTED: return "unsupported size (EVD matrix does not fit shared memory)";
+        case LCF_ERR_ALLOC: return "allocation failed";
+        case LCF_ERR_CUDA: return "CUDA error";
+        case LCF_ERR_NOT_CONVERGED: return "EVD did not converge";
+    }
+    return "unknown status";
+}
+
+extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, const lcf_windows* win,
+                                      const lcf_thresh* thr) {
+    if (!out) return LCF_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!win || !thr) return LCF_ERR_INVALID_ARG;
+    if (Nz < 1 || Nx < 1 || N < 2 || win->Kz < 1 || win->Kx < 1) return LCF_ERR_INVALID_ARG;
+    if ((long long)Nz * Nx > (1LL << 30) || (long long)win->Kz * win->Kx > 65535) return LCF_ERR_INVALID_ARG;
+    if (thr->mode < 0 || thr->mode > 3 || (thr->precision != 0 && thr->precision != 1)) return LCF_ERR_INVALID_ARG;
+    const bool fixed = thr->mode == LCF_HARD_FIXED || thr->mode == LCF_SOFT_FIXED;
+    const bool soft = thr->mode == LCF_SOFT_FIXED || thr->mode == LCF_SOFT_ENERGY;
+    if (fixed && (thr->k_fixed < 0 || thr->k_fixed > N)) return LCF_ERR_INVALID_ARG;
+    if (!fixed && !(thr->energy_frac > 0.0 && thr->energy_frac < 1.0)) return LCF_ERR_INVALID_ARG;
+    if (soft && !(thr->beta > 0.0)) return LCF_ERR_INVALID_ARG;
+    if (!std::isfinite(win->sigma_z) || !std::isfinite(win->sigma_x) || !std::isfinite(win->trunc_sigmas))
+        return LCF_ERR_INVALID_ARG;
+
+    lcf_plan* p = new (std::nothrow) lcf_plan();
+    if (!p) return LCF_ERR_ALLOC;
+    p->Nz = Nz; p->Nx = Nx; p->N = N; p->Kz = win->Kz; p->Kx = win->Kx; p->K = win->Kz * win->Kx;
+    p->P = (long long)Nz * Nx;
+    p->win = *win; p->thr = *thr; p->prec = thr->precision;
+    p->esz = p->prec ? 8 : 4;
+    p->NP = (N + 1) / 2; p->Ns = 2 * p->NP;
+    p->max_sweeps = p->prec ? 40 : 24;
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&p->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        delete p;
+        return LCF_ERR_CUDA;
+    }
+
+    // ---- windows ----
+    std::vector<int> zlo, zhi, xlo, xhi;
+    axis_windows(Nz, p->Kz, (double)win->sigma_z, (double)win->trunc_sigmas, p->gz_h, zlo, zhi);
+    axis_windows(Nx, p->Kx, (double)win->sigma_x, (double)win->trunc_sigmas, p->gx_h, xlo, xhi);
+    p->box_h.resize(p->K);
+    long long off = 0;
+    for (int kx = 0; kx < p->Kx; ++kx)
+        for (int kz = 0; kz < p->Kz; ++kz) {
+            WinBox& b = p->box_h[kx * p->Kz + kz];
+            b.kz = kz; b.kx = kx; b.pad_ = 0;
+            b.z0 = zlo[kz]; b.Lz = zhi[kz] >= zlo[kz] ? zhi[kz] - zlo[kz] + 1 : 0;
+            b.x0 = xlo[kx]; b.Lx = xhi[kx] >= xlo[kx] ? xhi[kx] - xlo[kx] + 1 : 0;
+            if (b.Lz == 0 || b.Lx == 0) { b.Lz = 0; b.Lx = 0; b.z0 = 0; b.x0 = 0; }
+            b.Pk = b.Lz * b.Lx;
+            b.tile_off = off;
+            off += b.Pk;
+        }
+    p->sumPk = off;
+    // windows covering each pixel coordinate (supports are intervals with monotone ends)
+    auto cover = [](int n, int K, const std::vector<int>& lo, const std::vector<int>& hi, std::vector<int>& klo,
+                    std::vector<int>& khi) {
+        klo.assign(n, 0); khi.assign(n, -1);
+        for (int i = 0; i < n; ++i) {
+            int a = K, b = -1;
+            for (int k = 0; k < K; ++k)
+                if (hi[k] >= lo[k] && i >= lo[k] && i <= hi[k]) { if (k < a) a = k; if (k > b) b = k; }
+            klo[i] = a; khi[i] = b;
+        }
+    };
+    std::vector<int> kzlo, kzhi, kxlo, kxhi;
+    cover(Nz, p->Kz, zlo, zhi, kzlo, kzhi);
+    cover(Nx, p->Kx, xlo, xhi, kxlo, kxhi);
+
+    // ---- kernel geometry ----
+    if (configure_gram(p) != cudaSuccess || configure_evd(p) != cudaSuccess || configure_project(p) != cudaSuccess ||
+        p->NP > 128) {
+        cudaGetLastError();
+        delete p;
+        return LCF_ERR_UNSUPPORTED;
+    }
+
+    // ---- Gram work items: each window's box split into pixel chunks (multiples of GRAM_TP) ----
+    std::vector<GramItem> gitems;
+    p->gfirst_h.assign(p->K + 1, 0);
+    {
+        long long target = p->sumPk / ((long long)p->num_sms * 6) + 1;
+        long long ch = ((target + GRAM_TP - 1) / GRAM_TP) * GRAM_TP;
+        if (ch < 4 * GRAM_TP) ch = 4 * GRAM_TP;
+        int slot = 0;
+        for (int k = 0; k < p->K; ++k) {
+            p->gfirst_h[k] = slot;
+            const int Pk = p->box_h[k].Pk;
+            if (Pk > 0) {
+                int nch = (int)((Pk + ch / 2) / ch);
+                if (nch < 1) nch = 1;
+                int per = (Pk + nch - 1) / nch;
+                per = ((per + GRAM_TP - 1) / GRAM_TP) * GRAM_TP;
+                for (int q0 = 0; q0 < Pk; q0 += per) {
+                    int q1 = q0 + per < Pk ? q0 + per : Pk;
+                    for (int b = 0; b < p->gram_batches; ++b) gitems.push_back({k, q0, q1, b, slot});
+                    ++slot;
+                }
+            }
+        }
+        p->gfirst_h[p->K] = slot;
+        p->n_gslots = slot;
+        p->n_gitems = (int)gitems.size();
+    }
+    // ---- projection work items ----
+    std::vector<ProjItem> pitems;
+    p->pfirst_h.assign(p->K + 1, 0);
+    for (int k = 0; k < p->K; ++k) {
+        p->pfirst_h[k] = (int)pitems.size();
+        for (int q0 = 0; q0 < p->box_h[k].Pk; q0 += PROJ_TPIX)
+            pitems.push_back({k, q0, q0 + PROJ_TPIX < p->box_h[k].Pk ? q0 + PROJ_TPIX : p->box_h[k].Pk});
+    }
+    p->pfirst_h[p->K] = (int)pitems.size();
+    p->n_pitems = (int)pitems.size();
+
+    // ---- device memory ----
+    const size_t N2 = (size_t)N * N, K = (size_t)p->K, Ns = (size_t)p->Ns, M = Ns - 1;
+    bool ok = true;
+    ok = ok && dev_upload(&p->gz_d, p->gz_h) && dev_upload(&p->gx_d, p->gx_h) && dev_upload(&p->box_d, p->box_h);
+    ok = ok && dev_upload(&p->kzlo_d, kzlo) && dev_upload(&p->kzhi_d, kzhi) && dev_upload(&p->kxlo_d, kxlo) &&
+         dev_upload(&p->kxhi_d, kxhi);
+    ok = ok && dev_upload(&p->gitems_d, gitems) && dev_upload(&p->gfirst_d, p->gfirst_h);
+    ok = ok && dev_upload(&p->pitems_d, pitems) && dev_upload(&p->pfirst_d, p->pfirst_h);
+    ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->gpart_d), (size_t)p->n_gslots * N2 * 2 * p->esz);
+    ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->R_d), K * N2 * 2 * p->esz);
+    ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->rotlog_d), K * p->max_sweeps * M * 3 * p->NP * p->esz);
+    ok = ok && dev_alloc(&p->lam_d, K * N) && dev_alloc(&p->order_d, K * N) && dev_alloc(&p->cut_d, K) &&
+         dev_alloc(&p->sweeps_d, K) && dev_alloc(&p->conv_d, K) && dev_alloc(&p->wslot_d, K * Ns) &&
+         dev_alloc(&p->wslot_dd_d, K * Ns) && dev_alloc(&p->wt_d, K * N);
+    ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->V_d), K * N * Ns * 2 * p->esz);
+    ok = ok && dev_alloc(&p->B_d, K * N * Ns);
+    ok = ok && dev_alloc(&p->tiles_d, (size_t)p->sumPk) && dev_alloc(&p->tsum_d, (size_t)p->n_pitems) &&
+         dev_alloc(&p->mean_d, K) && dev_alloc(&p->alpha_d, K);
+    if (!ok) {
+        cudaGetLastError();
+        free_plan_device(p);
+        delete p;
+        return LCF_ERR_ALLOC;
+    }
+    // the Gram kernel leaves the non-canonical half of each partial unwritten; clear once so no
+    // uninitialised memory is ever read by tools (the loader never reads that half)
+    cudaMemset(p->gpart_d, 0, (size_t)p->n_gslots * N2 * 2 * p->esz);
+    if (cudaDeviceSynchronize() != cudaSuccess) {
+        free_plan_device(p);
+        delete p;
+        return LCF_ERR_CUDA;
+    }
+    *out = p;
+    return LCF_OK;
+}
+
+extern "C" lcf_status lcf_plan_destroy(lcf_plan* p) {
+    if (!p) return LCF_OK;
+    if (p->ran) cudaStreamSynchronize(p->last_stream);
+    free_plan_device(p);
+    cudaGetLastError();
+    delete p;
+    return LCF_OK;
+}
+
+extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev, void* stream) {
+    if (!p || !iq_dev || !pd_dev) return LCF_ERR_INVALID_ARG;
+    if (p->cuda_failed) return LCF_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const float2* iq = reinterpret_cast<const float2*>(iq_dev);
+    const bool tm = p->timing && p->timer.have;
+    cudaError_t e = cudaSuccess;
+    auto mark = [&](int i) { if (tm && e == cudaSuccess) e = cudaEventRecord(p->timer.ev[i], st); };
+    mark(0);
+    if (e == cudaSuccess) e = launch_gram(p, iq, st);
+    mark(1);
+    if (e == cudaSuccess) e = launch_jacobi(p, st);
+    mark(2);
+    if (e == cudaSuccess) e = launch_vbuild(p, st);
+    mark(3);
+    if (e == cudaSuccess) e = launch_project(p, iq, st);
+    mark(4);
+    if (e == cudaSuccess) e = launch_combine(p, pd_dev, st);
+    mark(5);
+    p->last_stream = st;
+    p->ran = true;
+    if (e != cudaSuccess) { p->cuda_failed = true; return LCF_ERR_CUDA; }
+    return LCF_OK;
+}
+
+extern "C" lcf_status lcf_filter_host(lcf_plan* p, const void* iq_host, float* pd_host, void* stream) {
+    if (!p || !iq_host || !pd_host) return LCF_ERR_INVALID_ARG;
+    if (p->cuda_failed) return LCF_ERR_CUDA;
+    const size_t iq_bytes = (size_t)p->N * p->P * sizeof(float2), pd_bytes = (size_t)p->P * sizeof(float);
+    if (!p->iq_stage_d) {
+        if (cudaMalloc(&p->iq_stage_d, iq_bytes) != cudaSuccess ||
+            cudaMalloc(reinterpret_cast<void**>(&p->pd_stage_d), pd_bytes) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(p->iq_stage_d); p->iq_stage_d = nullptr;
+            return LCF_ERR_ALLOC;
+        }
+    }
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (cudaMemcpyAsync(p->iq_stage_d, iq_host, iq_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+        p->cuda_failed = true;
+        return LCF_ERR_CUDA;
+    }
+    lcf_status s = lcf_filter(p, p->iq_stage_d, p->pd_stage_d, stream);
+    if (s != LCF_OK) return s;
+    if (cudaMemcpyAsync(pd_host, p->pd_stage_d, pd_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) {
+        p->cuda_failed = true;
+        return LCF_ERR_CUDA;
+    }
+    return LCF_OK;
+}
+
+extern "C" int lcf_num_windows(const lcf_plan* p) { return p ? p->K : 0; }
+
+extern "C" lcf_status lcf_get_eigenvalues(lcf_plan* p, double* lam) {
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK || !lam) return s != LCF_OK ? s : LCF_ERR_INVALID_ARG;
+    if (cudaMemcpy(lam, p->lam_d, sizeof(double) * p->K * p->N, cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    return conv_status(p);
+}
+
+extern "C" lcf_status lcf_get_cutoffs(lcf_plan* p, int* c) {
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK || !c) return s != LCF_OK ? s : LCF_ERR_INVALID_ARG;
+    if (cudaMemcpy(c, p->cut_d, sizeof(int) * p->K, cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    return conv_status(p);
+}
+
+extern "C" lcf_status lcf_get_sweeps(lcf_plan* p, int* sw) {
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK || !sw) return s != LCF_OK ? s : LCF_ERR_INVALID_ARG;
+    if (cudaMemcpy(sw, p->sweeps_d, sizeof(int) * p->K, cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    return conv_status(p);
+}
+
+extern "C" lcf_status lcf_get_weights(lcf_plan* p, double* wt) {
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK || !wt) return s != LCF_OK ? s : LCF_ERR_INVALID_ARG;
+    if (cudaMemcpy(wt, p->wt_d, sizeof(double) * p->K * p->N, cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    return conv_status(p);
+}
+
+extern "C" lcf_status lcf_get_window_means(lcf_plan* p, double* m) {
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK || !m) return s != LCF_OK ? s : LCF_ERR_INVALID_ARG;
+    if (cudaMemcpy(m, p->mean_d, sizeof(double) * p->K, cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    return conv_status(p);
+}
+
+extern "C" lcf_status lcf_get_gram(lcf_plan* p, double* R) {
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK || !R) return s != LCF_OK ? s : LCF_ERR_INVALID_ARG;
+    const size_t n = (size_t)p->K * p->N * p->N * 2;
+    if (p->prec == 1) {
+        if (cudaMemcpy(R, p->R_d, n * sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    } else {
+        std::vector<float> tmp(n);
+        if (cudaMemcpy(tmp.data(), p->R_d, n * sizeof(float), cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+        for (size_t i = 0; i < n; ++i) R[i] = (double)tmp[i];
+    }
+    return conv_status(p);
+}
+
+extern "C" lcf_status lcf_get_eigenvectors(lcf_plan* p, double* V) {
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK || !V) return s != LCF_OK ? s : LCF_ERR_INVALID_ARG;
+    const size_t K = p->K, N = p->N, Ns = p->Ns, n = K * N * Ns * 2;
+    std::vector<double> tmp(n);
+    if (p->prec == 1) {
+        if (cudaMemcpy(tmp.data(), p->V_d, n * sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    } else {
+        std::vector<float> t32(n);
+        if (cudaMemcpy(t32.data(), p->V_d, n * sizeof(float), cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+        for (size_t i = 0; i < n; ++i) tmp[i] = (double)t32[i];
+    }
+    std::vector<int> order(K * N);
+    if (cudaMemcpy(order.data(), p->order_d, sizeof(int) * K * N, cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    for (size_t k = 0; k < K; ++k)
+        for (size_t a = 0; a < N; ++a)
+            for (size_t i = 0; i < N; ++i) {
+                const size_t u = (size_t)order[k * N + i];
+                const double* src = &tmp[((k * N + a) * Ns + u) * 2];
+                double* dst = &V[((k * N + a) * N + i) * 2];
+                dst[0] = src[0]; dst[1] = src[1];
+            }
+    return conv_status(p);
+}
+
+extern "C" lcf_status lcf_get_filters(lcf_plan* p, double* F) {
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK || !F) return s != LCF_OK ? s : LCF_ERR_INVALID_ARG;
+    const size_t n = (size_t)p->K * p->N * p->N * 2;
+    if (!p->F_d && cudaMalloc(reinterpret_cast<void**>(&p->F_d), n * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        p->F_d = nullptr;
+        return LCF_ERR_ALLOC;
+    }
+    if (launch_build_filters(p, p->last_stream) != cudaSuccess || cudaStreamSynchronize(p->last_stream) != cudaSuccess)
+        return LCF_ERR_CUDA;
+    if (cudaMemcpy(F, p->F_d, n * sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    return conv_status(p);
+}
+
+extern "C" lcf_status lcf_set_timing(lcf_plan* p, int enabled) {
+    if (!p) return LCF_ERR_INVALID_ARG;
+    if (enabled && !p->timer.have) {
+        for (auto& e : p->timer.ev)
+            if (cudaEventCreate(&e) != cudaSuccess) return LCF_ERR_CUDA;
+        p->timer.have = true;
+    }
+    p->timing = enabled != 0;
+    return LCF_OK;
+}
+
+extern "C" lcf_status lcf_get_stage_ms(lcf_plan* p, float ms[5]) {
+    if (!p || !ms || !p->timing || !p->timer.have) return LCF_ERR_INVALID_ARG;
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK) return s;
+    for (int i = 0; i < 5; ++i)
+        if (cudaEventElapsedTime(&ms[i], p->timer.ev[i], p->timer.ev[i + 1]) != cudaSuccess) return LCF_ERR_CUDA;
+    return LCF_OK;
+}
+
+extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
+    if (!p || !w) return LCF_ERR_INVALID_ARG;
+    const double N = p->N, S = (double)p->sumPk;
+    w->sum_Pk = S;
+    w->gram_flops = 8.0 * S * N * (N + 1.0) / 2.0;   // Hermitian half, 8 real flops per complex MAC
+    w->proj_flops = 8.0 * S * N * N;                 // dense N x N projector factor
+    w->hbm_bytes = 8.0 * N * (double)p->P + 4.0 * (double)p->P;
+    w->launches = 6;
+    return LCF_OK;
+}

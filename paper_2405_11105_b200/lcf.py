@@ -1,0 +1,226 @@
+"""ctypes binding of liblcf.so (include/lcf.h).  Argument marshalling only: every step of the path
+runs in the CUDA kernels behind the C ABI.  PyTorch is used by callers for device memory and
+streams; this module needs only raw pointers.
+
+There is no CPU fallback: if liblcf.so is missing or does not load, `load()` raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+HERE = Path(__file__).resolve().parent
+LIB_PATH = HERE / "liblcf.so"
+
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY = 0, 1, 2, 3
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_NOT_CONVERGED = range(6)
+
+EXPORTS = [
+    "lcf_plan_create", "lcf_filter", "lcf_filter_host", "lcf_plan_destroy", "lcf_num_windows",
+    "lcf_get_eigenvalues", "lcf_get_cutoffs", "lcf_get_sweeps", "lcf_get_gram", "lcf_get_eigenvectors",
+    "lcf_get_weights", "lcf_get_filters", "lcf_get_window_means", "lcf_set_timing", "lcf_get_stage_ms",
+    "lcf_get_work", "lcf_measure_peak", "lcf_status_string",
+]
+
+
+class Windows(C.Structure):
+    _fields_ = [("Kz", C.c_int), ("Kx", C.c_int), ("sigma_z", C.c_float), ("sigma_x", C.c_float),
+                ("trunc_sigmas", C.c_float)]
+
+
+class Thresh(C.Structure):
+    _fields_ = [("mode", C.c_int), ("k_fixed", C.c_int), ("energy_frac", C.c_double), ("beta", C.c_double),
+                ("precision", C.c_int)]
+
+
+class Work(C.Structure):
+    _fields_ = [("gram_flops", C.c_double), ("proj_flops", C.c_double), ("hbm_bytes", C.c_double),
+                ("sum_Pk", C.c_double), ("launches", C.c_int)]
+
+
+class LcfError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        self.status = status
+        super().__init__(f"{what}: {status_string(status)} (lcf_status {status})")
+
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """dlopen liblcf.so; raises if it has not been built (python -m paper_2405_11105_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2405_11105_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(str(LIB_PATH))
+        vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
+        L.lcf_plan_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.POINTER(Windows), C.POINTER(Thresh)]
+        L.lcf_filter.argtypes = [vp, vp, vp, vp]
+        L.lcf_filter_host.argtypes = [vp, vp, vp, vp]
+        L.lcf_plan_destroy.argtypes = [vp]
+        L.lcf_num_windows.argtypes = [vp]
+        for name in ("lcf_get_eigenvalues", "lcf_get_gram", "lcf_get_eigenvectors", "lcf_get_weights",
+                     "lcf_get_filters", "lcf_get_window_means"):
+            getattr(L, name).argtypes = [vp, dp]
+        L.lcf_get_cutoffs.argtypes = [vp, ip]
+        L.lcf_get_sweeps.argtypes = [vp, ip]
+        L.lcf_set_timing.argtypes = [vp, C.c_int]
+        L.lcf_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
+        L.lcf_get_work.argtypes = [vp, C.POINTER(Work)]
+        L.lcf_measure_peak.argtypes = [C.c_int, dp]
+        L.lcf_status_string.argtypes = [C.c_int]
+        L.lcf_status_string.restype = C.c_char_p
+        for name in EXPORTS:
+            if name != "lcf_status_string":
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def status_string(status: int) -> str:
+    return load().lcf_status_string(int(status)).decode()
+
+
+def measure_peak(kind: int) -> float:
+    """TFLOP/s of the FP32 FFMA (0), packed FFMA2 (1) or FP64 DFMA (2) pipe on the current device."""
+    v = C.c_double(0.0)
+    st = load().lcf_measure_peak(int(kind), C.byref(v))
+    if st != OK:
+        raise LcfError(st, "lcf_measure_peak")
+    return float(v.value)
+
+
+def _ptr(x) -> int:
+    """Raw address of a torch tensor (data_ptr), numpy array or int."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return int(x.data_ptr())
+    if isinstance(x, np.ndarray):
+        return int(x.ctypes.data)
+    raise TypeError(type(x))
+
+
+def _stream(s) -> int:
+    if s is None:
+        return 0
+    if isinstance(s, int):
+        return s
+    return int(s.cuda_stream)          # torch.cuda.Stream
+
+
+class Plan:
+    """lcf_plan_create / lcf_filter / lcf_plan_destroy plus the diagnostic getters."""
+
+    def __init__(self, Nz: int, Nx: int, N: int, Kz: int, Kx: int, sigma_z: float, sigma_x: float, trunc: float,
+                 mode: int, k_fixed: int = 0, energy_frac: float = 0.995, beta: float = 0.5, precision: int = 0):
+        L = load()
+        self._h = C.c_void_p(None)
+        self.Nz, self.Nx, self.N, self.K = int(Nz), int(Nx), int(N), int(Kz) * int(Kx)
+        w = Windows(int(Kz), int(Kx), float(sigma_z), float(sigma_x), float(trunc))
+        t = Thresh(int(mode), int(k_fixed), float(energy_frac), float(beta), int(precision))
+        st = L.lcf_plan_create(C.byref(self._h), int(Nz), int(Nx), int(N), C.byref(w), C.byref(t))
+        if st != OK:
+            self._h = C.c_void_p(None)
+            raise LcfError(st, "lcf_plan_create")
+
+    @classmethod
+    def from_spec(cls, Nz: int, Nx: int, N: int, filt) -> "Plan":
+        """filt: an object with the fields of synth.FilterSpec."""
+        return cls(Nz, Nx, N, filt.Kz, filt.Kx, filt.sigma_z, filt.sigma_x, filt.trunc, filt.mode, filt.k_fixed,
+                   filt.energy_frac, filt.beta, filt.precision)
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            load().lcf_plan_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    # ---- hot path ----
+    def filter(self, iq_dev, pd_dev, stream=None):
+        """iq_dev: complex64 device tensor [N][Nx][Nz] (or address); pd_dev: float32 [Nx][Nz]. Asynchronous."""
+        st = load().lcf_filter(self._h, _ptr(iq_dev), _ptr(pd_dev), _stream(stream))
+        if st != OK:
+            raise LcfError(st, "lcf_filter")
+
+    def filter_host(self, iq_host, pd_host, stream=None):
+        """Host buffers (numpy / pinned torch tensors); copies, filters, copies back, synchronises."""
+        st = load().lcf_filter_host(self._h, _ptr(iq_host), _ptr(pd_host), _stream(stream))
+        if st != OK:
+            raise LcfError(st, "lcf_filter_host")
+
+    # ---- diagnostics ----
+    def _get_d(self, fn, shape, allow_unconverged=False):
+        out = np.empty(shape, dtype=np.float64)
+        st = getattr(load(), fn)(self._h, out.ctypes.data_as(C.POINTER(C.c_double)))
+        if st != OK and not (allow_unconverged and st == ERR_NOT_CONVERGED):
+            raise LcfError(st, fn)
+        return out
+
+    def _get_i(self, fn, allow_unconverged=False):
+        out = np.empty(self.K, dtype=np.int32)
+        st = getattr(load(), fn)(self._h, out.ctypes.data_as(C.POINTER(C.c_int)))
+        if st != OK and not (allow_unconverged and st == ERR_NOT_CONVERGED):
+            raise LcfError(st, fn)
+        return out
+
+    def eigenvalues(self, **kw):
+        return self._get_d("lcf_get_eigenvalues", (self.K, self.N), **kw)
+
+    def cutoffs(self, **kw):
+        return self._get_i("lcf_get_cutoffs", **kw)
+
+    def sweeps(self, **kw):
+        return self._get_i("lcf_get_sweeps", **kw)
+
+    def weights(self, **kw):
+        return self._get_d("lcf_get_weights", (self.K, self.N), **kw)
+
+    def window_means(self, **kw):
+        return self._get_d("lcf_get_window_means", (self.K,), **kw)
+
+    def gram(self, **kw):
+        return self._get_d("lcf_get_gram", (self.K, self.N, self.N, 2), **kw).view(np.complex128)[..., 0]
+
+    def eigenvectors(self, **kw):
+        return self._get_d("lcf_get_eigenvectors", (self.K, self.N, self.N, 2), **kw).view(np.complex128)[..., 0]
+
+    def filters(self, **kw):
+        return self._get_d("lcf_get_filters", (self.K, self.N, self.N, 2), **kw).view(np.complex128)[..., 0]
+
+    # ---- measurement ----
+    def set_timing(self, enabled: bool):
+        st = load().lcf_set_timing(self._h, int(bool(enabled)))
+        if st != OK:
+            raise LcfError(st, "lcf_set_timing")
+
+    def stage_ms(self):
+        ms = (C.c_float * 5)()
+        st = load().lcf_get_stage_ms(self._h, ms)
+        if st != OK:
+            raise LcfError(st, "lcf_get_stage_ms")
+        return dict(zip(("gram", "evd", "weights_projector", "projection", "combine"), [float(v) for v in ms]))
+
+    def work(self) -> dict:
+        w = Work()
+        st = load().lcf_get_work(self._h, C.byref(w))
+        if st != OK:
+            raise LcfError(st, "lcf_get_work")
+        return {k: getattr(w, k) for k, _ in Work._fields_}
