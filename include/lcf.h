@@ -105,9 +105,10 @@ lcf_status lcf_get_filters(lcf_plan* plan, double* F /* HOST [K][N][N][2] */);
 lcf_status lcf_get_window_means(lcf_plan* plan, double* m /* HOST [K] */);
 
 /* ---- measurement helpers ---- */
-/* Device time in ms of each stage of the most recent lcf_filter call when the plan has timing
- * enabled: [gram, evd, weights_projector, projection, combine].  Enabling timing records CUDA
- * events on the caller's stream between the launches (no synchronisation in lcf_filter). */
+/* Mean device time in ms of each stage -- [gram, evd, weights_projector, projection, combine] --
+ * over the lcf_filter calls made since timing was last enabled (at most the last 64).  With timing
+ * enabled lcf_filter records CUDA events on the caller's stream between its launches; it still
+ * does not synchronise.  lcf_get_stage_ms synchronises the stream. */
 lcf_status lcf_set_timing(lcf_plan* plan, int enabled);
 lcf_status lcf_get_stage_ms(lcf_plan* plan, float ms[5] /* HOST */);
 /* Algorithmic work of one lcf_filter call: Hermitian-half Gram flops,

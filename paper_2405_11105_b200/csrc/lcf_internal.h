@@ -37,9 +37,11 @@ constexpr int PROJ_STAGES = 3;
 constexpr int VB_WARPS = 8;        // warps per CTA of the weights/projector kernel
 constexpr int VB_ROWS = 2;         // rows of V per warp
 
+constexpr int TIMER_RING = 64;     // lcf_filter calls whose stage events are kept
 struct StageTimer {
-    cudaEvent_t ev[6];
+    cudaEvent_t ev[TIMER_RING][6];
     bool have = false;
+    long long calls = 0;           // calls recorded since timing was (re)enabled
 };
 
 }  // namespace lcf

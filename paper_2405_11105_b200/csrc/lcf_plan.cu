@@ -60,7 +60,8 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->tiles_d); cudaFree(p->tsum_d); cudaFree(p->mean_d); cudaFree(p->alpha_d);
     cudaFree(p->F_d); cudaFree(p->iq_stage_d); cudaFree(p->pd_stage_d);
     if (p->timer.have)
-        for (auto& e : p->timer.ev) cudaEventDestroy(e);
+        for (auto& set : p->timer.ev)
+            for (auto& e : set) cudaEventDestroy(e);
 }
 
 lcf_status sync_plan(lcf_plan* p) {
@@ -256,7 +257,8 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     const float2* iq = reinterpret_cast<const float2*>(iq_dev);
     const bool tm = p->timing && p->timer.have;
     cudaError_t e = cudaSuccess;
-    auto mark = [&](int i) { if (tm && e == cudaSuccess) e = cudaEventRecord(p->timer.ev[i], st); };
+    cudaEvent_t* evs = p->timer.ev[p->timer.calls % TIMER_RING];
+    auto mark = [&](int i) { if (tm && e == cudaSuccess) e = cudaEventRecord(evs[i], st); };
     mark(0);
     if (e == cudaSuccess) e = launch_gram(p, iq, st);
     mark(1);
@@ -268,6 +270,7 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     mark(4);
     if (e == cudaSuccess) e = launch_combine(p, pd_dev, st);
     mark(5);
+    if (tm) ++p->timer.calls;
     p->last_stream = st;
     p->ran = true;
     if (e != cudaSuccess) { p->cuda_failed = true; return LCF_ERR_CUDA; }
@@ -395,20 +398,29 @@ extern "C" lcf_status lcf_get_filters(lcf_plan* p, double* F) {
 extern "C" lcf_status lcf_set_timing(lcf_plan* p, int enabled) {
     if (!p) return LCF_ERR_INVALID_ARG;
     if (enabled && !p->timer.have) {
-        for (auto& e : p->timer.ev)
-            if (cudaEventCreate(&e) != cudaSuccess) return LCF_ERR_CUDA;
+        for (auto& set : p->timer.ev)
+            for (auto& e : set)
+                if (cudaEventCreate(&e) != cudaSuccess) return LCF_ERR_CUDA;
         p->timer.have = true;
     }
     p->timing = enabled != 0;
+    p->timer.calls = 0;
     return LCF_OK;
 }
 
 extern "C" lcf_status lcf_get_stage_ms(lcf_plan* p, float ms[5]) {
-    if (!p || !ms || !p->timing || !p->timer.have) return LCF_ERR_INVALID_ARG;
+    if (!p || !ms || !p->timing || !p->timer.have || p->timer.calls == 0) return LCF_ERR_INVALID_ARG;
     lcf_status s = sync_plan(p);
     if (s != LCF_OK) return s;
-    for (int i = 0; i < 5; ++i)
-        if (cudaEventElapsedTime(&ms[i], p->timer.ev[i], p->timer.ev[i + 1]) != cudaSuccess) return LCF_ERR_CUDA;
+    const long long n = p->timer.calls < TIMER_RING ? p->timer.calls : TIMER_RING;
+    double acc[5] = {0, 0, 0, 0, 0};
+    for (long long c = 0; c < n; ++c)
+        for (int i = 0; i < 5; ++i) {
+            float t = 0.f;
+            if (cudaEventElapsedTime(&t, p->timer.ev[c][i], p->timer.ev[c][i + 1]) != cudaSuccess) return LCF_ERR_CUDA;
+            acc[i] += t;
+        }
+    for (int i = 0; i < 5; ++i) ms[i] = (float)(acc[i] / (double)n);
     return LCF_OK;
 }
 

@@ -1,0 +1,125 @@
+"""CPU-only checks of the product's host side: liblcf.so builds, loads and exports every symbol
+include/lcf.h declares; argument validation returns status codes (no CUDA call is made before the
+arguments are validated); the library refuses to run without a GPU; the ensemble sharding used for
+multi-GPU runs is a partition (world_size 2, gloo)."""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def lcf():
+    from paper_2405_11105_b200 import build, lcf as binding
+    build.build()
+    binding.load()
+    return binding
+
+
+def test_library_exports_every_declared_symbol(lcf):
+    header = (ROOT / "include" / "lcf.h").read_text()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(lcf_[a-z_]+)\s*\(", header))
+    assert {"lcf_plan_create", "lcf_filter", "lcf_plan_destroy"} <= declared
+    lib = C.CDLL(str(lcf.LIB_PATH))
+    for name in sorted(declared):
+        assert hasattr(lib, name), f"{name} declared in include/lcf.h but not exported"
+    assert declared == set(lcf.EXPORTS)
+
+
+def test_status_strings(lcf):
+    seen = {lcf.status_string(s) for s in range(6)}
+    assert len(seen) == 6 and "ok" in seen
+    assert lcf.status_string(99) == "unknown status"
+
+
+def _create(lcf, Nz=8, Nx=8, N=4, Kz=1, Kx=1, sz=0.0, sx=0.0, tr=0.0, mode=0, k=1, frac=0.995, beta=0.5, prec=0):
+    L = lcf.load()
+    h = C.c_void_p(None)
+    w = lcf.Windows(Kz, Kx, sz, sx, tr)
+    t = lcf.Thresh(mode, k, frac, beta, prec)
+    st = L.lcf_plan_create(C.byref(h), Nz, Nx, N, C.byref(w), C.byref(t))
+    return st, h
+
+
+@pytest.mark.parametrize("kw", [
+    dict(Nz=0), dict(Nx=-1), dict(N=1), dict(Kz=0), dict(Kx=0), dict(mode=4), dict(mode=-1),
+    dict(k=-1), dict(k=5), dict(mode=1, frac=1.0), dict(mode=3, frac=0.0), dict(mode=2, beta=0.0),
+    dict(prec=2), dict(sz=float("nan")), dict(tr=float("inf")),
+])
+def test_invalid_arguments_are_refused(lcf, kw):
+    st, h = _create(lcf, **kw)
+    assert st == lcf.ERR_INVALID_ARG and not h.value
+
+
+def test_null_pointers(lcf):
+    L = lcf.load()
+    assert L.lcf_plan_create(None, 8, 8, 4, None, None) == lcf.ERR_INVALID_ARG
+    assert L.lcf_plan_destroy(None) == lcf.OK
+    assert L.lcf_filter(None, None, None, None) == lcf.ERR_INVALID_ARG
+    assert L.lcf_num_windows(None) == 0
+    assert L.lcf_measure_peak(7, None) == lcf.ERR_INVALID_ARG
+
+
+def test_no_cpu_fallback(lcf):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    st, h = _create(lcf)
+    assert st == lcf.ERR_CUDA and not h.value            # fails loudly, does not compute on the host
+    with pytest.raises(lcf.LcfError):
+        lcf.Plan(8, 8, 4, 1, 1, 0.0, 0.0, 0.0, 0, 1)
+
+
+def test_product_never_imports_the_oracle():
+    pkg = ROOT / "paper_2405_11105_b200"
+    for f in list(pkg.rglob("*.py")) + list(pkg.rglob("*.cu")) + list(pkg.rglob("*.h")):
+        txt = f.read_text()
+        assert "lcf_oracle" not in txt and "from oracle" not in txt and "import oracle" not in txt, f
+
+
+def test_ensemble_shard_is_a_partition():
+    from paper_2405_11105_b200.shard import ensemble_shard
+    for n in (0, 1, 7, 16):
+        for w in (1, 2, 3, 8):
+            parts = [ensemble_shard(n, r, w) for r in range(w)]
+            assert sorted(sum(parts, [])) == list(range(n))
+            assert max(len(p) for p in parts) - min(len(p) for p in parts) <= 1
+    with pytest.raises(ValueError):
+        ensemble_shard(4, 2, 2)
+
+
+_WORKER = r"""
+import os, sys
+import numpy as np, torch, torch.distributed as dist
+sys.path.insert(0, os.environ["LCF_ROOT"])
+from paper_2405_11105_b200.shard import ensemble_shard, gather_images
+dist.init_process_group("gloo")
+r, w = dist.get_rank(), dist.get_world_size()
+n = 5
+mine = ensemble_shard(n, r, w)
+local = {e: torch.full((2, 3), float(e)) for e in mine}          # stand-in for the filtered images
+imgs = gather_images(local, n)
+assert len(imgs) == n and all(float(imgs[e][0, 0]) == e for e in range(n))
+dist.barrier()
+dist.destroy_process_group()
+print("rank", r, "ok", mine)
+"""
+
+
+def test_two_rank_ensemble_sharding_gloo(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER)
+    env = dict(os.environ, LCF_ROOT=str(ROOT), MASTER_ADDR="127.0.0.1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+           "--master-addr", "127.0.0.1", "--master-port", "29571", str(script)]
+    out = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=240)
+    assert out.returncode == 0, out.stdout + out.stderr
+    assert "rank 0 ok [0, 2, 4]" in out.stdout and "rank 1 ok [1, 3]" in out.stdout

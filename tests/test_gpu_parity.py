@@ -1,0 +1,253 @@
+"""GPU parity: the CUDA path (through the C ABI of liblcf.so) against the float64 oracle, element by
+element on the same seeded inputs.
+
+Gates (BASELINE.json north_star, restated in DESIGN.md "Parity gates"):
+  * eigenvalues within 1e-5 * lambda_max per window;
+  * cut-offs c_k equal (integers; both sides decide them from their own eigenvalues in double
+    cumulative sums -- DESIGN.md "Discrete decisions");
+  * clutter-subspace projector Pi_c = sum_{i<=c} v_i v_i^H: ||Pi_gpu - Pi_oracle||_F <= 1e-4
+    (eigenvectors themselves are only defined up to phase);
+  * power-Doppler pixels within 60 dB of the image maximum: relative error <= 1e-3.
+The oracle is never on the product path; it is only the expected value here.
+"""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+from paper_2405_11105_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+LAM_TOL, PROJ_TOL, PD_TOL, PD_FLOOR = 1e-5, 1e-4, 1e-3, 1e-6
+
+
+@pytest.fixture(scope="module")
+def lcf():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2405_11105_b200 import build, lcf as binding
+    build.build()
+    binding.load()          # raises if the library is missing: no fallback
+    return binding
+
+
+def gpu_run(lcf, iq, filt, want=("lam", "c")):
+    import torch
+    N, Nx, Nz = iq.shape
+    iq_d = torch.from_numpy(np.ascontiguousarray(iq)).cuda()
+    pd_d = torch.full((Nx, Nz), float("nan"), dtype=torch.float32, device="cuda")
+    with lcf.Plan.from_spec(Nz, Nx, N, filt) as plan:
+        plan.filter(iq_d, pd_d)
+        torch.cuda.synchronize()
+        out = {"PD": pd_d.cpu().numpy().astype(np.float64)}
+        if "lam" in want:
+            out["lam"] = plan.eigenvalues()
+        if "c" in want:
+            out["c"] = plan.cutoffs()
+        if "R" in want:
+            out["R"] = plan.gram()
+        if "V" in want:
+            out["V"] = plan.eigenvectors()
+        if "F" in want:
+            out["F"] = plan.filters()
+        if "wt" in want:
+            out["wt"] = plan.weights()
+        if "mean" in want:
+            out["mean"] = plan.window_means()
+        out["sweeps"] = plan.sweeps()
+    return out
+
+
+def check_pd(pd, ref, tol=PD_TOL):
+    assert np.isfinite(pd).all()
+    mx = ref.max()
+    if mx <= 0:
+        assert np.abs(pd).max() == 0
+        return 0.0
+    m = ref >= PD_FLOOR * mx
+    rel = np.abs(pd - ref)[m] / ref[m]
+    assert rel.max() <= tol, f"PD max rel err {rel.max():.3e} > {tol}"
+    # below the floor: no garbage (absolute bound relative to the floor)
+    assert np.abs(pd - ref)[~m].max(initial=0.0) <= tol * PD_FLOOR * mx * 10 + 1e-30
+    return float(rel.max())
+
+
+def check_spectrum(g, o):
+    lmax = np.maximum(o["lam"][:, :1], 1e-300)
+    err = (np.abs(g["lam"] - o["lam"]) / lmax).max()
+    assert err <= LAM_TOL, f"eigenvalue err {err:.3e} lambda_max"
+    assert np.array_equal(g["c"], o["c"]), (g["c"], o["c"])
+    assert (np.diff(g["lam"], axis=1) <= 0).all()          # descending
+
+
+def projector_err(oracle, Vg, R_oracle, c):
+    """|| sum_{i<c} v_i v_i^H (gpu) - same (oracle Jacobi on the oracle's R) ||_F"""
+    _, Vo, _ = oracle.jacobi(R_oracle)
+    Pg = Vg[:, :c] @ Vg[:, :c].conj().T
+    Po = Vo[:, :c] @ Vo[:, :c].conj().T
+    return float(np.linalg.norm(Pg - Po))
+
+
+def full_config_case(lcf, oracle, cfg, ens=0, proj_windows=None):
+    seq = synth.generate(cfg)
+    iq = np.ascontiguousarray(synth.ensemble(seq, cfg, ens))
+    o = oracle.run_config(iq, cfg.filt, want_R=True)
+    g = gpu_run(lcf, iq, cfg.filt, want=("lam", "c", "V", "R", "mean"))
+    check_spectrum(g, o)
+    scale = np.abs(o["R"]).max(axis=(1, 2), keepdims=True)
+    gram_tol = 1e-12 if cfg.filt.precision == 1 else 1e-5
+    assert (np.abs(g["R"] - o["R"]) / scale).max() <= gram_tol
+    K = o["lam"].shape[0]
+    ks = range(K) if proj_windows is None else proj_windows
+    for k in ks:
+        c = int(o["c"][k])
+        if 0 < c < cfg.data.N:
+            e = projector_err(oracle, g["V"][k], o["R"][k], c)
+            assert e <= PROJ_TOL, f"window {k}: projector err {e:.3e}"
+    assert np.allclose(g["mean"], o["mean"], rtol=1e-3)
+    return check_pd(g["PD"], o["PD"])
+
+
+# ------------------------------------------------------------------ the five BASELINE.json configs
+def test_config0_tiny_local(lcf, oracle):
+    full_config_case(lcf, oracle, synth.baseline_configs()[0])
+
+
+def test_config1_global_evd(lcf, oracle):
+    full_config_case(lcf, oracle, synth.baseline_configs()[1])
+
+
+def test_config2_metric_workload(lcf, oracle):
+    # the bench workload, same plan parameters and launch configuration as bench.py
+    full_config_case(lcf, oracle, synth.baseline_configs()[2], proj_windows=[0, 9, 27, 36, 63])
+
+
+def test_config3_large_long_packet(lcf, oracle):
+    full_config_case(lcf, oracle, synth.baseline_configs()[3], proj_windows=[0, 100, 191])
+
+
+def test_config4_streaming_ensembles(lcf, oracle):
+    cfg = synth.baseline_configs()[4]
+    seq = synth.generate(cfg)
+    import torch
+    d = cfg.data
+    seq_d = torch.from_numpy(seq).cuda()                      # the whole 900-frame sequence, once
+    pd_d = torch.empty((d.Nx, d.Nz), dtype=torch.float32, device="cuda")
+    with lcf.Plan.from_spec(d.Nz, d.Nx, d.N, cfg.filt) as plan:
+        for e in (0, 7, 15):
+            # ensemble e is a pointer offset into the resident sequence (no copy)
+            view = seq_d[e * cfg.stride:e * cfg.stride + d.N]
+            assert view.is_contiguous()
+            plan.filter(view, pd_d)
+            torch.cuda.synchronize()
+            g = {"PD": pd_d.cpu().numpy().astype(np.float64), "lam": plan.eigenvalues(), "c": plan.cutoffs()}
+            o = oracle.run_config(np.ascontiguousarray(synth.ensemble(seq, cfg, e)), cfg.filt)
+            check_spectrum(g, o)
+            check_pd(g["PD"], o["PD"])
+
+
+# ------------------------------------------------------------------ shapes, modes, edge cases
+SMALL = [
+    # Nz, Nx, N, Kz, Kx, sigma, trunc, mode, k, precision
+    (50, 37, 33, 2, 3, 9.0, 3.0, synth.HARD_ENERGY, 0, 0),        # odd N (padded pivot), ragged tiles
+    (50, 37, 33, 2, 3, 9.0, 3.0, synth.SOFT_ENERGY, 0, 1),        # same in fp64 Gram/EVD
+    (64, 48, 100, 3, 2, 12.0, 2.5, synth.SOFT_FIXED, 5, 0),       # N = 100 (13 x 13 thread tiles, 7 K-chunks)
+    (40, 40, 16, 1, 1, 0.0, 0.0, synth.HARD_FIXED, 3, 1),         # all-ones window
+    (40, 24, 24, 2, 2, 30.0, 0.0, synth.HARD_FIXED, 2, 0),        # Gaussian, no truncation
+    (33, 65, 2, 2, 2, 8.0, 3.0, synth.HARD_FIXED, 1, 1),          # N = 2: one rotation, no blocks
+    (96, 80, 140, 2, 2, 20.0, 3.0, synth.HARD_ENERGY, 0, 0),      # N > 128: 3 pivots per lane, 2 Gram batches
+]
+
+
+@pytest.mark.parametrize("Nz,Nx,N,Kz,Kx,sigma,trunc,mode,k,prec", SMALL)
+def test_small_shapes_and_modes(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, trunc, mode, k, prec):
+    cfg = synth.baseline_configs()[2]
+    d = replace(cfg.data, Nz=Nz, Nx=Nx, N=N, n_frames=N, seed=100 + N, n_vessels=3, tissue_db=40.0, noise_db=-55.0)
+    f = synth.FilterSpec(Kz, Kx, sigma, sigma, trunc, mode, k_fixed=k, precision=prec)
+    iq = synth.generate_sequence(d)
+    o = oracle.run_config(iq, f, want_R=True, want_F=True)
+    g = gpu_run(lcf, iq, f, want=("lam", "c", "R", "F", "wt"))
+    check_spectrum(g, o)
+    check_pd(g["PD"], o["PD"])
+    soft = mode in (synth.SOFT_FIXED, synth.SOFT_ENERGY)
+    for kk in range(Kz * Kx):
+        wt_o = oracle.weights(N, soft, int(o["c"][kk]), f.beta)
+        assert np.allclose(g["wt"][kk], wt_o, rtol=0, atol=1e-12)
+    if not soft and prec == 1:
+        # hard filter matrix F = I - Pi_c is well conditioned when the cut sits in a spectral gap
+        lam = o["lam"]
+        for kk in range(Kz * Kx):
+            c = int(o["c"][kk])
+            if 0 < c < N and (lam[kk, c - 1] - lam[kk, c]) > 1e-6 * lam[kk, 0]:
+                assert np.linalg.norm(g["F"][kk] - o["F"][kk]) <= 1e-6
+
+
+def test_allpass_and_allstop(lcf, oracle):
+    iq = synth.random_cube(32, 24, 12, seed=5)
+    f0 = synth.FilterSpec(2, 2, 8.0, 8.0, 3.0, synth.HARD_FIXED, k_fixed=0)
+    g = gpu_run(lcf, iq, f0)
+    o = oracle.run_config(iq, f0)
+    check_pd(g["PD"], o["PD"], tol=1e-4)          # all weights 1: PD_k = w^2 |s_p|^2 (energy reproduced)
+    fN = replace(f0, k_fixed=12)
+    g = gpu_run(lcf, iq, fN)
+    assert np.array_equal(g["PD"], np.zeros_like(g["PD"]))   # everything removed: alpha_k = 0, PD = 0
+
+
+def test_rank_r_clutter_removed(lcf):
+    r = 3
+    iq = synth.rank_r_clutter(48, 40, 20, r, seed=9)
+    f = synth.FilterSpec(2, 2, 12.0, 12.0, 3.0, synth.HARD_FIXED, k_fixed=r, precision=1)
+    import torch
+    iq_d = torch.from_numpy(iq).cuda()
+    pd_d = torch.empty((40, 48), dtype=torch.float32, device="cuda")
+    with lcf.Plan.from_spec(48, 40, 20, f) as plan:
+        plan.filter(iq_d, pd_d)
+        torch.cuda.synchronize()
+        means = plan.window_means()
+        lam = plan.eigenvalues()
+    # residual power / input power per window: complex64 rounding of S leaves ~1e-14
+    assert (means * 48 * 40 / lam.sum(axis=1)).max() <= 1e-10
+
+
+def test_empty_window_support(lcf):
+    # sigma so small that no pixel lies within trunc*sigma of the half-integer centres: P_k = 0
+    iq = synth.random_cube(8, 8, 6, seed=2)
+    f = synth.FilterSpec(2, 2, 0.1, 0.1, 1.0, synth.HARD_FIXED, k_fixed=1)
+    g = gpu_run(lcf, iq, f)
+    assert np.array_equal(g["PD"], np.zeros((8, 8)))
+    assert np.array_equal(g["lam"], np.zeros((4, 6)))
+
+
+def test_deterministic_and_stream_and_host_path(lcf):
+    import torch
+    cfg = synth.baseline_configs()[0]
+    iq = synth.generate(cfg)
+    d = cfg.data
+    iq_d = torch.from_numpy(iq).cuda()
+    a = torch.empty((d.Nx, d.Nz), dtype=torch.float32, device="cuda")
+    b = torch.empty_like(a)
+    st = torch.cuda.Stream()
+    with lcf.Plan.from_spec(d.Nz, d.Nx, d.N, cfg.filt) as plan:
+        plan.filter(iq_d, a)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            plan.filter(iq_d, b, stream=st)
+        st.synchronize()
+        assert torch.equal(a, b)                         # bit-identical: no atomics anywhere
+        pinned_in = torch.from_numpy(iq).pin_memory()
+        pinned_out = torch.empty((d.Nx, d.Nz), dtype=torch.float32).pin_memory()
+        plan.filter_host(pinned_in, pinned_out)
+        assert torch.equal(pinned_out, a.cpu())
+
+
+def test_unsupported_and_limits(lcf):
+    # N = 300 needs a 300 x 300 complex triangle (> 227 KB): refused at create, not at filter
+    with pytest.raises(lcf.LcfError) as ei:
+        lcf.Plan(64, 64, 300, 1, 1, 0.0, 0.0, 0.0, synth.HARD_FIXED, 1)
+    assert ei.value.status == lcf.ERR_UNSUPPORTED
+    # the largest supported fp32 size still creates and runs
+    iq = synth.random_cube(16, 16, 200, seed=3)
+    f = synth.FilterSpec(1, 1, 0.0, 0.0, 0.0, synth.HARD_FIXED, k_fixed=1)
+    g = gpu_run(lcf, iq, f)
+    assert np.isfinite(g["PD"]).all() and g["sweeps"].max() < 24
