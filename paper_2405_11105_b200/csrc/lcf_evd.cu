@@ -45,7 +45,7 @@ struct JacArgs {
     int Tn;                 // Gram tile grid (canonical entry rule)
     int max_sweeps;
     const int* gfirst;      // [K+1]
-    const void* part;       // [slot][N][N] complex T
+    const double2* part;    // [slot][N][N] complex double
     void* R;                // [K][N][N] complex T
     void* rotlog;           // [K][max_sweeps*M][3][NP] T
     double* lam;            // [K][N] descending
@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
 
     // ---- load: R = sum of the Gram partials (fixed order), canonical half per entry ----
     {
-        const C* part = reinterpret_cast<const C*>(a.part);
+        const double2* part = a.part;
         C* Rk = reinterpret_cast<C*>(a.R) + (size_t)k * N * N;
         const int s0 = a.gfirst[k], s1 = a.gfirst[k + 1];
         const int nup = Ns * (Ns + 1) / 2;
@@ -113,10 +113,12 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
             if (v < N) {
                 const bool direct = (u % a.Tn) <= (v % a.Tn);
                 const size_t idx = direct ? (size_t)u * N + v : (size_t)v * N + u;
+                double dre = 0.0, dim = 0.0;
                 for (int s = s0; s < s1; ++s) {
-                    C x = part[(size_t)s * N * N + idx];
-                    re += x.x; im += x.y;
+                    const double2 x = part[(size_t)s * N * N + idx];
+                    dre += x.x; dim += x.y;
                 }
+                re = (T)dre; im = (T)dim;
                 if (!direct) im = -im;
                 if (u == v) im = T(0);
                 C o; o.x = re; o.y = im;

@@ -9,8 +9,12 @@
 // (ti, tj) owns rows {ti + Tn*ii} and columns {tj + Tn*jj} (strided, so a warp's operand reads are
 // bank-conflict free); only tiles with ti <= tj are computed (Hermitian symmetry) -- entry (i, j) is
 // canonical iff (i mod Tn) <= (j mod Tn), the other half is its conjugate.  Partial sums go to a
-// per-chunk buffer that the EVD kernel's loader reduces in a fixed order (deterministic, no atomics).
-// T = float: FP32 FMA.  T = double: the fp32 samples are widened, products are exact in fp64.
+// per-chunk fp64 buffer that the EVD kernel's loader reduces in a fixed order (deterministic, no
+// atomics).  T = float: FP32 FMA (products exact inside the FMA), but an fp32 accumulator only ever
+// sums GRAM_FLUSH_TILES * GRAM_TP pixels: it is then added into the CTA's fp64 partial and cleared.
+// A plain fp32 running sum over a whole chunk (thousands of pixels) loses ~1e-5 of |R|, which the
+// 60-70 dB clutter-to-blood ratio amplifies into >1e-3 power-Doppler errors.
+// T = double: the fp32 samples are widened, products are exact in fp64, one store at the end.
 #include "lcf_internal.h"
 
 namespace lcf {
@@ -25,7 +29,7 @@ struct GramArgs {
     int Nx;
     const WinBox* box;
     const GramItem* items;
-    void* part;  // [slot][N][N] complex T
+    double2* part;  // [slot][N][N] complex double
 };
 
 template <typename T> struct Cx;
@@ -102,6 +106,34 @@ __global__ void __launch_bounds__(GRAM_THREADS, (sizeof(T) == 4 ? 2 : 1)) gram_k
         cp_async_commit();
     };
 
+    // add the register tile into this CTA's fp64 partial (first flush overwrites: no memset needed)
+    int nflushed = 0;
+    auto flush = [&](bool first) {
+        if (active) {
+            double2* out = a.part + (size_t)it.pslot * N * N + (size_t)ti * N + tj;
+#pragma unroll
+            for (int i = 0; i < TM; ++i) {
+                if (ti + Tn * i < N) {
+#pragma unroll
+                    for (int j = 0; j < TM; ++j) {
+                        if (tj + Tn * j < N) {
+                            double2* o = out + Tn * j;
+                            double2 v = make_double2(0.0, 0.0);
+                            if (!first) v = *o;
+                            v.x += (double)acc_re[i][j]; v.y += (double)acc_im[i][j];
+                            *o = v;
+                        }
+                    }
+                }
+                out += (size_t)Tn * N;
+                asm volatile("" ::: "memory");   // one row of the tile at a time: bounds the live loads
+#pragma unroll
+                for (int j = 0; j < TM; ++j) { acc_re[i][j] = T(0); acc_im[i][j] = T(0); }
+            }
+        }
+        ++nflushed;
+    };
+
     long long off; T w;
     bool valid = pixel(0, off, w);
     issue(off, valid);
@@ -161,21 +193,8 @@ __global__ void __launch_bounds__(GRAM_THREADS, (sizeof(T) == 4 ? 2 : 1)) gram_k
                 }
             }
         }
-    }
-    if (active) {
-        C* out = reinterpret_cast<C*>(a.part) + (size_t)it.pslot * N * N;
-#pragma unroll
-        for (int i = 0; i < TM; ++i) {
-            int row = ti + Tn * i;
-            if (row >= N) continue;
-#pragma unroll
-            for (int j = 0; j < TM; ++j) {
-                int col = tj + Tn * j;
-                if (col >= N) continue;
-                C v; v.x = acc_re[i][j]; v.y = acc_im[i][j];
-                out[(size_t)row * N + col] = v;
-            }
-        }
+        // single flush site (keeps the accumulators out of local memory)
+        if (tile + 1 == ntile || (sizeof(T) == 4 && (tile + 1) % GRAM_FLUSH_TILES == 0)) flush(nflushed == 0);
     }
 }
 

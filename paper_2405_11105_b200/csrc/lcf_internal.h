@@ -30,6 +30,7 @@ struct ProjItem {
 };
 
 constexpr int GRAM_TP = 32;        // pixels per shared-memory tile of the Gram kernel
+constexpr int GRAM_FLUSH_TILES = 16; // fp32 accumulators are folded into the fp64 partial every 16 tiles (512 px)
 constexpr int GRAM_THREADS = 160;  // max thread tiles per Gram CTA (136 upper tiles at N=128)
 constexpr int PROJ_TPIX = 64;      // pixels per projection CTA
 constexpr int PROJ_KT = 16;        // frames per pipeline stage of the projection kernel
@@ -71,7 +72,7 @@ struct lcf_plan {
     lcf::GramItem* gitems_d = nullptr;
     int n_gitems = 0, n_gslots = 0, gram_Tn = 0, gram_TM = 0, gram_tiles_per_batch = 0, gram_batches = 0;
     int* gfirst_d = nullptr;
-    void* gpart_d = nullptr;   // [n_gslots][N][N] complex real
+    double2* gpart_d = nullptr; // [n_gslots][N][N] complex double (canonical half written)
     void* R_d = nullptr;       // [K][N][N] complex real (full Hermitian)
     // EVD
     void* rotlog_d = nullptr;  // [K][max_sweeps*(Ns-1)][3][NP] real

@@ -213,7 +213,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
          dev_upload(&p->kxhi_d, kxhi);
     ok = ok && dev_upload(&p->gitems_d, gitems) && dev_upload(&p->gfirst_d, p->gfirst_h);
     ok = ok && dev_upload(&p->pitems_d, pitems) && dev_upload(&p->pfirst_d, p->pfirst_h);
-    ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->gpart_d), (size_t)p->n_gslots * N2 * 2 * p->esz);
+    ok = ok && dev_alloc(&p->gpart_d, (size_t)p->n_gslots * N2);
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->R_d), K * N2 * 2 * p->esz);
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->rotlog_d), K * p->max_sweeps * M * 3 * p->NP * p->esz);
     ok = ok && dev_alloc(&p->lam_d, K * N) && dev_alloc(&p->order_d, K * N) && dev_alloc(&p->cut_d, K) &&
@@ -231,7 +231,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     }
     // the Gram kernel leaves the non-canonical half of each partial unwritten; clear once so no
     // uninitialised memory is ever read by tools (the loader never reads that half)
-    cudaMemset(p->gpart_d, 0, (size_t)p->n_gslots * N2 * 2 * p->esz);
+    cudaMemset(p->gpart_d, 0, (size_t)p->n_gslots * N2 * sizeof(double2));
     if (cudaDeviceSynchronize() != cudaSuccess) {
         free_plan_device(p);
         delete p;
