@@ -123,6 +123,11 @@ lcf_status lcf_get_work(const lcf_plan* plan, lcf_work* out /* HOST */);
 lcf_status lcf_measure_peak(int kind, double* tflops /* HOST */);
 
 const char* lcf_status_string(lcf_status s);
+/* After LCF_ERR_CUDA from lcf_filter: "<stage>: <CUDA error string>" of the first failed launch
+ * (stages: gram, evd, weights/projector, projection, combine); "" if none.  HOST string owned by
+ * the plan.  Launch failures are sticky; asynchronous execution faults surface at the next call
+ * that synchronises (run with CUDA_LAUNCH_BLOCKING=1 to attribute them to a stage). */
+const char* lcf_last_error(const lcf_plan* plan);
 
 #ifdef __cplusplus
 }

@@ -43,6 +43,7 @@ __device__ __forceinline__ void pair_pq(int m, int s, int M, int& p, int& q) {
 struct JacArgs {
     int N, NP, M, Ns;       // Ns = 2 NP slots, M = Ns - 1
     int Tn;                 // Gram tile grid (canonical entry rule)
+    int from_R;             // 1: R already holds the reduced Hermitian matrices (tensor-core Gram)
     int max_sweeps;
     const int* gfirst;      // [K+1]
     const double2* part;    // [slot][N][N] complex double
@@ -110,7 +111,10 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
             while ((u + 1) * (2 * Ns - u) / 2 <= e) ++u;
             int v = u + (e - u * (2 * Ns - u + 1) / 2);
             T re = T(0), im = T(0);
-            if (v < N) {
+            if (v < N && a.from_R) {
+                const C x = Rk[(size_t)u * N + v];
+                re = x.x; im = (u == v) ? T(0) : x.y;
+            } else if (v < N) {
                 const bool direct = (u % a.Tn) <= (v % a.Tn);
                 const size_t idx = direct ? (size_t)u * N + v : (size_t)v * N + u;
                 double dre = 0.0, dim = 0.0;
@@ -434,6 +438,7 @@ cudaError_t configure_evd(lcf_plan* p) {
 cudaError_t launch_jacobi(lcf_plan* p, cudaStream_t st) {
     JacArgs a;
     a.N = p->N; a.NP = p->NP; a.M = p->Ns - 1; a.Ns = p->Ns; a.Tn = p->gram_Tn; a.max_sweeps = p->max_sweeps;
+    a.from_R = p->gram_tc ? 1 : 0;
     a.gfirst = p->gfirst_d; a.part = p->gpart_d; a.R = p->R_d; a.rotlog = p->rotlog_d;
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;

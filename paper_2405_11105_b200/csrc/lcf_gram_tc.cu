@@ -1,0 +1,407 @@
+// lcf_gram_tc.cu -- kernel 1, tensor-core path: batched window-weighted complex Gram (Eq. 12,
+// PAPER.md:149-152) on tcgen05 with a 3xTF32 split, for precision 0 and N <= 128.
+//
+//   R_k[i][j] = sum_p w_k(p)^2 conj(S[i][p]) S[j][p]            X = W_k S (Eq. 11), X = Xr + i Xi
+//   Re R = Xr Xr^T + Xi Xi^T          Im R = G - G^T,  G = Xr Xi^T          (frames x frames, K = pixels)
+//
+// Every fp32 sample is split x = hi + lo (hi = x rounded to TF32, lo = (x - hi) rounded to TF32), so
+//   Re R = D0 + H + H^T      D0 = Rh Rh^T + Ih Ih^T        H = Rh Rl^T + Ih Il^T
+//   Im R = (G0 + L) - (G0 + L)^T     G0 = Rh Ih^T          L = Rh Il^T - Ih Rl^T
+// (the lo.lo products, 2^-22 of a term, are dropped).  Seven 128 x Np x 8 tcgen05.mma per 8 pixels
+// into four TMEM accumulators (4 x 128 columns = all 512).
+//
+// Persistent CTAs (one per SM) walk a static, contiguous slice of the global list of 16-pixel
+// tiles (16 z-contiguous pixels of one window: one 128-byte row per frame), cut into segments at
+// window boundaries.  Roles (320 threads):
+//   warp 0      TMA producer: [N frames][16 px] complex64 box -> 128B-swizzled raw stage, plus the
+//               16 window weights of the tile;
+//   warps 2-9   converters: raw stage -> w * s -> hi/lo -> four K-major operand tiles (canonical
+//               no-swizzle core-matrix layout) -> fence.proxy.async -> mbarrier;
+//   warp 1      one thread issues the MMAs and commits them to mbarriers.
+// tcgen05 accumulates in fp32 with truncation (measured: 2^24 + 1.5 -> 2^24), a bias that grows
+// with the number of adds into a large running sum; D0 and G0 are therefore drained every
+// GTC_GROUP tiles (128 pixels = 32 adds) into fp32 registers of the converter warps (round to
+// nearest), H and L (2^-11 of the main terms) stay in TMEM for the whole segment.  Each segment
+// ends by writing four 128 x 128 fp32 partials; gram_tc_reduce_kernel sums a window's segments in
+// fp64, applies the (anti)symmetrisation above and writes the full Hermitian R_k.
+#include <cuda.h>
+
+#include "lcf_internal.h"
+#include "lcf_sm100.cuh"
+
+namespace lcf {
+
+using namespace sm100;
+
+constexpr int GTC_PX = 16;                 // pixels per tile
+constexpr int GTC_RT = 128;                // operand tile rows (frames, zero padded)
+constexpr int GTC_RAW_STAGES = 4;
+constexpr int GTC_OP_STAGES = 4;
+constexpr int GTC_LAG = 3;                 // tiles the converters run ahead before draining a group
+constexpr int GTC_CONV_WARPS = 8;
+constexpr int GTC_THREADS = 32 * (2 + GTC_CONV_WARPS);
+constexpr int GTC_TILE_BYTES = GTC_RT * GTC_PX * 4;      // one operand tile: 8 KB
+constexpr int GTC_OP_BYTES = 4 * GTC_TILE_BYTES;         // Rh, Ih, Rl, Il
+constexpr int GTC_LBO = GTC_RT * 16;                     // next 4-pixel K chunk
+constexpr int GTC_SBO = 128;                             // next 8-frame row group
+
+struct GtcArgs {
+    int N, Np, Nz, Nx, Kz;
+    int group;                 // tiles per D0/G0 drain
+    const double* gz;          // [Kz][Nz]
+    const double* gx;          // [Kx][Nx]
+    const WinBox* box;
+    const GtcSeg* segs;
+    const int* cta_first;      // [grid+1]
+    float* part;               // [nseg][4][128][128]
+    uint32_t raw_stride;       // bytes between raw stages (multiple of 1024)
+};
+
+struct GtcBars {
+    uint64_t full[GTC_RAW_STAGES], empty[GTC_RAW_STAGES];
+    uint64_t opfull[GTC_OP_STAGES], opempty[GTC_OP_STAGES];
+    uint64_t accfull, accempty;
+    uint32_t tmem_base;
+    alignas(16) float wts[GTC_RAW_STAGES][GTC_PX];
+};
+
+__device__ __forceinline__ void split_tf32(float v, float& hi, float& lo) {
+    // round to nearest (ties away) on the 13 dropped mantissa bits, in integer arithmetic
+    hi = __uint_as_float((__float_as_uint(v) + 0x1000u) & 0xFFFFE000u);
+    const float r = v - hi;     // exact
+    lo = __uint_as_float((__float_as_uint(r) + 0x1000u) & 0xFFFFE000u);
+}
+
+__global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_constant__ CUtensorMap tmap, GtcArgs a) {
+    extern __shared__ __align__(1024) unsigned char smem_dyn[];
+    unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
+    unsigned char* raw = sbase;                                               // [RAW_STAGES][raw_stride]
+    unsigned char* ops = sbase + (size_t)GTC_RAW_STAGES * a.raw_stride;       // [OP_STAGES][GTC_OP_BYTES]
+    GtcBars* bars = reinterpret_cast<GtcBars*>(ops + (size_t)GTC_OP_STAGES * GTC_OP_BYTES);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int N = a.N;
+    const int seg0 = a.cta_first[blockIdx.x], seg1 = a.cta_first[blockIdx.x + 1];
+
+    // ---- one-time setup: zero the operand stages (rows >= N are never written), barriers, TMEM
+    for (int i = tid * 16; i < GTC_OP_STAGES * GTC_OP_BYTES; i += GTC_THREADS * 16) *reinterpret_cast<uint4*>(ops + i) = make_uint4(0, 0, 0, 0);
+    fence_proxy_async_smem();
+    if (tid == 0) {
+        for (int s = 0; s < GTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], GTC_CONV_WARPS * 32); }
+        for (int s = 0; s < GTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], GTC_CONV_WARPS * 32); mbar_init(&bars->opempty[s], 1); }
+        mbar_init(&bars->accfull, 1);
+        mbar_init(&bars->accempty, GTC_CONV_WARPS * 32);
+        mbar_fence_init();
+    }
+    if (warp == 1) tmem_alloc<512>(&bars->tmem_base);
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
+    const uint32_t tmem = bars->tmem_base;
+
+    if (warp == 0) {
+        // =========================== TMA producer ===========================
+        if (lane == 0) tma_prefetch_desc(&tmap);
+        uint32_t it = 0;
+        for (int sg = seg0; sg < seg1; ++sg) {
+            const GtcSeg seg = a.segs[sg];
+            const WinBox bx = a.box[seg.k];
+            const int ze = bx.z0 & ~1;    // TMA needs a 16-byte aligned start in the swizzled inner dimension
+            const int ntz = (bx.z0 + bx.Lz - ze + GTC_PX - 1) / GTC_PX;
+            const double* gz = a.gz + (size_t)bx.kz * a.Nz;
+            const double* gx = a.gx + (size_t)bx.kx * a.Nx;
+            for (int t = 0; t < seg.ntile; ++t, ++it) {
+                const int s = it % GTC_RAW_STAGES;
+                const uint32_t ph = (it / GTC_RAW_STAGES) & 1;
+                const int tau = seg.tile0 + t;
+                const int txi = tau / ntz, tzi = tau - txi * ntz;
+                const int z = ze + tzi * GTC_PX, x = bx.x0 + txi;
+                mbar_wait(&bars->empty[s], ph ^ 1);
+                if (lane < GTC_PX) {
+                    const int zz = z + lane;
+                    float w = 0.f;
+                    if (zz < a.Nz && x < a.Nx) w = (float)(gz[zz] * gx[x]);
+                    bars->wts[s][lane] = w;
+                }
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive_expect_tx(&bars->full[s], (uint32_t)((N + 7) / 8 * 8) * 128u);
+                    tma_load_3d(raw + (size_t)s * a.raw_stride, &tmap, 2 * z, x, 0, &bars->full[s]);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // =========================== MMA issuer ===========================
+        if (lane == 0) {
+            const uint32_t idesc = make_idesc_tf32(GTC_RT, a.Np, false, false, false, false);
+            const uint32_t idesc_na = make_idesc_tf32(GTC_RT, a.Np, false, false, true, false);
+            const uint32_t tD0 = tmem, tG0 = tmem + 128, tH = tmem + 256, tL = tmem + 384;
+            uint32_t it = 0, gc = 0;
+            for (int sg = seg0; sg < seg1; ++sg) {
+                const int nt = a.segs[sg].ntile;
+                for (int t = 0; t < nt; ++t, ++it) {
+                    const int o = it % GTC_OP_STAGES;
+                    const uint32_t pho = (it / GTC_OP_STAGES) & 1;
+                    const bool group_first = (t % a.group) == 0;
+                    const bool group_last = ((t + 1) % a.group) == 0 || t + 1 == nt;
+                    mbar_wait(&bars->opfull[o], pho);
+                    if (group_first) mbar_wait(&bars->accempty, (gc & 1) ^ 1);
+                    tc_fence_after_sync();
+                    const uint32_t ob = smem_u32(ops + (size_t)o * GTC_OP_BYTES);
+#pragma unroll
+                    for (int ks = 0; ks < GTC_PX / 8; ++ks) {
+                        const uint32_t koff = ks * 2 * GTC_LBO;
+                        const uint64_t dRh = make_smem_desc(ob + 0 * GTC_TILE_BYTES + koff, GTC_LBO, GTC_SBO, SWZ_NONE);
+                        const uint64_t dIh = make_smem_desc(ob + 1 * GTC_TILE_BYTES + koff, GTC_LBO, GTC_SBO, SWZ_NONE);
+                        const uint64_t dRl = make_smem_desc(ob + 2 * GTC_TILE_BYTES + koff, GTC_LBO, GTC_SBO, SWZ_NONE);
+                        const uint64_t dIl = make_smem_desc(ob + 3 * GTC_TILE_BYTES + koff, GTC_LBO, GTC_SBO, SWZ_NONE);
+                        const uint32_t accg = (group_first && ks == 0) ? 0u : 1u;   // D0, G0 restart per group
+                        const uint32_t accs = (t == 0 && ks == 0) ? 0u : 1u;        // H, L restart per segment
+                        mma_tf32(tD0, dRh, dRh, idesc, accg);
+                        mma_tf32(tD0, dIh, dIh, idesc, 1u);
+                        mma_tf32(tG0, dRh, dIh, idesc, accg);
+                        mma_tf32(tH, dRh, dRl, idesc, accs);
+                        mma_tf32(tH, dIh, dIl, idesc, 1u);
+                        mma_tf32(tL, dRh, dIl, idesc, accs);
+                        mma_tf32(tL, dIh, dRl, idesc_na, 1u);
+                    }
+                    mma_commit(&bars->opempty[o]);
+                    if (group_last) { mma_commit(&bars->accfull); ++gc; }
+                }
+            }
+        }
+    } else {
+        // =========================== converters / accumulator drain ===========================
+        const int cw = warp - 2;                      // 0..7
+        const int quad = warp & 3;                    // TMEM lane quadrant this warp may touch
+        const int half = cw >> 2;                     // which 64 columns of D0 / G0 this warp keeps
+        const uint32_t tlane = tmem + ((uint32_t)(quad * 32) << 16);
+        const int row = quad * 32 + lane;
+        float acc[128];
+#pragma unroll
+        for (int i = 0; i < 128; ++i) acc[i] = 0.f;
+        const int nwt = 4 * ((N + 31) / 32);          // warp tasks per tile: (4-pixel chunk, 32-frame block)
+        uint32_t it = 0, gc = 0;
+
+        auto drain_group = [&]() {                    // D0, G0 of the finished group -> registers
+            mbar_wait(&bars->accfull, gc & 1);
+            tc_fence_after_sync();
+#pragma unroll
+            for (int blk = 0; blk < 8; ++blk) {
+                uint32_t v[16];
+                const uint32_t col = (blk < 4 ? 0u : 128u) + half * 64 + (blk & 3) * 16;
+                tmem_ld16(tlane + col, v);
+                tmem_ld_wait();
+#pragma unroll
+                for (int j = 0; j < 16; ++j) acc[blk * 16 + j] += __uint_as_float(v[j]);
+            }
+        };
+        auto release_acc = [&]() {
+            tc_fence_before_sync();
+            mbar_arrive(&bars->accempty);
+            ++gc;
+        };
+
+        for (int sg = seg0; sg < seg1; ++sg) {
+            const GtcSeg seg = a.segs[sg];
+            const int nt = seg.ntile;
+            const int ngroups = (nt + a.group - 1) / a.group;
+            int drained = 0;
+            for (int t = 0; t < nt; ++t, ++it) {
+                const int s = it % GTC_RAW_STAGES, o = it % GTC_OP_STAGES;
+                const uint32_t ph = (it / GTC_RAW_STAGES) & 1, pho = (it / GTC_OP_STAGES) & 1;
+                const unsigned char* rs = raw + (size_t)s * a.raw_stride;
+                unsigned char* os = ops + (size_t)o * GTC_OP_BYTES;
+                mbar_wait(&bars->full[s], ph);
+                mbar_wait(&bars->opempty[o], pho ^ 1);
+                for (int wt = cw; wt < nwt; wt += GTC_CONV_WARPS) {
+                    const int c4 = wt & 3, fr = (wt >> 2) * 32 + lane;
+                    if (fr < N) {
+                        const float4 w4 = *reinterpret_cast<const float4*>(&bars->wts[s][c4 * 4]);
+                        const uint32_t rowoff = (uint32_t)fr * 128u, sw = (uint32_t)(fr & 7);
+                        const float4 p01 = *reinterpret_cast<const float4*>(rs + rowoff + (((2 * c4) ^ sw) << 4));
+                        const float4 p23 = *reinterpret_cast<const float4*>(rs + rowoff + (((2 * c4 + 1) ^ sw) << 4));
+                        float4 rh, ih, rl, il;
+                        split_tf32(w4.x * p01.x, rh.x, rl.x); split_tf32(w4.x * p01.y, ih.x, il.x);
+                        split_tf32(w4.y * p01.z, rh.y, rl.y); split_tf32(w4.y * p01.w, ih.y, il.y);
+                        split_tf32(w4.z * p23.x, rh.z, rl.z); split_tf32(w4.z * p23.y, ih.z, il.z);
+                        split_tf32(w4.w * p23.z, rh.w, rl.w); split_tf32(w4.w * p23.w, ih.w, il.w);
+                        unsigned char* dst = os + (size_t)c4 * GTC_LBO + (size_t)fr * 16;
+                        *reinterpret_cast<float4*>(dst + 0 * GTC_TILE_BYTES) = rh;
+                        *reinterpret_cast<float4*>(dst + 1 * GTC_TILE_BYTES) = ih;
+                        *reinterpret_cast<float4*>(dst + 2 * GTC_TILE_BYTES) = rl;
+                        *reinterpret_cast<float4*>(dst + 3 * GTC_TILE_BYTES) = il;
+                    }
+                }
+                mbar_arrive(&bars->empty[s]);         // raw stage (and its weights) consumed
+                fence_proxy_async_smem();
+                mbar_arrive(&bars->opfull[o]);
+                // drain finished, non-final groups a few tiles late so the MMA queue stays fed
+                while (drained < ngroups - 1 && (drained + 1) * a.group - 1 <= t - GTC_LAG) {
+                    drain_group();
+                    release_acc();
+                    ++drained;
+                }
+            }
+            while (drained < ngroups - 1) { drain_group(); release_acc(); ++drained; }
+            // ---- segment end: last group, then the four partials of this segment
+            drain_group();
+            float* out = a.part + (size_t)sg * 4 * 128 * 128 + (size_t)row * 128 + half * 64;
+#pragma unroll
+            for (int m = 0; m < 2; ++m) {
+#pragma unroll
+                for (int j = 0; j < 64; j += 4)
+                    *reinterpret_cast<float4*>(out + (size_t)m * 128 * 128 + j) =
+                        make_float4(acc[m * 64 + j], acc[m * 64 + j + 1], acc[m * 64 + j + 2], acc[m * 64 + j + 3]);
+            }
+#pragma unroll
+            for (int i = 0; i < 128; ++i) acc[i] = 0.f;
+#pragma unroll
+            for (int blk = 0; blk < 8; ++blk) {
+                uint32_t v[16];
+                const int m = 2 + (blk >> 2);
+                const uint32_t col = (uint32_t)m * 128u + half * 64 + (blk & 3) * 16;
+                tmem_ld16(tlane + col, v);
+                tmem_ld_wait();
+                float* o2 = out + (size_t)m * 128 * 128 + (blk & 3) * 16;
+#pragma unroll
+                for (int j = 0; j < 16; j += 4)
+                    *reinterpret_cast<float4*>(o2 + j) = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]),
+                                                                     __uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
+            }
+            release_acc();
+        }
+    }
+    tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc<512>(tmem);
+}
+
+// R_k = sum over the window's segments, in fp64:  Re R = D0 + H + H^T,  Im R = (G0 + L) - (G0 + L)^T
+template <typename T>
+__global__ void gram_tc_reduce_kernel(const float* part, const int* seg_first, int N, void* Rv) {
+    const int k = blockIdx.z;
+    const int i = blockIdx.y * 16 + threadIdx.y, j = blockIdx.x * 16 + threadIdx.x;
+    if (i >= N || j >= N) return;
+    double re = 0.0, im = 0.0;
+    for (int s = seg_first[k]; s < seg_first[k + 1]; ++s) {
+        const float* p = part + (size_t)s * 4 * 128 * 128;
+        const size_t ij = (size_t)i * 128 + j, ji = (size_t)j * 128 + i;
+        re += (double)p[ij] + ((double)p[2 * 16384 + ij] + (double)p[2 * 16384 + ji]);
+        im += ((double)p[16384 + ij] - (double)p[16384 + ji]) + ((double)p[3 * 16384 + ij] - (double)p[3 * 16384 + ji]);
+    }
+    if (i == j) im = 0.0;
+    if (sizeof(T) == 4) {
+        float2* R = reinterpret_cast<float2*>(Rv) + (size_t)k * N * N;
+        R[(size_t)i * N + j] = make_float2((float)re, (float)im);
+    } else {
+        double2* R = reinterpret_cast<double2*>(Rv) + (size_t)k * N * N;
+        R[(size_t)i * N + j] = make_double2(re, im);
+    }
+}
+
+// ---------------------------------------------------------------- host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// [N][Nx][Nz] complex64 seen as float [N][Nx][2 Nz]; box = 16 pixels x 1 x N frames, 128B swizzle
+static bool encode_iq_map(lcf_plan* p, const void* iq) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[3] = {(cuuint64_t)2 * p->Nz, (cuuint64_t)p->Nx, (cuuint64_t)p->N};
+    cuuint64_t strides[2] = {(cuuint64_t)p->Nz * 8, (cuuint64_t)p->P * 8};
+    cuuint32_t box[3] = {2 * GTC_PX, 1, (cuuint32_t)((p->N + 7) / 8 * 8)};   // whole 1024-byte swizzle atoms; frames >= N are zero-filled
+    cuuint32_t es[3] = {1, 1, 1};
+    CUresult r = fn(reinterpret_cast<CUtensorMap*>(p->gtc_tmap), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(iq), dims,
+                    strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return false;
+    p->gtc_tmap_iq = iq;
+    return true;
+}
+
+bool gram_tc_eligible(const lcf_plan* p) {
+    return p->prec == 0 && p->N <= 128 && p->N >= 2 && (p->Nz % 2) == 0 && encode_fn() != nullptr;
+}
+
+// work decomposition: static contiguous slices of the global tile list, cut at window boundaries
+cudaError_t configure_gram_tc(lcf_plan* p, std::vector<GtcSeg>& segs, std::vector<int>& cta_first, std::vector<int>& seg_first) {
+    const int K = p->K;
+    std::vector<long long> nt(K);
+    long long T = 0;
+    for (int k = 0; k < K; ++k) {
+        const WinBox& b = p->box_h[k];
+        nt[k] = b.Pk > 0 ? (long long)((b.z0 + b.Lz - (b.z0 & ~1) + GTC_PX - 1) / GTC_PX) * b.Lx : 0;
+        T += nt[k];
+    }
+    int grid = (int)(T < p->num_sms ? T : p->num_sms);
+    if (grid < 1) grid = 1;
+    p->gtc_grid = grid;
+    segs.clear();
+    cta_first.assign(grid + 1, 0);
+    seg_first.assign(K + 1, 0);
+    // global tile g in [0,T): window by prefix sums
+    std::vector<long long> pre(K + 1, 0);
+    for (int k = 0; k < K; ++k) pre[k + 1] = pre[k] + nt[k];
+    std::vector<std::vector<GtcSeg>> per_cta(grid);
+    for (int b = 0; b < grid; ++b) {
+        long long g0 = T * b / grid, g1 = T * (b + 1) / grid;
+        int k = 0;
+        while (g0 < g1) {
+            while (k < K && pre[k + 1] <= g0) ++k;
+            long long e = pre[k + 1] < g1 ? pre[k + 1] : g1;
+            per_cta[b].push_back({k, (int)(g0 - pre[k]), (int)(e - g0), 0});
+            g0 = e;
+        }
+    }
+    for (int b = 0; b < grid; ++b) {
+        cta_first[b] = (int)segs.size();
+        for (auto& s : per_cta[b]) segs.push_back(s);
+    }
+    cta_first[grid] = (int)segs.size();
+    // segments are in global tile order, so each window's segments are contiguous
+    int si = 0;
+    for (int k = 0; k < K; ++k) {
+        seg_first[k] = si;
+        while (si < (int)segs.size() && segs[si].k == k) ++si;
+    }
+    seg_first[K] = si;
+    p->gtc_nseg = (int)segs.size();
+    p->gtc_raw_stride = (uint32_t)(((size_t)p->N * 128 + 1023) / 1024 * 1024);
+    p->gtc_smem = 1024 + (size_t)GTC_RAW_STAGES * p->gtc_raw_stride + (size_t)GTC_OP_STAGES * GTC_OP_BYTES + sizeof(GtcBars);
+    if (p->gtc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
+    return cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gtc_smem);
+}
+
+cudaError_t launch_gram_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
+    if (p->gtc_nseg == 0) return cudaSuccess;
+    if (p->gtc_tmap_iq != (const void*)iq && !encode_iq_map(p, iq)) return cudaErrorInvalidValue;
+    GtcArgs a;
+    a.N = p->N; a.Np = (p->N + 15) / 16 * 16; a.Nz = p->Nz; a.Nx = p->Nx; a.Kz = p->Kz;
+    a.group = p->gtc_group;
+    a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->gtc_segs_d; a.cta_first = p->gtc_cta_first_d;
+    a.part = p->gtc_part_d; a.raw_stride = p->gtc_raw_stride;
+    gram_tc_kernel<<<p->gtc_grid, GTC_THREADS, p->gtc_smem, st>>>(*reinterpret_cast<const CUtensorMap*>(p->gtc_tmap), a);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    dim3 blk(16, 16), grid((p->N + 15) / 16, (p->N + 15) / 16, p->K);
+    gram_tc_reduce_kernel<float><<<grid, blk, 0, st>>>(p->gtc_part_d, p->gtc_seg_first_d, p->N, p->R_d);
+    return cudaGetLastError();
+}
+
+}  // namespace lcf

@@ -28,6 +28,10 @@ struct GramItem {
 struct ProjItem {
     int k, q0, q1;
 };
+// One segment of the tensor-core Gram: `ntile` consecutive 16-pixel tiles of window k from tile0.
+struct GtcSeg {
+    int k, tile0, ntile, pad_;
+};
 
 constexpr int GRAM_TP = 32;        // pixels per shared-memory tile of the Gram kernel
 constexpr int GRAM_FLUSH_TILES = 16; // fp32 accumulators are folded into the fp64 partial every 16 tiles (512 px)
@@ -74,6 +78,16 @@ struct lcf_plan {
     int* gfirst_d = nullptr;
     double2* gpart_d = nullptr; // [n_gslots][N][N] complex double (canonical half written)
     void* R_d = nullptr;       // [K][N][N] complex real (full Hermitian)
+    // tensor-core Gram (precision 0, N <= 128): lcf_gram_tc.cu
+    bool gram_tc = false;
+    int gtc_grid = 0, gtc_nseg = 0, gtc_group = 8;
+    uint32_t gtc_raw_stride = 0;
+    size_t gtc_smem = 0;
+    lcf::GtcSeg* gtc_segs_d = nullptr;
+    int *gtc_cta_first_d = nullptr, *gtc_seg_first_d = nullptr;
+    float* gtc_part_d = nullptr;            // [nseg][4][128][128]
+    alignas(64) unsigned char gtc_tmap[128];  // CUtensorMap of the last iq pointer
+    const void* gtc_tmap_iq = nullptr;
     // EVD
     void* rotlog_d = nullptr;  // [K][max_sweeps*(Ns-1)][3][NP] real
     double* lam_d = nullptr;   // [K][N] descending
@@ -102,6 +116,7 @@ struct lcf_plan {
     cudaStream_t last_stream = nullptr;
     bool ran = false;
     bool cuda_failed = false;
+    char last_error[160] = "";   // stage and CUDA error string of the first failed launch
     bool timing = false;
     lcf::StageTimer timer;
     int smem_optin = 0;
@@ -123,4 +138,7 @@ cudaError_t launch_build_filters(lcf_plan* p, cudaStream_t st);
 cudaError_t configure_gram(lcf_plan* p);     // each: opt-in shared memory size, launch geometry
 cudaError_t configure_evd(lcf_plan* p);
 cudaError_t configure_project(lcf_plan* p);
+bool gram_tc_eligible(const lcf_plan* p);
+cudaError_t configure_gram_tc(lcf_plan* p, std::vector<GtcSeg>& segs, std::vector<int>& cta_first, std::vector<int>& seg_first);
+cudaError_t launch_gram_tc(lcf_plan* p, const float2* iq, cudaStream_t st);
 }  // namespace lcf

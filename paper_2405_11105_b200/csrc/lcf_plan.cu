@@ -3,6 +3,7 @@
 // steps a1..a5), diagnostics getters.  Host code only builds tables and moves bytes; every step of
 // the path runs in the kernels of lcf_gram.cu / lcf_evd.cu / lcf_project.cu.
 #include <cmath>
+#include <cstdio>
 #include <cstring>
 #include <new>
 
@@ -59,6 +60,7 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->V_d); cudaFree(p->B_d); cudaFree(p->pitems_d); cudaFree(p->pfirst_d);
     cudaFree(p->tiles_d); cudaFree(p->tsum_d); cudaFree(p->mean_d); cudaFree(p->alpha_d);
     cudaFree(p->F_d); cudaFree(p->iq_stage_d); cudaFree(p->pd_stage_d);
+    cudaFree(p->gtc_segs_d); cudaFree(p->gtc_cta_first_d); cudaFree(p->gtc_seg_first_d); cudaFree(p->gtc_part_d);
     if (p->timer.have)
         for (auto& set : p->timer.ev)
             for (auto& e : set) cudaEventDestroy(e);
@@ -167,10 +169,18 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
         return LCF_ERR_UNSUPPORTED;
     }
 
+    // ---- tensor-core Gram decomposition (precision 0, N <= 128, even Nz) ----
+    std::vector<GtcSeg> gtc_segs;
+    std::vector<int> gtc_cta_first, gtc_seg_first;
+    p->gram_tc = gram_tc_eligible(p);
+    if (p->gram_tc && configure_gram_tc(p, gtc_segs, gtc_cta_first, gtc_seg_first) != cudaSuccess) {
+        cudaGetLastError();
+        p->gram_tc = false;
+    }
     // ---- Gram work items: each window's box split into pixel chunks (multiples of GRAM_TP) ----
     std::vector<GramItem> gitems;
     p->gfirst_h.assign(p->K + 1, 0);
-    {
+    if (!p->gram_tc) {
         long long target = p->sumPk / ((long long)p->num_sms * 6) + 1;
         long long ch = ((target + GRAM_TP - 1) / GRAM_TP) * GRAM_TP;
         if (ch < 4 * GRAM_TP) ch = 4 * GRAM_TP;
@@ -214,6 +224,11 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     ok = ok && dev_upload(&p->gitems_d, gitems) && dev_upload(&p->gfirst_d, p->gfirst_h);
     ok = ok && dev_upload(&p->pitems_d, pitems) && dev_upload(&p->pfirst_d, p->pfirst_h);
     ok = ok && dev_alloc(&p->gpart_d, (size_t)p->n_gslots * N2);
+    if (p->gram_tc) {
+        ok = ok && dev_upload(&p->gtc_segs_d, gtc_segs) && dev_upload(&p->gtc_cta_first_d, gtc_cta_first) &&
+             dev_upload(&p->gtc_seg_first_d, gtc_seg_first) &&
+             dev_alloc(&p->gtc_part_d, (size_t)(p->gtc_nseg ? p->gtc_nseg : 1) * 4 * 128 * 128);
+    }
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->R_d), K * N2 * 2 * p->esz);
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->rotlog_d), K * p->max_sweeps * M * 3 * p->NP * p->esz);
     ok = ok && dev_alloc(&p->lam_d, K * N) && dev_alloc(&p->order_d, K * N) && dev_alloc(&p->cut_d, K) &&
@@ -259,17 +274,23 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     cudaError_t e = cudaSuccess;
     cudaEvent_t* evs = p->timer.ev[p->timer.calls % TIMER_RING];
     auto mark = [&](int i) { if (tm && e == cudaSuccess) e = cudaEventRecord(evs[i], st); };
+    int stage = 0;
+    auto run = [&](int id, cudaError_t r) { if (e == cudaSuccess && r != cudaSuccess) { e = r; stage = id; } };
     mark(0);
-    if (e == cudaSuccess) e = launch_gram(p, iq, st);
+    if (e == cudaSuccess) run(1, p->gram_tc ? launch_gram_tc(p, iq, st) : launch_gram(p, iq, st));
     mark(1);
-    if (e == cudaSuccess) e = launch_jacobi(p, st);
+    if (e == cudaSuccess) run(2, launch_jacobi(p, st));
     mark(2);
-    if (e == cudaSuccess) e = launch_vbuild(p, st);
+    if (e == cudaSuccess) run(3, launch_vbuild(p, st));
     mark(3);
-    if (e == cudaSuccess) e = launch_project(p, iq, st);
+    if (e == cudaSuccess) run(4, launch_project(p, iq, st));
     mark(4);
-    if (e == cudaSuccess) e = launch_combine(p, pd_dev, st);
+    if (e == cudaSuccess) run(5, launch_combine(p, pd_dev, st));
     mark(5);
+    if (e != cudaSuccess) {
+        static const char* names[] = {"event record", "gram", "evd", "weights/projector", "projection", "combine"};
+        snprintf(p->last_error, sizeof(p->last_error), "%s: %s", names[stage], cudaGetErrorString(e));
+    }
     if (tm) ++p->timer.calls;
     p->last_stream = st;
     p->ran = true;
@@ -303,6 +324,8 @@ extern "C" lcf_status lcf_filter_host(lcf_plan* p, const void* iq_host, float* p
     }
     return LCF_OK;
 }
+
+extern "C" const char* lcf_last_error(const lcf_plan* p) { return p ? p->last_error : "null plan"; }
 
 extern "C" int lcf_num_windows(const lcf_plan* p) { return p ? p->K : 0; }
 
@@ -431,6 +454,6 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
     w->gram_flops = 8.0 * S * N * (N + 1.0) / 2.0;   // Hermitian half, 8 real flops per complex MAC
     w->proj_flops = 8.0 * S * N * N;                 // dense N x N projector factor
     w->hbm_bytes = 8.0 * N * (double)p->P + 4.0 * (double)p->P;
-    w->launches = 6;
+    w->launches = p->gram_tc ? 7 : 6;
     return LCF_OK;
 }

@@ -21,7 +21,7 @@ EXPORTS = [
     "lcf_plan_create", "lcf_filter", "lcf_filter_host", "lcf_plan_destroy", "lcf_num_windows",
     "lcf_get_eigenvalues", "lcf_get_cutoffs", "lcf_get_sweeps", "lcf_get_gram", "lcf_get_eigenvectors",
     "lcf_get_weights", "lcf_get_filters", "lcf_get_window_means", "lcf_set_timing", "lcf_get_stage_ms",
-    "lcf_get_work", "lcf_measure_peak", "lcf_status_string",
+    "lcf_get_work", "lcf_measure_peak", "lcf_status_string", "lcf_last_error",
 ]
 
 
@@ -74,8 +74,10 @@ def load() -> C.CDLL:
         L.lcf_measure_peak.argtypes = [C.c_int, dp]
         L.lcf_status_string.argtypes = [C.c_int]
         L.lcf_status_string.restype = C.c_char_p
+        L.lcf_last_error.argtypes = [vp]
+        L.lcf_last_error.restype = C.c_char_p
         for name in EXPORTS:
-            if name != "lcf_status_string":
+            if name not in ("lcf_status_string", "lcf_last_error"):
                 getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -158,7 +160,7 @@ class Plan:
         """iq_dev: complex64 device tensor [N][Nx][Nz] (or address); pd_dev: float32 [Nx][Nz]. Asynchronous."""
         st = load().lcf_filter(self._h, _ptr(iq_dev), _ptr(pd_dev), _stream(stream))
         if st != OK:
-            raise LcfError(st, "lcf_filter")
+            raise LcfError(st, "lcf_filter [" + load().lcf_last_error(self._h).decode() + "]")
 
     def filter_host(self, iq_host, pd_host, stream=None):
         """Host buffers (numpy / pinned torch tensors); copies, filters, copies back, synchronises."""
