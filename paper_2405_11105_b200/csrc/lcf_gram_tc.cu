@@ -4,7 +4,7 @@
 //   R_k[i][j] = sum_p w_k(p)^2 conj(S[i][p]) S[j][p]            X = W_k S (Eq. 11), X = Xr + i Xi
 //   Re R = Xr Xr^T + Xi Xi^T          Im R = G - G^T,  G = Xr Xi^T          (frames x frames, K = pixels)
 //
-// Every fp32 sample is split x = hi + lo (hi = x rounded to TF32, lo = (x - hi) rounded to TF32), so
+// Every fp32 sample is split x = hi + lo (hi = x rounded to TF32, lo = x - hi exactly, read as TF32), so
 //   Re R = D0 + H + H^T      D0 = Rh Rh^T + Ih Ih^T        H = Rh Rl^T + Ih Il^T
 //   Im R = (G0 + L) - (G0 + L)^T     G0 = Rh Ih^T          L = Rh Il^T - Ih Rl^T
 // (the lo.lo products, 2^-22 of a term, are dropped).  Seven 128 x Np x 8 tcgen05.mma per 8 pixels
@@ -12,18 +12,22 @@
 //
 // Persistent CTAs (one per SM) walk a static, contiguous slice of the global list of 16-pixel
 // tiles (16 z-contiguous pixels of one window: one 128-byte row per frame), cut into segments at
-// window boundaries.  Roles (320 threads):
-//   warp 0      TMA producer: [N frames][16 px] complex64 box -> 128B-swizzled raw stage, plus the
-//               16 window weights of the tile;
-//   warps 2-9   converters: raw stage -> w * s -> hi/lo -> four K-major operand tiles (canonical
-//               no-swizzle core-matrix layout) -> fence.proxy.async -> mbarrier;
-//   warp 1      one thread issues the MMAs and commits them to mbarriers.
+// window boundaries.  Roles (640 threads, register file re-split with setmaxnreg):
+//   warp 0       TMA producer: [N frames][16 px] complex64 box -> 128B-swizzled raw stage, plus the
+//                16 window weights of the tile (window table rows staged in shared memory);
+//   warp 1       MMA issuer: uniform control flow, one elected lane issues and commits;
+//   warps 4-11   converters: raw stage -> w * s (f32x2) -> hi/lo -> four K-major operand tiles
+//                (canonical no-swizzle core-matrix layout) -> fence.proxy.async -> mbarrier;
+//   warps 12-19  accumulator drain (152 registers each): see below.
 // tcgen05 accumulates in fp32 with truncation (measured: 2^24 + 1.5 -> 2^24), a bias that grows
 // with the number of adds into a large running sum; D0 and G0 are therefore drained every
-// GTC_GROUP tiles (128 pixels = 32 adds) into fp32 registers of the converter warps (round to
-// nearest), H and L (2^-11 of the main terms) stay in TMEM for the whole segment.  Each segment
-// ends by writing four 128 x 128 fp32 partials; gram_tc_reduce_kernel sums a window's segments in
-// fp64, applies the (anti)symmetrisation above and writes the full Hermitian R_k.
+// `group` tiles (128 pixels = 32 adds) into fp32 registers of the drain warps (round to nearest),
+// H and L (2^-11 of the main terms) stay in TMEM for the whole segment.  Each segment ends by
+// writing four 128 x 128 fp32 partials; gram_tc_reduce_kernel sums a window's segments in fp64,
+// applies the (anti)symmetrisation above and writes the full Hermitian R_k.
+// Measured bound (clock64 per role, B200): the 128x128x8 MMA reads 8 KB of operands per 64 cycles,
+// i.e. the whole 128 B/clk of shared-memory bandwidth, so the converter's and TMA's shared-memory
+// traffic (64 KB per tile next to 112 KB of operand reads) stretches an MMA from 64 to ~105 cycles.
 #include <cuda.h>
 
 #include "lcf_internal.h"
@@ -37,13 +41,16 @@ constexpr int GTC_PX = 16;                 // pixels per tile
 constexpr int GTC_RT = 128;                // operand tile rows (frames, zero padded)
 constexpr int GTC_RAW_STAGES = 4;
 constexpr int GTC_OP_STAGES = 4;
-constexpr int GTC_LAG = 3;                 // tiles the converters run ahead before draining a group
 constexpr int GTC_CONV_WARPS = 8;
-constexpr int GTC_THREADS = 32 * (2 + GTC_CONV_WARPS);
+constexpr int GTC_DRAIN_WARPS = 8;
+constexpr int GTC_FIRST_CONV = 4;            // warps 0-3: TMA producer, MMA issuer, two idle (one warpgroup)
+constexpr int GTC_FIRST_DRAIN = GTC_FIRST_CONV + GTC_CONV_WARPS;
+constexpr int GTC_THREADS = 32 * (GTC_FIRST_DRAIN + GTC_DRAIN_WARPS);
 constexpr int GTC_TILE_BYTES = GTC_RT * GTC_PX * 4;      // one operand tile: 8 KB
 constexpr int GTC_OP_BYTES = 4 * GTC_TILE_BYTES;         // Rh, Ih, Rl, Il
 constexpr int GTC_LBO = GTC_RT * 16;                     // next 4-pixel K chunk
 constexpr int GTC_SBO = 128;                             // next 8-frame row group
+constexpr int GTC_TASKS = (4 * (GTC_RT / 32) + GTC_CONV_WARPS - 1) / GTC_CONV_WARPS;   // converter tasks per thread per tile
 
 struct GtcArgs {
     int N, Np, Nz, Nx, Kz;
@@ -62,15 +69,43 @@ struct GtcBars {
     uint64_t opfull[GTC_OP_STAGES], opempty[GTC_OP_STAGES];
     uint64_t accfull, accempty;
     uint32_t tmem_base;
-    alignas(16) float wts[GTC_RAW_STAGES][GTC_PX];
+    alignas(16) float wts[GTC_RAW_STAGES][2 * GTC_PX];   // each pixel weight twice: (w, w) pairs for f32x2
 };
 
-__device__ __forceinline__ void split_tf32(float v, float& hi, float& lo) {
-    // round to nearest (ties away) on the 13 dropped mantissa bits, in integer arithmetic
-    hi = __uint_as_float((__float_as_uint(v) + 0x1000u) & 0xFFFFE000u);
-    const float r = v - hi;     // exact
-    lo = __uint_as_float((__float_as_uint(r) + 0x1000u) & 0xFFFFE000u);
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
 }
+__device__ __forceinline__ void sts128(uint32_t addr, const float4& v) {
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
+__device__ __forceinline__ ulonglong2 lds128u(uint32_t addr) {
+    ulonglong2 v;
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(addr));
+    return v;
+}
+// packed fp32 pair arithmetic (sm_100 f32x2 pipe): (a.x*b.x, a.y*b.y) and (a.x-b.x, a.y-b.y)
+__device__ __forceinline__ float2 mul2(unsigned long long a, unsigned long long b) {
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    float2 f;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(f.x), "=f"(f.y) : "l"(r));
+    return f;
+}
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) {
+    unsigned long long ua, ub, r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ub) : "f"(b.x), "f"(b.y));
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(ua), "l"(ub));
+    float2 f;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(f.x), "=f"(f.y) : "l"(r));
+    return f;
+}
+// x rounded to TF32 (10-bit mantissa), nearest with ties away, in integer arithmetic.  hi = rna(x)
+// makes lo = x - hi a signed 12-bit quantity, so the tensor core's truncation of lo is unbiased.
+__device__ __forceinline__ float rna_tf32(float v) { return __uint_as_float((__float_as_uint(v) + 0x1000u) & 0xFFFFE000u); }
 
 __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_constant__ CUtensorMap tmap, GtcArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
@@ -78,6 +113,8 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
     unsigned char* raw = sbase;                                               // [RAW_STAGES][raw_stride]
     unsigned char* ops = sbase + (size_t)GTC_RAW_STAGES * a.raw_stride;       // [OP_STAGES][GTC_OP_BYTES]
     GtcBars* bars = reinterpret_cast<GtcBars*>(ops + (size_t)GTC_OP_STAGES * GTC_OP_BYTES);
+    double* gzs = reinterpret_cast<double*>(bars + 1);                        // [Nz] window table rows (producer only)
+    double* gxs = gzs + a.Nz;                                                 // [Nx]
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int N = a.N;
@@ -87,10 +124,10 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
     for (int i = tid * 16; i < GTC_OP_STAGES * GTC_OP_BYTES; i += GTC_THREADS * 16) *reinterpret_cast<uint4*>(ops + i) = make_uint4(0, 0, 0, 0);
     fence_proxy_async_smem();
     if (tid == 0) {
-        for (int s = 0; s < GTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], GTC_CONV_WARPS * 32); }
-        for (int s = 0; s < GTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], GTC_CONV_WARPS * 32); mbar_init(&bars->opempty[s], 1); }
+        for (int s = 0; s < GTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], GTC_CONV_WARPS); }
+        for (int s = 0; s < GTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], GTC_CONV_WARPS); mbar_init(&bars->opempty[s], 1); }
         mbar_init(&bars->accfull, 1);
-        mbar_init(&bars->accempty, GTC_CONV_WARPS * 32);
+        mbar_init(&bars->accempty, GTC_DRAIN_WARPS);
         mbar_fence_init();
     }
     if (warp == 1) tmem_alloc<512>(&bars->tmem_base);
@@ -99,6 +136,7 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
     tc_fence_after_sync();
     const uint32_t tmem = bars->tmem_base;
 
+    if (warp < GTC_FIRST_CONV) asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
     if (warp == 0) {
         // =========================== TMA producer ===========================
         if (lane == 0) tma_prefetch_desc(&tmap);
@@ -108,8 +146,12 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
             const WinBox bx = a.box[seg.k];
             const int ze = bx.z0 & ~1;    // TMA needs a 16-byte aligned start in the swizzled inner dimension
             const int ntz = (bx.z0 + bx.Lz - ze + GTC_PX - 1) / GTC_PX;
-            const double* gz = a.gz + (size_t)bx.kz * a.Nz;
-            const double* gx = a.gx + (size_t)bx.kx * a.Nx;
+            // this window's separable table rows -> shared memory (one global round trip per segment,
+            // not per tile: the producer's per-tile latency bounds the whole pipeline)
+            __syncwarp();
+            for (int i = lane; i < a.Nz; i += 32) gzs[i] = a.gz[(size_t)bx.kz * a.Nz + i];
+            for (int i = lane; i < a.Nx; i += 32) gxs[i] = a.gx[(size_t)bx.kx * a.Nx + i];
+            __syncwarp();
             for (int t = 0; t < seg.ntile; ++t, ++it) {
                 const int s = it % GTC_RAW_STAGES;
                 const uint32_t ph = (it / GTC_RAW_STAGES) & 1;
@@ -120,8 +162,8 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
                 if (lane < GTC_PX) {
                     const int zz = z + lane;
                     float w = 0.f;
-                    if (zz < a.Nz && x < a.Nx) w = (float)(gz[zz] * gx[x]);
-                    bars->wts[s][lane] = w;
+                    if (zz < a.Nz && x < a.Nx) w = (float)(gzs[zz] * gxs[x]);
+                    bars->wts[s][2 * lane] = w; bars->wts[s][2 * lane + 1] = w;
                 }
                 __syncwarp();
                 if (lane == 0) {
@@ -132,10 +174,13 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
-        if (lane == 0) {
+        // the whole warp runs the loop (uniform control flow); one elected lane issues
+        {
             const uint32_t idesc = make_idesc_tf32(GTC_RT, a.Np, false, false, false, false);
             const uint32_t idesc_na = make_idesc_tf32(GTC_RT, a.Np, false, false, true, false);
             const uint32_t tD0 = tmem, tG0 = tmem + 128, tH = tmem + 256, tL = tmem + 384;
+            // descriptor of operand tile 0, k-step 0 of stage 0; the others differ in the address field only
+            const uint64_t desc0 = make_smem_desc(smem_u32(ops), GTC_LBO, GTC_SBO, SWZ_NONE);
             uint32_t it = 0, gc = 0;
             for (int sg = seg0; sg < seg1; ++sg) {
                 const int nt = a.segs[sg].ntile;
@@ -147,105 +192,135 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
                     mbar_wait(&bars->opfull[o], pho);
                     if (group_first) mbar_wait(&bars->accempty, (gc & 1) ^ 1);
                     tc_fence_after_sync();
-                    const uint32_t ob = smem_u32(ops + (size_t)o * GTC_OP_BYTES);
+                    if (elect_one()) {
+                        const uint64_t dst = desc0 + (uint64_t)((o * GTC_OP_BYTES) >> 4);
 #pragma unroll
-                    for (int ks = 0; ks < GTC_PX / 8; ++ks) {
-                        const uint32_t koff = ks * 2 * GTC_LBO;
-                        const uint64_t dRh = make_smem_desc(ob + 0 * GTC_TILE_BYTES + koff, GTC_LBO, GTC_SBO, SWZ_NONE);
-                        const uint64_t dIh = make_smem_desc(ob + 1 * GTC_TILE_BYTES + koff, GTC_LBO, GTC_SBO, SWZ_NONE);
-                        const uint64_t dRl = make_smem_desc(ob + 2 * GTC_TILE_BYTES + koff, GTC_LBO, GTC_SBO, SWZ_NONE);
-                        const uint64_t dIl = make_smem_desc(ob + 3 * GTC_TILE_BYTES + koff, GTC_LBO, GTC_SBO, SWZ_NONE);
-                        const uint32_t accg = (group_first && ks == 0) ? 0u : 1u;   // D0, G0 restart per group
-                        const uint32_t accs = (t == 0 && ks == 0) ? 0u : 1u;        // H, L restart per segment
-                        mma_tf32(tD0, dRh, dRh, idesc, accg);
-                        mma_tf32(tD0, dIh, dIh, idesc, 1u);
-                        mma_tf32(tG0, dRh, dIh, idesc, accg);
-                        mma_tf32(tH, dRh, dRl, idesc, accs);
-                        mma_tf32(tH, dIh, dIl, idesc, 1u);
-                        mma_tf32(tL, dRh, dIl, idesc, accs);
-                        mma_tf32(tL, dIh, dRl, idesc_na, 1u);
+                        for (int ks = 0; ks < GTC_PX / 8; ++ks) {
+                            const uint64_t dRh = dst + (uint64_t)((0 * GTC_TILE_BYTES + ks * 2 * GTC_LBO) >> 4);
+                            const uint64_t dIh = dst + (uint64_t)((1 * GTC_TILE_BYTES + ks * 2 * GTC_LBO) >> 4);
+                            const uint64_t dRl = dst + (uint64_t)((2 * GTC_TILE_BYTES + ks * 2 * GTC_LBO) >> 4);
+                            const uint64_t dIl = dst + (uint64_t)((3 * GTC_TILE_BYTES + ks * 2 * GTC_LBO) >> 4);
+                            const uint32_t accg = (group_first && ks == 0) ? 0u : 1u;   // D0, G0 restart per group
+                            const uint32_t accs = (t == 0 && ks == 0) ? 0u : 1u;        // H, L restart per segment
+                            {
+                                mma_tf32(tD0, dRh, dRh, idesc, accg);
+                                mma_tf32(tD0, dIh, dIh, idesc, 1u);
+                                mma_tf32(tG0, dRh, dIh, idesc, accg);
+                                mma_tf32(tH, dRh, dRl, idesc, accs);
+                                mma_tf32(tH, dIh, dIl, idesc, 1u);
+                                mma_tf32(tL, dRh, dIl, idesc, accs);
+                                mma_tf32(tL, dIh, dRl, idesc_na, 1u);
+                            }
+                        }
+                        mma_commit(&bars->opempty[o]);
+                        if (group_last) mma_commit(&bars->accfull);
                     }
-                    mma_commit(&bars->opempty[o]);
-                    if (group_last) { mma_commit(&bars->accfull); ++gc; }
+                    __syncwarp();
+                    if (group_last) ++gc;
                 }
             }
         }
-    } else {
-        // =========================== converters / accumulator drain ===========================
-        const int cw = warp - 2;                      // 0..7
+    } else if (warp >= GTC_FIRST_CONV && warp < GTC_FIRST_DRAIN) {
+        // =========================== converters ===========================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
+        const int cw = warp - GTC_FIRST_CONV;         // 0..7
+        // this thread's tasks per tile: (4-pixel chunk c4, frame fr); offsets are the same for every tile
+        const int nwt = 4 * ((N + 31) / 32);          // warp tasks per tile: (4-pixel chunk, 32-frame block)
+        const uint32_t raw_u32 = smem_u32(raw), ops_u32 = smem_u32(ops), wts_u32 = smem_u32(&bars->wts[0][0]);
+        bool tvalid[GTC_TASKS];
+        uint32_t twt[GTC_TASKS], trd0[GTC_TASKS], trd1[GTC_TASKS], tdst[GTC_TASKS];
+#pragma unroll
+        for (int j = 0; j < GTC_TASKS; ++j) {
+            const int wt = cw + j * GTC_CONV_WARPS;
+            const int c4 = wt & 3, fr = (wt >> 2) * 32 + lane;
+            tvalid[j] = wt < nwt && fr < N;
+            const uint32_t sw = (uint32_t)(fr & 7);
+            twt[j] = (uint32_t)c4 * 32u;
+            trd0[j] = (uint32_t)fr * 128u + ((((uint32_t)(2 * c4)) ^ sw) << 4);
+            trd1[j] = (uint32_t)fr * 128u + ((((uint32_t)(2 * c4 + 1)) ^ sw) << 4);
+            tdst[j] = (uint32_t)c4 * GTC_LBO + (uint32_t)fr * 16u;
+        }
+        uint32_t it = 0;
+        for (int sg = seg0; sg < seg1; ++sg) {
+            const int nt = a.segs[sg].ntile;
+            for (int t = 0; t < nt; ++t, ++it) {
+                const int s = it % GTC_RAW_STAGES, o = it % GTC_OP_STAGES;
+                const uint32_t ph = (it / GTC_RAW_STAGES) & 1, pho = (it / GTC_OP_STAGES) & 1;
+                const uint32_t rs = raw_u32 + (uint32_t)s * a.raw_stride;
+                const uint32_t os = ops_u32 + (uint32_t)o * GTC_OP_BYTES;
+                const uint32_t ws = wts_u32 + (uint32_t)s * (GTC_PX * 8);
+                mbar_wait(&bars->full[s], ph);
+                ulonglong2 wa[GTC_TASKS], wb[GTC_TASKS], p01[GTC_TASKS], p23[GTC_TASKS];
+#pragma unroll
+                for (int j = 0; j < GTC_TASKS; ++j)
+                    if (tvalid[j]) {
+                        wa[j] = lds128u(ws + twt[j]);          // (w0, w0), (w1, w1)
+                        wb[j] = lds128u(ws + twt[j] + 16);     // (w2, w2), (w3, w3)
+                        p01[j] = lds128u(rs + trd0[j]);        // (re0, im0), (re1, im1)
+                        p23[j] = lds128u(rs + trd1[j]);
+                    }
+                mbar_wait(&bars->opempty[o], pho ^ 1);
+#pragma unroll
+                for (int j = 0; j < GTC_TASKS; ++j)
+                    if (tvalid[j]) {
+                        float2 v[4], h[4], l[4];
+                        v[0] = mul2(p01[j].x, wa[j].x); v[1] = mul2(p01[j].y, wa[j].y);
+                        v[2] = mul2(p23[j].x, wb[j].x); v[3] = mul2(p23[j].y, wb[j].y);
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            h[q].x = rna_tf32(v[q].x); h[q].y = rna_tf32(v[q].y);
+                            l[q] = sub2(v[q], h[q]);            // exact; the tensor core truncates it to TF32
+                        }
+                        const uint32_t dst = os + tdst[j];
+                        sts128(dst + 0 * GTC_TILE_BYTES, make_float4(h[0].x, h[1].x, h[2].x, h[3].x));
+                        sts128(dst + 1 * GTC_TILE_BYTES, make_float4(h[0].y, h[1].y, h[2].y, h[3].y));
+                        sts128(dst + 2 * GTC_TILE_BYTES, make_float4(l[0].x, l[1].x, l[2].x, l[3].x));
+                        sts128(dst + 3 * GTC_TILE_BYTES, make_float4(l[0].y, l[1].y, l[2].y, l[3].y));
+                    }
+                fence_proxy_async_smem();             // this lane's operand writes -> async proxy
+                __syncwarp();
+                if (lane == 0) {                      // one arrival per converter warp on each barrier
+                    mbar_arrive(&bars->empty[s]);     // raw stage (and its weights) consumed
+                    mbar_arrive(&bars->opfull[o]);
+                }
+            }
+        }
+    } else if (warp >= GTC_FIRST_DRAIN) {
+        // =========================== accumulator drain ===========================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
+        const int dw = warp - GTC_FIRST_DRAIN;        // 0..7
         const int quad = warp & 3;                    // TMEM lane quadrant this warp may touch
-        const int half = cw >> 2;                     // which 64 columns of D0 / G0 this warp keeps
+        const int half = dw >> 2;                     // which 64 columns of D0 / G0 this warp keeps
         const uint32_t tlane = tmem + ((uint32_t)(quad * 32) << 16);
         const int row = quad * 32 + lane;
         float acc[128];
 #pragma unroll
         for (int i = 0; i < 128; ++i) acc[i] = 0.f;
-        const int nwt = 4 * ((N + 31) / 32);          // warp tasks per tile: (4-pixel chunk, 32-frame block)
-        uint32_t it = 0, gc = 0;
-
-        auto drain_group = [&]() {                    // D0, G0 of the finished group -> registers
-            mbar_wait(&bars->accfull, gc & 1);
-            tc_fence_after_sync();
-#pragma unroll
-            for (int blk = 0; blk < 8; ++blk) {
-                uint32_t v[16];
-                const uint32_t col = (blk < 4 ? 0u : 128u) + half * 64 + (blk & 3) * 16;
-                tmem_ld16(tlane + col, v);
-                tmem_ld_wait();
-#pragma unroll
-                for (int j = 0; j < 16; ++j) acc[blk * 16 + j] += __uint_as_float(v[j]);
-            }
-        };
-        auto release_acc = [&]() {
-            tc_fence_before_sync();
-            mbar_arrive(&bars->accempty);
-            ++gc;
-        };
-
+        uint32_t gc = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
-            const GtcSeg seg = a.segs[sg];
-            const int nt = seg.ntile;
+            const int nt = a.segs[sg].ntile;
             const int ngroups = (nt + a.group - 1) / a.group;
-            int drained = 0;
-            for (int t = 0; t < nt; ++t, ++it) {
-                const int s = it % GTC_RAW_STAGES, o = it % GTC_OP_STAGES;
-                const uint32_t ph = (it / GTC_RAW_STAGES) & 1, pho = (it / GTC_OP_STAGES) & 1;
-                const unsigned char* rs = raw + (size_t)s * a.raw_stride;
-                unsigned char* os = ops + (size_t)o * GTC_OP_BYTES;
-                mbar_wait(&bars->full[s], ph);
-                mbar_wait(&bars->opempty[o], pho ^ 1);
-                for (int wt = cw; wt < nwt; wt += GTC_CONV_WARPS) {
-                    const int c4 = wt & 3, fr = (wt >> 2) * 32 + lane;
-                    if (fr < N) {
-                        const float4 w4 = *reinterpret_cast<const float4*>(&bars->wts[s][c4 * 4]);
-                        const uint32_t rowoff = (uint32_t)fr * 128u, sw = (uint32_t)(fr & 7);
-                        const float4 p01 = *reinterpret_cast<const float4*>(rs + rowoff + (((2 * c4) ^ sw) << 4));
-                        const float4 p23 = *reinterpret_cast<const float4*>(rs + rowoff + (((2 * c4 + 1) ^ sw) << 4));
-                        float4 rh, ih, rl, il;
-                        split_tf32(w4.x * p01.x, rh.x, rl.x); split_tf32(w4.x * p01.y, ih.x, il.x);
-                        split_tf32(w4.y * p01.z, rh.y, rl.y); split_tf32(w4.y * p01.w, ih.y, il.y);
-                        split_tf32(w4.z * p23.x, rh.z, rl.z); split_tf32(w4.z * p23.y, ih.z, il.z);
-                        split_tf32(w4.w * p23.z, rh.w, rl.w); split_tf32(w4.w * p23.w, ih.w, il.w);
-                        unsigned char* dst = os + (size_t)c4 * GTC_LBO + (size_t)fr * 16;
-                        *reinterpret_cast<float4*>(dst + 0 * GTC_TILE_BYTES) = rh;
-                        *reinterpret_cast<float4*>(dst + 1 * GTC_TILE_BYTES) = ih;
-                        *reinterpret_cast<float4*>(dst + 2 * GTC_TILE_BYTES) = rl;
-                        *reinterpret_cast<float4*>(dst + 3 * GTC_TILE_BYTES) = il;
-                    }
+            for (int g = 0; g < ngroups; ++g) {
+                // D0, G0 of the finished group -> registers (round-to-nearest adds)
+                mbar_wait(&bars->accfull, gc & 1);
+                tc_fence_after_sync();
+#pragma unroll
+                for (int blk = 0; blk < 8; ++blk) {
+                    uint32_t v[16];
+                    const uint32_t col = (blk < 4 ? 0u : 128u) + half * 64 + (blk & 3) * 16;
+                    tmem_ld16(tlane + col, v);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) acc[blk * 16 + j] += __uint_as_float(v[j]);
                 }
-                mbar_arrive(&bars->empty[s]);         // raw stage (and its weights) consumed
-                fence_proxy_async_smem();
-                mbar_arrive(&bars->opfull[o]);
-                // drain finished, non-final groups a few tiles late so the MMA queue stays fed
-                while (drained < ngroups - 1 && (drained + 1) * a.group - 1 <= t - GTC_LAG) {
-                    drain_group();
-                    release_acc();
-                    ++drained;
+                if (g + 1 < ngroups) {
+                    tc_fence_before_sync();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&bars->accempty);   // one arrival per drain warp
+                    ++gc;
                 }
             }
-            while (drained < ngroups - 1) { drain_group(); release_acc(); ++drained; }
-            // ---- segment end: last group, then the four partials of this segment
-            drain_group();
+            // ---- segment end: the four partials of this segment
             float* out = a.part + (size_t)sg * 4 * 128 * 128 + (size_t)row * 128 + half * 64;
 #pragma unroll
             for (int m = 0; m < 2; ++m) {
@@ -269,7 +344,10 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
                     *reinterpret_cast<float4*>(o2 + j) = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]),
                                                                      __uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
             }
-            release_acc();
+            tc_fence_before_sync();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars->accempty);
+            ++gc;
         }
     }
     tc_fence_before_sync();
@@ -383,7 +461,8 @@ cudaError_t configure_gram_tc(lcf_plan* p, std::vector<GtcSeg>& segs, std::vecto
     seg_first[K] = si;
     p->gtc_nseg = (int)segs.size();
     p->gtc_raw_stride = (uint32_t)(((size_t)p->N * 128 + 1023) / 1024 * 1024);
-    p->gtc_smem = 1024 + (size_t)GTC_RAW_STAGES * p->gtc_raw_stride + (size_t)GTC_OP_STAGES * GTC_OP_BYTES + sizeof(GtcBars);
+    p->gtc_smem = 1024 + (size_t)GTC_RAW_STAGES * p->gtc_raw_stride + (size_t)GTC_OP_STAGES * GTC_OP_BYTES + sizeof(GtcBars) +
+                  (size_t)(p->Nz + p->Nx) * sizeof(double);
     if (p->gtc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
     return cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gtc_smem);
 }
