@@ -32,6 +32,11 @@ struct ProjItem {
 struct GtcSeg {
     int k, tile0, ntile, pad_;
 };
+// One segment of the tensor-core projection: `ntile` consecutive 64-pixel tiles of window k,
+// eigen-column block b.
+struct PtcSeg {
+    int k, b, tile0, ntile;
+};
 
 constexpr int GRAM_TP = 32;        // pixels per shared-memory tile of the Gram kernel
 constexpr int GRAM_FLUSH_TILES = 16; // fp32 accumulators are folded into the fp64 partial every 16 tiles (512 px)
@@ -88,6 +93,16 @@ struct lcf_plan {
     float* gtc_part_d = nullptr;            // [nseg][4][128][128]
     alignas(64) unsigned char gtc_tmap[128];  // CUtensorMap of the last iq pointer
     const void* gtc_tmap_iq = nullptr;
+    // tensor-core projection (N <= 128): lcf_project_tc.cu
+    bool proj_tc = false;
+    int ptc_grid = 0, ptc_nseg = 0, ptc_NB = 0, ptc_Kp = 0;
+    size_t ptc_smem = 0;
+    lcf::PtcSeg* ptc_segs_d = nullptr;
+    int* ptc_cta_first_d = nullptr;
+    float* ptc_bpack_d = nullptr;           // [K][NB][Kp/4][256][4]
+    float* ptc_part_d = nullptr;            // [NB][sum_k P_k]
+    alignas(64) unsigned char ptc_tmap[128];
+    const void* ptc_tmap_iq = nullptr;
     // EVD
     void* rotlog_d = nullptr;  // [K][max_sweeps*(Ns-1)][3][NP] real
     double* lam_d = nullptr;   // [K][N] descending
@@ -141,4 +156,7 @@ cudaError_t configure_project(lcf_plan* p);
 bool gram_tc_eligible(const lcf_plan* p);
 cudaError_t configure_gram_tc(lcf_plan* p, std::vector<GtcSeg>& segs, std::vector<int>& cta_first, std::vector<int>& seg_first);
 cudaError_t launch_gram_tc(lcf_plan* p, const float2* iq, cudaStream_t st);
+bool project_tc_eligible(const lcf_plan* p);
+cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::vector<int>& cta_first);
+cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st);
 }  // namespace lcf

@@ -60,6 +60,7 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->V_d); cudaFree(p->B_d); cudaFree(p->pitems_d); cudaFree(p->pfirst_d);
     cudaFree(p->tiles_d); cudaFree(p->tsum_d); cudaFree(p->mean_d); cudaFree(p->alpha_d);
     cudaFree(p->F_d); cudaFree(p->iq_stage_d); cudaFree(p->pd_stage_d);
+    cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d);
     cudaFree(p->gtc_segs_d); cudaFree(p->gtc_cta_first_d); cudaFree(p->gtc_seg_first_d); cudaFree(p->gtc_part_d);
     if (p->timer.have)
         for (auto& set : p->timer.ev)
@@ -177,6 +178,13 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
         cudaGetLastError();
         p->gram_tc = false;
     }
+    std::vector<PtcSeg> ptc_segs;
+    std::vector<int> ptc_cta_first;
+    p->proj_tc = project_tc_eligible(p);
+    if (p->proj_tc && configure_project_tc(p, ptc_segs, ptc_cta_first) != cudaSuccess) {
+        cudaGetLastError();
+        p->proj_tc = false;
+    }
     // ---- Gram work items: each window's box split into pixel chunks (multiples of GRAM_TP) ----
     std::vector<GramItem> gitems;
     p->gfirst_h.assign(p->K + 1, 0);
@@ -228,6 +236,11 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
         ok = ok && dev_upload(&p->gtc_segs_d, gtc_segs) && dev_upload(&p->gtc_cta_first_d, gtc_cta_first) &&
              dev_upload(&p->gtc_seg_first_d, gtc_seg_first) &&
              dev_alloc(&p->gtc_part_d, (size_t)(p->gtc_nseg ? p->gtc_nseg : 1) * 4 * 128 * 128);
+    }
+    if (p->proj_tc) {
+        ok = ok && dev_upload(&p->ptc_segs_d, ptc_segs) && dev_upload(&p->ptc_cta_first_d, ptc_cta_first) &&
+             dev_alloc(&p->ptc_bpack_d, K * p->ptc_NB * (size_t)(p->ptc_Kp / 4) * 1024) &&
+             dev_alloc(&p->ptc_part_d, (size_t)p->ptc_NB * (size_t)(p->sumPk ? p->sumPk : 1));
     }
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->R_d), K * N2 * 2 * p->esz);
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->rotlog_d), K * p->max_sweeps * M * 3 * p->NP * p->esz);
@@ -283,7 +296,7 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     mark(2);
     if (e == cudaSuccess) run(3, launch_vbuild(p, st));
     mark(3);
-    if (e == cudaSuccess) run(4, launch_project(p, iq, st));
+    if (e == cudaSuccess) run(4, p->proj_tc ? launch_project_tc(p, iq, st) : launch_project(p, iq, st));
     mark(4);
     if (e == cudaSuccess) run(5, launch_combine(p, pd_dev, st));
     mark(5);
@@ -454,6 +467,6 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
     w->gram_flops = 8.0 * S * N * (N + 1.0) / 2.0;   // Hermitian half, 8 real flops per complex MAC
     w->proj_flops = 8.0 * S * N * N;                 // dense N x N projector factor
     w->hbm_bytes = 8.0 * N * (double)p->P + 4.0 * (double)p->P;
-    w->launches = p->gram_tc ? 7 : 6;
+    w->launches = 6 + (p->gram_tc ? 1 : 0) + (p->proj_tc ? 2 : 0);
     return LCF_OK;
 }

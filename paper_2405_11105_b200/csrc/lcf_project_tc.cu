@@ -1,0 +1,423 @@
+// lcf_project_tc.cu -- kernel 4a, tensor-core path: fused projection + |.|^2 slow-time sum (Eq. 4,
+// PAPER.md:57-63) on tcgen05 with a 3xTF32 split, for N <= 128.
+//
+//   U[p][u] = sum_t S[t][p] B_k[t][u],  B_k = V_k diag(wt)     PD_k(p) = w_k(p)^2 sum_u |U[p][u]|^2
+//
+// Real formulation.  Rows m of the A operand are the interleaved re/im samples of 64 pixels
+// (m = 2p: Re S, m = 2p+1: Im S), K = frames, and one CTA works on a block of 64 eigen-columns u
+// whose operand tile stays resident in shared memory for a whole segment:
+//   B tile rows  [0,64) Re B hi   [64,128) Im B hi   [128,192) Re B lo   [192,256) Im B lo
+//   D[:, 0:256] += A_hi * B[0:256]^T        D[:, 0:128] += A_lo * B[0:128]^T        (two MMAs / 8 frames)
+//   P_r[m][u] = D[m][u] + D[m][128+u] = X_m . Re B_u      P_i[m][u] = D[m][64+u] + D[m][192+u]
+//   U_r = P_r[2p] - P_i[2p+1]      U_i = P_i[2p] + P_r[2p+1]
+// (hi = x rounded to TF32, lo = x - hi; the lo.lo products, 2^-22 of a term, are dropped).  Stacking
+// B hi over B lo makes one N = 256 MMA do two of the three products: the MMA reads 12 KB instead of
+// 16 KB of shared memory, which is what bounds these kernels (lcf_gram_tc.cu).
+//
+// Persistent CTAs walk a static slice of the list of (window, column block, 64-pixel tile) jobs,
+// cut into segments at (window, block) changes.  Roles (512 threads):
+//   warp 0      producer: the segment's packed B block (one bulk copy), then per 16 frames one TMA
+//               box [16 frames][4 x][16 z] complex64 -> raw stage (no swizzle: rows of 512 bytes);
+//   warp 1      MMA issuer (uniform control flow, one elected lane);
+//   warps 4-11  converters: raw [t][m] -> K-major A_hi / A_lo tiles (the transposition happens in
+//               registers: 4 frames of one row = one 16-byte core-matrix row);
+//   warps 12-15 epilogue: TMEM -> registers, pair exchange by shuffle, |U|^2 summed over the 64
+//               columns, times w^2, one float per (block, pixel); two accumulator buffers so the
+//               epilogue of a tile overlaps the MMAs of the next.
+// proj_tc_pack_kernel builds the B blocks from B_k; proj_tc_finish_kernel adds the column blocks
+// into the per-window PD tiles and the per-chunk sums that the alpha / combine kernels use.
+#include <cuda.h>
+
+#include "lcf_internal.h"
+#include "lcf_sm100.cuh"
+
+namespace lcf {
+
+using namespace sm100;
+
+constexpr int PTC_TZ = 16, PTC_TX = 4;                     // pixel tile: 16 z x 4 x = 64 pixels = 128 rows
+constexpr int PTC_ROWS = 128;
+constexpr int PTC_KC = 16;                                 // frames per A stage
+constexpr int PTC_UB = 64;                                 // eigen-columns per block
+constexpr int PTC_RAW_STAGES = 4, PTC_OP_STAGES = 3;
+constexpr int PTC_RAW_BYTES = PTC_KC * PTC_ROWS * 4;       // 8 KB
+constexpr int PTC_A_BYTES = PTC_KC * PTC_ROWS * 4;         // one of A_hi / A_lo per stage: 8 KB
+constexpr int PTC_OP_BYTES = 2 * PTC_A_BYTES;
+constexpr int PTC_A_LBO = PTC_ROWS * 16;                   // 2048: next 4-frame chunk of A
+constexpr int PTC_B_LBO = 256 * 16;                        // 4096: next 4-frame chunk of B
+constexpr int PTC_SBO = 128;
+constexpr int PTC_CONV_WARPS = 8, PTC_EPI_WARPS = 4;
+constexpr int PTC_FIRST_CONV = 4, PTC_FIRST_EPI = PTC_FIRST_CONV + PTC_CONV_WARPS;
+constexpr int PTC_THREADS = 32 * (PTC_FIRST_EPI + PTC_EPI_WARPS);
+
+struct PtcArgs {
+    int N, Kp, Nz, Nx;             // Kp = N rounded up to 8 frames
+    const double* gz;              // [Kz][Nz]
+    const double* gx;              // [Kx][Nx]
+    const WinBox* box;
+    const PtcSeg* segs;
+    const int* cta_first;          // [grid+1]
+    const float* bpack;            // [K][NB][Kp/4][256][4]
+    int NB;
+    float* part;                   // [NB][sum_k P_k]
+    long long sumPk;
+};
+
+struct PtcBars {
+    uint64_t full[PTC_RAW_STAGES], empty[PTC_RAW_STAGES];
+    uint64_t opfull[PTC_OP_STAGES], opempty[PTC_OP_STAGES];
+    uint64_t accfull[2], accempty[2];
+    uint64_t bfull, bfree;
+    uint32_t tmem_base;
+};
+
+__device__ __forceinline__ float ptc_lds32(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void ptc_sts128(uint32_t addr, float x, float y, float z, float w) {
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
+// x rounded to TF32, nearest with ties away (so the remainder x - hi is a signed 12-bit quantity)
+__device__ __forceinline__ float ptc_rna(float v) { return __uint_as_float((__float_as_uint(v) + 0x1000u) & 0xFFFFE000u); }
+
+__global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid_constant__ CUtensorMap tmap, PtcArgs a) {
+    extern __shared__ __align__(1024) unsigned char smem_dyn[];
+    unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
+    unsigned char* bsm = sbase;                                               // resident B block (<= 128 KB)
+    unsigned char* raw = sbase + 32 * 4096;                                   // [RAW_STAGES][8 KB]
+    unsigned char* ops = raw + PTC_RAW_STAGES * PTC_RAW_BYTES;                // [OP_STAGES][A_hi 8 KB | A_lo 8 KB]
+    PtcBars* bars = reinterpret_cast<PtcBars*>(ops + PTC_OP_STAGES * PTC_OP_BYTES);
+    double* gzs = reinterpret_cast<double*>(bars + 1);                        // [Nz] window table rows (epilogue only)
+    double* gxs = gzs + a.Nz;                                                 // [Nx]
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int seg0 = a.cta_first[blockIdx.x], seg1 = a.cta_first[blockIdx.x + 1];
+    const int nst = (a.Kp + PTC_KC - 1) / PTC_KC;          // A stages per tile
+    const int nks_total = a.Kp / 8;                        // 8-frame MMA steps per tile
+    const uint32_t bbytes = (uint32_t)(a.Kp / 4) * 4096u;
+
+    if (tid == 0) {
+        for (int s = 0; s < PTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], PTC_CONV_WARPS); }
+        for (int s = 0; s < PTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], PTC_CONV_WARPS); mbar_init(&bars->opempty[s], 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(&bars->accfull[b], 1); mbar_init(&bars->accempty[b], PTC_EPI_WARPS); }
+        mbar_init(&bars->bfull, 1);
+        mbar_init(&bars->bfree, 1);
+        mbar_fence_init();
+    }
+    if (warp == 1) tmem_alloc<512>(&bars->tmem_base);
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
+    const uint32_t tmem = bars->tmem_base;
+
+    if (warp == 0) {
+        // =========================== producer ===========================
+        if (lane == 0) tma_prefetch_desc(&tmap);
+        uint32_t it = 0;
+        for (int sg = seg0; sg < seg1; ++sg) {
+            const PtcSeg seg = a.segs[sg];
+            const WinBox bx = a.box[seg.k];
+            const int ze = bx.z0 & ~1;                     // 16-byte aligned start of the TMA inner dimension
+            const int ntz = (bx.z0 + bx.Lz - ze + PTC_TZ - 1) / PTC_TZ;
+            if (sg > seg0) mbar_wait(&bars->bfree, (uint32_t)(sg - seg0 - 1) & 1);   // MMAs of the old block done
+            if (lane == 0) {
+                mbar_arrive_expect_tx(&bars->bfull, bbytes);
+                bulk_load(bsm, a.bpack + ((size_t)seg.k * a.NB + seg.b) * (size_t)(a.Kp / 4) * 1024, bbytes, &bars->bfull);
+            }
+            for (int t = 0; t < seg.ntile; ++t) {
+                const int tau = seg.tile0 + t;
+                const int txi = tau / ntz, tzi = tau - txi * ntz;
+                const int z = ze + tzi * PTC_TZ, x = bx.x0 + txi * PTC_TX;
+                for (int st = 0; st < nst; ++st, ++it) {
+                    const int s = it % PTC_RAW_STAGES;
+                    mbar_wait(&bars->empty[s], ((it / PTC_RAW_STAGES) & 1) ^ 1);
+                    if (lane == 0) {
+                        mbar_arrive_expect_tx(&bars->full[s], PTC_RAW_BYTES);
+                        tma_load_3d(raw + (size_t)s * PTC_RAW_BYTES, &tmap, 2 * z, x, st * PTC_KC, &bars->full[s]);
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // =========================== MMA issuer ===========================
+        const uint32_t idesc256 = make_idesc_tf32(PTC_ROWS, 256, false, false, false, false);
+        const uint32_t idesc128 = make_idesc_tf32(PTC_ROWS, 128, false, false, false, false);
+        const uint64_t descA0 = make_smem_desc(smem_u32(ops), PTC_A_LBO, PTC_SBO, SWZ_NONE);
+        const uint64_t descB0 = make_smem_desc(smem_u32(bsm), PTC_B_LBO, PTC_SBO, SWZ_NONE);
+        uint32_t it = 0, tl = 0;
+        for (int sg = seg0; sg < seg1; ++sg) {
+            const int nt = a.segs[sg].ntile;
+            mbar_wait(&bars->bfull, (uint32_t)(sg - seg0) & 1);
+            for (int t = 0; t < nt; ++t, ++tl) {
+                const uint32_t buf = tl & 1;
+                mbar_wait(&bars->accempty[buf], ((tl >> 1) & 1) ^ 1);
+                const uint32_t tD = tmem + buf * 256;
+                for (int st = 0; st < nst; ++st, ++it) {
+                    const int o = it % PTC_OP_STAGES;
+                    mbar_wait(&bars->opfull[o], (it / PTC_OP_STAGES) & 1);
+                    tc_fence_after_sync();
+                    if (elect_one()) {
+                        const int nks = nks_total - 2 * st < 2 ? nks_total - 2 * st : 2;
+                        for (int ks = 0; ks < nks; ++ks) {
+                            const uint64_t dAh = descA0 + (uint64_t)((o * PTC_OP_BYTES + ks * 2 * PTC_A_LBO) >> 4);
+                            const uint64_t dAl = dAh + (uint64_t)(PTC_A_BYTES >> 4);
+                            const uint64_t dB = descB0 + (uint64_t)(((2 * st + ks) * 2 * PTC_B_LBO) >> 4);
+                            mma_tf32(tD, dAh, dB, idesc256, (st == 0 && ks == 0) ? 0u : 1u);
+                            mma_tf32(tD, dAl, dB, idesc128, 1u);
+                        }
+                        mma_commit(&bars->opempty[o]);
+                        if (st + 1 == nst) mma_commit(&bars->accfull[buf]);
+                    }
+                    __syncwarp();
+                }
+            }
+            if (elect_one()) mma_commit(&bars->bfree);     // every MMA that reads this B block has completed
+            __syncwarp();
+        }
+    } else if (warp >= PTC_FIRST_CONV && warp < PTC_FIRST_EPI) {
+        // =========================== converters ===========================
+        const int cw = warp - PTC_FIRST_CONV;
+        const uint32_t raw_u32 = smem_u32(raw), ops_u32 = smem_u32(ops);
+        uint32_t trd[2], tdst[2];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int wt = cw + j * PTC_CONV_WARPS;        // 16 warp tasks: (4-frame chunk c4, 32-row block)
+            const int c4 = wt & 3, m = (wt >> 2) * 32 + lane;
+            trd[j] = (uint32_t)(4 * c4) * (PTC_ROWS * 4) + (uint32_t)m * 4u;
+            tdst[j] = (uint32_t)c4 * PTC_A_LBO + (uint32_t)m * 16u;
+        }
+        uint32_t it = 0;
+        for (int sg = seg0; sg < seg1; ++sg) {
+            const int nstages = a.segs[sg].ntile * nst;
+            for (int q = 0; q < nstages; ++q, ++it) {
+                const int s = it % PTC_RAW_STAGES, o = it % PTC_OP_STAGES;
+                const uint32_t rs = raw_u32 + (uint32_t)s * PTC_RAW_BYTES, os = ops_u32 + (uint32_t)o * PTC_OP_BYTES;
+                mbar_wait(&bars->full[s], (it / PTC_RAW_STAGES) & 1);
+                float v[2][4];
+#pragma unroll
+                for (int j = 0; j < 2; ++j)
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) v[j][i] = ptc_lds32(rs + trd[j] + (uint32_t)i * (PTC_ROWS * 4));
+                mbar_wait(&bars->opempty[o], ((it / PTC_OP_STAGES) & 1) ^ 1);
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    float h[4], l[4];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) { h[i] = ptc_rna(v[j][i]); l[i] = v[j][i] - h[i]; }
+                    ptc_sts128(os + tdst[j], h[0], h[1], h[2], h[3]);
+                    ptc_sts128(os + PTC_A_BYTES + tdst[j], l[0], l[1], l[2], l[3]);
+                }
+                fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive(&bars->empty[s]);
+                    mbar_arrive(&bars->opfull[o]);
+                }
+            }
+        }
+    } else if (warp >= PTC_FIRST_EPI) {
+        // =========================== epilogue ===========================
+        const int quad = warp & 3;
+        const uint32_t tlane = tmem + ((uint32_t)(quad * 32) << 16);
+        const int m = quad * 32 + lane;
+        const int pix = m >> 1, xi = pix >> 4, zi = pix & 15;
+        uint32_t tl = 0;
+        int curk = -1;
+        for (int sg = seg0; sg < seg1; ++sg) {
+            const PtcSeg seg = a.segs[sg];
+            const WinBox bx = a.box[seg.k];
+            const int ze = bx.z0 & ~1;
+            const int ntz = (bx.z0 + bx.Lz - ze + PTC_TZ - 1) / PTC_TZ;
+            if (seg.k != curk) {
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                const int et = tid - PTC_FIRST_EPI * 32;
+                for (int i = et; i < a.Nz; i += 128) gzs[i] = a.gz[(size_t)bx.kz * a.Nz + i];
+                for (int i = et; i < a.Nx; i += 128) gxs[i] = a.gx[(size_t)bx.kx * a.Nx + i];
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                curk = seg.k;
+            }
+            float* out = a.part + (size_t)seg.b * a.sumPk + bx.tile_off;
+            for (int t = 0; t < seg.ntile; ++t, ++tl) {
+                const uint32_t buf = tl & 1;
+                const int tau = seg.tile0 + t;
+                const int txi = tau / ntz, tzi = tau - txi * ntz;
+                const int zz = ze + tzi * PTC_TZ + zi, xx = bx.x0 + txi * PTC_TX + xi;
+                mbar_wait(&bars->accfull[buf], (tl >> 1) & 1);
+                tc_fence_after_sync();
+                float acc = 0.f;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    uint32_t va[16], vb[16], vc[16], vd[16];
+                    const uint32_t col = buf * 256 + j * 16;
+                    tmem_ld16(tlane + col, va);
+                    tmem_ld16(tlane + col + 64, vb);
+                    tmem_ld16(tlane + col + 128, vc);
+                    tmem_ld16(tlane + col + 192, vd);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        const float pr = __uint_as_float(va[i]) + __uint_as_float(vc[i]);
+                        const float pi = __uint_as_float(vb[i]) + __uint_as_float(vd[i]);
+                        const float po = __shfl_xor_sync(0xffffffffu, pi, 1);
+                        const float val = (lane & 1) ? pr + po : pr - po;   // odd row: Im U, even row: Re U
+                        acc = fmaf(val, val, acc);
+                    }
+                }
+                tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bars->accempty[buf]);
+                acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+                if (!(lane & 1) && zz >= bx.z0 && zz < bx.z0 + bx.Lz && xx < bx.x0 + bx.Lx) {
+                    const double w = gzs[zz] * gxs[xx];
+                    out[(size_t)(xx - bx.x0) * bx.Lz + (zz - bx.z0)] = (float)(w * w) * acc;
+                }
+            }
+        }
+    }
+    tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc<512>(tmem);
+}
+
+// B_k [N][Ns] complex (row = frame, column = eigen slot) -> per (window, 64-column block) the
+// resident operand tile [Kp/4 chunks][256 rows][4 frames]: rows = Re hi | Im hi | Re lo | Im lo
+__global__ void proj_tc_pack_kernel(const float2* B, int N, int Ns, int Kp, int NB, float* bpack) {
+    const int kb = blockIdx.x;                       // k * NB + b
+    const int k = kb / NB, b = kb - k * NB;
+    const float2* Bk = B + (size_t)k * N * Ns;
+    float* out = bpack + (size_t)kb * (Kp / 4) * 1024;
+    for (int e = threadIdx.x; e < (Kp / 4) * 256; e += blockDim.x) {
+        const int c4 = e >> 8, r = e & 255;
+        const int u = b * PTC_UB + (r & 63);
+        const bool im = (r >> 6) & 1, lo = r >= 128;
+        float v[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int t = 4 * c4 + i;
+            float x = 0.f;
+            if (t < N && u < Ns) { const float2 c = Bk[(size_t)t * Ns + u]; x = im ? c.y : c.x; }
+            const float h = ptc_rna(x);
+            v[i] = lo ? x - h : h;
+        }
+        *reinterpret_cast<float4*>(out + (size_t)e * 4) = make_float4(v[0], v[1], v[2], v[3]);
+    }
+}
+
+// PD_k tile = sum over the column blocks; per-chunk sums for alpha_kernel (same items as project_kernel)
+__global__ void proj_tc_finish_kernel(const float* part, long long sumPk, int NB, const WinBox* box, const ProjItem* items,
+                                      float* tiles, float* tsum) {
+    const ProjItem it = items[blockIdx.x];
+    const long long off = box[it.k].tile_off;
+    const int q = it.q0 + threadIdx.x;
+    float v = 0.f;
+    if (q < it.q1) {
+        for (int b = 0; b < NB; ++b) v += part[(size_t)b * sumPk + off + q];
+        tiles[off + q] = v;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __shared__ float ws[PROJ_TPIX / 32];
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float t = 0.f;
+        for (int w = 0; w < PROJ_TPIX / 32; ++w) t += ws[w];
+        tsum[blockIdx.x] = t;
+    }
+}
+
+// ---------------------------------------------------------------- host side
+typedef CUresult (*PtcEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static PtcEncodeFn ptc_encode_fn() {
+    static PtcEncodeFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<PtcEncodeFn>(p);
+    }
+    return fn;
+}
+
+// [N][Nx][Nz] complex64 seen as float [N][Nx][2 Nz]; box = 16 z x 4 x x 16 frames, no swizzle
+static bool ptc_encode_map(lcf_plan* p, const void* iq) {
+    PtcEncodeFn fn = ptc_encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[3] = {(cuuint64_t)2 * p->Nz, (cuuint64_t)p->Nx, (cuuint64_t)p->N};
+    cuuint64_t strides[2] = {(cuuint64_t)p->Nz * 8, (cuuint64_t)p->P * 8};
+    cuuint32_t box[3] = {2 * PTC_TZ, PTC_TX, PTC_KC};
+    cuuint32_t es[3] = {1, 1, 1};
+    CUresult r = fn(reinterpret_cast<CUtensorMap*>(p->ptc_tmap), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(iq), dims,
+                    strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return false;
+    p->ptc_tmap_iq = iq;
+    return true;
+}
+
+bool project_tc_eligible(const lcf_plan* p) {
+    return p->N <= 128 && p->N >= PTC_KC && (p->Nz % 2) == 0 && p->Nz >= PTC_TZ && p->Nx >= PTC_TX && ptc_encode_fn() != nullptr;
+}
+
+// jobs = (window, column block, tile) in that order; static contiguous slices, cut at (window, block)
+cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::vector<int>& cta_first) {
+    const int K = p->K;
+    p->ptc_NB = (p->Ns + PTC_UB - 1) / PTC_UB;
+    p->ptc_Kp = (p->N + 7) / 8 * 8;
+    const int NB = p->ptc_NB;
+    std::vector<long long> pre((size_t)K * NB + 1, 0);
+    for (int k = 0; k < K; ++k) {
+        const WinBox& b = p->box_h[k];
+        const long long nt = b.Pk > 0 ? (long long)((b.z0 + b.Lz - (b.z0 & ~1) + PTC_TZ - 1) / PTC_TZ) * ((b.Lx + PTC_TX - 1) / PTC_TX) : 0;
+        for (int j = 0; j < NB; ++j) pre[(size_t)k * NB + j + 1] = pre[(size_t)k * NB + j] + nt;
+    }
+    const long long T = pre[(size_t)K * NB];
+    int grid = (int)(T < p->num_sms ? T : p->num_sms);
+    if (grid < 1) grid = 1;
+    p->ptc_grid = grid;
+    segs.clear();
+    cta_first.assign(grid + 1, 0);
+    size_t j = 0;
+    for (int c = 0; c < grid; ++c) {
+        cta_first[c] = (int)segs.size();
+        long long g0 = T * c / grid, g1 = T * (c + 1) / grid;
+        while (g0 < g1) {
+            while (j < (size_t)K * NB && pre[j + 1] <= g0) ++j;
+            const long long e = pre[j + 1] < g1 ? pre[j + 1] : g1;
+            segs.push_back({(int)(j / NB), (int)(j % NB), (int)(g0 - pre[j]), (int)(e - g0)});
+            g0 = e;
+        }
+    }
+    cta_first[grid] = (int)segs.size();
+    p->ptc_nseg = (int)segs.size();
+    p->ptc_smem = 1024 + 32 * 4096 + (size_t)PTC_RAW_STAGES * PTC_RAW_BYTES + (size_t)PTC_OP_STAGES * PTC_OP_BYTES + sizeof(PtcBars) + 16 +
+                  (size_t)(p->Nz + p->Nx) * sizeof(double);
+    if (p->ptc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
+    return cudaFuncSetAttribute(project_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ptc_smem);
+}
+
+cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
+    if (p->ptc_nseg == 0 || p->n_pitems == 0) return cudaSuccess;
+    if (p->ptc_tmap_iq != (const void*)iq && !ptc_encode_map(p, iq)) return cudaErrorInvalidValue;
+    proj_tc_pack_kernel<<<p->K * p->ptc_NB, 256, 0, st>>>(p->B_d, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    PtcArgs a;
+    a.N = p->N; a.Kp = p->ptc_Kp; a.Nz = p->Nz; a.Nx = p->Nx;
+    a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->ptc_segs_d; a.cta_first = p->ptc_cta_first_d;
+    a.bpack = p->ptc_bpack_d; a.NB = p->ptc_NB; a.part = p->ptc_part_d; a.sumPk = p->sumPk;
+    project_tc_kernel<<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(*reinterpret_cast<const CUtensorMap*>(p->ptc_tmap), a);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    proj_tc_finish_kernel<<<p->n_pitems, PROJ_TPIX, 0, st>>>(p->ptc_part_d, p->sumPk, p->ptc_NB, p->box_d, p->pitems_d, p->tiles_d, p->tsum_d);
+    return cudaGetLastError();
+}
+
+}  // namespace lcf
