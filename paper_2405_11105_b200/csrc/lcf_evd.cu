@@ -42,12 +42,8 @@ __device__ __forceinline__ void pair_pq(int m, int s, int M, int& p, int& q) {
 
 struct JacArgs {
     int N, NP, M, Ns;       // Ns = 2 NP slots, M = Ns - 1
-    int Tn;                 // Gram tile grid (canonical entry rule)
-    int from_R;             // 1: R already holds the reduced Hermitian matrices (tensor-core Gram)
     int max_sweeps;
-    const int* gfirst;      // [K+1]
-    const double2* part;    // [slot][N][N] complex double
-    void* R;                // [K][N][N] complex T
+    const void* R;          // [K][N][N] complex T, full Hermitian
     void* rotlog;           // [K][max_sweeps*M][3][NP] T
     double* lam;            // [K][N] descending
     int* order;             // [K][N]
@@ -97,11 +93,9 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
     T* red = pgi + NP;                                     // [32]
     auto rowoff = [Ns](int u) { return (u * (2 * Ns - u - 1)) / 2 - u - 1; };
 
-    // ---- load: R = sum of the Gram partials (fixed order), canonical half per entry ----
+    // ---- load the upper triangle of R_k (reduced by the Gram stage) ----
     {
-        const double2* part = a.part;
-        C* Rk = reinterpret_cast<C*>(a.R) + (size_t)k * N * N;
-        const int s0 = a.gfirst[k], s1 = a.gfirst[k + 1];
+        const C* Rk = reinterpret_cast<const C*>(a.R) + (size_t)k * N * N;
         const int nup = Ns * (Ns + 1) / 2;
         for (int e = tid; e < nup; e += nthr) {
             // e -> (u, v), u <= v, row-major over the upper triangle of Ns x Ns
@@ -111,23 +105,9 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
             while ((u + 1) * (2 * Ns - u) / 2 <= e) ++u;
             int v = u + (e - u * (2 * Ns - u + 1) / 2);
             T re = T(0), im = T(0);
-            if (v < N && a.from_R) {
+            if (v < N) {
                 const C x = Rk[(size_t)u * N + v];
                 re = x.x; im = (u == v) ? T(0) : x.y;
-            } else if (v < N) {
-                const bool direct = (u % a.Tn) <= (v % a.Tn);
-                const size_t idx = direct ? (size_t)u * N + v : (size_t)v * N + u;
-                double dre = 0.0, dim = 0.0;
-                for (int s = s0; s < s1; ++s) {
-                    const double2 x = part[(size_t)s * N * N + idx];
-                    dre += x.x; dim += x.y;
-                }
-                re = (T)dre; im = (T)dim;
-                if (!direct) im = -im;
-                if (u == v) im = T(0);
-                C o; o.x = re; o.y = im;
-                Rk[(size_t)u * N + v] = o;
-                if (u != v) { o.y = -im; Rk[(size_t)v * N + u] = o; }
             }
             if (u == v) d[u] = re;
             else { C o; o.x = re; o.y = im; S[rowoff(u) + v] = o; }
@@ -437,9 +417,8 @@ cudaError_t configure_evd(lcf_plan* p) {
 
 cudaError_t launch_jacobi(lcf_plan* p, cudaStream_t st) {
     JacArgs a;
-    a.N = p->N; a.NP = p->NP; a.M = p->Ns - 1; a.Ns = p->Ns; a.Tn = p->gram_Tn; a.max_sweeps = p->max_sweeps;
-    a.from_R = p->gram_tc ? 1 : 0;
-    a.gfirst = p->gfirst_d; a.part = p->gpart_d; a.R = p->R_d; a.rotlog = p->rotlog_d;
+    a.N = p->N; a.NP = p->NP; a.M = p->Ns - 1; a.Ns = p->Ns; a.max_sweeps = p->max_sweeps;
+    a.R = p->R_d; a.rotlog = p->rotlog_d;
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta;

@@ -217,15 +217,42 @@ cudaError_t configure_gram(lcf_plan* p) {
     return cudaFuncSetAttribute(gram_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gram_smem);
 }
 
+// R_k = sum of the window's per-chunk fp64 partials in a fixed order (deterministic, no atomics);
+// entry (u, v) is canonical in the partial iff (u mod Tn) <= (v mod Tn), otherwise its conjugate is.
+template <typename T>
+__global__ void gram_reduce_kernel(const double2* part, const int* gfirst, int N, int Tn, void* Rv) {
+    using C = typename Cx<T>::type;
+    const int k = blockIdx.z;
+    const int u = blockIdx.y * 16 + threadIdx.y, v = blockIdx.x * 16 + threadIdx.x;
+    if (u >= N || v >= N) return;
+    const bool direct = (u % Tn) <= (v % Tn);
+    const size_t idx = direct ? (size_t)u * N + v : (size_t)v * N + u;
+    double re = 0.0, im = 0.0;
+    for (int s = gfirst[k]; s < gfirst[k + 1]; ++s) {
+        const double2 x = part[(size_t)s * N * N + idx];
+        re += x.x; im += x.y;
+    }
+    if (!direct) im = -im;
+    if (u == v) im = 0.0;
+    C o; o.x = (T)re; o.y = (T)im;
+    reinterpret_cast<C*>(Rv)[(size_t)k * N * N + (size_t)u * N + v] = o;
+}
+
 cudaError_t launch_gram(lcf_plan* p, const float2* iq, cudaStream_t st) {
     GramArgs a;
     a.iq = iq; a.N = p->N; a.Nz = p->Nz; a.Kz = p->Kz; a.P = p->P; a.Nx = p->Nx;
     a.Tn = p->gram_Tn; a.ntiles = p->gram_Tn * (p->gram_Tn + 1) / 2; a.tiles_per_batch = p->gram_tiles_per_batch;
     a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.items = p->gitems_d; a.part = p->gpart_d;
     int threads = ((p->gram_tiles_per_batch + 31) / 32) * 32;
-    if (p->n_gitems == 0) return cudaSuccess;
-    if (p->prec == 1) gram_kernel<double><<<p->n_gitems, threads, p->gram_smem, st>>>(a);
-    else gram_kernel<float><<<p->n_gitems, threads, p->gram_smem, st>>>(a);
+    if (p->n_gitems > 0) {
+        if (p->prec == 1) gram_kernel<double><<<p->n_gitems, threads, p->gram_smem, st>>>(a);
+        else gram_kernel<float><<<p->n_gitems, threads, p->gram_smem, st>>>(a);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    dim3 blk(16, 16), grid((p->N + 15) / 16, (p->N + 15) / 16, p->K);
+    if (p->prec == 1) gram_reduce_kernel<double><<<grid, blk, 0, st>>>(p->gpart_d, p->gfirst_d, p->N, p->gram_Tn, p->R_d);
+    else gram_reduce_kernel<float><<<grid, blk, 0, st>>>(p->gpart_d, p->gfirst_d, p->N, p->gram_Tn, p->R_d);
     return cudaGetLastError();
 }
 

@@ -178,6 +178,11 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
         cudaGetLastError();
         p->gram_tc = false;
     }
+    p->evd_chol = evd_chol_eligible(p);
+    if (p->evd_chol && configure_evd_chol(p) != cudaSuccess) {
+        cudaGetLastError();
+        p->evd_chol = false;
+    }
     std::vector<PtcSeg> ptc_segs;
     std::vector<int> ptc_cta_first;
     p->proj_tc = project_tc_eligible(p);
@@ -292,9 +297,9 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     mark(0);
     if (e == cudaSuccess) run(1, p->gram_tc ? launch_gram_tc(p, iq, st) : launch_gram(p, iq, st));
     mark(1);
-    if (e == cudaSuccess) run(2, launch_jacobi(p, st));
+    if (e == cudaSuccess) run(2, p->evd_chol ? launch_evd_chol(p, st) : launch_jacobi(p, st));
     mark(2);
-    if (e == cudaSuccess) run(3, launch_vbuild(p, st));
+    if (e == cudaSuccess && !p->evd_chol) run(3, launch_vbuild(p, st));
     mark(3);
     if (e == cudaSuccess) run(4, p->proj_tc ? launch_project_tc(p, iq, st) : launch_project(p, iq, st));
     mark(4);
@@ -467,6 +472,6 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
     w->gram_flops = 8.0 * S * N * (N + 1.0) / 2.0;   // Hermitian half, 8 real flops per complex MAC
     w->proj_flops = 8.0 * S * N * N;                 // dense N x N projector factor
     w->hbm_bytes = 8.0 * N * (double)p->P + 4.0 * (double)p->P;
-    w->launches = 6 + (p->gram_tc ? 1 : 0) + (p->proj_tc ? 2 : 0);
+    w->launches = 2 + (p->evd_chol ? 1 : 2) + (p->proj_tc ? 3 : 1) + 2;   // gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
     return LCF_OK;
 }
