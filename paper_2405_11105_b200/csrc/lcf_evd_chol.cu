@@ -2,7 +2,8 @@
 // PAPER.md:48-50) by pivoted Cholesky + one-sided Jacobi, fused with the eigen-weights and the
 // projector factor B_k = V_k diag(wt) (Eq. 9).
 //
-// One CTA (1024 threads) per window; the matrix lives in shared memory, column-major.
+// One CTA (512 threads) per window; the matrix lives in shared memory, column-major, real and
+// imaginary planes apart so that two rows make one f32x2 operand (packed FP32 pipe).
 //   1. R' = R + delta I, delta = 3e-5 max_i R_ii (a shift moves eigenvalues, not eigenvectors; it
 //      makes the fp32 matrix numerically positive definite and gives rank-deficient windows a
 //      complete orthonormal basis).
@@ -17,13 +18,15 @@
 //      lambda_u = |g_u|^2 - delta.  After the pivoted Cholesky G^H G is strongly diagonally
 //      dominant for the graded spectra of clutter-dominated windows (Veselic/Hari, Drmac), so 3-5
 //      sweeps replace the 9-10 of two-sided Jacobi on R, and each sweep touches one matrix, not two.
-//      16 threads own one column pair per step: 3 dot products reduced by shuffles, one rotation,
+//      8 threads own one column pair per step: 3 dot products reduced by shuffles, one rotation,
 //      one barrier per step.  Like two-sided Jacobi this resolves the small (blood / noise)
 //      eigen-directions to high relative accuracy: the singular values of G span only the square
 //      root of the eigenvalue range.
 //   4. Rank the eigenvalues (descending), cut-off rule, eigen-weights, then write V_k and
 //      B_k = V_k diag(wt) straight from shared memory.
 #include <cfloat>
+#include <cstdio>
+#include <cstdlib>
 
 #include "lcf_internal.h"
 
@@ -45,6 +48,7 @@ struct EcArgs {
     float2* B;                    // [K][N][Ns]
     int mode, k_fixed;
     double energy_frac, beta;
+    long long* dbg;
 };
 
 __device__ __forceinline__ void ec_pair_pq(int m, int s, int M, int& p, int& q) {
@@ -57,135 +61,186 @@ __device__ __forceinline__ void ec_pair_pq(int m, int s, int M, int& p, int& q) 
     }
 }
 
-__global__ void __launch_bounds__(1024, 1) evd_chol_kernel(EcArgs a) {
+constexpr int EC_THREADS = 512;   // 8 threads per column pair (NP <= 64 pairs)
+
+__device__ __forceinline__ unsigned long long ec_fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ unsigned long long ec_mul2(unsigned long long a, unsigned long long b) {
+    unsigned long long d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ unsigned long long ec_pack(float x, float y) {
+    unsigned long long d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(x), "f"(y));
+    return d;
+}
+__device__ __forceinline__ float ec_hsum(unsigned long long v) {
+    float x, y;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v));
+    return x + y;
+}
+
+template <int NC, bool FULL>
+__global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = a.N, NP = a.NP, Ns = a.Ns, LD = a.LD, M = Ns - 1;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int k = blockIdx.x;
-    float2* G = reinterpret_cast<float2*>(smem_raw);                 // [Ns][LD], element (row i, col u) at u*LD + i
-    float2* lj = G + (size_t)Ns * LD;                                // [LD] current Cholesky column
-    float* lam_s = reinterpret_cast<float*>(lj + LD);                // [Ns] eigenvalue of slot u
+    // planar storage: real and imaginary parts of column u at Gr/Gi + u*LD (LD floats, multiple of 4)
+    float* Gr = reinterpret_cast<float*>(smem_raw);                  // [Ns][LD]
+    float* Gi = Gr + (size_t)Ns * LD;                                // [Ns][LD]
+    float* ljr = Gi + (size_t)Ns * LD;                               // [LD] current Cholesky column
+    float* lji = ljr + LD;                                           // [LD]
+    float* lam_s = lji + LD;                                         // [Ns] eigenvalue of slot u
     float* inv_s = lam_s + Ns;                                       // [Ns] 1 / |g_u|
     float* wsl = inv_s + Ns;                                         // [Ns] eigen-weight of slot u
-    double* lsort = reinterpret_cast<double*>(wsl + Ns);             // [N] sorted eigenvalues
+    float* red = wsl + Ns;                                           // [32]
+    double* lsort = reinterpret_cast<double*>(red + 32);             // [Ns] sorted eigenvalues
     int* act = reinterpret_cast<int*>(lsort + Ns);                   // [Ns] row/column still in the trailing matrix
-    float* red = reinterpret_cast<float*>(act + Ns);                 // [32]
-    int* ish = reinterpret_cast<int*>(red + 32);                     // [4] pivot, flags
-    float* fsh = reinterpret_cast<float*>(ish + 4);                  // [4] pivot value, scale
+    int* ish = act + Ns;                                             // [4] pivot, cut-off
+    int* alist = ish + 4;                                            // [Ns] compacted active columns
+    int* apos = alist + Ns;                                          // [Ns] position of a column in alist
+    unsigned long long* key = reinterpret_cast<unsigned long long*>(apos + Ns);   // [2] packed (pivot value, index)
 
-    // ---- load R (row-major [i][j]) into column-major G; zero the padding
+    // ---- load R (row-major [i][j]) into the column-major planes; zero the padding
     const float2* Rk = a.R + (size_t)k * N * N;
-    for (int e = tid; e < Ns * LD; e += 1024) G[e] = make_float2(0.f, 0.f);
+    for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) Gr[e] = 0.f;
     __syncthreads();
-    for (int e = tid; e < N * N; e += 1024) {
+    for (int e = tid; e < N * N; e += EC_THREADS) {
         const int i = e / N, j = e - i * N;                          // coalesced read of row i
-        G[(size_t)j * LD + i] = Rk[e];
+        const float2 x = Rk[e];
+        Gr[(size_t)j * LD + i] = x.x;
+        Gi[(size_t)j * LD + i] = x.y;
     }
     if (tid < Ns) act[tid] = tid < N ? 1 : 0;
+    if (tid < 2) key[tid] = 0ull;
     __syncthreads();
     float md = 0.f;
-    if (tid < N) md = G[(size_t)tid * LD + tid].x;
+    if (tid < N) md = Gr[(size_t)tid * LD + tid];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) md = fmaxf(md, __shfl_xor_sync(0xffffffffu, md, o));
     if (lane == 0) red[warp] = md;
     __syncthreads();
     float maxdiag = 0.f;
-    for (int w = 0; w < 32; ++w) maxdiag = fmaxf(maxdiag, red[w]);
+    for (int w = 0; w < EC_THREADS / 32; ++w) maxdiag = fmaxf(maxdiag, red[w]);
     const float delta = 3e-5f * maxdiag;
     int sweep = 0, converged = 1;
+    long long tc0 = clock64(), tc1 = 0, tc2 = 0;
 
     if (maxdiag > 0.f) {
-        if (tid < N) { G[(size_t)tid * LD + tid].x += delta; G[(size_t)tid * LD + tid].y = 0.f; }
+        if (tid < N) { Gr[(size_t)tid * LD + tid] += delta; Gi[(size_t)tid * LD + tid] = 0.f; }
         __syncthreads();
-        // ---- 2. pivoted Cholesky, in place
+        // ---- 2. pivoted Cholesky, in place.  Two barriers per step: the next pivot (largest
+        // remaining diagonal entry) is found by the trailing update itself with a packed
+        // (value, index) atomicMax, and the update runs over a compacted list of active columns.
+        const int nchc = (N + 3) >> 2;                               // 4-row chunks per column
+        if (tid < N) {
+            alist[tid] = tid; apos[tid] = tid;
+            const float d = fmaxf(Gr[(size_t)tid * LD + tid], 0.f);
+            atomicMax(&key[0], ((unsigned long long)__float_as_uint(d) << 32) | (unsigned)(N - 1 - tid));
+        }
+        __syncthreads();
         for (int j = 0; j < N; ++j) {
-            if (warp == 0) {
-                float best = -FLT_MAX; int bi = N;
-                for (int i = lane; i < N; i += 32)
-                    if (act[i]) { const float d = G[(size_t)i * LD + i].x; if (d > best) { best = d; bi = i; } }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
-                    const float ob = __shfl_xor_sync(0xffffffffu, best, o);
-                    const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                    if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
-                }
-                if (lane == 0) {
-                    // a non-positive pivot can only come from rounding: clamp (the column is then ~0)
-                    const float piv = fmaxf(best, 1e-30f * maxdiag + 1e-37f);
-                    ish[0] = bi; fsh[0] = sqrtf(piv); fsh[1] = rsqrtf(piv);
-                }
-            }
-            __syncthreads();
-            const int pv = ish[0];
-            const float dsq = fsh[0], sc = fsh[1];
+            const unsigned long long kj = key[j & 1];
+            const int pv = N - 1 - (int)(kj & 0xffffffffu);
+            // a non-positive pivot can only come from rounding: clamp (the column is then ~0)
+            const float piv = fmaxf(__uint_as_float((unsigned)(kj >> 32)), 1e-30f * maxdiag + 1e-37f);
+            const float dsq = sqrtf(piv), sc = rsqrtf(piv);
+            const int na = N - 1 - j;                                // active columns after removing pv
             if (tid < LD) {
-                float2 v = make_float2(0.f, 0.f);
-                if (tid == pv) v.x = dsq;
-                else if (tid < N && act[tid]) { const float2 x = G[(size_t)pv * LD + tid]; v = make_float2(x.x * sc, x.y * sc); }
-                G[(size_t)pv * LD + tid] = v;                         // Cholesky column pi_j, zero in eliminated rows
-                lj[tid] = (tid == pv) ? make_float2(0.f, 0.f) : v;    // multiplier for the trailing update
+                float vr = 0.f, vi = 0.f;
+                if (tid == pv) vr = dsq;
+                else if (tid < N && act[tid]) { vr = Gr[(size_t)pv * LD + tid] * sc; vi = Gi[(size_t)pv * LD + tid] * sc; }
+                Gr[(size_t)pv * LD + tid] = vr;                       // Cholesky column pi_j, zero in eliminated rows
+                Gi[(size_t)pv * LD + tid] = vi;
+                ljr[tid] = (tid == pv) ? 0.f : vr;                    // multiplier for the trailing update
+                lji[tid] = (tid == pv) ? 0.f : vi;
+            }
+            if (tid == 0) {                                          // drop pv from the active list (swap with last)
+                const int ps = apos[pv], last = alist[na];
+                alist[ps] = last; apos[last] = ps;
+                key[(j + 1) & 1] = 0ull;
             }
             __syncthreads();
             if (tid == 0) act[pv] = 0;
-            // trailing update A[i][l] -= L[i] conj(L[l]) on the still-active columns l (8 threads per column)
-            {
-                const int l = tid >> 3, rr = tid & 7;
-                if (l < N && l != pv && act[l]) {
-                    const float2 ll = lj[l];
-                    float2* col = G + (size_t)l * LD;
-                    for (int i0 = 2 * rr; i0 < N; i0 += 16) {
-                        float4 x = *reinterpret_cast<float4*>(&col[i0]);
-                        const float4 m2 = *reinterpret_cast<const float4*>(&lj[i0]);
-                        // x -= m * conj(ll)
-                        x.x -= m2.x * ll.x + m2.y * ll.y;  x.y -= m2.y * ll.x - m2.x * ll.y;
-                        x.z -= m2.z * ll.x + m2.w * ll.y;  x.w -= m2.w * ll.x - m2.z * ll.y;
-                        *reinterpret_cast<float4*>(&col[i0]) = x;
-                    }
+            // trailing update A[i][l] -= L[i] conj(L[l]) over (active column, 4-row chunk) items
+            for (int idx = tid; idx < na * nchc; idx += EC_THREADS) {
+                const int ci = idx / nchc, chk = idx - ci * nchc;
+                const int l = alist[ci];
+                const float lr = ljr[l], li = lji[l];
+                float* cr = Gr + (size_t)l * LD + 4 * chk;
+                float* ci_ = Gi + (size_t)l * LD + 4 * chk;
+                float4 xr = *reinterpret_cast<float4*>(cr);
+                float4 xi = *reinterpret_cast<float4*>(ci_);
+                const float4 mr = *reinterpret_cast<const float4*>(&ljr[4 * chk]);
+                const float4 mi = *reinterpret_cast<const float4*>(&lji[4 * chk]);
+                // x -= m * conj(l):  re -= mr lr + mi li,  im -= mi lr - mr li
+                xr.x -= mr.x * lr + mi.x * li;  xi.x -= mi.x * lr - mr.x * li;
+                xr.y -= mr.y * lr + mi.y * li;  xi.y -= mi.y * lr - mr.y * li;
+                xr.z -= mr.z * lr + mi.z * li;  xi.z -= mi.z * lr - mr.z * li;
+                xr.w -= mr.w * lr + mi.w * li;  xi.w -= mi.w * lr - mr.w * li;
+                *reinterpret_cast<float4*>(cr) = xr;
+                *reinterpret_cast<float4*>(ci_) = xi;
+                if (chk == (l >> 2)) {                               // this chunk holds the diagonal entry A[l][l]
+                    const int w = l & 3;
+                    const float d = fmaxf(w == 0 ? xr.x : w == 1 ? xr.y : w == 2 ? xr.z : xr.w, 0.f);
+                    atomicMax(&key[(j + 1) & 1], ((unsigned long long)__float_as_uint(d) << 32) | (unsigned)(N - 1 - l));
                 }
             }
             __syncthreads();
         }
-        // ---- 3. one-sided Jacobi on the columns of G
+        tc1 = clock64();
+        // ---- 3. one-sided Jacobi on the columns of G: 8 threads per pair, 4-row chunks t + 8c
         const float tol = 4.f * sqrtf((float)N) * FLT_EPSILON;
         const float tol2 = tol * tol;
-        const int m = tid >> 4, r = tid & 15;
-        const unsigned hmask = (lane < 16) ? 0x0000ffffu : 0xffff0000u;   // m < NP is uniform per half warp
+        const int m = tid >> 3, r = tid & 7;
+        const unsigned qmask = 0xffu << (lane & 24);                 // the pair's 8 lanes (m < NP is uniform over them)
+        const int nch = (N + 3) >> 2;                                // 4-row chunks per column
         converged = 0;
         for (;;) {
             int any = 0;
             for (int s = 0; s < M; ++s) {
-                int rot = 0;
                 if (m < NP) {
                     int p, q; ec_pair_pq(m, s, M, p, q);
-                    float2* gp = G + (size_t)p * LD;
-                    float2* gq = G + (size_t)q * LD;
-                    float4 xp[4], xq[4];
-                    float app = 0.f, aqq = 0.f, xr = 0.f, xi = 0.f;
+                    float* pr_ = Gr + (size_t)p * LD; float* pi_ = Gi + (size_t)p * LD;
+                    float* qr_ = Gr + (size_t)q * LD; float* qi_ = Gi + (size_t)q * LD;
+                    ulonglong2 PR[NC], PI[NC], QR[NC], QI[NC];
+                    unsigned long long app2 = 0ull, aqq2 = 0ull, re2 = 0ull, ima2 = 0ull, imb2 = 0ull;
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        const int i0 = 2 * r + 32 * c;
-                        if (i0 < N) {
-                            xp[c] = *reinterpret_cast<const float4*>(&gp[i0]);
-                            xq[c] = *reinterpret_cast<const float4*>(&gq[i0]);
-                            app = fmaf(xp[c].x, xp[c].x, fmaf(xp[c].y, xp[c].y, fmaf(xp[c].z, xp[c].z, fmaf(xp[c].w, xp[c].w, app))));
-                            aqq = fmaf(xq[c].x, xq[c].x, fmaf(xq[c].y, xq[c].y, fmaf(xq[c].z, xq[c].z, fmaf(xq[c].w, xq[c].w, aqq))));
-                            // conj(g_p) g_q
-                            xr = fmaf(xp[c].x, xq[c].x, fmaf(xp[c].y, xq[c].y, fmaf(xp[c].z, xq[c].z, fmaf(xp[c].w, xq[c].w, xr))));
-                            xi = fmaf(xp[c].x, xq[c].y, fmaf(-xp[c].y, xq[c].x, fmaf(xp[c].z, xq[c].w, fmaf(-xp[c].w, xq[c].z, xi))));
+                    for (int c = 0; c < NC; ++c) {
+                        const int ch = r + 8 * c;
+                        if (FULL || ch < nch) {
+                            PR[c] = *reinterpret_cast<const ulonglong2*>(&pr_[4 * ch]);
+                            PI[c] = *reinterpret_cast<const ulonglong2*>(&pi_[4 * ch]);
+                            QR[c] = *reinterpret_cast<const ulonglong2*>(&qr_[4 * ch]);
+                            QI[c] = *reinterpret_cast<const ulonglong2*>(&qi_[4 * ch]);
+                            app2 = ec_fma2(PR[c].x, PR[c].x, app2); app2 = ec_fma2(PI[c].x, PI[c].x, app2);
+                            app2 = ec_fma2(PR[c].y, PR[c].y, app2); app2 = ec_fma2(PI[c].y, PI[c].y, app2);
+                            aqq2 = ec_fma2(QR[c].x, QR[c].x, aqq2); aqq2 = ec_fma2(QI[c].x, QI[c].x, aqq2);
+                            aqq2 = ec_fma2(QR[c].y, QR[c].y, aqq2); aqq2 = ec_fma2(QI[c].y, QI[c].y, aqq2);
+                            // conj(g_p) g_q = (pr qr + pi qi) + i (pr qi - pi qr)
+                            re2 = ec_fma2(PR[c].x, QR[c].x, re2);   re2 = ec_fma2(PI[c].x, QI[c].x, re2);
+                            re2 = ec_fma2(PR[c].y, QR[c].y, re2);   re2 = ec_fma2(PI[c].y, QI[c].y, re2);
+                            ima2 = ec_fma2(PR[c].x, QI[c].x, ima2); imb2 = ec_fma2(PI[c].x, QR[c].x, imb2);
+                            ima2 = ec_fma2(PR[c].y, QI[c].y, ima2); imb2 = ec_fma2(PI[c].y, QR[c].y, imb2);
                         }
                     }
+                    float app = ec_hsum(app2), aqq = ec_hsum(aqq2), xr = ec_hsum(re2), xi = ec_hsum(ima2) - ec_hsum(imb2);
 #pragma unroll
-                    for (int o = 8; o > 0; o >>= 1) {                 // within the pair's 16 lanes
-                        app += __shfl_xor_sync(hmask, app, o);
-                        aqq += __shfl_xor_sync(hmask, aqq, o);
-                        xr += __shfl_xor_sync(hmask, xr, o);
-                        xi += __shfl_xor_sync(hmask, xi, o);
+                    for (int o = 4; o > 0; o >>= 1) {
+                        app += __shfl_xor_sync(qmask, app, o);
+                        aqq += __shfl_xor_sync(qmask, aqq, o);
+                        xr += __shfl_xor_sync(qmask, xr, o);
+                        xi += __shfl_xor_sync(qmask, xi, o);
                     }
                     const float absa2 = xr * xr + xi * xi;
                     if (absa2 > tol2 * app * aqq && absa2 > 0.f) {
-                        rot = 1;
+                        any = 1;
                         const float inv = rsqrtf(absa2);
-                        const float absa = absa2 * inv;
                         const float tau = (aqq - app) * (0.5f * inv);
                         const float at = fabsf(tau);
                         float t = (at > 1e8f) ? 0.5f / at : 1.f / (at + sqrtf(1.f + tau * tau));
@@ -193,52 +248,59 @@ __global__ void __launch_bounds__(1024, 1) evd_chol_kernel(EcArgs a) {
                         const float cs = rsqrtf(1.f + t * t);
                         const float sn = t * cs;
                         const float gr = sn * xr * inv, gi = sn * xi * inv;
-                        (void)absa;
+                        const unsigned long long c2 = ec_pack(cs, cs), gr2 = ec_pack(gr, gr), gi2 = ec_pack(gi, gi);
+                        const unsigned long long ngr2 = ec_pack(-gr, -gr), ngi2 = ec_pack(-gi, -gi);
 #pragma unroll
-                        for (int c = 0; c < 4; ++c) {
-                            const int i0 = 2 * r + 32 * c;
-                            if (i0 < N) {
-                                float4 np_, nq_;
+                        for (int c = 0; c < NC; ++c) {
+                            const int ch = r + 8 * c;
+                            if (FULL || ch < nch) {
+                                ulonglong2 npr, npi, nqr, nqi;
                                 // g_p' = c g_p - conj(g) g_q,   g_q' = g g_p + c g_q
-                                np_.x = cs * xp[c].x - (gr * xq[c].x + gi * xq[c].y);
-                                np_.y = cs * xp[c].y - (gr * xq[c].y - gi * xq[c].x);
-                                np_.z = cs * xp[c].z - (gr * xq[c].z + gi * xq[c].w);
-                                np_.w = cs * xp[c].w - (gr * xq[c].w - gi * xq[c].z);
-                                nq_.x = (gr * xp[c].x - gi * xp[c].y) + cs * xq[c].x;
-                                nq_.y = (gr * xp[c].y + gi * xp[c].x) + cs * xq[c].y;
-                                nq_.z = (gr * xp[c].z - gi * xp[c].w) + cs * xq[c].z;
-                                nq_.w = (gr * xp[c].w + gi * xp[c].z) + cs * xq[c].w;
-                                *reinterpret_cast<float4*>(&gp[i0]) = np_;
-                                *reinterpret_cast<float4*>(&gq[i0]) = nq_;
+                                npr.x = ec_fma2(ngi2, QI[c].x, ec_fma2(ngr2, QR[c].x, ec_mul2(c2, PR[c].x)));
+                                npr.y = ec_fma2(ngi2, QI[c].y, ec_fma2(ngr2, QR[c].y, ec_mul2(c2, PR[c].y)));
+                                npi.x = ec_fma2(gi2, QR[c].x, ec_fma2(ngr2, QI[c].x, ec_mul2(c2, PI[c].x)));
+                                npi.y = ec_fma2(gi2, QR[c].y, ec_fma2(ngr2, QI[c].y, ec_mul2(c2, PI[c].y)));
+                                nqr.x = ec_fma2(c2, QR[c].x, ec_fma2(ngi2, PI[c].x, ec_mul2(gr2, PR[c].x)));
+                                nqr.y = ec_fma2(c2, QR[c].y, ec_fma2(ngi2, PI[c].y, ec_mul2(gr2, PR[c].y)));
+                                nqi.x = ec_fma2(c2, QI[c].x, ec_fma2(gi2, PR[c].x, ec_mul2(gr2, PI[c].x)));
+                                nqi.y = ec_fma2(c2, QI[c].y, ec_fma2(gi2, PR[c].y, ec_mul2(gr2, PI[c].y)));
+                                *reinterpret_cast<ulonglong2*>(&pr_[4 * ch]) = npr;
+                                *reinterpret_cast<ulonglong2*>(&pi_[4 * ch]) = npi;
+                                *reinterpret_cast<ulonglong2*>(&qr_[4 * ch]) = nqr;
+                                *reinterpret_cast<ulonglong2*>(&qi_[4 * ch]) = nqi;
                             }
                         }
                     }
                 }
-                any |= __syncthreads_or(rot);
+                __syncthreads();
             }
             ++sweep;
-            if (!any) { converged = 1; break; }
+            if (!__syncthreads_or(any)) { converged = 1; break; }
             if (sweep == a.max_sweeps) break;
         }
     } else {
         // zero matrix (empty window): V = I, all eigenvalues 0
-        if (tid < N) G[(size_t)tid * LD + tid] = make_float2(1.f, 0.f);
+        if (tid < N) Gr[(size_t)tid * LD + tid] = 1.f;
         __syncthreads();
     }
 
+    tc2 = clock64();
     // ---- 4. eigenvalues = squared column norms - delta, eigenvectors = normalised columns
     {
-        const int u = tid >> 3, rr = tid & 7;                        // 8 threads per column
+        const int u = tid >> 2, rr = tid & 3;                        // 4 threads per column
         float nn = 0.f;
         if (u < Ns) {
-            const float2* col = G + (size_t)u * LD;
-            for (int i0 = 2 * rr; i0 < N; i0 += 16) {
-                const float4 x = *reinterpret_cast<const float4*>(&col[i0]);
+            const float* cr = Gr + (size_t)u * LD;
+            const float* ci = Gi + (size_t)u * LD;
+            for (int i0 = 4 * rr; i0 < N; i0 += 16) {
+                const float4 x = *reinterpret_cast<const float4*>(&cr[i0]);
+                const float4 y = *reinterpret_cast<const float4*>(&ci[i0]);
                 nn = fmaf(x.x, x.x, fmaf(x.y, x.y, fmaf(x.z, x.z, fmaf(x.w, x.w, nn))));
+                nn = fmaf(y.x, y.x, fmaf(y.y, y.y, fmaf(y.z, y.z, fmaf(y.w, y.w, nn))));
             }
         }
 #pragma unroll
-        for (int o = 4; o > 0; o >>= 1) nn += __shfl_xor_sync(0xffffffffu, nn, o);
+        for (int o = 2; o > 0; o >>= 1) nn += __shfl_xor_sync(0xffffffffu, nn, o);
         if (u < Ns && rr == 0) {
             lam_s[u] = (maxdiag > 0.f && u < N) ? nn - delta : 0.f;
             inv_s[u] = nn > 0.f ? rsqrtf(nn) : 0.f;
@@ -297,27 +359,32 @@ __global__ void __launch_bounds__(1024, 1) evd_chol_kernel(EcArgs a) {
     // V[a][u] = G[a][u] / |g_u|,  B = V diag(wt): lanes run over the slot u (coalesced global writes)
     float2* Vk = a.V + (size_t)k * N * Ns;
     float2* Bk = a.B + (size_t)k * N * Ns;
-    for (int e = tid; e < N * Ns; e += 1024) {
+    if (a.dbg && k == 0 && tid == 0) { a.dbg[0] = tc1 - tc0; a.dbg[1] = tc2 - tc1; a.dbg[2] = clock64() - tc2; a.dbg[3] = sweep; }
+    for (int e = tid; e < N * Ns; e += EC_THREADS) {
         const int row = e / Ns, u = e - row * Ns;
-        const float2 x = G[(size_t)u * LD + row];
         const float s1 = inv_s[u], w = wsl[u];
-        const float2 v = make_float2(x.x * s1, x.y * s1);
+        const float2 v = make_float2(Gr[(size_t)u * LD + row] * s1, Gi[(size_t)u * LD + row] * s1);
         Vk[e] = v;
         Bk[e] = make_float2(v.x * w, v.y * w);
     }
 }
 
 static size_t ec_smem_bytes(int Ns, int LD) {
-    return (size_t)Ns * LD * 8 + (size_t)LD * 8 + 3 * (size_t)Ns * 4 + (size_t)Ns * 8 + (size_t)Ns * 4 + 32 * 4 + 16 + 16 + 64;
+    return (size_t)Ns * LD * 8 + (size_t)LD * 8 + 3 * (size_t)Ns * 4 + 32 * 4 + (size_t)Ns * 8 + 3 * (size_t)Ns * 4 + 16 + 16 + 64;
 }
 
 bool evd_chol_eligible(const lcf_plan* p) { return p->prec == 0 && p->N <= 128 && p->N >= 2; }
 
 cudaError_t configure_evd_chol(lcf_plan* p) {
-    p->ec_LD = ((p->N + 1) & ~1) + 2;
+    p->ec_LD = ((p->N + 3) & ~3) + 4;   // floats per column plane: whole float4 chunks, +4 shifts the banks column to column
     p->ec_smem = ec_smem_bytes(p->Ns, p->ec_LD);
     if (p->ec_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
-    return cudaFuncSetAttribute(evd_chol_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ec_smem);
+    cudaError_t e = cudaSuccess;
+#define EC_SET(NC, FULL) if (e == cudaSuccess) e = cudaFuncSetAttribute(evd_chol_kernel<NC, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ec_smem)
+    EC_SET(1, false); EC_SET(2, false); EC_SET(3, false); EC_SET(4, false);
+    EC_SET(1, true); EC_SET(2, true); EC_SET(3, true); EC_SET(4, true);
+#undef EC_SET
+    return e;
 }
 
 cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st) {
@@ -328,7 +395,16 @@ cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st) {
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
     a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta;
-    evd_chol_kernel<<<p->K, 1024, p->ec_smem, st>>>(a);
+    static long long* dbg_d = nullptr;
+    a.dbg = nullptr;
+    if (getenv("LCF_EC_PROFILE")) { if (!dbg_d) cudaMalloc(&dbg_d, 64); a.dbg = dbg_d; }
+    const int nch = (p->N + 3) / 4, nc = (nch + 7) / 8;
+    const bool full = (p->N % 32) == 0;
+#define EC_RUN(NC) do { if (full) evd_chol_kernel<NC, true><<<p->K, EC_THREADS, p->ec_smem, st>>>(a); \
+                        else evd_chol_kernel<NC, false><<<p->K, EC_THREADS, p->ec_smem, st>>>(a); } while (0)
+    switch (nc) { case 1: EC_RUN(1); break; case 2: EC_RUN(2); break; case 3: EC_RUN(3); break; default: EC_RUN(4); break; }
+#undef EC_RUN
+    if (a.dbg) { long long h[4]; cudaMemcpy(h, dbg_d, 32, cudaMemcpyDeviceToHost); fprintf(stderr, "evd: chol %lld jacobi %lld (%lld sweeps) tail %lld cycles\n", h[0], h[1], h[3], h[2]); }
     return cudaGetLastError();
 }
 
