@@ -112,10 +112,15 @@ lcf_status lcf_get_window_means(lcf_plan* plan, double* m /* HOST [K] */);
 lcf_status lcf_set_timing(lcf_plan* plan, int enabled);
 lcf_status lcf_get_stage_ms(lcf_plan* plan, float ms[5] /* HOST */);
 /* Algorithmic work of one lcf_filter call: Hermitian-half Gram flops,
- * projection flops, compulsory HBM bytes, sum_k P_k, kernel launches per call. */
+ * projection flops, compulsory HBM bytes, sum_k P_k, kernel launches per call; which kernels the
+ * plan selected (1 = tcgen05 Gram / Cholesky + one-sided Jacobi EVD / tcgen05 projection, 0 = the
+ * FP32/FP64 CUDA-core kernels) and, for the tensor-core kernels, the flops the MMAs execute
+ * (3xTF32 split, padded tiles) -- the algorithmic flops are what the rooflines are quoted on. */
 typedef struct {
     double gram_flops, proj_flops, hbm_bytes, sum_Pk;
     int launches;
+    int gram_tc, evd_chol, proj_tc;
+    double gram_tensor_flops, proj_tensor_flops;
 } lcf_work;
 lcf_status lcf_get_work(const lcf_plan* plan, lcf_work* out /* HOST */);
 /* Arithmetic-pipe microbenchmark on the current device: kind 0 = FP32 FFMA, 1 = FP32 packed

@@ -37,7 +37,8 @@ class Thresh(C.Structure):
 
 class Work(C.Structure):
     _fields_ = [("gram_flops", C.c_double), ("proj_flops", C.c_double), ("hbm_bytes", C.c_double),
-                ("sum_Pk", C.c_double), ("launches", C.c_int)]
+                ("sum_Pk", C.c_double), ("launches", C.c_int), ("gram_tc", C.c_int), ("evd_chol", C.c_int),
+                ("proj_tc", C.c_int), ("gram_tensor_flops", C.c_double), ("proj_tensor_flops", C.c_double)]
 
 
 class LcfError(RuntimeError):
