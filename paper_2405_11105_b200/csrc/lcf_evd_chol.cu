@@ -25,8 +25,6 @@
 //   4. Rank the eigenvalues (descending), cut-off rule, eigen-weights, then write V_k and
 //      B_k = V_k diag(wt) straight from shared memory.
 #include <cfloat>
-#include <cstdio>
-#include <cstdlib>
 
 #include "lcf_internal.h"
 
@@ -48,7 +46,9 @@ struct EcArgs {
     float2* B;                    // [K][N][Ns]
     int mode, k_fixed;
     double energy_frac, beta;
-    long long* dbg;
+    int chol_only;                // 1: stop after the Cholesky factor and write it to gfac / shift (cluster Jacobi follows)
+    float* gfac;                  // [K][2][Ns][LD] real plane, imaginary plane of G, column-major
+    float* shift;                 // [K] delta, or -1 for an all-zero matrix
 };
 
 __device__ __forceinline__ void ec_pair_pq(int m, int s, int M, int& p, int& q) {
@@ -129,7 +129,6 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     for (int w = 0; w < EC_THREADS / 32; ++w) maxdiag = fmaxf(maxdiag, red[w]);
     const float delta = 3e-5f * maxdiag;
     int sweep = 0, converged = 1;
-    long long tc0 = clock64(), tc1 = 0, tc2 = 0;
 
     if (maxdiag > 0.f) {
         if (tid < N) { Gr[(size_t)tid * LD + tid] += delta; Gi[(size_t)tid * LD + tid] = 0.f; }
@@ -193,7 +192,12 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
             }
             __syncthreads();
         }
-        tc1 = clock64();
+        if (a.chol_only) {
+            float* gout = a.gfac + (size_t)k * 2 * Ns * LD;
+            for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) gout[e] = Gr[e];
+            if (tid == 0) a.shift[k] = delta;
+            return;
+        }
         // ---- 3. one-sided Jacobi on the columns of G: 8 threads per pair, 4-row chunks t + 8c
         const float tol = 4.f * sqrtf((float)N) * FLT_EPSILON;
         const float tol2 = tol * tol;
@@ -282,9 +286,14 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         // zero matrix (empty window): V = I, all eigenvalues 0
         if (tid < N) Gr[(size_t)tid * LD + tid] = 1.f;
         __syncthreads();
+        if (a.chol_only) {
+            float* gout = a.gfac + (size_t)k * 2 * Ns * LD;
+            for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) gout[e] = Gr[e];
+            if (tid == 0) a.shift[k] = -1.f;
+            return;
+        }
     }
 
-    tc2 = clock64();
     // ---- 4. eigenvalues = squared column norms - delta, eigenvectors = normalised columns
     {
         const int u = tid >> 2, rr = tid & 3;                        // 4 threads per column
@@ -359,7 +368,6 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     // V[a][u] = G[a][u] / |g_u|,  B = V diag(wt): lanes run over the slot u (coalesced global writes)
     float2* Vk = a.V + (size_t)k * N * Ns;
     float2* Bk = a.B + (size_t)k * N * Ns;
-    if (a.dbg && k == 0 && tid == 0) { a.dbg[0] = tc1 - tc0; a.dbg[1] = tc2 - tc1; a.dbg[2] = clock64() - tc2; a.dbg[3] = sweep; }
     for (int e = tid; e < N * Ns; e += EC_THREADS) {
         const int row = e / Ns, u = e - row * Ns;
         const float s1 = inv_s[u], w = wsl[u];
@@ -387,24 +395,21 @@ cudaError_t configure_evd_chol(lcf_plan* p) {
     return e;
 }
 
-cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st) {
+cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only) {
     EcArgs a;
+    a.chol_only = chol_only ? 1 : 0; a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d;
     a.N = p->N; a.NP = p->NP; a.Ns = p->Ns; a.LD = p->ec_LD; a.max_sweeps = 30;
     a.R = reinterpret_cast<const float2*>(p->R_d);
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
     a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta;
-    static long long* dbg_d = nullptr;
-    a.dbg = nullptr;
-    if (getenv("LCF_EC_PROFILE")) { if (!dbg_d) cudaMalloc(&dbg_d, 64); a.dbg = dbg_d; }
     const int nch = (p->N + 3) / 4, nc = (nch + 7) / 8;
     const bool full = (p->N % 32) == 0;
 #define EC_RUN(NC) do { if (full) evd_chol_kernel<NC, true><<<p->K, EC_THREADS, p->ec_smem, st>>>(a); \
                         else evd_chol_kernel<NC, false><<<p->K, EC_THREADS, p->ec_smem, st>>>(a); } while (0)
     switch (nc) { case 1: EC_RUN(1); break; case 2: EC_RUN(2); break; case 3: EC_RUN(3); break; default: EC_RUN(4); break; }
 #undef EC_RUN
-    if (a.dbg) { long long h[4]; cudaMemcpy(h, dbg_d, 32, cudaMemcpyDeviceToHost); fprintf(stderr, "evd: chol %lld jacobi %lld (%lld sweeps) tail %lld cycles\n", h[0], h[1], h[3], h[2]); }
     return cudaGetLastError();
 }
 

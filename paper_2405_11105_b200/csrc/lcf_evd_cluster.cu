@@ -1,0 +1,360 @@
+// lcf_evd_cluster.cu -- kernel 2+3, one-sided Jacobi spread over a 2-CTA thread-block cluster
+// (precision 0, even N, 32 <= N <= 128).  The single-CTA kernel of lcf_evd_chol.cu is bound by
+// shared-memory bandwidth (the whole N x N matrix crosses the 128 B/clk crossbar twice per
+// rotation step) and uses 64 of 148 SMs at 64 windows; here each matrix gets two SMs.
+//
+// Input: the shifted, pivoted Cholesky factor G of R_k (lcf_evd_chol.cu run with chol_only).
+// The n = N/2 column pairs of a step are laid out as a systolic array (Brent-Luk): pair i holds
+// the columns (top[i], bot[i]); after every rotation step top[] shifts one pair up, bot[] one pair
+// down, with the turn-arounds  top[0] fixed, bot[0] -> top[1], top[n-1] -> bot[n-1],  which visits
+// every column pair once in 2n-1 steps.  CTA 0 owns pairs [0, h), CTA 1 pairs [h, n): a pair's two
+// columns (all N rows) are always in one CTA, so the dot products need no cross-CTA reduction; a
+// rotated column is written straight into its destination slot of the other buffer (double
+// buffering), which for the two columns that cross the CTA boundary is a DSMEM store into the peer
+// CTA's shared memory.  One cluster barrier per step covers both the local and the remote hazard.
+// 16 threads own a pair (8 rows each, real and imaginary planes apart, packed f32x2 math).
+// Epilogue as in lcf_evd_chol.cu: lambda = |g|^2 - delta, ranking, cut-off rule, eigen-weights,
+// V_k = normalised columns, B_k = V_k diag(wt).
+#include <cfloat>
+
+#include "lcf_internal.h"
+
+namespace lcf {
+
+constexpr int ECL_THREADS = 512;
+constexpr int ECL_PL = 32;                     // pair slots per CTA (n <= 64)
+
+struct EclArgs {
+    int N, n, h, LD, LDg;                      // n pairs, CTA 0 owns [0, h); LD floats per column plane here, LDg in gfac
+    int max_sweeps;
+    const float* gfac;                         // [K][2][N][LDg]
+    const float* shift;                        // [K]
+    double* lam; int* order; int* cut; int* sweeps; int* conv;
+    float* wslot; double* wslot_dd; double* wt;
+    float2* V; float2* B;                      // [K][N][N]
+    int mode, k_fixed;
+    double energy_frac, beta;
+};
+
+__device__ __forceinline__ unsigned long long ecl_fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ unsigned long long ecl_mul2(unsigned long long a, unsigned long long b) {
+    unsigned long long d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ unsigned long long ecl_pack(float x, float y) {
+    unsigned long long d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(x), "f"(y));
+    return d;
+}
+__device__ __forceinline__ float ecl_hsum(unsigned long long v) {
+    float x, y;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v));
+    return x + y;
+}
+__device__ __forceinline__ uint32_t ecl_smem(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+// address of the same shared-memory location in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t ecl_mapa(uint32_t addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void ecl_st_cluster(uint32_t addr, ulonglong2 v) {
+    asm volatile("st.shared::cluster.v2.b64 [%0], {%1, %2};" ::"r"(addr), "l"(v.x), "l"(v.y) : "memory");
+}
+__device__ __forceinline__ void ecl_st_local(uint32_t addr, ulonglong2 v) {
+    asm volatile("st.shared.v2.b64 [%0], {%1, %2};" ::"r"(addr), "l"(v.x), "l"(v.y) : "memory");
+}
+__device__ __forceinline__ void ecl_st_cluster_f32(uint32_t addr, float v) {
+    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void ecl_cluster_sync() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t ecl_cluster_rank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+
+// column slot (buffer b, row t: 0 top / 1 bottom, local pair j): real plane, then imaginary plane
+__device__ __forceinline__ int ecl_slot(int b, int t, int j, int LD) { return (((b * 2 + t) * ECL_PL + j) * 2) * LD; }
+
+template <int NC, bool FULL>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jacobi_cluster_kernel(EclArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = a.N, n = a.n, h = a.h, LD = a.LD, Ns = N;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const uint32_t rank = ecl_cluster_rank(), peer = rank ^ 1u;
+    const int k = blockIdx.x >> 1;
+    const int p0 = rank ? h : 0, npl = rank ? n - h : h;          // this CTA's pairs [p0, p0 + npl)
+    float* buf = reinterpret_cast<float*>(smem_raw);                 // [2 buffers][2 rows][ECL_PL][2 planes][LD]
+    float* lam_s = buf + (size_t)2 * 2 * ECL_PL * 2 * LD;            // [Ns] eigenvalue of slot u (all slots, both CTAs)
+    float* inv_s = lam_s + Ns;                                       // [Ns]
+    float* wsl = inv_s + Ns;                                         // [Ns]
+    float* flg = wsl + Ns;                                           // [2 parities][2 ranks] "rotated in this sweep"
+    double* lsort = reinterpret_cast<double*>(flg + 4);              // [Ns]
+    int* ish = reinterpret_cast<int*>(lsort + Ns);                   // [4]
+    const uint32_t buf_u32 = ecl_smem(buf), buf_peer = ecl_mapa(buf_u32, peer);
+
+    // ---- initial placement: top[i] = column 2i, bot[i] = column 2i+1
+    const float* gk = a.gfac + (size_t)k * 2 * N * a.LDg;
+    const int nch = (N + 3) >> 2;                                    // 4-row chunks per column
+    for (int e = tid; e < npl * 2 * 2 * nch; e += ECL_THREADS) {
+        const int ch = e % nch; int q = e / nch;
+        const int pl = q & 1; q >>= 1;
+        const int t = q & 1, j = q >> 1;
+        const int col = 2 * (p0 + j) + t;
+        const float4 v = *reinterpret_cast<const float4*>(gk + ((size_t)pl * N + col) * a.LDg + 4 * ch);
+        *reinterpret_cast<float4*>(buf + ecl_slot(0, t, j, LD) + pl * LD + 4 * ch) = v;
+    }
+    const float shiftv = a.shift[k];
+    const float delta = shiftv < 0.f ? 0.f : shiftv;
+    ecl_cluster_sync();                                              // both CTAs resident, buffers filled
+
+    // ---- one-sided Jacobi sweeps
+    const float tol = 4.f * sqrtf((float)N) * FLT_EPSILON;
+    const float tol2 = tol * tol;
+    const int j = tid >> 4, r = tid & 15;                            // local pair, lane within the pair
+    const int gi = p0 + j;                                           // global pair index
+    const unsigned hmask = (lane < 16) ? 0x0000ffffu : 0xffff0000u;  // j < npl is uniform per half warp
+    // destinations of this pair's columns after the step (row, global pair): see the header
+    int dPt, dPi, dQt, dQi;
+    if (gi == 0) { dPt = 0; dPi = 0; dQt = 0; dQi = 1; }
+    else { dQt = 1; dQi = gi - 1; if (gi == n - 1) { dPt = 1; dPi = n - 1; } else { dPt = 0; dPi = gi + 1; } }
+    if (n == 1) { dPt = 0; dPi = 0; dQt = 1; dQi = 0; }
+    const bool Prem = (dPi >= h) != (rank == 1), Qrem = (dQi >= h) != (rank == 1);
+    const int dPj = dPi - (dPi >= h ? h : 0), dQj = dQi - (dQi >= h ? h : 0);
+    const int M = 2 * n - 1;
+    int b = 0, sweep = 0, converged = 0;
+    for (;;) {
+        int any = 0;
+        for (int s = 0; s < M; ++s) {
+            if (j < npl) {
+                const float* pr_ = buf + ecl_slot(b, 0, j, LD); const float* pi_ = pr_ + LD;
+                const float* qr_ = buf + ecl_slot(b, 1, j, LD); const float* qi_ = qr_ + LD;
+                ulonglong2 PR[NC], PI[NC], QR[NC], QI[NC];
+                unsigned long long app2 = 0ull, aqq2 = 0ull, re2 = 0ull, ima2 = 0ull, imb2 = 0ull;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const int ch = r + 16 * c;
+                    PR[c] = PI[c] = QR[c] = QI[c] = make_ulonglong2(0ull, 0ull);
+                    if (FULL || ch < nch) {
+                        PR[c] = *reinterpret_cast<const ulonglong2*>(&pr_[4 * ch]);
+                        PI[c] = *reinterpret_cast<const ulonglong2*>(&pi_[4 * ch]);
+                        QR[c] = *reinterpret_cast<const ulonglong2*>(&qr_[4 * ch]);
+                        QI[c] = *reinterpret_cast<const ulonglong2*>(&qi_[4 * ch]);
+                        app2 = ecl_fma2(PR[c].x, PR[c].x, app2); app2 = ecl_fma2(PI[c].x, PI[c].x, app2);
+                        app2 = ecl_fma2(PR[c].y, PR[c].y, app2); app2 = ecl_fma2(PI[c].y, PI[c].y, app2);
+                        aqq2 = ecl_fma2(QR[c].x, QR[c].x, aqq2); aqq2 = ecl_fma2(QI[c].x, QI[c].x, aqq2);
+                        aqq2 = ecl_fma2(QR[c].y, QR[c].y, aqq2); aqq2 = ecl_fma2(QI[c].y, QI[c].y, aqq2);
+                        re2 = ecl_fma2(PR[c].x, QR[c].x, re2);   re2 = ecl_fma2(PI[c].x, QI[c].x, re2);
+                        re2 = ecl_fma2(PR[c].y, QR[c].y, re2);   re2 = ecl_fma2(PI[c].y, QI[c].y, re2);
+                        ima2 = ecl_fma2(PR[c].x, QI[c].x, ima2); imb2 = ecl_fma2(PI[c].x, QR[c].x, imb2);
+                        ima2 = ecl_fma2(PR[c].y, QI[c].y, ima2); imb2 = ecl_fma2(PI[c].y, QR[c].y, imb2);
+                    }
+                }
+                float app = ecl_hsum(app2), aqq = ecl_hsum(aqq2), xr = ecl_hsum(re2), xi = ecl_hsum(ima2) - ecl_hsum(imb2);
+#pragma unroll
+                for (int o = 8; o > 0; o >>= 1) {
+                    app += __shfl_xor_sync(hmask, app, o);
+                    aqq += __shfl_xor_sync(hmask, aqq, o);
+                    xr += __shfl_xor_sync(hmask, xr, o);
+                    xi += __shfl_xor_sync(hmask, xi, o);
+                }
+                const float absa2 = xr * xr + xi * xi;
+                const bool rot = absa2 > tol2 * app * aqq && absa2 > 0.f;
+                float cs = 1.f, gr = 0.f, gim = 0.f;
+                if (rot) {
+                    any = 1;
+                    // t only steers the rotation (a slightly off angle costs convergence, not accuracy):
+                    // approximate sqrt and reciprocal; c^2 + s^2 = 1 rests on one Newton step on rsqrt
+                    const float inv = rsqrtf(absa2);
+                    const float tau = (aqq - app) * (0.5f * inv);
+                    const float at = fminf(fabsf(tau), 1e18f);
+                    const float w1 = fmaf(at, at, 1.f);
+                    const float t0 = __fdividef(1.f, at + w1 * rsqrtf(w1));
+                    const float t = copysignf(t0, tau);
+                    const float x1 = fmaf(t, t, 1.f);
+                    float c0 = rsqrtf(x1);
+                    c0 = c0 * fmaf(-0.5f * x1, c0 * c0, 1.5f);
+                    cs = c0;
+                    const float sn = t * cs;
+                    gr = sn * xr * inv; gim = sn * xi * inv;
+                }
+                const unsigned long long c2 = ecl_pack(cs, cs), gr2 = ecl_pack(gr, gr), gi2 = ecl_pack(gim, gim);
+                const unsigned long long ngr2 = ecl_pack(-gr, -gr), ngi2 = ecl_pack(-gim, -gim);
+                // destination slots in the other buffer (local generic pointer or peer DSMEM address)
+                const int oP = ecl_slot(b ^ 1, dPt, dPj, LD), oQ = ecl_slot(b ^ 1, dQt, dQj, LD);
+                const uint32_t aP = (Prem ? buf_peer : buf_u32) + (uint32_t)oP * 4u;
+                const uint32_t aQ = (Qrem ? buf_peer : buf_u32) + (uint32_t)oQ * 4u;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const int ch = r + 16 * c;
+                    if (FULL || ch < nch) {
+                        ulonglong2 npr, npi, nqr, nqi;
+                        // g_p' = c g_p - conj(g) g_q,   g_q' = g g_p + c g_q   (identity when not rotating)
+                        npr.x = ecl_fma2(ngi2, QI[c].x, ecl_fma2(ngr2, QR[c].x, ecl_mul2(c2, PR[c].x)));
+                        npr.y = ecl_fma2(ngi2, QI[c].y, ecl_fma2(ngr2, QR[c].y, ecl_mul2(c2, PR[c].y)));
+                        npi.x = ecl_fma2(gi2, QR[c].x, ecl_fma2(ngr2, QI[c].x, ecl_mul2(c2, PI[c].x)));
+                        npi.y = ecl_fma2(gi2, QR[c].y, ecl_fma2(ngr2, QI[c].y, ecl_mul2(c2, PI[c].y)));
+                        nqr.x = ecl_fma2(c2, QR[c].x, ecl_fma2(ngi2, PI[c].x, ecl_mul2(gr2, PR[c].x)));
+                        nqr.y = ecl_fma2(c2, QR[c].y, ecl_fma2(ngi2, PI[c].y, ecl_mul2(gr2, PR[c].y)));
+                        nqi.x = ecl_fma2(c2, QI[c].x, ecl_fma2(gi2, PR[c].x, ecl_mul2(gr2, PI[c].x)));
+                        nqi.y = ecl_fma2(c2, QI[c].y, ecl_fma2(gi2, PR[c].y, ecl_mul2(gr2, PI[c].y)));
+                        if (Prem) { ecl_st_cluster(aP + (uint32_t)(16 * ch), npr); ecl_st_cluster(aP + (uint32_t)(4 * LD + 16 * ch), npi); }
+                        else { ecl_st_local(aP + (uint32_t)(16 * ch), npr); ecl_st_local(aP + (uint32_t)(4 * LD + 16 * ch), npi); }
+                        if (Qrem) { ecl_st_cluster(aQ + (uint32_t)(16 * ch), nqr); ecl_st_cluster(aQ + (uint32_t)(4 * LD + 16 * ch), nqi); }
+                        else { ecl_st_local(aQ + (uint32_t)(16 * ch), nqr); ecl_st_local(aQ + (uint32_t)(4 * LD + 16 * ch), nqi); }
+                    }
+                }
+            }
+            ecl_cluster_sync();
+            b ^= 1;
+        }
+        ++sweep;
+        // "any rotation in this sweep", over both CTAs
+        const int mine = __syncthreads_or(any);
+        if (tid == 0) {
+            const uint32_t fa = ecl_smem(&flg[(sweep & 1) * 2 + rank]);
+            ecl_st_cluster_f32(fa, (float)mine);
+            ecl_st_cluster_f32(ecl_mapa(fa, peer), (float)mine);
+        }
+        ecl_cluster_sync();
+        const bool more = flg[(sweep & 1) * 2] != 0.f || flg[(sweep & 1) * 2 + 1] != 0.f;
+        if (!more) { converged = 1; break; }
+        if (sweep == a.max_sweeps) break;
+    }
+
+    // ---- eigenvalues and 1/|g| of this CTA's columns (8 threads per column), published to both CTAs
+    {
+        const int cl = tid >> 3, rr = tid & 7;                       // local column: (pair cl >> 1, row cl & 1)
+        float nn = 0.f;
+        if (cl < 2 * npl) {
+            const float* cr = buf + ecl_slot(b, cl & 1, cl >> 1, LD);
+            const float* ci = cr + LD;
+            for (int i0 = 4 * rr; i0 < N; i0 += 32) {
+                const float4 x = *reinterpret_cast<const float4*>(&cr[i0]);
+                const float4 y = *reinterpret_cast<const float4*>(&ci[i0]);
+                nn = fmaf(x.x, x.x, fmaf(x.y, x.y, fmaf(x.z, x.z, fmaf(x.w, x.w, nn))));
+                nn = fmaf(y.x, y.x, fmaf(y.y, y.y, fmaf(y.z, y.z, fmaf(y.w, y.w, nn))));
+            }
+        }
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) nn += __shfl_xor_sync(0xffffffffu, nn, o);
+        if (cl < 2 * npl && rr == 0) {
+            const int u = 2 * (p0 + (cl >> 1)) + (cl & 1);
+            const float lamv = shiftv < 0.f ? 0.f : nn - delta;
+            const float invv = nn > 0.f ? rsqrtf(nn) : 0.f;
+            const uint32_t la = ecl_smem(&lam_s[u]), ia = ecl_smem(&inv_s[u]);
+            ecl_st_cluster_f32(la, lamv); ecl_st_cluster_f32(ecl_mapa(la, peer), lamv);
+            ecl_st_cluster_f32(ia, invv); ecl_st_cluster_f32(ecl_mapa(ia, peer), invv);
+        }
+    }
+    ecl_cluster_sync();
+    // ---- rank (descending, ties by slot), cut-off, eigen-weights: both CTAs compute, CTA 0 writes
+    float myl = 0.f;
+    int rnk = 0;
+    if (tid < N) {
+        myl = lam_s[tid];
+        for (int q = 0; q < N; ++q) {
+            const float lq = lam_s[q];
+            rnk += (lq > myl) || (lq == myl && q < tid);
+        }
+        lsort[rnk] = (double)myl;
+        if (rank == 0) {
+            a.lam[(size_t)k * N + rnk] = (double)myl;
+            a.order[(size_t)k * N + rnk] = tid;
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int c = a.k_fixed;
+        if (a.mode == LCF_HARD_ENERGY || a.mode == LCF_SOFT_ENERGY) {
+            double tot = 0.0;
+            for (int i = 0; i < N; ++i) tot += lsort[i] > 0.0 ? lsort[i] : 0.0;
+            double cum = 0.0;
+            c = N;
+            for (int mm = 1; mm <= N; ++mm) {
+                cum += lsort[mm - 1] > 0.0 ? lsort[mm - 1] : 0.0;
+                if (cum > a.energy_frac * tot) { c = mm; break; }
+            }
+        }
+        ish[1] = c;
+        if (rank == 0) { a.cut[k] = c; a.sweeps[k] = sweep; a.conv[k] = converged; }
+    }
+    __syncthreads();
+    {
+        const int c = ish[1];
+        const bool soft = (a.mode == LCF_SOFT_FIXED || a.mode == LCF_SOFT_ENERGY);
+        if (tid < N) {
+            const int i1 = rnk + 1;                                  // 1-based order of the eigenvalue in slot tid
+            double w;
+            if (soft) w = 1.0 / (1.0 + exp(-a.beta * (double)(i1 - c)));
+            else w = (i1 <= c) ? 0.0 : 1.0;
+            wsl[tid] = (float)w;
+            if (rank == 0) {
+                a.wt[(size_t)k * N + rnk] = w;
+                a.wslot[(size_t)k * Ns + tid] = (float)w;
+                a.wslot_dd[(size_t)k * Ns + tid] = w;
+            }
+        }
+    }
+    __syncthreads();
+    // ---- V[row][u] = G[row][u] / |g_u|, B = V diag(wt) for this CTA's slots u in [2 p0, 2 p0 + 2 npl)
+    float2* Vk = a.V + (size_t)k * N * Ns;
+    float2* Bk = a.B + (size_t)k * N * Ns;
+    const int ncl = 2 * npl;
+    for (int e = tid; e < N * ncl; e += ECL_THREADS) {
+        const int row = e / ncl, cl = e - row * ncl;
+        const int u = 2 * p0 + cl;
+        const float* cr = buf + ecl_slot(b, cl & 1, cl >> 1, LD);
+        const float s1 = inv_s[u], w = wsl[u];
+        const float2 v = make_float2(cr[row] * s1, cr[LD + row] * s1);
+        Vk[(size_t)row * Ns + u] = v;
+        Bk[(size_t)row * Ns + u] = make_float2(v.x * w, v.y * w);
+    }
+    ecl_cluster_sync();                                              // no CTA leaves while its shared memory may be addressed
+}
+
+static size_t ecl_smem_bytes(int N, int LD) {
+    return (size_t)2 * 2 * ECL_PL * 2 * LD * 4 + 3 * (size_t)N * 4 + 16 + (size_t)N * 8 + 16 + 64;
+}
+
+bool evd_cluster_eligible(const lcf_plan* p) { return p->prec == 0 && (p->N % 2) == 0 && p->N >= 32 && p->N <= 128; }
+
+cudaError_t configure_evd_cluster(lcf_plan* p) {
+    p->ecl_smem = ecl_smem_bytes(p->N, p->ec_LD);
+    if (p->ecl_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
+    cudaError_t e = cudaSuccess;
+#define ECL_SET(NC, FULL) if (e == cudaSuccess) e = cudaFuncSetAttribute(jacobi_cluster_kernel<NC, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ecl_smem)
+    ECL_SET(1, false); ECL_SET(2, false); ECL_SET(1, true); ECL_SET(2, true);
+#undef ECL_SET
+    return e;
+}
+
+cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st) {
+    EclArgs a;
+    a.N = p->N; a.n = p->N / 2; a.h = (a.n + 1) / 2; a.LD = p->ec_LD; a.LDg = p->ec_LD; a.max_sweeps = 30;
+    a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d;
+    a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
+    a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
+    a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
+    a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta;
+    const int nch = (p->N + 3) / 4, nc = (nch + 15) / 16;
+    const bool full = (p->N % 64) == 0;
+    if (nc == 1) {
+        if (full) jacobi_cluster_kernel<1, true><<<2 * p->K, ECL_THREADS, p->ecl_smem, st>>>(a);
+        else jacobi_cluster_kernel<1, false><<<2 * p->K, ECL_THREADS, p->ecl_smem, st>>>(a);
+    } else {
+        if (full) jacobi_cluster_kernel<2, true><<<2 * p->K, ECL_THREADS, p->ecl_smem, st>>>(a);
+        else jacobi_cluster_kernel<2, false><<<2 * p->K, ECL_THREADS, p->ecl_smem, st>>>(a);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace lcf

@@ -94,9 +94,11 @@ struct lcf_plan {
     alignas(64) unsigned char gtc_tmap[128];  // CUtensorMap of the last iq pointer
     const void* gtc_tmap_iq = nullptr;
     // Cholesky + one-sided Jacobi EVD (precision 0, N <= 128): lcf_evd_chol.cu
-    bool evd_chol = false;
+    bool evd_chol = false, evd_cluster = false;   // cluster: Cholesky kernel, then one-sided Jacobi on 2-CTA clusters
     int ec_LD = 0;
-    size_t ec_smem = 0;
+    size_t ec_smem = 0, ecl_smem = 0;
+    float* ec_gfac_d = nullptr;             // [K][2][Ns][LD] Cholesky factor planes
+    float* ec_shift_d = nullptr;            // [K]
     // tensor-core projection (N <= 128): lcf_project_tc.cu
     bool proj_tc = false;
     int ptc_grid = 0, ptc_nseg = 0, ptc_NB = 0, ptc_Kp = 0;
@@ -162,7 +164,10 @@ cudaError_t configure_gram_tc(lcf_plan* p, std::vector<GtcSeg>& segs, std::vecto
 cudaError_t launch_gram_tc(lcf_plan* p, const float2* iq, cudaStream_t st);
 bool evd_chol_eligible(const lcf_plan* p);
 cudaError_t configure_evd_chol(lcf_plan* p);
-cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st);
+cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only);
+bool evd_cluster_eligible(const lcf_plan* p);
+cudaError_t configure_evd_cluster(lcf_plan* p);
+cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st);
 bool project_tc_eligible(const lcf_plan* p);
 cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::vector<int>& cta_first);
 cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st);

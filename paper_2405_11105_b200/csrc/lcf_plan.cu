@@ -60,6 +60,7 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->V_d); cudaFree(p->B_d); cudaFree(p->pitems_d); cudaFree(p->pfirst_d);
     cudaFree(p->tiles_d); cudaFree(p->tsum_d); cudaFree(p->mean_d); cudaFree(p->alpha_d);
     cudaFree(p->F_d); cudaFree(p->iq_stage_d); cudaFree(p->pd_stage_d);
+    cudaFree(p->ec_gfac_d); cudaFree(p->ec_shift_d);
     cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d);
     cudaFree(p->gtc_segs_d); cudaFree(p->gtc_cta_first_d); cudaFree(p->gtc_seg_first_d); cudaFree(p->gtc_part_d);
     if (p->timer.have)
@@ -183,6 +184,11 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
         cudaGetLastError();
         p->evd_chol = false;
     }
+    p->evd_cluster = p->evd_chol && evd_cluster_eligible(p);
+    if (p->evd_cluster && configure_evd_cluster(p) != cudaSuccess) {
+        cudaGetLastError();
+        p->evd_cluster = false;
+    }
     std::vector<PtcSeg> ptc_segs;
     std::vector<int> ptc_cta_first;
     p->proj_tc = project_tc_eligible(p);
@@ -242,6 +248,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
              dev_upload(&p->gtc_seg_first_d, gtc_seg_first) &&
              dev_alloc(&p->gtc_part_d, (size_t)(p->gtc_nseg ? p->gtc_nseg : 1) * 4 * 128 * 128);
     }
+    if (p->evd_cluster) ok = ok && dev_alloc(&p->ec_gfac_d, K * 2 * Ns * (size_t)p->ec_LD) && dev_alloc(&p->ec_shift_d, K);
     if (p->proj_tc) {
         ok = ok && dev_upload(&p->ptc_segs_d, ptc_segs) && dev_upload(&p->ptc_cta_first_d, ptc_cta_first) &&
              dev_alloc(&p->ptc_bpack_d, K * p->ptc_NB * (size_t)(p->ptc_Kp / 4) * 1024) &&
@@ -297,7 +304,8 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     mark(0);
     if (e == cudaSuccess) run(1, p->gram_tc ? launch_gram_tc(p, iq, st) : launch_gram(p, iq, st));
     mark(1);
-    if (e == cudaSuccess) run(2, p->evd_chol ? launch_evd_chol(p, st) : launch_jacobi(p, st));
+    if (e == cudaSuccess) run(2, p->evd_chol ? launch_evd_chol(p, st, p->evd_cluster) : launch_jacobi(p, st));
+    if (e == cudaSuccess && p->evd_cluster) run(2, launch_evd_cluster(p, st));
     mark(2);
     if (e == cudaSuccess && !p->evd_chol) run(3, launch_vbuild(p, st));
     mark(3);
@@ -472,7 +480,7 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
     w->gram_flops = 8.0 * S * N * (N + 1.0) / 2.0;   // Hermitian half, 8 real flops per complex MAC
     w->proj_flops = 8.0 * S * N * N;                 // dense N x N projector factor
     w->hbm_bytes = 8.0 * N * (double)p->P + 4.0 * (double)p->P;
-    w->launches = 2 + (p->evd_chol ? 1 : 2) + (p->proj_tc ? 3 : 1) + 2;   // gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
+    w->launches = 2 + (p->evd_chol ? (p->evd_cluster ? 2 : 1) : 2) + (p->proj_tc ? 3 : 1) + 2;   // gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
     w->gram_tc = p->gram_tc ? 1 : 0; w->evd_chol = p->evd_chol ? 1 : 0; w->proj_tc = p->proj_tc ? 1 : 0;
     w->gram_tensor_flops = 0.0; w->proj_tensor_flops = 0.0;
     for (int k = 0; k < p->K; ++k) {
