@@ -133,21 +133,29 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     if (maxdiag > 0.f) {
         if (tid < N) { Gr[(size_t)tid * LD + tid] += delta; Gi[(size_t)tid * LD + tid] = 0.f; }
         __syncthreads();
-        // ---- 2. pivoted Cholesky, in place.  Two barriers per step: the next pivot (largest
-        // remaining diagonal entry) is found by the trailing update itself with a packed
-        // (value, index) atomicMax, and the update runs over a compacted list of active columns.
+        // ---- 2. pivoted Cholesky, in place.  Two barriers per step: the trailing update keeps a copy of
+        // the diagonal, every warp searches it for the next pivot, and the update runs over a
+        // compacted list of active columns.
         const int nchc = (N + 3) >> 2;                               // 4-row chunks per column
+        float* dgs = lam_s;                                          // [N] current diagonal of the trailing matrix, -1 once eliminated
         if (tid < N) {
             alist[tid] = tid; apos[tid] = tid;
             const float d = fmaxf(Gr[(size_t)tid * LD + tid], 0.f);
-            atomicMax(&key[0], ((unsigned long long)__float_as_uint(d) << 32) | (unsigned)(N - 1 - tid));
+            dgs[tid] = d;
         }
         __syncthreads();
         for (int j = 0; j < N; ++j) {
-            const unsigned long long kj = key[j & 1];
-            const int pv = N - 1 - (int)(kj & 0xffffffffu);
+            // every warp finds the pivot (largest remaining diagonal entry, ties to the lowest index) itself
+            float best = -1.f; int pv = N;
+            for (int i = lane; i < N; i += 32) { const float d = dgs[i]; if (d > best) { best = d; pv = i; } }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const float ob = __shfl_xor_sync(0xffffffffu, best, o);
+                const int oi = __shfl_xor_sync(0xffffffffu, pv, o);
+                if (ob > best || (ob == best && oi < pv)) { best = ob; pv = oi; }
+            }
             // a non-positive pivot can only come from rounding: clamp (the column is then ~0)
-            const float piv = fmaxf(__uint_as_float((unsigned)(kj >> 32)), 1e-30f * maxdiag + 1e-37f);
+            const float piv = fmaxf(best, 1e-30f * maxdiag + 1e-37f);
             const float dsq = sqrtf(piv), sc = rsqrtf(piv);
             const int na = N - 1 - j;                                // active columns after removing pv
             if (tid < LD) {
@@ -162,7 +170,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
             if (tid == 0) {                                          // drop pv from the active list (swap with last)
                 const int ps = apos[pv], last = alist[na];
                 alist[ps] = last; apos[last] = ps;
-                key[(j + 1) & 1] = 0ull;
+                dgs[pv] = -1.f;                                      // eliminated
             }
             __syncthreads();
             if (tid == 0) act[pv] = 0;
@@ -187,7 +195,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
                 if (chk == (l >> 2)) {                               // this chunk holds the diagonal entry A[l][l]
                     const int w = l & 3;
                     const float d = fmaxf(w == 0 ? xr.x : w == 1 ? xr.y : w == 2 ? xr.z : xr.w, 0.f);
-                    atomicMax(&key[(j + 1) & 1], ((unsigned long long)__float_as_uint(d) << 32) | (unsigned)(N - 1 - l));
+                    dgs[l] = d;
                 }
             }
             __syncthreads();
