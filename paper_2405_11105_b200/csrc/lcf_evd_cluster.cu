@@ -131,8 +131,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
     const int dPj = dPi - (dPi >= h ? h : 0), dQj = dQi - (dQi >= h ? h : 0);
     const int M = 2 * n - 1;
     int b = 0, sweep = 0, converged = 0;
+    bool last = false;
     for (;;) {
-        int any = 0;
+        int any = 0, big = 0;
         for (int s = 0; s < M; ++s) {
             if (j < npl) {
                 const float* pr_ = buf + ecl_slot(b, 0, j, LD); const float* pi_ = pr_ + LD;
@@ -171,6 +172,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                 float cs = 1.f, gr = 0.f, gim = 0.f;
                 if (rot) {
                     any = 1;
+                    if (absa2 > 1e-6f * app * aqq) big = 1;            // |cos(g_p, g_q)| > 1e-3
                     // t only steers the rotation (a slightly off angle costs convergence, not accuracy):
                     // approximate sqrt and reciprocal; c^2 + s^2 = 1 rests on one Newton step on rsqrt
                     const float inv = rsqrtf(absa2);
@@ -217,17 +219,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
             b ^= 1;
         }
         ++sweep;
-        // "any rotation in this sweep", over both CTAs
-        const int mine = __syncthreads_or(any);
+        // Over both CTAs: did this sweep rotate at all, and was any rotated pair still far (cosine
+        // above 1e-3) from orthogonal?  Jacobi converges quadratically at the end: once every cosine
+        // of a sweep is below 1e-3 the next sweep leaves them at ~1e-6, under the tolerance, so that
+        // sweep is the last one and the usual rotation-free confirmation sweep is not run.
+        const int mine = __syncthreads_or(any) + __syncthreads_or(big);
         if (tid == 0) {
             const uint32_t fa = ecl_smem(&flg[(sweep & 1) * 2 + rank]);
             ecl_st_cluster_f32(fa, (float)mine);
             ecl_st_cluster_f32(ecl_mapa(fa, peer), (float)mine);
         }
         ecl_cluster_sync();
-        const bool more = flg[(sweep & 1) * 2] != 0.f || flg[(sweep & 1) * 2 + 1] != 0.f;
-        if (!more) { converged = 1; break; }
+        const float f0 = flg[(sweep & 1) * 2], f1 = flg[(sweep & 1) * 2 + 1];
+        if (last || (f0 == 0.f && f1 == 0.f)) { converged = 1; break; }
         if (sweep == a.max_sweeps) break;
+        if (f0 < 2.f && f1 < 2.f) last = true;
     }
 
     // ---- eigenvalues and 1/|g| of this CTA's columns (8 threads per column), published to both CTAs
