@@ -54,7 +54,7 @@ def parse_args():
 
 def workload_name(cfg) -> str:
     d, f = cfg.data, cfg.filt
-    mode = {0: "hard_fixed", 1: "hard_energy", 2: "soft_fixed", 3: "soft_energy"}[f.mode]
+    mode = {0: "hard_fixed", 1: "hard_energy", 2: "soft_fixed", 3: "soft_energy", 4: "hard_median", 5: "soft_median"}[f.mode]
     return (f"{cfg.name}: IQ {d.Nz}x{d.Nx}x{d.N} complex64, {f.Kz}x{f.Kx} windows sigma={f.sigma_z:g} "
             f"trunc={f.trunc:g}, {mode}, precision={f.precision}")
 
@@ -133,7 +133,7 @@ def oracle_sample(cfg, iq, n_windows: int):
     threads = min(len(ks), os.cpu_count() or 1)
 
     def one(k):
-        return orc.window(iq, gz[k % f.Kz], gx[k // f.Kz], f.mode, f.k_fixed, f.energy_frac, f.beta)["PDk"]
+        return orc.window(iq, gz[k % f.Kz], gx[k // f.Kz], f.mode, f.k_fixed, f.energy_frac, f.beta, f.cut_scale)["PDk"]
 
     t0 = time.perf_counter()
     with ThreadPoolExecutor(max_workers=threads) as ex:           # ctypes releases the GIL

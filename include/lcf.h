@@ -55,7 +55,10 @@ typedef enum {
     LCF_HARD_FIXED = 0,  /* wt_i = 0 for i <= k_fixed, 1 above (i is 1-based)          */
     LCF_HARD_ENERGY = 1, /* hard, c = min{m : sum_{i<=m} max(l_i,0) > energy_frac * sum_i max(l_i,0)}*/
     LCF_SOFT_FIXED = 2,  /* wt_i = 1 / (1 + exp(-beta (i - k_fixed)))  (Eq. 9)     */
-    LCF_SOFT_ENERGY = 3  /* sigmoid centred on the energy-rule c                                     */
+    LCF_SOFT_ENERGY = 3, /* sigmoid centred on the energy-rule c                                     */
+    LCF_HARD_MEDIAN = 4, /* hard, c = #{i : l_i > cut_scale * median(l)}  (method 3, Eq. 7,
+                            PAPER.md:90-96; even count: mean of the two middle eigenvalues)         */
+    LCF_SOFT_MEDIAN = 5  /* sigmoid (Eq. 9) centred on the median-rule c                             */
 } lcf_thresh_mode;
 
 typedef struct {
@@ -63,6 +66,7 @@ typedef struct {
     int k_fixed;        /* 0 <= k_fixed <= N (FIXED modes)                                      */
     double energy_frac; /* in (0, 1) (ENERGY modes)                                             */
     double beta;        /* > 0 (SOFT modes)                                                     */
+    double cut_scale;   /* > 0 (MEDIAN modes): the scaling factor beta of Eq. 7               */
     int precision;      /* 0: fp32 Gram + fp32 EVD.  1: exact-product fp64 Gram + fp64 EVD
                            (single precision can hamper the EVD).  The projection
                            is fp32 in both.                                                     */

@@ -12,6 +12,7 @@
  *   gram           Eq. 12, PAPER.md:149-152 (R = sum_p w_p^2 s_p^H s_p); Eq. 1
  *   jacobi         Eq. 2,  PAPER.md:48-50   (R = V Lambda V^H, eigenvalues sorted descending)
  *   weights        PAPER.md:57-59 (hard: first k components zeroed), Eq. 9 PAPER.md:111-118 (sigmoid)
+ *   cutoff_median  Eq. 7,  PAPER.md:90-96   (method 3: threshold = scale * median eigenvalue)
  *   filter         Eq. 4,  PAPER.md:57-59   (F = V Lambda^ V^H)
  *   project_pd     Eq. 4 + PAPER.md:63      (C^ = C_w F; PD = sum over slow time of |C^|^2)
  *   combine        Eq. 13, PAPER.md:154-156 (PD_final = sum_k alpha_k PD_k, alpha_k = 1/mean(PD_k))
@@ -41,7 +42,8 @@
 #define RE(A, i, j, n) ((A)[2 * ((size_t)(i) * (n) + (j))])
 #define IM(A, i, j, n) ((A)[2 * ((size_t)(i) * (n) + (j)) + 1])
 
-enum { LCFO_HARD_FIXED = 0, LCFO_HARD_ENERGY = 1, LCFO_SOFT_FIXED = 2, LCFO_SOFT_ENERGY = 3 };
+enum { LCFO_HARD_FIXED = 0, LCFO_HARD_ENERGY = 1, LCFO_SOFT_FIXED = 2, LCFO_SOFT_ENERGY = 3,
+       LCFO_HARD_MEDIAN = 4, LCFO_SOFT_MEDIAN = 5 };
 
 int lcf_oracle_num_threads(void) {
 #ifdef _OPENMP
@@ -210,6 +212,19 @@ int lcf_oracle_cutoff_energy(const double *lam, int N, double frac) {
     return N;
 }
 
+/* Method 3, Eq. 7: threshold T = scale * lambda_median; "the eigen components with
+ * eigenvalues larger than this threshold ... can thus be removed": c = #{i : lam_i > T}.
+ * lam is sorted descending.  Median of an even count = mean of the two middle values (MATLAB's
+ * median; the paper does not say -- DESIGN.md "Readings"). */
+int lcf_oracle_cutoff_median(const double *lam, int N, double scale) {
+    double med = (N % 2) ? lam[(N - 1) / 2] : 0.5 * (lam[N / 2 - 1] + lam[N / 2]);
+    double T = scale * med;
+    int c = 0;
+    for (int i = 0; i < N; ++i)
+        if (lam[i] > T) ++c;
+    return c;
+}
+
 /* Eigen weights, 1-based order i (stored at wt[i-1]).
  * hard: wt_i = 0 for i <= c, 1 for i > c.
  * soft (Eq. 9): wt_i = 1 / (1 + exp(-beta (i - c))). */
@@ -272,7 +287,7 @@ void lcf_oracle_project_pd(const float *iq, int N, int Nx, int Nz, const double 
 /* One window k = (kz, kx) end to end.  Any output pointer may be NULL except lam.
  * Returns Jacobi sweeps (or -1).  c_out = number of rejected components. */
 int lcf_oracle_window(const float *iq, int N, int Nx, int Nz, const double *gz, const double *gx,
-                      int mode, int k_fixed, double frac, double beta,
+                      int mode, int k_fixed, double frac, double beta, double cut_scale,
                       double *R_out, double *lam, double *V_out, int *c_out, double *wt_out,
                       double *F_out, double *PDk_out, double *mean_out) {
     size_t nn = (size_t)N * N, P = (size_t)Nx * Nz;
@@ -283,8 +298,10 @@ int lcf_oracle_window(const float *iq, int N, int Nx, int Nz, const double *gz, 
     double *PDk = (double *)malloc(sizeof(double) * P);
     lcf_oracle_gram(iq, N, Nx, Nz, gz, gx, R);
     int sweeps = lcf_oracle_jacobi(R, N, lam, V);
-    int c = (mode == LCFO_HARD_ENERGY || mode == LCFO_SOFT_ENERGY) ? lcf_oracle_cutoff_energy(lam, N, frac) : k_fixed;
-    int soft = (mode == LCFO_SOFT_FIXED || mode == LCFO_SOFT_ENERGY);
+    int c = k_fixed;
+    if (mode == LCFO_HARD_ENERGY || mode == LCFO_SOFT_ENERGY) c = lcf_oracle_cutoff_energy(lam, N, frac);
+    if (mode == LCFO_HARD_MEDIAN || mode == LCFO_SOFT_MEDIAN) c = lcf_oracle_cutoff_median(lam, N, cut_scale);
+    int soft = (mode == LCFO_SOFT_FIXED || mode == LCFO_SOFT_ENERGY || mode == LCFO_SOFT_MEDIAN);
     lcf_oracle_weights(N, soft, c, beta, wt);
     lcf_oracle_filter(V, wt, N, F);
     lcf_oracle_project_pd(iq, N, Nx, Nz, gz, gx, F, PDk);
@@ -321,7 +338,7 @@ void lcf_oracle_combine(const double *PDk_all /* [K][P] */, int K, size_t P, dou
  * Returns 0, or -(k+1) for the first window whose Jacobi iteration did not converge. */
 int lcf_oracle_run(const float *iq, int N, int Nx, int Nz, int Kz, int Kx,
                    double sigma_z, double sigma_x, double trunc,
-                   int mode, int k_fixed, double frac, double beta,
+                   int mode, int k_fixed, double frac, double beta, double cut_scale,
                    double *PD /* [Nx][Nz] */, double *lam_all /* [K][N] */, int *c_all /* [K] */,
                    double *mean_all, double *R_all, double *F_all) {
     int K = Kz * Kx;
@@ -343,7 +360,7 @@ int lcf_oracle_run(const float *iq, int N, int Nx, int Nz, int Kz, int Kx,
         int kz = k % Kz, kx = k / Kz;
         const double *gzk = gz + (size_t)kz * Nz, *gxk = gx + (size_t)kx * Nx;
         double *PDk = (double *)malloc(sizeof(double) * P);
-        status[k] = lcf_oracle_window(iq, N, Nx, Nz, gzk, gxk, mode, k_fixed, frac, beta,
+        status[k] = lcf_oracle_window(iq, N, Nx, Nz, gzk, gxk, mode, k_fixed, frac, beta, cut_scale,
                                       R_all ? R_all + 2 * nn * k : NULL, lam_all + (size_t)N * k, NULL,
                                       c_all + k, NULL, F_all ? F_all + 2 * nn * k : NULL, PDk, means + k);
         int z0 = Nz, z1 = -1, x0 = Nx, x1 = -1;

@@ -18,7 +18,7 @@ _SRC = _HERE / "lcf_oracle.c"
 _LIB = _HERE / "liblcf_oracle.so"
 _lib = None
 
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY = 0, 1, 2, 3
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN = 0, 1, 2, 3, 4, 5
 
 
 def build(force: bool = False) -> Path:
@@ -46,6 +46,8 @@ def _load():
         L.lcf_oracle_jacobi.restype = C.c_int
         L.lcf_oracle_cutoff_energy.argtypes = [dp, C.c_int, C.c_double]
         L.lcf_oracle_cutoff_energy.restype = C.c_int
+        L.lcf_oracle_cutoff_median.argtypes = [dp, C.c_int, C.c_double]
+        L.lcf_oracle_cutoff_median.restype = C.c_int
         L.lcf_oracle_weights.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, dp]
         L.lcf_oracle_weights.restype = None
         L.lcf_oracle_filter.argtypes = [dp, dp, C.c_int, dp]
@@ -53,13 +55,13 @@ def _load():
         L.lcf_oracle_project_pd.argtypes = [fp, C.c_int, C.c_int, C.c_int, dp, dp, dp, dp]
         L.lcf_oracle_project_pd.restype = None
         L.lcf_oracle_window.argtypes = [fp, C.c_int, C.c_int, C.c_int, dp, dp, C.c_int, C.c_int,
-                                        C.c_double, C.c_double, dp, dp, dp, ip, dp, dp, dp, dp]
+                                        C.c_double, C.c_double, C.c_double, dp, dp, dp, ip, dp, dp, dp, dp]
         L.lcf_oracle_window.restype = C.c_int
         L.lcf_oracle_combine.argtypes = [dp, C.c_int, C.c_size_t, dp, dp]
         L.lcf_oracle_combine.restype = None
         L.lcf_oracle_run.argtypes = [fp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
                                      C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
-                                     dp, dp, ip, dp, dp, dp]
+                                     C.c_double, dp, dp, ip, dp, dp, dp]
         L.lcf_oracle_run.restype = C.c_int
         _lib = L
     return _lib
@@ -122,6 +124,11 @@ def cutoff_energy(lam: np.ndarray, frac: float) -> int:
     return int(_load().lcf_oracle_cutoff_energy(_d(lam), lam.shape[0], float(frac)))
 
 
+def cutoff_median(lam: np.ndarray, scale: float) -> int:
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    return int(_load().lcf_oracle_cutoff_median(_d(lam), lam.size, float(scale)))
+
+
 def weights(N: int, soft: bool, c: int, beta: float) -> np.ndarray:
     wt = np.empty(N, dtype=np.float64)
     _load().lcf_oracle_weights(N, int(bool(soft)), int(c), float(beta), _d(wt))
@@ -146,7 +153,7 @@ def project_pd(iq: np.ndarray, gz: np.ndarray, gx: np.ndarray, F: np.ndarray) ->
 
 
 def window(iq: np.ndarray, gz: np.ndarray, gx: np.ndarray, mode: int, k_fixed: int = 0,
-           frac: float = 0.995, beta: float = 0.5) -> dict:
+           frac: float = 0.995, beta: float = 0.5, cut_scale: float = 1.0) -> dict:
     """One window end to end with every intermediate."""
     a, p, N, Nx, Nz = _iq(iq)
     gz = np.ascontiguousarray(gz, dtype=np.float64); gx = np.ascontiguousarray(gx, dtype=np.float64)
@@ -154,7 +161,7 @@ def window(iq: np.ndarray, gz: np.ndarray, gx: np.ndarray, mode: int, k_fixed: i
     F = np.empty((N, N), dtype=np.complex128)
     lam = np.empty(N); wt = np.empty(N); PDk = np.empty((Nx, Nz)); mean = C.c_double(0.0); c = C.c_int(0)
     sweeps = _load().lcf_oracle_window(p, N, Nx, Nz, _d(gz), _d(gx), int(mode), int(k_fixed), float(frac),
-                                       float(beta), _d(R), _d(lam), _d(V), C.byref(c), _d(wt), _d(F),
+                                       float(beta), float(cut_scale), _d(R), _d(lam), _d(V), C.byref(c), _d(wt), _d(F),
                                        _d(PDk), C.byref(mean))
     if sweeps < 0:
         raise RuntimeError("oracle Jacobi did not converge")
@@ -173,7 +180,7 @@ def combine(PDk_all: np.ndarray):
 
 def run(iq: np.ndarray, Kz: int, Kx: int, sigma_z: float, sigma_x: float, trunc: float, mode: int,
         k_fixed: int = 0, frac: float = 0.995, beta: float = 0.5, want_R: bool = False,
-        want_F: bool = False) -> dict:
+        want_F: bool = False, cut_scale: float = 1.0) -> dict:
     """Whole path for one ensemble (OpenMP over windows)."""
     a, p, N, Nx, Nz = _iq(iq)
     K = Kz * Kx
@@ -181,7 +188,7 @@ def run(iq: np.ndarray, Kz: int, Kx: int, sigma_z: float, sigma_x: float, trunc:
     R = np.empty((K, N, N), dtype=np.complex128) if want_R else None
     F = np.empty((K, N, N), dtype=np.complex128) if want_F else None
     rc = _load().lcf_oracle_run(p, N, Nx, Nz, Kz, Kx, float(sigma_z), float(sigma_x), float(trunc), int(mode),
-                                int(k_fixed), float(frac), float(beta), _d(PD), _d(lam),
+                                int(k_fixed), float(frac), float(beta), float(cut_scale), _d(PD), _d(lam),
                                 c.ctypes.data_as(C.POINTER(C.c_int)), _d(mean),
                                 _d(R) if want_R else None, _d(F) if want_F else None)
     if rc != 0:
@@ -192,4 +199,4 @@ def run(iq: np.ndarray, Kz: int, Kx: int, sigma_z: float, sigma_x: float, trunc:
 def run_config(iq: np.ndarray, filt, **kw) -> dict:
     """run() with a synth.FilterSpec-like object (fields Kz, Kx, sigma_z, sigma_x, trunc, mode, ...)."""
     return run(iq, filt.Kz, filt.Kx, filt.sigma_z, filt.sigma_x, filt.trunc, filt.mode, filt.k_fixed,
-               filt.energy_frac, filt.beta, **kw)
+               filt.energy_frac, filt.beta, cut_scale=getattr(filt, "cut_scale", 1.0), **kw)

@@ -22,6 +22,7 @@
 #include <cfloat>
 
 #include "lcf_internal.h"
+#include "lcf_thresh.cuh"
 
 namespace lcf {
 
@@ -54,7 +55,7 @@ struct JacArgs {
     double* wslot_dd;       // [K][Ns]
     double* wt;             // [K][N]
     int mode, k_fixed;
-    double energy_frac, beta;
+    double energy_frac, beta, cut_scale;
 };
 
 template <typename T> __device__ __forceinline__ T eps_of();
@@ -254,17 +255,7 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
     }
     __syncthreads();
     if (tid == 0) {
-        int c = a.k_fixed;
-        if (a.mode == LCF_HARD_ENERGY || a.mode == LCF_SOFT_ENERGY) {
-            double tot = 0.0;
-            for (int i = 0; i < N; ++i) tot += lsort[i] > 0.0 ? lsort[i] : 0.0;
-            double cum = 0.0;
-            c = N;
-            for (int m = 1; m <= N; ++m) {
-                cum += lsort[m - 1] > 0.0 ? lsort[m - 1] : 0.0;
-                if (cum > a.energy_frac * tot) { c = m; break; }
-            }
-        }
+        const int c = thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
         *csh = c;
         a.cut[k] = c;
         a.sweeps[k] = sweep;
@@ -272,13 +263,12 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
     }
     __syncthreads();
     const int c = *csh;
-    const bool soft = (a.mode == LCF_SOFT_FIXED || a.mode == LCF_SOFT_ENERGY);
+    const bool soft = thresh_is_soft(a.mode);
     if (tid < Ns) {   // blockDim.x >= Ns (configure_evd)
         double w = 0.0;
         if (tid < N) {
             const int i1 = rank + 1;  // 1-based order of the eigenvalue held by index tid
-            if (soft) w = 1.0 / (1.0 + exp(-a.beta * (double)(i1 - c)));
-            else w = (i1 <= c) ? 0.0 : 1.0;
+            w = thresh_weight(soft, a.beta, i1, c);
             a.wt[(size_t)k * N + rank] = w;
         }
         a.wslot[(size_t)k * Ns + tid] = (float)w;
@@ -421,7 +411,7 @@ cudaError_t launch_jacobi(lcf_plan* p, cudaStream_t st) {
     a.R = p->R_d; a.rotlog = p->rotlog_d;
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
-    a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta;
+    a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
     if (p->prec == 1) jacobi_kernel<double><<<p->K, p->jac_threads, p->jac_smem, st>>>(a);
     else jacobi_kernel<float><<<p->K, p->jac_threads, p->jac_smem, st>>>(a);
     return cudaGetLastError();

@@ -27,6 +27,7 @@
 #include <cfloat>
 
 #include "lcf_internal.h"
+#include "lcf_thresh.cuh"
 
 namespace lcf {
 
@@ -45,7 +46,7 @@ struct EcArgs {
     float2* V;                    // [K][N][Ns]
     float2* B;                    // [K][N][Ns]
     int mode, k_fixed;
-    double energy_frac, beta;
+    double energy_frac, beta, cut_scale;
     int chol_only;                // 1: stop after the Cholesky factor and write it to gfac / shift (cluster Jacobi follows)
     float* gfac;                  // [K][2][Ns][LD] real plane, imaginary plane of G, column-major
     float* shift;                 // [K] delta, or -1 for an all-zero matrix
@@ -175,6 +176,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
             __syncthreads();
             if (tid == 0) act[pv] = 0;
             // trailing update A[i][l] -= L[i] conj(L[l]) over (active column, 4-row chunk) items
+#pragma unroll 4
             for (int idx = tid; idx < na * nchc; idx += EC_THREADS) {
                 const int ci = idx / nchc, chk = idx - ci * nchc;
                 const int l = alist[ci];
@@ -339,17 +341,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     }
     __syncthreads();
     if (tid == 0) {
-        int c = a.k_fixed;
-        if (a.mode == LCF_HARD_ENERGY || a.mode == LCF_SOFT_ENERGY) {
-            double tot = 0.0;
-            for (int i = 0; i < N; ++i) tot += lsort[i] > 0.0 ? lsort[i] : 0.0;
-            double cum = 0.0;
-            c = N;
-            for (int mm = 1; mm <= N; ++mm) {
-                cum += lsort[mm - 1] > 0.0 ? lsort[mm - 1] : 0.0;
-                if (cum > a.energy_frac * tot) { c = mm; break; }
-            }
-        }
+        const int c = thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
         ish[1] = c;
         a.cut[k] = c;
         a.sweeps[k] = sweep;
@@ -358,13 +350,12 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     __syncthreads();
     {
         const int c = ish[1];
-        const bool soft = (a.mode == LCF_SOFT_FIXED || a.mode == LCF_SOFT_ENERGY);
+        const bool soft = thresh_is_soft(a.mode);
         if (tid < Ns) {
             double w = 0.0;
             if (tid < N) {
                 const int i1 = rank + 1;                             // 1-based order of the eigenvalue in slot tid
-                if (soft) w = 1.0 / (1.0 + exp(-a.beta * (double)(i1 - c)));
-                else w = (i1 <= c) ? 0.0 : 1.0;
+                w = thresh_weight(soft, a.beta, i1, c);
                 a.wt[(size_t)k * N + rank] = w;
             }
             wsl[tid] = (float)w;
@@ -411,7 +402,7 @@ cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only) {
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
-    a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta;
+    a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
     const int nch = (p->N + 3) / 4, nc = (nch + 7) / 8;
     const bool full = (p->N % 32) == 0;
 #define EC_RUN(NC) do { if (full) evd_chol_kernel<NC, true><<<p->K, EC_THREADS, p->ec_smem, st>>>(a); \

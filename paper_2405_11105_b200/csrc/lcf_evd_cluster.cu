@@ -18,6 +18,7 @@
 #include <cfloat>
 
 #include "lcf_internal.h"
+#include "lcf_thresh.cuh"
 
 namespace lcf {
 
@@ -33,7 +34,7 @@ struct EclArgs {
     float* wslot; double* wslot_dd; double* wt;
     float2* V; float2* B;                      // [K][N][N]
     int mode, k_fixed;
-    double energy_frac, beta;
+    double energy_frac, beta, cut_scale;
 };
 
 __device__ __forceinline__ unsigned long long ecl_fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
@@ -279,29 +280,18 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
     }
     __syncthreads();
     if (tid == 0) {
-        int c = a.k_fixed;
-        if (a.mode == LCF_HARD_ENERGY || a.mode == LCF_SOFT_ENERGY) {
-            double tot = 0.0;
-            for (int i = 0; i < N; ++i) tot += lsort[i] > 0.0 ? lsort[i] : 0.0;
-            double cum = 0.0;
-            c = N;
-            for (int mm = 1; mm <= N; ++mm) {
-                cum += lsort[mm - 1] > 0.0 ? lsort[mm - 1] : 0.0;
-                if (cum > a.energy_frac * tot) { c = mm; break; }
-            }
-        }
+        const int c = thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
         ish[1] = c;
         if (rank == 0) { a.cut[k] = c; a.sweeps[k] = sweep; a.conv[k] = converged; }
     }
     __syncthreads();
     {
         const int c = ish[1];
-        const bool soft = (a.mode == LCF_SOFT_FIXED || a.mode == LCF_SOFT_ENERGY);
+        const bool soft = thresh_is_soft(a.mode);
         if (tid < N) {
             const int i1 = rnk + 1;                                  // 1-based order of the eigenvalue in slot tid
             double w;
-            if (soft) w = 1.0 / (1.0 + exp(-a.beta * (double)(i1 - c)));
-            else w = (i1 <= c) ? 0.0 : 1.0;
+            w = thresh_weight(soft, a.beta, i1, c);
             wsl[tid] = (float)w;
             if (rank == 0) {
                 a.wt[(size_t)k * N + rnk] = w;
@@ -350,7 +340,7 @@ cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st) {
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
-    a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta;
+    a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
     const int nch = (p->N + 3) / 4, nc = (nch + 15) / 16;
     const bool full = (p->N % 64) == 0;
     if (nc == 1) {

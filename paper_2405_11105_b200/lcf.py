@@ -14,7 +14,7 @@ import numpy as np
 HERE = Path(__file__).resolve().parent
 LIB_PATH = HERE / "liblcf.so"
 
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY = 0, 1, 2, 3
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN = 0, 1, 2, 3, 4, 5
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_NOT_CONVERGED = range(6)
 
 EXPORTS = [
@@ -32,7 +32,7 @@ class Windows(C.Structure):
 
 class Thresh(C.Structure):
     _fields_ = [("mode", C.c_int), ("k_fixed", C.c_int), ("energy_frac", C.c_double), ("beta", C.c_double),
-                ("precision", C.c_int)]
+                ("cut_scale", C.c_double), ("precision", C.c_int)]
 
 
 class Work(C.Structure):
@@ -122,12 +122,13 @@ class Plan:
     """lcf_plan_create / lcf_filter / lcf_plan_destroy plus the diagnostic getters."""
 
     def __init__(self, Nz: int, Nx: int, N: int, Kz: int, Kx: int, sigma_z: float, sigma_x: float, trunc: float,
-                 mode: int, k_fixed: int = 0, energy_frac: float = 0.995, beta: float = 0.5, precision: int = 0):
+                 mode: int, k_fixed: int = 0, energy_frac: float = 0.995, beta: float = 0.5, precision: int = 0,
+                 cut_scale: float = 1.0):
         L = load()
         self._h = C.c_void_p(None)
         self.Nz, self.Nx, self.N, self.K = int(Nz), int(Nx), int(N), int(Kz) * int(Kx)
         w = Windows(int(Kz), int(Kx), float(sigma_z), float(sigma_x), float(trunc))
-        t = Thresh(int(mode), int(k_fixed), float(energy_frac), float(beta), int(precision))
+        t = Thresh(int(mode), int(k_fixed), float(energy_frac), float(beta), float(cut_scale), int(precision))
         st = L.lcf_plan_create(C.byref(self._h), int(Nz), int(Nx), int(N), C.byref(w), C.byref(t))
         if st != OK:
             self._h = C.c_void_p(None)
@@ -137,7 +138,7 @@ class Plan:
     def from_spec(cls, Nz: int, Nx: int, N: int, filt) -> "Plan":
         """filt: an object with the fields of synth.FilterSpec."""
         return cls(Nz, Nx, N, filt.Kz, filt.Kx, filt.sigma_z, filt.sigma_x, filt.trunc, filt.mode, filt.k_fixed,
-                   filt.energy_frac, filt.beta, filt.precision)
+                   filt.energy_frac, filt.beta, filt.precision, getattr(filt, "cut_scale", 1.0))
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -20,7 +20,7 @@ from typing import Optional
 import numpy as np
 
 # threshold modes (values match include/lcf.h lcf_thresh_mode)
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY = 0, 1, 2, 3
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN = 0, 1, 2, 3, 4, 5
 
 
 @dataclass(frozen=True)
@@ -51,6 +51,7 @@ class FilterSpec:
     energy_frac: float = 0.995
     beta: float = 0.5
     precision: int = 0          # 0 = fp32 Gram+EVD, 1 = fp64 Gram+EVD
+    cut_scale: float = 1.0      # beta of Eq. 7 (MEDIAN modes)
 
 
 @dataclass(frozen=True)

@@ -157,6 +157,9 @@ SMALL = [
     (40, 24, 24, 2, 2, 30.0, 0.0, synth.HARD_FIXED, 2, 0),        # Gaussian, no truncation
     (33, 65, 2, 2, 2, 8.0, 3.0, synth.HARD_FIXED, 1, 1),          # N = 2: one rotation, no blocks
     (96, 80, 140, 2, 2, 20.0, 3.0, synth.HARD_ENERGY, 0, 0),      # N > 128: 3 pivots per lane, 2 Gram batches
+    (64, 48, 64, 2, 2, 14.0, 3.0, synth.SOFT_MEDIAN, 0, 0),       # method 3 (median rule) + sigmoid, cluster EVD path
+    (64, 48, 40, 2, 2, 14.0, 3.0, synth.HARD_MEDIAN, 0, 1),       # hard median cut (fp64: a hard cut 40 dB down needs it)
+    (50, 37, 24, 1, 2, 12.0, 3.0, synth.HARD_MEDIAN, 0, 1),       # median rule in the fp64 path
 ]
 
 
@@ -164,13 +167,19 @@ SMALL = [
 def test_small_shapes_and_modes(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, trunc, mode, k, prec):
     cfg = synth.baseline_configs()[2]
     d = replace(cfg.data, Nz=Nz, Nx=Nx, N=N, n_frames=N, seed=100 + N, n_vessels=3, tissue_db=40.0, noise_db=-55.0)
-    f = synth.FilterSpec(Kz, Kx, sigma, sigma, trunc, mode, k_fixed=k, precision=prec)
+    median = mode in (synth.HARD_MEDIAN, synth.SOFT_MEDIAN)
+    # median rule: a scaling factor that puts the threshold in the gap between tissue and blood / noise
+    f = synth.FilterSpec(Kz, Kx, sigma, sigma, trunc, mode, k_fixed=k, precision=prec, cut_scale=300.0 if median else 1.0)
     iq = synth.generate_sequence(d)
     o = oracle.run_config(iq, f, want_R=True, want_F=True)
+    if median:
+        T = f.cut_scale * np.median(o["lam"], axis=1, keepdims=True)
+        assert (np.abs(o["lam"] - T) > 1e-3 * T).all(), "test spectrum has an eigenvalue on the threshold"
+        assert (o["c"] > 0).all() and (o["c"] < N // 2).all()
     g = gpu_run(lcf, iq, f, want=("lam", "c", "R", "F", "wt"))
     check_spectrum(g, o)
     check_pd(g["PD"], o["PD"])
-    soft = mode in (synth.SOFT_FIXED, synth.SOFT_ENERGY)
+    soft = mode in (synth.SOFT_FIXED, synth.SOFT_ENERGY, synth.SOFT_MEDIAN)
     for kk in range(Kz * Kx):
         wt_o = oracle.weights(N, soft, int(o["c"][kk]), f.beta)
         assert np.allclose(g["wt"][kk], wt_o, rtol=0, atol=1e-12)

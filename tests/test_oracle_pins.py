@@ -183,6 +183,43 @@ def test_energy_cutoff_bruteforce(oracle):
         assert oracle.cutoff_energy(lam, frac) == want
 
 
+def test_median_cutoff_pins(oracle):
+    # method 3 (Eq. 7): T = scale * median eigenvalue, c = # eigenvalues above T
+    lam = np.array([100.0, 40.0, 9.0, 3.0, 2.0, 1.0, 0.5])                         # odd: median = 3
+    assert oracle.cutoff_median(lam, 1.0) == 3                                     # 100, 40, 9 > 3
+    assert oracle.cutoff_median(lam, 3.0) == 2                                     # 9 is not > 9
+    assert oracle.cutoff_median(lam, 2.9) == 3
+    assert oracle.cutoff_median(lam, 50.0) == 0
+    lam = np.array([8.0, 6.0, 4.0, 2.0])                                           # even: median = 5
+    assert oracle.cutoff_median(lam, 1.0) == 2
+    assert oracle.cutoff_median(lam, 1.2) == 1                                     # 6 is not > 6
+    assert oracle.cutoff_median(np.ones(6), 1.0) == 0                              # flat spectrum: nothing above
+    # against numpy's median (same even-count convention as MATLAB) on random descending spectra
+    rng = np.random.default_rng(11)
+    for n in (2, 3, 8, 33, 128):
+        for _ in range(20):
+            lam = np.sort(rng.random(n) ** 6)[::-1]
+            beta = rng.uniform(0.5, 20.0)
+            assert oracle.cutoff_median(lam, beta) == int((lam > beta * np.median(lam)).sum())
+    # the worked value in the paper's Fig. 2a (scaling factor 1.43) belongs to the authors' data:
+    # it cannot be reproduced here; a low-rank-plus-white-noise spectrum stands in:
+    lam = np.concatenate([[1e6, 3e4, 2e3], np.linspace(1.3, 0.7, 47)])
+    assert oracle.cutoff_median(lam, 1.43) == 3
+
+
+def test_median_mode_runs_like_fixed_cut(oracle):
+    # a window whose median rule gives c must equal the fixed-cut result with k_fixed = c
+    iq = synth.random_cube(16, 12, 10, seed=4)
+    gz = oracle.axis_windows(16, 1, 0.0, 0.0)[0]; gx = oracle.axis_windows(12, 1, 0.0, 0.0)[0]
+    a = oracle.window(iq, gz, gx, synth.HARD_MEDIAN, cut_scale=1.5)
+    b = oracle.window(iq, gz, gx, synth.HARD_FIXED, k_fixed=a["c"])
+    assert a["c"] == int((a["lam"] > 1.5 * np.median(a["lam"])).sum())
+    assert np.array_equal(a["wt"], b["wt"]) and np.array_equal(a["PDk"], b["PDk"])
+    s1 = oracle.window(iq, gz, gx, synth.SOFT_MEDIAN, beta=0.7, cut_scale=1.5)
+    s2 = oracle.window(iq, gz, gx, synth.SOFT_FIXED, k_fixed=a["c"], beta=0.7)
+    assert np.array_equal(s1["wt"], s2["wt"])
+
+
 def test_weights_closed_forms(oracle):
     assert np.array_equal(oracle.weights(6, False, 2, 0.5), [0, 0, 1, 1, 1, 1])
     assert np.array_equal(oracle.weights(3, False, 0, 0.5), [1, 1, 1])
