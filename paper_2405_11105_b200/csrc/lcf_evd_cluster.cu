@@ -85,6 +85,94 @@ __device__ __forceinline__ uint32_t ecl_cluster_rank() {
 // column slot (buffer b, row t: 0 top / 1 bottom, local pair j): real plane, then imaginary plane
 __device__ __forceinline__ int ecl_slot(int b, int t, int j, int LD) { return (((b * 2 + t) * ECL_PL + j) * 2) * LD; }
 
+// Shared tail of the cluster kernels: eigenvalues (|g|^2 - delta) and 1/|g| of this CTA's ncl columns
+// (local column cl = global slot u0 + cl, real plane at colptr(cl), imaginary plane LD floats on),
+// published to both CTAs; ranking, cut-off rule, eigen-weights; V_k and B_k = V_k diag(wt).
+template <class ColPtr>
+__device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t rank, uint32_t peer, int u0, int ncl, ColPtr colptr,
+                                             float* lam_s, float* inv_s, float* wsl, double* lsort, int* ish,
+                                             float shiftv, float delta, int sweep, int converged) {
+    const int N = a.N, Ns = a.N, LD = a.LD;
+    const int tid = threadIdx.x;
+    // ---- eigenvalues and 1/|g| of this CTA's columns (8 threads per column), published to both CTAs
+    {
+        const int cl = tid >> 3, rr = tid & 7;                       // local column: (pair cl >> 1, row cl & 1)
+        float nn = 0.f;
+        if (cl < ncl) {
+            const float* cr = colptr(cl);
+            const float* ci = cr + LD;
+            for (int i0 = 4 * rr; i0 < N; i0 += 32) {
+                const float4 x = *reinterpret_cast<const float4*>(&cr[i0]);
+                const float4 y = *reinterpret_cast<const float4*>(&ci[i0]);
+                nn = fmaf(x.x, x.x, fmaf(x.y, x.y, fmaf(x.z, x.z, fmaf(x.w, x.w, nn))));
+                nn = fmaf(y.x, y.x, fmaf(y.y, y.y, fmaf(y.z, y.z, fmaf(y.w, y.w, nn))));
+            }
+        }
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) nn += __shfl_xor_sync(0xffffffffu, nn, o);
+        if (cl < ncl && rr == 0) {
+            const int u = u0 + cl;
+            const float lamv = shiftv < 0.f ? 0.f : nn - delta;
+            const float invv = nn > 0.f ? rsqrtf(nn) : 0.f;
+            const uint32_t la = ecl_smem(&lam_s[u]), ia = ecl_smem(&inv_s[u]);
+            ecl_st_cluster_f32(la, lamv); ecl_st_cluster_f32(ecl_mapa(la, peer), lamv);
+            ecl_st_cluster_f32(ia, invv); ecl_st_cluster_f32(ecl_mapa(ia, peer), invv);
+        }
+    }
+    ecl_cluster_sync();
+    // ---- rank (descending, ties by slot), cut-off, eigen-weights: both CTAs compute, CTA 0 writes
+    float myl = 0.f;
+    int rnk = 0;
+    if (tid < N) {
+        myl = lam_s[tid];
+        for (int q = 0; q < N; ++q) {
+            const float lq = lam_s[q];
+            rnk += (lq > myl) || (lq == myl && q < tid);
+        }
+        lsort[rnk] = (double)myl;
+        if (rank == 0) {
+            a.lam[(size_t)k * N + rnk] = (double)myl;
+            a.order[(size_t)k * N + rnk] = tid;
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        const int c = thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
+        ish[1] = c;
+        if (rank == 0) { a.cut[k] = c; a.sweeps[k] = sweep; a.conv[k] = converged; }
+    }
+    __syncthreads();
+    {
+        const int c = ish[1];
+        const bool soft = thresh_is_soft(a.mode);
+        if (tid < N) {
+            const int i1 = rnk + 1;                                  // 1-based order of the eigenvalue in slot tid
+            double w;
+            w = thresh_weight(soft, a.beta, i1, c);
+            wsl[tid] = (float)w;
+            if (rank == 0) {
+                a.wt[(size_t)k * N + rnk] = w;
+                a.wslot[(size_t)k * Ns + tid] = (float)w;
+                a.wslot_dd[(size_t)k * Ns + tid] = w;
+            }
+        }
+    }
+    __syncthreads();
+    // ---- V[row][u] = G[row][u] / |g_u|, B = V diag(wt) for this CTA's slots u in [u0, u0 + ncl)
+    float2* Vk = a.V + (size_t)k * N * Ns;
+    float2* Bk = a.B + (size_t)k * N * Ns;
+    for (int e = tid; e < N * ncl; e += ECL_THREADS) {
+        const int row = e / ncl, cl = e - row * ncl;
+        const int u = u0 + cl;
+        const float* cr = colptr(cl);
+        const float s1 = inv_s[u], w = wsl[u];
+        const float2 v = make_float2(cr[row] * s1, cr[LD + row] * s1);
+        Vk[(size_t)row * Ns + u] = v;
+        Bk[(size_t)row * Ns + u] = make_float2(v.x * w, v.y * w);
+    }
+    ecl_cluster_sync();                                              // no CTA leaves while its shared memory may be addressed
+}
+
 template <int NC, bool FULL>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jacobi_cluster_kernel(EclArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -237,84 +325,200 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
         if (f0 < 2.f && f1 < 2.f) last = true;
     }
 
-    // ---- eigenvalues and 1/|g| of this CTA's columns (8 threads per column), published to both CTAs
+    ecl_epilogue(a, k, rank, peer, 2 * p0, 2 * npl,
+                 [&](int cl) { return (const float*)(buf + ecl_slot(b, cl & 1, cl >> 1, LD)); },
+                 lam_s, inv_s, wsl, lsort, ish, shiftv, delta, sweep, converged);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Block variant (N % 4 == 0): the systolic array moves BLOCKS of two columns.  One warp owns a block
+// pair (top block A0 A1, bottom block B0 B1; lane r holds rows 4r..4r+3 of the four columns in
+// registers) and per block step rotates the four cross pairs as two rounds of two independent
+// rotations -- (A0,B0)+(A1,B1), then (A0,B1)+(A1,B0) -- and, at the first block step of a sweep, the
+// inner pairs (A0,A1)+(B0,B1).  Every column pair is still met once per sweep, but the columns
+// cross shared memory (and the cluster barrier is paid) once per TWO rotation rounds, the two
+// rotations of a round overlap their latency chains, and the halves of the warp compute one
+// rotation's parameters each instead of all lanes repeating the same one.
+constexpr int ECB_PL = 16;                     // block-pair slots per CTA (N <= 128: 32 block pairs)
+__device__ __forceinline__ int ecb_slot(int b, int t, int j, int cb, int LD) { return ((((b * 2 + t) * ECB_PL + j) * 2 + cb) * 2) * LD; }
+
+struct EcbCol { ulonglong2 re, im; };          // 4 rows of one column: (r0,r1),(r2,r3) real and imaginary
+
+// rotate the pairs (X, Y) and (Z, W) at once; returns bit 0: rotated, bit 1: a rotated pair had cosine > 1e-3
+__device__ __forceinline__ int ecb_round(EcbCol& X, EcbCol& Y, EcbCol& Z, EcbCol& W, int lane, float tol2) {
+    float v1[4], v2[4];
     {
-        const int cl = tid >> 3, rr = tid & 7;                       // local column: (pair cl >> 1, row cl & 1)
-        float nn = 0.f;
-        if (cl < 2 * npl) {
-            const float* cr = buf + ecl_slot(b, cl & 1, cl >> 1, LD);
-            const float* ci = cr + LD;
-            for (int i0 = 4 * rr; i0 < N; i0 += 32) {
-                const float4 x = *reinterpret_cast<const float4*>(&cr[i0]);
-                const float4 y = *reinterpret_cast<const float4*>(&ci[i0]);
-                nn = fmaf(x.x, x.x, fmaf(x.y, x.y, fmaf(x.z, x.z, fmaf(x.w, x.w, nn))));
-                nn = fmaf(y.x, y.x, fmaf(y.y, y.y, fmaf(y.z, y.z, fmaf(y.w, y.w, nn))));
-            }
-        }
+        unsigned long long app2 = ecl_fma2(X.re.x, X.re.x, ecl_fma2(X.im.x, X.im.x, ecl_fma2(X.re.y, X.re.y, ecl_mul2(X.im.y, X.im.y))));
+        unsigned long long aqq2 = ecl_fma2(Y.re.x, Y.re.x, ecl_fma2(Y.im.x, Y.im.x, ecl_fma2(Y.re.y, Y.re.y, ecl_mul2(Y.im.y, Y.im.y))));
+        unsigned long long re2 = ecl_fma2(X.re.x, Y.re.x, ecl_fma2(X.im.x, Y.im.x, ecl_fma2(X.re.y, Y.re.y, ecl_mul2(X.im.y, Y.im.y))));
+        unsigned long long ia2 = ecl_fma2(X.re.x, Y.im.x, ecl_mul2(X.re.y, Y.im.y));
+        unsigned long long ib2 = ecl_fma2(X.im.x, Y.re.x, ecl_mul2(X.im.y, Y.re.y));
+        v1[0] = ecl_hsum(app2); v1[1] = ecl_hsum(aqq2); v1[2] = ecl_hsum(re2); v1[3] = ecl_hsum(ia2) - ecl_hsum(ib2);
+    }
+    {
+        unsigned long long app2 = ecl_fma2(Z.re.x, Z.re.x, ecl_fma2(Z.im.x, Z.im.x, ecl_fma2(Z.re.y, Z.re.y, ecl_mul2(Z.im.y, Z.im.y))));
+        unsigned long long aqq2 = ecl_fma2(W.re.x, W.re.x, ecl_fma2(W.im.x, W.im.x, ecl_fma2(W.re.y, W.re.y, ecl_mul2(W.im.y, W.im.y))));
+        unsigned long long re2 = ecl_fma2(Z.re.x, W.re.x, ecl_fma2(Z.im.x, W.im.x, ecl_fma2(Z.re.y, W.re.y, ecl_mul2(Z.im.y, W.im.y))));
+        unsigned long long ia2 = ecl_fma2(Z.re.x, W.im.x, ecl_mul2(Z.re.y, W.im.y));
+        unsigned long long ib2 = ecl_fma2(Z.im.x, W.re.x, ecl_mul2(Z.im.y, W.re.y));
+        v2[0] = ecl_hsum(app2); v2[1] = ecl_hsum(aqq2); v2[2] = ecl_hsum(re2); v2[3] = ecl_hsum(ia2) - ecl_hsum(ib2);
+    }
+    // lanes 0-15 end up with the sums of (X, Y), lanes 16-31 with those of (Z, W)
+    const bool lo = lane < 16;
+    float v[4];
 #pragma unroll
-        for (int o = 4; o > 0; o >>= 1) nn += __shfl_xor_sync(0xffffffffu, nn, o);
-        if (cl < 2 * npl && rr == 0) {
-            const int u = 2 * (p0 + (cl >> 1)) + (cl & 1);
-            const float lamv = shiftv < 0.f ? 0.f : nn - delta;
-            const float invv = nn > 0.f ? rsqrtf(nn) : 0.f;
-            const uint32_t la = ecl_smem(&lam_s[u]), ia = ecl_smem(&inv_s[u]);
-            ecl_st_cluster_f32(la, lamv); ecl_st_cluster_f32(ecl_mapa(la, peer), lamv);
-            ecl_st_cluster_f32(ia, invv); ecl_st_cluster_f32(ecl_mapa(ia, peer), invv);
-        }
+    for (int i = 0; i < 4; ++i) {
+        const float send = lo ? v2[i] : v1[i];
+        v[i] = (lo ? v1[i] : v2[i]) + __shfl_xor_sync(0xffffffffu, send, 16);
     }
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+    const float app = v[0], aqq = v[1], xr = v[2], xi = v[3];
+    const float absa2 = xr * xr + xi * xi;
+    float cs = 1.f, gr = 0.f, gi = 0.f;
+    int flags = 0;
+    if (absa2 > tol2 * app * aqq && absa2 > 0.f) {
+        flags = 1 | (absa2 > 1e-6f * app * aqq ? 2 : 0);
+        const float inv = rsqrtf(absa2);
+        const float tau = (aqq - app) * (0.5f * inv);
+        const float at = fminf(fabsf(tau), 1e18f);
+        const float w1 = fmaf(at, at, 1.f);
+        const float t = copysignf(__fdividef(1.f, at + w1 * rsqrtf(w1)), tau);
+        const float x1 = fmaf(t, t, 1.f);
+        float c0 = rsqrtf(x1);
+        c0 = c0 * fmaf(-0.5f * x1, c0 * c0, 1.5f);           // one Newton step: c^2 + s^2 = 1 to rounding
+        cs = c0;
+        const float sn = t * cs;
+        gr = sn * xr * inv; gi = sn * xi * inv;
+    }
+    // each half computed one rotation; swap so that every lane has both
+    const float ocs = __shfl_xor_sync(0xffffffffu, cs, 16), ogr = __shfl_xor_sync(0xffffffffu, gr, 16), ogi = __shfl_xor_sync(0xffffffffu, gi, 16);
+    const float c1 = lo ? cs : ocs, r1 = lo ? gr : ogr, i1 = lo ? gi : ogi;     // rotation of (X, Y)
+    const float c2_ = lo ? ocs : cs, r2_ = lo ? ogr : gr, i2_ = lo ? ogi : gi;  // rotation of (Z, W)
+    auto apply = [](EcbCol& P, EcbCol& Q, float c, float gr_, float gi_) {
+        const unsigned long long c2 = ecl_pack(c, c), g2 = ecl_pack(gr_, gr_), h2 = ecl_pack(gi_, gi_);
+        const unsigned long long ng2 = ecl_pack(-gr_, -gr_), nh2 = ecl_pack(-gi_, -gi_);
+        EcbCol np_, nq_;
+        // g_p' = c g_p - conj(g) g_q,   g_q' = g g_p + c g_q
+        np_.re.x = ecl_fma2(nh2, Q.im.x, ecl_fma2(ng2, Q.re.x, ecl_mul2(c2, P.re.x)));
+        np_.re.y = ecl_fma2(nh2, Q.im.y, ecl_fma2(ng2, Q.re.y, ecl_mul2(c2, P.re.y)));
+        np_.im.x = ecl_fma2(h2, Q.re.x, ecl_fma2(ng2, Q.im.x, ecl_mul2(c2, P.im.x)));
+        np_.im.y = ecl_fma2(h2, Q.re.y, ecl_fma2(ng2, Q.im.y, ecl_mul2(c2, P.im.y)));
+        nq_.re.x = ecl_fma2(c2, Q.re.x, ecl_fma2(nh2, P.im.x, ecl_mul2(g2, P.re.x)));
+        nq_.re.y = ecl_fma2(c2, Q.re.y, ecl_fma2(nh2, P.im.y, ecl_mul2(g2, P.re.y)));
+        nq_.im.x = ecl_fma2(c2, Q.im.x, ecl_fma2(h2, P.re.x, ecl_mul2(g2, P.im.x)));
+        nq_.im.y = ecl_fma2(c2, Q.im.y, ecl_fma2(h2, P.re.y, ecl_mul2(g2, P.im.y)));
+        P = np_; Q = nq_;
+    };
+    apply(X, Y, c1, r1, i1);
+    apply(Z, W, c2_, r2_, i2_);
+    return flags;
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jacobi_cluster_block_kernel(EclArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = a.N, LD = a.LD, Ns = N;
+    const int n = N / 4, h = (n + 1) / 2;                            // block pairs; CTA 0 owns [0, h)
+    const int tid = threadIdx.x, lane = tid & 31;
+    const uint32_t rank = ecl_cluster_rank(), peer = rank ^ 1u;
+    const int k = blockIdx.x >> 1;
+    const int p0 = rank ? h : 0, npl = rank ? n - h : h;
+    float* buf = reinterpret_cast<float*>(smem_raw);                 // [2 buffers][2 rows][ECB_PL][2 columns][2 planes][LD]
+    float* lam_s = buf + (size_t)2 * 2 * ECB_PL * 2 * 2 * LD;
+    float* inv_s = lam_s + Ns;
+    float* wsl = inv_s + Ns;
+    float* flg = wsl + Ns;
+    double* lsort = reinterpret_cast<double*>(flg + 4);
+    int* ish = reinterpret_cast<int*>(lsort + Ns);
+    const uint32_t buf_u32 = ecl_smem(buf), buf_peer = ecl_mapa(buf_u32, peer);
+
+    // ---- initial placement: block pair i = columns 4i .. 4i+3 (top block 4i, 4i+1; bottom block 4i+2, 4i+3)
+    const float* gk = a.gfac + (size_t)k * 2 * N * a.LDg;
+    const int nch = N >> 2;                                          // 4-row chunks per column (<= 32)
+    for (int e = tid; e < npl * 4 * 2 * nch; e += ECL_THREADS) {
+        const int ch = e % nch; int q = e / nch;
+        const int pl = q & 1; q >>= 1;
+        const int cb = q & 1; q >>= 1;
+        const int t = q & 1, j = q >> 1;
+        const int col = 4 * (p0 + j) + 2 * t + cb;
+        const float4 v = *reinterpret_cast<const float4*>(gk + ((size_t)pl * N + col) * a.LDg + 4 * ch);
+        *reinterpret_cast<float4*>(buf + ecb_slot(0, t, j, cb, LD) + pl * LD + 4 * ch) = v;
+    }
+    const float shiftv = a.shift[k];
+    const float delta = shiftv < 0.f ? 0.f : shiftv;
     ecl_cluster_sync();
-    // ---- rank (descending, ties by slot), cut-off, eigen-weights: both CTAs compute, CTA 0 writes
-    float myl = 0.f;
-    int rnk = 0;
-    if (tid < N) {
-        myl = lam_s[tid];
-        for (int q = 0; q < N; ++q) {
-            const float lq = lam_s[q];
-            rnk += (lq > myl) || (lq == myl && q < tid);
-        }
-        lsort[rnk] = (double)myl;
-        if (rank == 0) {
-            a.lam[(size_t)k * N + rnk] = (double)myl;
-            a.order[(size_t)k * N + rnk] = tid;
-        }
-    }
-    __syncthreads();
-    if (tid == 0) {
-        const int c = thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
-        ish[1] = c;
-        if (rank == 0) { a.cut[k] = c; a.sweeps[k] = sweep; a.conv[k] = converged; }
-    }
-    __syncthreads();
-    {
-        const int c = ish[1];
-        const bool soft = thresh_is_soft(a.mode);
-        if (tid < N) {
-            const int i1 = rnk + 1;                                  // 1-based order of the eigenvalue in slot tid
-            double w;
-            w = thresh_weight(soft, a.beta, i1, c);
-            wsl[tid] = (float)w;
-            if (rank == 0) {
-                a.wt[(size_t)k * N + rnk] = w;
-                a.wslot[(size_t)k * Ns + tid] = (float)w;
-                a.wslot_dd[(size_t)k * Ns + tid] = w;
+
+    const float tol = 4.f * sqrtf((float)N) * FLT_EPSILON;
+    const float tol2 = tol * tol;
+    const int j = tid >> 5;                                          // local block pair = warp
+    const int gi = p0 + j;
+    const bool rowok = lane < nch;                                   // this lane's 4 rows exist
+    int dPt, dPi, dQt, dQi;                                          // destinations of the top / bottom block (row, block pair)
+    if (gi == 0) { dPt = 0; dPi = 0; dQt = 0; dQi = 1; }
+    else { dQt = 1; dQi = gi - 1; if (gi == n - 1) { dPt = 1; dPi = n - 1; } else { dPt = 0; dPi = gi + 1; } }
+    if (n == 1) { dPt = 0; dPi = 0; dQt = 1; dQi = 0; }
+    const bool Prem = (dPi >= h) != (rank == 1), Qrem = (dQi >= h) != (rank == 1);
+    const int dPj = dPi - (dPi >= h ? h : 0), dQj = dQi - (dQi >= h ? h : 0);
+    const int M = 2 * n - 1;
+    int b = 0, sweep = 0, converged = 0;
+    bool last = false;
+    for (;;) {
+        int fl = 0;
+        for (int s = 0; s < M; ++s) {
+            if (j < npl) {
+                EcbCol A0, A1, B0, B1;
+                const ulonglong2 z2 = make_ulonglong2(0ull, 0ull);
+                A0.re = A0.im = A1.re = A1.im = B0.re = B0.im = B1.re = B1.im = z2;
+                if (rowok) {
+                    const float* t0 = buf + ecb_slot(b, 0, j, 0, LD) + 4 * lane;
+                    const float* b0 = buf + ecb_slot(b, 1, j, 0, LD) + 4 * lane;
+                    A0.re = *reinterpret_cast<const ulonglong2*>(t0);          A0.im = *reinterpret_cast<const ulonglong2*>(t0 + LD);
+                    A1.re = *reinterpret_cast<const ulonglong2*>(t0 + 2 * LD); A1.im = *reinterpret_cast<const ulonglong2*>(t0 + 3 * LD);
+                    B0.re = *reinterpret_cast<const ulonglong2*>(b0);          B0.im = *reinterpret_cast<const ulonglong2*>(b0 + LD);
+                    B1.re = *reinterpret_cast<const ulonglong2*>(b0 + 2 * LD); B1.im = *reinterpret_cast<const ulonglong2*>(b0 + 3 * LD);
+                }
+                if (s == 0) fl |= ecb_round(A0, A1, B0, B1, lane, tol2);     // inner pairs, once per sweep
+                fl |= ecb_round(A0, B0, A1, B1, lane, tol2);
+                fl |= ecb_round(A0, B1, A1, B0, lane, tol2);
+                if (rowok) {
+                    const uint32_t aP = (Prem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dPt, dPj, 0, LD) + 4 * lane) * 4u;
+                    const uint32_t aQ = (Qrem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dQt, dQj, 0, LD) + 4 * lane) * 4u;
+                    const uint32_t L4 = (uint32_t)LD * 4u;
+                    if (Prem) {
+                        ecl_st_cluster(aP, A0.re); ecl_st_cluster(aP + L4, A0.im); ecl_st_cluster(aP + 2 * L4, A1.re); ecl_st_cluster(aP + 3 * L4, A1.im);
+                    } else {
+                        ecl_st_local(aP, A0.re); ecl_st_local(aP + L4, A0.im); ecl_st_local(aP + 2 * L4, A1.re); ecl_st_local(aP + 3 * L4, A1.im);
+                    }
+                    if (Qrem) {
+                        ecl_st_cluster(aQ, B0.re); ecl_st_cluster(aQ + L4, B0.im); ecl_st_cluster(aQ + 2 * L4, B1.re); ecl_st_cluster(aQ + 3 * L4, B1.im);
+                    } else {
+                        ecl_st_local(aQ, B0.re); ecl_st_local(aQ + L4, B0.im); ecl_st_local(aQ + 2 * L4, B1.re); ecl_st_local(aQ + 3 * L4, B1.im);
+                    }
+                }
             }
+            ecl_cluster_sync();
+            b ^= 1;
         }
+        ++sweep;
+        // see jacobi_cluster_kernel: stop without a confirmation sweep once a sweep only made small rotations
+        const int mine = __syncthreads_or(fl & 1) + __syncthreads_or(fl & 2);
+        if (tid == 0) {
+            const uint32_t fa = ecl_smem(&flg[(sweep & 1) * 2 + rank]);
+            ecl_st_cluster_f32(fa, (float)mine);
+            ecl_st_cluster_f32(ecl_mapa(fa, peer), (float)mine);
+        }
+        ecl_cluster_sync();
+        const float f0 = flg[(sweep & 1) * 2], f1 = flg[(sweep & 1) * 2 + 1];
+        if (last || (f0 == 0.f && f1 == 0.f)) { converged = 1; break; }
+        if (sweep == a.max_sweeps) break;
+        if (f0 < 2.f && f1 < 2.f) last = true;
     }
-    __syncthreads();
-    // ---- V[row][u] = G[row][u] / |g_u|, B = V diag(wt) for this CTA's slots u in [2 p0, 2 p0 + 2 npl)
-    float2* Vk = a.V + (size_t)k * N * Ns;
-    float2* Bk = a.B + (size_t)k * N * Ns;
-    const int ncl = 2 * npl;
-    for (int e = tid; e < N * ncl; e += ECL_THREADS) {
-        const int row = e / ncl, cl = e - row * ncl;
-        const int u = 2 * p0 + cl;
-        const float* cr = buf + ecl_slot(b, cl & 1, cl >> 1, LD);
-        const float s1 = inv_s[u], w = wsl[u];
-        const float2 v = make_float2(cr[row] * s1, cr[LD + row] * s1);
-        Vk[(size_t)row * Ns + u] = v;
-        Bk[(size_t)row * Ns + u] = make_float2(v.x * w, v.y * w);
-    }
-    ecl_cluster_sync();                                              // no CTA leaves while its shared memory may be addressed
+
+    ecl_epilogue(a, k, rank, peer, 4 * p0, 4 * npl,
+                 [&](int cl) { return (const float*)(buf + ecb_slot(b, (cl >> 1) & 1, cl >> 2, cl & 1, LD)); },
+                 lam_s, inv_s, wsl, lsort, ish, shiftv, delta, sweep, converged);
 }
 
 static size_t ecl_smem_bytes(int N, int LD) {
@@ -330,6 +534,7 @@ cudaError_t configure_evd_cluster(lcf_plan* p) {
 #define ECL_SET(NC, FULL) if (e == cudaSuccess) e = cudaFuncSetAttribute(jacobi_cluster_kernel<NC, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ecl_smem)
     ECL_SET(1, false); ECL_SET(2, false); ECL_SET(1, true); ECL_SET(2, true);
 #undef ECL_SET
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(jacobi_cluster_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ecl_smem);
     return e;
 }
 
@@ -341,6 +546,10 @@ cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st) {
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
     a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
+    if (p->N % 4 == 0) {
+        jacobi_cluster_block_kernel<<<2 * p->K, ECL_THREADS, p->ecl_smem, st>>>(a);
+        return cudaGetLastError();
+    }
     const int nch = (p->N + 3) / 4, nc = (nch + 15) / 16;
     const bool full = (p->N % 64) == 0;
     if (nc == 1) {
