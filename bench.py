@@ -284,7 +284,7 @@ def run_ours(args, cfg):
     kern = {
         "gram": {"kernel": "gram_tc_kernel" if work["gram_tc"] else "gram_kernel", "flops": work["gram_flops"],
                  "bound": "tensor" if work["gram_tc"] else "alu", "executed_flops": work["gram_tensor_flops"] or None},
-        "evd": {"kernel": "evd_chol_kernel" if work["evd_chol"] else "jacobi_kernel", "flops": evd_flops, "bound": "alu",
+        "evd": {"kernel": "evd_chol_kernel (Cholesky) + jacobi_cluster_*_kernel | evd_chol_kernel" if work["evd_chol"] else "jacobi_kernel + vbuild_kernel", "flops": evd_flops, "bound": "alu",
                 "executed_flops": None},
         "projection": {"kernel": "project_tc_kernel" if work["proj_tc"] else "project_kernel", "flops": work["proj_flops"],
                        "bound": "tensor" if work["proj_tc"] else "alu", "executed_flops": work["proj_tensor_flops"] or None},
