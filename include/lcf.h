@@ -88,6 +88,13 @@ lcf_status lcf_filter(lcf_plan* plan, const void* iq_dev, float* pd_dev, void* s
  * first use (LCF_ERR_ALLOC on failure). */
 lcf_status lcf_filter_host(lcf_plan* plan, const void* iq_host, float* pd_host, void* stream);
 
+/* `count` ensembles from HOST buffers, pipelined: the host->device copy of ensemble i+1 (on a
+ * plan-owned copy stream, two staging buffers) overlaps the kernels of ensemble i on `stream`; each
+ * image is copied back as soon as it is done.  iq_hosts / pd_hosts: HOST arrays of `count` HOST
+ * pointers (pinned memory for the copies to be asynchronous).  Returns after everything has
+ * completed (synchronises both streams).  Results are identical to `count` lcf_filter_host calls. */
+lcf_status lcf_filter_host_batch(lcf_plan* plan, const void* const* iq_hosts, float* const* pd_hosts, int count, void* stream);
+
 /* Frees everything.  lcf_plan_destroy(NULL) is a no-op returning LCF_OK. */
 lcf_status lcf_plan_destroy(lcf_plan* plan);
 

@@ -133,6 +133,11 @@ struct lcf_plan {
     // host staging for lcf_filter_host
     void* iq_stage_d = nullptr;
     float* pd_stage_d = nullptr;
+    // second staging set, copy stream and events of lcf_filter_host_batch
+    void* iq_stage2_d = nullptr;
+    float* pd_stage2_d = nullptr;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
 
     cudaStream_t last_stream = nullptr;
     bool ran = false;

@@ -61,6 +61,9 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->V_d); cudaFree(p->B_d); cudaFree(p->pitems_d); cudaFree(p->pfirst_d);
     cudaFree(p->tiles_d); cudaFree(p->tsum_d); cudaFree(p->mean_d); cudaFree(p->alpha_d);
     cudaFree(p->F_d); cudaFree(p->iq_stage_d); cudaFree(p->pd_stage_d);
+    cudaFree(p->iq_stage2_d); cudaFree(p->pd_stage2_d);
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    for (int i = 0; i < 2; ++i) { if (p->ev_copied[i]) cudaEventDestroy(p->ev_copied[i]); if (p->ev_done[i]) cudaEventDestroy(p->ev_done[i]); }
     cudaFree(p->ec_gfac_d); cudaFree(p->ec_shift_d);
     cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d);
     cudaFree(p->gtc_segs_d); cudaFree(p->gtc_cta_first_d); cudaFree(p->gtc_seg_first_d); cudaFree(p->gtc_part_d);
@@ -356,6 +359,45 @@ extern "C" lcf_status lcf_filter_host(lcf_plan* p, const void* iq_host, float* p
 }
 
 extern "C" const char* lcf_last_error(const lcf_plan* p) { return p ? p->last_error : "null plan"; }
+
+extern "C" lcf_status lcf_filter_host_batch(lcf_plan* p, const void* const* iq_hosts, float* const* pd_hosts, int count, void* stream) {
+    if (!p || !iq_hosts || !pd_hosts || count < 0) return LCF_ERR_INVALID_ARG;
+    for (int i = 0; i < count; ++i)
+        if (!iq_hosts[i] || !pd_hosts[i]) return LCF_ERR_INVALID_ARG;
+    if (p->cuda_failed) return LCF_ERR_CUDA;
+    if (count == 0) return LCF_OK;
+    const size_t iq_bytes = (size_t)p->N * p->P * sizeof(float2), pd_bytes = (size_t)p->P * sizeof(float);
+    // staging buffers, copy stream and events are created on first use
+    void** iqs[2] = {&p->iq_stage_d, &p->iq_stage2_d};
+    float** pds[2] = {&p->pd_stage_d, &p->pd_stage2_d};
+    for (int b = 0; b < 2; ++b) {
+        if (!*iqs[b] && cudaMalloc(iqs[b], iq_bytes) != cudaSuccess) { cudaGetLastError(); *iqs[b] = nullptr; return LCF_ERR_ALLOC; }
+        if (!*pds[b] && cudaMalloc(reinterpret_cast<void**>(pds[b]), pd_bytes) != cudaSuccess) { cudaGetLastError(); *pds[b] = nullptr; return LCF_ERR_ALLOC; }
+        if (!p->ev_copied[b] && cudaEventCreateWithFlags(&p->ev_copied[b], cudaEventDisableTiming) != cudaSuccess) return LCF_ERR_CUDA;
+        if (!p->ev_done[b] && cudaEventCreateWithFlags(&p->ev_done[b], cudaEventDisableTiming) != cudaSuccess) return LCF_ERR_CUDA;
+    }
+    if (!p->copy_stream && cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return LCF_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream), cs = p->copy_stream;
+    cudaError_t e = cudaSuccess;
+    lcf_status ls = LCF_OK;
+    for (int i = 0; i < count && e == cudaSuccess && ls == LCF_OK; ++i) {
+        const int b = i & 1;
+        // the staging buffer is free once the kernels of ensemble i-2 have read it
+        if (i >= 2) e = cudaStreamWaitEvent(cs, p->ev_done[b], 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(*iqs[b], iq_hosts[i], iq_bytes, cudaMemcpyHostToDevice, cs);
+        if (e == cudaSuccess) e = cudaEventRecord(p->ev_copied[b], cs);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, p->ev_copied[b], 0);
+        if (e != cudaSuccess) break;
+        ls = lcf_filter(p, *iqs[b], *pds[b], stream);
+        if (ls != LCF_OK) break;
+        e = cudaEventRecord(p->ev_done[b], st);          // input consumed (and image ready)
+        if (e == cudaSuccess) e = cudaMemcpyAsync(pd_hosts[i], *pds[b], pd_bytes, cudaMemcpyDeviceToHost, st);
+    }
+    cudaError_t e2 = cudaStreamSynchronize(cs), e3 = cudaStreamSynchronize(st);
+    if (ls != LCF_OK) return ls;
+    if (e != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) { p->cuda_failed = true; return LCF_ERR_CUDA; }
+    return LCF_OK;
+}
 
 extern "C" int lcf_num_windows(const lcf_plan* p) { return p ? p->K : 0; }
 

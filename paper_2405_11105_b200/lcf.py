@@ -18,7 +18,7 @@ HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN = 0, 
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_NOT_CONVERGED = range(6)
 
 EXPORTS = [
-    "lcf_plan_create", "lcf_filter", "lcf_filter_host", "lcf_plan_destroy", "lcf_num_windows",
+    "lcf_plan_create", "lcf_filter", "lcf_filter_host", "lcf_filter_host_batch", "lcf_plan_destroy", "lcf_num_windows",
     "lcf_get_eigenvalues", "lcf_get_cutoffs", "lcf_get_sweeps", "lcf_get_gram", "lcf_get_eigenvectors",
     "lcf_get_weights", "lcf_get_filters", "lcf_get_window_means", "lcf_set_timing", "lcf_get_stage_ms",
     "lcf_get_work", "lcf_measure_peak", "lcf_status_string", "lcf_last_error",
@@ -62,6 +62,7 @@ def load() -> C.CDLL:
         L.lcf_plan_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.POINTER(Windows), C.POINTER(Thresh)]
         L.lcf_filter.argtypes = [vp, vp, vp, vp]
         L.lcf_filter_host.argtypes = [vp, vp, vp, vp]
+        L.lcf_filter_host_batch.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp]
         L.lcf_plan_destroy.argtypes = [vp]
         L.lcf_num_windows.argtypes = [vp]
         for name in ("lcf_get_eigenvalues", "lcf_get_gram", "lcf_get_eigenvectors", "lcf_get_weights",
@@ -169,6 +170,17 @@ class Plan:
         st = load().lcf_filter_host(self._h, _ptr(iq_host), _ptr(pd_host), _stream(stream))
         if st != OK:
             raise LcfError(st, "lcf_filter_host")
+
+    def filter_host_batch(self, iq_hosts, pd_hosts, stream=None):
+        """Lists of host buffers (pinned): pipelined copies and kernels; returns when all are done."""
+        n = len(iq_hosts)
+        if len(pd_hosts) != n:
+            raise ValueError("iq_hosts and pd_hosts differ in length")
+        ia = (C.c_void_p * n)(*[_ptr(x) for x in iq_hosts])
+        pa = (C.c_void_p * n)(*[_ptr(x) for x in pd_hosts])
+        st = load().lcf_filter_host_batch(self._h, ia, pa, n, _stream(stream))
+        if st != OK:
+            raise LcfError(st, "lcf_filter_host_batch [" + load().lcf_last_error(self._h).decode() + "]")
 
     # ---- diagnostics ----
     def _get_d(self, fn, shape, allow_unconverged=False):

@@ -250,6 +250,25 @@ def test_deterministic_and_stream_and_host_path(lcf):
         assert torch.equal(pinned_out, a.cpu())
 
 
+def test_host_batch_matches_single_calls(lcf):
+    import torch
+    cfg = synth.baseline_configs()[0]
+    d = cfg.data
+    filt = replace(cfg.filt, precision=0, mode=synth.SOFT_ENERGY)
+    iqs = [torch.from_numpy(synth.random_cube(d.Nz, d.Nx, d.N, seed=20 + i)).pin_memory() for i in range(5)]
+    with lcf.Plan.from_spec(d.Nz, d.Nx, d.N, filt) as plan:
+        single = []
+        for iq in iqs:
+            pd = torch.empty((d.Nx, d.Nz), dtype=torch.float32).pin_memory()
+            plan.filter_host(iq, pd)
+            single.append(pd.clone())
+        outs = [torch.full((d.Nx, d.Nz), float("nan"), dtype=torch.float32).pin_memory() for _ in iqs]
+        plan.filter_host_batch(iqs, outs, torch.cuda.current_stream())
+        for a_, b_ in zip(single, outs):
+            assert torch.equal(a_, b_)                      # same kernels, same order: bit-identical
+        plan.filter_host_batch([], [])                      # empty batch is a no-op
+
+
 def test_unsupported_and_limits(lcf):
     # N = 300 needs a 300 x 300 complex triangle (> 227 KB): refused at create, not at filter
     with pytest.raises(lcf.LcfError) as ei:
