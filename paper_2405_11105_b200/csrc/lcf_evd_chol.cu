@@ -15,13 +15,15 @@
 //      rotation J of columns (p, q) chosen from the 2x2 Gram [[|g_p|^2, g_p^H g_q], [., |g_q|^2]]
 //      makes them orthogonal; G <- G J.  At convergence G W = U Sigma, so R' = U Sigma^2 U^H: the
 //      normalised columns ARE the eigenvectors (no separate accumulation of V) and
-//      lambda_u = |g_u|^2 - delta.  After the pivoted Cholesky G^H G is strongly diagonally
-//      dominant for the graded spectra of clutter-dominated windows (Veselic/Hari, Drmac), so 3-5
-//      sweeps replace the 9-10 of two-sided Jacobi on R, and each sweep touches one matrix, not two.
+//      lambda_u = |g_u|^2 - delta.  The singular values of G span only the square root of the
+//      eigenvalue range, so the small (blood / noise) eigen-directions keep the relative accuracy
+//      that makes Jacobi the right fp32 solver here (a tridiagonal QR in fp32 would lose them
+//      under the 50-60 dB of clutter).  Measured: 8-10 sweeps, as many as two-sided Jacobi on R
+//      needs -- the flat noise floor, not the graded clutter part, sets the sweep count -- but each
+//      sweep touches one matrix instead of two (no V accumulation) with unit-stride columns.
 //      8 threads own one column pair per step: 3 dot products reduced by shuffles, one rotation,
-//      one barrier per step.  Like two-sided Jacobi this resolves the small (blood / noise)
-//      eigen-directions to high relative accuracy: the singular values of G span only the square
-//      root of the eigenvalue range.
+//      one barrier per step.  (With even N >= 32 only steps 1-2 run here, `chol_only`, and the
+//      sweeps run on 2-CTA clusters: lcf_evd_cluster.cu.)
 //   4. Rank the eigenvalues (descending), cut-off rule, eigen-weights, then write V_k and
 //      B_k = V_k diag(wt) straight from shared memory.
 #include <cfloat>
@@ -105,7 +107,6 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     int* ish = act + Ns;                                             // [4] pivot, cut-off
     int* alist = ish + 4;                                            // [Ns] compacted active columns
     int* apos = alist + Ns;                                          // [Ns] position of a column in alist
-    unsigned long long* key = reinterpret_cast<unsigned long long*>(apos + Ns);   // [2] packed (pivot value, index)
 
     // ---- load R (row-major [i][j]) into the column-major planes; zero the padding
     const float2* Rk = a.R + (size_t)k * N * N;
@@ -118,7 +119,6 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         Gi[(size_t)j * LD + i] = x.y;
     }
     if (tid < Ns) act[tid] = tid < N ? 1 : 0;
-    if (tid < 2) key[tid] = 0ull;
     __syncthreads();
     float md = 0.f;
     if (tid < N) md = Gr[(size_t)tid * LD + tid];

@@ -12,7 +12,9 @@
 // rotated column is written straight into its destination slot of the other buffer (double
 // buffering), which for the two columns that cross the CTA boundary is a DSMEM store into the peer
 // CTA's shared memory.  One cluster barrier per step covers both the local and the remote hazard.
-// 16 threads own a pair (8 rows each, real and imaginary planes apart, packed f32x2 math).
+// jacobi_cluster_kernel: 16 threads own a pair (8 rows each, real and imaginary planes apart, packed
+// f32x2 math), any even N.  jacobi_cluster_block_kernel (N % 4 == 0, the one config 2 and 4 use): the
+// array moves blocks of two columns, see below.
 // Epilogue as in lcf_evd_chol.cu: lambda = |g|^2 - delta, ranking, cut-off rule, eigen-weights,
 // V_k = normalised columns, B_k = V_k diag(wt).
 #include <cfloat>
