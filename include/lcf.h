@@ -58,7 +58,11 @@ typedef enum {
     LCF_SOFT_ENERGY = 3, /* sigmoid centred on the energy-rule c                                     */
     LCF_HARD_MEDIAN = 4, /* hard, c = #{i : l_i > cut_scale * median(l)}  (method 3, Eq. 7,
                             PAPER.md:90-96; even count: mean of the two middle eigenvalues)         */
-    LCF_SOFT_MEDIAN = 5  /* sigmoid (Eq. 9) centred on the median-rule c                             */
+    LCF_SOFT_MEDIAN = 5, /* sigmoid (Eq. 9) centred on the median-rule c                             */
+    LCF_HARD_CURVATURE = 6, /* hard, c = index of the maximum curvature of the normalised log-eigenvalue
+                            curve cut_scale * N * log10(l_n) / log10(l_1)  (method 1, Eq. 6,
+                            PAPER.md:77-83; finite differences as in DESIGN.md "Readings")          */
+    LCF_SOFT_CURVATURE = 7  /* sigmoid (Eq. 9) centred on the curvature-rule c                       */
 } lcf_thresh_mode;
 
 typedef struct {
@@ -66,7 +70,7 @@ typedef struct {
     int k_fixed;        /* 0 <= k_fixed <= N (FIXED modes)                                      */
     double energy_frac; /* in (0, 1) (ENERGY modes)                                             */
     double beta;        /* > 0 (SOFT modes)                                                     */
-    double cut_scale;   /* > 0 (MEDIAN modes): the scaling factor beta of Eq. 7               */
+    double cut_scale;   /* > 0 (MEDIAN, CURVATURE modes): the scaling factor beta of Eq. 7 / Eq. 6 */
     int precision;      /* 0: fp32 Gram + fp32 EVD.  1: exact-product fp64 Gram + fp64 EVD
                            (single precision can hamper the EVD).  The projection
                            is fp32 in both.                                                     */

@@ -13,6 +13,7 @@
  *   jacobi         Eq. 2,  PAPER.md:48-50   (R = V Lambda V^H, eigenvalues sorted descending)
  *   weights        PAPER.md:57-59 (hard: first k components zeroed), Eq. 9 PAPER.md:111-118 (sigmoid)
  *   cutoff_median  Eq. 7,  PAPER.md:90-96   (method 3: threshold = scale * median eigenvalue)
+ *   cutoff_curvature Eq. 6, PAPER.md:77-83  (method 1: maximum curvature of the log-eigenvalue curve)
  *   filter         Eq. 4,  PAPER.md:57-59   (F = V Lambda^ V^H)
  *   project_pd     Eq. 4 + PAPER.md:63      (C^ = C_w F; PD = sum over slow time of |C^|^2)
  *   combine        Eq. 13, PAPER.md:154-156 (PD_final = sum_k alpha_k PD_k, alpha_k = 1/mean(PD_k))
@@ -43,7 +44,7 @@
 #define IM(A, i, j, n) ((A)[2 * ((size_t)(i) * (n) + (j)) + 1])
 
 enum { LCFO_HARD_FIXED = 0, LCFO_HARD_ENERGY = 1, LCFO_SOFT_FIXED = 2, LCFO_SOFT_ENERGY = 3,
-       LCFO_HARD_MEDIAN = 4, LCFO_SOFT_MEDIAN = 5 };
+       LCFO_HARD_MEDIAN = 4, LCFO_SOFT_MEDIAN = 5, LCFO_HARD_CURVATURE = 6, LCFO_SOFT_CURVATURE = 7 };
 
 int lcf_oracle_num_threads(void) {
 #ifdef _OPENMP
@@ -225,6 +226,35 @@ int lcf_oracle_cutoff_median(const double *lam, int N, double scale) {
     return c;
 }
 
+/* Method 1, Eq. 6: "considering the eigenvalue as a function of eigenvalue order n
+ * in logarithmic scale, y(n) = log10 lambda_n ... the curve is normalized as beta y(n)/y(1) Nt before
+ * computing the curvature" K = |y''| / (1 + y'^2)^(3/2); "the maximum curvature gives the estimate of
+ * threshold cutoff (denoted as k), which is used as the number of eigen components to be rejected".
+ * Not in the paper: derivatives are central differences
+ * y'(n) = (y(n+1) - y(n-1))/2, y''(n) = y(n+1) - 2 y(n) + y(n-1) on n = 2..N-1; eigenvalues are
+ * floored at 1e-12 lambda_1 so that the logarithm exists; the lowest n wins a tie; N < 3,
+ * lambda_1 <= 0 or log10 lambda_1 = 0 (normalisation undefined) give k = 0. */
+int lcf_oracle_cutoff_curvature(const double *lam, int N, double scale) {
+    if (N < 3 || !(lam[0] > 0.0)) return 0;
+    double y1 = log10(lam[0]);
+    if (y1 == 0.0) return 0;
+    double *y = (double *)malloc(sizeof(double) * (size_t)N);
+    for (int n = 0; n < N; ++n) {
+        double l = lam[n] > 1e-12 * lam[0] ? lam[n] : 1e-12 * lam[0];
+        y[n] = scale * (log10(l) / y1) * (double)N;
+    }
+    int k = 0;
+    double best = -1.0;
+    for (int n = 2; n <= N - 1; ++n) { /* 1-based order n, y[n-1] */
+        double d1 = (y[n] - y[n - 2]) / 2.0;
+        double d2 = y[n] - 2.0 * y[n - 1] + y[n - 2];
+        double kap = fabs(d2) / pow(1.0 + d1 * d1, 1.5);
+        if (kap > best) { best = kap; k = n; }
+    }
+    free(y);
+    return k;
+}
+
 /* Eigen weights, 1-based order i (stored at wt[i-1]).
  * hard: wt_i = 0 for i <= c, 1 for i > c.
  * soft (Eq. 9): wt_i = 1 / (1 + exp(-beta (i - c))). */
@@ -301,7 +331,8 @@ int lcf_oracle_window(const float *iq, int N, int Nx, int Nz, const double *gz, 
     int c = k_fixed;
     if (mode == LCFO_HARD_ENERGY || mode == LCFO_SOFT_ENERGY) c = lcf_oracle_cutoff_energy(lam, N, frac);
     if (mode == LCFO_HARD_MEDIAN || mode == LCFO_SOFT_MEDIAN) c = lcf_oracle_cutoff_median(lam, N, cut_scale);
-    int soft = (mode == LCFO_SOFT_FIXED || mode == LCFO_SOFT_ENERGY || mode == LCFO_SOFT_MEDIAN);
+    if (mode == LCFO_HARD_CURVATURE || mode == LCFO_SOFT_CURVATURE) c = lcf_oracle_cutoff_curvature(lam, N, cut_scale);
+    int soft = (mode == LCFO_SOFT_FIXED || mode == LCFO_SOFT_ENERGY || mode == LCFO_SOFT_MEDIAN || mode == LCFO_SOFT_CURVATURE);
     lcf_oracle_weights(N, soft, c, beta, wt);
     lcf_oracle_filter(V, wt, N, F);
     lcf_oracle_project_pd(iq, N, Nx, Nz, gz, gx, F, PDk);

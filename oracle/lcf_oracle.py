@@ -18,7 +18,7 @@ _SRC = _HERE / "lcf_oracle.c"
 _LIB = _HERE / "liblcf_oracle.so"
 _lib = None
 
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN = 0, 1, 2, 3, 4, 5
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE = range(8)
 
 
 def build(force: bool = False) -> Path:
@@ -48,6 +48,8 @@ def _load():
         L.lcf_oracle_cutoff_energy.restype = C.c_int
         L.lcf_oracle_cutoff_median.argtypes = [dp, C.c_int, C.c_double]
         L.lcf_oracle_cutoff_median.restype = C.c_int
+        L.lcf_oracle_cutoff_curvature.argtypes = [dp, C.c_int, C.c_double]
+        L.lcf_oracle_cutoff_curvature.restype = C.c_int
         L.lcf_oracle_weights.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, dp]
         L.lcf_oracle_weights.restype = None
         L.lcf_oracle_filter.argtypes = [dp, dp, C.c_int, dp]
@@ -127,6 +129,11 @@ def cutoff_energy(lam: np.ndarray, frac: float) -> int:
 def cutoff_median(lam: np.ndarray, scale: float) -> int:
     lam = np.ascontiguousarray(lam, dtype=np.float64)
     return int(_load().lcf_oracle_cutoff_median(_d(lam), lam.size, float(scale)))
+
+
+def cutoff_curvature(lam: np.ndarray, scale: float) -> int:
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    return int(_load().lcf_oracle_cutoff_curvature(_d(lam), lam.size, float(scale)))
 
 
 def weights(N: int, soft: bool, c: int, beta: float) -> np.ndarray:

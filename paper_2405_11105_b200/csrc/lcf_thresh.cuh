@@ -3,6 +3,10 @@
 //   energy     c = min{m : sum_{i<=m} max(l_i,0) > frac * sum_i max(l_i,0)}    BASELINE.json configs 2-4
 //   median     c = #{i : l_i > cut_scale * median(l)}       method 3, Eq. 7
 //              (median of an even count = mean of the two middle values, as MATLAB's median)
+//   curvature  c = argmax_n K(n), K = |y''| / (1 + y'^2)^(3/2) of the normalised log-eigenvalue curve
+//              y(n) = cut_scale * N * log10(l_n) / log10(l_1)         method 1, Eq. 6
+//              (central differences on n = 2..N-1, eigenvalues floored at 1e-12 l_1, lowest n on ties:
+//              DESIGN.md "Readings")
 //   hard       wt_i = 0 for i <= c, 1 above
 //   soft       wt_i = 1 / (1 + exp(-beta (i - c)))          method 5, Eq. 9
 // i is the 1-based order of the eigenvalue (descending).  Everything in double on the sorted
@@ -13,7 +17,7 @@
 namespace lcf {
 
 __host__ __device__ inline bool thresh_is_soft(int mode) {
-    return mode == LCF_SOFT_FIXED || mode == LCF_SOFT_ENERGY || mode == LCF_SOFT_MEDIAN;
+    return mode == LCF_SOFT_FIXED || mode == LCF_SOFT_ENERGY || mode == LCF_SOFT_MEDIAN || mode == LCF_SOFT_CURVATURE;
 }
 
 __device__ inline int thresh_cutoff(int mode, int k_fixed, double energy_frac, double cut_scale, const double* lsort, int N) {
@@ -32,6 +36,25 @@ __device__ inline int thresh_cutoff(int mode, int k_fixed, double energy_frac, d
         const double T = cut_scale * med;
         int c = 0;
         while (c < N && lsort[c] > T) ++c;      // sorted descending
+        return c;
+    }
+    if (mode == LCF_HARD_CURVATURE || mode == LCF_SOFT_CURVATURE) {
+        if (N < 3 || !(lsort[0] > 0.0)) return 0;
+        const double y1 = log10(lsort[0]);
+        if (y1 == 0.0) return 0;
+        const double sc = cut_scale * (double)N / y1, fl = 1e-12 * lsort[0];
+        double ym = sc * y1;                                              // y(n-1)
+        double y0 = sc * log10(lsort[1] > fl ? lsort[1] : fl);            // y(n)
+        double best = -1.0;
+        int c = 0;
+        for (int n = 2; n <= N - 1; ++n) {                                // 1-based n
+            const double yp = sc * log10(lsort[n] > fl ? lsort[n] : fl);  // y(n+1)
+            const double d1 = 0.5 * (yp - ym), d2 = yp - 2.0 * y0 + ym;
+            const double q = 1.0 + d1 * d1;
+            const double kap = fabs(d2) / (q * sqrt(q));
+            if (kap > best) { best = kap; c = n; }
+            ym = y0; y0 = yp;
+        }
         return c;
     }
     return k_fixed;

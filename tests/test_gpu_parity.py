@@ -160,6 +160,8 @@ SMALL = [
     (64, 48, 64, 2, 2, 14.0, 3.0, synth.SOFT_MEDIAN, 0, 0),       # method 3 (median rule) + sigmoid, cluster EVD path
     (64, 48, 40, 2, 2, 14.0, 3.0, synth.HARD_MEDIAN, 0, 1),       # hard median cut (fp64: a hard cut 40 dB down needs it)
     (50, 37, 24, 1, 2, 12.0, 3.0, synth.HARD_MEDIAN, 0, 1),       # median rule in the fp64 path
+    (64, 48, 64, 2, 2, 14.0, 3.0, synth.SOFT_CURVATURE, 0, 1),    # method 1 (maximum curvature) + sigmoid: the knee cut needs fp64
+    (50, 37, 32, 1, 2, 12.0, 3.0, synth.HARD_CURVATURE, 0, 1),    # hard curvature cut, fp64 path
 ]
 
 
@@ -168,6 +170,7 @@ def test_small_shapes_and_modes(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, trunc, mo
     cfg = synth.baseline_configs()[2]
     d = replace(cfg.data, Nz=Nz, Nx=Nx, N=N, n_frames=N, seed=100 + N, n_vessels=3, tissue_db=40.0, noise_db=-55.0)
     median = mode in (synth.HARD_MEDIAN, synth.SOFT_MEDIAN)
+    curv = mode in (synth.HARD_CURVATURE, synth.SOFT_CURVATURE)
     # median rule: a scaling factor that puts the threshold in the gap between tissue and blood / noise
     f = synth.FilterSpec(Kz, Kx, sigma, sigma, trunc, mode, k_fixed=k, precision=prec, cut_scale=300.0 if median else 1.0)
     iq = synth.generate_sequence(d)
@@ -179,7 +182,9 @@ def test_small_shapes_and_modes(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, trunc, mo
     g = gpu_run(lcf, iq, f, want=("lam", "c", "R", "F", "wt"))
     check_spectrum(g, o)
     check_pd(g["PD"], o["PD"])
-    soft = mode in (synth.SOFT_FIXED, synth.SOFT_ENERGY, synth.SOFT_MEDIAN)
+    if curv:
+        assert (o["c"] >= 2).all() and (o["c"] <= N // 2).all(), o["c"]     # the knee, not the noise tail
+    soft = mode in (synth.SOFT_FIXED, synth.SOFT_ENERGY, synth.SOFT_MEDIAN, synth.SOFT_CURVATURE)
     for kk in range(Kz * Kx):
         wt_o = oracle.weights(N, soft, int(o["c"][kk]), f.beta)
         assert np.allclose(g["wt"][kk], wt_o, rtol=0, atol=1e-12)

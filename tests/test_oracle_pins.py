@@ -207,6 +207,38 @@ def test_median_cutoff_pins(oracle):
     assert oracle.cutoff_median(lam, 1.43) == 3
 
 
+def test_curvature_cutoff_pins(oracle):
+    # method 1 (Eq. 6): a log-eigenvalue curve made of two straight lines has zero
+    # second difference everywhere except at the kink, so the maximum curvature sits exactly there
+    N = 40
+    n = np.arange(1, N + 1)
+    for k0 in (3, 5, 9, 17, 21):
+        f = np.where(n <= k0, 6.0 - 0.5 * (n - 1), 6.0 - 0.5 * (k0 - 1) - 0.02 * (n - k0))
+        for beta in (0.3, 1.0, 2.5):
+            assert oracle.cutoff_curvature(10.0 ** f, beta) == k0
+    # the units of the eigenvalues enter through the paper's normalisation by log10(lambda_1):
+    # a straight log-curve has no curvature anywhere -> first candidate (n = 2) by the tie rule
+    assert oracle.cutoff_curvature(10.0 ** (5.0 - 0.1 * n), 1.0) == 2
+    # the floor at 1e-12 lambda_1 (our reading) bends a curve that falls below it
+    f = 6.0 - 0.5 * (n - 1)
+    assert oracle.cutoff_curvature(10.0 ** f, 1.0) == 25                          # 6 - 0.5 * 24 = -6 = log10(1e-12 * 1e6)
+    # degenerate inputs
+    assert oracle.cutoff_curvature(np.array([4.0, 2.0]), 1.0) == 0              # N < 3: no interior point
+    assert oracle.cutoff_curvature(np.array([1.0, 0.5, 0.1, 0.01]), 1.0) == 0   # log10(lambda_1) = 0
+    assert oracle.cutoff_curvature(np.zeros(5), 1.0) == 0
+    # a circle: y(n) on an arc of radius r has curvature 1/r everywhere; bending the arc more sharply
+    # around one index must move the maximum there (numerical check of |y''|/(1+y'^2)^(3/2))
+    N = 64
+    n = np.arange(1, N + 1, dtype=np.float64)
+    y = 40.0 - 0.05 * n - 3.0 / (1.0 + np.exp(-(n - 20.0) * 2.0))
+    # logistic step centred at 20: |y''| peaks one to two samples either side of the centre, y' is largest at it
+    lam = 10.0 ** (y * (6.0 / y[0]))                # y(1) -> log10(lambda_1) = 6; normalised curve = N * y / y[0] * beta
+    k = oracle.cutoff_curvature(lam, 1.0)
+    yy = 1.0 * N * np.log10(lam) / np.log10(lam[0])
+    d1 = (yy[2:] - yy[:-2]) / 2; d2 = yy[2:] - 2 * yy[1:-1] + yy[:-2]
+    assert k == int(np.argmax(np.abs(d2) / (1 + d1 ** 2) ** 1.5)) + 2 and 17 <= k <= 23
+
+
 def test_median_mode_runs_like_fixed_cut(oracle):
     # a window whose median rule gives c must equal the fixed-cut result with k_fixed = c
     iq = synth.random_cube(16, 12, 10, seed=4)
