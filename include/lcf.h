@@ -62,14 +62,17 @@ typedef enum {
     LCF_HARD_CURVATURE = 6, /* hard, c = index of the maximum curvature of the normalised log-eigenvalue
                             curve cut_scale * N * log10(l_n) / log10(l_1)  (method 1, Eq. 6,
                             PAPER.md:77-83; finite differences as in DESIGN.md "Readings")          */
-    LCF_SOFT_CURVATURE = 7  /* sigmoid (Eq. 9) centred on the curvature-rule c                       */
+    LCF_SOFT_CURVATURE = 7, /* sigmoid (Eq. 9) centred on the curvature-rule c                       */
+    LCF_SOFT_ADAPTIVE = 8   /* wt_i = win(i) / l_i^beta normalised to max 1, win = right half of a
+                            Gaussian window (method 6, Eq. 10); no cut-off: c = 0;
+                            the weights follow the small eigenvalues, so use precision = 1          */
 } lcf_thresh_mode;
 
 typedef struct {
     int mode;           /* lcf_thresh_mode                                                      */
     int k_fixed;        /* 0 <= k_fixed <= N (FIXED modes)                                      */
     double energy_frac; /* in (0, 1) (ENERGY modes)                                             */
-    double beta;        /* > 0 (SOFT modes)                                                     */
+    double beta;        /* > 0 (SOFT modes: sigmoid sharpness; ADAPTIVE: the exponent of Eq. 10)  */
     double cut_scale;   /* > 0 (MEDIAN, CURVATURE modes): the scaling factor beta of Eq. 7 / Eq. 6 */
     int precision;      /* 0: fp32 Gram + fp32 EVD.  1: exact-product fp64 Gram + fp64 EVD
                            (single precision can hamper the EVD).  The projection

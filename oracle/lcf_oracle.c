@@ -14,6 +14,7 @@
  *   weights        PAPER.md:57-59 (hard: first k components zeroed), Eq. 9 PAPER.md:111-118 (sigmoid)
  *   cutoff_median  Eq. 7,  PAPER.md:90-96   (method 3: threshold = scale * median eigenvalue)
  *   cutoff_curvature Eq. 6, PAPER.md:77-83  (method 1: maximum curvature of the log-eigenvalue curve)
+ *   weights_adaptive Eq. 10, PAPER.md:120-126 (method 6: Gaussian window over inverse eigenvalue power)
  *   filter         Eq. 4,  PAPER.md:57-59   (F = V Lambda^ V^H)
  *   project_pd     Eq. 4 + PAPER.md:63      (C^ = C_w F; PD = sum over slow time of |C^|^2)
  *   combine        Eq. 13, PAPER.md:154-156 (PD_final = sum_k alpha_k PD_k, alpha_k = 1/mean(PD_k))
@@ -44,7 +45,8 @@
 #define IM(A, i, j, n) ((A)[2 * ((size_t)(i) * (n) + (j)) + 1])
 
 enum { LCFO_HARD_FIXED = 0, LCFO_HARD_ENERGY = 1, LCFO_SOFT_FIXED = 2, LCFO_SOFT_ENERGY = 3,
-       LCFO_HARD_MEDIAN = 4, LCFO_SOFT_MEDIAN = 5, LCFO_HARD_CURVATURE = 6, LCFO_SOFT_CURVATURE = 7 };
+       LCFO_HARD_MEDIAN = 4, LCFO_SOFT_MEDIAN = 5, LCFO_HARD_CURVATURE = 6, LCFO_SOFT_CURVATURE = 7,
+       LCFO_SOFT_ADAPTIVE = 8 };
 
 int lcf_oracle_num_threads(void) {
 #ifdef _OPENMP
@@ -265,6 +267,25 @@ void lcf_oracle_weights(int N, int soft, int c, double beta, double *wt) {
     }
 }
 
+/* Method 6, Eq. 10: wt_i = win(i) / lambda_i^beta, "win(i) represents the Gaussian
+ * window center at i=0 (generated by 'gausswin' function in Matlab). The weighting function wt_i is
+ * normalized before assigning to eigenvalues".  Not in the paper: win is the
+ * right half of gausswin(2N-1) with MATLAB's default alpha = 2.5, i.e.
+ * win(i) = exp(-(alpha (i-1)/(N-1))^2 / 2), i = 1..N (1 at the largest eigenvalue); "normalized" =
+ * divided by the largest weight; eigenvalues are floored at 1e-12 lambda_1. */
+void lcf_oracle_weights_adaptive(const double *lam, int N, double beta, double *wt) {
+    double mx = 0.0;
+    for (int i = 1; i <= N; ++i) {
+        double l = lam[i - 1] > 1e-12 * lam[0] ? lam[i - 1] : 1e-12 * lam[0];
+        double x = 2.5 * (double)(i - 1) / (double)(N - 1);
+        double w = (lam[0] > 0.0) ? exp(-0.5 * x * x) / pow(l, beta) : 0.0;
+        wt[i - 1] = w;
+        if (w > mx) mx = w;
+    }
+    if (mx > 0.0)
+        for (int i = 0; i < N; ++i) wt[i] /= mx;
+}
+
 /* Eq. 4, PAPER.md:57-59 with Lambda^ = diag(wt):  F = V diag(wt) V^H. */
 void lcf_oracle_filter(const double *V, const double *wt, int N, double *F) {
     for (int a = 0; a < N; ++a)
@@ -333,7 +354,8 @@ int lcf_oracle_window(const float *iq, int N, int Nx, int Nz, const double *gz, 
     if (mode == LCFO_HARD_MEDIAN || mode == LCFO_SOFT_MEDIAN) c = lcf_oracle_cutoff_median(lam, N, cut_scale);
     if (mode == LCFO_HARD_CURVATURE || mode == LCFO_SOFT_CURVATURE) c = lcf_oracle_cutoff_curvature(lam, N, cut_scale);
     int soft = (mode == LCFO_SOFT_FIXED || mode == LCFO_SOFT_ENERGY || mode == LCFO_SOFT_MEDIAN || mode == LCFO_SOFT_CURVATURE);
-    lcf_oracle_weights(N, soft, c, beta, wt);
+    if (mode == LCFO_SOFT_ADAPTIVE) { c = 0; lcf_oracle_weights_adaptive(lam, N, beta, wt); }
+    else lcf_oracle_weights(N, soft, c, beta, wt);
     lcf_oracle_filter(V, wt, N, F);
     lcf_oracle_project_pd(iq, N, Nx, Nz, gz, gx, F, PDk);
     double m = 0.0;

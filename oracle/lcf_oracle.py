@@ -18,7 +18,7 @@ _SRC = _HERE / "lcf_oracle.c"
 _LIB = _HERE / "liblcf_oracle.so"
 _lib = None
 
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE = range(8)
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE = range(9)
 
 
 def build(force: bool = False) -> Path:
@@ -52,6 +52,8 @@ def _load():
         L.lcf_oracle_cutoff_curvature.restype = C.c_int
         L.lcf_oracle_weights.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, dp]
         L.lcf_oracle_weights.restype = None
+        L.lcf_oracle_weights_adaptive.argtypes = [dp, C.c_int, C.c_double, dp]
+        L.lcf_oracle_weights_adaptive.restype = None
         L.lcf_oracle_filter.argtypes = [dp, dp, C.c_int, dp]
         L.lcf_oracle_filter.restype = None
         L.lcf_oracle_project_pd.argtypes = [fp, C.c_int, C.c_int, C.c_int, dp, dp, dp, dp]
@@ -139,6 +141,13 @@ def cutoff_curvature(lam: np.ndarray, scale: float) -> int:
 def weights(N: int, soft: bool, c: int, beta: float) -> np.ndarray:
     wt = np.empty(N, dtype=np.float64)
     _load().lcf_oracle_weights(N, int(bool(soft)), int(c), float(beta), _d(wt))
+    return wt
+
+
+def weights_adaptive(lam: np.ndarray, beta: float) -> np.ndarray:
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    wt = np.empty(lam.size)
+    _load().lcf_oracle_weights_adaptive(_d(lam), lam.size, float(beta), _d(wt))
     return wt
 
 

@@ -236,6 +236,7 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
     }
 
     // ---- epilogue: rank eigenvalues (descending, ties by index), cut-off, eigen-weights ----
+    __shared__ double wnorm_sh;                            // normalisation of the adaptive weights (method 6)
     double* lsort = reinterpret_cast<double*>(smem_raw);  // reuse the matrix storage: [N] sorted
     int* csh = reinterpret_cast<int*>(lsort + Ns);
     T myl = T(0);
@@ -255,7 +256,8 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
     }
     __syncthreads();
     if (tid == 0) {
-        const int c = thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
+        const int c = thresh_is_adaptive(a.mode) ? 0 : thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
+        if (thresh_is_adaptive(a.mode)) wnorm_sh = thresh_adaptive_norm(lsort, N, a.beta);
         *csh = c;
         a.cut[k] = c;
         a.sweeps[k] = sweep;
@@ -268,7 +270,8 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
         double w = 0.0;
         if (tid < N) {
             const int i1 = rank + 1;  // 1-based order of the eigenvalue held by index tid
-            w = thresh_weight(soft, a.beta, i1, c);
+            w = thresh_is_adaptive(a.mode) ? thresh_adaptive_raw((double)myl, lsort[0], i1, N, a.beta) / wnorm_sh
+                                             : thresh_weight(soft, a.beta, i1, c);
             a.wt[(size_t)k * N + rank] = w;
         }
         a.wslot[(size_t)k * Ns + tid] = (float)w;

@@ -90,6 +90,7 @@ __device__ __forceinline__ float ec_hsum(unsigned long long v) {
 template <int NC, bool FULL>
 __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double wnorm_sh;                                      // normalisation of the adaptive weights (method 6)
     const int N = a.N, NP = a.NP, Ns = a.Ns, LD = a.LD, M = Ns - 1;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int k = blockIdx.x;
@@ -341,7 +342,8 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     }
     __syncthreads();
     if (tid == 0) {
-        const int c = thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
+        const int c = thresh_is_adaptive(a.mode) ? 0 : thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
+        if (thresh_is_adaptive(a.mode)) wnorm_sh = thresh_adaptive_norm(lsort, N, a.beta);
         ish[1] = c;
         a.cut[k] = c;
         a.sweeps[k] = sweep;
@@ -355,7 +357,8 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
             double w = 0.0;
             if (tid < N) {
                 const int i1 = rank + 1;                             // 1-based order of the eigenvalue in slot tid
-                w = thresh_weight(soft, a.beta, i1, c);
+                w = thresh_is_adaptive(a.mode) ? thresh_adaptive_raw((double)myl, lsort[0], i1, N, a.beta) / wnorm_sh
+                                             : thresh_weight(soft, a.beta, i1, c);
                 a.wt[(size_t)k * N + rank] = w;
             }
             wsl[tid] = (float)w;

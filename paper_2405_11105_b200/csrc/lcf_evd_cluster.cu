@@ -96,6 +96,7 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
                                              float shiftv, float delta, int sweep, int converged) {
     const int N = a.N, Ns = a.N, LD = a.LD;
     const int tid = threadIdx.x;
+    __shared__ double wnorm_sh;                                      // normalisation of the adaptive weights (method 6)
     // ---- eigenvalues and 1/|g| of this CTA's columns (8 threads per column), published to both CTAs
     {
         const int cl = tid >> 3, rr = tid & 7;                       // local column: (pair cl >> 1, row cl & 1)
@@ -139,7 +140,8 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
     }
     __syncthreads();
     if (tid == 0) {
-        const int c = thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
+        const int c = thresh_is_adaptive(a.mode) ? 0 : thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
+        if (thresh_is_adaptive(a.mode)) wnorm_sh = thresh_adaptive_norm(lsort, N, a.beta);
         ish[1] = c;
         if (rank == 0) { a.cut[k] = c; a.sweeps[k] = sweep; a.conv[k] = converged; }
     }
@@ -150,7 +152,8 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
         if (tid < N) {
             const int i1 = rnk + 1;                                  // 1-based order of the eigenvalue in slot tid
             double w;
-            w = thresh_weight(soft, a.beta, i1, c);
+            w = thresh_is_adaptive(a.mode) ? thresh_adaptive_raw((double)myl, lsort[0], i1, N, a.beta) / wnorm_sh
+                                             : thresh_weight(soft, a.beta, i1, c);
             wsl[tid] = (float)w;
             if (rank == 0) {
                 a.wt[(size_t)k * N + rnk] = w;

@@ -9,6 +9,9 @@
 //              DESIGN.md "Readings")
 //   hard       wt_i = 0 for i <= c, 1 above
 //   soft       wt_i = 1 / (1 + exp(-beta (i - c)))          method 5, Eq. 9
+//   adaptive   wt_i = win(i) / l_i^beta, normalised to max 1     method 6, Eq. 10
+//              win = right half of MATLAB's gausswin(2N-1): exp(-(2.5 (i-1)/(N-1))^2 / 2); eigenvalues
+//              floored at 1e-12 l_1; no cut-off (c = 0)
 // i is the 1-based order of the eigenvalue (descending).  Everything in double on the sorted
 // eigenvalues, one thread per window: O(N).
 #pragma once
@@ -17,7 +20,8 @@
 namespace lcf {
 
 __host__ __device__ inline bool thresh_is_soft(int mode) {
-    return mode == LCF_SOFT_FIXED || mode == LCF_SOFT_ENERGY || mode == LCF_SOFT_MEDIAN || mode == LCF_SOFT_CURVATURE;
+    return mode == LCF_SOFT_FIXED || mode == LCF_SOFT_ENERGY || mode == LCF_SOFT_MEDIAN || mode == LCF_SOFT_CURVATURE ||
+           mode == LCF_SOFT_ADAPTIVE;
 }
 
 __device__ inline int thresh_cutoff(int mode, int k_fixed, double energy_frac, double cut_scale, const double* lsort, int N) {
@@ -58,6 +62,26 @@ __device__ inline int thresh_cutoff(int mode, int k_fixed, double energy_frac, d
         return c;
     }
     return k_fixed;
+}
+
+__host__ __device__ inline bool thresh_is_adaptive(int mode) { return mode == LCF_SOFT_ADAPTIVE; }
+
+// un-normalised adaptive weight of the i1-th largest eigenvalue lam (relative to lam1 = largest: the
+// constant lam1^beta cancels in the normalisation and keeps the powers in range)
+__device__ inline double thresh_adaptive_raw(double lam, double lam1, int i1, int N, double beta) {
+    if (!(lam1 > 0.0)) return 0.0;
+    const double r = lam > 1e-12 * lam1 ? lam / lam1 : 1e-12;
+    const double x = 2.5 * (double)(i1 - 1) / (double)(N - 1);
+    return exp(-0.5 * x * x) * pow(r, -beta);
+}
+// max_i of the above over the sorted spectrum (one thread)
+__device__ inline double thresh_adaptive_norm(const double* lsort, int N, double beta) {
+    double m = 0.0;
+    for (int i = 1; i <= N; ++i) {
+        const double w = thresh_adaptive_raw(lsort[i - 1], lsort[0], i, N, beta);
+        if (w > m) m = w;
+    }
+    return m > 0.0 ? m : 1.0;
 }
 
 __device__ inline double thresh_weight(bool soft, double beta, int i1, int c) {

@@ -162,6 +162,7 @@ SMALL = [
     (50, 37, 24, 1, 2, 12.0, 3.0, synth.HARD_MEDIAN, 0, 1),       # median rule in the fp64 path
     (64, 48, 64, 2, 2, 14.0, 3.0, synth.SOFT_CURVATURE, 0, 1),    # method 1 (maximum curvature) + sigmoid: the knee cut needs fp64
     (50, 37, 32, 1, 2, 12.0, 3.0, synth.HARD_CURVATURE, 0, 1),    # hard curvature cut, fp64 path
+    (50, 37, 24, 2, 1, 12.0, 3.0, synth.SOFT_ADAPTIVE, 0, 1),     # method 6 adaptive weights (follow the small eigenvalues: fp64)
 ]
 
 
@@ -186,6 +187,10 @@ def test_small_shapes_and_modes(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, trunc, mo
         assert (o["c"] >= 2).all() and (o["c"] <= N // 2).all(), o["c"]     # the knee, not the noise tail
     soft = mode in (synth.SOFT_FIXED, synth.SOFT_ENERGY, synth.SOFT_MEDIAN, synth.SOFT_CURVATURE)
     for kk in range(Kz * Kx):
+        if mode == synth.SOFT_ADAPTIVE:
+            wt_o = oracle.weights_adaptive(o["lam"][kk], f.beta)
+            assert np.allclose(g["wt"][kk], wt_o, rtol=1e-6, atol=1e-12)   # weights depend on the eigenvalues themselves
+            continue
         wt_o = oracle.weights(N, soft, int(o["c"][kk]), f.beta)
         assert np.allclose(g["wt"][kk], wt_o, rtol=0, atol=1e-12)
     if not soft and prec == 1:

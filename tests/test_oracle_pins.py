@@ -239,6 +239,28 @@ def test_curvature_cutoff_pins(oracle):
     assert k == int(np.argmax(np.abs(d2) / (1 + d1 ** 2) ** 1.5)) + 2 and 17 <= k <= 23
 
 
+def test_adaptive_weights_pins(oracle):
+    # method 6 (Eq. 10): wt_i = win(i) / lambda_i^beta, normalised to max 1
+    from scipy.signal.windows import gaussian
+    for N in (5, 32, 101):
+        # flat spectrum (or beta -> 0): the weights are the window itself = right half of gausswin(2N-1, 2.5),
+        # whose standard deviation in samples is (L-1)/(2 alpha) = (N-1)/2.5
+        win = gaussian(2 * N - 1, std=(N - 1) / 2.5)[N - 1:]
+        assert np.allclose(oracle.weights_adaptive(np.full(N, 7.0), 1.3), win, rtol=0, atol=1e-15)
+        assert np.allclose(oracle.weights_adaptive(np.sort(np.random.default_rng(N).random(N))[::-1] + 1, 1e-12), win, atol=1e-10)
+    # hand-computed: N = 3, lambda = (100, 10, 1), beta = 1: raw = [1/100, e^-0.78125/10, e^-3.125/1]
+    raw = np.array([0.01, np.exp(-0.78125) / 10, np.exp(-3.125)])
+    assert np.allclose(oracle.weights_adaptive(np.array([100.0, 10.0, 1.0]), 1.0), raw / raw.max(), rtol=1e-14)
+    # scale invariance (normalisation removes lambda units), maximum exactly 1, floor at 1e-12 lambda_1
+    lam = np.sort(np.random.default_rng(3).random(20) ** 5)[::-1] + 1e-3
+    w = oracle.weights_adaptive(lam, 0.8)
+    assert w.max() == 1.0 and (w >= 0).all()
+    assert np.allclose(oracle.weights_adaptive(1e6 * lam, 0.8), w, rtol=1e-12)
+    a = oracle.weights_adaptive(np.array([1.0, 0.5, 0.0, -1e-9]), 1.0)
+    b = oracle.weights_adaptive(np.array([1.0, 0.5, 1e-12, 1e-12]), 1.0)
+    assert np.array_equal(a, b)
+
+
 def test_median_mode_runs_like_fixed_cut(oracle):
     # a window whose median rule gives c must equal the fixed-cut result with k_fixed = c
     iq = synth.random_cube(16, 12, 10, seed=4)
