@@ -266,7 +266,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                 float cs = 1.f, gr = 0.f, gim = 0.f;
                 if (rot) {
                     any = 1;
-                    if (absa2 > 1e-6f * app * aqq) big = 1;            // |cos(g_p, g_q)| > 1e-3
+                    if (absa2 > tol * app * aqq) big = 1;              // cos^2 > tol: the next sweep could still rotate
                     // t only steers the rotation (a slightly off angle costs convergence, not accuracy):
                     // approximate sqrt and reciprocal; c^2 + s^2 = 1 rests on one Newton step on rsqrt
                     const float inv = rsqrtf(absa2);
@@ -313,10 +313,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
             b ^= 1;
         }
         ++sweep;
-        // Over both CTAs: did this sweep rotate at all, and was any rotated pair still far (cosine
-        // above 1e-3) from orthogonal?  Jacobi converges quadratically at the end: once every cosine
-        // of a sweep is below 1e-3 the next sweep leaves them at ~1e-6, under the tolerance, so that
-        // sweep is the last one and the usual rotation-free confirmation sweep is not run.
+        // Over both CTAs: did this sweep rotate at all, and was any rotated pair still far (squared
+        // cosine above tol) from orthogonal?  Jacobi converges quadratically at the end: once every
+        // cosine of a sweep is below sqrt(tol) the next sweep leaves them at ~tol, which the sweep after
+        // would not rotate, so that next sweep is the last one and the usual rotation-free
+        // confirmation sweep is not run.
         const int mine = __syncthreads_or(any) + __syncthreads_or(big);
         if (tid == 0) {
             const uint32_t fa = ecl_smem(&flg[(sweep & 1) * 2 + rank]);
@@ -349,8 +350,8 @@ __device__ __forceinline__ int ecb_slot(int b, int t, int j, int cb, int LD) { r
 
 struct EcbCol { ulonglong2 re, im; };          // 4 rows of one column: (r0,r1),(r2,r3) real and imaginary
 
-// rotate the pairs (X, Y) and (Z, W) at once; returns bit 0: rotated, bit 1: a rotated pair had cosine > 1e-3
-__device__ __forceinline__ int ecb_round(EcbCol& X, EcbCol& Y, EcbCol& Z, EcbCol& W, int lane, float tol2) {
+// rotate the pairs (X, Y) and (Z, W) at once; returns bit 0: rotated, bit 1: a rotated pair had squared cosine > big2
+__device__ __forceinline__ int ecb_round(EcbCol& X, EcbCol& Y, EcbCol& Z, EcbCol& W, int lane, float tol2, float big2) {
     float v1[4], v2[4];
     {
         unsigned long long app2 = ecl_fma2(X.re.x, X.re.x, ecl_fma2(X.im.x, X.im.x, ecl_fma2(X.re.y, X.re.y, ecl_mul2(X.im.y, X.im.y))));
@@ -385,7 +386,7 @@ __device__ __forceinline__ int ecb_round(EcbCol& X, EcbCol& Y, EcbCol& Z, EcbCol
     float cs = 1.f, gr = 0.f, gi = 0.f;
     int flags = 0;
     if (absa2 > tol2 * app * aqq && absa2 > 0.f) {
-        flags = 1 | (absa2 > 1e-6f * app * aqq ? 2 : 0);
+        flags = 1 | (absa2 > big2 * app * aqq ? 2 : 0);
         const float inv = rsqrtf(absa2);
         const float tau = (aqq - app) * (0.5f * inv);
         const float at = fminf(fabsf(tau), 1e18f);
@@ -484,9 +485,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                     B0.re = *reinterpret_cast<const ulonglong2*>(b0);          B0.im = *reinterpret_cast<const ulonglong2*>(b0 + LD);
                     B1.re = *reinterpret_cast<const ulonglong2*>(b0 + 2 * LD); B1.im = *reinterpret_cast<const ulonglong2*>(b0 + 3 * LD);
                 }
-                if (s == 0) fl |= ecb_round(A0, A1, B0, B1, lane, tol2);     // inner pairs, once per sweep
-                fl |= ecb_round(A0, B0, A1, B1, lane, tol2);
-                fl |= ecb_round(A0, B1, A1, B0, lane, tol2);
+                if (s == 0) fl |= ecb_round(A0, A1, B0, B1, lane, tol2, tol);     // inner pairs, once per sweep
+                fl |= ecb_round(A0, B0, A1, B1, lane, tol2, tol);
+                fl |= ecb_round(A0, B1, A1, B0, lane, tol2, tol);
                 if (rowok) {
                     const uint32_t aP = (Prem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dPt, dPj, 0, LD) + 4 * lane) * 4u;
                     const uint32_t aQ = (Qrem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dQt, dQj, 0, LD) + 4 * lane) * 4u;
