@@ -65,6 +65,7 @@ __device__ __forceinline__ void ec_pair_pq(int m, int s, int M, int& p, int& q) 
 }
 
 constexpr int EC_THREADS = 512;   // 8 threads per column pair (NP <= 64 pairs)
+constexpr int EC_PS = 264, EC_PI = 132;   // floats per partial vector (N <= 128; EC_PS % 32 == 8), offset of its imaginary half
 
 __device__ __forceinline__ unsigned long long ec_fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
     unsigned long long d;
@@ -97,29 +98,25 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     // planar storage: real and imaginary parts of column u at Gr/Gi + u*LD (LD floats, multiple of 4)
     float* Gr = reinterpret_cast<float*>(smem_raw);                  // [Ns][LD]
     float* Gi = Gr + (size_t)Ns * LD;                                // [Ns][LD]
-    float* ljr = Gi + (size_t)Ns * LD;                               // [LD] current Cholesky column
-    float* lji = ljr + LD;                                           // [LD]
-    float* lam_s = lji + LD;                                         // [Ns] eigenvalue of slot u
+    float* part = Gi + (size_t)Ns * LD;                              // [16][EC_PS] per-warp partial Schur columns (re at 0, im at EC_PI)
+    float* lam_s = part + (EC_THREADS / 32) * EC_PS;                 // [Ns] eigenvalue of slot u
     float* inv_s = lam_s + Ns;                                       // [Ns] 1 / |g_u|
     float* wsl = inv_s + Ns;                                         // [Ns] eigen-weight of slot u
     float* red = wsl + Ns;                                           // [32]
     double* lsort = reinterpret_cast<double*>(red + 32);             // [Ns] sorted eigenvalues
-    int* act = reinterpret_cast<int*>(lsort + Ns);                   // [Ns] row/column still in the trailing matrix
-    int* ish = act + Ns;                                             // [4] pivot, cut-off
-    int* alist = ish + 4;                                            // [Ns] compacted active columns
-    int* apos = alist + Ns;                                          // [Ns] position of a column in alist
+    int* ish = reinterpret_cast<int*>(lsort + Ns);                                             // [4] pivot, cut-off
+    int* alist = ish + 4;                                            // [Ns] pivot order of the Cholesky steps
 
-    // ---- load R (row-major [i][j]) into the column-major planes; zero the padding
+    // ---- load R (row-major [i][j]) into the column-major planes (conflict-free: row i lands in column i); zero the padding
     const float2* Rk = a.R + (size_t)k * N * N;
     for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) Gr[e] = 0.f;
     __syncthreads();
     for (int e = tid; e < N * N; e += EC_THREADS) {
-        const int i = e / N, j = e - i * N;                          // coalesced read of row i
+        const int i = e / N, j = e - i * N;                          // coalesced read of row i = conj of column i (R is Hermitian)
         const float2 x = Rk[e];
-        Gr[(size_t)j * LD + i] = x.x;
-        Gi[(size_t)j * LD + i] = x.y;
+        Gr[(size_t)i * LD + j] = x.x;
+        Gi[(size_t)i * LD + j] = -x.y;
     }
-    if (tid < Ns) act[tid] = tid < N ? 1 : 0;
     __syncthreads();
     float md = 0.f;
     if (tid < N) md = Gr[(size_t)tid * LD + tid];
@@ -135,71 +132,95 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     if (maxdiag > 0.f) {
         if (tid < N) { Gr[(size_t)tid * LD + tid] += delta; Gi[(size_t)tid * LD + tid] = 0.f; }
         __syncthreads();
-        // ---- 2. pivoted Cholesky, in place.  Two barriers per step: the trailing update keeps a copy of
-        // the diagonal, every warp searches it for the next pivot, and the update runs over a
-        // compacted list of active columns.
+        // ---- 2. pivoted Cholesky, left-looking: R stays untouched until a column is chosen.  Step j
+        // picks the largest remaining diagonal entry, forms that column's Schur complement as
+        // R[:, pv] - G[:, e_0..e_{j-1}] conj(G[pv, e_0..e_{j-1}]) (a matrix-vector product over the
+        // finished columns: warp w takes every 16th of them, lane r rows 4r..4r+3, and the 16 partial
+        // vectors are summed through `part`), scales it into column pv and downdates the diagonal.
+        // Shared-memory traffic per step is the finished columns read once, against the whole
+        // trailing matrix read and written by a right-looking update.
+        // The pivot search is a warp-wide integer maximum (redux) over keys that hold the diagonal
+        // entry's top 25 bits above 127 - row (ties, and near-ties within 2^-16, go to the lowest row):
+        // each warp reduces its 8 rows when it downdates them, and after the step's barrier every warp
+        // reduces the 16 warp keys.
         const int nchc = (N + 3) >> 2;                               // 4-row chunks per column
-        float* dgs = lam_s;                                          // [N] current diagonal of the trailing matrix, -1 once eliminated
-        if (tid < N) {
-            alist[tid] = tid; apos[tid] = tid;
-            const float d = fmaxf(Gr[(size_t)tid * LD + tid], 0.f);
-            dgs[tid] = d;
+        float* dgs = lam_s;                                          // [N] current diagonal of the Schur complement, -1 once eliminated
+        unsigned* wkey = reinterpret_cast<unsigned*>(red);           // [16] per-warp pivot keys
+        const int ri = tid >> 2, rq = tid & 3;                       // downdate phase: 4 threads per row
+        {
+            unsigned key = 0u;
+            if (rq == 0 && ri < N) {
+                const float d = fmaxf(Gr[(size_t)ri * LD + ri], 0.f);
+                dgs[ri] = d;
+                key = (__float_as_uint(d) & ~127u) | (unsigned)(127 - ri);
+            }
+            key = __reduce_max_sync(0xffffffffu, key);
+            if (lane == 0) wkey[warp] = key;
         }
         __syncthreads();
-        for (int j = 0; j < N; ++j) {
-            // every warp finds the pivot (largest remaining diagonal entry, ties to the lowest index) itself
-            float best = -1.f; int pv = N;
-            for (int i = lane; i < N; i += 32) { const float d = dgs[i]; if (d > best) { best = d; pv = i; } }
+        int ecol[8];                                                 // slots of this warp's finished columns (steps warp, warp + 16, ...)
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const float ob = __shfl_xor_sync(0xffffffffu, best, o);
-                const int oi = __shfl_xor_sync(0xffffffffu, pv, o);
-                if (ob > best || (ob == best && oi < pv)) { best = ob; pv = oi; }
-            }
+        for (int m = 0; m < 8; ++m) ecol[m] = 0;
+        for (int j = 0; j < N; ++j) {
+            unsigned kk = lane < EC_THREADS / 32 ? wkey[lane] : 0u;
+            kk = __reduce_max_sync(0xffffffffu, kk);
+            const int pv = 127 - (int)(kk & 127u);
             // a non-positive pivot can only come from rounding: clamp (the column is then ~0)
-            const float piv = fmaxf(best, 1e-30f * maxdiag + 1e-37f);
-            const float dsq = sqrtf(piv), sc = rsqrtf(piv);
-            const int na = N - 1 - j;                                // active columns after removing pv
-            if (tid < LD) {
-                float vr = 0.f, vi = 0.f;
-                if (tid == pv) vr = dsq;
-                else if (tid < N && act[tid]) { vr = Gr[(size_t)pv * LD + tid] * sc; vi = Gi[(size_t)pv * LD + tid] * sc; }
-                Gr[(size_t)pv * LD + tid] = vr;                       // Cholesky column pi_j, zero in eliminated rows
-                Gi[(size_t)pv * LD + tid] = vi;
-                ljr[tid] = (tid == pv) ? 0.f : vr;                    // multiplier for the trailing update
-                lji[tid] = (tid == pv) ? 0.f : vi;
-            }
-            if (tid == 0) {                                          // drop pv from the active list (swap with last)
-                const int ps = apos[pv], last = alist[na];
-                alist[ps] = last; apos[last] = ps;
-                dgs[pv] = -1.f;                                      // eliminated
-            }
-            __syncthreads();
-            if (tid == 0) act[pv] = 0;
-            // trailing update A[i][l] -= L[i] conj(L[l]) over (active column, 4-row chunk) items
-#pragma unroll 4
-            for (int idx = tid; idx < na * nchc; idx += EC_THREADS) {
-                const int ci = idx / nchc, chk = idx - ci * nchc;
-                const int l = alist[ci];
-                const float lr = ljr[l], li = lji[l];
-                float* cr = Gr + (size_t)l * LD + 4 * chk;
-                float* ci_ = Gi + (size_t)l * LD + 4 * chk;
-                float4 xr = *reinterpret_cast<float4*>(cr);
-                float4 xi = *reinterpret_cast<float4*>(ci_);
-                const float4 mr = *reinterpret_cast<const float4*>(&ljr[4 * chk]);
-                const float4 mi = *reinterpret_cast<const float4*>(&lji[4 * chk]);
-                // x -= m * conj(l):  re -= mr lr + mi li,  im -= mi lr - mr li
-                xr.x -= mr.x * lr + mi.x * li;  xi.x -= mi.x * lr - mr.x * li;
-                xr.y -= mr.y * lr + mi.y * li;  xi.y -= mi.y * lr - mr.y * li;
-                xr.z -= mr.z * lr + mi.z * li;  xi.z -= mi.z * lr - mr.z * li;
-                xr.w -= mr.w * lr + mi.w * li;  xi.w -= mi.w * lr - mr.w * li;
-                *reinterpret_cast<float4*>(cr) = xr;
-                *reinterpret_cast<float4*>(ci_) = xi;
-                if (chk == (l >> 2)) {                               // this chunk holds the diagonal entry A[l][l]
-                    const int w = l & 3;
-                    const float d = fmaxf(w == 0 ? xr.x : w == 1 ? xr.y : w == 2 ? xr.z : xr.w, 0.f);
-                    dgs[l] = d;
+            const float piv = fmaxf(dgs[pv], 1e-30f * maxdiag + 1e-37f);
+            const float sc = rsqrtf(piv), dsq = piv * sc;
+            if (lane < nchc) {
+                float4 ar = make_float4(0.f, 0.f, 0.f, 0.f), ai = ar;
+                const int cnt = (j - warp + EC_THREADS / 32 - 1) / (EC_THREADS / 32);   // finished columns of this warp
+#pragma unroll
+                for (int m = 0; m < 8; ++m) {
+                    if (m < cnt) {
+                        const float* cr = Gr + (size_t)ecol[m] * LD;
+                        const float* ci = Gi + (size_t)ecol[m] * LD;
+                        const float lr = cr[pv], li = ci[pv], nli = -li;
+                        const float4 xr = *reinterpret_cast<const float4*>(&cr[4 * lane]);
+                        const float4 xi = *reinterpret_cast<const float4*>(&ci[4 * lane]);
+                        // x * conj(l):  re += xr lr + xi li,  im += xi lr - xr li
+                        ar.x = fmaf(xr.x, lr, fmaf(xi.x, li, ar.x));  ai.x = fmaf(xi.x, lr, fmaf(xr.x, nli, ai.x));
+                        ar.y = fmaf(xr.y, lr, fmaf(xi.y, li, ar.y));  ai.y = fmaf(xi.y, lr, fmaf(xr.y, nli, ai.y));
+                        ar.z = fmaf(xr.z, lr, fmaf(xi.z, li, ar.z));  ai.z = fmaf(xi.z, lr, fmaf(xr.z, nli, ai.z));
+                        ar.w = fmaf(xr.w, lr, fmaf(xi.w, li, ar.w));  ai.w = fmaf(xi.w, lr, fmaf(xr.w, nli, ai.w));
+                    }
                 }
+                *reinterpret_cast<float4*>(&part[warp * EC_PS + 4 * lane]) = ar;
+                *reinterpret_cast<float4*>(&part[warp * EC_PS + EC_PI + 4 * lane]) = ai;
+            }
+#pragma unroll
+            for (int m = 0; m < 8; ++m) if (j == warp + m * (EC_THREADS / 32)) ecol[m] = pv;   // column j is finished after this step
+            __syncthreads();
+            {
+                // thread rq of row ri sums the partials of warps rq, rq+4, rq+8, rq+12 (conflict-free: EC_PS % 32 == 8)
+                float sr = 0.f, si = 0.f, d = -1.f, cr0 = 0.f, ci0 = 0.f;
+                if (ri < N) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        sr += part[(rq + 4 * u) * EC_PS + ri];
+                        si += part[(rq + 4 * u) * EC_PS + EC_PI + ri];
+                    }
+                    if (rq == 0) { d = dgs[ri]; cr0 = Gr[(size_t)pv * LD + ri]; ci0 = Gi[(size_t)pv * LD + ri]; }
+                }
+                sr += __shfl_xor_sync(0xffffffffu, sr, 1);  si += __shfl_xor_sync(0xffffffffu, si, 1);
+                sr += __shfl_xor_sync(0xffffffffu, sr, 2);  si += __shfl_xor_sync(0xffffffffu, si, 2);
+                unsigned key = 0u;
+                if (rq == 0 && ri < N) {
+                    float vr = 0.f, vi = 0.f;                        // Cholesky column pi_j is zero in eliminated rows
+                    if (ri == pv) { vr = dsq; dgs[ri] = -1.f; }
+                    else if (d >= 0.f) {
+                        vr = (cr0 - sr) * sc;
+                        vi = (ci0 - si) * sc;
+                        const float nd = fmaxf(d - (vr * vr + vi * vi), 0.f);
+                        dgs[ri] = nd;
+                        key = (__float_as_uint(nd) & ~127u) | (unsigned)(127 - ri);
+                    }
+                    Gr[(size_t)pv * LD + ri] = vr;
+                    Gi[(size_t)pv * LD + ri] = vi;
+                }
+                key = __reduce_max_sync(0xffffffffu, key);
+                if (lane == 0) wkey[warp] = key;
             }
             __syncthreads();
         }
@@ -380,7 +401,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
 }
 
 static size_t ec_smem_bytes(int Ns, int LD) {
-    return (size_t)Ns * LD * 8 + (size_t)LD * 8 + 3 * (size_t)Ns * 4 + 32 * 4 + (size_t)Ns * 8 + 3 * (size_t)Ns * 4 + 16 + 16 + 64;
+    return (size_t)Ns * LD * 8 + (size_t)(EC_THREADS / 32) * EC_PS * 4 + 3 * (size_t)Ns * 4 + 32 * 4 + (size_t)Ns * 8 + 3 * (size_t)Ns * 4 + 16 + 16 + 64;
 }
 
 bool evd_chol_eligible(const lcf_plan* p) { return p->prec == 0 && p->N <= 128 && p->N >= 2; }
