@@ -75,6 +75,30 @@ __device__ __forceinline__ void ecl_st_local(uint32_t addr, ulonglong2 v) {
 __device__ __forceinline__ void ecl_st_cluster_f32(uint32_t addr, float v) {
     asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
 }
+// remote store that reports its bytes to an mbarrier of the destination CTA (both addresses shared::cluster)
+__device__ __forceinline__ void ecl_st_async(uint32_t addr, ulonglong2 v, uint32_t mbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1, %2}, [%3];"
+                 ::"r"(addr), "l"(v.x), "l"(v.y), "r"(mbar) : "memory");
+}
+__device__ __forceinline__ void ecl_mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void ecl_mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void ecl_mbar_arrive_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void ecl_mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done = 0;
+    const long long t0 = clock64();
+    for (;;) {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (done) break;
+        if (clock64() - t0 > 4000000000ll) __trap();                 // a lost signal must not hang the device
+    }
+}
 __device__ __forceinline__ void ecl_cluster_sync() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
@@ -438,7 +462,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
     float* flg = wsl + Ns;
     double* lsort = reinterpret_cast<double*>(flg + 4);
     int* ish = reinterpret_cast<int*>(lsort + Ns);
+    uint64_t* fullb = reinterpret_cast<uint64_t*>(ish + 4);         // [2 buffers][ECB_PL] "both blocks of this pair have arrived"
     const uint32_t buf_u32 = ecl_smem(buf), buf_peer = ecl_mapa(buf_u32, peer);
+    const uint32_t full_u32 = ecl_smem(fullb), full_peer = ecl_mapa(full_u32, peer);
 
     // ---- initial placement: block pair i = columns 4i .. 4i+3 (top block 4i, 4i+1; bottom block 4i+2, 4i+3)
     const float* gk = a.gfac + (size_t)k * 2 * N * a.LDg;
@@ -454,12 +480,30 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
     }
     const float shiftv = a.shift[k];
     const float delta = shiftv < 0.f ? 0.f : shiftv;
+    const int j = tid >> 5;                                          // local block pair = warp
+    const int gi = p0 + j;
+    // Dataflow between block pairs: a pair's two blocks for the next step come from its ring
+    // neighbours gi - 1 and gi + 1 (itself at the ends).  A neighbour in this CTA stores them and
+    // arrives on the pair's mbarrier; the neighbour across the cluster sends them with st.async, whose
+    // bytes the mbarrier counts.  The pair's warp posts its own arrival (with the expected remote
+    // bytes) one use ahead, so a phase completes exactly when both blocks are in place, and no
+    // CTA- or cluster-wide barrier is needed inside a sweep.  Overwriting is safe without an "empty"
+    // signal: every link is two-way, so a neighbour can only be two steps ahead after it has
+    // consumed what this pair sent one step ahead, which this pair sends after reading its inputs.
+    const int lo = gi > 0 ? gi - 1 : 0, hi = gi < n - 1 ? gi + 1 : n - 1;
+    const int nloc = (int)((lo >= h) == (gi >= h)) + (int)((hi >= h) == (gi >= h));
+    const uint32_t txb = (uint32_t)(2 - nloc) * 64u * (uint32_t)nch;       // bytes of the blocks that arrive by st.async
+    if (j < npl && lane == 0) {
+        ecl_mbar_init(full_u32 + 8u * (uint32_t)j, 1u + (uint32_t)nloc);
+        ecl_mbar_init(full_u32 + 8u * (uint32_t)(ECB_PL + j), 1u + (uint32_t)nloc);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        ecl_mbar_arrive_tx(full_u32 + 8u * (uint32_t)j, txb);                // buffer 0 is refilled at step 1
+        ecl_mbar_arrive_tx(full_u32 + 8u * (uint32_t)(ECB_PL + j), txb);     // buffer 1 is filled at step 0
+    }
     ecl_cluster_sync();
 
     const float tol = 4.f * sqrtf((float)N) * FLT_EPSILON;
     const float tol2 = tol * tol;
-    const int j = tid >> 5;                                          // local block pair = warp
-    const int gi = p0 + j;
     const bool rowok = lane < nch;                                   // this lane's 4 rows exist
     int dPt, dPi, dQt, dQi;                                          // destinations of the top / bottom block (row, block pair)
     if (gi == 0) { dPt = 0; dPi = 0; dQt = 0; dQi = 1; }
@@ -469,11 +513,17 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
     const int dPj = dPi - (dPi >= h ? h : 0), dQj = dQi - (dQi >= h ? h : 0);
     const int M = 2 * n - 1;
     int b = 0, sweep = 0, converged = 0;
+    unsigned t = 0;                                                  // steps so far, over all sweeps
     bool last = false;
     for (;;) {
         int fl = 0;
-        for (int s = 0; s < M; ++s) {
+        for (int s = 0; s < M; ++s, ++t) {
             if (j < npl) {
+                if (t > 0) {
+                    const uint32_t fb = full_u32 + 8u * (uint32_t)(b * ECB_PL + j);
+                    ecl_mbar_wait(fb, ((t - 1) >> 1) & 1u);
+                    if (lane == 0) ecl_mbar_arrive_tx(fb, txb);      // this pair's arrival for the buffer's next use
+                }
                 EcbCol A0, A1, B0, B1;
                 const ulonglong2 z2 = make_ulonglong2(0ull, 0ull);
                 A0.re = A0.im = A1.re = A1.im = B0.re = B0.im = B1.re = B1.im = z2;
@@ -488,23 +538,29 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                 if (s == 0) fl |= ecb_round(A0, A1, B0, B1, lane, tol2, tol);     // inner pairs, once per sweep
                 fl |= ecb_round(A0, B0, A1, B1, lane, tol2, tol);
                 fl |= ecb_round(A0, B1, A1, B0, lane, tol2, tol);
+                const uint32_t mP = (Prem ? full_peer : full_u32) + 8u * (uint32_t)((b ^ 1) * ECB_PL + dPj);
+                const uint32_t mQ = (Qrem ? full_peer : full_u32) + 8u * (uint32_t)((b ^ 1) * ECB_PL + dQj);
                 if (rowok) {
                     const uint32_t aP = (Prem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dPt, dPj, 0, LD) + 4 * lane) * 4u;
                     const uint32_t aQ = (Qrem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dQt, dQj, 0, LD) + 4 * lane) * 4u;
                     const uint32_t L4 = (uint32_t)LD * 4u;
                     if (Prem) {
-                        ecl_st_cluster(aP, A0.re); ecl_st_cluster(aP + L4, A0.im); ecl_st_cluster(aP + 2 * L4, A1.re); ecl_st_cluster(aP + 3 * L4, A1.im);
+                        ecl_st_async(aP, A0.re, mP); ecl_st_async(aP + L4, A0.im, mP); ecl_st_async(aP + 2 * L4, A1.re, mP); ecl_st_async(aP + 3 * L4, A1.im, mP);
                     } else {
                         ecl_st_local(aP, A0.re); ecl_st_local(aP + L4, A0.im); ecl_st_local(aP + 2 * L4, A1.re); ecl_st_local(aP + 3 * L4, A1.im);
                     }
                     if (Qrem) {
-                        ecl_st_cluster(aQ, B0.re); ecl_st_cluster(aQ + L4, B0.im); ecl_st_cluster(aQ + 2 * L4, B1.re); ecl_st_cluster(aQ + 3 * L4, B1.im);
+                        ecl_st_async(aQ, B0.re, mQ); ecl_st_async(aQ + L4, B0.im, mQ); ecl_st_async(aQ + 2 * L4, B1.re, mQ); ecl_st_async(aQ + 3 * L4, B1.im, mQ);
                     } else {
                         ecl_st_local(aQ, B0.re); ecl_st_local(aQ + L4, B0.im); ecl_st_local(aQ + 2 * L4, B1.re); ecl_st_local(aQ + 3 * L4, B1.im);
                     }
                 }
+                __syncwarp();
+                if (lane == 0) {                                     // blocks stored in this CTA: arrive for the whole warp
+                    if (!Prem) ecl_mbar_arrive(mP);
+                    if (!Qrem) ecl_mbar_arrive(mQ);
+                }
             }
-            ecl_cluster_sync();
             b ^= 1;
         }
         ++sweep;
@@ -522,13 +578,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
         if (f0 < 2.f && f1 < 2.f) last = true;
     }
 
+    if (j < npl) ecl_mbar_wait(full_u32 + 8u * (uint32_t)(b * ECB_PL + j), ((t - 1) >> 1) & 1u);   // the last step's blocks
+    ecl_cluster_sync();
     ecl_epilogue(a, k, rank, peer, 4 * p0, 4 * npl,
                  [&](int cl) { return (const float*)(buf + ecb_slot(b, (cl >> 1) & 1, cl >> 2, cl & 1, LD)); },
                  lam_s, inv_s, wsl, lsort, ish, shiftv, delta, sweep, converged);
 }
 
 static size_t ecl_smem_bytes(int N, int LD) {
-    return (size_t)2 * 2 * ECL_PL * 2 * LD * 4 + 3 * (size_t)N * 4 + 16 + (size_t)N * 8 + 16 + 64;
+    return (size_t)2 * 2 * ECL_PL * 2 * LD * 4 + 3 * (size_t)N * 4 + 16 + (size_t)N * 8 + 16 + 2 * ECB_PL * 8 + 64;
 }
 
 bool evd_cluster_eligible(const lcf_plan* p) { return p->prec == 0 && (p->N % 2) == 0 && p->N >= 32 && p->N <= 128; }
