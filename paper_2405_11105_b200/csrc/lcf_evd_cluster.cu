@@ -80,6 +80,13 @@ __device__ __forceinline__ void ecl_st_async(uint32_t addr, ulonglong2 v, uint32
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1, %2}, [%3];"
                  ::"r"(addr), "l"(v.x), "l"(v.y), "r"(mbar) : "memory");
 }
+__device__ __forceinline__ void ecl_st_async_f32(uint32_t addr, float v, uint32_t mbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];"
+                 ::"r"(addr), "r"(__float_as_uint(v)), "r"(mbar) : "memory");
+}
+__device__ __forceinline__ void ecl_st_local_f32(uint32_t addr, float v) {
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
 __device__ __forceinline__ void ecl_mbar_init(uint32_t bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
@@ -366,7 +373,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
 // registers) and per block step rotates the four cross pairs as two rounds of two independent
 // rotations -- (A0,B0)+(A1,B1), then (A0,B1)+(A1,B0) -- and, at the first block step of a sweep, the
 // inner pairs (A0,A1)+(B0,B1).  Every column pair is still met once per sweep, but the columns
-// cross shared memory (and the cluster barrier is paid) once per TWO rotation rounds, the two
+// cross shared memory (and the hand-over to the neighbours is paid) once per TWO rotation rounds, the two
 // rotations of a round overlap their latency chains, and the halves of the warp compute one
 // rotation's parameters each instead of all lanes repeating the same one.
 constexpr int ECB_PL = 16;                     // block-pair slots per CTA (N <= 128: 32 block pairs)
@@ -374,59 +381,84 @@ __device__ __forceinline__ int ecb_slot(int b, int t, int j, int cb, int LD) { r
 
 struct EcbCol { ulonglong2 re, im; };          // 4 rows of one column: (r0,r1),(r2,r3) real and imaginary
 
-// rotate the pairs (X, Y) and (Z, W) at once; returns bit 0: rotated, bit 1: a rotated pair had squared cosine > big2
-__device__ __forceinline__ int ecb_round(EcbCol& X, EcbCol& Y, EcbCol& Z, EcbCol& W, int lane, float tol2, float big2) {
-    float v1[4], v2[4];
+// squared norms of four columns, exact, in every lane (10 shuffles: the four sums are folded onto
+// quarter warps on the way down and broadcast at the end)
+__device__ __forceinline__ void ecb_norms4(const EcbCol& X, const EcbCol& Y, const EcbCol& Z, const EcbCol& W, int lane,
+                                           float& nX, float& nY, float& nZ, float& nW) {
+    auto nrm = [](const EcbCol& C) {
+        return ecl_hsum(ecl_fma2(C.re.x, C.re.x, ecl_fma2(C.im.x, C.im.x, ecl_fma2(C.re.y, C.re.y, ecl_mul2(C.im.y, C.im.y)))));
+    };
+    const float a0 = nrm(X), a1 = nrm(Y), a2 = nrm(Z), a3 = nrm(W);
+    const bool h16 = (lane & 16) != 0, h8 = (lane & 8) != 0;
+    // lanes with bit 4 clear keep (X, Y), the others (Z, W); then bit 3 picks one of the two
+    float k0 = (h16 ? a2 : a0) + __shfl_xor_sync(0xffffffffu, h16 ? a0 : a2, 16);
+    float k1 = (h16 ? a3 : a1) + __shfl_xor_sync(0xffffffffu, h16 ? a1 : a3, 16);
+    float v = (h8 ? k1 : k0) + __shfl_xor_sync(0xffffffffu, h8 ? k0 : k1, 8);
+    v += __shfl_xor_sync(0xffffffffu, v, 4);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    nX = __shfl_sync(0xffffffffu, v, 0);  nY = __shfl_sync(0xffffffffu, v, 8);
+    nZ = __shfl_sync(0xffffffffu, v, 16); nW = __shfl_sync(0xffffffffu, v, 24);
+}
+
+// Rotate the pairs (X, Y) and (Z, W) at once; returns bit 0: rotated, bit 1: a rotated pair had
+// squared cosine > big2.  The squared column norms are carried along instead of recomputed: a rotation by
+// tangent t of the pair (p, q) with inner product a changes them to |g_p|^2 - t |a| and
+// |g_q|^2 + t |a| (exactly, for the exact rotation), so a round needs only the inner products.
+// The carried values are refreshed from the columns at the first block step of every sweep and
+// whenever an update cancels more than three quarters of a norm.
+__device__ __forceinline__ int ecb_round_tracked(EcbCol& X, EcbCol& Y, EcbCol& Z, EcbCol& W, float& nX, float& nY, float& nZ, float& nW,
+                                                 int lane, float tol2, float big2) {
+    float v1[2], v2[2];
     {
-        unsigned long long app2 = ecl_fma2(X.re.x, X.re.x, ecl_fma2(X.im.x, X.im.x, ecl_fma2(X.re.y, X.re.y, ecl_mul2(X.im.y, X.im.y))));
-        unsigned long long aqq2 = ecl_fma2(Y.re.x, Y.re.x, ecl_fma2(Y.im.x, Y.im.x, ecl_fma2(Y.re.y, Y.re.y, ecl_mul2(Y.im.y, Y.im.y))));
         unsigned long long re2 = ecl_fma2(X.re.x, Y.re.x, ecl_fma2(X.im.x, Y.im.x, ecl_fma2(X.re.y, Y.re.y, ecl_mul2(X.im.y, Y.im.y))));
         unsigned long long ia2 = ecl_fma2(X.re.x, Y.im.x, ecl_mul2(X.re.y, Y.im.y));
         unsigned long long ib2 = ecl_fma2(X.im.x, Y.re.x, ecl_mul2(X.im.y, Y.re.y));
-        v1[0] = ecl_hsum(app2); v1[1] = ecl_hsum(aqq2); v1[2] = ecl_hsum(re2); v1[3] = ecl_hsum(ia2) - ecl_hsum(ib2);
+        v1[0] = ecl_hsum(re2); v1[1] = ecl_hsum(ia2) - ecl_hsum(ib2);
     }
     {
-        unsigned long long app2 = ecl_fma2(Z.re.x, Z.re.x, ecl_fma2(Z.im.x, Z.im.x, ecl_fma2(Z.re.y, Z.re.y, ecl_mul2(Z.im.y, Z.im.y))));
-        unsigned long long aqq2 = ecl_fma2(W.re.x, W.re.x, ecl_fma2(W.im.x, W.im.x, ecl_fma2(W.re.y, W.re.y, ecl_mul2(W.im.y, W.im.y))));
         unsigned long long re2 = ecl_fma2(Z.re.x, W.re.x, ecl_fma2(Z.im.x, W.im.x, ecl_fma2(Z.re.y, W.re.y, ecl_mul2(Z.im.y, W.im.y))));
         unsigned long long ia2 = ecl_fma2(Z.re.x, W.im.x, ecl_mul2(Z.re.y, W.im.y));
         unsigned long long ib2 = ecl_fma2(Z.im.x, W.re.x, ecl_mul2(Z.im.y, W.re.y));
-        v2[0] = ecl_hsum(app2); v2[1] = ecl_hsum(aqq2); v2[2] = ecl_hsum(re2); v2[3] = ecl_hsum(ia2) - ecl_hsum(ib2);
+        v2[0] = ecl_hsum(re2); v2[1] = ecl_hsum(ia2) - ecl_hsum(ib2);
     }
-    // lanes 0-15 end up with the sums of (X, Y), lanes 16-31 with those of (Z, W)
+    // lanes 0-15 end up with the inner product of (X, Y), lanes 16-31 with that of (Z, W)
     const bool lo = lane < 16;
-    float v[4];
+    float xr = (lo ? v1[0] : v2[0]) + __shfl_xor_sync(0xffffffffu, lo ? v2[0] : v1[0], 16);
+    float xi = (lo ? v1[1] : v2[1]) + __shfl_xor_sync(0xffffffffu, lo ? v2[1] : v1[1], 16);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const float send = lo ? v2[i] : v1[i];
-        v[i] = (lo ? v1[i] : v2[i]) + __shfl_xor_sync(0xffffffffu, send, 16);
+    for (int o = 8; o > 0; o >>= 1) {
+        xr += __shfl_xor_sync(0xffffffffu, xr, o);
+        xi += __shfl_xor_sync(0xffffffffu, xi, o);
     }
-#pragma unroll
-    for (int o = 8; o > 0; o >>= 1)
-#pragma unroll
-        for (int i = 0; i < 4; ++i) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
-    const float app = v[0], aqq = v[1], xr = v[2], xi = v[3];
+    const float app = lo ? nX : nZ, aqq = lo ? nY : nW;
     const float absa2 = xr * xr + xi * xi;
-    float cs = 1.f, gr = 0.f, gi = 0.f;
-    int flags = 0;
-    if (absa2 > tol2 * app * aqq && absa2 > 0.f) {
-        flags = 1 | (absa2 > big2 * app * aqq ? 2 : 0);
-        const float inv = rsqrtf(absa2);
-        const float tau = (aqq - app) * (0.5f * inv);
-        const float at = fminf(fabsf(tau), 1e18f);
-        const float w1 = fmaf(at, at, 1.f);
-        const float t = copysignf(__fdividef(1.f, at + w1 * rsqrtf(w1)), tau);
-        const float x1 = fmaf(t, t, 1.f);
-        float c0 = rsqrtf(x1);
-        c0 = c0 * fmaf(-0.5f * x1, c0 * c0, 1.5f);           // one Newton step: c^2 + s^2 = 1 to rounding
-        cs = c0;
-        const float sn = t * cs;
-        gr = sn * xr * inv; gi = sn * xi * inv;
-    }
+    // Rotation that annihilates a:  with alpha = (|g_q|^2 - |g_p|^2) / 2 and r = sqrt(alpha^2 + |a|^2),
+    // c^2 = (1 + |alpha| / r) / 2 and g = sign(alpha) a / (2 r c)  (the inner rotation, tangent
+    // t = |g| / c <= 1): two dependent MUFU.RSQ.  c then takes one Newton step towards
+    // sqrt(1 - |g|^2) with the residual 1 - c^2 - |g|^2 formed around zero (not around 1, where the
+    // change of binade biases the rounding), so the rotation is unitary to rounding, without bias,
+    // whatever the error of the two approximate reciprocal square roots.  Branch-free: a pair below
+    // the tolerance gets c = 1, g = 0.
+    const float pq = app * aqq;
+    const bool rot = absa2 > tol2 * pq && absa2 > 0.f;
+    const float alpha = 0.5f * (aqq - app);
+    const float rinv = rsqrtf(fmaxf(fmaf(alpha, alpha, absa2), 1e-37f));
+    const float c2h = fmaf(0.5f * fabsf(alpha), rinv, 0.5f);         // c^2, in [0.5, 1]
+    const float rc = rsqrtf(c2h);                                     // 1 / c
+    const float cs0 = c2h * rc;
+    const float kk = rot ? copysignf(0.5f * rinv * rc, alpha) : 0.f; // g = kk a
+    const float gr = kk * xr, gi = kk * xi;
+    const float resid = fmaf(-cs0, cs0, 1.f) - fmaf(gr, gr, gi * gi);
+    const float cs = rot ? fmaf(0.5f * rc, resid, cs0) : 1.f;
+    const float d = kk * absa2 * rc;                                 // t |a|,  t = |g| / c
+    int flags = rot ? (1 | (absa2 > big2 * pq ? 2 : 0)) : 0;
+    if (app - d < 0.25f * app || aqq + d < 0.25f * aqq) flags |= 4;
     // each half computed one rotation; swap so that every lane has both
-    const float ocs = __shfl_xor_sync(0xffffffffu, cs, 16), ogr = __shfl_xor_sync(0xffffffffu, gr, 16), ogi = __shfl_xor_sync(0xffffffffu, gi, 16);
-    const float c1 = lo ? cs : ocs, r1 = lo ? gr : ogr, i1 = lo ? gi : ogi;     // rotation of (X, Y)
-    const float c2_ = lo ? ocs : cs, r2_ = lo ? ogr : gr, i2_ = lo ? ogi : gi;  // rotation of (Z, W)
+    const float ocs = __shfl_xor_sync(0xffffffffu, cs, 16), ogr = __shfl_xor_sync(0xffffffffu, gr, 16);
+    const float ogi = __shfl_xor_sync(0xffffffffu, gi, 16), od = __shfl_xor_sync(0xffffffffu, d, 16);
+    const float c1 = lo ? cs : ocs, r1 = lo ? gr : ogr, i1 = lo ? gi : ogi, d1 = lo ? d : od;      // rotation of (X, Y)
+    const float c2_ = lo ? ocs : cs, r2_ = lo ? ogr : gr, i2_ = lo ? ogi : gi, d2 = lo ? od : d;   // rotation of (Z, W)
     auto apply = [](EcbCol& P, EcbCol& Q, float c, float gr_, float gi_) {
         const unsigned long long c2 = ecl_pack(c, c), g2 = ecl_pack(gr_, gr_), h2 = ecl_pack(gi_, gi_);
         const unsigned long long ng2 = ecl_pack(-gr_, -gr_), nh2 = ecl_pack(-gi_, -gi_);
@@ -444,7 +476,9 @@ __device__ __forceinline__ int ecb_round(EcbCol& X, EcbCol& Y, EcbCol& Z, EcbCol
     };
     apply(X, Y, c1, r1, i1);
     apply(Z, W, c2_, r2_, i2_);
-    return flags;
+    nX -= d1; nY += d1; nZ -= d2; nW += d2;
+    if (__any_sync(0xffffffffu, flags & 4)) ecb_norms4(X, Y, Z, W, lane, nX, nY, nZ, nW);
+    return flags & 3;
 }
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jacobi_cluster_block_kernel(EclArgs a) {
@@ -492,7 +526,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
     // consumed what this pair sent one step ahead, which this pair sends after reading its inputs.
     const int lo = gi > 0 ? gi - 1 : 0, hi = gi < n - 1 ? gi + 1 : n - 1;
     const int nloc = (int)((lo >= h) == (gi >= h)) + (int)((hi >= h) == (gi >= h));
-    const uint32_t txb = (uint32_t)(2 - nloc) * 64u * (uint32_t)nch;       // bytes of the blocks that arrive by st.async
+    const uint32_t txb = (uint32_t)(2 - nloc) * (64u * (uint32_t)nch + 8u);   // bytes of the blocks (+ two norms each) that arrive by st.async
     if (j < npl && lane == 0) {
         ecl_mbar_init(full_u32 + 8u * (uint32_t)j, 1u + (uint32_t)nloc);
         ecl_mbar_init(full_u32 + 8u * (uint32_t)(ECB_PL + j), 1u + (uint32_t)nloc);
@@ -535,9 +569,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                     B0.re = *reinterpret_cast<const ulonglong2*>(b0);          B0.im = *reinterpret_cast<const ulonglong2*>(b0 + LD);
                     B1.re = *reinterpret_cast<const ulonglong2*>(b0 + 2 * LD); B1.im = *reinterpret_cast<const ulonglong2*>(b0 + 3 * LD);
                 }
-                if (s == 0) fl |= ecb_round(A0, A1, B0, B1, lane, tol2, tol);     // inner pairs, once per sweep
-                fl |= ecb_round(A0, B0, A1, B1, lane, tol2, tol);
-                fl |= ecb_round(A0, B1, A1, B0, lane, tol2, tol);
+                // squared norms of the four columns: carried with the blocks (first padding row of the
+                // real plane), refreshed from the columns at the first block step of every sweep
+                float nA0, nA1, nB0, nB1;
+                if (s == 0) {
+                    ecb_norms4(A0, A1, B0, B1, lane, nA0, nA1, nB0, nB1);
+                    fl |= ecb_round_tracked(A0, A1, B0, B1, nA0, nA1, nB0, nB1, lane, tol2, tol);   // inner pairs, once per sweep
+                } else {
+                    const float* t0 = buf + ecb_slot(b, 0, j, 0, LD) + N;
+                    const float* b0 = buf + ecb_slot(b, 1, j, 0, LD) + N;
+                    nA0 = t0[0]; nA1 = t0[2 * LD]; nB0 = b0[0]; nB1 = b0[2 * LD];
+                }
+                fl |= ecb_round_tracked(A0, B0, A1, B1, nA0, nB0, nA1, nB1, lane, tol2, tol);
+                fl |= ecb_round_tracked(A0, B1, A1, B0, nA0, nB1, nA1, nB0, lane, tol2, tol);
                 const uint32_t mP = (Prem ? full_peer : full_u32) + 8u * (uint32_t)((b ^ 1) * ECB_PL + dPj);
                 const uint32_t mQ = (Qrem ? full_peer : full_u32) + 8u * (uint32_t)((b ^ 1) * ECB_PL + dQj);
                 if (rowok) {
@@ -554,6 +598,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                     } else {
                         ecl_st_local(aQ, B0.re); ecl_st_local(aQ + L4, B0.im); ecl_st_local(aQ + 2 * L4, B1.re); ecl_st_local(aQ + 3 * L4, B1.im);
                     }
+                }
+                if (lane == 0) {                                     // the norms travel with their columns
+                    const uint32_t nP = (Prem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dPt, dPj, 0, LD) + N) * 4u;
+                    const uint32_t nQ = (Qrem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dQt, dQj, 0, LD) + N) * 4u;
+                    const uint32_t L8 = (uint32_t)LD * 8u;
+                    if (Prem) { ecl_st_async_f32(nP, nA0, mP); ecl_st_async_f32(nP + L8, nA1, mP); }
+                    else { ecl_st_local_f32(nP, nA0); ecl_st_local_f32(nP + L8, nA1); }
+                    if (Qrem) { ecl_st_async_f32(nQ, nB0, mQ); ecl_st_async_f32(nQ + L8, nB1, mQ); }
+                    else { ecl_st_local_f32(nQ, nB0); ecl_st_local_f32(nQ + L8, nB1); }
                 }
                 __syncwarp();
                 if (lane == 0) {                                     // blocks stored in this CTA: arrive for the whole warp
