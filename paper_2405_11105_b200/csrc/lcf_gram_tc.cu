@@ -7,8 +7,13 @@
 // Every fp32 sample is split x = hi + lo (hi = x rounded to TF32, lo = x - hi exactly, read as TF32), so
 //   Re R = D0 + H + H^T      D0 = Rh Rh^T + Ih Ih^T        H = Rh Rl^T + Ih Il^T
 //   Im R = (G0 + L) - (G0 + L)^T     G0 = Rh Ih^T          L = Rh Il^T - Ih Rl^T
-// (the lo.lo products, 2^-22 of a term, are dropped).  Seven 128 x Np x 8 tcgen05.mma per 8 pixels
-// into four TMEM accumulators (4 x 128 columns = all 512).
+// (the lo.lo products, 2^-22 of a term, are dropped).  The operand tiles are stacked, [Rh | Rl] and
+// [Ih | Il] (hi rows, then the lo rows from row Np), so that three 128 x 2Np x 8 tcgen05.mma
+// and one 128 x Np x 8 per 8 pixels do the seven products:
+//   [D0 | H] += Rh^T [Rh | Rl]     [D0 | H] += Ih^T [Ih | Il]     [G0 | L] += Rh^T [Ih | Il]     L -= Ih^T Rl
+// (an MMA with N = 2Np reads its A tile once for two products: 44 KB instead of 56 KB of operands
+// per 8 pixels, and shared-memory bandwidth is what bounds this kernel).  Two TMEM accumulators of
+// 2Np columns at columns 0 and 256.
 //
 // Persistent CTAs (one per SM) walk a static, contiguous slice of the global list of 16-pixel
 // tiles (16 z-contiguous pixels of one window: one 128-byte row per frame), cut into segments at
@@ -21,7 +26,8 @@
 //   warps 12-19  accumulator drain (152 registers each): see below.
 // tcgen05 accumulates in fp32 with truncation (measured: 2^24 + 1.5 -> 2^24), a bias that grows
 // with the number of adds into a large running sum; D0 and G0 are therefore drained every
-// `group` tiles (128 pixels = 32 adds) into fp32 registers of the drain warps (round to nearest),
+// `group` tiles (128 pixels = 32 adds) into fp32 registers of the drain warps (round to nearest)
+// and zeroed there with tcgen05.st (the fused MMAs have one accumulate flag for D0 and H together),
 // H and L (2^-11 of the main terms) stay in TMEM for the whole segment.  Each segment ends by
 // writing four 128 x 128 fp32 partials; gram_tc_reduce_kernel sums a window's segments in fp64,
 // applies the (anti)symmetrisation above and writes the full Hermitian R_k.
@@ -46,9 +52,9 @@ constexpr int GTC_DRAIN_WARPS = 8;
 constexpr int GTC_FIRST_CONV = 4;            // warps 0-3: TMA producer, MMA issuer, two idle (one warpgroup)
 constexpr int GTC_FIRST_DRAIN = GTC_FIRST_CONV + GTC_CONV_WARPS;
 constexpr int GTC_THREADS = 32 * (GTC_FIRST_DRAIN + GTC_DRAIN_WARPS);
-constexpr int GTC_TILE_BYTES = GTC_RT * GTC_PX * 4;      // one operand tile: 8 KB
-constexpr int GTC_OP_BYTES = 4 * GTC_TILE_BYTES;         // Rh, Ih, Rl, Il
-constexpr int GTC_LBO = GTC_RT * 16;                     // next 4-pixel K chunk
+constexpr int GTC_PAIR_BYTES = 2 * GTC_RT * GTC_PX * 4;  // one stacked operand (hi rows, then lo rows from row Np): 16 KB
+constexpr int GTC_OP_BYTES = 2 * GTC_PAIR_BYTES;         // [Rh | Rl], [Ih | Il]
+constexpr int GTC_LBO = 2 * GTC_RT * 16;                 // next 4-pixel K chunk (256 rows of 16 bytes)
 constexpr int GTC_SBO = 128;                             // next 8-frame row group
 constexpr int GTC_TASKS = (4 * (GTC_RT / 32) + GTC_CONV_WARPS - 1) / GTC_CONV_WARPS;   // converter tasks per thread per tile
 
@@ -171,11 +177,12 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
         // =========================== MMA issuer ===========================
         // the whole warp runs the loop (uniform control flow); one elected lane issues
         {
-            const uint32_t idesc = make_idesc_tf32(GTC_RT, a.Np, false, false, false, false);
+            const uint32_t idesc2 = make_idesc_tf32(GTC_RT, 2 * a.Np, false, false, false, false);
             const uint32_t idesc_na = make_idesc_tf32(GTC_RT, a.Np, false, false, true, false);
-            const uint32_t tD0 = tmem, tG0 = tmem + 128, tH = tmem + 256, tL = tmem + 384;
-            // descriptor of operand tile 0, k-step 0 of stage 0; the others differ in the address field only
+            const uint32_t tDH = tmem, tGL = tmem + 256;   // [D0 | H] and [G0 | L], each Np + Np columns
+            // descriptor of the stacked operand [Rh | Rl], k-step 0 of stage 0; the others differ in the address field only
             const uint64_t desc0 = make_smem_desc(smem_u32(ops), GTC_LBO, GTC_SBO, SWZ_NONE);
+            const uint64_t lo_off = (uint64_t)((a.Np * 16) >> 4);
             uint32_t it = 0, gc = 0;
             for (int sg = seg0; sg < seg1; ++sg) {
                 const int nt = a.segs[sg].ntile;
@@ -191,21 +198,14 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
                         const uint64_t dst = desc0 + (uint64_t)((o * GTC_OP_BYTES) >> 4);
 #pragma unroll
                         for (int ks = 0; ks < GTC_PX / 8; ++ks) {
-                            const uint64_t dRh = dst + (uint64_t)((0 * GTC_TILE_BYTES + ks * 2 * GTC_LBO) >> 4);
-                            const uint64_t dIh = dst + (uint64_t)((1 * GTC_TILE_BYTES + ks * 2 * GTC_LBO) >> 4);
-                            const uint64_t dRl = dst + (uint64_t)((2 * GTC_TILE_BYTES + ks * 2 * GTC_LBO) >> 4);
-                            const uint64_t dIl = dst + (uint64_t)((3 * GTC_TILE_BYTES + ks * 2 * GTC_LBO) >> 4);
-                            const uint32_t accg = (group_first && ks == 0) ? 0u : 1u;   // D0, G0 restart per group
-                            const uint32_t accs = (t == 0 && ks == 0) ? 0u : 1u;        // H, L restart per segment
-                            {
-                                mma_tf32(tD0, dRh, dRh, idesc, accg);
-                                mma_tf32(tD0, dIh, dIh, idesc, 1u);
-                                mma_tf32(tG0, dRh, dIh, idesc, accg);
-                                mma_tf32(tH, dRh, dRl, idesc, accs);
-                                mma_tf32(tH, dIh, dIl, idesc, 1u);
-                                mma_tf32(tL, dRh, dIl, idesc, accs);
-                                mma_tf32(tL, dIh, dRl, idesc_na, 1u);
-                            }
+                            const uint64_t dR = dst + (uint64_t)((ks * 2 * GTC_LBO) >> 4);                    // [Rh | Rl]
+                            const uint64_t dI = dst + (uint64_t)((GTC_PAIR_BYTES + ks * 2 * GTC_LBO) >> 4);   // [Ih | Il]
+                            const uint32_t accs = (t == 0 && ks == 0) ? 0u : 1u;   // everything restarts per segment;
+                            // D0 and G0 are zeroed by the drain warps at group ends (a fused MMA has one flag)
+                            mma_tf32(tDH, dR, dR, idesc2, accs);                   // Rh^T [Rh | Rl]
+                            mma_tf32(tDH, dI, dI, idesc2, 1u);                     // Ih^T [Ih | Il]
+                            mma_tf32(tGL, dR, dI, idesc2, accs);                   // Rh^T [Ih | Il]
+                            mma_tf32(tGL + (uint32_t)a.Np, dI, dR + lo_off, idesc_na, 1u);   // L -= Ih^T Rl
                         }
                         mma_commit(&bars->opempty[o]);
                         if (group_last) mma_commit(&bars->accfull);
@@ -221,6 +221,7 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
         const int cw = warp - GTC_FIRST_CONV;         // 0..7
         // this thread's tasks per tile: (4-pixel chunk c4, frame fr); offsets are the same for every tile
         const int nwt = 4 * ((N + 31) / 32);          // warp tasks per tile: (4-pixel chunk, 32-frame block)
+        const uint32_t lo_bytes = (uint32_t)a.Np * 16u;
         const uint32_t raw_u32 = smem_u32(raw), ops_u32 = smem_u32(ops), wts_u32 = smem_u32(&bars->wts[0][0]);
         bool tvalid[GTC_TASKS];
         uint32_t twt[GTC_TASKS], trd0[GTC_TASKS], trd1[GTC_TASKS], tdst[GTC_TASKS];
@@ -233,7 +234,7 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
             twt[j] = (uint32_t)c4 * 32u;
             trd0[j] = (uint32_t)fr * 128u + ((((uint32_t)(2 * c4)) ^ sw) << 4);
             trd1[j] = (uint32_t)fr * 128u + ((((uint32_t)(2 * c4 + 1)) ^ sw) << 4);
-            tdst[j] = (uint32_t)c4 * GTC_LBO + (uint32_t)fr * 16u;
+            tdst[j] = (uint32_t)c4 * GTC_LBO + (uint32_t)fr * 16u;      // hi row; the lo row is Np rows further
         }
         uint32_t it = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
@@ -267,10 +268,10 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
                             l[q] = sub2(v[q], h[q]);            // exact; the tensor core truncates it to TF32
                         }
                         const uint32_t dst = os + tdst[j];
-                        sts128(dst + 0 * GTC_TILE_BYTES, make_float4(h[0].x, h[1].x, h[2].x, h[3].x));
-                        sts128(dst + 1 * GTC_TILE_BYTES, make_float4(h[0].y, h[1].y, h[2].y, h[3].y));
-                        sts128(dst + 2 * GTC_TILE_BYTES, make_float4(l[0].x, l[1].x, l[2].x, l[3].x));
-                        sts128(dst + 3 * GTC_TILE_BYTES, make_float4(l[0].y, l[1].y, l[2].y, l[3].y));
+                        sts128(dst, make_float4(h[0].x, h[1].x, h[2].x, h[3].x));
+                        sts128(dst + GTC_PAIR_BYTES, make_float4(h[0].y, h[1].y, h[2].y, h[3].y));
+                        sts128(dst + lo_bytes, make_float4(l[0].x, l[1].x, l[2].x, l[3].x));
+                        sts128(dst + GTC_PAIR_BYTES + lo_bytes, make_float4(l[0].y, l[1].y, l[2].y, l[3].y));
                     }
                 fence_proxy_async_smem();             // this lane's operand writes -> async proxy
                 __syncwarp();
@@ -301,14 +302,23 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
                 tc_fence_after_sync();
 #pragma unroll
                 for (int blk = 0; blk < 8; ++blk) {
-                    uint32_t v[16];
-                    const uint32_t col = (blk < 4 ? 0u : 128u) + half * 64 + (blk & 3) * 16;
-                    tmem_ld16(tlane + col, v);
-                    tmem_ld_wait();
+                    const int cj = half * 64 + (blk & 3) * 16;             // column inside D0 (blk < 4) / G0
+                    if (cj < a.Np) {
+                        uint32_t v[16];
+                        tmem_ld16(tlane + (blk < 4 ? 0u : 256u) + (uint32_t)cj, v);
+                        tmem_ld_wait();
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) acc[blk * 16 + j] += __uint_as_float(v[j]);
+                        for (int j = 0; j < 16; ++j) acc[blk * 16 + j] += __uint_as_float(v[j]);
+                    }
                 }
                 if (g + 1 < ngroups) {
+                    // the next group accumulates onto zeros again (H and L next to them keep running)
+#pragma unroll
+                    for (int blk = 0; blk < 8; ++blk) {
+                        const int cj = half * 64 + (blk & 3) * 16;
+                        if (cj < a.Np) tmem_st16_zero(tlane + (blk < 4 ? 0u : 256u) + (uint32_t)cj);
+                    }
+                    tmem_st_wait();
                     tc_fence_before_sync();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&bars->accempty);   // one arrival per drain warp
@@ -328,16 +338,18 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
             for (int i = 0; i < 128; ++i) acc[i] = 0.f;
 #pragma unroll
             for (int blk = 0; blk < 8; ++blk) {
-                uint32_t v[16];
-                const int m = 2 + (blk >> 2);
-                const uint32_t col = (uint32_t)m * 128u + half * 64 + (blk & 3) * 16;
-                tmem_ld16(tlane + col, v);
-                tmem_ld_wait();
-                float* o2 = out + (size_t)m * 128 * 128 + (blk & 3) * 16;
+                const int m = 2 + (blk >> 2);                              // partial 2 = H, 3 = L
+                const int cj = half * 64 + (blk & 3) * 16;
+                if (cj < a.Np) {
+                    uint32_t v[16];
+                    tmem_ld16(tlane + (blk < 4 ? 0u : 256u) + (uint32_t)(a.Np + cj), v);
+                    tmem_ld_wait();
+                    float* o2 = out + (size_t)m * 128 * 128 + (blk & 3) * 16;
 #pragma unroll
-                for (int j = 0; j < 16; j += 4)
-                    *reinterpret_cast<float4*>(o2 + j) = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]),
-                                                                     __uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
+                    for (int j = 0; j < 16; j += 4)
+                        *reinterpret_cast<float4*>(o2 + j) = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]),
+                                                                         __uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
+                }
             }
             tc_fence_before_sync();
             __syncwarp();
