@@ -109,6 +109,7 @@ struct lcf_plan {
     float* ptc_part_d = nullptr;            // [NB][sum_k P_k]
     alignas(64) unsigned char ptc_tmap[128];
     const void* ptc_tmap_iq = nullptr;
+    uint32_t* amax_d = nullptr;             // bits of max |re|, |im| over the ensemble (tensor-core paths scale by a power of two)
     // EVD
     void* rotlog_d = nullptr;  // [K][max_sweeps*(Ns-1)][3][NP] real
     double* lam_d = nullptr;   // [K][N] descending
@@ -176,4 +177,5 @@ cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st);
 bool project_tc_eligible(const lcf_plan* p);
 cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::vector<int>& cta_first);
 cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st);
+cudaError_t launch_absmax(lcf_plan* p, const float2* iq, cudaStream_t st);
 }  // namespace lcf

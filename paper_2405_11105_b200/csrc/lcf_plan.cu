@@ -65,7 +65,7 @@ void free_plan_device(lcf_plan* p) {
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (int i = 0; i < 2; ++i) { if (p->ev_copied[i]) cudaEventDestroy(p->ev_copied[i]); if (p->ev_done[i]) cudaEventDestroy(p->ev_done[i]); }
     cudaFree(p->ec_gfac_d); cudaFree(p->ec_shift_d);
-    cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d);
+    cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d); cudaFree(p->amax_d);
     cudaFree(p->gtc_segs_d); cudaFree(p->gtc_cta_first_d); cudaFree(p->gtc_seg_first_d); cudaFree(p->gtc_part_d);
     if (p->timer.have)
         for (auto& set : p->timer.ev)
@@ -259,9 +259,10 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     if (p->evd_cluster) ok = ok && dev_alloc(&p->ec_gfac_d, K * 2 * Ns * (size_t)p->ec_LD) && dev_alloc(&p->ec_shift_d, K);
     if (p->proj_tc) {
         ok = ok && dev_upload(&p->ptc_segs_d, ptc_segs) && dev_upload(&p->ptc_cta_first_d, ptc_cta_first) &&
-             dev_alloc(&p->ptc_bpack_d, K * p->ptc_NB * (size_t)(p->ptc_Kp / 4) * 1024) &&
+             dev_alloc(&p->ptc_bpack_d, K * p->ptc_NB * (size_t)(p->ptc_Kp / 8) * 1024) &&
              dev_alloc(&p->ptc_part_d, (size_t)p->ptc_NB * (size_t)(p->sumPk ? p->sumPk : 1));
     }
+    if (p->gram_tc || p->proj_tc) ok = ok && dev_alloc(&p->amax_d, 1);
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->R_d), K * N2 * 2 * p->esz);
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->rotlog_d), K * p->max_sweeps * M * 3 * p->NP * p->esz);
     ok = ok && dev_alloc(&p->lam_d, K * N) && dev_alloc(&p->order_d, K * N) && dev_alloc(&p->cut_d, K) &&
@@ -310,6 +311,7 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     int stage = 0;
     auto run = [&](int id, cudaError_t r) { if (e == cudaSuccess && r != cudaSuccess) { e = r; stage = id; } };
     mark(0);
+    if (e == cudaSuccess && (p->gram_tc || p->proj_tc)) run(1, launch_absmax(p, iq, st));
     if (e == cudaSuccess) run(1, p->gram_tc ? launch_gram_tc(p, iq, st) : launch_gram(p, iq, st));
     mark(1);
     if (e == cudaSuccess) run(2, p->evd_chol ? launch_evd_chol(p, st, p->evd_cluster) : launch_jacobi(p, st));

@@ -7,26 +7,31 @@
 // (m = 2p: Re S, m = 2p+1: Im S), K = frames, and one CTA works on a block of 64 eigen-columns u
 // whose operand tile stays resident in shared memory for a whole segment:
 //   B tile rows  [0,64) Re B hi   [64,128) Im B hi   [128,192) Re B lo   [192,256) Im B lo
-//   D[:, 0:256] += A_hi * B[0:256]^T        D[:, 0:128] += A_lo * B[0:128]^T        (two MMAs / 8 frames)
+//   D[:, 0:256] += A_hi * B[0:256]^T        D[:, 0:128] += A_lo * B[0:128]^T        (two MMAs / 16 frames)
 //   P_r[m][u] = D[m][u] + D[m][128+u] = X_m . Re B_u      P_i[m][u] = D[m][64+u] + D[m][192+u]
 //   U_r = P_r[2p] - P_i[2p+1]      U_i = P_i[2p] + P_r[2p+1]
-// (hi = x rounded to TF32, lo = x - hi; the lo.lo products, 2^-22 of a term, are dropped).  Stacking
-// B hi over B lo makes one N = 256 MMA do two of the three products: the MMA reads 12 KB instead of
-// 16 KB of shared memory, which is what bounds these kernels (lcf_gram_tc.cu).
+// Split precision on the FP16 tensor path (.kind::f16, twice the TF32 rate and half the operand
+// bytes): every fp32 value x, scaled by a power of two, is hi + lo with hi = fp16(x) and
+// lo = fp16(x - hi), 22 significant bits together; the products hi.hi + hi.lo + lo.hi are
+// accumulated in fp32 and the lo.lo term (2^-22 of a term) is dropped.  The data are scaled so that
+// max |S| lands in [256, 512) (absmax_kernel), B (entries <= 1 in modulus) by 256: lo then stays a
+// normal fp16 number down to 2^-9 of the maximum and an absolute 2^-25 of it below.  Stacking B hi
+// over B lo makes one N = 256 MMA do two of the three products.
 //
 // Persistent CTAs walk a static slice of the list of (window, column block, 64-pixel tile) jobs,
 // cut into segments at (window, block) changes.  Roles (512 threads):
 //   warp 0      producer: the segment's packed B block (one bulk copy), then per 16 frames one TMA
 //               box [16 frames][4 x][16 z] complex64 -> raw stage (no swizzle: rows of 512 bytes);
 //   warp 1      MMA issuer (uniform control flow, one elected lane);
-//   warps 4-11  converters: raw [t][m] -> K-major A_hi / A_lo tiles (the transposition happens in
-//               registers: 4 frames of one row = one 16-byte core-matrix row);
+//   warps 4-11  converters: raw [t][m] -> K-major fp16 A_hi / A_lo tiles (the transposition happens in
+//               registers: 8 frames of one row = one 16-byte core-matrix row);
 //   warps 12-15 epilogue: TMEM -> registers, pair exchange by shuffle, |U|^2 summed over the 64
 //               columns, times w^2, one float per (block, pixel); two accumulator buffers so the
 //               epilogue of a tile overlaps the MMAs of the next.
 // proj_tc_pack_kernel builds the B blocks from B_k; proj_tc_finish_kernel adds the column blocks
 // into the per-window PD tiles and the per-chunk sums that the alpha / combine kernels use.
 #include <cuda.h>
+#include <cuda_fp16.h>
 
 #include "lcf_internal.h"
 #include "lcf_sm100.cuh"
@@ -39,25 +44,28 @@ constexpr int PTC_TZ = 16, PTC_TX = 4;                     // pixel tile: 16 z x
 constexpr int PTC_ROWS = 128;
 constexpr int PTC_KC = 16;                                 // frames per A stage
 constexpr int PTC_UB = 64;                                 // eigen-columns per block
-constexpr int PTC_RAW_STAGES = 4, PTC_OP_STAGES = 3;
-constexpr int PTC_RAW_BYTES = PTC_KC * PTC_ROWS * 4;       // 8 KB
-constexpr int PTC_A_BYTES = PTC_KC * PTC_ROWS * 4;         // one of A_hi / A_lo per stage: 8 KB
+constexpr int PTC_RAW_STAGES = 6, PTC_OP_STAGES = 6;
+constexpr int PTC_RAW_BYTES = PTC_KC * PTC_ROWS * 4;       // 8 KB of fp32
+constexpr int PTC_A_BYTES = PTC_KC * PTC_ROWS * 2;         // one of A_hi / A_lo per stage: 4 KB of fp16
 constexpr int PTC_OP_BYTES = 2 * PTC_A_BYTES;
-constexpr int PTC_A_LBO = PTC_ROWS * 16;                   // 2048: next 4-frame chunk of A
-constexpr int PTC_B_LBO = 256 * 16;                        // 4096: next 4-frame chunk of B
+constexpr int PTC_A_LBO = PTC_ROWS * 16;                   // 2048: next 8-frame chunk of A
+constexpr int PTC_B_LBO = 256 * 16;                        // 4096: next 8-frame chunk of B
+constexpr int PTC_B_SMEM = (128 / 8) * PTC_B_LBO;          // resident B block: 64 KB
 constexpr int PTC_SBO = 128;
+constexpr float PTC_B_SCALE = 256.f;
 constexpr int PTC_CONV_WARPS = 8, PTC_EPI_WARPS = 4;
 constexpr int PTC_FIRST_CONV = 4, PTC_FIRST_EPI = PTC_FIRST_CONV + PTC_CONV_WARPS;
 constexpr int PTC_THREADS = 32 * (PTC_FIRST_EPI + PTC_EPI_WARPS);
 
 struct PtcArgs {
-    int N, Kp, Nz, Nx;             // Kp = N rounded up to 8 frames
+    int N, Kp, Nz, Nx;             // Kp = N rounded up to 16 frames
     const double* gz;              // [Kz][Nz]
     const double* gx;              // [Kx][Nx]
     const WinBox* box;
     const PtcSeg* segs;
     const int* cta_first;          // [grid+1]
-    const float* bpack;            // [K][NB][Kp/4][256][4]
+    const float* bpack;            // [K][NB][Kp/8][256][8] fp16 (pointer in float units: 1024 floats per chunk)
+    const uint32_t* amax;          // bits of max |S|
     int NB;
     float* part;                   // [NB][sum_k P_k]
     long long sumPk;
@@ -79,15 +87,32 @@ __device__ __forceinline__ float ptc_lds32(uint32_t addr) {
 __device__ __forceinline__ void ptc_sts128(uint32_t addr, float x, float y, float z, float w) {
     asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
 }
-// x rounded to TF32, nearest with ties away (so the remainder x - hi is a signed 12-bit quantity)
-__device__ __forceinline__ float ptc_rna(float v) { return __uint_as_float((__float_as_uint(v) + 0x1000u) & 0xFFFFE000u); }
+__device__ __forceinline__ void ptc_sts128u(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+// (a, b) -> packed fp16 pairs hi = fp16(x), lo = fp16(x - hi); the lower half holds a
+__device__ __forceinline__ void ptc_split(float a, float b, uint32_t& hi, uint32_t& lo) {
+    const __half2 h = __floats2half2_rn(a, b);
+    const float2 hf = __half22float2(h);
+    const __half2 l = __floats2half2_rn(a - hf.x, b - hf.y);
+    hi = *reinterpret_cast<const uint32_t*>(&h);
+    lo = *reinterpret_cast<const uint32_t*>(&l);
+}
+// power of two that brings the ensemble's largest |re|, |im| into [256, 512)
+__host__ __device__ __forceinline__ int ptc_scale_exp(uint32_t amax_bits) {
+    const int ex = (int)((amax_bits >> 23) & 0xffu);
+    if (ex == 0 || ex == 255) return 0;
+    int k = 8 - (ex - 127);
+    return k < -100 ? -100 : (k > 100 ? 100 : k);
+}
+__device__ __forceinline__ float ptc_scale(uint32_t amax_bits) { return __uint_as_float((uint32_t)(127 + ptc_scale_exp(amax_bits)) << 23); }
 
 __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid_constant__ CUtensorMap tmap, PtcArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
-    unsigned char* bsm = sbase;                                               // resident B block (<= 128 KB)
-    unsigned char* raw = sbase + 32 * 4096;                                   // [RAW_STAGES][8 KB]
-    unsigned char* ops = raw + PTC_RAW_STAGES * PTC_RAW_BYTES;                // [OP_STAGES][A_hi 8 KB | A_lo 8 KB]
+    unsigned char* bsm = sbase;                                               // resident B block (<= 64 KB)
+    unsigned char* raw = sbase + PTC_B_SMEM;                                  // [RAW_STAGES][8 KB]
+    unsigned char* ops = raw + PTC_RAW_STAGES * PTC_RAW_BYTES;                // [OP_STAGES][A_hi 4 KB | A_lo 4 KB]
     PtcBars* bars = reinterpret_cast<PtcBars*>(ops + PTC_OP_STAGES * PTC_OP_BYTES);
     double* gzs = reinterpret_cast<double*>(bars + 1);                        // [Nz] window table rows (epilogue only)
     double* gxs = gzs + a.Nz;                                                 // [Nx]
@@ -95,8 +120,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int seg0 = a.cta_first[blockIdx.x], seg1 = a.cta_first[blockIdx.x + 1];
     const int nst = (a.Kp + PTC_KC - 1) / PTC_KC;          // A stages per tile
-    const int nks_total = a.Kp / 8;                        // 8-frame MMA steps per tile
-    const uint32_t bbytes = (uint32_t)(a.Kp / 4) * 4096u;
+    const uint32_t bbytes = (uint32_t)(a.Kp / 8) * 4096u;
 
     if (tid == 0) {
         for (int s = 0; s < PTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], PTC_CONV_WARPS); }
@@ -124,7 +148,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
             if (sg > seg0) mbar_wait(&bars->bfree, (uint32_t)(sg - seg0 - 1) & 1);   // MMAs of the old block done
             if (lane == 0) {
                 mbar_arrive_expect_tx(&bars->bfull, bbytes);
-                bulk_load(bsm, a.bpack + ((size_t)seg.k * a.NB + seg.b) * (size_t)(a.Kp / 4) * 1024, bbytes, &bars->bfull);
+                bulk_load(bsm, a.bpack + ((size_t)seg.k * a.NB + seg.b) * (size_t)(a.Kp / 8) * 1024, bbytes, &bars->bfull);
             }
             for (int t = 0; t < seg.ntile; ++t) {
                 const int tau = seg.tile0 + t;
@@ -142,8 +166,8 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
-        const uint32_t idesc256 = make_idesc_tf32(PTC_ROWS, 256, false, false, false, false);
-        const uint32_t idesc128 = make_idesc_tf32(PTC_ROWS, 128, false, false, false, false);
+        const uint32_t idesc256 = make_idesc_f16(PTC_ROWS, 256, false, false);
+        const uint32_t idesc128 = make_idesc_f16(PTC_ROWS, 128, false, false);
         const uint64_t descA0 = make_smem_desc(smem_u32(ops), PTC_A_LBO, PTC_SBO, SWZ_NONE);
         const uint64_t descB0 = make_smem_desc(smem_u32(bsm), PTC_B_LBO, PTC_SBO, SWZ_NONE);
         uint32_t it = 0, tl = 0;
@@ -159,14 +183,11 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                     mbar_wait(&bars->opfull[o], (it / PTC_OP_STAGES) & 1);
                     tc_fence_after_sync();
                     if (elect_one()) {
-                        const int nks = nks_total - 2 * st < 2 ? nks_total - 2 * st : 2;
-                        for (int ks = 0; ks < nks; ++ks) {
-                            const uint64_t dAh = descA0 + (uint64_t)((o * PTC_OP_BYTES + ks * 2 * PTC_A_LBO) >> 4);
-                            const uint64_t dAl = dAh + (uint64_t)(PTC_A_BYTES >> 4);
-                            const uint64_t dB = descB0 + (uint64_t)(((2 * st + ks) * 2 * PTC_B_LBO) >> 4);
-                            mma_tf32(tD, dAh, dB, idesc256, (st == 0 && ks == 0) ? 0u : 1u);
-                            mma_tf32(tD, dAl, dB, idesc128, 1u);
-                        }
+                        const uint64_t dAh = descA0 + (uint64_t)((o * PTC_OP_BYTES) >> 4);
+                        const uint64_t dAl = dAh + (uint64_t)(PTC_A_BYTES >> 4);
+                        const uint64_t dB = descB0 + (uint64_t)((st * 2 * PTC_B_LBO) >> 4);
+                        mma_f16(tD, dAh, dB, idesc256, st == 0 ? 0u : 1u);
+                        mma_f16(tD, dAl, dB, idesc128, 1u);
                         mma_commit(&bars->opempty[o]);
                         if (st + 1 == nst) mma_commit(&bars->accfull[buf]);
                     }
@@ -180,14 +201,11 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
         // =========================== converters ===========================
         const int cw = warp - PTC_FIRST_CONV;
         const uint32_t raw_u32 = smem_u32(raw), ops_u32 = smem_u32(ops);
-        uint32_t trd[2], tdst[2];
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            const int wt = cw + j * PTC_CONV_WARPS;        // 16 warp tasks: (4-frame chunk c4, 32-row block)
-            const int c4 = wt & 3, m = (wt >> 2) * 32 + lane;
-            trd[j] = (uint32_t)(4 * c4) * (PTC_ROWS * 4) + (uint32_t)m * 4u;
-            tdst[j] = (uint32_t)c4 * PTC_A_LBO + (uint32_t)m * 16u;
-        }
+        // 8 warp tasks per stage: (8-frame chunk c8, 32-row block); this warp's task is fixed
+        const int c8 = cw & 1, m = (cw >> 1) * 32 + lane;
+        const uint32_t trd = (uint32_t)(8 * c8) * (PTC_ROWS * 4) + (uint32_t)m * 4u;
+        const uint32_t tdst = (uint32_t)c8 * PTC_A_LBO + (uint32_t)m * 16u;
+        const float scale = ptc_scale(*a.amax);
         uint32_t it = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
             const int nstages = a.segs[sg].ntile * nst;
@@ -195,20 +213,15 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                 const int s = it % PTC_RAW_STAGES, o = it % PTC_OP_STAGES;
                 const uint32_t rs = raw_u32 + (uint32_t)s * PTC_RAW_BYTES, os = ops_u32 + (uint32_t)o * PTC_OP_BYTES;
                 mbar_wait(&bars->full[s], (it / PTC_RAW_STAGES) & 1);
-                float v[2][4];
+                float v[8];
 #pragma unroll
-                for (int j = 0; j < 2; ++j)
+                for (int i = 0; i < 8; ++i) v[i] = ptc_lds32(rs + trd + (uint32_t)i * (PTC_ROWS * 4)) * scale;
+                uint32_t h[4], l[4];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) v[j][i] = ptc_lds32(rs + trd[j] + (uint32_t)i * (PTC_ROWS * 4));
+                for (int i = 0; i < 4; ++i) ptc_split(v[2 * i], v[2 * i + 1], h[i], l[i]);
                 mbar_wait(&bars->opempty[o], ((it / PTC_OP_STAGES) & 1) ^ 1);
-#pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    float h[4], l[4];
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) { h[i] = ptc_rna(v[j][i]); l[i] = v[j][i] - h[i]; }
-                    ptc_sts128(os + tdst[j], h[0], h[1], h[2], h[3]);
-                    ptc_sts128(os + PTC_A_BYTES + tdst[j], l[0], l[1], l[2], l[3]);
-                }
+                ptc_sts128u(os + tdst, h[0], h[1], h[2], h[3]);
+                ptc_sts128u(os + PTC_A_BYTES + tdst, l[0], l[1], l[2], l[3]);
                 fence_proxy_async_smem();
                 __syncwarp();
                 if (lane == 0) {
@@ -223,6 +236,8 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
         const uint32_t tlane = tmem + ((uint32_t)(quad * 32) << 16);
         const int m = quad * 32 + lane;
         const int pix = m >> 1, xi = pix >> 4, zi = pix & 15;
+        // 1 / (data scale x B scale): exact power of two, applied to U before squaring
+        const float unscale = __uint_as_float((uint32_t)(127 - 8 - ptc_scale_exp(*a.amax)) << 23);
         uint32_t tl = 0;
         int curk = -1;
         for (int sg = seg0; sg < seg1; ++sg) {
@@ -261,7 +276,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                         const float pr = __uint_as_float(va[i]) + __uint_as_float(vc[i]);
                         const float pi = __uint_as_float(vb[i]) + __uint_as_float(vd[i]);
                         const float po = __shfl_xor_sync(0xffffffffu, pi, 1);
-                        const float val = (lane & 1) ? pr + po : pr - po;   // odd row: Im U, even row: Re U
+                        const float val = ((lane & 1) ? pr + po : pr - po) * unscale;   // odd row: Im U, even row: Re U
                         acc = fmaf(val, val, acc);
                     }
                 }
@@ -282,26 +297,48 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
 }
 
 // B_k [N][Ns] complex (row = frame, column = eigen slot) -> per (window, 64-column block) the
-// resident operand tile [Kp/4 chunks][256 rows][4 frames]: rows = Re hi | Im hi | Re lo | Im lo
+// resident fp16 operand tile [Kp/8 chunks][256 rows][8 frames]: rows = Re hi | Im hi | Re lo | Im lo of 256 B
 __global__ void proj_tc_pack_kernel(const float2* B, int N, int Ns, int Kp, int NB, float* bpack) {
     const int kb = blockIdx.x;                       // k * NB + b
     const int k = kb / NB, b = kb - k * NB;
     const float2* Bk = B + (size_t)k * N * Ns;
-    float* out = bpack + (size_t)kb * (Kp / 4) * 1024;
-    for (int e = threadIdx.x; e < (Kp / 4) * 256; e += blockDim.x) {
-        const int c4 = e >> 8, r = e & 255;
+    uint4* out = reinterpret_cast<uint4*>(bpack + (size_t)kb * (Kp / 8) * 1024);
+    for (int e = threadIdx.x; e < (Kp / 8) * 256; e += blockDim.x) {
+        const int c8 = e >> 8, r = e & 255;
         const int u = b * PTC_UB + (r & 63);
         const bool im = (r >> 6) & 1, lo = r >= 128;
-        float v[4];
+        float x[8];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int t = 4 * c4 + i;
-            float x = 0.f;
-            if (t < N && u < Ns) { const float2 c = Bk[(size_t)t * Ns + u]; x = im ? c.y : c.x; }
-            const float h = ptc_rna(x);
-            v[i] = lo ? x - h : h;
+        for (int i = 0; i < 8; ++i) {
+            const int t = 8 * c8 + i;
+            x[i] = 0.f;
+            if (t < N && u < Ns) { const float2 c = Bk[(size_t)t * Ns + u]; x[i] = (im ? c.y : c.x) * PTC_B_SCALE; }
         }
-        *reinterpret_cast<float4*>(out + (size_t)e * 4) = make_float4(v[0], v[1], v[2], v[3]);
+        uint32_t h[4], l[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) ptc_split(x[2 * i], x[2 * i + 1], h[i], l[i]);
+        out[e] = lo ? make_uint4(l[0], l[1], l[2], l[3]) : make_uint4(h[0], h[1], h[2], h[3]);
+    }
+}
+
+// bits of max(|re|, |im|) over the ensemble (non-negative floats order like their bit patterns)
+__global__ void absmax_kernel(const float4* x, size_t n4, const float* tail, int ntail, uint32_t* out) {
+    float m = 0.f;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+        const float4 v = __ldg(&x[i]);
+        m = fmaxf(fmaxf(m, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
+    }
+    if (blockIdx.x == 0 && (int)threadIdx.x < ntail) m = fmaxf(m, fabsf(tail[threadIdx.x]));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    __shared__ float ws[32];
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        m = threadIdx.x < (blockDim.x >> 5) ? ws[threadIdx.x] : 0.f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (threadIdx.x == 0 && m == m) atomicMax(out, __float_as_uint(m));
     }
 }
 
@@ -370,7 +407,7 @@ bool project_tc_eligible(const lcf_plan* p) {
 cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::vector<int>& cta_first) {
     const int K = p->K;
     p->ptc_NB = (p->Ns + PTC_UB - 1) / PTC_UB;
-    p->ptc_Kp = (p->N + 7) / 8 * 8;
+    p->ptc_Kp = (p->N + 15) / 16 * 16;
     const int NB = p->ptc_NB;
     std::vector<long long> pre((size_t)K * NB + 1, 0);
     for (int k = 0; k < K; ++k) {
@@ -397,7 +434,7 @@ cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::ve
     }
     cta_first[grid] = (int)segs.size();
     p->ptc_nseg = (int)segs.size();
-    p->ptc_smem = 1024 + 32 * 4096 + (size_t)PTC_RAW_STAGES * PTC_RAW_BYTES + (size_t)PTC_OP_STAGES * PTC_OP_BYTES + sizeof(PtcBars) + 16 +
+    p->ptc_smem = 1024 + PTC_B_SMEM + (size_t)PTC_RAW_STAGES * PTC_RAW_BYTES + (size_t)PTC_OP_STAGES * PTC_OP_BYTES + sizeof(PtcBars) + 16 +
                   (size_t)(p->Nz + p->Nx) * sizeof(double);
     if (p->ptc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
     return cudaFuncSetAttribute(project_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ptc_smem);
@@ -412,11 +449,21 @@ cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     PtcArgs a;
     a.N = p->N; a.Kp = p->ptc_Kp; a.Nz = p->Nz; a.Nx = p->Nx;
     a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->ptc_segs_d; a.cta_first = p->ptc_cta_first_d;
-    a.bpack = p->ptc_bpack_d; a.NB = p->ptc_NB; a.part = p->ptc_part_d; a.sumPk = p->sumPk;
+    a.bpack = p->ptc_bpack_d; a.amax = p->amax_d; a.NB = p->ptc_NB; a.part = p->ptc_part_d; a.sumPk = p->sumPk;
     project_tc_kernel<<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(*reinterpret_cast<const CUtensorMap*>(p->ptc_tmap), a);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     proj_tc_finish_kernel<<<p->n_pitems, PROJ_TPIX, 0, st>>>(p->ptc_part_d, p->sumPk, p->ptc_NB, p->box_d, p->pitems_d, p->tiles_d, p->tsum_d);
+    return cudaGetLastError();
+}
+
+// amax_d <- bits of the largest |re|, |im| of the ensemble (the tensor-core kernels scale by a power of two)
+cudaError_t launch_absmax(lcf_plan* p, const float2* iq, cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(p->amax_d, 0, sizeof(uint32_t), st);
+    if (e != cudaSuccess) return e;
+    const size_t nf = (size_t)p->N * p->P * 2, n4 = nf / 4;
+    absmax_kernel<<<p->num_sms * 4, 512, 0, st>>>(reinterpret_cast<const float4*>(iq), n4, reinterpret_cast<const float*>(iq) + n4 * 4,
+                                                   (int)(nf - n4 * 4), p->amax_d);
     return cudaGetLastError();
 }
 
