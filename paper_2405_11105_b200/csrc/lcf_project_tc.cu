@@ -44,7 +44,7 @@ constexpr int PTC_TZ = 16, PTC_TX = 4;                     // pixel tile: 16 z x
 constexpr int PTC_ROWS = 128;
 constexpr int PTC_KC = 16;                                 // frames per A stage
 constexpr int PTC_UB = 64;                                 // eigen-columns per block
-constexpr int PTC_RAW_STAGES = 6, PTC_OP_STAGES = 6;
+constexpr int PTC_RAW_STAGES = 8, PTC_OP_STAGES = 8;
 constexpr int PTC_RAW_BYTES = PTC_KC * PTC_ROWS * 4;       // 8 KB of fp32
 constexpr int PTC_A_BYTES = PTC_KC * PTC_ROWS * 2;         // one of A_hi / A_lo per stage: 4 KB of fp16
 constexpr int PTC_OP_BYTES = 2 * PTC_A_BYTES;
@@ -54,6 +54,9 @@ constexpr int PTC_B_SMEM = (128 / 8) * PTC_B_LBO;          // resident B block: 
 constexpr int PTC_SBO = 128;
 constexpr float PTC_B_SCALE = 256.f;
 constexpr int PTC_CONV_WARPS = 8, PTC_EPI_WARPS = 4;
+constexpr int PTC_CONV_GROUPS = 4;                         // converter groups working on alternate stages
+// a group must see every use of the stages it touches (an mbarrier waiter may not skip a phase)
+static_assert(PTC_RAW_STAGES % PTC_CONV_GROUPS == 0 && PTC_OP_STAGES % PTC_CONV_GROUPS == 0, "stages per group");
 constexpr int PTC_FIRST_CONV = 4, PTC_FIRST_EPI = PTC_FIRST_CONV + PTC_CONV_WARPS;
 constexpr int PTC_THREADS = 32 * (PTC_FIRST_EPI + PTC_EPI_WARPS);
 
@@ -123,8 +126,8 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
     const uint32_t bbytes = (uint32_t)(a.Kp / 8) * 4096u;
 
     if (tid == 0) {
-        for (int s = 0; s < PTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], PTC_CONV_WARPS); }
-        for (int s = 0; s < PTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], PTC_CONV_WARPS); mbar_init(&bars->opempty[s], 1); }
+        for (int s = 0; s < PTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], PTC_CONV_WARPS / PTC_CONV_GROUPS); }
+        for (int s = 0; s < PTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], PTC_CONV_WARPS / PTC_CONV_GROUPS); mbar_init(&bars->opempty[s], 1); }
         for (int b = 0; b < 2; ++b) { mbar_init(&bars->accfull[b], 1); mbar_init(&bars->accempty[b], PTC_EPI_WARPS); }
         mbar_init(&bars->bfull, 1);
         mbar_init(&bars->bfree, 1);
@@ -201,27 +204,44 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
         // =========================== converters ===========================
         const int cw = warp - PTC_FIRST_CONV;
         const uint32_t raw_u32 = smem_u32(raw), ops_u32 = smem_u32(ops);
-        // 8 warp tasks per stage: (8-frame chunk c8, 32-row block); this warp's task is fixed
-        const int c8 = cw & 1, m = (cw >> 1) * 32 + lane;
-        const uint32_t trd = (uint32_t)(8 * c8) * (PTC_ROWS * 4) + (uint32_t)m * 4u;
-        const uint32_t tdst = (uint32_t)c8 * PTC_A_LBO + (uint32_t)m * 16u;
+        // 8 warp tasks per stage: (8-frame chunk c8, 32-row block).  The converter warps form
+        // PTC_CONV_GROUPS groups that take alternate stages (a warp does 8 / warps-per-group tasks of its
+        // stage), so the load -> convert -> store -> fence latency of one stage overlaps the next.
+        constexpr int WPG = PTC_CONV_WARPS / PTC_CONV_GROUPS, TPW = 8 / WPG;    // warps per group, tasks per warp
+        const int grp = cw / WPG, gw = cw % WPG;
+        uint32_t trd[TPW], tdst[TPW];
+#pragma unroll
+        for (int j = 0; j < TPW; ++j) {
+            const int wt = gw + j * WPG;
+            const int c8 = wt & 1, m = (wt >> 1) * 32 + lane;
+            trd[j] = (uint32_t)(8 * c8) * (PTC_ROWS * 4) + (uint32_t)m * 4u;
+            tdst[j] = (uint32_t)c8 * PTC_A_LBO + (uint32_t)m * 16u;
+        }
         const float scale = ptc_scale(*a.amax);
         uint32_t it = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
             const int nstages = a.segs[sg].ntile * nst;
             for (int q = 0; q < nstages; ++q, ++it) {
+                if ((int)(it % PTC_CONV_GROUPS) != grp) continue;
                 const int s = it % PTC_RAW_STAGES, o = it % PTC_OP_STAGES;
                 const uint32_t rs = raw_u32 + (uint32_t)s * PTC_RAW_BYTES, os = ops_u32 + (uint32_t)o * PTC_OP_BYTES;
                 mbar_wait(&bars->full[s], (it / PTC_RAW_STAGES) & 1);
-                float v[8];
+                float v[TPW][8];
 #pragma unroll
-                for (int i = 0; i < 8; ++i) v[i] = ptc_lds32(rs + trd + (uint32_t)i * (PTC_ROWS * 4)) * scale;
-                uint32_t h[4], l[4];
+                for (int j = 0; j < TPW; ++j)
 #pragma unroll
-                for (int i = 0; i < 4; ++i) ptc_split(v[2 * i], v[2 * i + 1], h[i], l[i]);
+                    for (int i = 0; i < 8; ++i) v[j][i] = ptc_lds32(rs + trd[j] + (uint32_t)i * (PTC_ROWS * 4)) * scale;
+                uint32_t h[TPW][4], l[TPW][4];
+#pragma unroll
+                for (int j = 0; j < TPW; ++j)
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) ptc_split(v[j][2 * i], v[j][2 * i + 1], h[j][i], l[j][i]);
                 mbar_wait(&bars->opempty[o], ((it / PTC_OP_STAGES) & 1) ^ 1);
-                ptc_sts128u(os + tdst, h[0], h[1], h[2], h[3]);
-                ptc_sts128u(os + PTC_A_BYTES + tdst, l[0], l[1], l[2], l[3]);
+#pragma unroll
+                for (int j = 0; j < TPW; ++j) {
+                    ptc_sts128u(os + tdst[j], h[j][0], h[j][1], h[j][2], h[j][3]);
+                    ptc_sts128u(os + PTC_A_BYTES + tdst[j], l[j][0], l[j][1], l[j][2], l[j][3]);
+                }
                 fence_proxy_async_smem();
                 __syncwarp();
                 if (lane == 0) {
