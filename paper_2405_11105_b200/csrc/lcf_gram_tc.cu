@@ -4,15 +4,17 @@
 //   R_k[i][j] = sum_p w_k(p)^2 conj(S[i][p]) S[j][p]            X = W_k S (Eq. 11), X = Xr + i Xi
 //   Re R = Xr Xr^T + Xi Xi^T          Im R = G - G^T,  G = Xr Xi^T          (frames x frames, K = pixels)
 //
-// Every fp32 sample is split x = hi + lo (hi = x rounded to TF32, lo = x - hi exactly, read as TF32), so
+// Every fp32 sample of X, scaled by a power of two so that max |S| lands in [256, 512)
+// (absmax_kernel), is split x = hi + lo with hi = fp16(x), lo = fp16(x - hi) (22 significant bits
+// together) for the FP16 tensor path (.kind::f16, K = 16 pixels = one tile per MMA), so
 //   Re R = D0 + H + H^T      D0 = Rh Rh^T + Ih Ih^T        H = Rh Rl^T + Ih Il^T
 //   Im R = (G0 + L) - (G0 + L)^T     G0 = Rh Ih^T          L = Rh Il^T - Ih Rl^T
 // (the lo.lo products, 2^-22 of a term, are dropped).  The operand tiles are stacked, [Rh | Rl] and
-// [Ih | Il] (hi rows, then the lo rows from row Np), so that three 128 x 2Np x 8 tcgen05.mma
-// and one 128 x Np x 8 per 8 pixels do the seven products:
+// [Ih | Il] (hi rows, then the lo rows from row Np), so that three 128 x 2Np x 16 tcgen05.mma
+// and one 128 x Np x 16 per 16 pixels do the seven products:
 //   [D0 | H] += Rh^T [Rh | Rl]     [D0 | H] += Ih^T [Ih | Il]     [G0 | L] += Rh^T [Ih | Il]     L -= Ih^T Rl
-// (an MMA with N = 2Np reads its A tile once for two products: 44 KB instead of 56 KB of operands
-// per 8 pixels, and shared-memory bandwidth is what bounds this kernel).  Two TMEM accumulators of
+// (an MMA with N = 2Np reads its A tile once for two products, and shared-memory bandwidth is what
+// bounds this kernel).  Two TMEM accumulators of
 // 2Np columns at columns 0 and 256.
 //
 // Persistent CTAs (one per SM) walk a static, contiguous slice of the global list of 16-pixel
@@ -52,11 +54,11 @@ constexpr int GTC_DRAIN_WARPS = 8;
 constexpr int GTC_FIRST_CONV = 4;            // warps 0-3: TMA producer, MMA issuer, two idle (one warpgroup)
 constexpr int GTC_FIRST_DRAIN = GTC_FIRST_CONV + GTC_CONV_WARPS;
 constexpr int GTC_THREADS = 32 * (GTC_FIRST_DRAIN + GTC_DRAIN_WARPS);
-constexpr int GTC_PAIR_BYTES = 2 * GTC_RT * GTC_PX * 4;  // one stacked operand (hi rows, then lo rows from row Np): 16 KB
+constexpr int GTC_PAIR_BYTES = 2 * GTC_RT * GTC_PX * 2;  // one stacked fp16 operand (hi rows, then lo rows from row Np): 8 KB
 constexpr int GTC_OP_BYTES = 2 * GTC_PAIR_BYTES;         // [Rh | Rl], [Ih | Il]
-constexpr int GTC_LBO = 2 * GTC_RT * 16;                 // next 4-pixel K chunk (256 rows of 16 bytes)
+constexpr int GTC_LBO = 2 * GTC_RT * 16;                 // next 8-pixel K chunk (256 rows of 16 bytes)
 constexpr int GTC_SBO = 128;                             // next 8-frame row group
-constexpr int GTC_TASKS = (4 * (GTC_RT / 32) + GTC_CONV_WARPS - 1) / GTC_CONV_WARPS;   // converter tasks per thread per tile
+constexpr int GTC_TASKS = (2 * (GTC_RT / 32) + GTC_CONV_WARPS - 1) / GTC_CONV_WARPS;   // converter tasks per thread per tile
 
 struct GtcArgs {
     int N, Np, Nz, Nx, Kz;
@@ -68,6 +70,7 @@ struct GtcArgs {
     const int* cta_first;      // [grid+1]
     float* part;               // [nseg][4][128][128]
     uint32_t raw_stride;       // bytes between raw stages (multiple of 1024)
+    const uint32_t* amax;      // bits of max |S| (power-of-two scaling of the fp16 operands)
 };
 
 struct GtcBars {
@@ -80,6 +83,10 @@ struct GtcBars {
 
 __device__ __forceinline__ void sts128(uint32_t addr, const float4& v) {
     asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
+__device__ __forceinline__ void sts128u(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
 
 __device__ __forceinline__ ulonglong2 lds128u(uint32_t addr) {
@@ -141,6 +148,7 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
     if (warp == 0) {
         // =========================== TMA producer ===========================
         if (lane == 0) tma_prefetch_desc(&tmap);
+        const double scale = (double)pow2f(pow2_scale_exp(*a.amax));   // folded into the window weights
         uint32_t it = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
             const GtcSeg seg = a.segs[sg];
@@ -163,7 +171,7 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
                 if (lane < GTC_PX) {
                     const int zz = z + lane;
                     float w = 0.f;
-                    if (zz < a.Nz && x < a.Nx) w = (float)(gzs[zz] * gxs[x]);
+                    if (zz < a.Nz && x < a.Nx) w = (float)(gzs[zz] * gxs[x] * scale);
                     bars->wts[s][2 * lane] = w; bars->wts[s][2 * lane + 1] = w;
                 }
                 __syncwarp();
@@ -177,8 +185,8 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
         // =========================== MMA issuer ===========================
         // the whole warp runs the loop (uniform control flow); one elected lane issues
         {
-            const uint32_t idesc2 = make_idesc_tf32(GTC_RT, 2 * a.Np, false, false, false, false);
-            const uint32_t idesc_na = make_idesc_tf32(GTC_RT, a.Np, false, false, true, false);
+            const uint32_t idesc2 = make_idesc_f16(GTC_RT, 2 * a.Np, false, false);
+            const uint32_t idesc_na = make_idesc_f16(GTC_RT, a.Np, true, false);
             const uint32_t tDH = tmem, tGL = tmem + 256;   // [D0 | H] and [G0 | L], each Np + Np columns
             // descriptor of the stacked operand [Rh | Rl], k-step 0 of stage 0; the others differ in the address field only
             const uint64_t desc0 = make_smem_desc(smem_u32(ops), GTC_LBO, GTC_SBO, SWZ_NONE);
@@ -196,17 +204,14 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
                     tc_fence_after_sync();
                     if (elect_one()) {
                         const uint64_t dst = desc0 + (uint64_t)((o * GTC_OP_BYTES) >> 4);
-#pragma unroll
-                        for (int ks = 0; ks < GTC_PX / 8; ++ks) {
-                            const uint64_t dR = dst + (uint64_t)((ks * 2 * GTC_LBO) >> 4);                    // [Rh | Rl]
-                            const uint64_t dI = dst + (uint64_t)((GTC_PAIR_BYTES + ks * 2 * GTC_LBO) >> 4);   // [Ih | Il]
-                            const uint32_t accs = (t == 0 && ks == 0) ? 0u : 1u;   // everything restarts per segment;
-                            // D0 and G0 are zeroed by the drain warps at group ends (a fused MMA has one flag)
-                            mma_tf32(tDH, dR, dR, idesc2, accs);                   // Rh^T [Rh | Rl]
-                            mma_tf32(tDH, dI, dI, idesc2, 1u);                     // Ih^T [Ih | Il]
-                            mma_tf32(tGL, dR, dI, idesc2, accs);                   // Rh^T [Ih | Il]
-                            mma_tf32(tGL + (uint32_t)a.Np, dI, dR + lo_off, idesc_na, 1u);   // L -= Ih^T Rl
-                        }
+                        const uint64_t dR = dst;                                           // [Rh | Rl], K = the tile's 16 pixels
+                        const uint64_t dI = dst + (uint64_t)(GTC_PAIR_BYTES >> 4);         // [Ih | Il]
+                        const uint32_t accs = (t == 0) ? 0u : 1u;   // everything restarts per segment;
+                        // D0 and G0 are zeroed by the drain warps at group ends (a fused MMA has one flag)
+                        mma_f16(tDH, dR, dR, idesc2, accs);                   // Rh^T [Rh | Rl]
+                        mma_f16(tDH, dI, dI, idesc2, 1u);                     // Ih^T [Ih | Il]
+                        mma_f16(tGL, dR, dI, idesc2, accs);                   // Rh^T [Ih | Il]
+                        mma_f16(tGL + (uint32_t)a.Np, dI, dR + lo_off, idesc_na, 1u);   // L -= Ih^T Rl
                         mma_commit(&bars->opempty[o]);
                         if (group_last) mma_commit(&bars->accfull);
                     }
@@ -220,21 +225,21 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
         asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
         const int cw = warp - GTC_FIRST_CONV;         // 0..7
         // this thread's tasks per tile: (4-pixel chunk c4, frame fr); offsets are the same for every tile
-        const int nwt = 4 * ((N + 31) / 32);          // warp tasks per tile: (4-pixel chunk, 32-frame block)
+        const int nwt = 2 * ((N + 31) / 32);          // warp tasks per tile: (8-pixel chunk, 32-frame block)
         const uint32_t lo_bytes = (uint32_t)a.Np * 16u;
         const uint32_t raw_u32 = smem_u32(raw), ops_u32 = smem_u32(ops), wts_u32 = smem_u32(&bars->wts[0][0]);
         bool tvalid[GTC_TASKS];
-        uint32_t twt[GTC_TASKS], trd0[GTC_TASKS], trd1[GTC_TASKS], tdst[GTC_TASKS];
+        uint32_t twt[GTC_TASKS], trd[GTC_TASKS][4], tdst[GTC_TASKS];
 #pragma unroll
         for (int j = 0; j < GTC_TASKS; ++j) {
             const int wt = cw + j * GTC_CONV_WARPS;
-            const int c4 = wt & 3, fr = (wt >> 2) * 32 + lane;
+            const int c8 = wt & 1, fr = (wt >> 1) * 32 + lane;
             tvalid[j] = wt < nwt && fr < N;
             const uint32_t sw = (uint32_t)(fr & 7);
-            twt[j] = (uint32_t)c4 * 32u;
-            trd0[j] = (uint32_t)fr * 128u + ((((uint32_t)(2 * c4)) ^ sw) << 4);
-            trd1[j] = (uint32_t)fr * 128u + ((((uint32_t)(2 * c4 + 1)) ^ sw) << 4);
-            tdst[j] = (uint32_t)c4 * GTC_LBO + (uint32_t)fr * 16u;      // hi row; the lo row is Np rows further
+            twt[j] = (uint32_t)c8 * 64u;                   // 8 pixels x (w, w)
+#pragma unroll
+            for (int u = 0; u < 4; ++u) trd[j][u] = (uint32_t)fr * 128u + ((((uint32_t)(4 * c8 + u)) ^ sw) << 4);
+            tdst[j] = (uint32_t)c8 * GTC_LBO + (uint32_t)fr * 16u;      // hi row; the lo row is Np rows further
         }
         uint32_t it = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
@@ -246,32 +251,32 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
                 const uint32_t os = ops_u32 + (uint32_t)o * GTC_OP_BYTES;
                 const uint32_t ws = wts_u32 + (uint32_t)s * (GTC_PX * 8);
                 mbar_wait(&bars->full[s], ph);
-                ulonglong2 wa[GTC_TASKS], wb[GTC_TASKS], p01[GTC_TASKS], p23[GTC_TASKS];
+                ulonglong2 wq[GTC_TASKS][4], pq[GTC_TASKS][4];
 #pragma unroll
                 for (int j = 0; j < GTC_TASKS; ++j)
                     if (tvalid[j]) {
-                        wa[j] = lds128u(ws + twt[j]);          // (w0, w0), (w1, w1)
-                        wb[j] = lds128u(ws + twt[j] + 16);     // (w2, w2), (w3, w3)
-                        p01[j] = lds128u(rs + trd0[j]);        // (re0, im0), (re1, im1)
-                        p23[j] = lds128u(rs + trd1[j]);
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            wq[j][u] = lds128u(ws + twt[j] + 16 * u);      // (w0, w0), (w1, w1) of pixels 2u, 2u+1 of the chunk
+                            pq[j][u] = lds128u(rs + trd[j][u]);            // (re0, im0), (re1, im1)
+                        }
                     }
                 mbar_wait(&bars->opempty[o], pho ^ 1);
 #pragma unroll
                 for (int j = 0; j < GTC_TASKS; ++j)
                     if (tvalid[j]) {
-                        float2 v[4], h[4], l[4];
-                        v[0] = mul2(p01[j].x, wa[j].x); v[1] = mul2(p01[j].y, wa[j].y);
-                        v[2] = mul2(p23[j].x, wb[j].x); v[3] = mul2(p23[j].y, wb[j].y);
+                        uint32_t rh[4], rl[4], ih[4], il[4];
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            h[q].x = rna_tf32(v[q].x); h[q].y = rna_tf32(v[q].y);
-                            l[q] = sub2(v[q], h[q]);            // exact; the tensor core truncates it to TF32
+                        for (int u = 0; u < 4; ++u) {
+                            const float2 v0 = mul2(pq[j][u].x, wq[j][u].x), v1 = mul2(pq[j][u].y, wq[j][u].y);
+                            f16_split2(v0.x, v1.x, rh[u], rl[u]);
+                            f16_split2(v0.y, v1.y, ih[u], il[u]);
                         }
                         const uint32_t dst = os + tdst[j];
-                        sts128(dst, make_float4(h[0].x, h[1].x, h[2].x, h[3].x));
-                        sts128(dst + GTC_PAIR_BYTES, make_float4(h[0].y, h[1].y, h[2].y, h[3].y));
-                        sts128(dst + lo_bytes, make_float4(l[0].x, l[1].x, l[2].x, l[3].x));
-                        sts128(dst + GTC_PAIR_BYTES + lo_bytes, make_float4(l[0].y, l[1].y, l[2].y, l[3].y));
+                        sts128u(dst, rh[0], rh[1], rh[2], rh[3]);
+                        sts128u(dst + GTC_PAIR_BYTES, ih[0], ih[1], ih[2], ih[3]);
+                        sts128u(dst + lo_bytes, rl[0], rl[1], rl[2], rl[3]);
+                        sts128u(dst + GTC_PAIR_BYTES + lo_bytes, il[0], il[1], il[2], il[3]);
                     }
                 fence_proxy_async_smem();             // this lane's operand writes -> async proxy
                 __syncwarp();
@@ -364,7 +369,7 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
 
 // R_k = sum over the window's segments, in fp64:  Re R = D0 + H + H^T,  Im R = (G0 + L) - (G0 + L)^T
 template <typename T>
-__global__ void gram_tc_reduce_kernel(const float* part, const int* seg_first, int N, void* Rv) {
+__global__ void gram_tc_reduce_kernel(const float* part, const int* seg_first, int N, const uint32_t* amax, void* Rv) {
     const int k = blockIdx.z;
     const int i = blockIdx.y * 16 + threadIdx.y, j = blockIdx.x * 16 + threadIdx.x;
     if (i >= N || j >= N) return;
@@ -376,6 +381,8 @@ __global__ void gram_tc_reduce_kernel(const float* part, const int* seg_first, i
         im += ((double)p[16384 + ij] - (double)p[16384 + ji]) + ((double)p[3 * 16384 + ij] - (double)p[3 * 16384 + ji]);
     }
     if (i == j) im = 0.0;
+    const double un = ldexp(1.0, -2 * pow2_scale_exp(*amax));   // the operands carried the power-of-two data scale
+    re *= un; im *= un;
     if (sizeof(T) == 4) {
         float2* R = reinterpret_cast<float2*>(Rv) + (size_t)k * N * N;
         R[(size_t)i * N + j] = make_float2((float)re, (float)im);
@@ -481,12 +488,12 @@ cudaError_t launch_gram_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     a.N = p->N; a.Np = (p->N + 15) / 16 * 16; a.Nz = p->Nz; a.Nx = p->Nx; a.Kz = p->Kz;
     a.group = p->gtc_group;
     a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->gtc_segs_d; a.cta_first = p->gtc_cta_first_d;
-    a.part = p->gtc_part_d; a.raw_stride = p->gtc_raw_stride;
+    a.part = p->gtc_part_d; a.raw_stride = p->gtc_raw_stride; a.amax = p->amax_d;
     gram_tc_kernel<<<p->gtc_grid, GTC_THREADS, p->gtc_smem, st>>>(*reinterpret_cast<const CUtensorMap*>(p->gtc_tmap), a);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     dim3 blk(16, 16), grid((p->N + 15) / 16, (p->N + 15) / 16, p->K);
-    gram_tc_reduce_kernel<float><<<grid, blk, 0, st>>>(p->gtc_part_d, p->gtc_seg_first_d, p->N, p->R_d);
+    gram_tc_reduce_kernel<float><<<grid, blk, 0, st>>>(p->gtc_part_d, p->gtc_seg_first_d, p->N, p->amax_d, p->R_d);
     return cudaGetLastError();
 }
 

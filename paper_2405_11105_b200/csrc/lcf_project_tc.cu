@@ -93,23 +93,6 @@ __device__ __forceinline__ void ptc_sts128(uint32_t addr, float x, float y, floa
 __device__ __forceinline__ void ptc_sts128u(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
-// (a, b) -> packed fp16 pairs hi = fp16(x), lo = fp16(x - hi); the lower half holds a
-__device__ __forceinline__ void ptc_split(float a, float b, uint32_t& hi, uint32_t& lo) {
-    const __half2 h = __floats2half2_rn(a, b);
-    const float2 hf = __half22float2(h);
-    const __half2 l = __floats2half2_rn(a - hf.x, b - hf.y);
-    hi = *reinterpret_cast<const uint32_t*>(&h);
-    lo = *reinterpret_cast<const uint32_t*>(&l);
-}
-// power of two that brings the ensemble's largest |re|, |im| into [256, 512)
-__host__ __device__ __forceinline__ int ptc_scale_exp(uint32_t amax_bits) {
-    const int ex = (int)((amax_bits >> 23) & 0xffu);
-    if (ex == 0 || ex == 255) return 0;
-    int k = 8 - (ex - 127);
-    return k < -100 ? -100 : (k > 100 ? 100 : k);
-}
-__device__ __forceinline__ float ptc_scale(uint32_t amax_bits) { return __uint_as_float((uint32_t)(127 + ptc_scale_exp(amax_bits)) << 23); }
-
 __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid_constant__ CUtensorMap tmap, PtcArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
@@ -217,7 +200,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
             trd[j] = (uint32_t)(8 * c8) * (PTC_ROWS * 4) + (uint32_t)m * 4u;
             tdst[j] = (uint32_t)c8 * PTC_A_LBO + (uint32_t)m * 16u;
         }
-        const float scale = ptc_scale(*a.amax);
+        const float scale = pow2f(pow2_scale_exp(*a.amax));
         uint32_t it = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
             const int nstages = a.segs[sg].ntile * nst;
@@ -235,7 +218,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
 #pragma unroll
                 for (int j = 0; j < TPW; ++j)
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) ptc_split(v[j][2 * i], v[j][2 * i + 1], h[j][i], l[j][i]);
+                    for (int i = 0; i < 4; ++i) f16_split2(v[j][2 * i], v[j][2 * i + 1], h[j][i], l[j][i]);
                 mbar_wait(&bars->opempty[o], ((it / PTC_OP_STAGES) & 1) ^ 1);
 #pragma unroll
                 for (int j = 0; j < TPW; ++j) {
@@ -257,7 +240,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
         const int m = quad * 32 + lane;
         const int pix = m >> 1, xi = pix >> 4, zi = pix & 15;
         // 1 / (data scale x B scale): exact power of two, applied to U before squaring
-        const float unscale = __uint_as_float((uint32_t)(127 - 8 - ptc_scale_exp(*a.amax)) << 23);
+        const float unscale = pow2f(-8 - pow2_scale_exp(*a.amax));
         uint32_t tl = 0;
         int curk = -1;
         for (int sg = seg0; sg < seg1; ++sg) {
@@ -336,7 +319,7 @@ __global__ void proj_tc_pack_kernel(const float2* B, int N, int Ns, int Kp, int 
         }
         uint32_t h[4], l[4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) ptc_split(x[2 * i], x[2 * i + 1], h[i], l[i]);
+        for (int i = 0; i < 4; ++i) f16_split2(x[2 * i], x[2 * i + 1], h[i], l[i]);
         out[e] = lo ? make_uint4(l[0], l[1], l[2], l[3]) : make_uint4(h[0], h[1], h[2], h[3]);
     }
 }

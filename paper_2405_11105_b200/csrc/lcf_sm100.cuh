@@ -5,6 +5,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <cstdint>
+#include <cuda_fp16.h>
 
 namespace lcf {
 namespace sm100 {
@@ -173,6 +174,24 @@ __device__ __forceinline__ float to_tf32(float x) {
     asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
     return __uint_as_float(r);
 }
+
+// ---------------------------------------------------------------- fp16 split precision
+// (a, b) -> packed fp16 pairs hi = fp16(x), lo = fp16(x - hi); the lower half holds a
+__device__ __forceinline__ void f16_split2(float a, float b, uint32_t& hi, uint32_t& lo) {
+    const __half2 h = __floats2half2_rn(a, b);
+    const float2 hf = __half22float2(h);
+    const __half2 l = __floats2half2_rn(a - hf.x, b - hf.y);
+    hi = *reinterpret_cast<const uint32_t*>(&h);
+    lo = *reinterpret_cast<const uint32_t*>(&l);
+}
+// exponent k of the power of two that brings a maximum with these float bits into [256, 512)
+__host__ __device__ __forceinline__ int pow2_scale_exp(uint32_t amax_bits) {
+    const int ex = (int)((amax_bits >> 23) & 0xffu);
+    if (ex == 0 || ex == 255) return 0;
+    const int k = 8 - (ex - 127);
+    return k < -100 ? -100 : (k > 100 ? 100 : k);
+}
+__device__ __forceinline__ float pow2f(int k) { return __uint_as_float((uint32_t)(127 + k) << 23); }
 
 }  // namespace sm100
 }  // namespace lcf
