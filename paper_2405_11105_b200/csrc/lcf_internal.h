@@ -85,7 +85,7 @@ struct lcf_plan {
     void* R_d = nullptr;       // [K][N][N] complex real (full Hermitian)
     // tensor-core Gram (precision 0, N <= 128): lcf_gram_tc.cu
     bool gram_tc = false;
-    int gtc_grid = 0, gtc_nseg = 0, gtc_group = 16;
+    int gtc_grid = 0, gtc_nseg = 0, gtc_group = 8;
     uint32_t gtc_raw_stride = 0;
     size_t gtc_smem = 0;
     lcf::GtcSeg* gtc_segs_d = nullptr;
