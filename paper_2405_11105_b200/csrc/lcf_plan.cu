@@ -529,7 +529,7 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
     w->gram_flops = 8.0 * S * N * (N + 1.0) / 2.0;   // Hermitian half, 8 real flops per complex MAC
     w->proj_flops = 8.0 * S * N * N;                 // dense N x N projector factor
     w->hbm_bytes = 8.0 * N * (double)p->P + 4.0 * (double)p->P;
-    w->launches = 2 + (p->evd_chol ? (p->evd_cluster ? 2 : 1) : 2) + (p->proj_tc ? 3 : 1) + 2;   // gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
+    w->launches = ((p->gram_tc || p->proj_tc) ? 1 : 0) + 2 + (p->evd_chol ? (p->evd_cluster ? 2 : 1) : 2) + (p->proj_tc ? 3 : 1) + 2;   // absmax, gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
     w->gram_tc = p->gram_tc ? 1 : 0; w->evd_chol = p->evd_chol ? 1 : 0; w->proj_tc = p->proj_tc ? 1 : 0;
     w->gram_tensor_flops = 0.0; w->proj_tensor_flops = 0.0;
     for (int k = 0; k < p->K; ++k) {
@@ -537,9 +537,9 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
         if (b.Pk == 0) continue;
         const double ntz = (double)((b.z0 + b.Lz - (b.z0 & ~1) + 15) / 16);
         const double Np = (double)((p->N + 15) / 16 * 16);
-        // Gram: 16-pixel tiles, per 8 pixels seven 128 x Np x 8 MMAs
+        // Gram: 16-pixel tiles, per tile three 128 x 2Np x 16 MMAs and one 128 x Np x 16 (= seven 128 x Np x 16 products)
         if (p->gram_tc) w->gram_tensor_flops += ntz * b.Lx * 2.0 * 7.0 * 2.0 * 128.0 * Np * 8.0;
-        // projection: 64-pixel tiles x column blocks, per 8 frames one 128x256x8 and one 128x128x8 MMA
+        // projection: 64-pixel tiles x column blocks, per 16 frames one 128x256x16 and one 128x128x16 MMA
         if (p->proj_tc)
             w->proj_tensor_flops += ntz * (double)((b.Lx + 3) / 4) * p->ptc_NB * (p->ptc_Kp / 8) * 2.0 * 128.0 * (256.0 + 128.0) * 8.0;
     }
