@@ -29,6 +29,7 @@
 #include <cfloat>
 
 #include "lcf_internal.h"
+#include "lcf_sm100.cuh"
 #include "lcf_thresh.cuh"
 
 namespace lcf {
@@ -37,6 +38,7 @@ struct EcArgs {
     int N, NP, Ns, LD;            // Ns = 2 NP column slots (one inert zero column if N is odd); LD = column stride
     int max_sweeps;
     const float2* R;              // [K][N][N] full Hermitian
+    const uint32_t* amax;         // non-null: R carries the power-of-two data scale of the tensor-core Gram (squared); eigenvalues are unscaled here
     double* lam;                  // [K][N] descending
     int* order;                   // [K][N] slot of the i-th largest eigenvalue
     int* cut;                     // [K]
@@ -349,6 +351,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     }
     __syncthreads();
     // rank (descending, ties by slot index), cut-off, eigen-weights: same rules as jacobi_kernel
+    const double un = a.amax ? ldexp(1.0, -2 * sm100::pow2_scale_exp(*a.amax)) : 1.0;
     float myl = 0.f;
     int rank = 0;
     if (tid < N) {
@@ -357,8 +360,8 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
             const float ljv = lam_s[j];
             rank += (ljv > myl) || (ljv == myl && j < tid);
         }
-        lsort[rank] = (double)myl;
-        a.lam[(size_t)k * N + rank] = (double)myl;
+        lsort[rank] = (double)myl * un;
+        a.lam[(size_t)k * N + rank] = (double)myl * un;
         a.order[(size_t)k * N + rank] = tid;
     }
     __syncthreads();
@@ -378,7 +381,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
             double w = 0.0;
             if (tid < N) {
                 const int i1 = rank + 1;                             // 1-based order of the eigenvalue in slot tid
-                w = thresh_is_adaptive(a.mode) ? thresh_adaptive_raw((double)myl, lsort[0], i1, N, a.beta) / wnorm_sh
+                w = thresh_is_adaptive(a.mode) ? thresh_adaptive_raw((double)myl * un, lsort[0], i1, N, a.beta) / wnorm_sh
                                              : thresh_weight(soft, a.beta, i1, c);
                 a.wt[(size_t)k * N + rank] = w;
             }
@@ -422,7 +425,7 @@ cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only) {
     EcArgs a;
     a.chol_only = chol_only ? 1 : 0; a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d;
     a.N = p->N; a.NP = p->NP; a.Ns = p->Ns; a.LD = p->ec_LD; a.max_sweeps = 30;
-    a.R = reinterpret_cast<const float2*>(p->R_d);
+    a.R = reinterpret_cast<const float2*>(p->R_d); a.amax = p->gram_tc ? p->amax_d : nullptr;
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;

@@ -20,6 +20,7 @@
 #include <cfloat>
 
 #include "lcf_internal.h"
+#include "lcf_sm100.cuh"
 #include "lcf_thresh.cuh"
 
 namespace lcf {
@@ -32,6 +33,7 @@ struct EclArgs {
     int max_sweeps;
     const float* gfac;                         // [K][2][N][LDg]
     const float* shift;                        // [K]
+    const uint32_t* amax;                      // non-null: the factors carry the data scale of the tensor-core Gram
     double* lam; int* order; int* cut; int* sweeps; int* conv;
     float* wslot; double* wslot_dd; double* wt;
     float2* V; float2* B;                      // [K][N][N]
@@ -155,6 +157,7 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
     }
     ecl_cluster_sync();
     // ---- rank (descending, ties by slot), cut-off, eigen-weights: both CTAs compute, CTA 0 writes
+    const double un = a.amax ? ldexp(1.0, -2 * sm100::pow2_scale_exp(*a.amax)) : 1.0;   // eigenvalues leave unscaled
     float myl = 0.f;
     int rnk = 0;
     if (tid < N) {
@@ -163,9 +166,9 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
             const float lq = lam_s[q];
             rnk += (lq > myl) || (lq == myl && q < tid);
         }
-        lsort[rnk] = (double)myl;
+        lsort[rnk] = (double)myl * un;
         if (rank == 0) {
-            a.lam[(size_t)k * N + rnk] = (double)myl;
+            a.lam[(size_t)k * N + rnk] = (double)myl * un;
             a.order[(size_t)k * N + rnk] = tid;
         }
     }
@@ -183,7 +186,7 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
         if (tid < N) {
             const int i1 = rnk + 1;                                  // 1-based order of the eigenvalue in slot tid
             double w;
-            w = thresh_is_adaptive(a.mode) ? thresh_adaptive_raw((double)myl, lsort[0], i1, N, a.beta) / wnorm_sh
+            w = thresh_is_adaptive(a.mode) ? thresh_adaptive_raw((double)myl * un, lsort[0], i1, N, a.beta) / wnorm_sh
                                              : thresh_weight(soft, a.beta, i1, c);
             wsl[tid] = (float)w;
             if (rank == 0) {
@@ -658,7 +661,7 @@ cudaError_t configure_evd_cluster(lcf_plan* p) {
 cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st) {
     EclArgs a;
     a.N = p->N; a.n = p->N / 2; a.h = (a.n + 1) / 2; a.LD = p->ec_LD; a.LDg = p->ec_LD; a.max_sweeps = 30;
-    a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d;
+    a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d; a.amax = p->gram_tc ? p->amax_d : nullptr;
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;

@@ -369,7 +369,9 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
 
 // R_k = sum over the window's segments, in fp64:  Re R = D0 + H + H^T,  Im R = (G0 + L) - (G0 + L)^T
 template <typename T>
-__global__ void gram_tc_reduce_kernel(const float* part, const int* seg_first, int N, const uint32_t* amax, void* Rv) {
+// R_k stays in the power-of-two data scale (squared): the fp32 EVD then works on numbers of a fixed
+// magnitude whatever the units of the input; the EVD kernels unscale the eigenvalues, lcf_get_gram R.
+__global__ void gram_tc_reduce_kernel(const float* part, const int* seg_first, int N, void* Rv) {
     const int k = blockIdx.z;
     const int i = blockIdx.y * 16 + threadIdx.y, j = blockIdx.x * 16 + threadIdx.x;
     if (i >= N || j >= N) return;
@@ -381,8 +383,6 @@ __global__ void gram_tc_reduce_kernel(const float* part, const int* seg_first, i
         im += ((double)p[16384 + ij] - (double)p[16384 + ji]) + ((double)p[3 * 16384 + ij] - (double)p[3 * 16384 + ji]);
     }
     if (i == j) im = 0.0;
-    const double un = ldexp(1.0, -2 * pow2_scale_exp(*amax));   // the operands carried the power-of-two data scale
-    re *= un; im *= un;
     if (sizeof(T) == 4) {
         float2* R = reinterpret_cast<float2*>(Rv) + (size_t)k * N * N;
         R[(size_t)i * N + j] = make_float2((float)re, (float)im);
@@ -493,7 +493,7 @@ cudaError_t launch_gram_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     dim3 blk(16, 16), grid((p->N + 15) / 16, (p->N + 15) / 16, p->K);
-    gram_tc_reduce_kernel<float><<<grid, blk, 0, st>>>(p->gtc_part_d, p->gtc_seg_first_d, p->N, p->amax_d, p->R_d);
+    gram_tc_reduce_kernel<float><<<grid, blk, 0, st>>>(p->gtc_part_d, p->gtc_seg_first_d, p->N, p->R_d);
     return cudaGetLastError();
 }
 

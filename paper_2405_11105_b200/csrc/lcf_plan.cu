@@ -8,6 +8,7 @@
 #include <new>
 
 #include "lcf_internal.h"
+#include "lcf_sm100.cuh"
 #include "lcf_thresh.cuh"
 
 using namespace lcf;
@@ -192,6 +193,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
         cudaGetLastError();
         p->evd_chol = false;
     }
+    if (!p->evd_chol) p->gram_tc = false;   // the tensor-core Gram leaves R in its data scale, which only these EVD kernels undo
     p->evd_cluster = p->evd_chol && evd_cluster_eligible(p);
     if (p->evd_cluster && configure_evd_cluster(p) != cudaSuccess) {
         cudaGetLastError();
@@ -448,7 +450,13 @@ extern "C" lcf_status lcf_get_gram(lcf_plan* p, double* R) {
     } else {
         std::vector<float> tmp(n);
         if (cudaMemcpy(tmp.data(), p->R_d, n * sizeof(float), cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
-        for (size_t i = 0; i < n; ++i) R[i] = (double)tmp[i];
+        double un = 1.0;
+        if (p->gram_tc) {   // the tensor-core Gram leaves R in its power-of-two data scale
+            uint32_t bits = 0;
+            if (cudaMemcpy(&bits, p->amax_d, sizeof(bits), cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+            un = std::ldexp(1.0, -2 * sm100::pow2_scale_exp(bits));
+        }
+        for (size_t i = 0; i < n; ++i) R[i] = (double)tmp[i] * un;
     }
     return conv_status(p);
 }

@@ -229,6 +229,26 @@ def test_rank_r_clutter_removed(lcf):
     assert (means * 48 * 40 / lam.sum(axis=1)).max() <= 1e-10
 
 
+def test_tensor_path_data_scale(lcf, oracle):
+    """The fp16 split-precision contractions scale the ensemble by a power of two taken from its
+    largest sample: tiny and huge amplitudes (far outside the fp16 range) must give the same
+    eigenvalues (up to the scale) and the same Eq. 13 image as the oracle on the unscaled data."""
+    cfg = synth.baseline_configs()[0]
+    d = cfg.data
+    iq = np.ascontiguousarray(synth.ensemble(synth.generate(cfg), cfg, 0))
+    f = replace(cfg.filt, mode=synth.SOFT_ENERGY, precision=0)
+    with lcf.Plan.from_spec(d.Nz, d.Nx, d.N, f) as plan:
+        w = plan.work()
+    assert w["gram_tc"] == 1 and w["proj_tc"] == 1
+    o = oracle.run_config(iq, f)
+    for c in (1.0, 1.37e-9, 7.7e5, 3.3e12):
+        g = gpu_run(lcf, (iq * np.complex64(c)).astype(np.complex64), f)
+        assert np.array_equal(g["c"], o["c"]), (c, g["c"], o["c"])
+        lmax = o["lam"][:, :1]
+        assert (np.abs(g["lam"] / (c * c) - o["lam"]) / lmax).max() <= LAM_TOL, c
+        check_pd(g["PD"], o["PD"])
+
+
 def test_empty_window_support(lcf):
     # sigma so small that no pixel lies within trunc*sigma of the half-integer centres: P_k = 0
     iq = synth.random_cube(8, 8, 6, seed=2)
