@@ -67,7 +67,7 @@ __device__ __forceinline__ void ec_pair_pq(int m, int s, int M, int& p, int& q) 
 }
 
 constexpr int EC_THREADS = 512;   // 8 threads per column pair (NP <= 64 pairs)
-constexpr int EC_PS = 264, EC_PI = 132;   // floats per partial vector (N <= 128; EC_PS % 32 == 8), offset of its imaginary half
+constexpr int EC_NB = 8;                   // Cholesky steps per block
 
 __device__ __forceinline__ unsigned long long ec_fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
     unsigned long long d;
@@ -100,8 +100,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     // planar storage: real and imaginary parts of column u at Gr/Gi + u*LD (LD floats, multiple of 4)
     float* Gr = reinterpret_cast<float*>(smem_raw);                  // [Ns][LD]
     float* Gi = Gr + (size_t)Ns * LD;                                // [Ns][LD]
-    float* part = Gi + (size_t)Ns * LD;                              // [16][EC_PS] per-warp partial Schur columns (re at 0, im at EC_PI)
-    float* lam_s = part + (EC_THREADS / 32) * EC_PS;                 // [Ns] eigenvalue of slot u
+    float* lam_s = Gi + (size_t)Ns * LD;                             // [Ns] eigenvalue of slot u
     float* inv_s = lam_s + Ns;                                       // [Ns] 1 / |g_u|
     float* wsl = inv_s + Ns;                                         // [Ns] eigen-weight of slot u
     float* red = wsl + Ns;                                           // [32]
@@ -134,97 +133,102 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     if (maxdiag > 0.f) {
         if (tid < N) { Gr[(size_t)tid * LD + tid] += delta; Gi[(size_t)tid * LD + tid] = 0.f; }
         __syncthreads();
-        // ---- 2. pivoted Cholesky, left-looking: R stays untouched until a column is chosen.  Step j
-        // picks the largest remaining diagonal entry, forms that column's Schur complement as
-        // R[:, pv] - G[:, e_0..e_{j-1}] conj(G[pv, e_0..e_{j-1}]) (a matrix-vector product over the
-        // finished columns: warp w takes every 16th of them, lane r rows 4r..4r+3, and the 16 partial
-        // vectors are summed through `part`), scales it into column pv and downdates the diagonal.
-        // Shared-memory traffic per step is the finished columns read once, against the whole
-        // trailing matrix read and written by a right-looking update.
-        // The pivot search is a warp-wide integer maximum (redux) over keys that hold the diagonal
-        // entry's top 25 bits above 127 - row (ties, and near-ties within 2^-16, go to the lowest row):
-        // each warp reduces its 8 rows when it downdates them, and after the step's barrier every warp
-        // reduces the 16 warp keys.
+        // ---- 2. pivoted Cholesky in blocks of EC_NB steps.  Inside a block the chosen column is
+        // brought up to date against the block's finished columns only (left-looking over at most
+        // EC_NB - 1 columns: one thread per row); at the end of a block every column still to be
+        // eliminated takes the block's rank-EC_NB update at once (right-looking: one warp per column,
+        // the block's columns held in registers), so the trailing matrix crosses shared memory once per
+        // EC_NB steps.  The pivot search is a warp-wide integer maximum (redux) over keys that hold the
+        // diagonal entry's top 25 bits above 127 - row (ties, and near-ties within 2^-16, go to the
+        // lowest row): each warp reduces its rows when it downdates them, and after the step's barrier
+        // every warp reduces the 16 warp keys.
         const int nchc = (N + 3) >> 2;                               // 4-row chunks per column
         float* dgs = lam_s;                                          // [N] current diagonal of the Schur complement, -1 once eliminated
         unsigned* wkey = reinterpret_cast<unsigned*>(red);           // [16] per-warp pivot keys
-        const int ri = tid >> 2, rq = tid & 3;                       // downdate phase: 4 threads per row
+        int* elist = alist;                                          // [N] pivot of step t = slot of Cholesky column t
         {
             unsigned key = 0u;
-            if (rq == 0 && ri < N) {
-                const float d = fmaxf(Gr[(size_t)ri * LD + ri], 0.f);
-                dgs[ri] = d;
-                key = (__float_as_uint(d) & ~127u) | (unsigned)(127 - ri);
+            if (tid < N) {
+                const float d = fmaxf(Gr[(size_t)tid * LD + tid], 0.f);
+                dgs[tid] = d;
+                key = (__float_as_uint(d) & ~127u) | (unsigned)(127 - tid);
             }
             key = __reduce_max_sync(0xffffffffu, key);
             if (lane == 0) wkey[warp] = key;
         }
         __syncthreads();
-        int ecol[8];                                                 // slots of this warp's finished columns (steps warp, warp + 16, ...)
-#pragma unroll
-        for (int m = 0; m < 8; ++m) ecol[m] = 0;
-        for (int j = 0; j < N; ++j) {
-            unsigned kk = lane < EC_THREADS / 32 ? wkey[lane] : 0u;
-            kk = __reduce_max_sync(0xffffffffu, kk);
-            const int pv = 127 - (int)(kk & 127u);
-            // a non-positive pivot can only come from rounding: clamp (the column is then ~0)
-            const float piv = fmaxf(dgs[pv], 1e-30f * maxdiag + 1e-37f);
-            const float sc = rsqrtf(piv), dsq = piv * sc;
-            if (lane < nchc) {
-                float4 ar = make_float4(0.f, 0.f, 0.f, 0.f), ai = ar;
-                const int cnt = (j - warp + EC_THREADS / 32 - 1) / (EC_THREADS / 32);   // finished columns of this warp
-#pragma unroll
-                for (int m = 0; m < 8; ++m) {
-                    if (m < cnt) {
-                        const float* cr = Gr + (size_t)ecol[m] * LD;
-                        const float* ci = Gi + (size_t)ecol[m] * LD;
-                        const float lr = cr[pv], li = ci[pv], nli = -li;
-                        const float4 xr = *reinterpret_cast<const float4*>(&cr[4 * lane]);
-                        const float4 xi = *reinterpret_cast<const float4*>(&ci[4 * lane]);
-                        // x * conj(l):  re += xr lr + xi li,  im += xi lr - xr li
-                        ar.x = fmaf(xr.x, lr, fmaf(xi.x, li, ar.x));  ai.x = fmaf(xi.x, lr, fmaf(xr.x, nli, ai.x));
-                        ar.y = fmaf(xr.y, lr, fmaf(xi.y, li, ar.y));  ai.y = fmaf(xi.y, lr, fmaf(xr.y, nli, ai.y));
-                        ar.z = fmaf(xr.z, lr, fmaf(xi.z, li, ar.z));  ai.z = fmaf(xi.z, lr, fmaf(xr.z, nli, ai.z));
-                        ar.w = fmaf(xr.w, lr, fmaf(xi.w, li, ar.w));  ai.w = fmaf(xi.w, lr, fmaf(xr.w, nli, ai.w));
-                    }
-                }
-                *reinterpret_cast<float4*>(&part[warp * EC_PS + 4 * lane]) = ar;
-                *reinterpret_cast<float4*>(&part[warp * EC_PS + EC_PI + 4 * lane]) = ai;
-            }
-#pragma unroll
-            for (int m = 0; m < 8; ++m) if (j == warp + m * (EC_THREADS / 32)) ecol[m] = pv;   // column j is finished after this step
-            __syncthreads();
-            {
-                // thread rq of row ri sums the partials of warps rq, rq+4, rq+8, rq+12 (conflict-free: EC_PS % 32 == 8)
-                float sr = 0.f, si = 0.f, d = -1.f, cr0 = 0.f, ci0 = 0.f;
-                if (ri < N) {
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        sr += part[(rq + 4 * u) * EC_PS + ri];
-                        si += part[(rq + 4 * u) * EC_PS + EC_PI + ri];
-                    }
-                    if (rq == 0) { d = dgs[ri]; cr0 = Gr[(size_t)pv * LD + ri]; ci0 = Gi[(size_t)pv * LD + ri]; }
-                }
-                sr += __shfl_xor_sync(0xffffffffu, sr, 1);  si += __shfl_xor_sync(0xffffffffu, si, 1);
-                sr += __shfl_xor_sync(0xffffffffu, sr, 2);  si += __shfl_xor_sync(0xffffffffu, si, 2);
+        for (int jb = 0; jb < N; jb += EC_NB) {
+            const int je = jb + EC_NB < N ? jb + EC_NB : N;
+            for (int j = jb; j < je; ++j) {
+                unsigned kk = lane < EC_THREADS / 32 ? wkey[lane] : 0u;
+                kk = __reduce_max_sync(0xffffffffu, kk);
+                const int pv = 127 - (int)(kk & 127u);
                 unsigned key = 0u;
-                if (rq == 0 && ri < N) {
-                    float vr = 0.f, vi = 0.f;                        // Cholesky column pi_j is zero in eliminated rows
-                    if (ri == pv) { vr = dsq; dgs[ri] = -1.f; }
-                    else if (d >= 0.f) {
-                        vr = (cr0 - sr) * sc;
-                        vi = (ci0 - si) * sc;
-                        const float nd = fmaxf(d - (vr * vr + vi * vi), 0.f);
-                        dgs[ri] = nd;
-                        key = (__float_as_uint(nd) & ~127u) | (unsigned)(127 - ri);
+                if (tid < N) {
+                    // a non-positive pivot can only come from rounding: clamp (the column is then ~0)
+                    const float piv = fmaxf(dgs[pv], 1e-30f * maxdiag + 1e-37f);
+                    const float sc = rsqrtf(piv), dsq = piv * sc;
+                    const int i = tid;
+                    float sr = 0.f, si = 0.f;
+                    for (int t = jb; t < j; ++t) {                   // G[i, e_t] conj(G[pv, e_t]) over the block's finished columns
+                        const float* cr = Gr + (size_t)elist[t] * LD;
+                        const float* ci = Gi + (size_t)elist[t] * LD;
+                        const float gr = cr[i], gi = ci[i], lr = cr[pv], li = ci[pv];
+                        sr = fmaf(gr, lr, fmaf(gi, li, sr));
+                        si = fmaf(gi, lr, fmaf(-gr, li, si));
                     }
-                    Gr[(size_t)pv * LD + ri] = vr;
-                    Gi[(size_t)pv * LD + ri] = vi;
+                    const float d = dgs[i];
+                    float vr = 0.f, vi = 0.f;                        // Cholesky column pi_j is zero in eliminated rows
+                    if (i == pv) { vr = dsq; dgs[i] = -1.f; }
+                    else if (d >= 0.f) {
+                        vr = (Gr[(size_t)pv * LD + i] - sr) * sc;
+                        vi = (Gi[(size_t)pv * LD + i] - si) * sc;
+                        const float nd = fmaxf(d - (vr * vr + vi * vi), 0.f);
+                        dgs[i] = nd;
+                        key = (__float_as_uint(nd) & ~127u) | (unsigned)(127 - i);
+                    }
+                    Gr[(size_t)pv * LD + i] = vr;
+                    Gi[(size_t)pv * LD + i] = vi;
+                    if (tid == 0) elist[j] = pv;
                 }
                 key = __reduce_max_sync(0xffffffffu, key);
                 if (lane == 0) wkey[warp] = key;
+                __syncthreads();
             }
-            __syncthreads();
+            if (je < N) {
+                // rank-(je - jb) update of the columns still to be eliminated
+                float4 gbr[EC_NB], gbi[EC_NB];
+                const float* gcol[EC_NB];
+#pragma unroll
+                for (int t = 0; t < EC_NB; ++t) {
+                    gcol[t] = Gr + (size_t)elist[jb + t < je ? jb + t : jb] * LD;
+                    gbr[t] = gbi[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (jb + t < je && lane < nchc) {
+                        gbr[t] = *reinterpret_cast<const float4*>(&gcol[t][4 * lane]);
+                        gbi[t] = *reinterpret_cast<const float4*>(&gcol[t][(size_t)Ns * LD + 4 * lane]);
+                    }
+                }
+                for (int l = warp; l < N; l += EC_THREADS / 32) {
+                    if (dgs[l] < 0.f) continue;                      // already a Cholesky column
+                    if (lane < nchc) {
+                        float* cr = Gr + (size_t)l * LD + 4 * lane;
+                        float* ci = Gi + (size_t)l * LD + 4 * lane;
+                        float4 xr = *reinterpret_cast<float4*>(cr), xi = *reinterpret_cast<float4*>(ci);
+#pragma unroll
+                        for (int t = 0; t < EC_NB; ++t) {
+                            // x -= g_t conj(G[l, e_t]):  re -= gr lr + gi li,  im -= gi lr - gr li  (zero columns for t >= je - jb)
+                            const float lr = gcol[t][l], li = gcol[t][(size_t)Ns * LD + l];
+                            xr.x -= gbr[t].x * lr + gbi[t].x * li;  xi.x -= gbi[t].x * lr - gbr[t].x * li;
+                            xr.y -= gbr[t].y * lr + gbi[t].y * li;  xi.y -= gbi[t].y * lr - gbr[t].y * li;
+                            xr.z -= gbr[t].z * lr + gbi[t].z * li;  xi.z -= gbi[t].z * lr - gbr[t].z * li;
+                            xr.w -= gbr[t].w * lr + gbi[t].w * li;  xi.w -= gbi[t].w * lr - gbr[t].w * li;
+                        }
+                        *reinterpret_cast<float4*>(cr) = xr;
+                        *reinterpret_cast<float4*>(ci) = xi;
+                    }
+                }
+                __syncthreads();
+            }
         }
         if (a.chol_only) {
             float* gout = a.gfac + (size_t)k * 2 * Ns * LD;
@@ -404,7 +408,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
 }
 
 static size_t ec_smem_bytes(int Ns, int LD) {
-    return (size_t)Ns * LD * 8 + (size_t)(EC_THREADS / 32) * EC_PS * 4 + 3 * (size_t)Ns * 4 + 32 * 4 + (size_t)Ns * 8 + 3 * (size_t)Ns * 4 + 16 + 16 + 64;
+    return (size_t)Ns * LD * 8 + 3 * (size_t)Ns * 4 + 32 * 4 + (size_t)Ns * 8 + 3 * (size_t)Ns * 4 + 16 + 16 + 64;
 }
 
 bool evd_chol_eligible(const lcf_plan* p) { return p->prec == 0 && p->N <= 128 && p->N >= 2; }
