@@ -31,7 +31,7 @@
 // `group` tiles (128 pixels = 32 adds) into fp32 registers of the drain warps (round to nearest)
 // and zeroed there with tcgen05.st (the fused MMAs have one accumulate flag for D0 and H together),
 // H and L (2^-11 of the main terms) stay in TMEM for the whole segment.  Each segment ends by
-// writing four 128 x 128 fp32 partials; gram_tc_reduce_kernel sums a window's segments in fp64,
+// writing two 128 x 128 fp32 partials (D0 / 2 + H and G0 + L); gram_tc_reduce_kernel sums a window's segments in fp64,
 // applies the (anti)symmetrisation above and writes the full Hermitian R_k.
 // Measured bound (clock64 per role, B200): the 128x128x8 MMA reads 8 KB of operands per 64 cycles,
 // i.e. the whole 128 B/clk of shared-memory bandwidth, so the converter's and TMA's shared-memory
@@ -68,7 +68,7 @@ struct GtcArgs {
     const WinBox* box;
     const GtcSeg* segs;
     const int* cta_first;      // [grid+1]
-    float* part;               // [nseg][4][128][128]
+    float* part;               // [nseg][2][128][128]
     uint32_t raw_stride;       // bytes between raw stages (multiple of 1024)
     const uint32_t* amax;      // bits of max |S| (power-of-two scaling of the fp16 operands)
 };
@@ -330,32 +330,29 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
                     ++gc;
                 }
             }
-            // ---- segment end: the four partials of this segment
-            float* out = a.part + (size_t)sg * 4 * 128 * 128 + (size_t)row * 128 + half * 64;
-#pragma unroll
-            for (int m = 0; m < 2; ++m) {
-#pragma unroll
-                for (int j = 0; j < 64; j += 4)
-                    *reinterpret_cast<float4*>(out + (size_t)m * 128 * 128 + j) =
-                        make_float4(acc[m * 64 + j], acc[m * 64 + j + 1], acc[m * 64 + j + 2], acc[m * 64 + j + 3]);
-            }
-#pragma unroll
-            for (int i = 0; i < 128; ++i) acc[i] = 0.f;
+            // ---- segment end: the two partials of this segment, P0 = D0 / 2 + H and P1 = G0 + L
+            // (Re R = P0 + P0^T since D0 is symmetric, Im R = P1 - P1^T)
+            float* out = a.part + (size_t)sg * 2 * 128 * 128 + (size_t)row * 128 + half * 64;
 #pragma unroll
             for (int blk = 0; blk < 8; ++blk) {
-                const int m = 2 + (blk >> 2);                              // partial 2 = H, 3 = L
+                const int m = blk >> 2;                                    // 0: D0 with H, 1: G0 with L
                 const int cj = half * 64 + (blk & 3) * 16;
                 if (cj < a.Np) {
                     uint32_t v[16];
                     tmem_ld16(tlane + (blk < 4 ? 0u : 256u) + (uint32_t)(a.Np + cj), v);
                     tmem_ld_wait();
+                    const float sc = m == 0 ? 0.5f : 1.f;
                     float* o2 = out + (size_t)m * 128 * 128 + (blk & 3) * 16;
 #pragma unroll
                     for (int j = 0; j < 16; j += 4)
-                        *reinterpret_cast<float4*>(o2 + j) = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]),
-                                                                         __uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
+                        *reinterpret_cast<float4*>(o2 + j) = make_float4(fmaf(sc, acc[blk * 16 + j], __uint_as_float(v[j])),
+                                                                         fmaf(sc, acc[blk * 16 + j + 1], __uint_as_float(v[j + 1])),
+                                                                         fmaf(sc, acc[blk * 16 + j + 2], __uint_as_float(v[j + 2])),
+                                                                         fmaf(sc, acc[blk * 16 + j + 3], __uint_as_float(v[j + 3])));
                 }
             }
+#pragma unroll
+            for (int i = 0; i < 128; ++i) acc[i] = 0.f;
             tc_fence_before_sync();
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars->accempty);
@@ -367,7 +364,7 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
     if (warp == 1) tmem_dealloc<512>(tmem);
 }
 
-// R_k = sum over the window's segments, in fp64:  Re R = D0 + H + H^T,  Im R = (G0 + L) - (G0 + L)^T
+// R_k = sum over the window's segments, in fp64:  Re R = P0 + P0^T,  Im R = P1 - P1^T  (P0 = D0 / 2 + H, P1 = G0 + L)
 template <typename T>
 // R_k stays in the power-of-two data scale (squared): the fp32 EVD then works on numbers of a fixed
 // magnitude whatever the units of the input; the EVD kernels unscale the eigenvalues, lcf_get_gram R.
@@ -377,10 +374,10 @@ __global__ void gram_tc_reduce_kernel(const float* part, const int* seg_first, i
     if (i >= N || j >= N) return;
     double re = 0.0, im = 0.0;
     for (int s = seg_first[k]; s < seg_first[k + 1]; ++s) {
-        const float* p = part + (size_t)s * 4 * 128 * 128;
+        const float* p = part + (size_t)s * 2 * 128 * 128;
         const size_t ij = (size_t)i * 128 + j, ji = (size_t)j * 128 + i;
-        re += (double)p[ij] + ((double)p[2 * 16384 + ij] + (double)p[2 * 16384 + ji]);
-        im += ((double)p[16384 + ij] - (double)p[16384 + ji]) + ((double)p[3 * 16384 + ij] - (double)p[3 * 16384 + ji]);
+        re += (double)p[ij] + (double)p[ji];
+        im += (double)p[16384 + ij] - (double)p[16384 + ji];
     }
     if (i == j) im = 0.0;
     if (sizeof(T) == 4) {

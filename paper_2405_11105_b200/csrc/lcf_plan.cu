@@ -256,7 +256,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     if (p->gram_tc) {
         ok = ok && dev_upload(&p->gtc_segs_d, gtc_segs) && dev_upload(&p->gtc_cta_first_d, gtc_cta_first) &&
              dev_upload(&p->gtc_seg_first_d, gtc_seg_first) &&
-             dev_alloc(&p->gtc_part_d, (size_t)(p->gtc_nseg ? p->gtc_nseg : 1) * 4 * 128 * 128);
+             dev_alloc(&p->gtc_part_d, (size_t)(p->gtc_nseg ? p->gtc_nseg : 1) * 2 * 128 * 128);
     }
     if (p->evd_cluster) ok = ok && dev_alloc(&p->ec_gfac_d, K * 2 * Ns * (size_t)p->ec_LD) && dev_alloc(&p->ec_shift_d, K);
     if (p->proj_tc) {
