@@ -287,8 +287,8 @@ def run_ours(args, cfg):
     # (DESIGN.md "Rooflines"); sweeps as measured on this input
     evd_flops = float(sweeps.sum()) * (36.0 * N * N * (N - 1) / 2 if work["evd_chol"] else 30.0 * N ** 3)
     # the contractions run on the FP16 tensor path (.kind::f16, fp32 accumulate): same nominal rate as bf16
-    tf32_peak = (peaks.get("bf16_tflops") or 1590.0)
-    tf32_src = ("MEASURED_PEAKS.json bf16_tflops (burst); fp16 has the same nominal rate" if peaks.get("bf16_tflops")
+    tensor_peak = (peaks.get("bf16_tflops") or 1590.0)
+    tensor_src = ("MEASURED_PEAKS.json bf16_tflops (burst); fp16 has the same nominal rate" if peaks.get("bf16_tflops")
                 else "fallback 1590 TFLOP/s bf16; fp16 has the same nominal rate")
     fp32_src = "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md Rooflines)"
     kern = {
@@ -304,11 +304,11 @@ def run_ours(args, cfg):
         ms = stages.get(sname)
         if not ms:
             continue
-        peak = tf32_peak if kd["bound"] == "tensor" else (NOMINAL_FP32_TFLOPS / 2 if cfg.filt.precision == 1 and sname != "projection" else NOMINAL_FP32_TFLOPS)
+        peak = tensor_peak if kd["bound"] == "tensor" else (NOMINAL_FP32_TFLOPS / 2 if cfg.filt.precision == 1 and sname != "projection" else NOMINAL_FP32_TFLOPS)
         ach = kd["flops"] / (ms * 1e-3) / 1e12
         per_kernel[sname] = {"kernel": kd["kernel"], "ms": ms, "bound": kd["bound"], "achieved": ach, "peak": peak,
                              "unit": "TFLOP/s", "frac": ach / peak, "algorithmic_flops_per_launch": kd["flops"],
-                             "peak_source": tf32_src if kd["bound"] == "tensor" else fp32_src}
+                             "peak_source": tensor_src if kd["bound"] == "tensor" else fp32_src}
         if kd["executed_flops"]:
             ex = kd["executed_flops"] / (ms * 1e-3) / 1e12
             per_kernel[sname].update({"executed_tflops": ex, "executed_frac": ex / peak,

@@ -74,9 +74,13 @@ typedef struct {
     double energy_frac; /* in (0, 1) (ENERGY modes)                                             */
     double beta;        /* > 0 (SOFT modes: sigmoid sharpness; ADAPTIVE: the exponent of Eq. 10)  */
     double cut_scale;   /* > 0 (MEDIAN, CURVATURE modes): the scaling factor beta of Eq. 7 / Eq. 6 */
-    int precision;      /* 0: fp32 Gram + fp32 EVD.  1: exact-product fp64 Gram + fp64 EVD
+    int precision;      /* 0: fp32-grade Gram + fp32 EVD.  1: exact-product fp64 Gram + fp64 EVD
                            (single precision can hamper the EVD).  The projection
-                           is fp32 in both.                                                     */
+                           is fp32-grade in both.  "fp32-grade": on the tensor-core kernels
+                           (N <= 128, even Nz) each fp32 operand, scaled by a power of two taken
+                           from the ensemble's largest sample, is the sum of two fp16 numbers (22
+                           significant bits) and products accumulate in fp32 (DESIGN.md section
+                           6); the CUDA-core kernels that cover the other shapes use fp32.      */
 } lcf_thresh;
 
 /* Builds window tables, the work decomposition and all device workspace on the current CUDA device.
@@ -133,7 +137,7 @@ lcf_status lcf_get_stage_ms(lcf_plan* plan, float ms[5] /* HOST */);
  * projection flops, compulsory HBM bytes, sum_k P_k, kernel launches per call; which kernels the
  * plan selected (1 = tcgen05 Gram / Cholesky + one-sided Jacobi EVD / tcgen05 projection, 0 = the
  * FP32/FP64 CUDA-core kernels) and, for the tensor-core kernels, the flops the MMAs execute
- * (3xTF32 split, padded tiles) -- the algorithmic flops are what the rooflines are quoted on. */
+ * (three fp16 products of hi/lo splits per fp32 product, padded tiles) -- the algorithmic flops are what the rooflines are quoted on. */
 typedef struct {
     double gram_flops, proj_flops, hbm_bytes, sum_Pk;
     int launches;

@@ -1,5 +1,5 @@
 // lcf_gram_tc.cu -- kernel 1, tensor-core path: batched window-weighted complex Gram (Eq. 12,
-// PAPER.md:149-152) on tcgen05 with a 3xTF32 split, for precision 0 and N <= 128.
+// PAPER.md:149-152) on tcgen05 in fp16 split precision (three fp16 products per fp32 product), for precision 0 and N <= 128.
 //
 //   R_k[i][j] = sum_p w_k(p)^2 conj(S[i][p]) S[j][p]            X = W_k S (Eq. 11), X = Xr + i Xi
 //   Re R = Xr Xr^T + Xi Xi^T          Im R = G - G^T,  G = Xr Xi^T          (frames x frames, K = pixels)
@@ -111,10 +111,6 @@ __device__ __forceinline__ float2 sub2(float2 a, float2 b) {
     asm("mov.b64 {%0, %1}, %2;" : "=f"(f.x), "=f"(f.y) : "l"(r));
     return f;
 }
-// x rounded to TF32 (10-bit mantissa), nearest with ties away, in integer arithmetic.  hi = rna(x)
-// makes lo = x - hi a signed 12-bit quantity, so the tensor core's truncation of lo is unbiased.
-__device__ __forceinline__ float rna_tf32(float v) { return __uint_as_float((__float_as_uint(v) + 0x1000u) & 0xFFFFE000u); }
-
 __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_constant__ CUtensorMap tmap, GtcArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);

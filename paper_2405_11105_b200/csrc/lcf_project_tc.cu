@@ -1,5 +1,5 @@
 // lcf_project_tc.cu -- kernel 4a, tensor-core path: fused projection + |.|^2 slow-time sum (Eq. 4,
-// PAPER.md:57-63) on tcgen05 with a 3xTF32 split, for N <= 128.
+// PAPER.md:57-63) on tcgen05 in fp16 split precision (three fp16 products per fp32 product), for N <= 128.
 //
 //   U[p][u] = sum_t S[t][p] B_k[t][u],  B_k = V_k diag(wt)     PD_k(p) = w_k(p)^2 sum_u |U[p][u]|^2
 //
