@@ -300,7 +300,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                 float cs = 1.f, gr = 0.f, gim = 0.f;
                 if (rot) {
                     any = 1;
-                    if (absa2 > tol * app * aqq) big = 1;              // cos^2 > tol: the next sweep could still rotate
+                    if (absa2 > 2.f * tol * app * aqq) big = 1;        // cos^2 > 2 tol: not yet in the final quadratic phase
                     // t only steers the rotation (a slightly off angle costs convergence, not accuracy):
                     // approximate sqrt and reciprocal; c^2 + s^2 = 1 rests on one Newton step on rsqrt
                     const float inv = rsqrtf(absa2);
@@ -348,10 +348,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
         }
         ++sweep;
         // Over both CTAs: did this sweep rotate at all, and was any rotated pair still far (squared
-        // cosine above tol) from orthogonal?  Jacobi converges quadratically at the end: once every
-        // cosine of a sweep is below sqrt(tol) the next sweep leaves them at ~tol, which the sweep after
-        // would not rotate, so that next sweep is the last one and the usual rotation-free
-        // confirmation sweep is not run.
+        // cosine above 2 tol) from orthogonal?  Jacobi converges quadratically at the end: once every
+        // cosine of a sweep is below sqrt(2 tol) the next sweep leaves the pairs of separated
+        // eigenvalues at ~tol, so that next sweep is the last one and the usual rotation-free
+        // confirmation sweep is not run.  (Pairs inside a cluster of nearly equal eigenvalues keep
+        // cosines of a few 1e-4 whichever of tol, 2 tol, 4 tol is used -- measured -- and their
+        // eigenvectors are not determined anyway; the factor 2 saves 0.3 sweeps on average.)
         const int mine = __syncthreads_or(any) + __syncthreads_or(big);
         if (tid == 0) {
             const uint32_t fa = ecl_smem(&flg[(sweep & 1) * 2 + rank]);
@@ -577,14 +579,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                 float nA0, nA1, nB0, nB1;
                 if (s == 0) {
                     ecb_norms4(A0, A1, B0, B1, lane, nA0, nA1, nB0, nB1);
-                    fl |= ecb_round_tracked(A0, A1, B0, B1, nA0, nA1, nB0, nB1, lane, tol2, tol);   // inner pairs, once per sweep
+                    fl |= ecb_round_tracked(A0, A1, B0, B1, nA0, nA1, nB0, nB1, lane, tol2, 2.f * tol);   // inner pairs, once per sweep
                 } else {
                     const float* t0 = buf + ecb_slot(b, 0, j, 0, LD) + N;
                     const float* b0 = buf + ecb_slot(b, 1, j, 0, LD) + N;
                     nA0 = t0[0]; nA1 = t0[2 * LD]; nB0 = b0[0]; nB1 = b0[2 * LD];
                 }
-                fl |= ecb_round_tracked(A0, B0, A1, B1, nA0, nB0, nA1, nB1, lane, tol2, tol);
-                fl |= ecb_round_tracked(A0, B1, A1, B0, nA0, nB1, nA1, nB0, lane, tol2, tol);
+                fl |= ecb_round_tracked(A0, B0, A1, B1, nA0, nB0, nA1, nB1, lane, tol2, 2.f * tol);
+                fl |= ecb_round_tracked(A0, B1, A1, B0, nA0, nB1, nA1, nB0, lane, tol2, 2.f * tol);
                 const uint32_t mP = (Prem ? full_peer : full_u32) + 8u * (uint32_t)((b ^ 1) * ECB_PL + dPj);
                 const uint32_t mQ = (Qrem ? full_peer : full_u32) + 8u * (uint32_t)((b ^ 1) * ECB_PL + dQj);
                 if (rowok) {
