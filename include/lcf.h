@@ -148,6 +148,10 @@ lcf_status lcf_get_work(const lcf_plan* plan, lcf_work* out /* HOST */);
 /* Arithmetic-pipe microbenchmark on the current device: kind 0 = FP32 FFMA, 1 = FP32 packed
  * FFMA2 (fma.rn.f32x2), 2 = FP64 DFMA.  Writes achieved TFLOP/s (2 flops per FMA lane). */
 lcf_status lcf_measure_peak(int kind, double* tflops /* HOST */);
+/* Host logic of the tensor-core path's power-of-two operand scaling: the
+ * exponent k with amax * 2^k in [256, 512) for a finite amax > 0 (clamped to [-100, 100]); 0 for
+ * amax = 0, denormal, infinite or NaN.  Host function, no device work. */
+int lcf_scale_exponent(float amax);
 
 const char* lcf_status_string(lcf_status s);
 /* After LCF_ERR_CUDA from lcf_filter: "<stage>: <CUDA error string>" of the first failed launch

@@ -553,3 +553,9 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
     }
     return LCF_OK;
 }
+
+extern "C" int lcf_scale_exponent(float amax) {
+    uint32_t bits;
+    std::memcpy(&bits, &amax, sizeof(bits));
+    return lcf::sm100::pow2_scale_exp(bits & 0x7fffffffu);
+}

@@ -21,7 +21,7 @@ EXPORTS = [
     "lcf_plan_create", "lcf_filter", "lcf_filter_host", "lcf_filter_host_batch", "lcf_plan_destroy", "lcf_num_windows",
     "lcf_get_eigenvalues", "lcf_get_cutoffs", "lcf_get_sweeps", "lcf_get_gram", "lcf_get_eigenvectors",
     "lcf_get_weights", "lcf_get_filters", "lcf_get_window_means", "lcf_set_timing", "lcf_get_stage_ms",
-    "lcf_get_work", "lcf_measure_peak", "lcf_status_string", "lcf_last_error",
+    "lcf_get_work", "lcf_measure_peak", "lcf_status_string", "lcf_last_error", "lcf_scale_exponent",
 ]
 
 
@@ -87,6 +87,13 @@ def load() -> C.CDLL:
 
 def status_string(status: int) -> str:
     return load().lcf_status_string(int(status)).decode()
+
+
+def scale_exponent(amax: float) -> int:
+    """k such that amax * 2**k lies in [256, 512): the operand scaling of the tensor-core kernels."""
+    L = load()
+    L.lcf_scale_exponent.argtypes = [C.c_float]
+    return int(L.lcf_scale_exponent(C.c_float(amax)))
 
 
 def measure_peak(kind: int) -> float:

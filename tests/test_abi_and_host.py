@@ -68,6 +68,18 @@ def test_null_pointers(lcf):
     assert L.lcf_measure_peak(7, None) == lcf.ERR_INVALID_ARG
 
 
+def test_scale_exponent_of_the_tensor_path(lcf):
+    """Host logic behind the fp16 split-precision kernels: amax * 2^k must land in [256, 512)."""
+    import math
+    for a in (1.0, 3.53, 255.9, 256.0, 511.9, 512.0, 1.37e-9, 7.7e5, 3.3e12, 6.1e-5, 65504.0, 1e-25, 1e30):
+        k = lcf.scale_exponent(a)
+        assert 256.0 <= math.ldexp(a, k) < 512.0, (a, k)
+        assert lcf.scale_exponent(-a) == k                     # the sign bit is ignored
+    for a in (0.0, float("inf"), float("nan"), 1e-40):          # nothing to scale by: zero, non-finite, denormal
+        assert lcf.scale_exponent(a) == 0
+    assert lcf.scale_exponent(1e-38) == 100 and lcf.scale_exponent(3e38) == -100   # clamped
+
+
 def test_no_cpu_fallback(lcf):
     import torch
     if torch.cuda.is_available():

@@ -163,6 +163,8 @@ SMALL = [
     (64, 48, 64, 2, 2, 14.0, 3.0, synth.SOFT_CURVATURE, 0, 1),    # method 1 (maximum curvature) + sigmoid: the knee cut needs fp64
     (50, 37, 32, 1, 2, 12.0, 3.0, synth.HARD_CURVATURE, 0, 1),    # hard curvature cut, fp64 path
     (50, 37, 24, 2, 1, 12.0, 3.0, synth.SOFT_ADAPTIVE, 0, 1),     # method 6 adaptive weights (follow the small eigenvalues: fp64)
+    (64, 48, 50, 2, 2, 14.0, 3.0, synth.SOFT_ENERGY, 0, 0),       # N = 50: even, not a multiple of 4 -> pair-systolic cluster Jacobi; operand rows padded to 64
+    (48, 40, 72, 2, 2, 12.0, 3.0, synth.SOFT_ENERGY, 0, 0),       # N = 72 = 16 * 4 + 8: padded K and N of the fp16 MMAs, 18 block pairs over two CTAs
 ]
 
 
