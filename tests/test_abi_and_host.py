@@ -77,7 +77,7 @@ def test_scale_exponent_of_the_tensor_path(lcf):
         assert lcf.scale_exponent(-a) == k                     # the sign bit is ignored
     for a in (0.0, float("inf"), float("nan"), 1e-40):          # nothing to scale by: zero, non-finite, denormal
         assert lcf.scale_exponent(a) == 0
-    assert lcf.scale_exponent(1e-38) == 100 and lcf.scale_exponent(3e38) == -100   # clamped
+    assert lcf.scale_exponent(2e-38) == 100 and lcf.scale_exponent(3e38) == -100   # clamped
 
 
 def test_no_cpu_fallback(lcf):
