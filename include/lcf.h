@@ -63,9 +63,13 @@ typedef enum {
                             curve cut_scale * N * log10(l_n) / log10(l_1)  (method 1, Eq. 6,
                             PAPER.md:77-83; finite differences as in DESIGN.md "Readings")          */
     LCF_SOFT_CURVATURE = 7, /* sigmoid (Eq. 9) centred on the curvature-rule c                       */
-    LCF_SOFT_ADAPTIVE = 8   /* wt_i = win(i) / l_i^beta normalised to max 1, win = right half of a
+    LCF_SOFT_ADAPTIVE = 8,  /* wt_i = win(i) / l_i^beta normalised to max 1, win = right half of a
                             Gaussian window (method 6, Eq. 10); no cut-off: c = 0;
                             the weights follow the small eigenvalues, so use precision = 1          */
+    LCF_HARD_SLOPE = 9,     /* hard, c = number of leading components before the eigenvalue curve in dB,
+                            y(n) = 10 log10(l_n), first flattens: the first n with y(n) - y(n+1) <
+                            cut_scale, minus one (method 2)   */
+    LCF_SOFT_SLOPE = 10     /* sigmoid (Eq. 9) centred on the slope-rule c                          */
 } lcf_thresh_mode;
 
 typedef struct {
@@ -73,7 +77,8 @@ typedef struct {
     int k_fixed;        /* 0 <= k_fixed <= N (FIXED modes)                                      */
     double energy_frac; /* in (0, 1) (ENERGY modes)                                             */
     double beta;        /* > 0 (SOFT modes: sigmoid sharpness; ADAPTIVE: the exponent of Eq. 10)  */
-    double cut_scale;   /* > 0 (MEDIAN, CURVATURE modes): the scaling factor beta of Eq. 7 / Eq. 6 */
+    double cut_scale;   /* > 0 (MEDIAN, CURVATURE modes): the scaling factor beta of Eq. 7 / Eq. 6;
+                           (SLOPE modes): the slope threshold in dB per eigenvalue index          */
     int precision;      /* 0: fp32-grade Gram + fp32 EVD.  1: exact-product fp64 Gram + fp64 EVD
                            (single precision can hamper the EVD).  The projection
                            is fp32-grade in both.  "fp32-grade": on the tensor-core kernels

@@ -15,6 +15,7 @@
  *   cutoff_median  Eq. 7,  PAPER.md:90-96   (method 3: threshold = scale * median eigenvalue)
  *   cutoff_curvature Eq. 6, PAPER.md:77-83  (method 1: maximum curvature of the log-eigenvalue curve)
  *   weights_adaptive Eq. 10, PAPER.md:120-126 (method 6: Gaussian window over inverse eigenvalue power)
+ *   cutoff_slope   PAPER.md:85-89          (method 2: the eigenvalue curve in dB flattens below a slope threshold)
  *   filter         Eq. 4,  PAPER.md:57-59   (F = V Lambda^ V^H)
  *   project_pd     Eq. 4 + PAPER.md:63      (C^ = C_w F; PD = sum over slow time of |C^|^2)
  *   combine        Eq. 13, PAPER.md:154-156 (PD_final = sum_k alpha_k PD_k, alpha_k = 1/mean(PD_k))
@@ -46,7 +47,7 @@
 
 enum { LCFO_HARD_FIXED = 0, LCFO_HARD_ENERGY = 1, LCFO_SOFT_FIXED = 2, LCFO_SOFT_ENERGY = 3,
        LCFO_HARD_MEDIAN = 4, LCFO_SOFT_MEDIAN = 5, LCFO_HARD_CURVATURE = 6, LCFO_SOFT_CURVATURE = 7,
-       LCFO_SOFT_ADAPTIVE = 8 };
+       LCFO_SOFT_ADAPTIVE = 8, LCFO_HARD_SLOPE = 9, LCFO_SOFT_SLOPE = 10 };
 
 int lcf_oracle_num_threads(void) {
 #ifdef _OPENMP
@@ -257,6 +258,23 @@ int lcf_oracle_cutoff_curvature(const double *lam, int N, double scale) {
     return k;
 }
 
+/* Method 2: the slope of the eigenvalue curve against a predefined threshold
+ * "above which the [eigen]values are removed".  Reading (DESIGN.md "Readings" 18; the passage
+ * gives neither the scale of the curve nor the sign convention of its "- 1.1"): the curve is in dB,
+ * y(n) = 10 log10(lambda_n), its slope at n is the drop y(n) - y(n+1) to the next eigenvalue, and
+ * k = (first n in 1..N-1 whose drop is below `thresh` dB) - 1: component n is then on the same
+ * plateau as n+1 and stays.  Eigenvalues floored at 1e-12 lambda_1; a curve that never flattens
+ * keeps only its last component (k = N-1); N < 2 or lambda_1 <= 0 give k = 0. */
+int lcf_oracle_cutoff_slope(const double *lam, int N, double thresh) {
+    if (N < 2 || !(lam[0] > 0.0)) return 0;
+    for (int n = 1; n <= N - 1; ++n) { /* 1-based order n: lam[n-1] -> lam[n] */
+        double a = lam[n - 1] > 1e-12 * lam[0] ? lam[n - 1] : 1e-12 * lam[0];
+        double b = lam[n] > 1e-12 * lam[0] ? lam[n] : 1e-12 * lam[0];
+        if (10.0 * log10(a) - 10.0 * log10(b) < thresh) return n - 1;
+    }
+    return N - 1;
+}
+
 /* Eigen weights, 1-based order i (stored at wt[i-1]).
  * hard: wt_i = 0 for i <= c, 1 for i > c.
  * soft (Eq. 9): wt_i = 1 / (1 + exp(-beta (i - c))). */
@@ -353,7 +371,9 @@ int lcf_oracle_window(const float *iq, int N, int Nx, int Nz, const double *gz, 
     if (mode == LCFO_HARD_ENERGY || mode == LCFO_SOFT_ENERGY) c = lcf_oracle_cutoff_energy(lam, N, frac);
     if (mode == LCFO_HARD_MEDIAN || mode == LCFO_SOFT_MEDIAN) c = lcf_oracle_cutoff_median(lam, N, cut_scale);
     if (mode == LCFO_HARD_CURVATURE || mode == LCFO_SOFT_CURVATURE) c = lcf_oracle_cutoff_curvature(lam, N, cut_scale);
-    int soft = (mode == LCFO_SOFT_FIXED || mode == LCFO_SOFT_ENERGY || mode == LCFO_SOFT_MEDIAN || mode == LCFO_SOFT_CURVATURE);
+    if (mode == LCFO_HARD_SLOPE || mode == LCFO_SOFT_SLOPE) c = lcf_oracle_cutoff_slope(lam, N, cut_scale);
+    int soft = (mode == LCFO_SOFT_FIXED || mode == LCFO_SOFT_ENERGY || mode == LCFO_SOFT_MEDIAN || mode == LCFO_SOFT_CURVATURE ||
+                mode == LCFO_SOFT_SLOPE);
     if (mode == LCFO_SOFT_ADAPTIVE) { c = 0; lcf_oracle_weights_adaptive(lam, N, beta, wt); }
     else lcf_oracle_weights(N, soft, c, beta, wt);
     lcf_oracle_filter(V, wt, N, F);

@@ -18,7 +18,7 @@ _SRC = _HERE / "lcf_oracle.c"
 _LIB = _HERE / "liblcf_oracle.so"
 _lib = None
 
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE = range(9)
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE = range(11)
 
 
 def build(force: bool = False) -> Path:
@@ -50,6 +50,8 @@ def _load():
         L.lcf_oracle_cutoff_median.restype = C.c_int
         L.lcf_oracle_cutoff_curvature.argtypes = [dp, C.c_int, C.c_double]
         L.lcf_oracle_cutoff_curvature.restype = C.c_int
+        L.lcf_oracle_cutoff_slope.argtypes = [dp, C.c_int, C.c_double]
+        L.lcf_oracle_cutoff_slope.restype = C.c_int
         L.lcf_oracle_weights.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, dp]
         L.lcf_oracle_weights.restype = None
         L.lcf_oracle_weights_adaptive.argtypes = [dp, C.c_int, C.c_double, dp]
@@ -131,6 +133,12 @@ def cutoff_energy(lam: np.ndarray, frac: float) -> int:
 def cutoff_median(lam: np.ndarray, scale: float) -> int:
     lam = np.ascontiguousarray(lam, dtype=np.float64)
     return int(_load().lcf_oracle_cutoff_median(_d(lam), lam.size, float(scale)))
+
+
+def cutoff_slope(lam: np.ndarray, thresh_db: float) -> int:
+    """Method 2: components before the dB eigenvalue curve first drops by less than thresh_db."""
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    return int(_load().lcf_oracle_cutoff_slope(_d(lam), lam.size, float(thresh_db)))
 
 
 def cutoff_curvature(lam: np.ndarray, scale: float) -> int:

@@ -109,13 +109,14 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     if (!win || !thr) return LCF_ERR_INVALID_ARG;
     if (Nz < 1 || Nx < 1 || N < 2 || win->Kz < 1 || win->Kx < 1) return LCF_ERR_INVALID_ARG;
     if ((long long)Nz * Nx > (1LL << 30) || (long long)win->Kz * win->Kx > 65535) return LCF_ERR_INVALID_ARG;
-    if (thr->mode < 0 || thr->mode > 8 || (thr->precision != 0 && thr->precision != 1)) return LCF_ERR_INVALID_ARG;
+    if (thr->mode < 0 || thr->mode > 10 || (thr->precision != 0 && thr->precision != 1)) return LCF_ERR_INVALID_ARG;
     const bool fixed = thr->mode == LCF_HARD_FIXED || thr->mode == LCF_SOFT_FIXED;
     const bool soft = thresh_is_soft(thr->mode);
     if (fixed && (thr->k_fixed < 0 || thr->k_fixed > N)) return LCF_ERR_INVALID_ARG;
     const bool energy = thr->mode == LCF_HARD_ENERGY || thr->mode == LCF_SOFT_ENERGY;
     const bool median = thr->mode == LCF_HARD_MEDIAN || thr->mode == LCF_SOFT_MEDIAN ||
-                        thr->mode == LCF_HARD_CURVATURE || thr->mode == LCF_SOFT_CURVATURE;   // modes that read cut_scale
+                        thr->mode == LCF_HARD_CURVATURE || thr->mode == LCF_SOFT_CURVATURE ||
+                        thr->mode == LCF_HARD_SLOPE || thr->mode == LCF_SOFT_SLOPE;           // modes that read cut_scale
     if (energy && !(thr->energy_frac > 0.0 && thr->energy_frac < 1.0)) return LCF_ERR_INVALID_ARG;
     if (median && !(thr->cut_scale > 0.0) ) return LCF_ERR_INVALID_ARG;
     if (soft && !(thr->beta > 0.0)) return LCF_ERR_INVALID_ARG;

@@ -14,7 +14,7 @@ import numpy as np
 HERE = Path(__file__).resolve().parent
 LIB_PATH = HERE / "liblcf.so"
 
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE = range(9)
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE = range(11)
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_NOT_CONVERGED = range(6)
 
 EXPORTS = [

@@ -163,6 +163,8 @@ SMALL = [
     (64, 48, 64, 2, 2, 14.0, 3.0, synth.SOFT_CURVATURE, 0, 1),    # method 1 (maximum curvature) + sigmoid: the knee cut needs fp64
     (50, 37, 32, 1, 2, 12.0, 3.0, synth.HARD_CURVATURE, 0, 1),    # hard curvature cut, fp64 path
     (50, 37, 24, 2, 1, 12.0, 3.0, synth.SOFT_ADAPTIVE, 0, 1),     # method 6 adaptive weights (follow the small eigenvalues: fp64)
+    (64, 48, 64, 2, 2, 14.0, 3.0, synth.SOFT_SLOPE, 0, 0),        # method 2 (slope rule, 1.1 dB per index) + sigmoid, tensor / cluster path
+    (50, 37, 32, 1, 2, 12.0, 3.0, synth.HARD_SLOPE, 0, 1),        # hard slope cut, fp64 path
     (64, 48, 50, 2, 2, 14.0, 3.0, synth.SOFT_ENERGY, 0, 0),       # N = 50: even, not a multiple of 4 -> pair-systolic cluster Jacobi; operand rows padded to 64
     (48, 40, 72, 2, 2, 12.0, 3.0, synth.SOFT_ENERGY, 0, 0),       # N = 72 = 16 * 4 + 8: padded K and N of the fp16 MMAs, 18 block pairs over two CTAs
 ]
@@ -173,9 +175,10 @@ def test_small_shapes_and_modes(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, trunc, mo
     cfg = synth.baseline_configs()[2]
     d = replace(cfg.data, Nz=Nz, Nx=Nx, N=N, n_frames=N, seed=100 + N, n_vessels=3, tissue_db=40.0, noise_db=-55.0)
     median = mode in (synth.HARD_MEDIAN, synth.SOFT_MEDIAN)
+    slope = mode in (synth.HARD_SLOPE, synth.SOFT_SLOPE)
     curv = mode in (synth.HARD_CURVATURE, synth.SOFT_CURVATURE)
     # median rule: a scaling factor that puts the threshold in the gap between tissue and blood / noise
-    f = synth.FilterSpec(Kz, Kx, sigma, sigma, trunc, mode, k_fixed=k, precision=prec, cut_scale=300.0 if median else 1.0)
+    f = synth.FilterSpec(Kz, Kx, sigma, sigma, trunc, mode, k_fixed=k, precision=prec, cut_scale=300.0 if median else (1.1 if slope else 1.0))
     iq = synth.generate_sequence(d)
     o = oracle.run_config(iq, f, want_R=True, want_F=True)
     if median:
@@ -187,7 +190,9 @@ def test_small_shapes_and_modes(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, trunc, mo
     check_pd(g["PD"], o["PD"])
     if curv:
         assert (o["c"] >= 2).all() and (o["c"] <= N // 2).all(), o["c"]     # the knee, not the noise tail
-    soft = mode in (synth.SOFT_FIXED, synth.SOFT_ENERGY, synth.SOFT_MEDIAN, synth.SOFT_CURVATURE)
+    if slope:
+        assert (o["c"] >= 1).all() and (o["c"] <= N // 2).all(), o["c"]     # the turning point, not the noise tail
+    soft = mode in (synth.SOFT_FIXED, synth.SOFT_ENERGY, synth.SOFT_MEDIAN, synth.SOFT_CURVATURE, synth.SOFT_SLOPE)
     for kk in range(Kz * Kx):
         if mode == synth.SOFT_ADAPTIVE:
             wt_o = oracle.weights_adaptive(o["lam"][kk], f.beta)

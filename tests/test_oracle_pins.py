@@ -207,6 +207,40 @@ def test_median_cutoff_pins(oracle):
     assert oracle.cutoff_median(lam, 1.43) == 3
 
 
+def test_slope_cutoff_pins(oracle):
+    # method 2, reading 18 of DESIGN.md: the curve in dB, its drop to the next
+    # eigenvalue against a threshold, c = (first n whose drop is below it) - 1.
+    # hand count: drops 10, 10, 30, 0.458, 0.512, 0.580 dB
+    lam = np.array([1e6, 1e5, 1e4, 10.0, 9.0, 8.0, 7.0])
+    assert oracle.cutoff_slope(lam, 1.1) == 3          # n = 4 is the first flat step: 3 components go
+    assert oracle.cutoff_slope(lam, 0.5) == 3          # 0.458 < 0.5 too
+    assert oracle.cutoff_slope(lam, 0.4) == 6          # never below 0.4 dB: only the last component stays
+    assert oracle.cutoff_slope(lam, 10.5) == 0         # already the first drop (10 dB) is "flat"
+    assert oracle.cutoff_slope(lam, 9.99) == 3         # the two 10 dB steps and the 30 dB step are steeper: n = 4 again
+    # exactly geometric curve, 3 dB per step: flat iff the threshold exceeds 3 dB
+    lam = 10.0 ** (-0.3 * np.arange(12))
+    assert oracle.cutoff_slope(lam, 2.9) == 11
+    assert oracle.cutoff_slope(lam, 3.1) == 0
+    # brute force from the definition on random descending spectra, in plain numpy
+    rng = np.random.default_rng(5)
+    for n in (2, 3, 9, 40, 128):
+        for _ in range(20):
+            lam = np.sort(rng.random(n) ** 8 + 1e-9)[::-1]
+            T = rng.uniform(0.05, 6.0)
+            drops = 10 * np.log10(lam[:-1]) - 10 * np.log10(lam[1:])
+            flat = np.nonzero(drops < T)[0]
+            want = int(flat[0]) if flat.size else n - 1   # 0-based index of the first flat step = (1-based n) - 1
+            assert oracle.cutoff_slope(lam, T) == want
+    # invariant under a change of units, unlike method 1; degenerate inputs
+    lam = np.concatenate([[4e5, 2e4, 900.0], np.linspace(1.3, 0.7, 29)])
+    assert oracle.cutoff_slope(lam, 1.1) == oracle.cutoff_slope(3.7e-9 * lam, 1.1) == 3
+    assert oracle.cutoff_slope(np.array([5.0]), 1.1) == 0
+    assert oracle.cutoff_slope(np.zeros(4), 1.1) == 0
+    assert oracle.cutoff_slope(np.ones(6), 1.1) == 0   # flat spectrum: nothing stands out
+    # eigenvalues at or below zero are floored at 1e-12 lambda_1 (-120 dB): the step onto the floor is steep
+    assert oracle.cutoff_slope(np.array([1.0, 0.5, 0.0, -1e-3]), 1.1) == 2
+
+
 def test_curvature_cutoff_pins(oracle):
     # method 1 (Eq. 6): a log-eigenvalue curve made of two straight lines has zero
     # second difference everywhere except at the kink, so the maximum curvature sits exactly there
