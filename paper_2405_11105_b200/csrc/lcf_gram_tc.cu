@@ -47,8 +47,8 @@ using namespace sm100;
 
 constexpr int GTC_PX = 16;                 // pixels per tile
 constexpr int GTC_RT = 128;                // operand tile rows (frames, zero padded)
-constexpr int GTC_RAW_STAGES = 4;
-constexpr int GTC_OP_STAGES = 4;
+constexpr int GTC_RAW_STAGES = 6;
+constexpr int GTC_OP_STAGES = 6;
 constexpr int GTC_CONV_WARPS = 8;
 constexpr int GTC_DRAIN_WARPS = 8;
 constexpr int GTC_FIRST_CONV = 4;            // warps 0-3: TMA producer, MMA issuer, two idle (one warpgroup)
@@ -58,7 +58,10 @@ constexpr int GTC_PAIR_BYTES = 2 * GTC_RT * GTC_PX * 2;  // one stacked fp16 ope
 constexpr int GTC_OP_BYTES = 2 * GTC_PAIR_BYTES;         // [Rh | Rl], [Ih | Il]
 constexpr int GTC_LBO = 2 * GTC_RT * 16;                 // next 8-pixel K chunk (256 rows of 16 bytes)
 constexpr int GTC_SBO = 128;                             // next 8-frame row group
-constexpr int GTC_TASKS = (2 * (GTC_RT / 32) + GTC_CONV_WARPS - 1) / GTC_CONV_WARPS;   // converter tasks per thread per tile
+constexpr int GTC_CONV_GROUPS = 2;           // converter groups working on alternate tiles
+constexpr int GTC_WPG = GTC_CONV_WARPS / GTC_CONV_GROUPS;
+// a group must see every use of the stages it touches (an mbarrier waiter may not skip a phase)
+static_assert(GTC_RAW_STAGES % GTC_CONV_GROUPS == 0 && GTC_OP_STAGES % GTC_CONV_GROUPS == 0, "stages per group");
 
 struct GtcArgs {
     int N, Np, Nz, Nx, Kz;
@@ -128,8 +131,8 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
     for (int i = tid * 16; i < GTC_OP_STAGES * GTC_OP_BYTES; i += GTC_THREADS * 16) *reinterpret_cast<uint4*>(ops + i) = make_uint4(0, 0, 0, 0);
     fence_proxy_async_smem();
     if (tid == 0) {
-        for (int s = 0; s < GTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], GTC_CONV_WARPS); }
-        for (int s = 0; s < GTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], GTC_CONV_WARPS); mbar_init(&bars->opempty[s], 1); }
+        for (int s = 0; s < GTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], GTC_WPG); }
+        for (int s = 0; s < GTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], GTC_WPG); mbar_init(&bars->opempty[s], 1); }
         mbar_init(&bars->accfull, 1);
         mbar_init(&bars->accempty, GTC_DRAIN_WARPS);
         mbar_fence_init();
@@ -224,59 +227,50 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
         const int nwt = 2 * ((N + 31) / 32);          // warp tasks per tile: (8-pixel chunk, 32-frame block)
         const uint32_t lo_bytes = (uint32_t)a.Np * 16u;
         const uint32_t raw_u32 = smem_u32(raw), ops_u32 = smem_u32(ops), wts_u32 = smem_u32(&bars->wts[0][0]);
-        bool tvalid[GTC_TASKS];
-        uint32_t twt[GTC_TASKS], trd[GTC_TASKS][4], tdst[GTC_TASKS];
-#pragma unroll
-        for (int j = 0; j < GTC_TASKS; ++j) {
-            const int wt = cw + j * GTC_CONV_WARPS;
-            const int c8 = wt & 1, fr = (wt >> 1) * 32 + lane;
-            tvalid[j] = wt < nwt && fr < N;
-            const uint32_t sw = (uint32_t)(fr & 7);
-            twt[j] = (uint32_t)c8 * 64u;                   // 8 pixels x (w, w)
-#pragma unroll
-            for (int u = 0; u < 4; ++u) trd[j][u] = (uint32_t)fr * 128u + ((((uint32_t)(4 * c8 + u)) ^ sw) << 4);
-            tdst[j] = (uint32_t)c8 * GTC_LBO + (uint32_t)fr * 16u;      // hi row; the lo row is Np rows further
-        }
+        // The converter warps form GTC_CONV_GROUPS groups that take alternate tiles, so that one
+        // group's load -> convert -> store -> fence latency overlaps the other's; a warp walks its
+        // tasks of a tile one after the other (same registers as one task).
+        const int grp = cw / GTC_WPG, gw = cw % GTC_WPG;
         uint32_t it = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
             const int nt = a.segs[sg].ntile;
             for (int t = 0; t < nt; ++t, ++it) {
+                if ((int)(it % GTC_CONV_GROUPS) != grp) continue;
                 const int s = it % GTC_RAW_STAGES, o = it % GTC_OP_STAGES;
                 const uint32_t ph = (it / GTC_RAW_STAGES) & 1, pho = (it / GTC_OP_STAGES) & 1;
                 const uint32_t rs = raw_u32 + (uint32_t)s * a.raw_stride;
                 const uint32_t os = ops_u32 + (uint32_t)o * GTC_OP_BYTES;
                 const uint32_t ws = wts_u32 + (uint32_t)s * (GTC_PX * 8);
                 mbar_wait(&bars->full[s], ph);
-                ulonglong2 wq[GTC_TASKS][4], pq[GTC_TASKS][4];
-#pragma unroll
-                for (int j = 0; j < GTC_TASKS; ++j)
-                    if (tvalid[j]) {
+                mbar_wait(&bars->opempty[o], pho ^ 1);
+#pragma unroll 1
+                for (int wt = gw; wt < nwt; wt += GTC_WPG) {
+                    const int c8 = wt & 1, fr = (wt >> 1) * 32 + lane;
+                    if (fr < N) {
+                        const uint32_t sw = (uint32_t)(fr & 7);
+                        ulonglong2 wq[4], pq[4];
 #pragma unroll
                         for (int u = 0; u < 4; ++u) {
-                            wq[j][u] = lds128u(ws + twt[j] + 16 * u);      // (w0, w0), (w1, w1) of pixels 2u, 2u+1 of the chunk
-                            pq[j][u] = lds128u(rs + trd[j][u]);            // (re0, im0), (re1, im1)
+                            wq[u] = lds128u(ws + (uint32_t)c8 * 64u + 16 * u);                                        // (w0, w0), (w1, w1) of pixels 2u, 2u+1 of the chunk
+                            pq[u] = lds128u(rs + (uint32_t)fr * 128u + ((((uint32_t)(4 * c8 + u)) ^ sw) << 4));      // (re0, im0), (re1, im1)
                         }
-                    }
-                mbar_wait(&bars->opempty[o], pho ^ 1);
-#pragma unroll
-                for (int j = 0; j < GTC_TASKS; ++j)
-                    if (tvalid[j]) {
                         uint32_t rh[4], rl[4], ih[4], il[4];
 #pragma unroll
                         for (int u = 0; u < 4; ++u) {
-                            const float2 v0 = mul2(pq[j][u].x, wq[j][u].x), v1 = mul2(pq[j][u].y, wq[j][u].y);
+                            const float2 v0 = mul2(pq[u].x, wq[u].x), v1 = mul2(pq[u].y, wq[u].y);
                             f16_split2(v0.x, v1.x, rh[u], rl[u]);
                             f16_split2(v0.y, v1.y, ih[u], il[u]);
                         }
-                        const uint32_t dst = os + tdst[j];
+                        const uint32_t dst = os + (uint32_t)c8 * GTC_LBO + (uint32_t)fr * 16u;      // hi row; the lo row is Np rows further
                         sts128u(dst, rh[0], rh[1], rh[2], rh[3]);
                         sts128u(dst + GTC_PAIR_BYTES, ih[0], ih[1], ih[2], ih[3]);
                         sts128u(dst + lo_bytes, rl[0], rl[1], rl[2], rl[3]);
                         sts128u(dst + GTC_PAIR_BYTES + lo_bytes, il[0], il[1], il[2], il[3]);
                     }
+                }
                 fence_proxy_async_smem();             // this lane's operand writes -> async proxy
                 __syncwarp();
-                if (lane == 0) {                      // one arrival per converter warp on each barrier
+                if (lane == 0) {                      // one arrival per converter warp of the group on each barrier
                     mbar_arrive(&bars->empty[s]);     // raw stage (and its weights) consumed
                     mbar_arrive(&bars->opfull[o]);
                 }
