@@ -302,26 +302,24 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
 // B_k [N][Ns] complex (row = frame, column = eigen slot) -> per (window, 64-column block) the
 // resident fp16 operand tile [Kp/8 chunks][256 rows][8 frames]: rows = Re hi | Im hi | Re lo | Im lo of 256 B
 __global__ void proj_tc_pack_kernel(const float2* B, int N, int Ns, int Kp, int NB, float* bpack) {
-    const int kb = blockIdx.x;                       // k * NB + b
+    const int kb = blockIdx.x / (Kp / 8), c8 = blockIdx.x - kb * (Kp / 8);   // kb = k * NB + b; one 8-frame chunk per CTA
     const int k = kb / NB, b = kb - k * NB;
     const float2* Bk = B + (size_t)k * N * Ns;
-    uint4* out = reinterpret_cast<uint4*>(bpack + (size_t)kb * (Kp / 8) * 1024);
-    for (int e = threadIdx.x; e < (Kp / 8) * 256; e += blockDim.x) {
-        const int c8 = e >> 8, r = e & 255;
-        const int u = b * PTC_UB + (r & 63);
-        const bool im = (r >> 6) & 1, lo = r >= 128;
-        float x[8];
+    uint4* out = reinterpret_cast<uint4*>(bpack + (size_t)kb * (Kp / 8) * 1024) + (size_t)c8 * 256;
+    const int r = threadIdx.x;                       // 256 rows: Re hi | Im hi | Re lo | Im lo
+    const int u = b * PTC_UB + (r & 63);
+    const bool im = (r >> 6) & 1, lo = r >= 128;
+    float x[8];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            const int t = 8 * c8 + i;
-            x[i] = 0.f;
-            if (t < N && u < Ns) { const float2 c = Bk[(size_t)t * Ns + u]; x[i] = (im ? c.y : c.x) * PTC_B_SCALE; }
-        }
-        uint32_t h[4], l[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) f16_split2(x[2 * i], x[2 * i + 1], h[i], l[i]);
-        out[e] = lo ? make_uint4(l[0], l[1], l[2], l[3]) : make_uint4(h[0], h[1], h[2], h[3]);
+    for (int i = 0; i < 8; ++i) {
+        const int t = 8 * c8 + i;
+        x[i] = 0.f;
+        if (t < N && u < Ns) { const float2 c = Bk[(size_t)t * Ns + u]; x[i] = (im ? c.y : c.x) * PTC_B_SCALE; }
     }
+    uint32_t h[4], l[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) f16_split2(x[2 * i], x[2 * i + 1], h[i], l[i]);
+    out[r] = lo ? make_uint4(l[0], l[1], l[2], l[3]) : make_uint4(h[0], h[1], h[2], h[3]);
 }
 
 // bits of max(|re|, |im|) over the ensemble (non-negative floats order like their bit patterns)
@@ -446,7 +444,7 @@ cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::ve
 cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     if (p->ptc_nseg == 0 || p->n_pitems == 0) return cudaSuccess;
     if (p->ptc_tmap_iq != (const void*)iq && !ptc_encode_map(p, iq)) return cudaErrorInvalidValue;
-    proj_tc_pack_kernel<<<p->K * p->ptc_NB, 256, 0, st>>>(p->B_d, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
+    proj_tc_pack_kernel<<<p->K * p->ptc_NB * (p->ptc_Kp / 8), 256, 0, st>>>(p->B_d, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     PtcArgs a;
