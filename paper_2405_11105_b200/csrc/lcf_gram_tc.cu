@@ -354,21 +354,30 @@ __global__ void __launch_bounds__(GTC_THREADS, 1) gram_tc_kernel(const __grid_co
     if (warp == 1) tmem_dealloc<512>(tmem);
 }
 
-// R_k = sum over the window's segments, in fp64:  Re R = P0 + P0^T,  Im R = P1 - P1^T  (P0 = D0 / 2 + H, P1 = G0 + L)
-template <typename T>
+// R_k = sum over the window's segments, in fp64:  Re R = P0 + P0^T,  Im R = P1 - P1^T  (P0 = D0 / 2 + H, P1 = G0 + L).
 // R_k stays in the power-of-two data scale (squared): the fp32 EVD then works on numbers of a fixed
 // magnitude whatever the units of the input; the EVD kernels unscale the eigenvalues, lcf_get_gram R.
+// One 16 x 16 tile of R per CTA; the transposed tile comes through shared memory so that both reads
+// of the partials are coalesced.
+template <typename T>
 __global__ void gram_tc_reduce_kernel(const float* part, const int* seg_first, int N, void* Rv) {
-    const int k = blockIdx.z;
-    const int i = blockIdx.y * 16 + threadIdx.y, j = blockIdx.x * 16 + threadIdx.x;
-    if (i >= N || j >= N) return;
+    __shared__ float t0[16][17], t1[16][17];
+    const int k = blockIdx.z, tx = threadIdx.x, ty = threadIdx.y;
+    const int i0 = blockIdx.y * 16, j0 = blockIdx.x * 16;
+    const int i = i0 + ty, j = j0 + tx;
     double re = 0.0, im = 0.0;
     for (int s = seg_first[k]; s < seg_first[k + 1]; ++s) {
         const float* p = part + (size_t)s * 2 * 128 * 128;
-        const size_t ij = (size_t)i * 128 + j, ji = (size_t)j * 128 + i;
-        re += (double)p[ij] + (double)p[ji];
-        im += (double)p[16384 + ij] - (double)p[16384 + ji];
+        const size_t ij = (size_t)i * 128 + j, tr = (size_t)(j0 + ty) * 128 + (i0 + tx);   // rows < 128 always exist
+        const float a0 = p[ij], a1 = p[16384 + ij];
+        __syncthreads();
+        t0[ty][tx] = p[tr];
+        t1[ty][tx] = p[16384 + tr];
+        __syncthreads();
+        re += (double)a0 + (double)t0[tx][ty];          // P0[i][j] + P0[j][i]
+        im += (double)a1 - (double)t1[tx][ty];
     }
+    if (i >= N || j >= N) return;
     if (i == j) im = 0.0;
     if (sizeof(T) == 4) {
         float2* R = reinterpret_cast<float2*>(Rv) + (size_t)k * N * N;
