@@ -325,12 +325,12 @@ def run_ours(args, cfg):
     if dom == "evd":
         roofline["note"] = ("the EVD is bound by instruction issue and dependency latency, not by a memory system: the "
                             "cluster Jacobi keeps the columns in registers (16 warps per SM, issue slots 63 % busy, FMA pipe "
-                            "49 %, profiles/r1f) and the flops counted here are the rotations' 36 per row and pair only")
+                            "49 %, profiles/r1g) and the flops counted here are the rotations' 36 per row and pair only")
         # DRAM bytes of one Cholesky + one cluster-Jacobi launch, from the ncu --set full capture
-        # profiles/r1f_ncu_full_summary.txt (dram__bytes_read.sum + dram__bytes_write.sum), config 2
+        # profiles/r1g_ncu_full_summary.txt (dram__bytes_read.sum + dram__bytes_write.sum), config 2
         if args.config == 2 and "jacobi_cluster" in roofline.get("kernel", ""):
             roofline["traffic"] = 8.4544e6 + 8.7168e6
-            roofline["traffic_source"] = "profiles/r1f_ncu_full_summary.txt"
+            roofline["traffic_source"] = "profiles/r1g_ncu_full_summary.txt"
 
     # ---- BASELINE.json config 4: 16 ensembles of 100 frames at stride 50 over one resident
     # 900-frame sequence (pointer offsets, no copies): sustained power-Doppler frames/s, latency
