@@ -15,7 +15,8 @@
  *   cutoff_median  Eq. 7,  PAPER.md:90-96   (method 3: threshold = scale * median eigenvalue)
  *   cutoff_curvature Eq. 6, PAPER.md:77-83  (method 1: maximum curvature of the log-eigenvalue curve)
  *   weights_adaptive Eq. 10, PAPER.md:120-126 (method 6: Gaussian window over inverse eigenvalue power)
- *   cutoff_slope   PAPER.md:85-89          (method 2: the eigenvalue curve in dB flattens below a slope threshold)
+ *   cutoff_slope   PAPER.md:85-89          (method 2: slope of the eigenvalue curve y(n) = lambda_n against a threshold)
+ *   cutoff_slope_db  same passage           (named variant: the same rule on the curve in dB)
  *   filter         Eq. 4,  PAPER.md:57-59   (F = V Lambda^ V^H)
  *   project_pd     Eq. 4 + PAPER.md:63      (C^ = C_w F; PD = sum over slow time of |C^|^2)
  *   combine        Eq. 13, PAPER.md:154-156 (PD_final = sum_k alpha_k PD_k, alpha_k = 1/mean(PD_k))
@@ -47,7 +48,7 @@
 
 enum { LCFO_HARD_FIXED = 0, LCFO_HARD_ENERGY = 1, LCFO_SOFT_FIXED = 2, LCFO_SOFT_ENERGY = 3,
        LCFO_HARD_MEDIAN = 4, LCFO_SOFT_MEDIAN = 5, LCFO_HARD_CURVATURE = 6, LCFO_SOFT_CURVATURE = 7,
-       LCFO_SOFT_ADAPTIVE = 8, LCFO_HARD_SLOPE = 9, LCFO_SOFT_SLOPE = 10 };
+       LCFO_SOFT_ADAPTIVE = 8, LCFO_HARD_SLOPE = 9, LCFO_SOFT_SLOPE = 10, LCFO_HARD_SLOPE_DB = 11, LCFO_SOFT_SLOPE_DB = 12 };
 
 int lcf_oracle_num_threads(void) {
 #ifdef _OPENMP
@@ -258,16 +259,34 @@ int lcf_oracle_cutoff_curvature(const double *lam, int N, double scale) {
     return k;
 }
 
-/* Method 2: the slope of the eigenvalue curve against a predefined threshold
- * "above which the [eigen]values are removed".  Reading (DESIGN.md "Readings" 18; the passage
- * gives neither the scale of the curve nor the sign convention of its "- 1.1"): the curve is in dB,
- * y(n) = 10 log10(lambda_n), its slope at n is the drop y(n) - y(n+1) to the next eigenvalue, and
- * k = (first n in 1..N-1 whose drop is below `thresh` dB) - 1: component n is then on the same
- * plateau as n+1 and stays.  Eigenvalues floored at 1e-12 lambda_1; a curve that never flattens
- * keeps only its last component (k = N-1); N < 2 or lambda_1 <= 0 give k = 0. */
+/* Method 2: "calculates the slope, or the first derivative of the singular value
+ * curve and requires a properly predefined slope threshold above which the singular values are
+ * removed ... the slope estimation of the eigenvalue curve y(n) = lambda_n and the identified
+ * eigenvalue cutoff based [on] a predefined slope threshold of -1.1."
+ * As printed: the curve is the eigenvalues themselves (linear, unlike method 1's log10).  The
+ * descending curve has slope y(n+1) - y(n) <= 0 (forward difference); the steep leading part
+ * (slope below -T, i.e. "above" the threshold in magnitude) is tissue and is removed; the cut is
+ * where the curve first flattens:  k = (first n in 1..N-1 with y(n) - y(n+1) < T) - 1.
+ * Reading (DESIGN.md "Readings" 18): the paper's -1.1 is in the units of the authors' data, so the
+ * curve is taken relative to its first point, y(n) = lambda_n / lambda_1, and `thresh` = T > 0 is
+ * the magnitude of the slope per eigenvalue index on that curve.  A curve that never flattens keeps
+ * only its last component (k = N-1); N < 2 or lambda_1 <= 0 give k = 0. */
 int lcf_oracle_cutoff_slope(const double *lam, int N, double thresh) {
     if (N < 2 || !(lam[0] > 0.0)) return 0;
     for (int n = 1; n <= N - 1; ++n) { /* 1-based order n: lam[n-1] -> lam[n] */
+        double drop = lam[n - 1] / lam[0] - lam[n] / lam[0];
+        if (drop < thresh) return n - 1;
+    }
+    return N - 1;
+}
+
+/* Named variant of method 2 (not the printed form): the same rule on the curve in dB,
+ * y(n) = 10 log10(lambda_n) -- independent of the units of the data without a normalisation, and
+ * the scale on which eigenvalue curves are usually drawn.  `thresh` = drop in dB per eigenvalue
+ * index; eigenvalues floored at 1e-12 lambda_1 so that the logarithm exists. */
+int lcf_oracle_cutoff_slope_db(const double *lam, int N, double thresh) {
+    if (N < 2 || !(lam[0] > 0.0)) return 0;
+    for (int n = 1; n <= N - 1; ++n) {
         double a = lam[n - 1] > 1e-12 * lam[0] ? lam[n - 1] : 1e-12 * lam[0];
         double b = lam[n] > 1e-12 * lam[0] ? lam[n] : 1e-12 * lam[0];
         if (10.0 * log10(a) - 10.0 * log10(b) < thresh) return n - 1;
@@ -372,8 +391,9 @@ int lcf_oracle_window(const float *iq, int N, int Nx, int Nz, const double *gz, 
     if (mode == LCFO_HARD_MEDIAN || mode == LCFO_SOFT_MEDIAN) c = lcf_oracle_cutoff_median(lam, N, cut_scale);
     if (mode == LCFO_HARD_CURVATURE || mode == LCFO_SOFT_CURVATURE) c = lcf_oracle_cutoff_curvature(lam, N, cut_scale);
     if (mode == LCFO_HARD_SLOPE || mode == LCFO_SOFT_SLOPE) c = lcf_oracle_cutoff_slope(lam, N, cut_scale);
+    if (mode == LCFO_HARD_SLOPE_DB || mode == LCFO_SOFT_SLOPE_DB) c = lcf_oracle_cutoff_slope_db(lam, N, cut_scale);
     int soft = (mode == LCFO_SOFT_FIXED || mode == LCFO_SOFT_ENERGY || mode == LCFO_SOFT_MEDIAN || mode == LCFO_SOFT_CURVATURE ||
-                mode == LCFO_SOFT_SLOPE);
+                mode == LCFO_SOFT_SLOPE || mode == LCFO_SOFT_SLOPE_DB);
     if (mode == LCFO_SOFT_ADAPTIVE) { c = 0; lcf_oracle_weights_adaptive(lam, N, beta, wt); }
     else lcf_oracle_weights(N, soft, c, beta, wt);
     lcf_oracle_filter(V, wt, N, F);
@@ -407,13 +427,14 @@ void lcf_oracle_combine(const double *PDk_all /* [K][P] */, int K, size_t P, dou
 
 /* Whole path for one ensemble: all K = Kz*Kx windows (k = kx*Kz + kz), then Eq. 13.
  * Windows are independent, so they run under OpenMP when compiled with it; the combination is
- * serial in k order.  Optional outputs (NULL to skip): R_all/F_all [K][N][N][2], mean_all [K].
+ * serial in k order.  Optional outputs (NULL to skip): R_all/F_all/V_all [K][N][N][2] (V: columns =
+ * eigenvectors, descending eigenvalue order), mean_all [K].
  * Returns 0, or -(k+1) for the first window whose Jacobi iteration did not converge. */
 int lcf_oracle_run(const float *iq, int N, int Nx, int Nz, int Kz, int Kx,
                    double sigma_z, double sigma_x, double trunc,
                    int mode, int k_fixed, double frac, double beta, double cut_scale,
                    double *PD /* [Nx][Nz] */, double *lam_all /* [K][N] */, int *c_all /* [K] */,
-                   double *mean_all, double *R_all, double *F_all) {
+                   double *mean_all, double *R_all, double *F_all, double *V_all) {
     int K = Kz * Kx;
     size_t P = (size_t)Nx * Nz, nn = (size_t)N * N;
     double *gz = (double *)malloc(sizeof(double) * (size_t)Kz * Nz);
@@ -434,8 +455,8 @@ int lcf_oracle_run(const float *iq, int N, int Nx, int Nz, int Kz, int Kx,
         const double *gzk = gz + (size_t)kz * Nz, *gxk = gx + (size_t)kx * Nx;
         double *PDk = (double *)malloc(sizeof(double) * P);
         status[k] = lcf_oracle_window(iq, N, Nx, Nz, gzk, gxk, mode, k_fixed, frac, beta, cut_scale,
-                                      R_all ? R_all + 2 * nn * k : NULL, lam_all + (size_t)N * k, NULL,
-                                      c_all + k, NULL, F_all ? F_all + 2 * nn * k : NULL, PDk, means + k);
+                                      R_all ? R_all + 2 * nn * k : NULL, lam_all + (size_t)N * k,
+                                      V_all ? V_all + 2 * nn * k : NULL, c_all + k, NULL, F_all ? F_all + 2 * nn * k : NULL, PDk, means + k);
         int z0 = Nz, z1 = -1, x0 = Nx, x1 = -1;
         for (int z = 0; z < Nz; ++z) if (gzk[z] != 0.0) { if (z < z0) z0 = z; if (z > z1) z1 = z; }
         for (int x = 0; x < Nx; ++x) if (gxk[x] != 0.0) { if (x < x0) x0 = x; if (x > x1) x1 = x; }

@@ -18,7 +18,7 @@ _SRC = _HERE / "lcf_oracle.c"
 _LIB = _HERE / "liblcf_oracle.so"
 _lib = None
 
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE = range(11)
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE, HARD_SLOPE_DB, SOFT_SLOPE_DB = range(13)
 
 
 def build(force: bool = False) -> Path:
@@ -52,6 +52,8 @@ def _load():
         L.lcf_oracle_cutoff_curvature.restype = C.c_int
         L.lcf_oracle_cutoff_slope.argtypes = [dp, C.c_int, C.c_double]
         L.lcf_oracle_cutoff_slope.restype = C.c_int
+        L.lcf_oracle_cutoff_slope_db.argtypes = [dp, C.c_int, C.c_double]
+        L.lcf_oracle_cutoff_slope_db.restype = C.c_int
         L.lcf_oracle_weights.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, dp]
         L.lcf_oracle_weights.restype = None
         L.lcf_oracle_weights_adaptive.argtypes = [dp, C.c_int, C.c_double, dp]
@@ -67,7 +69,7 @@ def _load():
         L.lcf_oracle_combine.restype = None
         L.lcf_oracle_run.argtypes = [fp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
                                      C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
-                                     C.c_double, dp, dp, ip, dp, dp, dp]
+                                     C.c_double, dp, dp, ip, dp, dp, dp, dp]
         L.lcf_oracle_run.restype = C.c_int
         _lib = L
     return _lib
@@ -135,10 +137,16 @@ def cutoff_median(lam: np.ndarray, scale: float) -> int:
     return int(_load().lcf_oracle_cutoff_median(_d(lam), lam.size, float(scale)))
 
 
-def cutoff_slope(lam: np.ndarray, thresh_db: float) -> int:
-    """Method 2: components before the dB eigenvalue curve first drops by less than thresh_db."""
+def cutoff_slope(lam: np.ndarray, thresh: float) -> int:
+    """Method 2 as printed: components before the curve lambda_n / lambda_1 first drops by less than thresh."""
     lam = np.ascontiguousarray(lam, dtype=np.float64)
-    return int(_load().lcf_oracle_cutoff_slope(_d(lam), lam.size, float(thresh_db)))
+    return int(_load().lcf_oracle_cutoff_slope(_d(lam), lam.size, float(thresh)))
+
+
+def cutoff_slope_db(lam: np.ndarray, thresh_db: float) -> int:
+    """Named variant of method 2: the same rule on the curve in dB."""
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    return int(_load().lcf_oracle_cutoff_slope_db(_d(lam), lam.size, float(thresh_db)))
 
 
 def cutoff_curvature(lam: np.ndarray, scale: float) -> int:
@@ -204,20 +212,21 @@ def combine(PDk_all: np.ndarray):
 
 def run(iq: np.ndarray, Kz: int, Kx: int, sigma_z: float, sigma_x: float, trunc: float, mode: int,
         k_fixed: int = 0, frac: float = 0.995, beta: float = 0.5, want_R: bool = False,
-        want_F: bool = False, cut_scale: float = 1.0) -> dict:
+        want_F: bool = False, cut_scale: float = 1.0, want_V: bool = False) -> dict:
     """Whole path for one ensemble (OpenMP over windows)."""
     a, p, N, Nx, Nz = _iq(iq)
     K = Kz * Kx
     PD = np.empty((Nx, Nz)); lam = np.empty((K, N)); c = np.empty(K, dtype=np.int32); mean = np.empty(K)
     R = np.empty((K, N, N), dtype=np.complex128) if want_R else None
     F = np.empty((K, N, N), dtype=np.complex128) if want_F else None
+    V = np.empty((K, N, N), dtype=np.complex128) if want_V else None
     rc = _load().lcf_oracle_run(p, N, Nx, Nz, Kz, Kx, float(sigma_z), float(sigma_x), float(trunc), int(mode),
                                 int(k_fixed), float(frac), float(beta), float(cut_scale), _d(PD), _d(lam),
                                 c.ctypes.data_as(C.POINTER(C.c_int)), _d(mean),
-                                _d(R) if want_R else None, _d(F) if want_F else None)
+                                _d(R) if want_R else None, _d(F) if want_F else None, _d(V) if want_V else None)
     if rc != 0:
         raise RuntimeError(f"oracle Jacobi did not converge for window {-rc - 1}")
-    return dict(PD=PD, lam=lam, c=c, mean=mean, R=R, F=F)
+    return dict(PD=PD, lam=lam, c=c, mean=mean, R=R, F=F, V=V)
 
 
 def run_config(iq: np.ndarray, filt, **kw) -> dict:

@@ -208,20 +208,54 @@ def test_median_cutoff_pins(oracle):
 
 
 def test_slope_cutoff_pins(oracle):
-    # method 2, reading 18 of DESIGN.md: the curve in dB, its drop to the next
-    # eigenvalue against a threshold, c = (first n whose drop is below it) - 1.
-    # hand count: drops 10, 10, 30, 0.458, 0.512, 0.580 dB
+    # method 2 as printed: slope of the eigenvalue curve y(n) = lambda_n, here relative to
+    # its first point (reading 18 of DESIGN.md); c = (first n whose drop y(n) - y(n+1) is below T) - 1.
+    # hand count: lambda / lambda_1 = 1, .5, .2, .19, .18, .17 -> drops .5, .3, .01, .01, .01
+    lam = np.array([100.0, 50.0, 20.0, 19.0, 18.0, 17.0])
+    assert oracle.cutoff_slope(lam, 0.05) == 2         # n = 3 is the first flat step: 2 components go
+    assert oracle.cutoff_slope(lam, 0.4) == 1          # 0.3 < 0.4: only the first step is steep
+    assert oracle.cutoff_slope(lam, 0.6) == 0          # already the first drop (0.5) is "flat"
+    assert oracle.cutoff_slope(lam, 0.005) == 5        # never below 0.005: only the last component stays
+    # the strict "<": a threshold exactly on a drop that floating point represents exactly (0.5) keeps that step steep
+    assert oracle.cutoff_slope(np.array([8.0, 4.0, 3.0]), 0.5) == 1
+    # exactly arithmetic curve (constant slope -1/16 per index, exact in binary): flat iff the threshold exceeds it
+    lam = 1.0 - np.arange(12) / 16.0
+    assert oracle.cutoff_slope(lam, 0.0624) == 11
+    assert oracle.cutoff_slope(lam, 0.0626) == 0
+    # brute force from the definition on random descending spectra: numpy's first difference of the curve
+    rng = np.random.default_rng(5)
+    for n in (2, 3, 9, 40, 128):
+        for _ in range(20):
+            lam = np.sort(rng.random(n) ** 8 + 1e-9)[::-1]
+            T = 10.0 ** rng.uniform(-6, -0.5)
+            slope = np.diff(lam / lam[0])                 # y(n+1) - y(n) <= 0
+            flat = np.nonzero(slope > -T)[0]              # slope above the (negative) threshold: flat
+            want = int(flat[0]) if flat.size else n - 1   # 0-based index of the first flat step = (1-based n) - 1
+            assert oracle.cutoff_slope(lam, T) == want
+    # unit-free through the normalisation by lambda_1 (a power of two keeps the quotients bit-identical)
+    lam = np.concatenate([[4e5, 2e4, 900.0], np.linspace(1.3, 0.7, 29)])
+    assert oracle.cutoff_slope(lam, 1e-3) == oracle.cutoff_slope(2.0 ** -30 * lam, 1e-3) == 3
+    # differs from the dB variant where the curve is steep in dB but already flat on the linear scale:
+    # drops 0.95, 0.04775, ... of lambda_1 (only the first is above 0.1) against 13.0, 13.5, 28.4, 0.07 dB
+    assert oracle.cutoff_slope(lam, 0.1) == 1 and oracle.cutoff_slope_db(lam, 1.0) == 3
+    assert oracle.cutoff_slope(np.array([5.0]), 0.1) == 0
+    assert oracle.cutoff_slope(np.zeros(4), 0.1) == 0
+    assert oracle.cutoff_slope(np.ones(6), 0.1) == 0   # flat spectrum: nothing stands out
+    assert oracle.cutoff_slope(np.array([1.0, 0.5, 0.0, -1e-3]), 0.1) == 2   # no floor on the linear curve: 0 -> -1e-3 is flat
+
+
+def test_slope_db_variant_pins(oracle):
+    # named variant: the same rule on y(n) = 10 log10(lambda_n).  hand count: drops 10, 10, 30, 0.458, 0.512, 0.580 dB
     lam = np.array([1e6, 1e5, 1e4, 10.0, 9.0, 8.0, 7.0])
-    assert oracle.cutoff_slope(lam, 1.1) == 3          # n = 4 is the first flat step: 3 components go
-    assert oracle.cutoff_slope(lam, 0.5) == 3          # 0.458 < 0.5 too
-    assert oracle.cutoff_slope(lam, 0.4) == 6          # never below 0.4 dB: only the last component stays
-    assert oracle.cutoff_slope(lam, 10.5) == 0         # already the first drop (10 dB) is "flat"
-    assert oracle.cutoff_slope(lam, 9.99) == 3         # the two 10 dB steps and the 30 dB step are steeper: n = 4 again
+    assert oracle.cutoff_slope_db(lam, 1.1) == 3       # n = 4 is the first flat step: 3 components go
+    assert oracle.cutoff_slope_db(lam, 0.5) == 3       # 0.458 < 0.5 too
+    assert oracle.cutoff_slope_db(lam, 0.4) == 6       # never below 0.4 dB: only the last component stays
+    assert oracle.cutoff_slope_db(lam, 10.5) == 0      # already the first drop (10 dB) is "flat"
+    assert oracle.cutoff_slope_db(lam, 9.99) == 3      # the two 10 dB steps and the 30 dB step are steeper: n = 4 again
     # exactly geometric curve, 3 dB per step: flat iff the threshold exceeds 3 dB
     lam = 10.0 ** (-0.3 * np.arange(12))
-    assert oracle.cutoff_slope(lam, 2.9) == 11
-    assert oracle.cutoff_slope(lam, 3.1) == 0
-    # brute force from the definition on random descending spectra, in plain numpy
+    assert oracle.cutoff_slope_db(lam, 2.9) == 11
+    assert oracle.cutoff_slope_db(lam, 3.1) == 0
     rng = np.random.default_rng(5)
     for n in (2, 3, 9, 40, 128):
         for _ in range(20):
@@ -229,16 +263,15 @@ def test_slope_cutoff_pins(oracle):
             T = rng.uniform(0.05, 6.0)
             drops = 10 * np.log10(lam[:-1]) - 10 * np.log10(lam[1:])
             flat = np.nonzero(drops < T)[0]
-            want = int(flat[0]) if flat.size else n - 1   # 0-based index of the first flat step = (1-based n) - 1
-            assert oracle.cutoff_slope(lam, T) == want
-    # invariant under a change of units, unlike method 1; degenerate inputs
+            want = int(flat[0]) if flat.size else n - 1
+            assert oracle.cutoff_slope_db(lam, T) == want
     lam = np.concatenate([[4e5, 2e4, 900.0], np.linspace(1.3, 0.7, 29)])
-    assert oracle.cutoff_slope(lam, 1.1) == oracle.cutoff_slope(3.7e-9 * lam, 1.1) == 3
-    assert oracle.cutoff_slope(np.array([5.0]), 1.1) == 0
-    assert oracle.cutoff_slope(np.zeros(4), 1.1) == 0
-    assert oracle.cutoff_slope(np.ones(6), 1.1) == 0   # flat spectrum: nothing stands out
+    assert oracle.cutoff_slope_db(lam, 1.1) == oracle.cutoff_slope_db(3.7e-9 * lam, 1.1) == 3
+    assert oracle.cutoff_slope_db(np.array([5.0]), 1.1) == 0
+    assert oracle.cutoff_slope_db(np.zeros(4), 1.1) == 0
+    assert oracle.cutoff_slope_db(np.ones(6), 1.1) == 0
     # eigenvalues at or below zero are floored at 1e-12 lambda_1 (-120 dB): the step onto the floor is steep
-    assert oracle.cutoff_slope(np.array([1.0, 0.5, 0.0, -1e-3]), 1.1) == 2
+    assert oracle.cutoff_slope_db(np.array([1.0, 0.5, 0.0, -1e-3]), 1.1) == 2
 
 
 def test_curvature_cutoff_pins(oracle):
@@ -467,3 +500,15 @@ def test_run_invariances_and_composition(oracle):
             pks.append(oracle.project_pd(iq, gz[kz], gx[kx], F))
     PD, _ = oracle.combine(np.stack(pks))
     assert np.allclose(PD, a["PD"], rtol=1e-12)
+    # the optional V output of run(): the eigenvectors of each window, descending order (what the GPU
+    # parity tests gate every window's clutter projector against), pinned to LAPACK on the same R
+    v = oracle.run(iq, 2, 2, 6.0, 5.0, 2.0, oracle.SOFT_ENERGY, frac=0.9, beta=0.5, want_R=True, want_V=True)
+    assert np.array_equal(v["PD"], a["PD"]) and np.array_equal(v["lam"], a["lam"])
+    for k in range(4):
+        R, V, lam = v["R"][k], v["V"][k], v["lam"][k]
+        assert np.allclose(V.conj().T @ V, np.eye(8), atol=1e-13)
+        assert np.linalg.norm(R @ V - V * lam) <= 1e-12 * np.linalg.norm(R)
+        wl, Vl = np.linalg.eigh(R)
+        c = int(v["c"][k])
+        Pl = Vl[:, ::-1][:, :c] @ Vl[:, ::-1][:, :c].conj().T
+        assert np.linalg.norm(V[:, :c] @ V[:, :c].conj().T - Pl) <= 1e-10
