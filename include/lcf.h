@@ -66,50 +66,65 @@ typedef enum {
     LCF_SOFT_ADAPTIVE = 8,  /* wt_i = win(i) / l_i^beta normalised to max 1, win = right half of a
                             Gaussian window (method 6, Eq. 10); no cut-off: c = 0;
                             the weights follow the small eigenvalues, so use precision = 1          */
-    LCF_HARD_SLOPE = 9,     /* hard, c = number of leading components before the eigenvalue curve in dB,
-                            y(n) = 10 log10(l_n), first flattens: the first n with y(n) - y(n+1) <
-                            cut_scale, minus one (method 2)   */
-    LCF_SOFT_SLOPE = 10     /* sigmoid (Eq. 9) centred on the slope-rule c                          */
+    LCF_HARD_SLOPE = 9,     /* hard, method 2 as printed: slope of the eigenvalue curve
+                            y(n) = l_n / l_1 (linear; relative to its first point so that the threshold
+                            has no units: DESIGN.md "Readings" 18); c = (first n in 1..N-1 with
+                            y(n) - y(n+1) < cut_scale) - 1: the steep leading components go            */
+    LCF_SOFT_SLOPE = 10,    /* sigmoid (Eq. 9) centred on the slope-rule c                          */
+    LCF_HARD_SLOPE_DB = 11, /* named variant of method 2: the same rule on y(n) = 10 log10(l_n), cut_scale
+                            in dB per eigenvalue index (eigenvalues floored at 1e-12 l_1)           */
+    LCF_SOFT_SLOPE_DB = 12  /* sigmoid (Eq. 9) centred on the dB-slope c                            */
 } lcf_thresh_mode;
 
 typedef struct {
-    int mode;           /* lcf_thresh_mode                                                      */
+    lcf_thresh_mode mode;
     int k_fixed;        /* 0 <= k_fixed <= N (FIXED modes)                                      */
     double energy_frac; /* in (0, 1) (ENERGY modes)                                             */
     double beta;        /* > 0 (SOFT modes: sigmoid sharpness; ADAPTIVE: the exponent of Eq. 10)  */
-    double cut_scale;   /* > 0 (MEDIAN, CURVATURE modes): the scaling factor beta of Eq. 7 / Eq. 6;
-                           (SLOPE modes): the slope threshold in dB per eigenvalue index          */
     int precision;      /* 0: fp32-grade Gram + fp32 EVD.  1: exact-product fp64 Gram + fp64 EVD
                            (single precision can hamper the EVD).  The projection
                            is fp32-grade in both.  "fp32-grade": on the tensor-core kernels
-                           (N <= 128, even Nz) each fp32 operand, scaled by a power of two taken
+                           (even Nz) each fp32 operand, scaled by a power of two taken
                            from the ensemble's largest sample, is the sum of two fp16 numbers (22
                            significant bits) and products accumulate in fp32 (DESIGN.md section
                            6); the CUDA-core kernels that cover the other shapes use fp32.      */
+    double cut_scale;   /* > 0 (MEDIAN, CURVATURE modes): the scaling factor beta of Eq. 7 / Eq. 6;
+                           (SLOPE modes): the slope threshold per eigenvalue index, as a fraction of
+                           l_1 (SLOPE) or in dB (SLOPE_DB)                                        */
 } lcf_thresh;
+
+/* the CUDA runtime's stream handle, so that this header stays plain C without cuda_runtime.h */
+#ifndef __CUDA_RUNTIME_H__
+#ifndef __DRIVER_TYPES_H__
+typedef struct CUstream_st* cudaStream_t;
+#endif
+#endif
 
 /* Builds window tables, the work decomposition and all device workspace on the current CUDA device.
  * Nz, Nx, N >= 1 (N >= 2).  *out is set to NULL on failure.  Synchronous (allocates, copies). */
 lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, const lcf_windows* win,
                            const lcf_thresh* thr);
 
-/* Enqueues the whole path on `stream` (a cudaStream_t passed as void*; NULL = default stream) and
- * returns without synchronising; no allocation, no host<->device copy.  One call in flight per plan
- * (the workspace is shared): use one plan per stream to pipeline.  iq_dev and pd_dev must not
- * alias.  Returns LCF_ERR_CUDA if a launch failed. */
-lcf_status lcf_filter(lcf_plan* plan, const void* iq_dev, float* pd_dev, void* stream);
+/* Enqueues the whole path on `stream` (NULL = default stream) and returns without synchronising; no
+ * allocation, no host<->device copy.  One call in flight per plan (the workspace is shared): use
+ * one plan per stream to pipeline.  iq_dev and pd_dev must not alias.  Returns LCF_ERR_CUDA if a
+ * launch failed.  Because it does not synchronise it cannot know whether the EVD of THIS call
+ * converged: that is reported by lcf_get_converged, by every getter, and by the host entry points. */
+lcf_status lcf_filter(lcf_plan* plan, const void* iq_dev, float* pd_dev, cudaStream_t stream);
 
 /* Same path with HOST buffers (pinned or pageable): copies iq_host -> plan-owned device staging,
  * filters, copies the image back and synchronises `stream`.  The staging buffers are allocated on
- * first use (LCF_ERR_ALLOC on failure). */
-lcf_status lcf_filter_host(lcf_plan* plan, const void* iq_host, float* pd_host, void* stream);
+ * first use (LCF_ERR_ALLOC on failure).  Returns LCF_ERR_NOT_CONVERGED (image written) if a
+ * window's EVD hit the sweep cap. */
+lcf_status lcf_filter_host(lcf_plan* plan, const void* iq_host, float* pd_host, cudaStream_t stream);
 
 /* `count` ensembles from HOST buffers, pipelined: the host->device copy of ensemble i+1 (on a
  * plan-owned copy stream, two staging buffers) overlaps the kernels of ensemble i on `stream`; each
  * image is copied back as soon as it is done.  iq_hosts / pd_hosts: HOST arrays of `count` HOST
  * pointers (pinned memory for the copies to be asynchronous).  Returns after everything has
- * completed (synchronises both streams).  Results are identical to `count` lcf_filter_host calls. */
-lcf_status lcf_filter_host_batch(lcf_plan* plan, const void* const* iq_hosts, float* const* pd_hosts, int count, void* stream);
+ * completed (synchronises both streams).  Results are identical to `count` lcf_filter_host calls.
+ * Returns LCF_ERR_NOT_CONVERGED (all images written) if any window of any ensemble hit the sweep cap. */
+lcf_status lcf_filter_host_batch(lcf_plan* plan, const void* const* iq_hosts, float* const* pd_hosts, int count, cudaStream_t stream);
 
 /* Frees everything.  lcf_plan_destroy(NULL) is a no-op returning LCF_OK. */
 lcf_status lcf_plan_destroy(lcf_plan* plan);
@@ -118,6 +133,13 @@ lcf_status lcf_plan_destroy(lcf_plan* plan);
  * device -> HOST and describes the most recent lcf_filter call.  They return
  * LCF_ERR_NOT_CONVERGED (after filling the output) if any window's EVD did not converge. ---- */
 int lcf_num_windows(const lcf_plan* plan);                         /* K = Kz*Kx (0 if plan NULL) */
+/* Synchronises the plan's last stream and reads one device counter: LCF_OK if every window's EVD
+ * of every lcf_filter call since the last lcf_get_converged (or plan creation) converged, else
+ * LCF_ERR_NOT_CONVERGED; *windows (HOST, may be NULL) = number of unconverged window EVDs. */
+lcf_status lcf_get_converged(lcf_plan* plan, int* windows);
+/* Caps the Jacobi sweeps of the following lcf_filter calls (0 = the kernels' defaults: 30 in the
+ * fp32 kernels, 40 in fp64).  For latency-bounded use and for testing the non-convergence report. */
+lcf_status lcf_set_max_sweeps(lcf_plan* plan, int max_sweeps);
 lcf_status lcf_get_eigenvalues(lcf_plan* plan, double* lam /* HOST [K][N], descending */);
 lcf_status lcf_get_cutoffs(lcf_plan* plan, int* c /* HOST [K]: rejected components per window */);
 lcf_status lcf_get_sweeps(lcf_plan* plan, int* sweeps /* HOST [K]: Jacobi sweeps used */);

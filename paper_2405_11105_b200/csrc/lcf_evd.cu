@@ -51,6 +51,7 @@ struct JacArgs {
     int* cut;               // [K]
     int* sweeps;            // [K]
     int* conv;              // [K]
+    int* nunconv;           // [1] count of window EVDs that hit the sweep cap
     float* wslot;           // [K][Ns]
     double* wslot_dd;       // [K][Ns]
     double* wt;             // [K][N]
@@ -262,6 +263,7 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
         a.cut[k] = c;
         a.sweeps[k] = sweep;
         a.conv[k] = converged;
+        if (!converged) atomicAdd(a.nunconv, 1);
     }
     __syncthreads();
     const int c = *csh;
@@ -403,16 +405,16 @@ cudaError_t configure_evd(lcf_plan* p) {
     if (thr < 32) thr = 32;
     p->jac_threads = thr;
     cudaError_t e;
-    if (p->prec == 1) e = cudaFuncSetAttribute(jacobi_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->jac_smem);
-    else e = cudaFuncSetAttribute(jacobi_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->jac_smem);
+    if (p->prec == 1) e = set_max_dyn_smem(jacobi_kernel<double>, p->smem_optin);
+    else e = set_max_dyn_smem(jacobi_kernel<float>, p->smem_optin);
     return e;
 }
 
 cudaError_t launch_jacobi(lcf_plan* p, cudaStream_t st) {
     JacArgs a;
-    a.N = p->N; a.NP = p->NP; a.M = p->Ns - 1; a.Ns = p->Ns; a.max_sweeps = p->max_sweeps;
+    a.N = p->N; a.NP = p->NP; a.M = p->Ns - 1; a.Ns = p->Ns; a.max_sweeps = (p->sweep_cap > 0 && p->sweep_cap < p->max_sweeps) ? p->sweep_cap : p->max_sweeps;   // the rotation log holds p->max_sweeps
     a.R = p->R_d; a.rotlog = p->rotlog_d;
-    a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
+    a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d; a.nunconv = p->nunconv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
     if (p->prec == 1) jacobi_kernel<double><<<p->K, p->jac_threads, p->jac_smem, st>>>(a);
@@ -423,7 +425,7 @@ cudaError_t launch_jacobi(lcf_plan* p, cudaStream_t st) {
 template <typename T>
 static cudaError_t launch_vbuild_t(lcf_plan* p, cudaStream_t st) {
     VbArgs a;
-    a.N = p->N; a.NP = p->NP; a.M = p->Ns - 1; a.Ns = p->Ns; a.max_sweeps = p->max_sweeps;
+    a.N = p->N; a.NP = p->NP; a.M = p->Ns - 1; a.Ns = p->Ns; a.max_sweeps = (p->sweep_cap > 0 && p->sweep_cap < p->max_sweeps) ? p->sweep_cap : p->max_sweeps;   // the rotation log holds p->max_sweeps
     a.rotlog = p->rotlog_d; a.sweeps = p->sweeps_d; a.wslot = p->wslot_d; a.V = p->V_d; a.B = p->B_d;
     dim3 grid((p->N + VB_WARPS * VB_ROWS - 1) / (VB_WARPS * VB_ROWS), p->K);
     size_t smem = (size_t)VB_WARPS * VB_ROWS * p->Ns * 2 * sizeof(T);

@@ -44,6 +44,7 @@ struct EcArgs {
     int* cut;                     // [K]
     int* sweeps;                  // [K]
     int* conv;                    // [K]
+    int* nunconv;                 // [1] count of window EVDs that hit the sweep cap
     float* wslot;                 // [K][Ns]
     double* wslot_dd;             // [K][Ns]
     double* wt;                   // [K][N]
@@ -376,6 +377,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         a.cut[k] = c;
         a.sweeps[k] = sweep;
         a.conv[k] = converged;
+        if (!converged) atomicAdd(a.nunconv, 1);
     }
     __syncthreads();
     {
@@ -418,7 +420,7 @@ cudaError_t configure_evd_chol(lcf_plan* p) {
     p->ec_smem = ec_smem_bytes(p->Ns, p->ec_LD);
     if (p->ec_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaSuccess;
-#define EC_SET(NC, FULL) if (e == cudaSuccess) e = cudaFuncSetAttribute(evd_chol_kernel<NC, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ec_smem)
+#define EC_SET(NC, FULL) if (e == cudaSuccess) e = set_max_dyn_smem(evd_chol_kernel<NC, FULL>, p->smem_optin)
     EC_SET(1, false); EC_SET(2, false); EC_SET(3, false); EC_SET(4, false);
     EC_SET(1, true); EC_SET(2, true); EC_SET(3, true); EC_SET(4, true);
 #undef EC_SET
@@ -428,9 +430,9 @@ cudaError_t configure_evd_chol(lcf_plan* p) {
 cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only) {
     EcArgs a;
     a.chol_only = chol_only ? 1 : 0; a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d;
-    a.N = p->N; a.NP = p->NP; a.Ns = p->Ns; a.LD = p->ec_LD; a.max_sweeps = 30;
+    a.N = p->N; a.NP = p->NP; a.Ns = p->Ns; a.LD = p->ec_LD; a.max_sweeps = p->sweep_cap > 0 ? p->sweep_cap : 30;
     a.R = reinterpret_cast<const float2*>(p->R_d); a.amax = p->gram_tc ? p->amax_d : nullptr;
-    a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
+    a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d; a.nunconv = p->nunconv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
     a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;

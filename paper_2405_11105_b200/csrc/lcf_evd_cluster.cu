@@ -35,6 +35,7 @@ struct EclArgs {
     const float* shift;                        // [K]
     const uint32_t* amax;                      // non-null: the factors carry the data scale of the tensor-core Gram
     double* lam; int* order; int* cut; int* sweeps; int* conv;
+    int* nunconv;                              // [1] count of window EVDs that hit the sweep cap
     float* wslot; double* wslot_dd; double* wt;
     float2* V; float2* B;                      // [K][N][N]
     int mode, k_fixed;
@@ -177,7 +178,7 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
         const int c = thresh_is_adaptive(a.mode) ? 0 : thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
         if (thresh_is_adaptive(a.mode)) wnorm_sh = thresh_adaptive_norm(lsort, N, a.beta);
         ish[1] = c;
-        if (rank == 0) { a.cut[k] = c; a.sweeps[k] = sweep; a.conv[k] = converged; }
+        if (rank == 0) { a.cut[k] = c; a.sweeps[k] = sweep; a.conv[k] = converged; if (!converged) atomicAdd(a.nunconv, 1); }
     }
     __syncthreads();
     {
@@ -362,9 +363,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
         }
         ecl_cluster_sync();
         const float f0 = flg[(sweep & 1) * 2], f1 = flg[(sweep & 1) * 2 + 1];
-        if (last || (f0 == 0.f && f1 == 0.f)) { converged = 1; break; }
+        // the sweep after an all-small sweep is the last one -- unless it still made a big rotation
+        // (then the quadratic phase had not been reached after all and the sweeps go on)
+        const bool small = f0 < 2.f && f1 < 2.f;
+        if ((last && small) || (f0 == 0.f && f1 == 0.f)) { converged = 1; break; }
         if (sweep == a.max_sweeps) break;
-        if (f0 < 2.f && f1 < 2.f) last = true;
+        last = small;
     }
 
     ecl_epilogue(a, k, rank, peer, 2 * p0, 2 * npl,
@@ -631,9 +635,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
         }
         ecl_cluster_sync();
         const float f0 = flg[(sweep & 1) * 2], f1 = flg[(sweep & 1) * 2 + 1];
-        if (last || (f0 == 0.f && f1 == 0.f)) { converged = 1; break; }
+        // the sweep after an all-small sweep is the last one -- unless it still made a big rotation
+        // (then the quadratic phase had not been reached after all and the sweeps go on)
+        const bool small = f0 < 2.f && f1 < 2.f;
+        if ((last && small) || (f0 == 0.f && f1 == 0.f)) { converged = 1; break; }
         if (sweep == a.max_sweeps) break;
-        if (f0 < 2.f && f1 < 2.f) last = true;
+        last = small;
     }
 
     if (j < npl) ecl_mbar_wait(full_u32 + 8u * (uint32_t)(b * ECB_PL + j), ((t - 1) >> 1) & 1u);   // the last step's blocks
@@ -653,18 +660,18 @@ cudaError_t configure_evd_cluster(lcf_plan* p) {
     p->ecl_smem = ecl_smem_bytes(p->N, p->ec_LD);
     if (p->ecl_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaSuccess;
-#define ECL_SET(NC, FULL) if (e == cudaSuccess) e = cudaFuncSetAttribute(jacobi_cluster_kernel<NC, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ecl_smem)
+#define ECL_SET(NC, FULL) if (e == cudaSuccess) e = set_max_dyn_smem(jacobi_cluster_kernel<NC, FULL>, p->smem_optin)
     ECL_SET(1, false); ECL_SET(2, false); ECL_SET(1, true); ECL_SET(2, true);
 #undef ECL_SET
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(jacobi_cluster_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ecl_smem);
+    if (e == cudaSuccess) e = set_max_dyn_smem(jacobi_cluster_block_kernel, p->smem_optin);
     return e;
 }
 
 cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st) {
     EclArgs a;
-    a.N = p->N; a.n = p->N / 2; a.h = (a.n + 1) / 2; a.LD = p->ec_LD; a.LDg = p->ec_LD; a.max_sweeps = 30;
+    a.N = p->N; a.n = p->N / 2; a.h = (a.n + 1) / 2; a.LD = p->ec_LD; a.LDg = p->ec_LD; a.max_sweeps = p->sweep_cap > 0 ? p->sweep_cap : 30;
     a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d; a.amax = p->gram_tc ? p->amax_d : nullptr;
-    a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d;
+    a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d; a.nunconv = p->nunconv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
     a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;

@@ -213,8 +213,8 @@ cudaError_t configure_gram(lcf_plan* p) {
     p->gram_tiles_per_batch = (ntiles + p->gram_batches - 1) / p->gram_batches;
     p->gram_smem = gram_smem_bytes(p->N, p->gram_Tn, dbl);
     if (p->gram_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
-    if (dbl) return cudaFuncSetAttribute(gram_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gram_smem);
-    return cudaFuncSetAttribute(gram_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gram_smem);
+    if (dbl) return set_max_dyn_smem(gram_kernel<double>, p->smem_optin);
+    return set_max_dyn_smem(gram_kernel<float>, p->smem_optin);
 }
 
 // R_k = sum of the window's per-chunk fp64 partials in a fixed order (deterministic, no atomics);

@@ -408,19 +408,20 @@ static EncodeTiledFn encode_fn() {
 }
 
 // [N][Nx][Nz] complex64 seen as float [N][Nx][2 Nz]; box = 16 pixels x 1 x N frames, 128B swizzle
-static bool encode_iq_map(lcf_plan* p, const void* iq) {
+static const CUtensorMap* encode_iq_map(lcf_plan* p, const void* iq) {
+    if (const unsigned char* m = p->gtc_tmaps.find(iq)) return reinterpret_cast<const CUtensorMap*>(m);
     EncodeTiledFn fn = encode_fn();
-    if (!fn) return false;
+    if (!fn) return nullptr;
+    unsigned char* slot = p->gtc_tmaps.slot(iq);
     cuuint64_t dims[3] = {(cuuint64_t)2 * p->Nz, (cuuint64_t)p->Nx, (cuuint64_t)p->N};
     cuuint64_t strides[2] = {(cuuint64_t)p->Nz * 8, (cuuint64_t)p->P * 8};
     cuuint32_t box[3] = {2 * GTC_PX, 1, (cuuint32_t)((p->N + 7) / 8 * 8)};   // whole 1024-byte swizzle atoms; frames >= N are zero-filled
     cuuint32_t es[3] = {1, 1, 1};
-    CUresult r = fn(reinterpret_cast<CUtensorMap*>(p->gtc_tmap), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(iq), dims,
+    CUresult r = fn(reinterpret_cast<CUtensorMap*>(slot), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(iq), dims,
                     strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return false;
-    p->gtc_tmap_iq = iq;
-    return true;
+    if (r != CUDA_SUCCESS) { p->gtc_tmaps.drop_last(iq); return nullptr; }
+    return reinterpret_cast<const CUtensorMap*>(slot);
 }
 
 bool gram_tc_eligible(const lcf_plan* p) {
@@ -474,18 +475,19 @@ cudaError_t configure_gram_tc(lcf_plan* p, std::vector<GtcSeg>& segs, std::vecto
     p->gtc_smem = 1024 + (size_t)GTC_RAW_STAGES * p->gtc_raw_stride + (size_t)GTC_OP_STAGES * GTC_OP_BYTES + sizeof(GtcBars) +
                   (size_t)(p->Nz + p->Nx) * sizeof(double);
     if (p->gtc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
-    return cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gtc_smem);
+    return set_max_dyn_smem(gram_tc_kernel, p->smem_optin);
 }
 
 cudaError_t launch_gram_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     if (p->gtc_nseg == 0) return cudaSuccess;
-    if (p->gtc_tmap_iq != (const void*)iq && !encode_iq_map(p, iq)) return cudaErrorInvalidValue;
+    const CUtensorMap* tmap = encode_iq_map(p, iq);
+    if (!tmap) return cudaErrorInvalidValue;
     GtcArgs a;
     a.N = p->N; a.Np = (p->N + 15) / 16 * 16; a.Nz = p->Nz; a.Nx = p->Nx; a.Kz = p->Kz;
     a.group = p->gtc_group;
     a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->gtc_segs_d; a.cta_first = p->gtc_cta_first_d;
     a.part = p->gtc_part_d; a.raw_stride = p->gtc_raw_stride; a.amax = p->amax_d;
-    gram_tc_kernel<<<p->gtc_grid, GTC_THREADS, p->gtc_smem, st>>>(*reinterpret_cast<const CUtensorMap*>(p->gtc_tmap), a);
+    gram_tc_kernel<<<p->gtc_grid, GTC_THREADS, p->gtc_smem, st>>>(*tmap, a);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     dim3 blk(16, 16), grid((p->N + 15) / 16, (p->N + 15) / 16, p->K);

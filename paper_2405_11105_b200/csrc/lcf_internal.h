@@ -47,6 +47,29 @@ constexpr int PROJ_STAGES = 3;
 constexpr int VB_WARPS = 8;        // warps per CTA of the weights/projector kernel
 constexpr int VB_ROWS = 2;         // rows of V per warp
 
+// CUtensorMaps of the IQ pointers a plan has seen (a streaming caller cycles through a few fixed
+// offsets into one resident sequence): encoded once per pointer, round-robin replacement.
+struct TmapCache {
+    static constexpr int CAP = 32;
+    const void* key[CAP] = {};
+    alignas(64) unsigned char map[CAP][128];
+    int n = 0, next = 0;
+    const unsigned char* find(const void* iq) const {
+        for (int i = 0; i < n; ++i)
+            if (key[i] == iq) return map[i];
+        return nullptr;
+    }
+    unsigned char* slot(const void* iq) {       // where to encode the map of a new pointer
+        const int i = n < CAP ? n++ : (next = (next + 1) % CAP);
+        key[i] = iq;
+        return map[i];
+    }
+    void drop_last(const void* iq) {            // encoding failed: forget the key
+        for (int i = 0; i < n; ++i)
+            if (key[i] == iq) key[i] = nullptr;
+    }
+};
+
 constexpr int TIMER_RING = 64;     // lcf_filter calls whose stage events are kept
 struct StageTimer {
     cudaEvent_t ev[TIMER_RING][6];
@@ -64,6 +87,7 @@ struct lcf_plan {
     int prec = 0;            // 0 fp32, 1 fp64 (Gram, Jacobi, V)
     int NP = 0, Ns = 0;      // rotation pairs per Jacobi step, slots (= 2*NP >= N)
     int max_sweeps = 0;
+    int sweep_cap = 0;       // lcf_set_max_sweeps: 0 = each EVD kernel's default
     size_t esz = 4;          // sizeof(real) of the Gram/EVD precision
 
     // host copies
@@ -91,8 +115,7 @@ struct lcf_plan {
     lcf::GtcSeg* gtc_segs_d = nullptr;
     int *gtc_cta_first_d = nullptr, *gtc_seg_first_d = nullptr;
     float* gtc_part_d = nullptr;            // [nseg][4][128][128]
-    alignas(64) unsigned char gtc_tmap[128];  // CUtensorMap of the last iq pointer
-    const void* gtc_tmap_iq = nullptr;
+    lcf::TmapCache gtc_tmaps;
     // Cholesky + one-sided Jacobi EVD (precision 0, N <= 128): lcf_evd_chol.cu
     bool evd_chol = false, evd_cluster = false;   // cluster: Cholesky kernel, then one-sided Jacobi on 2-CTA clusters
     int ec_LD = 0;
@@ -107,8 +130,7 @@ struct lcf_plan {
     int* ptc_cta_first_d = nullptr;
     float* ptc_bpack_d = nullptr;           // [K][NB][Kp/4][256][4]
     float* ptc_part_d = nullptr;            // [NB][sum_k P_k]
-    alignas(64) unsigned char ptc_tmap[128];
-    const void* ptc_tmap_iq = nullptr;
+    lcf::TmapCache ptc_tmaps;
     uint32_t* amax_d = nullptr;             // bits of max |re|, |im| over the ensemble (tensor-core paths scale by a power of two)
     // EVD
     void* rotlog_d = nullptr;  // [K][max_sweeps*(Ns-1)][3][NP] real
@@ -117,6 +139,7 @@ struct lcf_plan {
     int* cut_d = nullptr;      // [K]
     int* sweeps_d = nullptr;   // [K]
     int* conv_d = nullptr;     // [K] 1 = converged
+    int* nunconv_d = nullptr;  // [1] window EVDs that hit the sweep cap since the counter was last read
     float* wslot_d = nullptr;  // [K][Ns] weight of the eigenvector sitting in slot s
     double* wslot_dd_d = nullptr;  // [K][Ns] same, double (diagnostic filter build)
     double* wt_d = nullptr;    // [K][N] weight by rank
@@ -155,6 +178,16 @@ struct lcf_plan {
 };
 
 namespace lcf {
+// The dynamic shared-memory limit of a kernel is a per-function, process-wide attribute: every
+// kernel gets the device's opt-in maximum (minus its static shared memory) once, so plans of
+// different sizes that are alive at the same time cannot lower each other's limit.
+template <class F>
+inline cudaError_t set_max_dyn_smem(F* fn, int optin) {
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes);
+}
 // each returns the cudaError_t of configuring/launching; kernels are asynchronous on `st`
 cudaError_t launch_gram(lcf_plan* p, const float2* iq, cudaStream_t st);
 cudaError_t launch_jacobi(lcf_plan* p, cudaStream_t st);

@@ -58,7 +58,7 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->kzlo_d); cudaFree(p->kzhi_d); cudaFree(p->kxlo_d); cudaFree(p->kxhi_d);
     cudaFree(p->gitems_d); cudaFree(p->gfirst_d); cudaFree(p->gpart_d); cudaFree(p->R_d);
     cudaFree(p->rotlog_d); cudaFree(p->lam_d); cudaFree(p->order_d); cudaFree(p->cut_d);
-    cudaFree(p->sweeps_d); cudaFree(p->conv_d); cudaFree(p->wslot_d); cudaFree(p->wslot_dd_d); cudaFree(p->wt_d);
+    cudaFree(p->sweeps_d); cudaFree(p->conv_d); cudaFree(p->nunconv_d); cudaFree(p->wslot_d); cudaFree(p->wslot_dd_d); cudaFree(p->wt_d);
     cudaFree(p->V_d); cudaFree(p->B_d); cudaFree(p->pitems_d); cudaFree(p->pfirst_d);
     cudaFree(p->tiles_d); cudaFree(p->tsum_d); cudaFree(p->mean_d); cudaFree(p->alpha_d);
     cudaFree(p->F_d); cudaFree(p->iq_stage_d); cudaFree(p->pd_stage_d);
@@ -88,6 +88,15 @@ lcf_status conv_status(lcf_plan* p) {
     return LCF_OK;
 }
 
+// reads and clears the count of window EVDs that hit the sweep cap (the caller has synchronised)
+lcf_status take_unconverged(lcf_plan* p, int* count) {
+    int n = 0;
+    if (cudaMemcpy(&n, p->nunconv_d, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    if (n != 0 && cudaMemset(p->nunconv_d, 0, sizeof(int)) != cudaSuccess) return LCF_ERR_CUDA;
+    if (count) *count = n;
+    return n ? LCF_ERR_NOT_CONVERGED : LCF_OK;
+}
+
 }  // namespace
 
 extern "C" const char* lcf_status_string(lcf_status s) {
@@ -109,14 +118,15 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     if (!win || !thr) return LCF_ERR_INVALID_ARG;
     if (Nz < 1 || Nx < 1 || N < 2 || win->Kz < 1 || win->Kx < 1) return LCF_ERR_INVALID_ARG;
     if ((long long)Nz * Nx > (1LL << 30) || (long long)win->Kz * win->Kx > 65535) return LCF_ERR_INVALID_ARG;
-    if (thr->mode < 0 || thr->mode > 10 || (thr->precision != 0 && thr->precision != 1)) return LCF_ERR_INVALID_ARG;
+    if ((int)thr->mode < 0 || (int)thr->mode > 12 || (thr->precision != 0 && thr->precision != 1)) return LCF_ERR_INVALID_ARG;
     const bool fixed = thr->mode == LCF_HARD_FIXED || thr->mode == LCF_SOFT_FIXED;
     const bool soft = thresh_is_soft(thr->mode);
     if (fixed && (thr->k_fixed < 0 || thr->k_fixed > N)) return LCF_ERR_INVALID_ARG;
     const bool energy = thr->mode == LCF_HARD_ENERGY || thr->mode == LCF_SOFT_ENERGY;
     const bool median = thr->mode == LCF_HARD_MEDIAN || thr->mode == LCF_SOFT_MEDIAN ||
                         thr->mode == LCF_HARD_CURVATURE || thr->mode == LCF_SOFT_CURVATURE ||
-                        thr->mode == LCF_HARD_SLOPE || thr->mode == LCF_SOFT_SLOPE;           // modes that read cut_scale
+                        thr->mode == LCF_HARD_SLOPE || thr->mode == LCF_SOFT_SLOPE ||
+                        thr->mode == LCF_HARD_SLOPE_DB || thr->mode == LCF_SOFT_SLOPE_DB;     // modes that read cut_scale
     if (energy && !(thr->energy_frac > 0.0 && thr->energy_frac < 1.0)) return LCF_ERR_INVALID_ARG;
     if (median && !(thr->cut_scale > 0.0) ) return LCF_ERR_INVALID_ARG;
     if (soft && !(thr->beta > 0.0)) return LCF_ERR_INVALID_ARG;
@@ -267,9 +277,10 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     }
     if (p->gram_tc || p->proj_tc) ok = ok && dev_alloc(&p->amax_d, 1);
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->R_d), K * N2 * 2 * p->esz);
-    ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->rotlog_d), K * p->max_sweeps * M * 3 * p->NP * p->esz);
+    // the rotation log is replayed by vbuild_kernel, which only follows the two-sided jacobi_kernel
+    if (!p->evd_chol) ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->rotlog_d), K * p->max_sweeps * M * 3 * p->NP * p->esz);
     ok = ok && dev_alloc(&p->lam_d, K * N) && dev_alloc(&p->order_d, K * N) && dev_alloc(&p->cut_d, K) &&
-         dev_alloc(&p->sweeps_d, K) && dev_alloc(&p->conv_d, K) && dev_alloc(&p->wslot_d, K * Ns) &&
+         dev_alloc(&p->sweeps_d, K) && dev_alloc(&p->conv_d, K) && dev_alloc(&p->nunconv_d, 1) && dev_alloc(&p->wslot_d, K * Ns) &&
          dev_alloc(&p->wslot_dd_d, K * Ns) && dev_alloc(&p->wt_d, K * N);
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->V_d), K * N * Ns * 2 * p->esz);
     ok = ok && dev_alloc(&p->B_d, K * N * Ns);
@@ -284,6 +295,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     // the Gram kernel leaves the non-canonical half of each partial unwritten; clear once so no
     // uninitialised memory is ever read by tools (the loader never reads that half)
     cudaMemset(p->gpart_d, 0, (size_t)p->n_gslots * N2 * sizeof(double2));
+    cudaMemset(p->nunconv_d, 0, sizeof(int));
     if (cudaDeviceSynchronize() != cudaSuccess) {
         free_plan_device(p);
         delete p;
@@ -302,10 +314,10 @@ extern "C" lcf_status lcf_plan_destroy(lcf_plan* p) {
     return LCF_OK;
 }
 
-extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev, void* stream) {
+extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev, cudaStream_t stream) {
     if (!p || !iq_dev || !pd_dev) return LCF_ERR_INVALID_ARG;
     if (p->cuda_failed) return LCF_ERR_CUDA;
-    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    cudaStream_t st = stream;
     const float2* iq = reinterpret_cast<const float2*>(iq_dev);
     const bool tm = p->timing && p->timer.have;
     cudaError_t e = cudaSuccess;
@@ -337,7 +349,7 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     return LCF_OK;
 }
 
-extern "C" lcf_status lcf_filter_host(lcf_plan* p, const void* iq_host, float* pd_host, void* stream) {
+extern "C" lcf_status lcf_filter_host(lcf_plan* p, const void* iq_host, float* pd_host, cudaStream_t stream) {
     if (!p || !iq_host || !pd_host) return LCF_ERR_INVALID_ARG;
     if (p->cuda_failed) return LCF_ERR_CUDA;
     const size_t iq_bytes = (size_t)p->N * p->P * sizeof(float2), pd_bytes = (size_t)p->P * sizeof(float);
@@ -349,7 +361,7 @@ extern "C" lcf_status lcf_filter_host(lcf_plan* p, const void* iq_host, float* p
             return LCF_ERR_ALLOC;
         }
     }
-    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    cudaStream_t st = stream;
     if (cudaMemcpyAsync(p->iq_stage_d, iq_host, iq_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) {
         p->cuda_failed = true;
         return LCF_ERR_CUDA;
@@ -361,12 +373,12 @@ extern "C" lcf_status lcf_filter_host(lcf_plan* p, const void* iq_host, float* p
         p->cuda_failed = true;
         return LCF_ERR_CUDA;
     }
-    return LCF_OK;
+    return take_unconverged(p, nullptr);
 }
 
 extern "C" const char* lcf_last_error(const lcf_plan* p) { return p ? p->last_error : "null plan"; }
 
-extern "C" lcf_status lcf_filter_host_batch(lcf_plan* p, const void* const* iq_hosts, float* const* pd_hosts, int count, void* stream) {
+extern "C" lcf_status lcf_filter_host_batch(lcf_plan* p, const void* const* iq_hosts, float* const* pd_hosts, int count, cudaStream_t stream) {
     if (!p || !iq_hosts || !pd_hosts || count < 0) return LCF_ERR_INVALID_ARG;
     for (int i = 0; i < count; ++i)
         if (!iq_hosts[i] || !pd_hosts[i]) return LCF_ERR_INVALID_ARG;
@@ -383,7 +395,7 @@ extern "C" lcf_status lcf_filter_host_batch(lcf_plan* p, const void* const* iq_h
         if (!p->ev_done[b] && cudaEventCreateWithFlags(&p->ev_done[b], cudaEventDisableTiming) != cudaSuccess) return LCF_ERR_CUDA;
     }
     if (!p->copy_stream && cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return LCF_ERR_CUDA;
-    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream), cs = p->copy_stream;
+    cudaStream_t st = stream, cs = p->copy_stream;
     cudaError_t e = cudaSuccess;
     lcf_status ls = LCF_OK;
     for (int i = 0; i < count && e == cudaSuccess && ls == LCF_OK; ++i) {
@@ -402,10 +414,23 @@ extern "C" lcf_status lcf_filter_host_batch(lcf_plan* p, const void* const* iq_h
     cudaError_t e2 = cudaStreamSynchronize(cs), e3 = cudaStreamSynchronize(st);
     if (ls != LCF_OK) return ls;
     if (e != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) { p->cuda_failed = true; return LCF_ERR_CUDA; }
-    return LCF_OK;
+    return take_unconverged(p, nullptr);
 }
 
 extern "C" int lcf_num_windows(const lcf_plan* p) { return p ? p->K : 0; }
+
+extern "C" lcf_status lcf_set_max_sweeps(lcf_plan* p, int max_sweeps) {
+    if (!p || max_sweeps < 0) return LCF_ERR_INVALID_ARG;
+    p->sweep_cap = max_sweeps;
+    return LCF_OK;
+}
+
+extern "C" lcf_status lcf_get_converged(lcf_plan* p, int* windows) {
+    if (windows) *windows = 0;
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK) return s;
+    return take_unconverged(p, windows);
+}
 
 extern "C" lcf_status lcf_get_eigenvalues(lcf_plan* p, double* lam) {
     lcf_status s = sync_plan(p);

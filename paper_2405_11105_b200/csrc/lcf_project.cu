@@ -237,7 +237,7 @@ cudaError_t configure_project(lcf_plan* p) {
     if (p->proj_threads > 256) return cudaErrorInvalidConfiguration;
     p->proj_smem = proj_smem_bytes(p->proj_nct);
     if (p->proj_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
-    return cudaFuncSetAttribute(project_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->proj_smem);
+    return set_max_dyn_smem(project_kernel, p->smem_optin);
 }
 
 cudaError_t launch_project(lcf_plan* p, const float2* iq, cudaStream_t st) {

@@ -385,19 +385,20 @@ static PtcEncodeFn ptc_encode_fn() {
 }
 
 // [N][Nx][Nz] complex64 seen as float [N][Nx][2 Nz]; box = 16 z x 4 x x 16 frames, no swizzle
-static bool ptc_encode_map(lcf_plan* p, const void* iq) {
+static const CUtensorMap* ptc_encode_map(lcf_plan* p, const void* iq) {
+    if (const unsigned char* m = p->ptc_tmaps.find(iq)) return reinterpret_cast<const CUtensorMap*>(m);
     PtcEncodeFn fn = ptc_encode_fn();
-    if (!fn) return false;
+    if (!fn) return nullptr;
+    unsigned char* slot = p->ptc_tmaps.slot(iq);
     cuuint64_t dims[3] = {(cuuint64_t)2 * p->Nz, (cuuint64_t)p->Nx, (cuuint64_t)p->N};
     cuuint64_t strides[2] = {(cuuint64_t)p->Nz * 8, (cuuint64_t)p->P * 8};
     cuuint32_t box[3] = {2 * PTC_TZ, PTC_TX, PTC_KC};
     cuuint32_t es[3] = {1, 1, 1};
-    CUresult r = fn(reinterpret_cast<CUtensorMap*>(p->ptc_tmap), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(iq), dims,
+    CUresult r = fn(reinterpret_cast<CUtensorMap*>(slot), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(iq), dims,
                     strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return false;
-    p->ptc_tmap_iq = iq;
-    return true;
+    if (r != CUDA_SUCCESS) { p->ptc_tmaps.drop_last(iq); return nullptr; }
+    return reinterpret_cast<const CUtensorMap*>(slot);
 }
 
 bool project_tc_eligible(const lcf_plan* p) {
@@ -438,12 +439,13 @@ cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::ve
     p->ptc_smem = 1024 + PTC_B_SMEM + (size_t)PTC_RAW_STAGES * PTC_RAW_BYTES + (size_t)PTC_OP_STAGES * PTC_OP_BYTES + sizeof(PtcBars) + 16 +
                   (size_t)(p->Nz + p->Nx) * sizeof(double);
     if (p->ptc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
-    return cudaFuncSetAttribute(project_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ptc_smem);
+    return set_max_dyn_smem(project_tc_kernel, p->smem_optin);
 }
 
 cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     if (p->ptc_nseg == 0 || p->n_pitems == 0) return cudaSuccess;
-    if (p->ptc_tmap_iq != (const void*)iq && !ptc_encode_map(p, iq)) return cudaErrorInvalidValue;
+    const CUtensorMap* tmap = ptc_encode_map(p, iq);
+    if (!tmap) return cudaErrorInvalidValue;
     proj_tc_pack_kernel<<<p->K * p->ptc_NB * (p->ptc_Kp / 8), 256, 0, st>>>(p->B_d, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -451,7 +453,7 @@ cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     a.N = p->N; a.Kp = p->ptc_Kp; a.Nz = p->Nz; a.Nx = p->Nx;
     a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->ptc_segs_d; a.cta_first = p->ptc_cta_first_d;
     a.bpack = p->ptc_bpack_d; a.amax = p->amax_d; a.NB = p->ptc_NB; a.part = p->ptc_part_d; a.sumPk = p->sumPk;
-    project_tc_kernel<<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(*reinterpret_cast<const CUtensorMap*>(p->ptc_tmap), a);
+    project_tc_kernel<<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(*tmap, a);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     proj_tc_finish_kernel<<<p->n_pitems, PROJ_TPIX, 0, st>>>(p->ptc_part_d, p->sumPk, p->ptc_NB, p->box_d, p->pitems_d, p->tiles_d, p->tsum_d);

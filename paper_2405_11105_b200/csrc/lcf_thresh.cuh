@@ -7,8 +7,10 @@
 //              y(n) = cut_scale * N * log10(l_n) / log10(l_1)         method 1, Eq. 6
 //              (central differences on n = 2..N-1, eigenvalues floored at 1e-12 l_1, lowest n on ties:
 //              DESIGN.md "Readings")
-//   slope      c = min{n in 1..N-1 : y(n) - y(n+1) < cut_scale} - 1,  y(n) = 10 log10(l_n) (dB per index;
-//              eigenvalues floored at 1e-12 l_1; N - 1 if the curve never flattens)   method 2
+//   slope      c = min{n in 1..N-1 : y(n) - y(n+1) < cut_scale} - 1 on the curve as printed, y(n) = l_n,
+//              taken relative to l_1 (N - 1 if the curve never flattens)           method 2
+//   slope_db   the same rule on y(n) = 10 log10(l_n) (dB per index; eigenvalues floored at 1e-12 l_1):
+//              a named variant, not the printed form (DESIGN.md "Readings" 18)
 //   hard       wt_i = 0 for i <= c, 1 above
 //   soft       wt_i = 1 / (1 + exp(-beta (i - c)))          method 5, Eq. 9
 //   adaptive   wt_i = win(i) / l_i^beta, normalised to max 1     method 6, Eq. 10
@@ -23,7 +25,7 @@ namespace lcf {
 
 __host__ __device__ inline bool thresh_is_soft(int mode) {
     return mode == LCF_SOFT_FIXED || mode == LCF_SOFT_ENERGY || mode == LCF_SOFT_MEDIAN || mode == LCF_SOFT_CURVATURE ||
-           mode == LCF_SOFT_ADAPTIVE || mode == LCF_SOFT_SLOPE;
+           mode == LCF_SOFT_ADAPTIVE || mode == LCF_SOFT_SLOPE || mode == LCF_SOFT_SLOPE_DB;
 }
 
 __device__ inline int thresh_cutoff(int mode, int k_fixed, double energy_frac, double cut_scale, const double* lsort, int N) {
@@ -64,6 +66,12 @@ __device__ inline int thresh_cutoff(int mode, int k_fixed, double energy_frac, d
         return c;
     }
     if (mode == LCF_HARD_SLOPE || mode == LCF_SOFT_SLOPE) {
+        if (N < 2 || !(lsort[0] > 0.0)) return 0;
+        for (int n = 1; n <= N - 1; ++n)                                  // 1-based n: drop from l_n to l_{n+1}, as a fraction of l_1
+            if (lsort[n - 1] / lsort[0] - lsort[n] / lsort[0] < cut_scale) return n - 1;
+        return N - 1;
+    }
+    if (mode == LCF_HARD_SLOPE_DB || mode == LCF_SOFT_SLOPE_DB) {
         if (N < 2 || !(lsort[0] > 0.0)) return 0;
         const double fl = 1e-12 * lsort[0];
         double y0 = 10.0 * log10(lsort[0]);

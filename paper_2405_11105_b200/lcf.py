@@ -14,7 +14,7 @@ import numpy as np
 HERE = Path(__file__).resolve().parent
 LIB_PATH = HERE / "liblcf.so"
 
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE = range(11)
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE, HARD_SLOPE_DB, SOFT_SLOPE_DB = range(13)
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_NOT_CONVERGED = range(6)
 
 EXPORTS = [
@@ -22,6 +22,7 @@ EXPORTS = [
     "lcf_get_eigenvalues", "lcf_get_cutoffs", "lcf_get_sweeps", "lcf_get_gram", "lcf_get_eigenvectors",
     "lcf_get_weights", "lcf_get_filters", "lcf_get_window_means", "lcf_set_timing", "lcf_get_stage_ms",
     "lcf_get_work", "lcf_measure_peak", "lcf_status_string", "lcf_last_error", "lcf_scale_exponent",
+    "lcf_get_converged", "lcf_set_max_sweeps",
 ]
 
 
@@ -32,7 +33,7 @@ class Windows(C.Structure):
 
 class Thresh(C.Structure):
     _fields_ = [("mode", C.c_int), ("k_fixed", C.c_int), ("energy_frac", C.c_double), ("beta", C.c_double),
-                ("cut_scale", C.c_double), ("precision", C.c_int)]
+                ("precision", C.c_int), ("cut_scale", C.c_double)]
 
 
 class Work(C.Structure):
@@ -71,6 +72,8 @@ def load() -> C.CDLL:
         L.lcf_get_cutoffs.argtypes = [vp, ip]
         L.lcf_get_sweeps.argtypes = [vp, ip]
         L.lcf_set_timing.argtypes = [vp, C.c_int]
+        L.lcf_set_max_sweeps.argtypes = [vp, C.c_int]
+        L.lcf_get_converged.argtypes = [vp, ip]
         L.lcf_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.lcf_get_work.argtypes = [vp, C.POINTER(Work)]
         L.lcf_measure_peak.argtypes = [C.c_int, dp]
@@ -136,7 +139,7 @@ class Plan:
         self._h = C.c_void_p(None)
         self.Nz, self.Nx, self.N, self.K = int(Nz), int(Nx), int(N), int(Kz) * int(Kx)
         w = Windows(int(Kz), int(Kx), float(sigma_z), float(sigma_x), float(trunc))
-        t = Thresh(int(mode), int(k_fixed), float(energy_frac), float(beta), float(cut_scale), int(precision))
+        t = Thresh(int(mode), int(k_fixed), float(energy_frac), float(beta), int(precision), float(cut_scale))
         st = L.lcf_plan_create(C.byref(self._h), int(Nz), int(Nx), int(N), C.byref(w), C.byref(t))
         if st != OK:
             self._h = C.c_void_p(None)
@@ -166,14 +169,37 @@ class Plan:
         self.destroy()
 
     # ---- hot path ----
+    def _check(self, t, what, numel, dtypes, cuda):
+        """A tensor / array argument must be what the raw pointer is taken to be (an int address is trusted)."""
+        if isinstance(t, int) or t is None:
+            return
+        dt = str(t.dtype).replace("torch.", "")
+        if dt not in dtypes:
+            raise TypeError(f"{what}: dtype {dt}, expected one of {dtypes}")
+        n = int(t.numel()) if hasattr(t, "numel") else int(t.size)
+        want = numel if dt.startswith("complex") or len(dtypes) == 1 else 2 * numel   # float32 view of complex64: (re, im) pairs
+        if n != want:
+            raise ValueError(f"{what}: {n} elements, expected {want}")
+        contiguous = t.is_contiguous() if hasattr(t, "is_contiguous") else bool(t.flags["C_CONTIGUOUS"])
+        if not contiguous:
+            raise ValueError(f"{what}: not contiguous")
+        if hasattr(t, "is_cuda") and bool(t.is_cuda) != cuda:
+            raise ValueError(f"{what}: must be a {'CUDA' if cuda else 'host'} tensor")
+        if not hasattr(t, "is_cuda") and cuda:
+            raise ValueError(f"{what}: must be a CUDA tensor")
+
     def filter(self, iq_dev, pd_dev, stream=None):
         """iq_dev: complex64 device tensor [N][Nx][Nz] (or address); pd_dev: float32 [Nx][Nz]. Asynchronous."""
+        self._check(iq_dev, "iq_dev", self.N * self.Nx * self.Nz, ("complex64", "float32"), True)
+        self._check(pd_dev, "pd_dev", self.Nx * self.Nz, ("float32",), True)
         st = load().lcf_filter(self._h, _ptr(iq_dev), _ptr(pd_dev), _stream(stream))
         if st != OK:
             raise LcfError(st, "lcf_filter [" + load().lcf_last_error(self._h).decode() + "]")
 
     def filter_host(self, iq_host, pd_host, stream=None):
         """Host buffers (numpy / pinned torch tensors); copies, filters, copies back, synchronises."""
+        self._check(iq_host, "iq_host", self.N * self.Nx * self.Nz, ("complex64", "float32"), False)
+        self._check(pd_host, "pd_host", self.Nx * self.Nz, ("float32",), False)
         st = load().lcf_filter_host(self._h, _ptr(iq_host), _ptr(pd_host), _stream(stream))
         if st != OK:
             raise LcfError(st, "lcf_filter_host")
@@ -183,11 +209,27 @@ class Plan:
         n = len(iq_hosts)
         if len(pd_hosts) != n:
             raise ValueError("iq_hosts and pd_hosts differ in length")
+        for a, b in zip(iq_hosts, pd_hosts):
+            self._check(a, "iq_host", self.N * self.Nx * self.Nz, ("complex64", "float32"), False)
+            self._check(b, "pd_host", self.Nx * self.Nz, ("float32",), False)
         ia = (C.c_void_p * n)(*[_ptr(x) for x in iq_hosts])
         pa = (C.c_void_p * n)(*[_ptr(x) for x in pd_hosts])
         st = load().lcf_filter_host_batch(self._h, ia, pa, n, _stream(stream))
         if st != OK:
             raise LcfError(st, "lcf_filter_host_batch [" + load().lcf_last_error(self._h).decode() + "]")
+
+    def set_max_sweeps(self, n: int):
+        st = load().lcf_set_max_sweeps(self._h, int(n))
+        if st != OK:
+            raise LcfError(st, "lcf_set_max_sweeps")
+
+    def unconverged(self) -> int:
+        """Window EVDs that hit the sweep cap since this was last asked (synchronises)."""
+        n = C.c_int(0)
+        st = load().lcf_get_converged(self._h, C.byref(n))
+        if st not in (OK, ERR_NOT_CONVERGED):
+            raise LcfError(st, "lcf_get_converged")
+        return int(n.value)
 
     # ---- diagnostics ----
     def _get_d(self, fn, shape, allow_unconverged=False):

@@ -44,13 +44,13 @@ def _create(lcf, Nz=8, Nx=8, N=4, Kz=1, Kx=1, sz=0.0, sx=0.0, tr=0.0, mode=0, k=
     L = lcf.load()
     h = C.c_void_p(None)
     w = lcf.Windows(Kz, Kx, sz, sx, tr)
-    t = lcf.Thresh(mode, k, frac, beta, cs, prec)
+    t = lcf.Thresh(mode, k, frac, beta, prec, cs)
     st = L.lcf_plan_create(C.byref(h), Nz, Nx, N, C.byref(w), C.byref(t))
     return st, h
 
 
 @pytest.mark.parametrize("kw", [
-    dict(Nz=0), dict(Nx=-1), dict(N=1), dict(Kz=0), dict(Kx=0), dict(mode=11), dict(mode=-1), dict(mode=8, beta=0.0), dict(mode=9, cs=0.0), dict(mode=10, cs=-2.0), dict(mode=10, beta=0.0), dict(mode=4, cs=0.0), dict(mode=5, cs=-1.0), dict(mode=6, cs=0.0),
+    dict(Nz=0), dict(Nx=-1), dict(N=1), dict(Kz=0), dict(Kx=0), dict(mode=13), dict(mode=-1), dict(mode=11, cs=0.0), dict(mode=12, beta=0.0), dict(mode=8, beta=0.0), dict(mode=9, cs=0.0), dict(mode=10, cs=-2.0), dict(mode=10, beta=0.0), dict(mode=4, cs=0.0), dict(mode=5, cs=-1.0), dict(mode=6, cs=0.0),
     dict(k=-1), dict(k=5), dict(mode=1, frac=1.0), dict(mode=3, frac=0.0), dict(mode=2, beta=0.0),
     dict(prec=2), dict(sz=float("nan")), dict(tr=float("inf")),
 ])
@@ -66,6 +66,33 @@ def test_null_pointers(lcf):
     assert L.lcf_filter(None, None, None, None) == lcf.ERR_INVALID_ARG
     assert L.lcf_num_windows(None) == 0
     assert L.lcf_measure_peak(7, None) == lcf.ERR_INVALID_ARG
+    assert L.lcf_get_converged(None, None) == lcf.ERR_INVALID_ARG
+    assert L.lcf_set_max_sweeps(None, 3) == lcf.ERR_INVALID_ARG
+
+
+def test_header_is_plain_c_and_matches_the_binding(tmp_path):
+    """include/lcf.h compiles as C without the CUDA headers (cudaStream_t is forward-declared), and the
+    struct layouts the ctypes binding assumes are the compiler's."""
+    from paper_2405_11105_b200 import lcf as binding
+    src = tmp_path / "t.c"
+    src.write_text(r"""
+#include <stddef.h>
+#include <stdio.h>
+#include "lcf.h"
+int main(void) {
+    lcf_status (*f)(lcf_plan*, const void*, float*, cudaStream_t) = lcf_filter; (void)f;
+    printf("%zu %zu %zu %zu %zu %zu %zu\n", sizeof(lcf_thresh), offsetof(lcf_thresh, k_fixed), offsetof(lcf_thresh, energy_frac),
+           offsetof(lcf_thresh, beta), offsetof(lcf_thresh, precision), offsetof(lcf_thresh, cut_scale), sizeof(lcf_windows));
+    return 0;
+}
+""")
+    exe = tmp_path / "t"
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", str(ROOT / "include"), str(src), "-o", str(exe),
+                    str(binding.LIB_PATH), "-Wl,-rpath," + str(binding.LIB_PATH.parent)], check=True)
+    out = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()
+    T = binding.Thresh
+    assert [int(v) for v in out] == [C.sizeof(T), T.k_fixed.offset, T.energy_frac.offset, T.beta.offset, T.precision.offset,
+                                     T.cut_scale.offset, C.sizeof(binding.Windows)]
 
 
 def test_scale_exponent_of_the_tensor_path(lcf):
@@ -117,9 +144,29 @@ dist.init_process_group("gloo")
 r, w = dist.get_rank(), dist.get_world_size()
 n = 5
 mine = ensemble_shard(n, r, w)
-local = {e: torch.full((2, 3), float(e)) for e in mine}          # stand-in for the filtered images
-imgs = gather_images(local, n)
-assert len(imgs) == n and all(float(imgs[e][0, 0]) == e for e in range(n))
+if torch.cuda.is_available():
+    # real lcf_filter output: every rank filters its own ensembles (all on the one visible GPU) and
+    # rank 0 checks the gathered images against filtering all of them itself
+    from paper_2405_11105_b200 import lcf, synth
+    def run(es):
+        out = {}
+        with lcf.Plan(16, 12, 8, 2, 2, 5.0, 5.0, 3.0, synth.SOFT_ENERGY) as plan:
+            for e in es:
+                iq = torch.from_numpy(synth.random_cube(16, 12, 8, seed=40 + e)).cuda()
+                pd = torch.empty((12, 16), dtype=torch.float32, device="cuda")
+                plan.filter(iq, pd)
+                torch.cuda.synchronize()
+                out[e] = pd.cpu()
+        return out
+    local = run(mine)
+    imgs = gather_images(local, n)
+    if r == 0:
+        ref = run(range(n))
+        assert all(torch.equal(imgs[e], ref[e]) for e in range(n))
+else:
+    local = {e: torch.full((2, 3), float(e)) for e in mine}      # no GPU here: stand-in images, the sharding logic only
+    imgs = gather_images(local, n)
+    assert len(imgs) == n and all(float(imgs[e][0, 0]) == e for e in range(n))
 dist.barrier()
 dist.destroy_process_group()
 sys.stdout.write(f"rank {r} ok {mine}\n"); sys.stdout.flush()
@@ -127,11 +174,15 @@ sys.stdout.write(f"rank {r} ok {mine}\n"); sys.stdout.flush()
 
 
 def test_two_rank_ensemble_sharding_gloo(tmp_path):
+    run_two_rank_workers(tmp_path, 29571)
+
+
+def run_two_rank_workers(tmp_path, port):
     script = tmp_path / "worker.py"
     script.write_text(_WORKER)
     env = dict(os.environ, LCF_ROOT=str(ROOT), MASTER_ADDR="127.0.0.1")
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
-           "--master-addr", "127.0.0.1", "--master-port", "29571", str(script)]
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(script)]
     out = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=240)
     assert out.returncode == 0, out.stdout + out.stderr
     lines = {ln.strip() for ln in out.stdout.splitlines()}
