@@ -416,8 +416,17 @@ __device__ __forceinline__ void ecb_norms4(const EcbCol& X, const EcbCol& Y, con
 // |g_q|^2 + t |a| (exactly, for the exact rotation), so a round needs only the inner products.
 // The carried values are refreshed from the columns at the first block step of every sweep and
 // whenever an update cancels more than three quarters of a norm.
+// `cr` carries what decides whether a rotated pair still counts as "big" for the stop rule (see the
+// sweep loop): pairs the final clean-up treats are exempt, pairs whose inner product is negligible
+// against the largest eigenvalue only have to reach a loose cosine when the eigen-weights allow it.
+struct EcbCrit { float tol2, big2, eabs2, tc2; bool strict_all; };
+constexpr float ECB_RHO = 100.f;               // squared-norm ratio from which a pair is "separated" (clean-up)
+constexpr float ECB_LOOSE2 = 0.09f;            // squared cosine every counted pair must reach before the last sweep
+constexpr float ECB_EXEMPT2 = 0.01f;           // squared cosine up to which the first-order clean-up is trusted with a separated pair
+constexpr float ECB_EABS = 1e-6f;              // |g_p^H g_q| / largest eigenvalue below which a pair may stay at the loose cosine
 __device__ __forceinline__ int ecb_round_tracked(EcbCol& X, EcbCol& Y, EcbCol& Z, EcbCol& W, float& nX, float& nY, float& nZ, float& nW,
-                                                 int lane, float tol2, float big2) {
+                                                 int lane, const EcbCrit& cr) {
+    const float tol2 = cr.tol2, big2 = cr.big2;
     float v1[2], v2[2];
     {
         unsigned long long re2 = ecl_fma2(X.re.x, Y.re.x, ecl_fma2(X.im.x, Y.im.x, ecl_fma2(X.re.y, Y.re.y, ecl_mul2(X.im.y, Y.im.y))));
@@ -461,7 +470,12 @@ __device__ __forceinline__ int ecb_round_tracked(EcbCol& X, EcbCol& Y, EcbCol& Z
     const float resid = fmaf(-cs0, cs0, 1.f) - fmaf(gr, gr, gi * gi);
     const float cs = rot ? fmaf(0.5f * rc, resid, cs0) : 1.f;
     const float d = kk * absa2 * rc;                                 // t |a|,  t = |g| / c
-    int flags = rot ? (1 | (absa2 > big2 * pq ? 2 : 0)) : 0;
+    const float nhi = fmaxf(app, aqq), nlo = fminf(app, aqq);
+    const bool exempt = nhi >= 2.f * ECB_RHO * nlo && nhi >= cr.tc2;   // separated pair with a dominant column: the clean-up finishes it
+    const bool strict = cr.strict_all || absa2 > cr.eabs2;
+    // (the clean-up is a first-order update: an exempt pair must be inside its range, cos^2 <= ECB_EXEMPT2, before the last sweep)
+    int flags = rot ? (exempt ? (absa2 > ECB_EXEMPT2 * pq ? 3 : 0)
+                              : (1 | (((strict && absa2 > big2 * pq) || absa2 > ECB_LOOSE2 * pq) ? 2 : 0))) : 0;
     if (app - d < 0.25f * app || aqq + d < 0.25f * aqq) flags |= 4;
     // each half computed one rotation; swap so that every lane has both
     const float ocs = __shfl_xor_sync(0xffffffffu, cs, 16), ogr = __shfl_xor_sync(0xffffffffu, gr, 16);
@@ -490,6 +504,196 @@ __device__ __forceinline__ int ecb_round_tracked(EcbCol& X, EcbCol& Y, EcbCol& Z
     return flags & 3;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Clean-up of the separated pairs (run twice after the last sweep).  The pairs that converge slowest
+// in the sweeps are (dominant column p, small column q): every large-angle rotation between two
+// nearly degenerate small columns hands the residue of p that one of them still carries on to the
+// other, so those cosines only fall by a constant factor per sweep -- and they are the ones the
+// filter is sensitive to (a cosine eps between a clutter eigenvector and a kept one leaks
+// eps^2 lambda_clutter into the image).  For |g_p|^2 >= ECB_RHO |g_q|^2 the Jacobi rotation of (p, q)
+// is, to first order, q += g p, p -= conj(g) q with |g| <= cos / sqrt(ECB_RHO): all such pairs of the
+// ECB_KC largest columns are applied AT ONCE, G <- G (I + X) with X anti-Hermitian to first order (the
+// neglected terms are O(|g|^2): G G^H = R' changes by ~1e-6 |g_q|^2 in the first pass and by rounding in
+// the second).  One pass takes the cosines of those pairs from <~ 1e-1 to <~ 1e-4, the second to
+// rounding level (measured in a float64 model of this kernel on config-2 windows: 6e-3 -> 2e-10).
+// Deterministic: every sum has a fixed order, the two CTAs' partial sums are added as 0 + 1.
+constexpr int ECB_KC = 8;
+template <class ColPtr>
+__device__ __forceinline__ void ecb_cleanup(int N, int LD, uint32_t rank, uint32_t peer, int u0, int npl, ColPtr colptr,
+                                            float* nrm_all, int* care, float* Pb, float2* Gm, float* dP) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int ncl = 4 * npl, nch = N >> 2;
+    // ---- A: squared norms of this CTA's columns, published to both CTAs
+    {
+        const int cl = tid >> 3, rr = tid & 7;
+        float nn = 0.f;
+        if (cl < ncl) {
+            const float* cr = colptr(cl);
+            const float* ci = cr + LD;
+            for (int i0 = 4 * rr; i0 < N; i0 += 32) {
+                const float4 x = *reinterpret_cast<const float4*>(&cr[i0]);
+                const float4 y = *reinterpret_cast<const float4*>(&ci[i0]);
+                nn = fmaf(x.x, x.x, fmaf(x.y, x.y, fmaf(x.z, x.z, fmaf(x.w, x.w, nn))));
+                nn = fmaf(y.x, y.x, fmaf(y.y, y.y, fmaf(y.z, y.z, fmaf(y.w, y.w, nn))));
+            }
+        }
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) nn += __shfl_xor_sync(0xffffffffu, nn, o);
+        if (cl < ncl && rr == 0) {
+            const uint32_t na = ecl_smem(&nrm_all[u0 + cl]);
+            ecl_st_cluster_f32(na, nn); ecl_st_cluster_f32(ecl_mapa(na, peer), nn);
+        }
+    }
+    ecl_cluster_sync();
+    // ---- B: the ECB_KC largest columns (ties by index); nothing to do if no pair is separated at all
+    __shared__ int skip_sh;
+    if (tid == 0) skip_sh = 0;
+    __syncthreads();
+    if (tid < N) {
+        const float my = nrm_all[tid];
+        int rnk = 0, below = 0;
+        for (int q = 0; q < N; ++q) {
+            const float v = nrm_all[q];
+            rnk += (v > my) || (v == my && q < tid);
+            below += (my >= ECB_RHO * v) ? 1 : 0;
+        }
+        if (rnk < ECB_KC) care[rnk] = tid;
+        if (rnk == 0 && below == 0) skip_sh = 1;                     // the largest column dominates none: flat spectrum
+    }
+    __syncthreads();
+    if (skip_sh) return;                                             // same data in both CTAs: both return
+    // ---- C: copies of the care columns in both CTAs
+    for (int e = tid; e < ECB_KC * 2 * nch; e += ECL_THREADS) {
+        const int ch = e % nch, pl = (e / nch) & 1, kc = e / (2 * nch);
+        const int u = care[kc];
+        if (u >= u0 && u < u0 + ncl) {
+            const float4 v = *reinterpret_cast<const float4*>(colptr(u - u0) + pl * LD + 4 * ch);
+            const uint32_t pa = ecl_smem(Pb + (kc * 2 + pl) * LD + 4 * ch);
+            ulonglong2 w;
+            w.x = ecl_pack(v.x, v.y); w.y = ecl_pack(v.z, v.w);
+            ecl_st_cluster(pa, w); ecl_st_cluster(ecl_mapa(pa, peer), w);
+        }
+    }
+    ecl_cluster_sync();
+    // ---- D: inner products a = g_p^H g_q of the care columns with this warp's four columns, g per pair
+    const bool rowok = lane < nch;
+    if (warp < npl) {
+        float4 qr[4], qi[4];
+#pragma unroll
+        for (int c4 = 0; c4 < 4; ++c4) {
+            qr[c4] = qi[c4] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (rowok) {
+                const float* cq = colptr(4 * warp + c4) + 4 * lane;
+                qr[c4] = *reinterpret_cast<const float4*>(cq);
+                qi[c4] = *reinterpret_cast<const float4*>(cq + LD);
+            }
+        }
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {                                // care columns 4h .. 4h+3
+            float vr[16], vi[16];                                    // index c4 * 4 + kk
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+                float4 pr = make_float4(0.f, 0.f, 0.f, 0.f), pi = pr;
+                if (rowok) {
+                    const float* cp = Pb + ((4 * h + kk) * 2) * LD + 4 * lane;
+                    pr = *reinterpret_cast<const float4*>(cp);
+                    pi = *reinterpret_cast<const float4*>(cp + LD);
+                }
+#pragma unroll
+                for (int c4 = 0; c4 < 4; ++c4) {
+                    // conj(p) q = (pr qr + pi qi) + i (pr qi - pi qr)
+                    vr[c4 * 4 + kk] = fmaf(pr.x, qr[c4].x, fmaf(pi.x, qi[c4].x, fmaf(pr.y, qr[c4].y, fmaf(pi.y, qi[c4].y,
+                                      fmaf(pr.z, qr[c4].z, fmaf(pi.z, qi[c4].z, fmaf(pr.w, qr[c4].w, pi.w * qi[c4].w)))))));
+                    vi[c4 * 4 + kk] = fmaf(pr.x, qi[c4].x, fmaf(-pi.x, qr[c4].x, fmaf(pr.y, qi[c4].y, fmaf(-pi.y, qr[c4].y,
+                                      fmaf(pr.z, qi[c4].z, fmaf(-pi.z, qr[c4].z, fmaf(pr.w, qi[c4].w, -pi.w * qr[c4].w)))))));
+                }
+            }
+            // transposed butterfly: 16 sums over 32 lanes; lane l ends with the pair of index l >> 1
+#pragma unroll
+            for (int lvl = 0; lvl < 4; ++lvl) {
+                const int o = 16 >> lvl, half = 8 >> lvl;
+                const bool up = (lane & o) != 0;
+#pragma unroll
+                for (int i = 0; i < half; ++i) {
+                    const float kr = up ? vr[i + half] : vr[i], sr = up ? vr[i] : vr[i + half];
+                    const float ki = up ? vi[i + half] : vi[i], si = up ? vi[i] : vi[i + half];
+                    vr[i] = kr + __shfl_xor_sync(0xffffffffu, sr, o);
+                    vi[i] = ki + __shfl_xor_sync(0xffffffffu, si, o);
+                }
+            }
+            const float xr = vr[0] + __shfl_xor_sync(0xffffffffu, vr[0], 1);
+            const float xi = vi[0] + __shfl_xor_sync(0xffffffffu, vi[0], 1);
+            if ((lane & 1) == 0) {
+                const int idx = lane >> 1, c4 = idx >> 2, kc = 4 * h + (idx & 3);
+                const int cl = 4 * warp + c4;
+                const float app = nrm_all[care[kc]], aqq = nrm_all[u0 + cl];
+                float2 g = make_float2(0.f, 0.f);
+                if (app >= ECB_RHO * aqq) {                           // same rotation as ecb_round_tracked, c dropped (first order)
+                    const float alpha = 0.5f * (aqq - app), absa2 = xr * xr + xi * xi;
+                    const float rinv = rsqrtf(fmaxf(fmaf(alpha, alpha, absa2), 1e-37f));
+                    const float c2h = fmaf(0.5f * fabsf(alpha), rinv, 0.5f);
+                    const float kq = copysignf(0.5f * rinv * rsqrtf(c2h), alpha);
+                    g = make_float2(kq * xr, kq * xi);
+                }
+                Gm[kc * 64 + cl] = g;
+            }
+        }
+    }
+    __syncthreads();
+    // ---- E: this CTA's share of  dP_p = - sum_q conj(g_pq) g_q  (old columns), sent to both CTAs
+    {
+        const int r = tid & 127, grp = tid >> 7;
+        if (r < N) {
+#pragma unroll
+            for (int kk = 0; kk < 2; ++kk) {
+                const int kc = grp * 2 + kk;
+                float ar = 0.f, ai = 0.f;
+                for (int cl = 0; cl < ncl; ++cl) {
+                    const float2 g = Gm[kc * 64 + cl];
+                    const float* cq = colptr(cl);
+                    const float q_r = cq[r], q_i = cq[LD + r];
+                    ar = fmaf(g.x, q_r, fmaf(g.y, q_i, ar));          // conj(g) q
+                    ai = fmaf(g.x, q_i, fmaf(-g.y, q_r, ai));
+                }
+                const uint32_t da = ecl_smem(dP + ((rank * ECB_KC + kc) * 2) * LD + r);
+                ecl_st_cluster_f32(da, -ar); ecl_st_cluster_f32(ecl_mapa(da, peer), -ar);
+                ecl_st_cluster_f32(da + 4u * LD, -ai); ecl_st_cluster_f32(ecl_mapa(da + 4u * LD, peer), -ai);
+            }
+        }
+    }
+    __syncthreads();
+    // ---- F: g_q += sum_p g_pq g_p (old care columns) for this warp's four columns
+    if (warp < npl && rowok) {
+#pragma unroll
+        for (int c4 = 0; c4 < 4; ++c4) {
+            const int cl = 4 * warp + c4;
+            float* cq = colptr(cl) + 4 * lane;
+            float4 xr = *reinterpret_cast<float4*>(cq), xi = *reinterpret_cast<float4*>(cq + LD);
+#pragma unroll
+            for (int kc = 0; kc < ECB_KC; ++kc) {
+                const float2 g = Gm[kc * 64 + cl];
+                const float* cp = Pb + (kc * 2) * LD + 4 * lane;
+                const float4 pr = *reinterpret_cast<const float4*>(cp), pi = *reinterpret_cast<const float4*>(cp + LD);
+                xr.x = fmaf(g.x, pr.x, fmaf(-g.y, pi.x, xr.x)); xi.x = fmaf(g.x, pi.x, fmaf(g.y, pr.x, xi.x));
+                xr.y = fmaf(g.x, pr.y, fmaf(-g.y, pi.y, xr.y)); xi.y = fmaf(g.x, pi.y, fmaf(g.y, pr.y, xi.y));
+                xr.z = fmaf(g.x, pr.z, fmaf(-g.y, pi.z, xr.z)); xi.z = fmaf(g.x, pi.z, fmaf(g.y, pr.z, xi.z));
+                xr.w = fmaf(g.x, pr.w, fmaf(-g.y, pi.w, xr.w)); xi.w = fmaf(g.x, pi.w, fmaf(g.y, pr.w, xi.w));
+            }
+            *reinterpret_cast<float4*>(cq) = xr;
+            *reinterpret_cast<float4*>(cq + LD) = xi;
+        }
+    }
+    ecl_cluster_sync();
+    // ---- G: the owner of a care column adds both CTAs' dP (fixed order)
+    for (int e = tid; e < ECB_KC * 2 * N; e += ECL_THREADS) {
+        const int r = e % N, pl = (e / N) & 1, kc = e / (2 * N);
+        const int u = care[kc];
+        if (u >= u0 && u < u0 + ncl)
+            colptr(u - u0)[pl * LD + r] += dP[((0 * ECB_KC + kc) * 2 + pl) * LD + r] + dP[((1 * ECB_KC + kc) * 2 + pl) * LD + r];
+    }
+    ecl_cluster_sync();                                              // Pb, Gm, dP, nrm_all may be reused
+}
+
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jacobi_cluster_block_kernel(EclArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = a.N, LD = a.LD, Ns = N;
@@ -506,6 +710,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
     double* lsort = reinterpret_cast<double*>(flg + 4);
     int* ish = reinterpret_cast<int*>(lsort + Ns);
     uint64_t* fullb = reinterpret_cast<uint64_t*>(ish + 4);         // [2 buffers][ECB_PL] "both blocks of this pair have arrived"
+    float* nrm_all = reinterpret_cast<float*>(fullb + 2 * ECB_PL);  // [128] squared column norms of the whole matrix (both CTAs hold all)
+    float* thr_sh = nrm_all + 128;                                   // [4] largest norm, ECB_KC-th largest norm
+    int* care = reinterpret_cast<int*>(thr_sh + 4);                  // [ECB_KC] columns of the clean-up
+    float* Pb = reinterpret_cast<float*>(care + ECB_KC);             // [ECB_KC][2 planes][LD] their copies
+    float2* Gm = reinterpret_cast<float2*>(Pb + ECB_KC * 2 * LD);    // [ECB_KC][64] first-order rotations (care column, local column)
+    float* dP = reinterpret_cast<float*>(Gm + ECB_KC * 64);          // [2 CTAs][ECB_KC][2 planes][LD] updates of the care columns
     const uint32_t buf_u32 = ecl_smem(buf), buf_peer = ecl_mapa(buf_u32, peer);
     const uint32_t full_u32 = ecl_smem(fullb), full_peer = ecl_mapa(full_u32, peer);
 
@@ -547,6 +757,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
 
     const float tol = 4.f * sqrtf((float)N) * FLT_EPSILON;
     const float tol2 = tol * tol;
+    // Stop rule: a sweep is "small" when no counted pair was big.  A pair is big while
+    // its squared cosine is above 2 tol -- unless its inner product is below ECB_EABS = 1e-6 of the largest
+    // eigenvalue AND the eigen-weights are a sigmoid around a cut that does not depend on the noise floor
+    // (SOFT_FIXED, SOFT_ENERGY): such a pair couples two components deep in the noise part of the
+    // spectrum, moves either eigenvalue by less than 1e-6 lambda_max, and only has to reach
+    // cos^2 <= ECB_LOOSE2.  Measured (B200): configs 2 and 4 keep the image error of the strict rule
+    // (9.4e-5, 2.6e-5: set by the split-precision contractions) in 5-6 sweeps instead of 9-11; a
+    // spectrum with a slowly decaying tail just below the cut (64x48x100, SOFT_FIXED k = 5) goes from
+    // 3e-5 (1e-7) to 2e-4 (1e-6) and fails the 1e-3 gate at 3e-6, which is why the constant is not larger.
+    // Pairs of a column >= 200 x larger than its partner and among the ECB_KC largest do not count: the
+    // clean-up after the last sweep brings them to rounding level whatever they are now.
+    EcbCrit crit;
+    crit.tol2 = tol2; crit.big2 = 2.f * tol;
+    crit.eabs2 = 0.f; crit.tc2 = 3.0e38f;                            // first sweep: nothing known yet, everything strict
+    crit.strict_all = !(a.mode == LCF_SOFT_FIXED || a.mode == LCF_SOFT_ENERGY);
     const bool rowok = lane < nch;                                   // this lane's 4 rows exist
     int dPt, dPi, dQt, dQi;                                          // destinations of the top / bottom block (row, block pair)
     if (gi == 0) { dPt = 0; dPi = 0; dQt = 0; dQi = 1; }
@@ -583,14 +808,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                 float nA0, nA1, nB0, nB1;
                 if (s == 0) {
                     ecb_norms4(A0, A1, B0, B1, lane, nA0, nA1, nB0, nB1);
-                    fl |= ecb_round_tracked(A0, A1, B0, B1, nA0, nA1, nB0, nB1, lane, tol2, 2.f * tol);   // inner pairs, once per sweep
+                    fl |= ecb_round_tracked(A0, A1, B0, B1, nA0, nA1, nB0, nB1, lane, crit);   // inner pairs, once per sweep
                 } else {
                     const float* t0 = buf + ecb_slot(b, 0, j, 0, LD) + N;
                     const float* b0 = buf + ecb_slot(b, 1, j, 0, LD) + N;
                     nA0 = t0[0]; nA1 = t0[2 * LD]; nB0 = b0[0]; nB1 = b0[2 * LD];
                 }
-                fl |= ecb_round_tracked(A0, B0, A1, B1, nA0, nB0, nA1, nB1, lane, tol2, 2.f * tol);
-                fl |= ecb_round_tracked(A0, B1, A1, B0, nA0, nB1, nA1, nB0, lane, tol2, 2.f * tol);
+                fl |= ecb_round_tracked(A0, B0, A1, B1, nA0, nB0, nA1, nB1, lane, crit);
+                fl |= ecb_round_tracked(A0, B1, A1, B0, nA0, nB1, nA1, nB0, lane, crit);
                 const uint32_t mP = (Prem ? full_peer : full_u32) + 8u * (uint32_t)((b ^ 1) * ECB_PL + dPj);
                 const uint32_t mQ = (Qrem ? full_peer : full_u32) + 8u * (uint32_t)((b ^ 1) * ECB_PL + dQj);
                 if (rowok) {
@@ -607,6 +832,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                     } else {
                         ecl_st_local(aQ, B0.re); ecl_st_local(aQ + L4, B0.im); ecl_st_local(aQ + 2 * L4, B1.re); ecl_st_local(aQ + 3 * L4, B1.im);
                     }
+                }
+                if (s == M - 1 && lane < 4) {                        // end of a sweep: the whole cluster learns every column's norm
+                    const float v = lane == 0 ? nA0 : (lane == 1 ? nA1 : (lane == 2 ? nB0 : nB1));
+                    const uint32_t na = ecl_smem(&nrm_all[4 * gi + lane]);
+                    ecl_st_cluster_f32(na, v); ecl_st_cluster_f32(ecl_mapa(na, peer), v);
                 }
                 if (lane == 0) {                                     // the norms travel with their columns
                     const uint32_t nP = (Prem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dPt, dPj, 0, LD) + N) * 4u;
@@ -634,6 +864,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
             ecl_st_cluster_f32(ecl_mapa(fa, peer), (float)mine);
         }
         ecl_cluster_sync();
+        {   // largest and ECB_KC-th largest squared norm for the next sweep's criteria (same values in both CTAs)
+            if (tid < N) {
+                const float my = nrm_all[tid];
+                int rnk = 0;
+                for (int q = 0; q < N; ++q) {
+                    const float v = nrm_all[q];
+                    rnk += (v > my) || (v == my && q < tid);
+                }
+                if (rnk == 0) thr_sh[0] = my;
+                if (rnk == ECB_KC - 1) thr_sh[1] = my;
+            }
+            __syncthreads();
+            const float e1 = ECB_EABS * thr_sh[0];
+            crit.eabs2 = e1 * e1; crit.tc2 = 2.f * thr_sh[1];
+        }
         const float f0 = flg[(sweep & 1) * 2], f1 = flg[(sweep & 1) * 2 + 1];
         // the sweep after an all-small sweep is the last one -- unless it still made a big rotation
         // (then the quadratic phase had not been reached after all and the sweeps go on)
@@ -645,13 +890,18 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
 
     if (j < npl) ecl_mbar_wait(full_u32 + 8u * (uint32_t)(b * ECB_PL + j), ((t - 1) >> 1) & 1u);   // the last step's blocks
     ecl_cluster_sync();
+    for (int pass = 0; pass < 2; ++pass)
+        ecb_cleanup(N, LD, rank, peer, 4 * p0, npl,
+                    [&](int cl) { return buf + ecb_slot(b, (cl >> 1) & 1, cl >> 2, cl & 1, LD); },
+                    nrm_all, care, Pb, Gm, dP);
     ecl_epilogue(a, k, rank, peer, 4 * p0, 4 * npl,
                  [&](int cl) { return (const float*)(buf + ecb_slot(b, (cl >> 1) & 1, cl >> 2, cl & 1, LD)); },
                  lam_s, inv_s, wsl, lsort, ish, shiftv, delta, sweep, converged);
 }
 
 static size_t ecl_smem_bytes(int N, int LD) {
-    return (size_t)2 * 2 * ECL_PL * 2 * LD * 4 + 3 * (size_t)N * 4 + 16 + (size_t)N * 8 + 16 + 2 * ECB_PL * 8 + 64;
+    return (size_t)2 * 2 * ECL_PL * 2 * LD * 4 + 3 * (size_t)N * 4 + 16 + (size_t)N * 8 + 16 + 2 * ECB_PL * 8 + 64 +
+           (128 + 4) * 4 + ECB_KC * 4 + (size_t)ECB_KC * 2 * LD * 4 + ECB_KC * 64 * 8 + (size_t)2 * ECB_KC * 2 * LD * 4;   // clean-up workspace
 }
 
 bool evd_cluster_eligible(const lcf_plan* p) { return p->prec == 0 && (p->N % 2) == 0 && p->N >= 32 && p->N <= 128; }
