@@ -99,15 +99,31 @@ __device__ __forceinline__ void ecl_mbar_arrive(uint32_t bar) {
 __device__ __forceinline__ void ecl_mbar_arrive_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ bool ecl_mbar_try(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    return done != 0;
+}
 __device__ __forceinline__ void ecl_mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t done = 0;
+    if (ecl_mbar_try(bar, parity)) return;
+    // still waiting: poll with nothing but the try_wait in the loop (a waiting warp shares its scheduler
+    // with working ones); the clock is only read every 64 Ki polls, for the watchdog
     const long long t0 = clock64();
-    for (;;) {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-        if (done) break;
-        if (clock64() - t0 > 4000000000ll) __trap();                 // a lost signal must not hang the device
+    for (uint32_t it = 1;; ++it) {
+        if (ecl_mbar_try(bar, parity)) return;
+        if ((it & 0xffffu) == 0u && clock64() - t0 > 4000000000ll) __trap();   // a lost signal must not hang the device
     }
+}
+__device__ __forceinline__ ulonglong2 ecl_ld_local(uint32_t addr) {
+    ulonglong2 v;
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ float ecl_ld_local_f32(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+    return v;
 }
 __device__ __forceinline__ void ecl_cluster_sync() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
@@ -780,6 +796,17 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
     const bool Prem = (dPi >= h) != (rank == 1), Qrem = (dQi >= h) != (rank == 1);
     const int dPj = dPi - (dPi >= h ? h : 0), dQj = dQi - (dQi >= h ? h : 0);
     const int M = 2 * n - 1;
+    // shared-window addresses of everything a step touches, for buffer 0 (buffer 1 is BST / MST bytes on)
+    const uint32_t BST = (uint32_t)ecb_slot(1, 0, 0, 0, LD) * 4u, MST = 8u * ECB_PL, L4 = (uint32_t)LD * 4u;
+    const uint32_t srcT = buf_u32 + (uint32_t)(ecb_slot(0, 0, j, 0, LD) + 4 * lane) * 4u;
+    const uint32_t srcB = buf_u32 + (uint32_t)(ecb_slot(0, 1, j, 0, LD) + 4 * lane) * 4u;
+    const uint32_t nrmT = buf_u32 + (uint32_t)(ecb_slot(0, 0, j, 0, LD) + N) * 4u;
+    const uint32_t nrmB = buf_u32 + (uint32_t)(ecb_slot(0, 1, j, 0, LD) + N) * 4u;
+    const uint32_t dstP = (Prem ? buf_peer : buf_u32) + (uint32_t)ecb_slot(0, dPt, dPj, 0, LD) * 4u;
+    const uint32_t dstQ = (Qrem ? buf_peer : buf_u32) + (uint32_t)ecb_slot(0, dQt, dQj, 0, LD) * 4u;
+    const uint32_t fb0 = full_u32 + 8u * (uint32_t)j;
+    const uint32_t mP0 = (Prem ? full_peer : full_u32) + 8u * (uint32_t)dPj;
+    const uint32_t mQ0 = (Qrem ? full_peer : full_u32) + 8u * (uint32_t)dQj;
     int b = 0, sweep = 0, converged = 0;
     unsigned t = 0;                                                  // steps so far, over all sweeps
     bool last = false;
@@ -787,8 +814,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
         int fl = 0;
         for (int s = 0; s < M; ++s, ++t) {
             if (j < npl) {
+                const uint32_t cb_ = b ? BST : 0u, nb_ = BST - cb_;  // byte offsets of the buffer read / written in this step
+                const uint32_t cm_ = b ? MST : 0u, nm_ = MST - cm_;
                 if (t > 0) {
-                    const uint32_t fb = full_u32 + 8u * (uint32_t)(b * ECB_PL + j);
+                    const uint32_t fb = fb0 + cm_;
                     ecl_mbar_wait(fb, ((t - 1) >> 1) & 1u);
                     if (lane == 0) ecl_mbar_arrive_tx(fb, txb);      // this pair's arrival for the buffer's next use
                 }
@@ -796,12 +825,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                 const ulonglong2 z2 = make_ulonglong2(0ull, 0ull);
                 A0.re = A0.im = A1.re = A1.im = B0.re = B0.im = B1.re = B1.im = z2;
                 if (rowok) {
-                    const float* t0 = buf + ecb_slot(b, 0, j, 0, LD) + 4 * lane;
-                    const float* b0 = buf + ecb_slot(b, 1, j, 0, LD) + 4 * lane;
-                    A0.re = *reinterpret_cast<const ulonglong2*>(t0);          A0.im = *reinterpret_cast<const ulonglong2*>(t0 + LD);
-                    A1.re = *reinterpret_cast<const ulonglong2*>(t0 + 2 * LD); A1.im = *reinterpret_cast<const ulonglong2*>(t0 + 3 * LD);
-                    B0.re = *reinterpret_cast<const ulonglong2*>(b0);          B0.im = *reinterpret_cast<const ulonglong2*>(b0 + LD);
-                    B1.re = *reinterpret_cast<const ulonglong2*>(b0 + 2 * LD); B1.im = *reinterpret_cast<const ulonglong2*>(b0 + 3 * LD);
+                    const uint32_t t0 = srcT + cb_, b0 = srcB + cb_;
+                    A0.re = ecl_ld_local(t0);          A0.im = ecl_ld_local(t0 + L4);
+                    A1.re = ecl_ld_local(t0 + 2 * L4); A1.im = ecl_ld_local(t0 + 3 * L4);
+                    B0.re = ecl_ld_local(b0);          B0.im = ecl_ld_local(b0 + L4);
+                    B1.re = ecl_ld_local(b0 + 2 * L4); B1.im = ecl_ld_local(b0 + 3 * L4);
                 }
                 // squared norms of the four columns: carried with the blocks (first padding row of the
                 // real plane), refreshed from the columns at the first block step of every sweep
@@ -810,18 +838,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                     ecb_norms4(A0, A1, B0, B1, lane, nA0, nA1, nB0, nB1);
                     fl |= ecb_round_tracked(A0, A1, B0, B1, nA0, nA1, nB0, nB1, lane, crit);   // inner pairs, once per sweep
                 } else {
-                    const float* t0 = buf + ecb_slot(b, 0, j, 0, LD) + N;
-                    const float* b0 = buf + ecb_slot(b, 1, j, 0, LD) + N;
-                    nA0 = t0[0]; nA1 = t0[2 * LD]; nB0 = b0[0]; nB1 = b0[2 * LD];
+                    nA0 = ecl_ld_local_f32(nrmT + cb_); nA1 = ecl_ld_local_f32(nrmT + cb_ + 2 * L4);
+                    nB0 = ecl_ld_local_f32(nrmB + cb_); nB1 = ecl_ld_local_f32(nrmB + cb_ + 2 * L4);
                 }
                 fl |= ecb_round_tracked(A0, B0, A1, B1, nA0, nB0, nA1, nB1, lane, crit);
                 fl |= ecb_round_tracked(A0, B1, A1, B0, nA0, nB1, nA1, nB0, lane, crit);
-                const uint32_t mP = (Prem ? full_peer : full_u32) + 8u * (uint32_t)((b ^ 1) * ECB_PL + dPj);
-                const uint32_t mQ = (Qrem ? full_peer : full_u32) + 8u * (uint32_t)((b ^ 1) * ECB_PL + dQj);
+                const uint32_t mP = mP0 + nm_, mQ = mQ0 + nm_;
                 if (rowok) {
-                    const uint32_t aP = (Prem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dPt, dPj, 0, LD) + 4 * lane) * 4u;
-                    const uint32_t aQ = (Qrem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dQt, dQj, 0, LD) + 4 * lane) * 4u;
-                    const uint32_t L4 = (uint32_t)LD * 4u;
+                    const uint32_t aP = dstP + nb_ + 16u * (uint32_t)lane, aQ = dstQ + nb_ + 16u * (uint32_t)lane;
                     if (Prem) {
                         ecl_st_async(aP, A0.re, mP); ecl_st_async(aP + L4, A0.im, mP); ecl_st_async(aP + 2 * L4, A1.re, mP); ecl_st_async(aP + 3 * L4, A1.im, mP);
                     } else {
@@ -839,13 +863,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                     ecl_st_cluster_f32(na, v); ecl_st_cluster_f32(ecl_mapa(na, peer), v);
                 }
                 if (lane == 0) {                                     // the norms travel with their columns
-                    const uint32_t nP = (Prem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dPt, dPj, 0, LD) + N) * 4u;
-                    const uint32_t nQ = (Qrem ? buf_peer : buf_u32) + (uint32_t)(ecb_slot(b ^ 1, dQt, dQj, 0, LD) + N) * 4u;
-                    const uint32_t L8 = (uint32_t)LD * 8u;
-                    if (Prem) { ecl_st_async_f32(nP, nA0, mP); ecl_st_async_f32(nP + L8, nA1, mP); }
-                    else { ecl_st_local_f32(nP, nA0); ecl_st_local_f32(nP + L8, nA1); }
-                    if (Qrem) { ecl_st_async_f32(nQ, nB0, mQ); ecl_st_async_f32(nQ + L8, nB1, mQ); }
-                    else { ecl_st_local_f32(nQ, nB0); ecl_st_local_f32(nQ + L8, nB1); }
+                    const uint32_t nP = dstP + nb_ + 4u * (uint32_t)N, nQ = dstQ + nb_ + 4u * (uint32_t)N;
+                    if (Prem) { ecl_st_async_f32(nP, nA0, mP); ecl_st_async_f32(nP + 2 * L4, nA1, mP); }
+                    else { ecl_st_local_f32(nP, nA0); ecl_st_local_f32(nP + 2 * L4, nA1); }
+                    if (Qrem) { ecl_st_async_f32(nQ, nB0, mQ); ecl_st_async_f32(nQ + 2 * L4, nB1, mQ); }
+                    else { ecl_st_local_f32(nQ, nB0); ecl_st_local_f32(nQ + 2 * L4, nB1); }
                 }
                 __syncwarp();
                 if (lane == 0) {                                     // blocks stored in this CTA: arrive for the whole warp
