@@ -1,5 +1,6 @@
 // lcf_project_tc.cu -- kernel 4a, tensor-core path: fused projection + |.|^2 slow-time sum (Eq. 4,
-// PAPER.md:57-63) on tcgen05 in fp16 split precision (three fp16 products per fp32 product), for N <= 128.
+// PAPER.md:57-63) on tcgen05 in fp16 split precision (three fp16 products per fp32 product), for N <= 256
+// (above 128 frames the resident B block grows past 64 KB and the pipeline runs with 4 stages instead of 8).
 //
 //   U[p][u] = sum_t S[t][p] B_k[t][u],  B_k = V_k diag(wt)     PD_k(p) = w_k(p)^2 sum_u |U[p][u]|^2
 //
@@ -50,13 +51,12 @@ constexpr int PTC_A_BYTES = PTC_KC * PTC_ROWS * 2;         // one of A_hi / A_lo
 constexpr int PTC_OP_BYTES = 2 * PTC_A_BYTES;
 constexpr int PTC_A_LBO = PTC_ROWS * 16;                   // 2048: next 8-frame chunk of A
 constexpr int PTC_B_LBO = 256 * 16;                        // 4096: next 8-frame chunk of B
-constexpr int PTC_B_SMEM = (128 / 8) * PTC_B_LBO;          // resident B block: 64 KB
 constexpr int PTC_SBO = 128;
 constexpr float PTC_B_SCALE = 256.f;
 constexpr int PTC_CONV_WARPS = 8, PTC_EPI_WARPS = 4;
 constexpr int PTC_CONV_GROUPS = 4;                         // converter groups working on alternate stages
 // a group must see every use of the stages it touches (an mbarrier waiter may not skip a phase)
-static_assert(PTC_RAW_STAGES % PTC_CONV_GROUPS == 0 && PTC_OP_STAGES % PTC_CONV_GROUPS == 0, "stages per group");
+static_assert(PTC_RAW_STAGES % PTC_CONV_GROUPS == 0 && PTC_OP_STAGES % PTC_CONV_GROUPS == 0 && 4 % PTC_CONV_GROUPS == 0, "stages per group");
 constexpr int PTC_FIRST_CONV = 4, PTC_FIRST_EPI = PTC_FIRST_CONV + PTC_CONV_WARPS;
 constexpr int PTC_THREADS = 32 * (PTC_FIRST_EPI + PTC_EPI_WARPS);
 
@@ -72,6 +72,7 @@ struct PtcArgs {
     int NB;
     float* part;                   // [NB][sum_k P_k]
     long long sumPk;
+    int nstg;                      // raw / operand stages in use: PTC_RAW_STAGES, or 4 when the B block needs the room
 };
 
 struct PtcBars {
@@ -96,10 +97,12 @@ __device__ __forceinline__ void ptc_sts128u(uint32_t addr, uint32_t x, uint32_t 
 __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid_constant__ CUtensorMap tmap, PtcArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
-    unsigned char* bsm = sbase;                                               // resident B block (<= 64 KB)
-    unsigned char* raw = sbase + PTC_B_SMEM;                                  // [RAW_STAGES][8 KB]
-    unsigned char* ops = raw + PTC_RAW_STAGES * PTC_RAW_BYTES;                // [OP_STAGES][A_hi 4 KB | A_lo 4 KB]
-    PtcBars* bars = reinterpret_cast<PtcBars*>(ops + PTC_OP_STAGES * PTC_OP_BYTES);
+    const int NSTG = a.nstg;                                                  // stages in use (raw and operand alike): 8 or 4
+    const uint32_t SMSK = (uint32_t)NSTG - 1u, SSH = NSTG == 8 ? 3u : 2u;
+    unsigned char* bsm = sbase;                                               // resident B block: Kp / 8 chunks of 4 KB
+    unsigned char* raw = sbase + (size_t)(a.Kp / 8) * PTC_B_LBO;              // [NSTG][8 KB]
+    unsigned char* ops = raw + NSTG * PTC_RAW_BYTES;                          // [NSTG][A_hi 4 KB | A_lo 4 KB]
+    PtcBars* bars = reinterpret_cast<PtcBars*>(ops + NSTG * PTC_OP_BYTES);
     double* gzs = reinterpret_cast<double*>(bars + 1);                        // [Nz] window table rows (epilogue only)
     double* gxs = gzs + a.Nz;                                                 // [Nx]
 
@@ -141,8 +144,8 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                 const int txi = tau / ntz, tzi = tau - txi * ntz;
                 const int z = ze + tzi * PTC_TZ, x = bx.x0 + txi * PTC_TX;
                 for (int st = 0; st < nst; ++st, ++it) {
-                    const int s = it % PTC_RAW_STAGES;
-                    mbar_wait(&bars->empty[s], ((it / PTC_RAW_STAGES) & 1) ^ 1);
+                    const int s = (it & SMSK);
+                    mbar_wait(&bars->empty[s], ((it >> SSH) & 1) ^ 1);
                     if (lane == 0) {
                         mbar_arrive_expect_tx(&bars->full[s], PTC_RAW_BYTES);
                         tma_load_3d(raw + (size_t)s * PTC_RAW_BYTES, &tmap, 2 * z, x, st * PTC_KC, &bars->full[s]);
@@ -165,8 +168,8 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                 mbar_wait(&bars->accempty[buf], ((tl >> 1) & 1) ^ 1);
                 const uint32_t tD = tmem + buf * 256;
                 for (int st = 0; st < nst; ++st, ++it) {
-                    const int o = it % PTC_OP_STAGES;
-                    mbar_wait(&bars->opfull[o], (it / PTC_OP_STAGES) & 1);
+                    const int o = (it & SMSK);
+                    mbar_wait(&bars->opfull[o], (it >> SSH) & 1);
                     tc_fence_after_sync();
                     if (elect_one()) {
                         const uint64_t dAh = descA0 + (uint64_t)((o * PTC_OP_BYTES) >> 4);
@@ -206,9 +209,9 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
             const int nstages = a.segs[sg].ntile * nst;
             for (int q = 0; q < nstages; ++q, ++it) {
                 if ((int)(it % PTC_CONV_GROUPS) != grp) continue;
-                const int s = it % PTC_RAW_STAGES, o = it % PTC_OP_STAGES;
+                const int s = (it & SMSK), o = (it & SMSK);
                 const uint32_t rs = raw_u32 + (uint32_t)s * PTC_RAW_BYTES, os = ops_u32 + (uint32_t)o * PTC_OP_BYTES;
-                mbar_wait(&bars->full[s], (it / PTC_RAW_STAGES) & 1);
+                mbar_wait(&bars->full[s], (it >> SSH) & 1);
                 float v[TPW][8];
 #pragma unroll
                 for (int j = 0; j < TPW; ++j)
@@ -219,7 +222,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                 for (int j = 0; j < TPW; ++j)
 #pragma unroll
                     for (int i = 0; i < 4; ++i) f16_split2(v[j][2 * i], v[j][2 * i + 1], h[j][i], l[j][i]);
-                mbar_wait(&bars->opempty[o], ((it / PTC_OP_STAGES) & 1) ^ 1);
+                mbar_wait(&bars->opempty[o], ((it >> SSH) & 1) ^ 1);
 #pragma unroll
                 for (int j = 0; j < TPW; ++j) {
                     ptc_sts128u(os + tdst[j], h[j][0], h[j][1], h[j][2], h[j][3]);
@@ -402,7 +405,7 @@ static const CUtensorMap* ptc_encode_map(lcf_plan* p, const void* iq) {
 }
 
 bool project_tc_eligible(const lcf_plan* p) {
-    return p->N <= 128 && p->N >= PTC_KC && (p->Nz % 2) == 0 && p->Nz >= PTC_TZ && p->Nx >= PTC_TX && ptc_encode_fn() != nullptr;
+    return p->N <= 256 && p->N >= PTC_KC && (p->Nz % 2) == 0 && p->Nz >= PTC_TZ && p->Nx >= PTC_TX && ptc_encode_fn() != nullptr;
 }
 
 // jobs = (window, column block, tile) in that order; static contiguous slices, cut at (window, block)
@@ -436,7 +439,8 @@ cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::ve
     }
     cta_first[grid] = (int)segs.size();
     p->ptc_nseg = (int)segs.size();
-    p->ptc_smem = 1024 + PTC_B_SMEM + (size_t)PTC_RAW_STAGES * PTC_RAW_BYTES + (size_t)PTC_OP_STAGES * PTC_OP_BYTES + sizeof(PtcBars) + 16 +
+    p->ptc_nstg = p->ptc_Kp <= 128 ? PTC_RAW_STAGES : 4;
+    p->ptc_smem = 1024 + (size_t)(p->ptc_Kp / 8) * PTC_B_LBO + (size_t)p->ptc_nstg * (PTC_RAW_BYTES + PTC_OP_BYTES) + sizeof(PtcBars) + 16 +
                   (size_t)(p->Nz + p->Nx) * sizeof(double);
     if (p->ptc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
     return set_max_dyn_smem(project_tc_kernel, p->smem_optin);
@@ -452,7 +456,7 @@ cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     PtcArgs a;
     a.N = p->N; a.Kp = p->ptc_Kp; a.Nz = p->Nz; a.Nx = p->Nx;
     a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->ptc_segs_d; a.cta_first = p->ptc_cta_first_d;
-    a.bpack = p->ptc_bpack_d; a.amax = p->amax_d; a.NB = p->ptc_NB; a.part = p->ptc_part_d; a.sumPk = p->sumPk;
+    a.bpack = p->ptc_bpack_d; a.amax = p->amax_d; a.NB = p->ptc_NB; a.part = p->ptc_part_d; a.sumPk = p->sumPk; a.nstg = p->ptc_nstg;
     project_tc_kernel<<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(*tmap, a);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
