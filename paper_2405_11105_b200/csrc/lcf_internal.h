@@ -38,6 +38,15 @@ struct PtcSeg {
     int k, b, tile0, ntile;
 };
 
+// Block-form tensor-core Gram (128 < N <= 256, lcf_gram_tc2.cu): a block of R_k (rows m0.., nc columns from c0,
+// frames f0 .. f0 + nbox loaded) and a segment of one (window, block) job.
+struct G2Block {
+    int m0, c0, nc, f0, nbox;
+};
+struct G2Seg {
+    int k, blk, tile0, ntile, cta;
+};
+
 constexpr int GRAM_TP = 32;        // pixels per shared-memory tile of the Gram kernel
 constexpr int GRAM_FLUSH_TILES = 16; // fp32 accumulators are folded into the fp64 partial every 16 tiles (512 px)
 constexpr int GRAM_THREADS = 160;  // max thread tiles per Gram CTA (136 upper tiles at N=128)
@@ -65,6 +74,27 @@ struct TmapCache {
         return map[i];
     }
     void drop_last(const void* iq) {            // encoding failed: forget the key
+        for (int i = 0; i < n; ++i)
+            if (key[i] == iq) key[i] = nullptr;
+    }
+};
+
+struct TmapCache3 {                             // same, three maps per pointer
+    static constexpr int CAP = 16;
+    const void* key[CAP] = {};
+    alignas(64) unsigned char map[CAP][384];
+    int n = 0, next = 0;
+    const unsigned char* find(const void* iq) const {
+        for (int i = 0; i < n; ++i)
+            if (key[i] == iq) return map[i];
+        return nullptr;
+    }
+    unsigned char* slot(const void* iq) {
+        const int i = n < CAP ? n++ : (next = (next + 1) % CAP);
+        key[i] = iq;
+        return map[i];
+    }
+    void drop_last(const void* iq) {
         for (int i = 0; i < n; ++i)
             if (key[i] == iq) key[i] = nullptr;
     }
@@ -116,6 +146,16 @@ struct lcf_plan {
     int *gtc_cta_first_d = nullptr, *gtc_seg_first_d = nullptr;
     float* gtc_part_d = nullptr;            // [nseg][4][128][128]
     lcf::TmapCache gtc_tmaps;
+    // block-form tensor-core Gram (precision 0, 128 < N <= 256): lcf_gram_tc2.cu
+    bool gram_tc2 = false;
+    int g2_grid = 0, g2_nseg = 0, g2_c1 = 0;
+    uint32_t g2_raw_stride = 0, g2_mat_bytes = 0;
+    size_t g2_smem = 0;
+    lcf::G2Block g2_blk[3] = {};
+    lcf::G2Seg* g2_segs_d = nullptr;
+    int *g2_cta_first_d = nullptr, *g2_seg_first_d = nullptr;
+    float* g2_part_d = nullptr;             // [nseg][2][128][128]
+    lcf::TmapCache3 g2_tmaps;
     // Cholesky + one-sided Jacobi EVD (precision 0, N <= 128): lcf_evd_chol.cu
     bool evd_chol = false, evd_cluster = false;   // cluster: Cholesky kernel, then one-sided Jacobi on 2-CTA clusters
     int ec_LD = 0;
@@ -201,6 +241,9 @@ cudaError_t configure_project(lcf_plan* p);
 bool gram_tc_eligible(const lcf_plan* p);
 cudaError_t configure_gram_tc(lcf_plan* p, std::vector<GtcSeg>& segs, std::vector<int>& cta_first, std::vector<int>& seg_first);
 cudaError_t launch_gram_tc(lcf_plan* p, const float2* iq, cudaStream_t st);
+bool gram_tc2_eligible(const lcf_plan* p);
+cudaError_t configure_gram_tc2(lcf_plan* p, std::vector<G2Seg>& segs, std::vector<int>& cta_first, std::vector<int>& seg_first);
+cudaError_t launch_gram_tc2(lcf_plan* p, const float2* iq, cudaStream_t st);
 bool evd_chol_eligible(const lcf_plan* p);
 cudaError_t configure_evd_chol(lcf_plan* p);
 cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only);

@@ -68,6 +68,7 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->ec_gfac_d); cudaFree(p->ec_shift_d);
     cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d); cudaFree(p->amax_d);
     cudaFree(p->gtc_segs_d); cudaFree(p->gtc_cta_first_d); cudaFree(p->gtc_seg_first_d); cudaFree(p->gtc_part_d);
+    cudaFree(p->g2_segs_d); cudaFree(p->g2_cta_first_d); cudaFree(p->g2_seg_first_d); cudaFree(p->g2_part_d);
     if (p->timer.have)
         for (auto& set : p->timer.ev)
             for (auto& e : set) cudaEventDestroy(e);
@@ -205,6 +206,13 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
         p->evd_chol = false;
     }
     if (!p->evd_chol) p->gram_tc = false;   // the tensor-core Gram leaves R in its data scale, which only these EVD kernels undo
+    std::vector<G2Seg> g2_segs;
+    std::vector<int> g2_cta_first, g2_seg_first;
+    p->gram_tc2 = gram_tc2_eligible(p);     // block form above 128 frames; its reduction undoes the data scale itself
+    if (p->gram_tc2 && configure_gram_tc2(p, g2_segs, g2_cta_first, g2_seg_first) != cudaSuccess) {
+        cudaGetLastError();
+        p->gram_tc2 = false;
+    }
     p->evd_cluster = p->evd_chol && evd_cluster_eligible(p);
     if (p->evd_cluster && configure_evd_cluster(p) != cudaSuccess) {
         cudaGetLastError();
@@ -220,7 +228,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     // ---- Gram work items: each window's box split into pixel chunks (multiples of GRAM_TP) ----
     std::vector<GramItem> gitems;
     p->gfirst_h.assign(p->K + 1, 0);
-    if (!p->gram_tc) {
+    if (!p->gram_tc && !p->gram_tc2) {
         long long target = p->sumPk / ((long long)p->num_sms * 6) + 1;
         long long ch = ((target + GRAM_TP - 1) / GRAM_TP) * GRAM_TP;
         if (ch < 4 * GRAM_TP) ch = 4 * GRAM_TP;
@@ -269,13 +277,18 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
              dev_upload(&p->gtc_seg_first_d, gtc_seg_first) &&
              dev_alloc(&p->gtc_part_d, (size_t)(p->gtc_nseg ? p->gtc_nseg : 1) * 2 * 128 * 128);
     }
+    if (p->gram_tc2) {
+        ok = ok && dev_upload(&p->g2_segs_d, g2_segs) && dev_upload(&p->g2_cta_first_d, g2_cta_first) &&
+             dev_upload(&p->g2_seg_first_d, g2_seg_first) &&
+             dev_alloc(&p->g2_part_d, (size_t)(p->g2_nseg ? p->g2_nseg : 1) * 2 * 128 * 128);
+    }
     if (p->evd_cluster) ok = ok && dev_alloc(&p->ec_gfac_d, K * 2 * Ns * (size_t)p->ec_LD) && dev_alloc(&p->ec_shift_d, K);
     if (p->proj_tc) {
         ok = ok && dev_upload(&p->ptc_segs_d, ptc_segs) && dev_upload(&p->ptc_cta_first_d, ptc_cta_first) &&
              dev_alloc(&p->ptc_bpack_d, K * p->ptc_NB * (size_t)(p->ptc_Kp / 8) * 1024) &&
              dev_alloc(&p->ptc_part_d, (size_t)p->ptc_NB * (size_t)(p->sumPk ? p->sumPk : 1));
     }
-    if (p->gram_tc || p->proj_tc) ok = ok && dev_alloc(&p->amax_d, 1);
+    if (p->gram_tc || p->gram_tc2 || p->proj_tc) ok = ok && dev_alloc(&p->amax_d, 1);
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->R_d), K * N2 * 2 * p->esz);
     // the rotation log is replayed by vbuild_kernel, which only follows the two-sided jacobi_kernel
     if (!p->evd_chol) ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->rotlog_d), K * p->max_sweeps * M * 3 * p->NP * p->esz);
@@ -326,8 +339,8 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     int stage = 0;
     auto run = [&](int id, cudaError_t r) { if (e == cudaSuccess && r != cudaSuccess) { e = r; stage = id; } };
     mark(0);
-    if (e == cudaSuccess && (p->gram_tc || p->proj_tc)) run(1, launch_absmax(p, iq, st));
-    if (e == cudaSuccess) run(1, p->gram_tc ? launch_gram_tc(p, iq, st) : launch_gram(p, iq, st));
+    if (e == cudaSuccess && (p->gram_tc || p->gram_tc2 || p->proj_tc)) run(1, launch_absmax(p, iq, st));
+    if (e == cudaSuccess) run(1, p->gram_tc ? launch_gram_tc(p, iq, st) : (p->gram_tc2 ? launch_gram_tc2(p, iq, st) : launch_gram(p, iq, st)));
     mark(1);
     if (e == cudaSuccess) run(2, p->evd_chol ? launch_evd_chol(p, st, p->evd_cluster) : launch_jacobi(p, st));
     if (e == cudaSuccess && p->evd_cluster) run(2, launch_evd_cluster(p, st));
@@ -563,8 +576,8 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
     w->gram_flops = 8.0 * S * N * (N + 1.0) / 2.0;   // Hermitian half, 8 real flops per complex MAC
     w->proj_flops = 8.0 * S * N * N;                 // dense N x N projector factor
     w->hbm_bytes = 8.0 * N * (double)p->P + 4.0 * (double)p->P;
-    w->launches = ((p->gram_tc || p->proj_tc) ? 1 : 0) + 2 + (p->evd_chol ? (p->evd_cluster ? 2 : 1) : 2) + (p->proj_tc ? 3 : 1) + 2;   // absmax, gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
-    w->gram_tc = p->gram_tc ? 1 : 0; w->evd_chol = p->evd_chol ? 1 : 0; w->proj_tc = p->proj_tc ? 1 : 0;
+    w->launches = ((p->gram_tc || p->gram_tc2 || p->proj_tc) ? 1 : 0) + 2 + (p->evd_chol ? (p->evd_cluster ? 2 : 1) : 2) + (p->proj_tc ? 3 : 1) + 2;   // absmax, gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
+    w->gram_tc = (p->gram_tc || p->gram_tc2) ? 1 : 0; w->evd_chol = p->evd_chol ? 1 : 0; w->proj_tc = p->proj_tc ? 1 : 0;
     w->gram_tensor_flops = 0.0; w->proj_tensor_flops = 0.0;
     for (int k = 0; k < p->K; ++k) {
         const WinBox& b = p->box_h[k];
@@ -573,6 +586,9 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
         const double Np = (double)((p->N + 15) / 16 * 16);
         // Gram: 16-pixel tiles, per tile three 128 x 2Np x 16 MMAs and one 128 x Np x 16 (= seven 128 x Np x 16 products)
         if (p->gram_tc) w->gram_tensor_flops += ntz * b.Lx * 2.0 * 7.0 * 2.0 * 128.0 * Np * 8.0;
+        // block form: per tile and block twelve 128 x nc x 16 MMAs
+        if (p->gram_tc2)
+            for (int j = 0; j < 3; ++j) w->gram_tensor_flops += ntz * b.Lx * 12.0 * 2.0 * 128.0 * p->g2_blk[j].nc * 16.0;
         // projection: 64-pixel tiles x column blocks, per 16 frames one 128x256x16 and one 128x128x16 MMA
         if (p->proj_tc)
             w->proj_tensor_flops += ntz * (double)((b.Lx + 3) / 4) * p->ptc_NB * (p->ptc_Kp / 8) * 2.0 * 128.0 * (256.0 + 128.0) * 8.0;

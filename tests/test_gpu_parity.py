@@ -309,7 +309,7 @@ def test_deterministic_and_stream_and_host_path(lcf):
 
 def test_b200_kernels_are_selected(lcf):
     """The metric workloads must run on the tcgen05 / cluster kernels, not on the CUDA-core fallback."""
-    for ci, want in ((2, (1, 1, 1)), (4, (1, 1, 1)), (0, (0, 0, 1)), (3, (0, 0, 1))):
+    for ci, want in ((2, (1, 1, 1)), (4, (1, 1, 1)), (0, (0, 0, 1)), (3, (1, 0, 1))):
         cfg = synth.baseline_configs()[ci]
         d = cfg.data
         with lcf.Plan.from_spec(d.Nz, d.Nx, d.N, cfg.filt) as plan:
