@@ -112,6 +112,16 @@ lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, const lcf_wind
  * converged: that is reported by lcf_get_converged, by every getter, and by the host entry points. */
 lcf_status lcf_filter(lcf_plan* plan, const void* iq_dev, float* pd_dev, cudaStream_t stream);
 
+/* `count` device-resident ensembles, pipelined on two lanes: a twin of the plan (same parameters, its own
+ * workspace, created on first use -- it doubles the plan's device memory) takes every other ensemble on a
+ * second internal stream, so the kernels of consecutive ensembles overlap (what the latency-bound EVD of
+ * one leaves idle, the contractions of the next use).  iq_devs / pd_devs: HOST arrays of `count` DEVICE
+ * pointers (distinct pd buffers).  Asynchronous and stream-ordered like lcf_filter: the lanes start
+ * after the work already enqueued on `stream`, and `stream` continues after both lanes are done.
+ * Results are bit-identical to `count` lcf_filter calls.  The getters afterwards describe the last
+ * even-indexed ensemble; lcf_get_converged counts both lanes. */
+lcf_status lcf_filter_batch(lcf_plan* plan, const void* const* iq_devs, float* const* pd_devs, int count, cudaStream_t stream);
+
 /* Same path with HOST buffers (pinned or pageable): copies iq_host -> plan-owned device staging,
  * filters, copies the image back and synchronises `stream`.  The staging buffers are allocated on
  * first use (LCF_ERR_ALLOC on failure).  Returns LCF_ERR_NOT_CONVERGED (image written) if a
@@ -119,8 +129,9 @@ lcf_status lcf_filter(lcf_plan* plan, const void* iq_dev, float* pd_dev, cudaStr
 lcf_status lcf_filter_host(lcf_plan* plan, const void* iq_host, float* pd_host, cudaStream_t stream);
 
 /* `count` ensembles from HOST buffers, pipelined: the host->device copy of ensemble i+1 (on a
- * plan-owned copy stream, two staging buffers) overlaps the kernels of ensemble i on `stream`; each
- * image is copied back as soon as it is done.  iq_hosts / pd_hosts: HOST arrays of `count` HOST
+ * plan-owned copy stream, two staging buffers) overlaps the kernels of ensemble i, which run on the two
+ * lanes of lcf_filter_batch; each image is copied back as soon as it is done.  `stream` is synchronised
+ * at entry.  iq_hosts / pd_hosts: HOST arrays of `count` HOST
  * pointers (pinned memory for the copies to be asynchronous).  Returns after everything has
  * completed (synchronises both streams).  Results are identical to `count` lcf_filter_host calls.
  * Returns LCF_ERR_NOT_CONVERGED (all images written) if any window of any ensemble hit the sweep cap. */
@@ -173,7 +184,8 @@ typedef struct {
 } lcf_work;
 lcf_status lcf_get_work(const lcf_plan* plan, lcf_work* out /* HOST */);
 /* Arithmetic-pipe microbenchmark on the current device: kind 0 = FP32 FFMA, 1 = FP32 packed
- * FFMA2 (fma.rn.f32x2), 2 = FP64 DFMA.  Writes achieved TFLOP/s (2 flops per FMA lane). */
+ * FFMA2 (fma.rn.f32x2), 2 = FP64 DFMA, 3 = tcgen05.mma.kind::f16 (128 x 256 x 16, operands resident
+ * in shared memory, fp32 accumulate in tensor memory).  Writes achieved TFLOP/s (2 flops per FMA). */
 lcf_status lcf_measure_peak(int kind, double* tflops /* HOST */);
 /* Host logic of the tensor-core path's power-of-two operand scaling: the
  * exponent k with amax * 2^k in [256, 512) for a finite amax > 0 (clamped to [-100, 100]); 0 for

@@ -64,6 +64,8 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->F_d); cudaFree(p->iq_stage_d); cudaFree(p->pd_stage_d);
     cudaFree(p->iq_stage2_d); cudaFree(p->pd_stage2_d);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    for (int i = 0; i < 2; ++i) { if (p->lane_st[i]) cudaStreamDestroy(p->lane_st[i]); if (p->ev_join[i]) cudaEventDestroy(p->ev_join[i]); }
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     for (int i = 0; i < 2; ++i) { if (p->ev_copied[i]) cudaEventDestroy(p->ev_copied[i]); if (p->ev_done[i]) cudaEventDestroy(p->ev_done[i]); }
     cudaFree(p->ec_gfac_d); cudaFree(p->ec_shift_d);
     cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d); cudaFree(p->amax_d);
@@ -92,10 +94,30 @@ lcf_status conv_status(lcf_plan* p) {
 // reads and clears the count of window EVDs that hit the sweep cap (the caller has synchronised)
 lcf_status take_unconverged(lcf_plan* p, int* count) {
     int n = 0;
-    if (cudaMemcpy(&n, p->nunconv_d, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
-    if (n != 0 && cudaMemset(p->nunconv_d, 0, sizeof(int)) != cudaSuccess) return LCF_ERR_CUDA;
+    for (lcf_plan* q = p; q; q = q->twin) {
+        int m = 0;
+        if (q != p && q->ran && cudaStreamSynchronize(q->last_stream) != cudaSuccess) return LCF_ERR_CUDA;
+        if (cudaMemcpy(&m, q->nunconv_d, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+        if (m != 0 && cudaMemset(q->nunconv_d, 0, sizeof(int)) != cudaSuccess) return LCF_ERR_CUDA;
+        n += m;
+    }
     if (count) *count = n;
     return n ? LCF_ERR_NOT_CONVERGED : LCF_OK;
+}
+
+// twin plan, lane streams and events of the two-lane batch entry points (first use)
+lcf_status ensure_lanes(lcf_plan* p) {
+    if (!p->twin) {
+        lcf_status s = lcf_plan_create(&p->twin, p->Nz, p->Nx, p->N, &p->win, &p->thr);
+        if (s != LCF_OK) { p->twin = nullptr; return s; }
+    }
+    p->twin->sweep_cap = p->sweep_cap;
+    for (int i = 0; i < 2; ++i) {
+        if (!p->lane_st[i] && cudaStreamCreateWithFlags(&p->lane_st[i], cudaStreamNonBlocking) != cudaSuccess) return LCF_ERR_CUDA;
+        if (!p->ev_join[i] && cudaEventCreateWithFlags(&p->ev_join[i], cudaEventDisableTiming) != cudaSuccess) return LCF_ERR_CUDA;
+    }
+    if (!p->ev_fork && cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess) return LCF_ERR_CUDA;
+    return LCF_OK;
 }
 
 }  // namespace
@@ -320,6 +342,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
 
 extern "C" lcf_status lcf_plan_destroy(lcf_plan* p) {
     if (!p) return LCF_OK;
+    if (p->twin) { lcf_plan_destroy(p->twin); p->twin = nullptr; }
     if (p->ran) cudaStreamSynchronize(p->last_stream);
     free_plan_device(p);
     cudaGetLastError();
@@ -358,6 +381,29 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     if (tm) ++p->timer.calls;
     p->last_stream = st;
     p->ran = true;
+    if (e != cudaSuccess) { p->cuda_failed = true; return LCF_ERR_CUDA; }
+    return LCF_OK;
+}
+
+extern "C" lcf_status lcf_filter_batch(lcf_plan* p, const void* const* iq_devs, float* const* pd_devs, int count, cudaStream_t stream) {
+    if (!p || !iq_devs || !pd_devs || count < 0) return LCF_ERR_INVALID_ARG;
+    for (int i = 0; i < count; ++i)
+        if (!iq_devs[i] || !pd_devs[i]) return LCF_ERR_INVALID_ARG;
+    if (p->cuda_failed) return LCF_ERR_CUDA;
+    if (count == 0) return LCF_OK;
+    lcf_status ls = ensure_lanes(p);
+    if (ls != LCF_OK) return ls;
+    // fork: both lanes start after everything already enqueued on the caller's stream
+    cudaError_t e = cudaEventRecord(p->ev_fork, stream);
+    for (int l = 0; l < 2 && e == cudaSuccess; ++l) e = cudaStreamWaitEvent(p->lane_st[l], p->ev_fork, 0);
+    for (int i = 0; i < count && e == cudaSuccess && ls == LCF_OK; ++i)
+        ls = lcf_filter((i & 1) ? p->twin : p, iq_devs[i], pd_devs[i], p->lane_st[i & 1]);
+    // join: the caller's stream continues when both lanes are done
+    for (int l = 0; l < 2 && e == cudaSuccess; ++l) {
+        e = cudaEventRecord(p->ev_join[l], p->lane_st[l]);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, p->ev_join[l], 0);
+    }
+    if (ls != LCF_OK) return ls;
     if (e != cudaSuccess) { p->cuda_failed = true; return LCF_ERR_CUDA; }
     return LCF_OK;
 }
@@ -408,25 +454,30 @@ extern "C" lcf_status lcf_filter_host_batch(lcf_plan* p, const void* const* iq_h
         if (!p->ev_done[b] && cudaEventCreateWithFlags(&p->ev_done[b], cudaEventDisableTiming) != cudaSuccess) return LCF_ERR_CUDA;
     }
     if (!p->copy_stream && cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return LCF_ERR_CUDA;
-    cudaStream_t st = stream, cs = p->copy_stream;
-    cudaError_t e = cudaSuccess;
-    lcf_status ls = LCF_OK;
+    lcf_status ls = ensure_lanes(p);
+    if (ls != LCF_OK) return ls;
+    // ensemble i: copy on the copy stream into staging buffer i & 1, kernels of lane i & 1 (plan or twin) on
+    // that lane's stream, image copied back on the lane's stream.  Two lanes: the kernels of consecutive
+    // ensembles overlap each other as well as the copies.
+    cudaStream_t cs = p->copy_stream;
+    cudaError_t e = cudaStreamSynchronize(stream);      // everything the caller enqueued before is done
     for (int i = 0; i < count && e == cudaSuccess && ls == LCF_OK; ++i) {
         const int b = i & 1;
+        cudaStream_t st = p->lane_st[b];
         // the staging buffer is free once the kernels of ensemble i-2 have read it
         if (i >= 2) e = cudaStreamWaitEvent(cs, p->ev_done[b], 0);
         if (e == cudaSuccess) e = cudaMemcpyAsync(*iqs[b], iq_hosts[i], iq_bytes, cudaMemcpyHostToDevice, cs);
         if (e == cudaSuccess) e = cudaEventRecord(p->ev_copied[b], cs);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(st, p->ev_copied[b], 0);
         if (e != cudaSuccess) break;
-        ls = lcf_filter(p, *iqs[b], *pds[b], stream);
+        ls = lcf_filter(b ? p->twin : p, *iqs[b], *pds[b], st);
         if (ls != LCF_OK) break;
         e = cudaEventRecord(p->ev_done[b], st);          // input consumed (and image ready)
         if (e == cudaSuccess) e = cudaMemcpyAsync(pd_hosts[i], *pds[b], pd_bytes, cudaMemcpyDeviceToHost, st);
     }
-    cudaError_t e2 = cudaStreamSynchronize(cs), e3 = cudaStreamSynchronize(st);
+    cudaError_t e2 = cudaStreamSynchronize(cs), e3 = cudaStreamSynchronize(p->lane_st[0]), e4 = cudaStreamSynchronize(p->lane_st[1]);
     if (ls != LCF_OK) return ls;
-    if (e != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) { p->cuda_failed = true; return LCF_ERR_CUDA; }
+    if (e != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) { p->cuda_failed = true; return LCF_ERR_CUDA; }
     return take_unconverged(p, nullptr);
 }
 

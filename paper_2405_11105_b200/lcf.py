@@ -18,7 +18,7 @@ HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_NOT_CONVERGED = range(6)
 
 EXPORTS = [
-    "lcf_plan_create", "lcf_filter", "lcf_filter_host", "lcf_filter_host_batch", "lcf_plan_destroy", "lcf_num_windows",
+    "lcf_plan_create", "lcf_filter", "lcf_filter_batch", "lcf_filter_host", "lcf_filter_host_batch", "lcf_plan_destroy", "lcf_num_windows",
     "lcf_get_eigenvalues", "lcf_get_cutoffs", "lcf_get_sweeps", "lcf_get_gram", "lcf_get_eigenvectors",
     "lcf_get_weights", "lcf_get_filters", "lcf_get_window_means", "lcf_set_timing", "lcf_get_stage_ms",
     "lcf_get_work", "lcf_measure_peak", "lcf_status_string", "lcf_last_error", "lcf_scale_exponent",
@@ -64,6 +64,7 @@ def load() -> C.CDLL:
         L.lcf_filter.argtypes = [vp, vp, vp, vp]
         L.lcf_filter_host.argtypes = [vp, vp, vp, vp]
         L.lcf_filter_host_batch.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp]
+        L.lcf_filter_batch.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp]
         L.lcf_plan_destroy.argtypes = [vp]
         L.lcf_num_windows.argtypes = [vp]
         for name in ("lcf_get_eigenvalues", "lcf_get_gram", "lcf_get_eigenvectors", "lcf_get_weights",
@@ -100,7 +101,7 @@ def scale_exponent(amax: float) -> int:
 
 
 def measure_peak(kind: int) -> float:
-    """TFLOP/s of the FP32 FFMA (0), packed FFMA2 (1) or FP64 DFMA (2) pipe on the current device."""
+    """TFLOP/s of the FP32 FFMA (0), packed FFMA2 (1), FP64 DFMA (2) pipe or the tcgen05 fp16 tensor path (3) on the current device."""
     v = C.c_double(0.0)
     st = load().lcf_measure_peak(int(kind), C.byref(v))
     if st != OK:
@@ -195,6 +196,20 @@ class Plan:
         st = load().lcf_filter(self._h, _ptr(iq_dev), _ptr(pd_dev), _stream(stream))
         if st != OK:
             raise LcfError(st, "lcf_filter [" + load().lcf_last_error(self._h).decode() + "]")
+
+    def filter_batch(self, iq_devs, pd_devs, stream=None):
+        """Lists of device tensors: consecutive ensembles overlap on the plan's two lanes. Asynchronous."""
+        n = len(iq_devs)
+        if len(pd_devs) != n:
+            raise ValueError("iq_devs and pd_devs differ in length")
+        for a, b in zip(iq_devs, pd_devs):
+            self._check(a, "iq_dev", self.N * self.Nx * self.Nz, ("complex64", "float32"), True)
+            self._check(b, "pd_dev", self.Nx * self.Nz, ("float32",), True)
+        ia = (C.c_void_p * n)(*[_ptr(x) for x in iq_devs])
+        pa = (C.c_void_p * n)(*[_ptr(x) for x in pd_devs])
+        st = load().lcf_filter_batch(self._h, ia, pa, n, _stream(stream))
+        if st != OK:
+            raise LcfError(st, "lcf_filter_batch [" + load().lcf_last_error(self._h).decode() + "]")
 
     def filter_host(self, iq_host, pd_host, stream=None):
         """Host buffers (numpy / pinned torch tensors); copies, filters, copies back, synchronises."""

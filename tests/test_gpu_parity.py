@@ -365,6 +365,38 @@ def test_two_plans_on_two_streams_interleaved(lcf):
         assert torch.equal(a_, b_)
 
 
+def test_filter_batch_two_lanes_matches_single_calls(lcf):
+    """lcf_filter_batch (twin plan, two internal streams, fork / join on the caller's stream) gives bit for bit
+    the images of single lcf_filter calls, is ordered after earlier work on the stream and before later work."""
+    import torch
+    cfg = synth.baseline_configs()[0]
+    d = cfg.data
+    filt = replace(cfg.filt, precision=0, mode=synth.SOFT_ENERGY)
+    st = torch.cuda.Stream()
+    with lcf.Plan.from_spec(d.Nz, d.Nx, d.N, filt) as plan:
+        iqs = [torch.from_numpy(synth.random_cube(d.Nz, d.Nx, d.N, seed=80 + i)).cuda() for i in range(5)]
+        single = []
+        for iq in iqs:
+            pd = torch.empty((d.Nx, d.Nz), dtype=torch.float32, device="cuda")
+            plan.filter(iq, pd)
+            torch.cuda.synchronize()
+            single.append(pd)
+        outs = [torch.full((d.Nx, d.Nz), float("nan"), dtype=torch.float32, device="cuda") for _ in iqs]
+        late = torch.zeros(5, device="cuda")
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            src = iqs[0].clone()                              # earlier work on the stream: the batch must see its result
+            plan.filter_batch([src] + iqs[1:], outs, st)
+            for i, o in enumerate(outs):                      # later work on the stream: must see the images
+                late[i] = o.sum()
+        st.synchronize()
+        for a_, b_ in zip(single, outs):
+            assert torch.equal(a_, b_)
+        assert torch.equal(late.cpu(), torch.stack([o.sum() for o in single]).cpu())
+        assert plan.unconverged() == 0
+        plan.filter_batch([], [])
+
+
 def test_plans_of_different_sizes_alive_together(lcf, oracle):
     """The opt-in shared-memory limit is a per-kernel, process-wide attribute: creating (and destroying) a
     smaller plan must not break a larger plan that already exists (every kernel family: tensor / cluster
