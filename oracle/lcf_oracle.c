@@ -17,6 +17,8 @@
  *   weights_adaptive Eq. 10, PAPER.md:120-126 (method 6: Gaussian window over inverse eigenvalue power)
  *   cutoff_slope   PAPER.md:85-89          (method 2: slope of the eigenvalue curve y(n) = lambda_n against a threshold)
  *   cutoff_slope_db  same passage           (named variant: the same rule on the curve in dB)
+ *   left_singular  PAPER.md:107            (U from C V = U D, lambda_i = sigma_i^2: spatial singular vectors)
+ *   cutoff_ncc     Eq. 8, PAPER.md:98-109   (method 4: cut-off that minimises the spatial NCC of tissue and blood images)
  *   filter         Eq. 4,  PAPER.md:57-59   (F = V Lambda^ V^H)
  *   project_pd     Eq. 4 + PAPER.md:63      (C^ = C_w F; PD = sum over slow time of |C^|^2)
  *   combine        Eq. 13, PAPER.md:154-156 (PD_final = sum_k alpha_k PD_k, alpha_k = 1/mean(PD_k))
@@ -48,7 +50,8 @@
 
 enum { LCFO_HARD_FIXED = 0, LCFO_HARD_ENERGY = 1, LCFO_SOFT_FIXED = 2, LCFO_SOFT_ENERGY = 3,
        LCFO_HARD_MEDIAN = 4, LCFO_SOFT_MEDIAN = 5, LCFO_HARD_CURVATURE = 6, LCFO_SOFT_CURVATURE = 7,
-       LCFO_SOFT_ADAPTIVE = 8, LCFO_HARD_SLOPE = 9, LCFO_SOFT_SLOPE = 10, LCFO_HARD_SLOPE_DB = 11, LCFO_SOFT_SLOPE_DB = 12 };
+       LCFO_SOFT_ADAPTIVE = 8, LCFO_HARD_SLOPE = 9, LCFO_SOFT_SLOPE = 10, LCFO_HARD_SLOPE_DB = 11, LCFO_SOFT_SLOPE_DB = 12,
+       LCFO_HARD_NCC = 13, LCFO_SOFT_NCC = 14 };
 
 int lcf_oracle_num_threads(void) {
 #ifdef _OPENMP
@@ -372,6 +375,68 @@ void lcf_oracle_project_pd(const float *iq, int N, int Nx, int Nz, const double 
     free(si);
 }
 
+/* "U can be calculated from the eigenvectors according to CV = UD and lambda_i = sigma_i^2":
+ * u_i = C_w v_i / sigma_i on the windowed data C_w = W C (Eq. 11), sigma_i = sqrt(lambda_i); only the
+ * magnitudes |u_i(p)| are used by method 4 and only they are returned:  Umag [P][N] (pixel p = z + Nz x,
+ * component i in the order of lam / V).  A component with lambda_i <= 1e-12 lambda_1 (sigma = 0 up to
+ * round-off: u undefined) gets |u_i| = 0. */
+void lcf_oracle_left_singular_mag(const float *iq, int N, int Nx, int Nz, const double *gz, const double *gx,
+                                  const double *lam, const double *V, double *Umag /* [P][N] */) {
+    size_t P = (size_t)Nx * Nz;
+    double *sr = (double *)malloc(sizeof(double) * N), *si = (double *)malloc(sizeof(double) * N);
+    for (int x = 0; x < Nx; ++x)
+        for (int z = 0; z < Nz; ++z) {
+            size_t p = (size_t)x * Nz + z;
+            double w = gz[z] * gx[x];
+            for (int t = 0; t < N; ++t) {
+                sr[t] = w * (double)iq[2 * ((size_t)t * P + p)];
+                si[t] = w * (double)iq[2 * ((size_t)t * P + p) + 1];
+            }
+            for (int i = 0; i < N; ++i) {
+                double ur = 0.0, ui = 0.0;                 /* (C_w V)[p][i] = sum_t s_t V[t][i] */
+                for (int t = 0; t < N; ++t) {
+                    double vr = RE(V, t, i, N), vi = IM(V, t, i, N);
+                    ur += sr[t] * vr - si[t] * vi;
+                    ui += sr[t] * vi + si[t] * vr;
+                }
+                double sig = (lam[i] > 1e-12 * lam[0] && lam[i] > 0.0) ? sqrt(lam[i]) : 0.0;
+                Umag[p * N + i] = sig > 0.0 ? hypot(ur, ui) / sig : 0.0;
+            }
+        }
+    free(sr);
+    free(si);
+}
+
+/* Method 4, Eq. 8: k = argmin_k NCC(k),
+ *   NCC(k) = sum_p I_T I_B / (sqrt(sum_p I_T^2) sqrt(sum_p I_B^2)),
+ * with the simplified images of PAPER.md:107 ("a given number fn of left singular vectors next to the
+ * cutoff k ... fn = 5, and w_i = 1"; the printed index ranges are garbled -- DESIGN.md "Readings" 19):
+ *   I_T(k) = sum_{i=k-fn+1}^{k} |u_i|      I_B(k) = sum_{i=k+1}^{k+fn} |u_i|       (1-based i, clipped to 1..N).
+ * k runs over 1..N-1 (at k = N there is no blood image); the lowest k wins a tie; a k whose I_T or I_B
+ * vanishes everywhere gets NCC = +inf (never chosen unless all do, then k = 1).  ncc [N] receives the
+ * curve (ncc[k-1] = NCC(k), ncc[N-1] = +inf) if not NULL.  Umag [P][N]. */
+int lcf_oracle_cutoff_ncc(const double *Umag, size_t P, int N, int fn, double *ncc) {
+    int best_k = 1;
+    double best = HUGE_VAL;
+    for (int k = 1; k <= N; ++k) {
+        double v = HUGE_VAL;
+        if (k <= N - 1) {
+            int t0 = k - fn + 1 < 1 ? 1 : k - fn + 1, b1 = k + fn > N ? N : k + fn;
+            double stb = 0.0, stt = 0.0, sbb = 0.0;
+            for (size_t p = 0; p < P; ++p) {
+                double it = 0.0, ib = 0.0;
+                for (int i = t0; i <= k; ++i) it += Umag[p * N + (i - 1)];
+                for (int i = k + 1; i <= b1; ++i) ib += Umag[p * N + (i - 1)];
+                stb += it * ib; stt += it * it; sbb += ib * ib;
+            }
+            if (stt > 0.0 && sbb > 0.0) v = stb / (sqrt(stt) * sqrt(sbb));
+        }
+        if (ncc) ncc[k - 1] = v;
+        if (v < best) { best = v; best_k = k; }
+    }
+    return best_k;
+}
+
 /* One window k = (kz, kx) end to end.  Any output pointer may be NULL except lam.
  * Returns Jacobi sweeps (or -1).  c_out = number of rejected components. */
 int lcf_oracle_window(const float *iq, int N, int Nx, int Nz, const double *gz, const double *gx,
@@ -392,8 +457,14 @@ int lcf_oracle_window(const float *iq, int N, int Nx, int Nz, const double *gz, 
     if (mode == LCFO_HARD_CURVATURE || mode == LCFO_SOFT_CURVATURE) c = lcf_oracle_cutoff_curvature(lam, N, cut_scale);
     if (mode == LCFO_HARD_SLOPE || mode == LCFO_SOFT_SLOPE) c = lcf_oracle_cutoff_slope(lam, N, cut_scale);
     if (mode == LCFO_HARD_SLOPE_DB || mode == LCFO_SOFT_SLOPE_DB) c = lcf_oracle_cutoff_slope_db(lam, N, cut_scale);
+    if (mode == LCFO_HARD_NCC || mode == LCFO_SOFT_NCC) {            /* method 4; method 5 on top of it as the paper pairs them */
+        double *Um = (double *)malloc(sizeof(double) * P * (size_t)N);
+        lcf_oracle_left_singular_mag(iq, N, Nx, Nz, gz, gx, lam, V, Um);
+        c = lcf_oracle_cutoff_ncc(Um, P, N, 5, NULL);
+        free(Um);
+    }
     int soft = (mode == LCFO_SOFT_FIXED || mode == LCFO_SOFT_ENERGY || mode == LCFO_SOFT_MEDIAN || mode == LCFO_SOFT_CURVATURE ||
-                mode == LCFO_SOFT_SLOPE || mode == LCFO_SOFT_SLOPE_DB);
+                mode == LCFO_SOFT_SLOPE || mode == LCFO_SOFT_SLOPE_DB || mode == LCFO_SOFT_NCC);
     if (mode == LCFO_SOFT_ADAPTIVE) { c = 0; lcf_oracle_weights_adaptive(lam, N, beta, wt); }
     else lcf_oracle_weights(N, soft, c, beta, wt);
     lcf_oracle_filter(V, wt, N, F);

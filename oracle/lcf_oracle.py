@@ -18,7 +18,7 @@ _SRC = _HERE / "lcf_oracle.c"
 _LIB = _HERE / "liblcf_oracle.so"
 _lib = None
 
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE, HARD_SLOPE_DB, SOFT_SLOPE_DB = range(13)
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE, HARD_SLOPE_DB, SOFT_SLOPE_DB, HARD_NCC, SOFT_NCC = range(15)
 
 
 def build(force: bool = False) -> Path:
@@ -54,6 +54,10 @@ def _load():
         L.lcf_oracle_cutoff_slope.restype = C.c_int
         L.lcf_oracle_cutoff_slope_db.argtypes = [dp, C.c_int, C.c_double]
         L.lcf_oracle_cutoff_slope_db.restype = C.c_int
+        L.lcf_oracle_left_singular_mag.argtypes = [fp, C.c_int, C.c_int, C.c_int, dp, dp, dp, dp, dp]
+        L.lcf_oracle_left_singular_mag.restype = None
+        L.lcf_oracle_cutoff_ncc.argtypes = [dp, C.c_size_t, C.c_int, C.c_int, dp]
+        L.lcf_oracle_cutoff_ncc.restype = C.c_int
         L.lcf_oracle_weights.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, dp]
         L.lcf_oracle_weights.restype = None
         L.lcf_oracle_weights_adaptive.argtypes = [dp, C.c_int, C.c_double, dp]
@@ -147,6 +151,26 @@ def cutoff_slope_db(lam: np.ndarray, thresh_db: float) -> int:
     """Named variant of method 2: the same rule on the curve in dB."""
     lam = np.ascontiguousarray(lam, dtype=np.float64)
     return int(_load().lcf_oracle_cutoff_slope_db(_d(lam), lam.size, float(thresh_db)))
+
+
+def left_singular_mag(iq: np.ndarray, gz: np.ndarray, gx: np.ndarray, lam: np.ndarray, V: np.ndarray) -> np.ndarray:
+    """|u_i(p)| of the windowed data's left singular vectors: [Nx][Nz][N]."""
+    a, p, N, Nx, Nz = _iq(iq)
+    gz = np.ascontiguousarray(gz, dtype=np.float64); gx = np.ascontiguousarray(gx, dtype=np.float64)
+    lam = np.ascontiguousarray(lam, dtype=np.float64); V = _c2d(V)
+    U = np.empty((Nx, Nz, N), dtype=np.float64)
+    _load().lcf_oracle_left_singular_mag(p, N, Nx, Nz, _d(gz), _d(gx), _d(lam), _d(V), _d(U))
+    return U
+
+
+def cutoff_ncc(Umag: np.ndarray, fn: int = 5):
+    """Method 4 (Eq. 8): (k, ncc curve [N]) from |u_i(p)| given as [..., N] (any leading pixel shape)."""
+    U = np.ascontiguousarray(Umag, dtype=np.float64)
+    N = U.shape[-1]
+    P = U.size // N
+    ncc = np.empty(N, dtype=np.float64)
+    k = int(_load().lcf_oracle_cutoff_ncc(_d(U), P, N, int(fn), _d(ncc)))
+    return k, ncc
 
 
 def cutoff_curvature(lam: np.ndarray, scale: float) -> int:

@@ -512,3 +512,84 @@ def test_run_invariances_and_composition(oracle):
         c = int(v["c"][k])
         Pl = Vl[:, ::-1][:, :c] @ Vl[:, ::-1][:, :c].conj().T
         assert np.linalg.norm(V[:, :c] @ V[:, :c].conj().T - Pl) <= 1e-10
+
+
+# ---------------------------------------------------------------- method 4: spatial NCC cut-off (Eq. 8)
+def test_left_singular_vectors_pins(oracle):
+    # C V = U D, lambda_i = sigma_i^2.  The magnitudes |u_i(p)| must be those of LAPACK's left
+    # singular vectors of the (windowed) Casorati matrix; each u_i has unit norm.
+    rng = np.random.default_rng(21)
+    Nz, Nx, N = 7, 5, 6
+    iq = (cn(rng, (N, Nx, Nz)) * np.array([9.0, 4.0, 2.0, 1.0, 0.5, 0.2])[:, None, None]).astype(np.complex64)
+    for gz, gx in ((np.ones(Nz), np.ones(Nx)), (np.linspace(0.2, 1.0, Nz), np.array([1.0, 0.5, 0.0, 0.7, 0.9]))):
+        R = oracle.gram(iq, gz, gx)
+        lam, V, _ = oracle.jacobi(R)
+        Um = oracle.left_singular_mag(iq, gz, gx, lam, V)                     # [Nx][Nz][N]
+        Cw = np.outer(gx, gz).reshape(-1, 1) * casorati(iq)
+        U, S, Vh = np.linalg.svd(Cw, full_matrices=False)
+        assert np.allclose(S ** 2, lam, rtol=1e-10)
+        assert np.allclose(Um.reshape(-1, N), np.abs(U), rtol=0, atol=1e-9)
+        assert np.allclose((Um.reshape(-1, N) ** 2).sum(0), 1.0, rtol=1e-10)
+        assert (Um[gx == 0] == 0).all()                                       # outside the window support
+    # a component with lambda = 0 (rank-deficient data) has no left singular vector: |u| = 0 by our reading
+    iq2 = synth.rank_r_clutter(6, 5, 5, 2, seed=3)
+    R = oracle.gram(iq2, np.ones(6), np.ones(5))
+    lam, V, _ = oracle.jacobi(R)
+    Um = oracle.left_singular_mag(iq2, np.ones(6), np.ones(5), lam, V)
+    assert (Um[..., 2:] == 0).all() and np.allclose((Um[..., :2] ** 2).sum((0, 1)), 1.0, rtol=1e-6)
+
+
+def test_ncc_cutoff_pins(oracle):
+    # Eq. 8 with the simplified images of PAPER.md:107 (fn components on either side of k).
+    # hand-built: components 1..k0 live on pixels [0, 10), components k0+1.. on pixels [10, 20): at k = k0 the tissue
+    # and blood images have disjoint supports -> NCC = 0 exactly; every other k mixes the two sets on one side.
+    P, N, fn = 20, 12, 5
+    for k0 in (3, 5, 6):
+        U = np.zeros((P, N))
+        U[:10, :k0] = 1.0 + 0.1 * np.arange(k0)
+        U[10:, k0:] = 2.0 + 0.1 * np.arange(N - k0)
+        k, ncc = oracle.cutoff_ncc(U, fn)
+        assert k == k0 and ncc[k0 - 1] == 0.0 and (np.delete(ncc, k0 - 1) > 0).all() and np.isinf(ncc[-1])
+    # identical spatial patterns in every component: NCC = 1 everywhere, the lowest k wins the tie
+    U = np.tile(np.linspace(1.0, 2.0, P)[:, None], (1, N))
+    k, ncc = oracle.cutoff_ncc(U, fn)
+    assert k == 1 and np.allclose(ncc[:-1], 1.0, rtol=1e-14)
+    # a k whose tissue (or blood) image vanishes everywhere is never chosen
+    U = np.abs(np.random.default_rng(0).standard_normal((P, N)))
+    U[:, :2] = 0.0
+    k, ncc = oracle.cutoff_ncc(U, 2)                                           # I_T(1), I_T(2) = 0
+    assert np.isinf(ncc[0]) and np.isinf(ncc[1]) and k >= 3
+    # brute force from the definition in numpy (1-based sums clipped to 1..N), random magnitudes, several fn
+    rng = np.random.default_rng(8)
+    for n, f in ((4, 5), (9, 2), (16, 5), (33, 5), (33, 1)):
+        U = np.abs(rng.standard_normal((37, n))) ** 3
+        k, ncc = oracle.cutoff_ncc(U, f)
+        ref = np.full(n, np.inf)
+        for kk in range(1, n):
+            it = U[:, max(kk - f, 0):kk].sum(1)                                 # i = kk-f+1 .. kk  (0-based columns kk-f .. kk-1)
+            ib = U[:, kk:min(kk + f, n)].sum(1)                                 # i = kk+1 .. kk+f
+            ref[kk - 1] = (it * ib).sum() / np.sqrt((it * it).sum() * (ib * ib).sum())
+        assert np.allclose(ncc, ref, rtol=1e-12) and k == int(np.argmin(ref)) + 1
+    # NCC is invariant to a common scaling of all magnitudes and to a permutation of the pixels
+    U = np.abs(rng.standard_normal((50, 14)))
+    k1, n1 = oracle.cutoff_ncc(U, 5)
+    k2, n2 = oracle.cutoff_ncc(7.3 * U[rng.permutation(50)], 5)
+    assert k1 == k2 and np.allclose(n1, n2, rtol=1e-12)
+
+
+def test_ncc_mode_runs_like_fixed_cut(oracle):
+    # method 4 end to end: the window's cut-off is the NCC minimum of its own left singular vectors, and
+    # the image equals the fixed-cut image with that k (hard, and method 5's sigmoid around it)
+    cfg = synth.scaled_config(synth.baseline_configs()[0], Nz=24, Nx=20, N=16, n_frames=16)
+    iq = synth.generate(cfg)
+    for mode_ncc, mode_fix in ((oracle.HARD_NCC, oracle.HARD_FIXED), (oracle.SOFT_NCC, oracle.SOFT_FIXED)):
+        a = oracle.run(iq, 2, 1, 8.0, 8.0, 3.0, mode_ncc, beta=0.7, want_R=True)
+        gz, gx = oracle.axis_windows(24, 2, 8.0, 3.0), oracle.axis_windows(20, 1, 8.0, 3.0)
+        PD = np.zeros((20, 24))
+        for kz in range(2):
+            lam, V, _ = oracle.jacobi(a["R"][kz])
+            k, _ = oracle.cutoff_ncc(oracle.left_singular_mag(iq, gz[kz], gx[0], lam, V), 5)
+            assert k == a["c"][kz] and 1 <= k <= 15
+            w = oracle.window(iq, gz[kz], gx[0], mode_fix, k_fixed=k, beta=0.7)
+            PD += w["PDk"] / w["mean"]
+        assert np.allclose(a["PD"], PD, rtol=1e-12)
