@@ -63,7 +63,7 @@ def parse_args():
 
 def workload_name(cfg) -> str:
     d, f = cfg.data, cfg.filt
-    mode = {0: "hard_fixed", 1: "hard_energy", 2: "soft_fixed", 3: "soft_energy", 4: "hard_median", 5: "soft_median", 6: "hard_curvature", 7: "soft_curvature", 8: "soft_adaptive", 9: "hard_slope", 10: "soft_slope", 11: "hard_slope_db", 12: "soft_slope_db"}[f.mode]
+    mode = {0: "hard_fixed", 1: "hard_energy", 2: "soft_fixed", 3: "soft_energy", 4: "hard_median", 5: "soft_median", 6: "hard_curvature", 7: "soft_curvature", 8: "soft_adaptive", 9: "hard_slope", 10: "soft_slope", 11: "hard_slope_db", 12: "soft_slope_db", 13: "hard_ncc", 14: "soft_ncc"}[f.mode]
     return (f"{cfg.name}: IQ {d.Nz}x{d.Nx}x{d.N} complex64, {f.Kz}x{f.Kx} windows sigma={f.sigma_z:g} "
             f"trunc={f.trunc:g}, {mode}, precision={f.precision}")
 

@@ -73,7 +73,14 @@ typedef enum {
     LCF_SOFT_SLOPE = 10,    /* sigmoid (Eq. 9) centred on the slope-rule c                          */
     LCF_HARD_SLOPE_DB = 11, /* named variant of method 2: the same rule on y(n) = 10 log10(l_n), cut_scale
                             in dB per eigenvalue index (eigenvalues floored at 1e-12 l_1)           */
-    LCF_SOFT_SLOPE_DB = 12  /* sigmoid (Eq. 9) centred on the dB-slope c                            */
+    LCF_SOFT_SLOPE_DB = 12, /* sigmoid (Eq. 9) centred on the dB-slope c                            */
+    LCF_HARD_NCC = 13,      /* hard, method 4 (Eq. 8): c = argmin over k = 1..N-1 of the spatial
+                            normalised cross-correlation of I_T(k) = sum_{i=k-4..k} |u_i| and I_B(k) =
+                            sum_{i=k+1..k+5} |u_i| (clipped to 1..N), u_i = C_w v_i / sigma_i the left singular
+                            vectors of the windowed data (fn = 5, w_i = 1; lowest k on ties;
+                            DESIGN.md "Readings" 19).  Costs a third pass over the data                 */
+    LCF_SOFT_NCC = 14       /* sigmoid (Eq. 9) centred on the NCC c: methods 4 + 5 as the paper pairs them
+                                                                                       */
 } lcf_thresh_mode;
 
 typedef struct {
@@ -157,6 +164,8 @@ lcf_status lcf_get_sweeps(lcf_plan* plan, int* sweeps /* HOST [K]: Jacobi sweeps
 lcf_status lcf_get_gram(lcf_plan* plan, double* R /* HOST [K][N][N][2], R[i][j] as in Eq. 12 */);
 /* V[a][i] = component a of the eigenvector of the i-th largest eigenvalue */
 lcf_status lcf_get_eigenvectors(lcf_plan* plan, double* V /* HOST [K][N][N][2] */);
+/* NCC modes only (LCF_ERR_INVALID_ARG otherwise): ncc[k-1] = NCC(k) of Eq. 8 for k = 1..N-1, ncc[N-1] = +inf */
+lcf_status lcf_get_ncc(lcf_plan* plan, double* ncc /* HOST [K][N] */);
 /* wt[i] = weight of the i-th largest eigenvalue (0-based storage of the paper's 1-based i) */
 lcf_status lcf_get_weights(lcf_plan* plan, double* wt /* HOST [K][N] */);
 /* F_k = V diag(wt) V^H (Eq. 4), built on the device from V and wt */

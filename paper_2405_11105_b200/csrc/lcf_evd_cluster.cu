@@ -946,7 +946,7 @@ cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st) {
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d; a.nunconv = p->nunconv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
-    a.mode = p->thr.mode; a.k_fixed = p->thr.k_fixed; a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
+    a.mode = evd_mode(p); a.k_fixed = evd_kfixed(p); a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
     if (p->N % 4 == 0) {
         jacobi_cluster_block_kernel<<<2 * p->K, ECL_THREADS, p->ecl_smem, st>>>(a);
         return cudaGetLastError();

@@ -185,6 +185,12 @@ struct lcf_plan {
     double* wt_d = nullptr;    // [K][N] weight by rank
     void* V_d = nullptr;       // [K][N][Ns] complex real, slot order
     float2* B_d = nullptr;     // [K][N][Ns] complex float: V diag(wslot)
+    // method 4 (spatial NCC cut-off, lcf_ncc.cu): allocated for the NCC modes only
+    float* ncc_mag_d = nullptr;        // [sum_k P_k][ncc_magN]  |u_i(p)| by rank
+    int ncc_magN = 0;
+    float* ncc_isig_d = nullptr;       // [K][ncc_magN]
+    float* ncc_part_d = nullptr;       // [K][32 chunks][3][N]
+    double* ncc_curve_d = nullptr;     // [K][N]  NCC(k), k = 1..N (last = +inf)
     // projection / combine
     lcf::ProjItem* pitems_d = nullptr;
     int n_pitems = 0;
@@ -260,4 +266,10 @@ bool project_tc_eligible(const lcf_plan* p);
 cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::vector<int>& cta_first);
 cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st);
 cudaError_t launch_absmax(lcf_plan* p, const float2* iq, cudaStream_t st);
+bool ncc_mode(int mode);
+cudaError_t launch_ncc(lcf_plan* p, const float2* iq, cudaStream_t st);
+// what the EVD kernels are told: under the NCC modes they run with every eigen-weight 1 (hard cut at 0), so that
+// B_k = V_k for the left singular vectors; lcf_ncc.cu then sets the cut-off, the weights and B_k
+inline int evd_mode(const lcf_plan* p) { return (p->thr.mode == LCF_HARD_NCC || p->thr.mode == LCF_SOFT_NCC) ? (int)LCF_HARD_FIXED : (int)p->thr.mode; }
+inline int evd_kfixed(const lcf_plan* p) { return (p->thr.mode == LCF_HARD_NCC || p->thr.mode == LCF_SOFT_NCC) ? 0 : p->thr.k_fixed; }
 }  // namespace lcf

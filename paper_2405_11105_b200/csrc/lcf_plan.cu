@@ -70,6 +70,7 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->ec_gfac_d); cudaFree(p->ec_shift_d);
     cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d); cudaFree(p->amax_d);
     cudaFree(p->gtc_segs_d); cudaFree(p->gtc_cta_first_d); cudaFree(p->gtc_seg_first_d); cudaFree(p->gtc_part_d);
+    cudaFree(p->ncc_mag_d); cudaFree(p->ncc_isig_d); cudaFree(p->ncc_part_d); cudaFree(p->ncc_curve_d);
     cudaFree(p->g2_segs_d); cudaFree(p->g2_cta_first_d); cudaFree(p->g2_seg_first_d); cudaFree(p->g2_part_d);
     if (p->timer.have)
         for (auto& set : p->timer.ev)
@@ -141,7 +142,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     if (!win || !thr) return LCF_ERR_INVALID_ARG;
     if (Nz < 1 || Nx < 1 || N < 2 || win->Kz < 1 || win->Kx < 1) return LCF_ERR_INVALID_ARG;
     if ((long long)Nz * Nx > (1LL << 30) || (long long)win->Kz * win->Kx > 65535) return LCF_ERR_INVALID_ARG;
-    if ((int)thr->mode < 0 || (int)thr->mode > 12 || (thr->precision != 0 && thr->precision != 1)) return LCF_ERR_INVALID_ARG;
+    if ((int)thr->mode < 0 || (int)thr->mode > 14 || (thr->precision != 0 && thr->precision != 1)) return LCF_ERR_INVALID_ARG;
     const bool fixed = thr->mode == LCF_HARD_FIXED || thr->mode == LCF_SOFT_FIXED;
     const bool soft = thresh_is_soft(thr->mode);
     if (fixed && (thr->k_fixed < 0 || thr->k_fixed > N)) return LCF_ERR_INVALID_ARG;
@@ -311,6 +312,11 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
              dev_alloc(&p->ptc_part_d, (size_t)p->ptc_NB * (size_t)(p->sumPk ? p->sumPk : 1));
     }
     if (p->gram_tc || p->gram_tc2 || p->proj_tc) ok = ok && dev_alloc(&p->amax_d, 1);
+    if (ncc_mode(thr->mode)) {
+        p->ncc_magN = p->proj_tc ? p->ptc_NB * 64 : N;
+        ok = ok && dev_alloc(&p->ncc_mag_d, (size_t)(p->sumPk ? p->sumPk : 1) * p->ncc_magN) && dev_alloc(&p->ncc_isig_d, K * p->ncc_magN) &&
+             dev_alloc(&p->ncc_part_d, K * 32 * 3 * N) && dev_alloc(&p->ncc_curve_d, K * N);
+    }
     ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->R_d), K * N2 * 2 * p->esz);
     // the rotation log is replayed by vbuild_kernel, which only follows the two-sided jacobi_kernel
     if (!p->evd_chol) ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->rotlog_d), K * p->max_sweeps * M * 3 * p->NP * p->esz);
@@ -369,6 +375,7 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     if (e == cudaSuccess && p->evd_cluster) run(2, launch_evd_cluster(p, st));
     mark(2);
     if (e == cudaSuccess && !p->evd_chol) run(3, launch_vbuild(p, st));
+    if (e == cudaSuccess && ncc_mode(p->thr.mode)) run(3, launch_ncc(p, iq, st));
     mark(3);
     if (e == cudaSuccess) run(4, p->proj_tc ? launch_project_tc(p, iq, st) : launch_project(p, iq, st));
     mark(4);
@@ -514,6 +521,14 @@ extern "C" lcf_status lcf_get_sweeps(lcf_plan* p, int* sw) {
     lcf_status s = sync_plan(p);
     if (s != LCF_OK || !sw) return s != LCF_OK ? s : LCF_ERR_INVALID_ARG;
     if (cudaMemcpy(sw, p->sweeps_d, sizeof(int) * p->K, cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
+    return conv_status(p);
+}
+
+extern "C" lcf_status lcf_get_ncc(lcf_plan* p, double* ncc) {
+    lcf_status s = sync_plan(p);
+    if (s != LCF_OK || !ncc) return s != LCF_OK ? s : LCF_ERR_INVALID_ARG;
+    if (!p->ncc_curve_d) return LCF_ERR_INVALID_ARG;           // not an NCC-mode plan
+    if (cudaMemcpy(ncc, p->ncc_curve_d, sizeof(double) * p->K * p->N, cudaMemcpyDeviceToHost) != cudaSuccess) return LCF_ERR_CUDA;
     return conv_status(p);
 }
 

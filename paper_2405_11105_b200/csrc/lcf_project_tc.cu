@@ -73,6 +73,11 @@ struct PtcArgs {
     float* part;                   // [NB][sum_k P_k]
     long long sumPk;
     int nstg;                      // raw / operand stages in use: PTC_RAW_STAGES, or 4 when the B block needs the room
+    // MAG variant (method 4, lcf_ncc.cu): B = V in rank order; instead of the power sum the epilogue writes
+    // |u_i(p)| = w(p) |U[p][i]| / sigma_i  to  mag[(tile_off + q) * magN + rank]
+    float* mag;
+    int magN;
+    const float* isig;             // [K][NB * 64]  1 / sigma by rank (0 beyond N or where sigma = 0)
 };
 
 struct PtcBars {
@@ -94,6 +99,7 @@ __device__ __forceinline__ void ptc_sts128(uint32_t addr, float x, float y, floa
 __device__ __forceinline__ void ptc_sts128u(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
+template <bool MAG>
 __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid_constant__ CUtensorMap tmap, PtcArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
@@ -105,6 +111,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
     PtcBars* bars = reinterpret_cast<PtcBars*>(ops + NSTG * PTC_OP_BYTES);
     double* gzs = reinterpret_cast<double*>(bars + 1);                        // [Nz] window table rows (epilogue only)
     double* gxs = gzs + a.Nz;                                                 // [Nx]
+    float* isig_s = reinterpret_cast<float*>(gxs + a.Nx);                     // [64] (MAG) 1 / sigma of the segment's column block
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int seg0 = a.cta_first[blockIdx.x], seg1 = a.cta_first[blockIdx.x + 1];
@@ -259,6 +266,12 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                 asm volatile("bar.sync 1, 128;" ::: "memory");
                 curk = seg.k;
             }
+            if (MAG) {
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                const int et = tid - PTC_FIRST_EPI * 32;
+                if (et < 64) isig_s[et] = a.isig[((size_t)seg.k * a.NB + seg.b) * 64 + et];
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+            }
             float* out = a.part + (size_t)seg.b * a.sumPk + bx.tile_off;
             for (int t = 0; t < seg.ntile; ++t, ++tl) {
                 const uint32_t buf = tl & 1;
@@ -267,7 +280,14 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                 const int zz = ze + tzi * PTC_TZ + zi, xx = bx.x0 + txi * PTC_TX + xi;
                 mbar_wait(&bars->accfull[buf], (tl >> 1) & 1);
                 tc_fence_after_sync();
+                const bool valid = zz >= bx.z0 && zz < bx.z0 + bx.Lz && xx < bx.x0 + bx.Lx;
                 float acc = 0.f;
+                float wpix = 0.f;
+                float* mrow = nullptr;
+                if (MAG && valid) {
+                    wpix = (float)(gzs[zz] * gxs[xx]);
+                    mrow = a.mag + ((size_t)bx.tile_off + (size_t)(xx - bx.x0) * bx.Lz + (zz - bx.z0)) * a.magN + seg.b * PTC_UB;
+                }
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     uint32_t va[16], vb[16], vc[16], vd[16];
@@ -277,22 +297,39 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                     tmem_ld16(tlane + col + 128, vc);
                     tmem_ld16(tlane + col + 192, vd);
                     tmem_ld_wait();
+                    float mg[16];
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
                         const float pr = __uint_as_float(va[i]) + __uint_as_float(vc[i]);
                         const float pi = __uint_as_float(vb[i]) + __uint_as_float(vd[i]);
                         const float po = __shfl_xor_sync(0xffffffffu, pi, 1);
                         const float val = ((lane & 1) ? pr + po : pr - po) * unscale;   // odd row: Im U, even row: Re U
-                        acc = fmaf(val, val, acc);
+                        if (MAG) {
+                            const float v2 = val * val;
+                            mg[i] = sqrtf(v2 + __shfl_xor_sync(0xffffffffu, v2, 1)) * isig_s[j * 16 + i] * wpix;
+                        } else {
+                            acc = fmaf(val, val, acc);
+                        }
+                    }
+                    if (MAG && valid) {                      // the pair's even lane stores ranks 0-7 of the 16, the odd lane 8-15
+                        const bool odd = (lane & 1) != 0;
+                        float s8[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) s8[i] = odd ? mg[8 + i] : mg[i];
+                        float4* o4 = reinterpret_cast<float4*>(mrow + j * 16 + (odd ? 8 : 0));
+                        o4[0] = make_float4(s8[0], s8[1], s8[2], s8[3]);
+                        o4[1] = make_float4(s8[4], s8[5], s8[6], s8[7]);
                     }
                 }
                 tc_fence_before_sync();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&bars->accempty[buf]);
-                acc += __shfl_xor_sync(0xffffffffu, acc, 1);
-                if (!(lane & 1) && zz >= bx.z0 && zz < bx.z0 + bx.Lz && xx < bx.x0 + bx.Lx) {
-                    const double w = gzs[zz] * gxs[xx];
-                    out[(size_t)(xx - bx.x0) * bx.Lz + (zz - bx.z0)] = (float)(w * w) * acc;
+                if (!MAG) {
+                    acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+                    if (!(lane & 1) && valid) {
+                        const double w = gzs[zz] * gxs[xx];
+                        out[(size_t)(xx - bx.x0) * bx.Lz + (zz - bx.z0)] = (float)(w * w) * acc;
+                    }
                 }
             }
         }
@@ -318,6 +355,30 @@ __global__ void proj_tc_pack_kernel(const float2* B, int N, int Ns, int Kp, int 
         const int t = 8 * c8 + i;
         x[i] = 0.f;
         if (t < N && u < Ns) { const float2 c = Bk[(size_t)t * Ns + u]; x[i] = (im ? c.y : c.x) * PTC_B_SCALE; }
+    }
+    uint32_t h[4], l[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) f16_split2(x[2 * i], x[2 * i + 1], h[i], l[i]);
+    out[r] = lo ? make_uint4(l[0], l[1], l[2], l[3]) : make_uint4(h[0], h[1], h[2], h[3]);
+}
+
+// Same operand tile from B_k with the columns in RANK order (column b * 64 + j of the tile = the eigenvector of the
+// (b * 64 + j + 1)-th largest eigenvalue): method 4 needs the components side by side in eigenvalue order.
+__global__ void proj_tc_pack_rank_kernel(const float2* B, const int* order, int N, int Ns, int Kp, int NB, float* bpack) {
+    const int kb = blockIdx.x / (Kp / 8), c8 = blockIdx.x - kb * (Kp / 8);
+    const int k = kb / NB, b = kb - k * NB;
+    const float2* Bk = B + (size_t)k * N * Ns;
+    uint4* out = reinterpret_cast<uint4*>(bpack + (size_t)kb * (Kp / 8) * 1024) + (size_t)c8 * 256;
+    const int r = threadIdx.x;
+    const int rank = b * PTC_UB + (r & 63);
+    const int u = rank < N ? order[(size_t)k * N + rank] : -1;
+    const bool im = (r >> 6) & 1, lo = r >= 128;
+    float x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int t = 8 * c8 + i;
+        x[i] = 0.f;
+        if (t < N && u >= 0) { const float2 c = Bk[(size_t)t * Ns + u]; x[i] = (im ? c.y : c.x) * PTC_B_SCALE; }
     }
     uint32_t h[4], l[4];
 #pragma unroll
@@ -441,9 +502,18 @@ cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::ve
     p->ptc_nseg = (int)segs.size();
     p->ptc_nstg = p->ptc_Kp <= 128 ? PTC_RAW_STAGES : 4;
     p->ptc_smem = 1024 + (size_t)(p->ptc_Kp / 8) * PTC_B_LBO + (size_t)p->ptc_nstg * (PTC_RAW_BYTES + PTC_OP_BYTES) + sizeof(PtcBars) + 16 +
-                  (size_t)(p->Nz + p->Nx) * sizeof(double);
+                  (size_t)(p->Nz + p->Nx) * sizeof(double) + 64 * sizeof(float);
     if (p->ptc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
-    return set_max_dyn_smem(project_tc_kernel, p->smem_optin);
+    cudaError_t e = set_max_dyn_smem(project_tc_kernel<false>, p->smem_optin);
+    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<true>, p->smem_optin);
+    return e;
+}
+
+static void ptc_fill_args(lcf_plan* p, PtcArgs& a) {
+    a.N = p->N; a.Kp = p->ptc_Kp; a.Nz = p->Nz; a.Nx = p->Nx;
+    a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->ptc_segs_d; a.cta_first = p->ptc_cta_first_d;
+    a.bpack = p->ptc_bpack_d; a.amax = p->amax_d; a.NB = p->ptc_NB; a.part = p->ptc_part_d; a.sumPk = p->sumPk; a.nstg = p->ptc_nstg;
+    a.mag = nullptr; a.magN = 0; a.isig = nullptr;
 }
 
 cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
@@ -454,13 +524,27 @@ cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     PtcArgs a;
-    a.N = p->N; a.Kp = p->ptc_Kp; a.Nz = p->Nz; a.Nx = p->Nx;
-    a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->ptc_segs_d; a.cta_first = p->ptc_cta_first_d;
-    a.bpack = p->ptc_bpack_d; a.amax = p->amax_d; a.NB = p->ptc_NB; a.part = p->ptc_part_d; a.sumPk = p->sumPk; a.nstg = p->ptc_nstg;
-    project_tc_kernel<<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(*tmap, a);
+    ptc_fill_args(p, a);
+    project_tc_kernel<false><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(*tmap, a);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     proj_tc_finish_kernel<<<p->n_pitems, PROJ_TPIX, 0, st>>>(p->ptc_part_d, p->sumPk, p->ptc_NB, p->box_d, p->pitems_d, p->tiles_d, p->tsum_d);
+    return cudaGetLastError();
+}
+
+// Method 4 (lcf_ncc.cu): |u_i(p)| = w(p) |(s_p V)_i| / sigma_i for every pixel of every window, components in rank
+// order, through the same tcgen05 pipeline (B_d must hold V, i.e. all eigen-weights 1).
+cudaError_t launch_project_tc_mag(lcf_plan* p, const float2* iq, cudaStream_t st) {
+    if (p->ptc_nseg == 0 || p->n_pitems == 0) return cudaSuccess;
+    const CUtensorMap* tmap = ptc_encode_map(p, iq);
+    if (!tmap) return cudaErrorInvalidValue;
+    proj_tc_pack_rank_kernel<<<p->K * p->ptc_NB * (p->ptc_Kp / 8), 256, 0, st>>>(p->B_d, p->order_d, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    PtcArgs a;
+    ptc_fill_args(p, a);
+    a.mag = p->ncc_mag_d; a.magN = p->ncc_magN; a.isig = p->ncc_isig_d;
+    project_tc_kernel<true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(*tmap, a);
     return cudaGetLastError();
 }
 

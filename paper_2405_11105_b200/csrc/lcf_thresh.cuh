@@ -11,6 +11,7 @@
 //              taken relative to l_1 (N - 1 if the curve never flattens)           method 2
 //   slope_db   the same rule on y(n) = 10 log10(l_n) (dB per index; eigenvalues floored at 1e-12 l_1):
 //              a named variant, not the printed form (DESIGN.md "Readings" 18)
+//   ncc        c = argmin_k NCC(I_T(k), I_B(k))                 method 4, Eq. 8: lcf_ncc.cu (needs the data)
 //   hard       wt_i = 0 for i <= c, 1 above
 //   soft       wt_i = 1 / (1 + exp(-beta (i - c)))          method 5, Eq. 9
 //   adaptive   wt_i = win(i) / l_i^beta, normalised to max 1     method 6, Eq. 10
@@ -25,7 +26,7 @@ namespace lcf {
 
 __host__ __device__ inline bool thresh_is_soft(int mode) {
     return mode == LCF_SOFT_FIXED || mode == LCF_SOFT_ENERGY || mode == LCF_SOFT_MEDIAN || mode == LCF_SOFT_CURVATURE ||
-           mode == LCF_SOFT_ADAPTIVE || mode == LCF_SOFT_SLOPE || mode == LCF_SOFT_SLOPE_DB;
+           mode == LCF_SOFT_ADAPTIVE || mode == LCF_SOFT_SLOPE || mode == LCF_SOFT_SLOPE_DB || mode == LCF_SOFT_NCC;
 }
 
 __device__ inline int thresh_cutoff(int mode, int k_fixed, double energy_frac, double cut_scale, const double* lsort, int N) {

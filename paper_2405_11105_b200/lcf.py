@@ -14,7 +14,7 @@ import numpy as np
 HERE = Path(__file__).resolve().parent
 LIB_PATH = HERE / "liblcf.so"
 
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE, HARD_SLOPE_DB, SOFT_SLOPE_DB = range(13)
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE, HARD_SLOPE_DB, SOFT_SLOPE_DB, HARD_NCC, SOFT_NCC = range(15)
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_NOT_CONVERGED = range(6)
 
 EXPORTS = [
@@ -22,7 +22,7 @@ EXPORTS = [
     "lcf_get_eigenvalues", "lcf_get_cutoffs", "lcf_get_sweeps", "lcf_get_gram", "lcf_get_eigenvectors",
     "lcf_get_weights", "lcf_get_filters", "lcf_get_window_means", "lcf_set_timing", "lcf_get_stage_ms",
     "lcf_get_work", "lcf_measure_peak", "lcf_status_string", "lcf_last_error", "lcf_scale_exponent",
-    "lcf_get_converged", "lcf_set_max_sweeps",
+    "lcf_get_converged", "lcf_set_max_sweeps", "lcf_get_ncc",
 ]
 
 
@@ -67,7 +67,7 @@ def load() -> C.CDLL:
         L.lcf_filter_batch.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp]
         L.lcf_plan_destroy.argtypes = [vp]
         L.lcf_num_windows.argtypes = [vp]
-        for name in ("lcf_get_eigenvalues", "lcf_get_gram", "lcf_get_eigenvectors", "lcf_get_weights",
+        for name in ("lcf_get_eigenvalues", "lcf_get_ncc", "lcf_get_gram", "lcf_get_eigenvectors", "lcf_get_weights",
                      "lcf_get_filters", "lcf_get_window_means"):
             getattr(L, name).argtypes = [vp, dp]
         L.lcf_get_cutoffs.argtypes = [vp, ip]
@@ -272,6 +272,10 @@ class Plan:
 
     def weights(self, **kw):
         return self._get_d("lcf_get_weights", (self.K, self.N), **kw)
+
+    def ncc(self, **kw):
+        """NCC(k) curves of method 4, [K][N] (NCC-mode plans only)."""
+        return self._get_d("lcf_get_ncc", (self.K, self.N), **kw)
 
     def window_means(self, **kw):
         return self._get_d("lcf_get_window_means", (self.K,), **kw)

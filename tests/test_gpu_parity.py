@@ -229,6 +229,61 @@ def test_small_shapes_and_modes(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, trunc, mo
                 assert np.linalg.norm(g["F"][kk] - o["F"][kk]) <= 1e-6
 
 
+NCC_CASES = [
+    # Nz, Nx, N, Kz, Kx, sigma, mode, precision
+    (64, 48, 64, 2, 2, 14.0, synth.HARD_NCC, 1),     # method 4, fp64 Gram/EVD, tcgen05 magnitude pass (two column blocks)
+    (64, 48, 64, 2, 2, 14.0, synth.SOFT_NCC, 0),     # methods 4 + 5 on the tensor / cluster path
+    (48, 40, 100, 2, 1, 12.0, synth.SOFT_NCC, 0),    # N = 100: padded column block
+    (45, 40, 32, 1, 2, 12.0, synth.HARD_NCC, 1),     # odd Nz: FP32 magnitude fallback
+    (40, 24, 12, 2, 1, 10.0, synth.SOFT_NCC, 1),     # N < 16: fallback, fn windows clipped at both ends
+]
+
+
+@pytest.mark.parametrize("Nz,Nx,N,Kz,Kx,sigma,mode,prec", NCC_CASES)
+def test_ncc_cutoff_method4(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, mode, prec):
+    """Method 4 (Eq. 8): the NCC curve of every window against the oracle's (computed from the
+    oracle's own eigenvectors), the argmin exactly where the oracle's minimum is distinct, and the image."""
+    cfg = synth.baseline_configs()[2]
+    d = replace(cfg.data, Nz=Nz, Nx=Nx, N=N, n_frames=N, seed=300 + N, n_vessels=3, tissue_db=40.0, noise_db=-55.0)
+    f = synth.FilterSpec(Kz, Kx, sigma, sigma, 3.0, mode, precision=prec, beta=0.7)
+    iq = synth.generate_sequence(d)
+    o = oracle.run_config(iq, f, want_V=True)
+    gz, gx = oracle.axis_windows(Nz, Kz, sigma, 3.0), oracle.axis_windows(Nx, Kx, sigma, 3.0)
+    import torch
+    iq_d = torch.from_numpy(iq).cuda()
+    pd_d = torch.full((Nx, Nz), float("nan"), dtype=torch.float32, device="cuda")
+    with lcf.Plan.from_spec(Nz, Nx, N, f) as plan:
+        plan.filter(iq_d, pd_d)
+        torch.cuda.synchronize()
+        g = {"lam": plan.eigenvalues(), "c": plan.cutoffs(), "ncc": plan.ncc(), "wt": plan.weights(),
+             "PD": pd_d.cpu().numpy().astype(np.float64)}
+    lmax = o["lam"][:, :1]
+    assert (np.abs(g["lam"] - o["lam"]) / lmax).max() <= LAM_TOL
+    for k in range(Kz * Kx):
+        Um = oracle.left_singular_mag(iq, gz[k % Kz], gx[k // Kz], o["lam"][k], o["V"][k])
+        kk, ncc_o = oracle.cutoff_ncc(Um, 5)
+        assert kk == o["c"][k]
+        fin = np.isfinite(ncc_o)
+        assert np.array_equal(np.isfinite(g["ncc"][k]), fin)
+        # the curve is a ratio of sums over |u_i|.  precision 1: 2e-4 everywhere.  precision 0: the fp32 EVD cannot resolve
+        # the individual singular vectors inside the flat noise floor (relative gaps ~1e-2, PAPER.md:262 is the paper's own
+        # caveat), so only the first quarter of the curve -- where tissue meets blood -- is held to 1e-2, the rest to 3e-2
+        tolk = np.full(N, 2e-4) if prec == 1 else np.where(np.arange(N) < N // 4, 1e-2, 3e-2)
+        with np.errstate(invalid="ignore"):
+            err = np.abs(g["ncc"][k] - ncc_o)
+        assert (err[fin] <= tolk[fin]).all(), (err[fin] / tolk[fin]).max()
+        # the minimum found must be the oracle's minimum up to those tolerances (equal when it is distinct)
+        gc = int(g["c"][k])
+        assert 1 <= gc <= N - 1 and ncc_o[gc - 1] - ncc_o[kk - 1] <= tolk[gc - 1] + tolk[kk - 1]
+        others = np.delete(np.arange(N)[fin], np.where(np.arange(N)[fin] == kk - 1))
+        if others.size == 0 or (ncc_o[others] - ncc_o[kk - 1] > tolk[others] + tolk[kk - 1]).all():
+            assert gc == kk, (k, gc, kk)
+        soft = mode == synth.SOFT_NCC
+        assert np.allclose(g["wt"][k], oracle.weights(N, soft, int(g["c"][k]), f.beta), rtol=0, atol=1e-12)
+    if np.array_equal(g["c"], o["c"]):
+        check_pd(g["PD"], o["PD"])
+
+
 def test_allpass_and_allstop(lcf, oracle):
     iq = synth.random_cube(32, 24, 12, seed=5)
     f0 = synth.FilterSpec(2, 2, 8.0, 8.0, 3.0, synth.HARD_FIXED, k_fixed=0)
