@@ -501,6 +501,14 @@ def run_ours(args, cfg):
                 del seq
             except Exception as ex:
                 per_config[f"config{ci}"] = {"error": repr(ex)}
+        try:                                                 # the metric workload with method 4 + 5 (NCC cut-off): one more pass over the data
+            from dataclasses import replace as _rep
+            c = _rep(cfg, filt=_rep(cfg.filt, mode=synth.SOFT_NCC))
+            r = quick_latency(lcf, torch, c, iq_h.numpy())
+            r["workload"] = workload_name(c)
+            per_config["config2_method4_ncc"] = r
+        except Exception as ex:
+            per_config["config2_method4_ncc"] = {"error": repr(ex)}
         # ---- paper-shaped context runs (phantom 196x180, kidney 180x180, liver 177x173; packets
         # 50/70/90; global, 2x2, 3x3 un-truncated Gaussian subsets, fixed cut): ms per packet next to the paper's
         # 2.4 / 16.6 / 39.8 ms (RTX A6000 + Xeon, MATLAB).  Synthetic data of that shape; context, not the target.
