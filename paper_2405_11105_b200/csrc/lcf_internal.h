@@ -171,6 +171,9 @@ struct lcf_plan {
     float* ptc_bpack_d = nullptr;           // [K][NB][Kp/4][256][4]
     float* ptc_part_d = nullptr;            // [NB][sum_k P_k]
     lcf::TmapCache ptc_tmaps;
+    bool ptc_pre = false, ptc_premaps_ready = false;   // pre-split fp16 planes of the ensemble (lcf_project_tc.cu, PRE variant)
+    void *ptc_sh_d = nullptr, *ptc_sl_d = nullptr;     // [Kp/8][Nx][Nz][2][8] fp16 hi / lo
+    alignas(64) unsigned char ptc_premaps[256];
     uint32_t* amax_d = nullptr;             // bits of max |re|, |im| over the ensemble (tensor-core paths scale by a power of two)
     // EVD
     void* rotlog_d = nullptr;  // [K][max_sweeps*(Ns-1)][3][NP] real
@@ -266,6 +269,7 @@ bool project_tc_eligible(const lcf_plan* p);
 cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::vector<int>& cta_first);
 cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st);
 cudaError_t launch_absmax(lcf_plan* p, const float2* iq, cudaStream_t st);
+cudaError_t launch_presplit(lcf_plan* p, const float2* iq, cudaStream_t st);
 bool ncc_mode(int mode);
 cudaError_t launch_ncc(lcf_plan* p, const float2* iq, cudaStream_t st);
 // what the EVD kernels are told: under the NCC modes they run with every eigen-weight 1 (hard cut at 0), so that

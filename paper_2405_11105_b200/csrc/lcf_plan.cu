@@ -70,6 +70,7 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->ec_gfac_d); cudaFree(p->ec_shift_d);
     cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d); cudaFree(p->amax_d);
     cudaFree(p->gtc_segs_d); cudaFree(p->gtc_cta_first_d); cudaFree(p->gtc_seg_first_d); cudaFree(p->gtc_part_d);
+    cudaFree(p->ptc_sh_d); cudaFree(p->ptc_sl_d);
     cudaFree(p->ncc_mag_d); cudaFree(p->ncc_isig_d); cudaFree(p->ncc_part_d); cudaFree(p->ncc_curve_d);
     cudaFree(p->g2_segs_d); cudaFree(p->g2_cta_first_d); cudaFree(p->g2_seg_first_d); cudaFree(p->g2_part_d);
     if (p->timer.have)
@@ -312,6 +313,10 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
              dev_alloc(&p->ptc_part_d, (size_t)p->ptc_NB * (size_t)(p->sumPk ? p->sumPk : 1));
     }
     if (p->gram_tc || p->gram_tc2 || p->proj_tc) ok = ok && dev_alloc(&p->amax_d, 1);
+    if (p->proj_tc && p->ptc_pre) {
+        const size_t plane = (size_t)(p->ptc_Kp / 8) * (size_t)p->P * 32;
+        ok = ok && dev_alloc(reinterpret_cast<unsigned char**>(&p->ptc_sh_d), plane) && dev_alloc(reinterpret_cast<unsigned char**>(&p->ptc_sl_d), plane);
+    }
     if (ncc_mode(thr->mode)) {
         p->ncc_magN = p->proj_tc ? p->ptc_NB * 64 : N;
         ok = ok && dev_alloc(&p->ncc_mag_d, (size_t)(p->sumPk ? p->sumPk : 1) * p->ncc_magN) && dev_alloc(&p->ncc_isig_d, K * p->ncc_magN) &&
@@ -369,6 +374,7 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     auto run = [&](int id, cudaError_t r) { if (e == cudaSuccess && r != cudaSuccess) { e = r; stage = id; } };
     mark(0);
     if (e == cudaSuccess && (p->gram_tc || p->gram_tc2 || p->proj_tc)) run(1, launch_absmax(p, iq, st));
+    if (e == cudaSuccess && p->proj_tc) run(1, launch_presplit(p, iq, st));
     if (e == cudaSuccess) run(1, p->gram_tc ? launch_gram_tc(p, iq, st) : (p->gram_tc2 ? launch_gram_tc2(p, iq, st) : launch_gram(p, iq, st)));
     mark(1);
     if (e == cudaSuccess) run(2, p->evd_chol ? launch_evd_chol(p, st, p->evd_cluster) : launch_jacobi(p, st));
@@ -642,7 +648,7 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
     w->gram_flops = 8.0 * S * N * (N + 1.0) / 2.0;   // Hermitian half, 8 real flops per complex MAC
     w->proj_flops = 8.0 * S * N * N;                 // dense N x N projector factor
     w->hbm_bytes = 8.0 * N * (double)p->P + 4.0 * (double)p->P;
-    w->launches = ((p->gram_tc || p->gram_tc2 || p->proj_tc) ? 1 : 0) + 2 + (p->evd_chol ? (p->evd_cluster ? 2 : 1) : 2) + (p->proj_tc ? 3 : 1) + 2;   // absmax, gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
+    w->launches = ((p->gram_tc || p->gram_tc2 || p->proj_tc) ? 1 : 0) + ((p->proj_tc && p->ptc_pre) ? 1 : 0) + 2 + (p->evd_chol ? (p->evd_cluster ? 2 : 1) : 2) + (p->proj_tc ? 3 : 1) + 2;   // absmax, gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
     w->gram_tc = (p->gram_tc || p->gram_tc2) ? 1 : 0; w->evd_chol = p->evd_chol ? 1 : 0; w->proj_tc = p->proj_tc ? 1 : 0;
     w->gram_tensor_flops = 0.0; w->proj_tensor_flops = 0.0;
     for (int k = 0; k < p->K; ++k) {

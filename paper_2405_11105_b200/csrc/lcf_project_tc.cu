@@ -33,6 +33,7 @@
 // into the per-window PD tiles and the per-chunk sums that the alpha / combine kernels use.
 #include <cuda.h>
 #include <cuda_fp16.h>
+#include <cstring>
 
 #include "lcf_internal.h"
 #include "lcf_sm100.cuh"
@@ -99,15 +100,21 @@ __device__ __forceinline__ void ptc_sts128(uint32_t addr, float x, float y, floa
 __device__ __forceinline__ void ptc_sts128u(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
-template <bool MAG>
-__global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid_constant__ CUtensorMap tmap, PtcArgs a) {
+// PRE: the ensemble was split once into fp16 hi / lo planes laid out so that a TMA box IS a K-major operand tile
+// (presplit_kernel below): the producer loads A_hi / A_lo straight into the operand stages and the converter
+// warps have nothing to do -- the projection has no window weight inside its contraction, so the conversion
+// need not be repeated for each of the ~15 windows and 2-4 column blocks that read a pixel.
+struct PtcMaps { CUtensorMap m[2]; };    // !PRE: m[0] = fp32 cube.  PRE: hi plane, lo plane
+
+template <bool MAG, bool PRE>
+__global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid_constant__ PtcMaps maps, PtcArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
     const int NSTG = a.nstg;                                                  // stages in use (raw and operand alike): 8 or 4
     const uint32_t SMSK = (uint32_t)NSTG - 1u, SSH = NSTG == 8 ? 3u : 2u;
     unsigned char* bsm = sbase;                                               // resident B block: Kp / 8 chunks of 4 KB
-    unsigned char* raw = sbase + (size_t)(a.Kp / 8) * PTC_B_LBO;              // [NSTG][8 KB]
-    unsigned char* ops = raw + NSTG * PTC_RAW_BYTES;                          // [NSTG][A_hi 4 KB | A_lo 4 KB]
+    unsigned char* raw = sbase + (size_t)(a.Kp / 8) * PTC_B_LBO;              // [NSTG][8 KB]   (none with PRE)
+    unsigned char* ops = raw + (PRE ? 0 : NSTG * PTC_RAW_BYTES);              // [NSTG][A_hi 4 KB | A_lo 4 KB]
     PtcBars* bars = reinterpret_cast<PtcBars*>(ops + NSTG * PTC_OP_BYTES);
     double* gzs = reinterpret_cast<double*>(bars + 1);                        // [Nz] window table rows (epilogue only)
     double* gxs = gzs + a.Nz;                                                 // [Nx]
@@ -120,7 +127,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
 
     if (tid == 0) {
         for (int s = 0; s < PTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], PTC_CONV_WARPS / PTC_CONV_GROUPS); }
-        for (int s = 0; s < PTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], PTC_CONV_WARPS / PTC_CONV_GROUPS); mbar_init(&bars->opempty[s], 1); }
+        for (int s = 0; s < PTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], PRE ? 1 : PTC_CONV_WARPS / PTC_CONV_GROUPS); mbar_init(&bars->opempty[s], 1); }
         for (int b = 0; b < 2; ++b) { mbar_init(&bars->accfull[b], 1); mbar_init(&bars->accempty[b], PTC_EPI_WARPS); }
         mbar_init(&bars->bfull, 1);
         mbar_init(&bars->bfree, 1);
@@ -134,7 +141,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
 
     if (warp == 0) {
         // =========================== producer ===========================
-        if (lane == 0) tma_prefetch_desc(&tmap);
+        if (lane == 0) { tma_prefetch_desc(&maps.m[0]); if (PRE) tma_prefetch_desc(&maps.m[1]); }
         uint32_t it = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
             const PtcSeg seg = a.segs[sg];
@@ -152,10 +159,19 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                 const int z = ze + tzi * PTC_TZ, x = bx.x0 + txi * PTC_TX;
                 for (int st = 0; st < nst; ++st, ++it) {
                     const int s = (it & SMSK);
-                    mbar_wait(&bars->empty[s], ((it >> SSH) & 1) ^ 1);
-                    if (lane == 0) {
-                        mbar_arrive_expect_tx(&bars->full[s], PTC_RAW_BYTES);
-                        tma_load_3d(raw + (size_t)s * PTC_RAW_BYTES, &tmap, 2 * z, x, st * PTC_KC, &bars->full[s]);
+                    if (PRE) {                             // operand tiles straight from the pre-split planes
+                        mbar_wait(&bars->opempty[s], ((it >> SSH) & 1) ^ 1);
+                        if (lane == 0) {
+                            mbar_arrive_expect_tx(&bars->opfull[s], PTC_OP_BYTES);
+                            tma_load_3d(ops + (size_t)s * PTC_OP_BYTES, &maps.m[0], 16 * z, x, 2 * st, &bars->opfull[s]);
+                            tma_load_3d(ops + (size_t)s * PTC_OP_BYTES + PTC_A_BYTES, &maps.m[1], 16 * z, x, 2 * st, &bars->opfull[s]);
+                        }
+                    } else {
+                        mbar_wait(&bars->empty[s], ((it >> SSH) & 1) ^ 1);
+                        if (lane == 0) {
+                            mbar_arrive_expect_tx(&bars->full[s], PTC_RAW_BYTES);
+                            tma_load_3d(raw + (size_t)s * PTC_RAW_BYTES, &maps.m[0], 2 * z, x, st * PTC_KC, &bars->full[s]);
+                        }
                     }
                 }
             }
@@ -193,7 +209,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
             if (elect_one()) mma_commit(&bars->bfree);     // every MMA that reads this B block has completed
             __syncwarp();
         }
-    } else if (warp >= PTC_FIRST_CONV && warp < PTC_FIRST_EPI) {
+    } else if (!PRE && warp >= PTC_FIRST_CONV && warp < PTC_FIRST_EPI) {
         // =========================== converters ===========================
         const int cw = warp - PTC_FIRST_CONV;
         const uint32_t raw_u32 = smem_u32(raw), ops_u32 = smem_u32(ops);
@@ -386,6 +402,34 @@ __global__ void proj_tc_pack_rank_kernel(const float2* B, const int* order, int 
     out[r] = lo ? make_uint4(l[0], l[1], l[2], l[3]) : make_uint4(h[0], h[1], h[2], h[3]);
 }
 
+// S -> fp16 hi / lo planes, scaled by the power of two of absmax_kernel, in the layout
+//   [t8 = frame / 8][x][z][re, im][frame % 8]      (32 bytes per pixel and 8-frame chunk)
+// so that the TMA box {16 z x 16 halves, 4 x, 2 chunks} lands in shared memory as the K-major A operand
+// [chunk][row m = (x, z, re/im)][8 frames] of project_tc_kernel.  Frames >= N are zero.
+__global__ void __launch_bounds__(256) presplit_kernel(const float2* iq, int N, int T8, long long P, const uint32_t* amax, uint4* sh, uint4* sl) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;        // (t8, pixel)
+    if (e >= (long long)T8 * P) return;
+    const long long pix = e % P;
+    const int t8 = (int)(e / P);
+    const float scale = pow2f(pow2_scale_exp(*amax));
+    float re[8], im[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int t = 8 * t8 + i;
+        float2 v = make_float2(0.f, 0.f);
+        if (t < N) v = iq[(size_t)t * P + pix];
+        re[i] = v.x * scale; im[i] = v.y * scale;
+    }
+    uint32_t h[8], l[8];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        f16_split2(re[2 * i], re[2 * i + 1], h[i], l[i]);
+        f16_split2(im[2 * i], im[2 * i + 1], h[4 + i], l[4 + i]);
+    }
+    sh[2 * e] = make_uint4(h[0], h[1], h[2], h[3]); sh[2 * e + 1] = make_uint4(h[4], h[5], h[6], h[7]);
+    sl[2 * e] = make_uint4(l[0], l[1], l[2], l[3]); sl[2 * e + 1] = make_uint4(l[4], l[5], l[6], l[7]);
+}
+
 // bits of max(|re|, |im|) over the ensemble (non-negative floats order like their bit patterns)
 __global__ void absmax_kernel(const float4* x, size_t n4, const float* tail, int ntail, uint32_t* out) {
     float m = 0.f;
@@ -465,6 +509,35 @@ static const CUtensorMap* ptc_encode_map(lcf_plan* p, const void* iq) {
     return reinterpret_cast<const CUtensorMap*>(slot);
 }
 
+// fp16 planes [T8][Nx][Nz * 16 halves]; box = {256 halves (16 z), 4 x, 2 chunks}, no swizzle
+static bool ptc_encode_premaps(lcf_plan* p) {
+    if (p->ptc_premaps_ready) return true;
+    PtcEncodeFn fn = ptc_encode_fn();
+    if (!fn || !p->ptc_sh_d || !p->ptc_sl_d) return false;
+    void* planes[2] = {p->ptc_sh_d, p->ptc_sl_d};
+    for (int i = 0; i < 2; ++i) {
+        cuuint64_t dims[3] = {(cuuint64_t)p->Nz * 16, (cuuint64_t)p->Nx, (cuuint64_t)(p->ptc_Kp / 8)};
+        cuuint64_t strides[2] = {(cuuint64_t)p->Nz * 32, (cuuint64_t)p->P * 32};
+        cuuint32_t box[3] = {16 * PTC_TZ, PTC_TX, 2};
+        cuuint32_t es[3] = {1, 1, 1};
+        CUresult r = fn(reinterpret_cast<CUtensorMap*>(p->ptc_premaps) + i, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, planes[i], dims, strides, box, es,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return false;
+    }
+    p->ptc_premaps_ready = true;
+    return true;
+}
+
+// the ensemble's fp16 hi / lo planes for the PRE variant (after absmax, before the projection)
+cudaError_t launch_presplit(lcf_plan* p, const float2* iq, cudaStream_t st) {
+    if (!p->ptc_pre) return cudaSuccess;
+    const long long n = (long long)(p->ptc_Kp / 8) * p->P;
+    presplit_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(iq, p->N, p->ptc_Kp / 8, p->P, p->amax_d, reinterpret_cast<uint4*>(p->ptc_sh_d),
+                                                                  reinterpret_cast<uint4*>(p->ptc_sl_d));
+    return cudaGetLastError();
+}
+
 bool project_tc_eligible(const lcf_plan* p) {
     return p->N <= 256 && p->N >= PTC_KC && (p->Nz % 2) == 0 && p->Nz >= PTC_TZ && p->Nx >= PTC_TX && ptc_encode_fn() != nullptr;
 }
@@ -500,13 +573,28 @@ cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::ve
     }
     cta_first[grid] = (int)segs.size();
     p->ptc_nseg = (int)segs.size();
-    p->ptc_nstg = p->ptc_Kp <= 128 ? PTC_RAW_STAGES : 4;
-    p->ptc_smem = 1024 + (size_t)(p->ptc_Kp / 8) * PTC_B_LBO + (size_t)p->ptc_nstg * (PTC_RAW_BYTES + PTC_OP_BYTES) + sizeof(PtcBars) + 16 +
+    p->ptc_pre = true;                                   // pre-split planes: no raw stages, always 8 operand stages
+    p->ptc_nstg = (p->ptc_pre || p->ptc_Kp <= 128) ? PTC_RAW_STAGES : 4;
+    p->ptc_smem = 1024 + (size_t)(p->ptc_Kp / 8) * PTC_B_LBO + (size_t)p->ptc_nstg * ((p->ptc_pre ? 0 : PTC_RAW_BYTES) + PTC_OP_BYTES) + sizeof(PtcBars) + 16 +
                   (size_t)(p->Nz + p->Nx) * sizeof(double) + 64 * sizeof(float);
     if (p->ptc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
-    cudaError_t e = set_max_dyn_smem(project_tc_kernel<false>, p->smem_optin);
-    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<true>, p->smem_optin);
+    cudaError_t e = set_max_dyn_smem(project_tc_kernel<false, false>, p->smem_optin);
+    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<true, false>, p->smem_optin);
+    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<false, true>, p->smem_optin);
+    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<true, true>, p->smem_optin);
     return e;
+}
+
+static bool ptc_fill_maps(lcf_plan* p, const void* iq, PtcMaps& maps) {
+    if (p->ptc_pre) {
+        if (!ptc_encode_premaps(p)) return false;
+        memcpy(&maps, p->ptc_premaps, sizeof(maps));
+        return true;
+    }
+    const CUtensorMap* tmap = ptc_encode_map(p, iq);
+    if (!tmap) return false;
+    maps.m[0] = *tmap; maps.m[1] = *tmap;
+    return true;
 }
 
 static void ptc_fill_args(lcf_plan* p, PtcArgs& a) {
@@ -518,14 +606,15 @@ static void ptc_fill_args(lcf_plan* p, PtcArgs& a) {
 
 cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     if (p->ptc_nseg == 0 || p->n_pitems == 0) return cudaSuccess;
-    const CUtensorMap* tmap = ptc_encode_map(p, iq);
-    if (!tmap) return cudaErrorInvalidValue;
+    PtcMaps maps;
+    if (!ptc_fill_maps(p, iq, maps)) return cudaErrorInvalidValue;
     proj_tc_pack_kernel<<<p->K * p->ptc_NB * (p->ptc_Kp / 8), 256, 0, st>>>(p->B_d, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     PtcArgs a;
     ptc_fill_args(p, a);
-    project_tc_kernel<false><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(*tmap, a);
+    if (p->ptc_pre) project_tc_kernel<false, true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
+    else project_tc_kernel<false, false><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     proj_tc_finish_kernel<<<p->n_pitems, PROJ_TPIX, 0, st>>>(p->ptc_part_d, p->sumPk, p->ptc_NB, p->box_d, p->pitems_d, p->tiles_d, p->tsum_d);
@@ -536,15 +625,16 @@ cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
 // order, through the same tcgen05 pipeline (B_d must hold V, i.e. all eigen-weights 1).
 cudaError_t launch_project_tc_mag(lcf_plan* p, const float2* iq, cudaStream_t st) {
     if (p->ptc_nseg == 0 || p->n_pitems == 0) return cudaSuccess;
-    const CUtensorMap* tmap = ptc_encode_map(p, iq);
-    if (!tmap) return cudaErrorInvalidValue;
+    PtcMaps maps;
+    if (!ptc_fill_maps(p, iq, maps)) return cudaErrorInvalidValue;
     proj_tc_pack_rank_kernel<<<p->K * p->ptc_NB * (p->ptc_Kp / 8), 256, 0, st>>>(p->B_d, p->order_d, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     PtcArgs a;
     ptc_fill_args(p, a);
     a.mag = p->ncc_mag_d; a.magN = p->ncc_magN; a.isig = p->ncc_isig_d;
-    project_tc_kernel<true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(*tmap, a);
+    if (p->ptc_pre) project_tc_kernel<true, true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
+    else project_tc_kernel<true, false><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
     return cudaGetLastError();
 }
 
