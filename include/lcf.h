@@ -119,6 +119,15 @@ lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, const lcf_wind
  * converged: that is reported by lcf_get_converged, by every getter, and by the host entry points. */
 lcf_status lcf_filter(lcf_plan* plan, const void* iq_dev, float* pd_dev, cudaStream_t stream);
 
+/* Sliding-window form of lcf_filter (packets in a sliding temporal window).  The caller promises
+ * that frames [0, N - stride) of this ensemble are frames [stride, N) of the ensemble of the previous
+ * lcf_filter_stream call on this plan: the covariance entries of those frames are taken from the previous
+ * call (shifted; rescaled by the exact power of two between the two data scales) and only the columns of the
+ * `stride` new frames are computed.  The first call, a call after lcf_filter, and stride = 0 or N compute
+ * everything.  Everything after the Gram is lcf_filter's.  Needs the tensor-core Gram path (precision 0,
+ * 32 <= N <= 128, even Nz): LCF_ERR_UNSUPPORTED otherwise.  Workspace is allocated on first use.  Asynchronous. */
+lcf_status lcf_filter_stream(lcf_plan* plan, const void* iq_dev, float* pd_dev, int stride, cudaStream_t stream);
+
 /* `count` device-resident ensembles, pipelined on two lanes: a twin of the plan (same parameters, its own
  * workspace, created on first use -- it doubles the plan's device memory) takes every other ensemble on a
  * second internal stream, so the kernels of consecutive ensembles overlap (what the latency-bound EVD of

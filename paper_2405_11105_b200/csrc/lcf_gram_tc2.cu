@@ -457,4 +457,105 @@ cudaError_t launch_gram_tc2(lcf_plan* p, const float2* iq, cudaStream_t st) {
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Sliding-window reuse (packets in a sliding temporal window), N <= 128.
+// If ensemble e+1 is ensemble e advanced by `s` frames, R_{e+1}[i][j] = R_e[i+s][j+s] for i, j < N - s: only the
+// columns of the s new frames are computed -- one block job per window, rows [0,128) x columns [c0, Np),
+// c0 = 16 floor((N - s) / 16), with the block-form kernel above -- and the rest is the previous R shifted (and
+// rescaled by the exact power of two between the two ensembles' data scales).  R stays in the data scale of the
+// tensor-core path (the Cholesky / cluster EVD kernels undo it).
+__global__ void gram_stream_assemble_kernel(const float* part, const int* seg_first, int N, int s, int c0, const float2* Rprev,
+                                            const uint32_t* amax_prev, const uint32_t* amax, float2* R) {
+    const int k = blockIdx.z;
+    const int i = blockIdx.y * 16 + threadIdx.y, j = blockIdx.x * 16 + threadIdx.x;
+    if (i >= N || j >= N) return;
+    const int a = i <= j ? i : j, b = i <= j ? j : i;          // the upper-triangle entry (a, b)
+    float re, im;
+    if (b < N - s) {
+        const float2 v = Rprev[((size_t)k * N + (a + s)) * N + (b + s)];
+        const float f = sm100::pow2f(2 * (sm100::pow2_scale_exp(*amax) - sm100::pow2_scale_exp(*amax_prev)));
+        re = v.x * f; im = v.y * f;
+    } else {
+        double sr = 0.0, si = 0.0;
+        for (int sg = seg_first[k]; sg < seg_first[k + 1]; ++sg) {
+            const float* p = part + (size_t)sg * 2 * 128 * 128 + (size_t)a * 128 + (b - c0);
+            sr += (double)p[0];
+            si += (double)p[16384];
+        }
+        re = (float)sr; im = (float)si;
+    }
+    if (i == j) im = 0.f;
+    if (i > j) im = -im;
+    R[((size_t)k * N + i) * N + j] = make_float2(re, im);
+}
+
+bool gram_stream_eligible(const lcf_plan* p) { return p->gram_tc && p->N <= 128 && p->N >= 32 && g2_encode_fn() != nullptr; }
+
+// one job per window, equal tile counts per CTA (the block is the same for every window)
+cudaError_t configure_gram_stream(lcf_plan* p, std::vector<G2Seg>& segs, std::vector<int>& cta_first, std::vector<int>& seg_first) {
+    const int K = p->K, N = p->N, Np = (N + 15) / 16 * 16;
+    std::vector<long long> pre(K + 1, 0);
+    for (int k = 0; k < K; ++k) {
+        const WinBox& b = p->box_h[k];
+        pre[k + 1] = pre[k] + (b.Pk > 0 ? (long long)((b.z0 + b.Lz - (b.z0 & ~1) + G2_PX - 1) / G2_PX) * b.Lx : 0);
+    }
+    const long long T = pre[K];
+    int grid = (int)(T < p->num_sms ? T : p->num_sms);
+    if (grid < 1) grid = 1;
+    p->g2_grid = grid;
+    segs.clear();
+    cta_first.assign(grid + 1, 0);
+    seg_first.assign(K + 1, 0);
+    std::vector<int> cta_of;
+    int k = 0;
+    for (int c = 0; c < grid; ++c) {
+        long long g0 = T * c / grid, g1 = T * (c + 1) / grid;
+        while (g0 < g1) {
+            while (k < K && pre[k + 1] <= g0) ++k;
+            const long long e = pre[k + 1] < g1 ? pre[k + 1] : g1;
+            segs.push_back({k, 0, (int)(g0 - pre[k]), (int)(e - g0), c});
+            g0 = e;
+        }
+    }
+    int si = 0;
+    for (int c = 0; c < grid; ++c) { cta_first[c] = si; while (si < (int)segs.size() && segs[si].cta == c) ++si; }
+    cta_first[grid] = (int)segs.size();
+    si = 0;
+    for (int kk = 0; kk < K; ++kk) { seg_first[kk] = si; while (si < (int)segs.size() && segs[si].k == kk) ++si; }
+    seg_first[K] = si;
+    p->g2_nseg = (int)segs.size();
+    const int nbox = (N + 7) / 8 * 8;
+    for (int b = 0; b < 3; ++b) p->g2_blk[b] = {0, 0, Np, 0, nbox};
+    p->g2_raw_stride = (uint32_t)(((size_t)nbox * 128 + 1023) / 1024 * 1024);
+    p->g2_mat_bytes = (uint32_t)(2 * Np * 16);
+    p->g2_smem = 1024 + (size_t)G2_STAGES * p->g2_raw_stride + (size_t)(4 * G2_STAGES + 1) * p->g2_mat_bytes + sizeof(G2Bars) + 16 +
+                 (size_t)(p->Nz + p->Nx) * sizeof(double);
+    if (p->g2_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
+    return set_max_dyn_smem(gram_tc2_kernel, p->smem_optin);
+}
+
+// R_d <- Gram of the ensemble at iq, given that the previous call's ensemble (whose R is in Rprev_d) was this one
+// shifted back by `stride` frames
+cudaError_t launch_gram_stream(lcf_plan* p, const float2* iq, int stride, cudaStream_t st) {
+    const int N = p->N, Np = (N + 15) / 16 * 16;
+    const G2Maps* maps = g2_encode_maps(p, iq);
+    if (!maps) return cudaErrorInvalidValue;
+    const int c0 = (N - stride) / 16 * 16;
+    G2Args a;
+    a.N = N; a.Np = Np; a.Nz = p->Nz; a.Nx = p->Nx;
+    a.group = p->gtc_group;
+    a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->g2_segs_d; a.cta_first = p->g2_cta_first_d;
+    a.part = p->g2_part_d; a.raw_stride = p->g2_raw_stride; a.mat_bytes = p->g2_mat_bytes; a.amax = p->amax_d;
+    for (int b = 0; b < 3; ++b) a.blk[b] = {0, c0, Np - c0, 0, p->g2_blk[0].nbox};
+    if (p->g2_nseg > 0) {
+        gram_tc2_kernel<<<p->g2_grid, G2_THREADS, p->g2_smem, st>>>(*maps, a);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    dim3 blk(16, 16), grid((N + 15) / 16, (N + 15) / 16, p->K);
+    gram_stream_assemble_kernel<<<grid, blk, 0, st>>>(p->g2_part_d, p->g2_seg_first_d, N, stride, c0, p->Rprev_d, p->amax_prev_d, p->amax_d,
+                                                       reinterpret_cast<float2*>(p->R_d));
+    return cudaGetLastError();
+}
+
 }  // namespace lcf

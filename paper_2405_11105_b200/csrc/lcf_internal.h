@@ -156,6 +156,10 @@ struct lcf_plan {
     int *g2_cta_first_d = nullptr, *g2_seg_first_d = nullptr;
     float* g2_part_d = nullptr;             // [nseg][2][128][128]
     lcf::TmapCache3 g2_tmaps;
+    // sliding-window reuse (lcf_filter_stream, N <= 128): the block-form kernel computes the new frames' columns only
+    bool strm_ready = false, strm_valid = false;
+    float2* Rprev_d = nullptr;              // [K][N][N] R of the previous lcf_filter_stream call (data scale of that call)
+    uint32_t* amax_prev_d = nullptr;
     // Cholesky + one-sided Jacobi EVD (precision 0, N <= 128): lcf_evd_chol.cu
     bool evd_chol = false, evd_cluster = false;   // cluster: Cholesky kernel, then one-sided Jacobi on 2-CTA clusters
     int ec_LD = 0;
@@ -259,6 +263,9 @@ cudaError_t launch_gram_tc(lcf_plan* p, const float2* iq, cudaStream_t st);
 bool gram_tc2_eligible(const lcf_plan* p);
 cudaError_t configure_gram_tc2(lcf_plan* p, std::vector<G2Seg>& segs, std::vector<int>& cta_first, std::vector<int>& seg_first);
 cudaError_t launch_gram_tc2(lcf_plan* p, const float2* iq, cudaStream_t st);
+bool gram_stream_eligible(const lcf_plan* p);
+cudaError_t configure_gram_stream(lcf_plan* p, std::vector<G2Seg>& segs, std::vector<int>& cta_first, std::vector<int>& seg_first);
+cudaError_t launch_gram_stream(lcf_plan* p, const float2* iq, int stride, cudaStream_t st);
 bool evd_chol_eligible(const lcf_plan* p);
 cudaError_t configure_evd_chol(lcf_plan* p);
 cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only);

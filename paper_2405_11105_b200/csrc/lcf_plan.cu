@@ -70,7 +70,7 @@ void free_plan_device(lcf_plan* p) {
     cudaFree(p->ec_gfac_d); cudaFree(p->ec_shift_d);
     cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d); cudaFree(p->amax_d);
     cudaFree(p->gtc_segs_d); cudaFree(p->gtc_cta_first_d); cudaFree(p->gtc_seg_first_d); cudaFree(p->gtc_part_d);
-    cudaFree(p->ptc_sh_d); cudaFree(p->ptc_sl_d);
+    cudaFree(p->ptc_sh_d); cudaFree(p->ptc_sl_d); cudaFree(p->Rprev_d); cudaFree(p->amax_prev_d);
     cudaFree(p->ncc_mag_d); cudaFree(p->ncc_isig_d); cudaFree(p->ncc_part_d); cudaFree(p->ncc_curve_d);
     cudaFree(p->g2_segs_d); cudaFree(p->g2_cta_first_d); cudaFree(p->g2_seg_first_d); cudaFree(p->g2_part_d);
     if (p->timer.have)
@@ -361,7 +361,8 @@ extern "C" lcf_status lcf_plan_destroy(lcf_plan* p) {
     return LCF_OK;
 }
 
-extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev, cudaStream_t stream) {
+// stride > 0: the Gram comes from the previous call's R and the new frames' columns (lcf_filter_stream)
+static lcf_status filter_impl(lcf_plan* p, const void* iq_dev, float* pd_dev, cudaStream_t stream, int stride) {
     if (!p || !iq_dev || !pd_dev) return LCF_ERR_INVALID_ARG;
     if (p->cuda_failed) return LCF_ERR_CUDA;
     cudaStream_t st = stream;
@@ -375,7 +376,14 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     mark(0);
     if (e == cudaSuccess && (p->gram_tc || p->gram_tc2 || p->proj_tc)) run(1, launch_absmax(p, iq, st));
     if (e == cudaSuccess && p->proj_tc) run(1, launch_presplit(p, iq, st));
-    if (e == cudaSuccess) run(1, p->gram_tc ? launch_gram_tc(p, iq, st) : (p->gram_tc2 ? launch_gram_tc2(p, iq, st) : launch_gram(p, iq, st)));
+    if (e == cudaSuccess) {
+        if (stride > 0) run(1, launch_gram_stream(p, iq, stride, st));
+        else run(1, p->gram_tc ? launch_gram_tc(p, iq, st) : (p->gram_tc2 ? launch_gram_tc2(p, iq, st) : launch_gram(p, iq, st)));
+    }
+    if (e == cudaSuccess && stride >= 0 && p->strm_ready) {       // keep R and its data scale for the next streamed call
+        run(1, cudaMemcpyAsync(p->Rprev_d, p->R_d, (size_t)p->K * p->N * p->N * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+        if (e == cudaSuccess) run(1, cudaMemcpyAsync(p->amax_prev_d, p->amax_d, sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
+    }
     mark(1);
     if (e == cudaSuccess) run(2, p->evd_chol ? launch_evd_chol(p, st, p->evd_cluster) : launch_jacobi(p, st));
     if (e == cudaSuccess && p->evd_cluster) run(2, launch_evd_cluster(p, st));
@@ -396,6 +404,31 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
     p->ran = true;
     if (e != cudaSuccess) { p->cuda_failed = true; return LCF_ERR_CUDA; }
     return LCF_OK;
+}
+
+extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev, cudaStream_t stream) {
+    if (p) p->strm_valid = false;                       // a plain call breaks the chain of streamed ensembles
+    return filter_impl(p, iq_dev, pd_dev, stream, -1);
+}
+
+extern "C" lcf_status lcf_filter_stream(lcf_plan* p, const void* iq_dev, float* pd_dev, int stride, cudaStream_t stream) {
+    if (!p || !iq_dev || !pd_dev || stride < 0 || stride > p->N) return LCF_ERR_INVALID_ARG;
+    if (!gram_stream_eligible(p)) return LCF_ERR_UNSUPPORTED;
+    if (!p->strm_ready) {                               // first use: segments, partials, the kept R
+        std::vector<G2Seg> segs;
+        std::vector<int> cta_first, seg_first;
+        if (configure_gram_stream(p, segs, cta_first, seg_first) != cudaSuccess) { cudaGetLastError(); return LCF_ERR_UNSUPPORTED; }
+        bool ok = dev_upload(&p->g2_segs_d, segs) && dev_upload(&p->g2_cta_first_d, cta_first) && dev_upload(&p->g2_seg_first_d, seg_first) &&
+                  dev_alloc(&p->g2_part_d, (size_t)(p->g2_nseg ? p->g2_nseg : 1) * 2 * 128 * 128) &&
+                  dev_alloc(&p->Rprev_d, (size_t)p->K * p->N * p->N) && dev_alloc(&p->amax_prev_d, 1);
+        if (!ok) { cudaGetLastError(); return LCF_ERR_ALLOC; }
+        p->strm_ready = true;
+    }
+    // stride = 0 or no previous streamed call: the whole Gram; otherwise only the new frames' columns
+    const bool reuse = p->strm_valid && stride > 0 && stride < p->N;
+    lcf_status s = filter_impl(p, iq_dev, pd_dev, stream, reuse ? stride : 0);
+    p->strm_valid = (s == LCF_OK);
+    return s;
 }
 
 extern "C" lcf_status lcf_filter_batch(lcf_plan* p, const void* const* iq_devs, float* const* pd_devs, int count, cudaStream_t stream) {

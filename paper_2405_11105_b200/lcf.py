@@ -18,7 +18,7 @@ HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_NOT_CONVERGED = range(6)
 
 EXPORTS = [
-    "lcf_plan_create", "lcf_filter", "lcf_filter_batch", "lcf_filter_host", "lcf_filter_host_batch", "lcf_plan_destroy", "lcf_num_windows",
+    "lcf_plan_create", "lcf_filter", "lcf_filter_batch", "lcf_filter_stream", "lcf_filter_host", "lcf_filter_host_batch", "lcf_plan_destroy", "lcf_num_windows",
     "lcf_get_eigenvalues", "lcf_get_cutoffs", "lcf_get_sweeps", "lcf_get_gram", "lcf_get_eigenvectors",
     "lcf_get_weights", "lcf_get_filters", "lcf_get_window_means", "lcf_set_timing", "lcf_get_stage_ms",
     "lcf_get_work", "lcf_measure_peak", "lcf_status_string", "lcf_last_error", "lcf_scale_exponent",
@@ -64,6 +64,7 @@ def load() -> C.CDLL:
         L.lcf_filter.argtypes = [vp, vp, vp, vp]
         L.lcf_filter_host.argtypes = [vp, vp, vp, vp]
         L.lcf_filter_host_batch.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp]
+        L.lcf_filter_stream.argtypes = [vp, vp, vp, C.c_int, vp]
         L.lcf_filter_batch.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp]
         L.lcf_plan_destroy.argtypes = [vp]
         L.lcf_num_windows.argtypes = [vp]
@@ -196,6 +197,14 @@ class Plan:
         st = load().lcf_filter(self._h, _ptr(iq_dev), _ptr(pd_dev), _stream(stream))
         if st != OK:
             raise LcfError(st, "lcf_filter [" + load().lcf_last_error(self._h).decode() + "]")
+
+    def filter_stream(self, iq_dev, pd_dev, stride: int, stream=None):
+        """Sliding-window call: this ensemble is the previous streamed one advanced by `stride` frames. Asynchronous."""
+        self._check(iq_dev, "iq_dev", self.N * self.Nx * self.Nz, ("complex64", "float32"), True)
+        self._check(pd_dev, "pd_dev", self.Nx * self.Nz, ("float32",), True)
+        st = load().lcf_filter_stream(self._h, _ptr(iq_dev), _ptr(pd_dev), int(stride), _stream(stream))
+        if st != OK:
+            raise LcfError(st, "lcf_filter_stream [" + load().lcf_last_error(self._h).decode() + "]")
 
     def filter_batch(self, iq_devs, pd_devs, stream=None):
         """Lists of device tensors: consecutive ensembles overlap on the plan's two lanes. Asynchronous."""

@@ -452,6 +452,47 @@ def test_filter_batch_two_lanes_matches_single_calls(lcf):
         plan.filter_batch([], [])
 
 
+@pytest.mark.parametrize("N,stride,Nz,Nx", [(100, 50, 96, 64), (64, 5, 64, 48), (128, 16, 64, 48), (48, 40, 64, 48)])
+def test_sliding_window_stream_reuses_the_gram(lcf, oracle, N, stride, Nz, Nx):
+    """lcf_filter_stream (sliding packets): ensemble e+1 = ensemble e advanced by `stride` frames; only the
+    new frames' Gram columns are computed.  Every streamed ensemble must agree with an independent lcf_filter of
+    the same frames (Gram 1e-5, eigenvalues, cut-offs, image) and the last one with the oracle."""
+    import torch
+    cfg = synth.baseline_configs()[4]
+    nfr = N + 4 * stride
+    d = replace(cfg.data, Nz=Nz, Nx=Nx, N=N, n_frames=nfr, seed=500 + N, n_vessels=3, drift_px=1.0)
+    f = synth.FilterSpec(2, 2, 14.0, 12.0, 3.0, synth.SOFT_ENERGY, precision=0)
+    seq = synth.generate_sequence(d)
+    seq_d = torch.from_numpy(seq).cuda()
+    a = torch.empty((Nx, Nz), dtype=torch.float32, device="cuda")
+    b = torch.empty_like(a)
+    with lcf.Plan.from_spec(Nz, Nx, N, f) as ps, lcf.Plan.from_spec(Nz, Nx, N, f) as pi:
+        for e in range(5):
+            view = seq_d[e * stride:e * stride + N]
+            ps.filter_stream(view, a, stride)
+            pi.filter(view, b)
+            torch.cuda.synchronize()
+            Rs, Ri = ps.gram(), pi.gram()
+            scale = np.abs(Ri).max(axis=(1, 2), keepdims=True)
+            assert (np.abs(Rs - Ri) / scale).max() <= 1e-5, (e, (np.abs(Rs - Ri) / scale).max())
+            ls, li = ps.eigenvalues(), pi.eigenvalues()
+            assert (np.abs(ls - li) / li[:, :1]).max() <= LAM_TOL
+            assert np.array_equal(ps.cutoffs(), pi.cutoffs())
+            check_pd(a.cpu().numpy().astype(np.float64), b.cpu().numpy().astype(np.float64))
+        o = oracle.run_config(np.ascontiguousarray(seq[4 * stride:4 * stride + N]), f)
+        check_pd(a.cpu().numpy().astype(np.float64), o["PD"])
+        # a plain lcf_filter in between breaks the chain: the next streamed call recomputes everything, same result
+        ps.filter(seq_d[:N], b)
+        ps.filter_stream(seq_d[4 * stride:4 * stride + N], b, stride)
+        torch.cuda.synchronize()
+        check_pd(b.cpu().numpy().astype(np.float64), o["PD"])
+    # not on the tensor-core Gram path -> refused, not silently recomputed
+    with lcf.Plan.from_spec(Nz, Nx, N, replace(f, precision=1)) as p1:
+        with pytest.raises(lcf.LcfError) as ei:
+            p1.filter_stream(seq_d[:N], a, stride)
+        assert ei.value.status == lcf.ERR_UNSUPPORTED
+
+
 def test_plans_of_different_sizes_alive_together(lcf, oracle):
     """The opt-in shared-memory limit is a per-kernel, process-wide attribute: creating (and destroying) a
     smaller plan must not break a larger plan that already exists (every kernel family: tensor / cluster
