@@ -117,6 +117,33 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
     }
     __syncthreads();
 
+    // fp32 only: bring the matrix to a fixed magnitude (largest diagonal entry in [1, 2)) by an exact power of
+    // two, so that the squares in the rotation and convergence tests neither underflow nor overflow whatever
+    // the units of the data (R ~ amplitude^2 P); the eigenvalues are unscaled in double at the end
+    int lam_exp = 0;
+    if (sizeof(T) == 4) {
+        T mx = T(0);
+        for (int u = tid; u < Ns; u += nthr) mx = fmaxf((float)mx, fabsf((float)d[u]));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = fmaxf((float)mx, __shfl_xor_sync(0xffffffffu, (float)mx, o));
+        __syncthreads();
+        if ((tid & 31) == 0) red[tid >> 5] = mx;
+        __syncthreads();
+        float m = 0.f;
+        for (int w = 0; w < (nthr + 31) >> 5; ++w) m = fmaxf(m, (float)red[w]);
+        if (m > 0.f && m < 3.0e38f) {
+            int ex;
+            frexpf(m, &ex);                                   // m = f 2^ex, f in [0.5, 1)
+            lam_exp = 1 - ex;                                 // m 2^lam_exp in [1, 2)
+            const T sc = (T)ldexpf(1.f, lam_exp < -120 ? -120 : (lam_exp > 120 ? 120 : lam_exp));
+            lam_exp = lam_exp < -120 ? -120 : (lam_exp > 120 ? 120 : lam_exp);
+            for (int e = tid; e < npk; e += nthr) { C x = S[e]; x.x *= sc; x.y *= sc; S[e] = x; }
+            for (int u = tid; u < Ns; u += nthr) d[u] *= sc;
+        }
+        __syncthreads();
+    }
+    const double lam_un = ldexp(1.0, -lam_exp);
+
     T fro2;
     {
         T acc = T(0);
@@ -251,8 +278,8 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
     }
     __syncthreads();  // all reads of d/S done before lsort overwrites S
     if (tid < N) {
-        lsort[rank] = (double)myl;
-        a.lam[(size_t)k * N + rank] = (double)myl;
+        lsort[rank] = (double)myl * lam_un;
+        a.lam[(size_t)k * N + rank] = (double)myl * lam_un;
         a.order[(size_t)k * N + rank] = tid;
     }
     __syncthreads();
@@ -272,7 +299,7 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
         double w = 0.0;
         if (tid < N) {
             const int i1 = rank + 1;  // 1-based order of the eigenvalue held by index tid
-            w = thresh_is_adaptive(a.mode) ? thresh_adaptive_raw((double)myl, lsort[0], i1, N, a.beta) / wnorm_sh
+            w = thresh_is_adaptive(a.mode) ? thresh_adaptive_raw((double)myl * lam_un, lsort[0], i1, N, a.beta) / wnorm_sh
                                              : thresh_weight(soft, a.beta, i1, c);
             a.wt[(size_t)k * N + rank] = w;
         }

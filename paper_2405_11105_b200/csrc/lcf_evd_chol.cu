@@ -55,6 +55,7 @@ struct EcArgs {
     int chol_only;                // 1: stop after the Cholesky factor and write it to gfac / shift (cluster Jacobi follows)
     float* gfac;                  // [K][2][Ns][LD] real plane, imaginary plane of G, column-major
     float* shift;                 // [K] delta, or -1 for an all-zero matrix
+    int* nexp;                    // [K] power-of-two exponent this kernel scaled R_k by (0 when R carries the tensor-core data scale)
 };
 
 __device__ __forceinline__ void ec_pair_pq(int m, int s, int M, int& p, int& q) {
@@ -128,6 +129,23 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     __syncthreads();
     float maxdiag = 0.f;
     for (int w = 0; w < EC_THREADS / 32; ++w) maxdiag = fmaxf(maxdiag, red[w]);
+    // R from the CUDA-core Gram is in raw units (amplitude^2 P): bring it to a fixed magnitude (largest diagonal entry
+    // in [1, 2)) by an exact power of two, so that the squared norms and their products in the Cholesky and Jacobi
+    // tests stay in range whatever the units; undone when the eigenvalues leave (the tensor-core Gram's R already
+    // has a fixed scale)
+    int nexp = 0;
+    if (!a.amax && maxdiag > 0.f && maxdiag < 3.0e38f) {
+        int ex;
+        frexpf(maxdiag, &ex);
+        nexp = 1 - ex;
+        nexp = nexp < -120 ? -120 : (nexp > 120 ? 120 : nexp);
+        const float sc = ldexpf(1.f, nexp);
+        __syncthreads();
+        for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) Gr[e] *= sc;
+        maxdiag *= sc;
+        __syncthreads();
+    }
+    if (tid == 0) a.nexp[k] = nexp;
     const float delta = 3e-5f * maxdiag;
     int sweep = 0, converged = 1;
 
@@ -356,7 +374,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     }
     __syncthreads();
     // rank (descending, ties by slot index), cut-off, eigen-weights: same rules as jacobi_kernel
-    const double un = a.amax ? ldexp(1.0, -2 * sm100::pow2_scale_exp(*a.amax)) : 1.0;
+    const double un = a.amax ? ldexp(1.0, -2 * sm100::pow2_scale_exp(*a.amax)) : ldexp(1.0, -nexp);
     float myl = 0.f;
     int rank = 0;
     if (tid < N) {
@@ -429,7 +447,7 @@ cudaError_t configure_evd_chol(lcf_plan* p) {
 
 cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only) {
     EcArgs a;
-    a.chol_only = chol_only ? 1 : 0; a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d;
+    a.chol_only = chol_only ? 1 : 0; a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d; a.nexp = p->ec_nexp_d;
     a.N = p->N; a.NP = p->NP; a.Ns = p->Ns; a.LD = p->ec_LD; a.max_sweeps = p->sweep_cap > 0 ? p->sweep_cap : 30;
     a.R = reinterpret_cast<const float2*>(p->R_d); a.amax = p->gram_tc ? p->amax_d : nullptr;
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d; a.nunconv = p->nunconv_d;

@@ -33,6 +33,7 @@ struct EclArgs {
     int max_sweeps;
     const float* gfac;                         // [K][2][N][LDg]
     const float* shift;                        // [K]
+    const int* nexp;                           // [K] power-of-two exponent the Cholesky kernel scaled R_k by
     const uint32_t* amax;                      // non-null: the factors carry the data scale of the tensor-core Gram
     double* lam; int* order; int* cut; int* sweeps; int* conv;
     int* nunconv;                              // [1] count of window EVDs that hit the sweep cap
@@ -174,7 +175,7 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
     }
     ecl_cluster_sync();
     // ---- rank (descending, ties by slot), cut-off, eigen-weights: both CTAs compute, CTA 0 writes
-    const double un = a.amax ? ldexp(1.0, -2 * sm100::pow2_scale_exp(*a.amax)) : 1.0;   // eigenvalues leave unscaled
+    const double un = a.amax ? ldexp(1.0, -2 * sm100::pow2_scale_exp(*a.amax)) : ldexp(1.0, -a.nexp[k]);   // eigenvalues leave unscaled
     float myl = 0.f;
     int rnk = 0;
     if (tid < N) {
@@ -942,7 +943,7 @@ cudaError_t configure_evd_cluster(lcf_plan* p) {
 cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st) {
     EclArgs a;
     a.N = p->N; a.n = p->N / 2; a.h = (a.n + 1) / 2; a.LD = p->ec_LD; a.LDg = p->ec_LD; a.max_sweeps = p->sweep_cap > 0 ? p->sweep_cap : 30;
-    a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d; a.amax = p->gram_tc ? p->amax_d : nullptr;
+    a.gfac = p->ec_gfac_d; a.shift = p->ec_shift_d; a.nexp = p->ec_nexp_d; a.amax = p->gram_tc ? p->amax_d : nullptr;
     a.lam = p->lam_d; a.order = p->order_d; a.cut = p->cut_d; a.sweeps = p->sweeps_d; a.conv = p->conv_d; a.nunconv = p->nunconv_d;
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;

@@ -166,6 +166,7 @@ struct lcf_plan {
     size_t ec_smem = 0, ecl_smem = 0;
     float* ec_gfac_d = nullptr;             // [K][2][Ns][LD] Cholesky factor planes
     float* ec_shift_d = nullptr;            // [K]
+    int* ec_nexp_d = nullptr;               // [K]
     // tensor-core projection (N <= 128): lcf_project_tc.cu
     bool proj_tc = false;
     int ptc_grid = 0, ptc_nseg = 0, ptc_NB = 0, ptc_Kp = 0, ptc_nstg = 0;

@@ -67,7 +67,7 @@ void free_plan_device(lcf_plan* p) {
     for (int i = 0; i < 2; ++i) { if (p->lane_st[i]) cudaStreamDestroy(p->lane_st[i]); if (p->ev_join[i]) cudaEventDestroy(p->ev_join[i]); }
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     for (int i = 0; i < 2; ++i) { if (p->ev_copied[i]) cudaEventDestroy(p->ev_copied[i]); if (p->ev_done[i]) cudaEventDestroy(p->ev_done[i]); }
-    cudaFree(p->ec_gfac_d); cudaFree(p->ec_shift_d);
+    cudaFree(p->ec_gfac_d); cudaFree(p->ec_shift_d); cudaFree(p->ec_nexp_d);
     cudaFree(p->ptc_segs_d); cudaFree(p->ptc_cta_first_d); cudaFree(p->ptc_bpack_d); cudaFree(p->ptc_part_d); cudaFree(p->amax_d);
     cudaFree(p->gtc_segs_d); cudaFree(p->gtc_cta_first_d); cudaFree(p->gtc_seg_first_d); cudaFree(p->gtc_part_d);
     cudaFree(p->ptc_sh_d); cudaFree(p->ptc_sl_d); cudaFree(p->Rprev_d); cudaFree(p->amax_prev_d);
@@ -307,6 +307,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
              dev_alloc(&p->g2_part_d, (size_t)(p->g2_nseg ? p->g2_nseg : 1) * 2 * 128 * 128);
     }
     if (p->evd_cluster) ok = ok && dev_alloc(&p->ec_gfac_d, K * 2 * Ns * (size_t)p->ec_LD) && dev_alloc(&p->ec_shift_d, K);
+    if (p->evd_chol) ok = ok && dev_alloc(&p->ec_nexp_d, K);
     if (p->proj_tc) {
         ok = ok && dev_upload(&p->ptc_segs_d, ptc_segs) && dev_upload(&p->ptc_cta_first_d, ptc_cta_first) &&
              dev_alloc(&p->ptc_bpack_d, K * p->ptc_NB * (size_t)(p->ptc_Kp / 8) * 1024) &&

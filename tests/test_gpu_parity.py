@@ -331,6 +331,25 @@ def test_tensor_path_data_scale(lcf, oracle):
         check_pd(g["PD"], o["PD"])
 
 
+@pytest.mark.parametrize("Nz,Nx,N", [(45, 40, 64), (45, 40, 24), (32, 32, 140)])
+def test_fallback_paths_data_scale(lcf, oracle, Nz, Nx, N):
+    """The FP32 CUDA-core Gram leaves R in raw units (amplitude^2 P): the EVD kernels behind it (cluster Jacobi after the
+    Cholesky kernel, single-CTA Cholesky + Jacobi, two-sided Jacobi above 128 frames) normalise it by a power of two,
+    so tiny and huge amplitudes give the same cut-offs, the eigenvalues up to the scale, and the same image."""
+    cfg = synth.baseline_configs()[2]
+    d = replace(cfg.data, Nz=Nz, Nx=Nx, N=N, n_frames=N, seed=700 + N, n_vessels=3, tissue_db=40.0, noise_db=-55.0)
+    f = synth.FilterSpec(2, 2, 10.0, 10.0, 3.0, synth.SOFT_ENERGY, precision=0)
+    iq = synth.generate_sequence(d)
+    with lcf.Plan.from_spec(Nz, Nx, N, f) as plan:
+        assert plan.work()["gram_tc"] == (1 if N > 128 else 0)
+    o = oracle.run_config(iq, f)
+    for c in (1.0, 2.3e-11, 4.1e8):
+        g = gpu_run(lcf, (iq * np.complex64(c)).astype(np.complex64), f)
+        assert np.array_equal(g["c"], o["c"]), (c, g["c"], o["c"])
+        assert (np.abs(g["lam"] / (c * c) - o["lam"]) / o["lam"][:, :1]).max() <= LAM_TOL, c
+        check_pd(g["PD"], o["PD"])
+
+
 def test_empty_window_support(lcf):
     # sigma so small that no pixel lies within trunc*sigma of the half-integer centres: P_k = 0
     iq = synth.random_cube(8, 8, 6, seed=2)
