@@ -7,7 +7,7 @@ A step = one pass of the whole hot path (Gram -> EVD -> weights -> projection ->
 section 8a) over one synthetic ensemble of BASELINE.json config 2 (256x256x128, 8x8 windows,
 sigma 24, 3-sigma boxes, soft energy-rule weights), through the C ABI.
 
-  value     K ensembles through one `lcf_filter_batch` call (the plan's two lanes overlap the kernels of
+  value     K ensembles through one `lcf_filter_batch` call (the plan's three lanes overlap the kernels of
             consecutive ensembles), inputs resident in HBM: a ring of 4 distinct ensembles (268 MB > the
             126 MB L2), CUDA events on the caller's stream, max over ranks.
   latency   single `lcf_filter` calls with the L2 flushed between them; the per-kernel stage times of
@@ -288,7 +288,7 @@ def run_ours(args, cfg):
     ring = [iq_h.cuda()] + [torch.from_numpy(ens(i)).cuda() for i in range(1, RING)]
     iq_d = ring[0]
     pd_d = torch.empty((d.Nx, d.Nz), dtype=torch.float32, device="cuda")
-    pd_ring = [pd_d, torch.empty_like(pd_d)]
+    pd_ring = [pd_d, torch.empty_like(pd_d), torch.empty_like(pd_d)]      # one image buffer per lane
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2, for the latency loop
     stream = torch.cuda.current_stream()
     plan = lcf.Plan.from_spec(d.Nz, d.Nx, d.N, cfg.filt)
@@ -299,10 +299,10 @@ def run_ours(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- throughput (`value`): K steps = one lcf_filter_batch call over the ring (two lanes inside the plan:
+    # ---- throughput (`value`): K steps = one lcf_filter_batch call over the ring (three lanes inside the plan:
     # the kernels of consecutive ensembles overlap), CUDA events on the caller's stream around it
     def batch(n):
-        plan.filter_batch([ring[i % RING] for i in range(n)], [pd_ring[i & 1] for i in range(n)], stream)
+        plan.filter_batch([ring[i % RING] for i in range(n)], [pd_ring[i % 3] for i in range(n)], stream)
     if args.warmup > 0:
         batch(max(args.warmup, 4))
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -427,7 +427,7 @@ def run_ours(args, cfg):
     roofline = dict(per_kernel[dom]) if dom else {"bound": "alu", "achieved": None, "peak": fp32_peak, "unit": "TFLOP/s", "frac": None}
     roofline.update({
         "traffic": None, "kernel_ms": roofline.get("ms"), "stages_ms": stages, "per_kernel": per_kernel,
-        "stage_times_from": "single lcf_filter calls with the L2 flushed (kernels timed alone; in the two-lane throughput loop they overlap)",
+        "stage_times_from": "single lcf_filter calls with the L2 flushed (kernels timed alone; in the three-lane throughput loop they overlap)",
         "live_pipe_peaks_tflops": live,
         "evd_sweeps": {"mean": float(sweeps.mean()), "max": int(sweeps.max())},
         "hbm": {"algorithmic_bytes": work["hbm_bytes"], "peak_gbs": peaks.get("hbm_gbs"),
@@ -466,13 +466,13 @@ def run_ours(args, cfg):
                 lat = np.array([a4.elapsed_time(b4) for a4, b4 in evs])
                 tot = evs[0][0].elapsed_time(evs[-1][1])
                 # sustained rate through the two-lane batch entry point (3 passes over the 16 ensembles)
-                pd4b = [pd4, torch.empty_like(pd4)]
+                pd4b = [pd4, torch.empty_like(pd4), torch.empty_like(pd4)]
                 n4 = 3 * len(views)
-                plan4.filter_batch(views[:4], [pd4b[i & 1] for i in range(4)], stream)
+                plan4.filter_batch(views[:4], [pd4b[i % 3] for i in range(4)], stream)
                 torch.cuda.synchronize()
                 s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 s0.record(stream)
-                plan4.filter_batch([views[i % len(views)] for i in range(n4)], [pd4b[i & 1] for i in range(n4)], stream)
+                plan4.filter_batch([views[i % len(views)] for i in range(n4)], [pd4b[i % 3] for i in range(n4)], stream)
                 s1.record(stream)
                 torch.cuda.synchronize()
                 tot_b = s0.elapsed_time(s1)
@@ -492,7 +492,7 @@ def run_ours(args, cfg):
                 assert plan4.unconverged() == 0
             streaming = {"workload": workload_name(cfg4) + f", {cfg4.n_ensembles} ensembles at stride {cfg4.stride} of a "
                          f"resident {d4.n_frames}-frame sequence, 3 passes, L2 not flushed (472 MB sequence > L2)",
-                         "pd_frames_per_s": n4 / (tot_b * 1e-3), "how": "lcf_filter_batch (two lanes), CUDA events around the call",
+                         "pd_frames_per_s": n4 / (tot_b * 1e-3), "how": "lcf_filter_batch (three lanes), CUDA events around the call",
                          "pd_frames_per_s_single_lane": len(evs) / (tot * 1e-3),
                          "latency_ms": {"median": float(np.median(lat)), "p95": float(np.percentile(lat, 95))},
                          "sliding_window_reuse": {"api": "lcf_filter_stream(stride=50): Gram columns of the new frames only, the rest shifted from the previous call",
@@ -594,7 +594,7 @@ def run_ours(args, cfg):
         "config": {"workload": workload_name(cfg),
                    "l2": f"ring of {RING} distinct resident ensembles ({RING * iq_h.numel() * 8 / 1e6:.0f} MB) > 126 MB L2, no flush needed",
                    "parallelism": f"ensemble-sharded x{world}, no collective",
-                   "timing": "CUDA events on the caller's stream around one lcf_filter_batch call of K ensembles (two lanes inside the plan)"},
+                   "timing": "CUDA events on the caller's stream around one lcf_filter_batch call of K ensembles (three lanes inside the plan)"},
         "latency_ms": {"median": float(np.median(step_ms)), "min": float(np.min(step_ms)),
                        "p95": float(np.percentile(step_ms, 95)), "calls": nlat,
                        "how": "single lcf_filter calls, CUDA events per call, 512 MiB buffer overwritten between calls (L2 flushed)"},

@@ -128,14 +128,14 @@ lcf_status lcf_filter(lcf_plan* plan, const void* iq_dev, float* pd_dev, cudaStr
  * 32 <= N <= 128, even Nz): LCF_ERR_UNSUPPORTED otherwise.  Workspace is allocated on first use.  Asynchronous. */
 lcf_status lcf_filter_stream(lcf_plan* plan, const void* iq_dev, float* pd_dev, int stride, cudaStream_t stream);
 
-/* `count` device-resident ensembles, pipelined on two lanes: a twin of the plan (same parameters, its own
- * workspace, created on first use -- it doubles the plan's device memory) takes every other ensemble on a
- * second internal stream, so the kernels of consecutive ensembles overlap (what the latency-bound EVD of
- * one leaves idle, the contractions of the next use).  iq_devs / pd_devs: HOST arrays of `count` DEVICE
- * pointers (distinct pd buffers).  Asynchronous and stream-ordered like lcf_filter: the lanes start
- * after the work already enqueued on `stream`, and `stream` continues after both lanes are done.
- * Results are bit-identical to `count` lcf_filter calls.  The getters afterwards describe the last
- * even-indexed ensemble; lcf_get_converged counts both lanes. */
+/* `count` device-resident ensembles, pipelined on three lanes: two twins of the plan (same parameters, their own
+ * workspace, created on first use -- they triple the plan's device memory) take the ensembles in turn on internal
+ * streams, so the kernels of consecutive ensembles overlap (what the latency-bound EVD of one leaves idle, the
+ * contractions of the next use).  iq_devs / pd_devs: HOST arrays of `count` DEVICE pointers; any three consecutive
+ * ensembles are in flight together and need distinct pd buffers.  Asynchronous and stream-ordered like
+ * lcf_filter: the lanes start after the work already enqueued on `stream`, and `stream` continues after all lanes
+ * are done.  Results are bit-identical to `count` lcf_filter calls.  The getters afterwards describe the last
+ * ensemble of lane 0 (index a multiple of 3); lcf_get_converged counts all lanes. */
 lcf_status lcf_filter_batch(lcf_plan* plan, const void* const* iq_devs, float* const* pd_devs, int count, cudaStream_t stream);
 
 /* Same path with HOST buffers (pinned or pageable): copies iq_host -> plan-owned device staging,
@@ -145,7 +145,7 @@ lcf_status lcf_filter_batch(lcf_plan* plan, const void* const* iq_devs, float* c
 lcf_status lcf_filter_host(lcf_plan* plan, const void* iq_host, float* pd_host, cudaStream_t stream);
 
 /* `count` ensembles from HOST buffers, pipelined: the host->device copy of ensemble i+1 (on a
- * plan-owned copy stream, two staging buffers) overlaps the kernels of ensemble i, which run on the two
+ * plan-owned copy stream, two staging buffers) overlaps the kernels of ensemble i, which run on two of the
  * lanes of lcf_filter_batch; each image is copied back as soon as it is done.  `stream` is synchronised
  * at entry.  iq_hosts / pd_hosts: HOST arrays of `count` HOST
  * pointers (pinned memory for the copies to be asynchronous).  Returns after everything has

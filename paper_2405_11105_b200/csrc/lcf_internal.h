@@ -217,11 +217,11 @@ struct lcf_plan {
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
 
-    // two-lane pipelining of lcf_filter_batch / lcf_filter_host_batch: a twin plan (same parameters, its own
-    // workspace) and one internal stream per lane, created on first use
-    lcf_plan* twin = nullptr;
-    cudaStream_t lane_st[2] = {nullptr, nullptr};
-    cudaEvent_t ev_fork = nullptr, ev_join[2] = {nullptr, nullptr};
+    // lane pipelining of lcf_filter_batch (three lanes) / lcf_filter_host_batch (two): twin plans (same parameters,
+    // their own workspace) and one internal stream per lane, created on first use
+    lcf_plan* twin = nullptr;               // chain: plan -> twin -> twin's twin (lane 0, 1, 2)
+    cudaStream_t lane_st[3] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
 
     cudaStream_t last_stream = nullptr;
     bool ran = false;
