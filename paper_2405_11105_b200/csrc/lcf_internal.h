@@ -169,7 +169,7 @@ struct lcf_plan {
     int* ec_nexp_d = nullptr;               // [K]
     // tensor-core projection (N <= 128): lcf_project_tc.cu
     bool proj_tc = false;
-    int ptc_grid = 0, ptc_nseg = 0, ptc_NB = 0, ptc_Kp = 0, ptc_nstg = 0;
+    int ptc_grid = 0, ptc_nseg = 0, ptc_NB = 0, ptc_Kp = 0, ptc_nstg = 0, ptc_G = 1;
     size_t ptc_smem = 0;
     lcf::PtcSeg* ptc_segs_d = nullptr;
     int* ptc_cta_first_d = nullptr;

@@ -355,6 +355,215 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
     if (warp == 1) tmem_dealloc<512>(tmem);
 }
 
+// ------------------------------------------------------------------------------------------------
+// project_tc2_kernel: the pre-split projection with up to TWO 64-column blocks of B resident, both fed by the same
+// A tiles.  project_tc_kernel re-reads every pixel once per (window, column block): 2.1 GB of L2 traffic per
+// ensemble at config 2 (5 TB/s, ~60 % of what a plain read loop gets from L2 on this part) next to a
+// shared-memory port that is already the bound.  Here a segment is a (window, block group) and per 16 frames
+//   D_j[:, 0:128] += A_hi Bh_j^T       D_j += A_hi Bl_j^T       D_j += A_lo Bh_j^T          (j = 0, 1: three N = 128 MMAs each)
+// with Bh_j / Bl_j the hi / lo halves (rows 0-127 / 128-255) of block j's resident tile: the lo products accumulate
+// into the hi product's columns, so a block needs 128 TMEM columns instead of 256 and two blocks are double-buffered
+// in the 512.  D_j[:, 0:64] = X . Re B, D_j[:, 64:128] = X . Im B.  Eight epilogue warps: two per TMEM lane quadrant,
+// one per block.  Groups hold one block when two do not fit in shared memory next to the stages (N > 152).
+constexpr int PT2_STAGES = 8;
+constexpr int PT2_EPI0 = 8;                                    // warps 8-15: epilogue; 0: producer; 1: MMA issuer
+struct Pt2Bars {
+    uint64_t opfull[PT2_STAGES], opempty[PT2_STAGES];
+    uint64_t accfull[2], accempty[2];
+    uint64_t bfull, bfree;
+    uint32_t tmem_base;
+};
+
+template <bool MAG>
+__global__ void __launch_bounds__(PTC_THREADS, 1) project_tc2_kernel(const __grid_constant__ PtcMaps maps, PtcArgs a, int G) {
+    extern __shared__ __align__(1024) unsigned char smem_dyn[];
+    unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
+    const uint32_t bbytes = (uint32_t)(a.Kp / 8) * PTC_B_LBO;                 // one resident B block
+    unsigned char* bsm = sbase;                                               // [G][bbytes]
+    unsigned char* ops = sbase + (size_t)G * bbytes;                          // [STAGES][A_hi 4 KB | A_lo 4 KB]
+    Pt2Bars* bars = reinterpret_cast<Pt2Bars*>(ops + PT2_STAGES * PTC_OP_BYTES);
+    double* gzs = reinterpret_cast<double*>(bars + 1);
+    double* gxs = gzs + a.Nz;
+    float* isig_s = reinterpret_cast<float*>(gxs + a.Nx);                     // [2][64] (MAG)
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int seg0 = a.cta_first[blockIdx.x], seg1 = a.cta_first[blockIdx.x + 1];
+    const int nst = (a.Kp + PTC_KC - 1) / PTC_KC;
+
+    if (tid == 0) {
+        for (int s = 0; s < PT2_STAGES; ++s) { mbar_init(&bars->opfull[s], 1); mbar_init(&bars->opempty[s], 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(&bars->accfull[b], 1); mbar_init(&bars->accempty[b], 8); }
+        mbar_init(&bars->bfull, 1);
+        mbar_init(&bars->bfree, 1);
+        mbar_fence_init();
+    }
+    if (warp == 1) tmem_alloc<512>(&bars->tmem_base);
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
+    const uint32_t tmem = bars->tmem_base;
+
+    if (warp == 0) {
+        // =========================== producer ===========================
+        if (lane == 0) { tma_prefetch_desc(&maps.m[0]); tma_prefetch_desc(&maps.m[1]); }
+        uint32_t it = 0;
+        for (int sg = seg0; sg < seg1; ++sg) {
+            const PtcSeg seg = a.segs[sg];                 // seg.b = block group
+            const WinBox bx = a.box[seg.k];
+            const int nb = a.NB - seg.b * G < G ? a.NB - seg.b * G : G;
+            const int ze = bx.z0 & ~1;
+            const int ntz = (bx.z0 + bx.Lz - ze + PTC_TZ - 1) / PTC_TZ;
+            if (sg > seg0) mbar_wait(&bars->bfree, (uint32_t)(sg - seg0 - 1) & 1);
+            if (lane == 0) {
+                mbar_arrive_expect_tx(&bars->bfull, bbytes * (uint32_t)nb);
+                for (int j = 0; j < nb; ++j)
+                    bulk_load(bsm + (size_t)j * bbytes, a.bpack + ((size_t)seg.k * a.NB + seg.b * G + j) * (size_t)(a.Kp / 8) * 1024, bbytes, &bars->bfull);
+            }
+            for (int t = 0; t < seg.ntile; ++t) {
+                const int tau = seg.tile0 + t;
+                const int txi = tau / ntz, tzi = tau - txi * ntz;
+                const int z = ze + tzi * PTC_TZ, x = bx.x0 + txi * PTC_TX;
+                for (int st = 0; st < nst; ++st, ++it) {
+                    const int s = it % PT2_STAGES;
+                    mbar_wait(&bars->opempty[s], ((it / PT2_STAGES) & 1) ^ 1);
+                    if (lane == 0) {
+                        mbar_arrive_expect_tx(&bars->opfull[s], PTC_OP_BYTES);
+                        tma_load_3d(ops + (size_t)s * PTC_OP_BYTES, &maps.m[0], 16 * z, x, 2 * st, &bars->opfull[s]);
+                        tma_load_3d(ops + (size_t)s * PTC_OP_BYTES + PTC_A_BYTES, &maps.m[1], 16 * z, x, 2 * st, &bars->opfull[s]);
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // =========================== MMA issuer ===========================
+        const uint32_t idesc = make_idesc_f16(PTC_ROWS, 128, false, false);
+        const uint64_t descA0 = make_smem_desc(smem_u32(ops), PTC_A_LBO, PTC_SBO, SWZ_NONE);
+        const uint64_t descB0 = make_smem_desc(smem_u32(bsm), PTC_B_LBO, PTC_SBO, SWZ_NONE);
+        uint32_t it = 0, tl = 0;
+        for (int sg = seg0; sg < seg1; ++sg) {
+            const PtcSeg seg = a.segs[sg];
+            const int nb = a.NB - seg.b * G < G ? a.NB - seg.b * G : G;
+            mbar_wait(&bars->bfull, (uint32_t)(sg - seg0) & 1);
+            for (int t = 0; t < seg.ntile; ++t, ++tl) {
+                const uint32_t buf = tl & 1;
+                mbar_wait(&bars->accempty[buf], ((tl >> 1) & 1) ^ 1);
+                for (int st = 0; st < nst; ++st, ++it) {
+                    const int o = it % PT2_STAGES;
+                    mbar_wait(&bars->opfull[o], (it / PT2_STAGES) & 1);
+                    tc_fence_after_sync();
+                    if (elect_one()) {
+                        const uint64_t dAh = descA0 + (uint64_t)((o * PTC_OP_BYTES) >> 4);
+                        const uint64_t dAl = dAh + (uint64_t)(PTC_A_BYTES >> 4);
+                        for (int j = 0; j < nb; ++j) {
+                            const uint32_t tD = tmem + buf * 256 + (uint32_t)j * 128;
+                            const uint64_t dBh = descB0 + (uint64_t)((j * bbytes + st * 2 * PTC_B_LBO) >> 4);
+                            const uint64_t dBl = dBh + (uint64_t)((128 * 16) >> 4);
+                            mma_f16(tD, dAh, dBh, idesc, st == 0 ? 0u : 1u);
+                            mma_f16(tD, dAh, dBl, idesc, 1u);
+                            mma_f16(tD, dAl, dBh, idesc, 1u);
+                        }
+                        mma_commit(&bars->opempty[o]);
+                        if (st + 1 == nst) mma_commit(&bars->accfull[buf]);
+                    }
+                    __syncwarp();
+                }
+            }
+            if (elect_one()) mma_commit(&bars->bfree);
+            __syncwarp();
+        }
+    } else if (warp >= PT2_EPI0) {
+        // =========================== epilogue: warp (quadrant, block j of the group) ===========================
+        const int quad = warp & 3, jb = (warp - PT2_EPI0) >> 2;
+        const uint32_t tlane = tmem + ((uint32_t)(quad * 32) << 16);
+        const int m = quad * 32 + lane;
+        const int pix = m >> 1, xi = pix >> 4, zi = pix & 15;
+        const float unscale = pow2f(-8 - pow2_scale_exp(*a.amax));
+        uint32_t tl = 0;
+        int curk = -1;
+        for (int sg = seg0; sg < seg1; ++sg) {
+            const PtcSeg seg = a.segs[sg];
+            const WinBox bx = a.box[seg.k];
+            const int nb = a.NB - seg.b * G < G ? a.NB - seg.b * G : G;
+            const bool mine = jb < nb;
+            const int blk = seg.b * G + jb;
+            const int ze = bx.z0 & ~1;
+            const int ntz = (bx.z0 + bx.Lz - ze + PTC_TZ - 1) / PTC_TZ;
+            if (seg.k != curk || MAG) {
+                asm volatile("bar.sync 1, 256;" ::: "memory");
+                const int et = tid - PT2_EPI0 * 32;
+                if (seg.k != curk) {
+                    for (int i = et; i < a.Nz; i += 256) gzs[i] = a.gz[(size_t)bx.kz * a.Nz + i];
+                    for (int i = et; i < a.Nx; i += 256) gxs[i] = a.gx[(size_t)bx.kx * a.Nx + i];
+                }
+                if (MAG && et < 128) isig_s[et] = (et >> 6) < nb ? a.isig[((size_t)seg.k * a.NB + seg.b * G + (et >> 6)) * 64 + (et & 63)] : 0.f;
+                asm volatile("bar.sync 1, 256;" ::: "memory");
+                curk = seg.k;
+            }
+            float* out = a.part + (size_t)(mine ? blk : 0) * a.sumPk + bx.tile_off;
+            for (int t = 0; t < seg.ntile; ++t, ++tl) {
+                const uint32_t buf = tl & 1;
+                const int tau = seg.tile0 + t;
+                const int txi = tau / ntz, tzi = tau - txi * ntz;
+                const int zz = ze + tzi * PTC_TZ + zi, xx = bx.x0 + txi * PTC_TX + xi;
+                mbar_wait(&bars->accfull[buf], (tl >> 1) & 1);
+                tc_fence_after_sync();
+                const bool valid = mine && zz >= bx.z0 && zz < bx.z0 + bx.Lz && xx < bx.x0 + bx.Lx;
+                float acc = 0.f, wpix = 0.f;
+                float* mrow = nullptr;
+                if (MAG && valid) {
+                    wpix = (float)(gzs[zz] * gxs[xx]);
+                    mrow = a.mag + ((size_t)bx.tile_off + (size_t)(xx - bx.x0) * bx.Lz + (zz - bx.z0)) * a.magN + blk * PTC_UB;
+                }
+                if (mine) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        uint32_t va[16], vb[16];
+                        const uint32_t col = buf * 256 + (uint32_t)jb * 128 + j * 16;
+                        tmem_ld16(tlane + col, va);
+                        tmem_ld16(tlane + col + 64, vb);
+                        tmem_ld_wait();
+                        float mg[16];
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) {
+                            const float pr = __uint_as_float(va[i]), pi = __uint_as_float(vb[i]);
+                            const float po = __shfl_xor_sync(0xffffffffu, pi, 1);
+                            const float val = ((lane & 1) ? pr + po : pr - po) * unscale;   // odd row: Im U, even row: Re U
+                            if (MAG) {
+                                const float v2 = val * val;
+                                mg[i] = sqrtf(v2 + __shfl_xor_sync(0xffffffffu, v2, 1)) * isig_s[jb * 64 + j * 16 + i] * wpix;
+                            } else {
+                                acc = fmaf(val, val, acc);
+                            }
+                        }
+                        if (MAG && valid) {
+                            const bool odd = (lane & 1) != 0;
+                            float s8[8];
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) s8[i] = odd ? mg[8 + i] : mg[i];
+                            float4* o4 = reinterpret_cast<float4*>(mrow + j * 16 + (odd ? 8 : 0));
+                            o4[0] = make_float4(s8[0], s8[1], s8[2], s8[3]);
+                            o4[1] = make_float4(s8[4], s8[5], s8[6], s8[7]);
+                        }
+                    }
+                }
+                tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bars->accempty[buf]);
+                if (!MAG && mine) {
+                    acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+                    if (!(lane & 1) && valid) {
+                        const double w = gzs[zz] * gxs[xx];
+                        out[(size_t)(xx - bx.x0) * bx.Lz + (zz - bx.z0)] = (float)(w * w) * acc;
+                    }
+                }
+            }
+        }
+    }
+    tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc<512>(tmem);
+}
+
 // B_k [N][Ns] complex (row = frame, column = eigen slot) -> per (window, 64-column block) the
 // resident fp16 operand tile [Kp/8 chunks][256 rows][8 frames]: rows = Re hi | Im hi | Re lo | Im lo of 256 B
 __global__ void proj_tc_pack_kernel(const float2* B, int N, int Ns, int Kp, int NB, float* bpack) {
@@ -548,38 +757,66 @@ cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::ve
     p->ptc_NB = (p->Ns + PTC_UB - 1) / PTC_UB;
     p->ptc_Kp = (p->N + 15) / 16 * 16;
     const int NB = p->ptc_NB;
-    std::vector<long long> pre((size_t)K * NB + 1, 0);
+    // block groups of the two-block kernel: two resident B blocks when they fit next to the stages
+    const size_t bbytes = (size_t)(p->ptc_Kp / 8) * PTC_B_LBO;
+    auto smem2 = [&](int G) {
+        return (size_t)1024 + G * bbytes + (size_t)PT2_STAGES * PTC_OP_BYTES + sizeof(Pt2Bars) + 16 + (size_t)(p->Nz + p->Nx) * sizeof(double) +
+               128 * sizeof(float);
+    };
+    int G = (NB >= 2 && smem2(2) <= (size_t)p->smem_optin) ? 2 : 1;
+    if (smem2(G) > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
+    p->ptc_pre = true;
+    p->ptc_G = G;
+    p->ptc_nstg = PT2_STAGES;
+    // one block per group (N > 152): project_tc_kernel's wide form (one N = 256 and one N = 128 MMA per 16 frames) reads
+    // fewer operand bytes per flop than three N = 128 MMAs (measured at config 3: 4.0 against 4.95 ms)
+    p->ptc_smem = G == 2 ? smem2(2)
+                         : 1024 + bbytes + (size_t)p->ptc_nstg * PTC_OP_BYTES + sizeof(PtcBars) + 16 + (size_t)(p->Nz + p->Nx) * sizeof(double) + 64 * sizeof(float);
+    if (p->ptc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
+    const int NG = (NB + G - 1) / G;
+    // jobs = (window, block group, tile); a tile of a group costs as many units as the group has blocks
+    std::vector<long long> pre((size_t)K * NG + 1, 0), ntile((size_t)K, 0);
+    std::vector<int> wg((size_t)NG);
+    for (int g = 0; g < NG; ++g) wg[g] = NB - g * G < G ? NB - g * G : G;
     for (int k = 0; k < K; ++k) {
         const WinBox& b = p->box_h[k];
-        const long long nt = b.Pk > 0 ? (long long)((b.z0 + b.Lz - (b.z0 & ~1) + PTC_TZ - 1) / PTC_TZ) * ((b.Lx + PTC_TX - 1) / PTC_TX) : 0;
-        for (int j = 0; j < NB; ++j) pre[(size_t)k * NB + j + 1] = pre[(size_t)k * NB + j] + nt;
+        ntile[k] = b.Pk > 0 ? (long long)((b.z0 + b.Lz - (b.z0 & ~1) + PTC_TZ - 1) / PTC_TZ) * ((b.Lx + PTC_TX - 1) / PTC_TX) : 0;
+        for (int g = 0; g < NG; ++g) pre[(size_t)k * NG + g + 1] = pre[(size_t)k * NG + g] + ntile[k] * wg[g];
     }
-    const long long T = pre[(size_t)K * NB];
-    int grid = (int)(T < p->num_sms ? T : p->num_sms);
+    const long long T = pre[(size_t)K * NG];
+    long long total_tiles = 0;
+    for (int k = 0; k < K; ++k) total_tiles += ntile[k] * NG;
+    int grid = (int)(total_tiles < p->num_sms ? total_tiles : p->num_sms);
     if (grid < 1) grid = 1;
     p->ptc_grid = grid;
     segs.clear();
     cta_first.assign(grid + 1, 0);
-    size_t j = 0;
-    for (int c = 0; c < grid; ++c) {
-        cta_first[c] = (int)segs.size();
-        long long g0 = T * c / grid, g1 = T * (c + 1) / grid;
-        while (g0 < g1) {
-            while (j < (size_t)K * NB && pre[j + 1] <= g0) ++j;
-            const long long e = pre[j + 1] < g1 ? pre[j + 1] : g1;
-            segs.push_back({(int)(j / NB), (int)(j % NB), (int)(g0 - pre[j]), (int)(e - g0)});
-            g0 = e;
+    std::vector<int> cta_of;
+    for (size_t j = 0; j < (size_t)K * NG; ++j) {
+        const int k = (int)(j / NG), g = (int)(j % NG);
+        const long long nt = ntile[k], w = wg[g];
+        long long t0 = 0;
+        while (t0 < nt) {                      // tile t starts at cost pre[j] + w t: it goes to the CTA whose equal share holds that point
+            long long c = (pre[j] + w * t0) * grid / (T > 0 ? T : 1);
+            if (c > grid - 1) c = grid - 1;
+            long long t1 = nt;
+            if (c < grid - 1) {
+                const long long bound = (T * (c + 1) + grid - 1) / grid;          // first cost not in share c
+                t1 = (bound - pre[j] + w - 1) / w;
+                if (t1 <= t0) t1 = t0 + 1;
+                if (t1 > nt) t1 = nt;
+            }
+            segs.push_back({k, g, (int)t0, (int)(t1 - t0)});
+            cta_of.push_back((int)c);
+            t0 = t1;
         }
     }
+    int si = 0;
+    for (int c = 0; c < grid; ++c) { cta_first[c] = si; while (si < (int)segs.size() && cta_of[si] <= c) ++si; }
     cta_first[grid] = (int)segs.size();
     p->ptc_nseg = (int)segs.size();
-    p->ptc_pre = true;                                   // pre-split planes: no raw stages, always 8 operand stages
-    p->ptc_nstg = (p->ptc_pre || p->ptc_Kp <= 128) ? PTC_RAW_STAGES : 4;
-    p->ptc_smem = 1024 + (size_t)(p->ptc_Kp / 8) * PTC_B_LBO + (size_t)p->ptc_nstg * ((p->ptc_pre ? 0 : PTC_RAW_BYTES) + PTC_OP_BYTES) + sizeof(PtcBars) + 16 +
-                  (size_t)(p->Nz + p->Nx) * sizeof(double) + 64 * sizeof(float);
-    if (p->ptc_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
-    cudaError_t e = set_max_dyn_smem(project_tc_kernel<false, false>, p->smem_optin);
-    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<true, false>, p->smem_optin);
+    cudaError_t e = set_max_dyn_smem(project_tc2_kernel<false>, p->smem_optin);
+    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc2_kernel<true>, p->smem_optin);
     if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<false, true>, p->smem_optin);
     if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<true, true>, p->smem_optin);
     return e;
@@ -613,8 +850,8 @@ cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     PtcArgs a;
     ptc_fill_args(p, a);
-    if (p->ptc_pre) project_tc_kernel<false, true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
-    else project_tc_kernel<false, false><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
+    if (p->ptc_G == 2) project_tc2_kernel<false><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a, 2);
+    else project_tc_kernel<false, true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     proj_tc_finish_kernel<<<p->n_pitems, PROJ_TPIX, 0, st>>>(p->ptc_part_d, p->sumPk, p->ptc_NB, p->box_d, p->pitems_d, p->tiles_d, p->tsum_d);
@@ -633,8 +870,8 @@ cudaError_t launch_project_tc_mag(lcf_plan* p, const float2* iq, cudaStream_t st
     PtcArgs a;
     ptc_fill_args(p, a);
     a.mag = p->ncc_mag_d; a.magN = p->ncc_magN; a.isig = p->ncc_isig_d;
-    if (p->ptc_pre) project_tc_kernel<true, true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
-    else project_tc_kernel<true, false><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
+    if (p->ptc_G == 2) project_tc2_kernel<true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a, 2);
+    else project_tc_kernel<true, true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
     return cudaGetLastError();
 }
 
