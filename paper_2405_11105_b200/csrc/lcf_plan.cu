@@ -321,7 +321,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     if (p->evd_chol) ok = ok && dev_alloc(&p->ec_nexp_d, K);
     if (p->proj_tc) {
         ok = ok && dev_upload(&p->ptc_segs_d, ptc_segs) && dev_upload(&p->ptc_cta_first_d, ptc_cta_first) &&
-             dev_alloc(&p->ptc_bpack_d, K * p->ptc_NB * (size_t)(p->ptc_Kp / 8) * 1024) &&
+             dev_alloc(&p->ptc_bpack_d, K * (size_t)(p->ptc_NB + 1) * (size_t)(p->ptc_Kp / 8) * 1024) &&
              dev_alloc(&p->ptc_part_d, (size_t)p->ptc_NB * (size_t)(p->sumPk ? p->sumPk : 1));
     }
     if (p->gram_tc || p->gram_tc2 || p->proj_tc) ok = ok && dev_alloc(&p->amax_d, 1);

@@ -378,9 +378,9 @@ template <bool MAG>
 __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc2_kernel(const __grid_constant__ PtcMaps maps, PtcArgs a, int G) {
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
-    const uint32_t bbytes = (uint32_t)(a.Kp / 8) * PTC_B_LBO;                 // one resident B block
-    unsigned char* bsm = sbase;                                               // [G][bbytes]
-    unsigned char* ops = sbase + (size_t)G * bbytes;                          // [STAGES][A_hi 4 KB | A_lo 4 KB]
+    const uint32_t bbytes = (uint32_t)(a.Kp / 8) * 2 * PTC_B_LBO;             // the resident group tile: 512 rows per chunk
+    unsigned char* bsm = sbase;
+    unsigned char* ops = sbase + bbytes;                                      // [STAGES][A_hi 4 KB | A_lo 4 KB]
     Pt2Bars* bars = reinterpret_cast<Pt2Bars*>(ops + PT2_STAGES * PTC_OP_BYTES);
     double* gzs = reinterpret_cast<double*>(bars + 1);
     double* gxs = gzs + a.Nz;
@@ -415,9 +415,8 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc2_kernel(const __gri
             const int ntz = (bx.z0 + bx.Lz - ze + PTC_TZ - 1) / PTC_TZ;
             if (sg > seg0) mbar_wait(&bars->bfree, (uint32_t)(sg - seg0 - 1) & 1);
             if (lane == 0) {
-                mbar_arrive_expect_tx(&bars->bfull, bbytes * (uint32_t)nb);
-                for (int j = 0; j < nb; ++j)
-                    bulk_load(bsm + (size_t)j * bbytes, a.bpack + ((size_t)seg.k * a.NB + seg.b * G + j) * (size_t)(a.Kp / 8) * 1024, bbytes, &bars->bfull);
+                mbar_arrive_expect_tx(&bars->bfull, bbytes);
+                bulk_load(bsm, a.bpack + ((size_t)seg.k * ((a.NB + 1) / 2) + seg.b) * (size_t)(a.Kp / 8) * 2048, bbytes, &bars->bfull);
             }
             for (int t = 0; t < seg.ntile; ++t) {
                 const int tau = seg.tile0 + t;
@@ -436,9 +435,9 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc2_kernel(const __gri
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
-        const uint32_t idesc = make_idesc_f16(PTC_ROWS, 128, false, false);
+        const uint32_t idesc256 = make_idesc_f16(PTC_ROWS, 256, false, false), idesc128 = make_idesc_f16(PTC_ROWS, 128, false, false);
         const uint64_t descA0 = make_smem_desc(smem_u32(ops), PTC_A_LBO, PTC_SBO, SWZ_NONE);
-        const uint64_t descB0 = make_smem_desc(smem_u32(bsm), PTC_B_LBO, PTC_SBO, SWZ_NONE);
+        const uint64_t descB0 = make_smem_desc(smem_u32(bsm), 2 * PTC_B_LBO, PTC_SBO, SWZ_NONE);
         uint32_t it = 0, tl = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
             const PtcSeg seg = a.segs[sg];
@@ -454,14 +453,14 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc2_kernel(const __gri
                     if (elect_one()) {
                         const uint64_t dAh = descA0 + (uint64_t)((o * PTC_OP_BYTES) >> 4);
                         const uint64_t dAl = dAh + (uint64_t)(PTC_A_BYTES >> 4);
-                        for (int j = 0; j < nb; ++j) {
-                            const uint32_t tD = tmem + buf * 256 + (uint32_t)j * 128;
-                            const uint64_t dBh = descB0 + (uint64_t)((j * bbytes + st * 2 * PTC_B_LBO) >> 4);
-                            const uint64_t dBl = dBh + (uint64_t)((128 * 16) >> 4);
-                            mma_f16(tD, dAh, dBh, idesc, st == 0 ? 0u : 1u);
-                            mma_f16(tD, dAh, dBl, idesc, 1u);
-                            mma_f16(tD, dAl, dBh, idesc, 1u);
-                        }
+                        // both blocks at once: B rows [0,256) = hi of block 0 | hi of block 1, rows [256,512) = their lo halves
+                        const uint32_t tD = tmem + buf * 256;
+                        const uint32_t idesc = nb == 2 ? idesc256 : idesc128;
+                        const uint64_t dBh = descB0 + (uint64_t)((st * 2 * 2 * PTC_B_LBO) >> 4);
+                        const uint64_t dBl = dBh + (uint64_t)((256 * 16) >> 4);
+                        mma_f16(tD, dAh, dBh, idesc, st == 0 ? 0u : 1u);
+                        mma_f16(tD, dAh, dBl, idesc, 1u);
+                        mma_f16(tD, dAl, dBh, idesc, 1u);
                         mma_commit(&bars->opempty[o]);
                         if (st + 1 == nst) mma_commit(&bars->accfull[buf]);
                     }
@@ -566,49 +565,37 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc2_kernel(const __gri
 
 // B_k [N][Ns] complex (row = frame, column = eigen slot) -> per (window, 64-column block) the
 // resident fp16 operand tile [Kp/8 chunks][256 rows][8 frames]: rows = Re hi | Im hi | Re lo | Im lo of 256 B
-__global__ void proj_tc_pack_kernel(const float2* B, int N, int Ns, int Kp, int NB, float* bpack) {
-    const int kb = blockIdx.x / (Kp / 8), c8 = blockIdx.x - kb * (Kp / 8);   // kb = k * NB + b; one 8-frame chunk per CTA
-    const int k = kb / NB, b = kb - k * NB;
+// GROUP2: two blocks share one tile of 512 rows per chunk, [hi b0 | hi b1 | lo b0 | lo b1] (128 rows each: Re 64, Im 64), so
+// that project_tc2_kernel's MMAs take both blocks' hi (or lo) rows as one N = 256 operand.  `order` (rank -> slot)
+// non-null: columns in rank order (method 4).
+template <bool GROUP2>
+__global__ void proj_tc_pack_kernel(const float2* B, const int* order, int N, int Ns, int Kp, int NB, float* bpack) {
+    constexpr int ROWS = GROUP2 ? 512 : 256;
+    const int NJ = GROUP2 ? (NB + 1) / 2 : NB;                                // tiles per window
+    const int kb = blockIdx.x / (Kp / 8), c8 = blockIdx.x - kb * (Kp / 8);   // kb = k * NJ + tile; one 8-frame chunk per CTA
+    const int k = kb / NJ, jt = kb - k * NJ;
     const float2* Bk = B + (size_t)k * N * Ns;
-    uint4* out = reinterpret_cast<uint4*>(bpack + (size_t)kb * (Kp / 8) * 1024) + (size_t)c8 * 256;
-    const int r = threadIdx.x;                       // 256 rows: Re hi | Im hi | Re lo | Im lo
-    const int u = b * PTC_UB + (r & 63);
-    const bool im = (r >> 6) & 1, lo = r >= 128;
-    float x[8];
+    uint4* out = reinterpret_cast<uint4*>(bpack + (size_t)kb * (Kp / 8) * (ROWS * 4)) + (size_t)c8 * ROWS;
+    for (int r = threadIdx.x; r < ROWS; r += blockDim.x) {
+        int b, col;
+        bool im, lo;
+        if (GROUP2) { const int part = r >> 7; b = jt * 2 + (part & 1); lo = part >= 2; im = (r >> 6) & 1; col = r & 63; }
+        else { b = jt; lo = r >= 128; im = (r >> 6) & 1; col = r & 63; }
+        const int cidx = b * PTC_UB + col;                                    // eigen slot, or rank
+        int u = -1;
+        if (b < NB) u = order ? (cidx < N ? order[(size_t)k * N + cidx] : -1) : (cidx < Ns ? cidx : -1);
+        float x[8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const int t = 8 * c8 + i;
-        x[i] = 0.f;
-        if (t < N && u < Ns) { const float2 c = Bk[(size_t)t * Ns + u]; x[i] = (im ? c.y : c.x) * PTC_B_SCALE; }
+        for (int i = 0; i < 8; ++i) {
+            const int t = 8 * c8 + i;
+            x[i] = 0.f;
+            if (t < N && u >= 0) { const float2 c = Bk[(size_t)t * Ns + u]; x[i] = (im ? c.y : c.x) * PTC_B_SCALE; }
+        }
+        uint32_t h[4], l[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) f16_split2(x[2 * i], x[2 * i + 1], h[i], l[i]);
+        out[r] = lo ? make_uint4(l[0], l[1], l[2], l[3]) : make_uint4(h[0], h[1], h[2], h[3]);
     }
-    uint32_t h[4], l[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) f16_split2(x[2 * i], x[2 * i + 1], h[i], l[i]);
-    out[r] = lo ? make_uint4(l[0], l[1], l[2], l[3]) : make_uint4(h[0], h[1], h[2], h[3]);
-}
-
-// Same operand tile from B_k with the columns in RANK order (column b * 64 + j of the tile = the eigenvector of the
-// (b * 64 + j + 1)-th largest eigenvalue): method 4 needs the components side by side in eigenvalue order.
-__global__ void proj_tc_pack_rank_kernel(const float2* B, const int* order, int N, int Ns, int Kp, int NB, float* bpack) {
-    const int kb = blockIdx.x / (Kp / 8), c8 = blockIdx.x - kb * (Kp / 8);
-    const int k = kb / NB, b = kb - k * NB;
-    const float2* Bk = B + (size_t)k * N * Ns;
-    uint4* out = reinterpret_cast<uint4*>(bpack + (size_t)kb * (Kp / 8) * 1024) + (size_t)c8 * 256;
-    const int r = threadIdx.x;
-    const int rank = b * PTC_UB + (r & 63);
-    const int u = rank < N ? order[(size_t)k * N + rank] : -1;
-    const bool im = (r >> 6) & 1, lo = r >= 128;
-    float x[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const int t = 8 * c8 + i;
-        x[i] = 0.f;
-        if (t < N && u >= 0) { const float2 c = Bk[(size_t)t * Ns + u]; x[i] = (im ? c.y : c.x) * PTC_B_SCALE; }
-    }
-    uint32_t h[4], l[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) f16_split2(x[2 * i], x[2 * i + 1], h[i], l[i]);
-    out[r] = lo ? make_uint4(l[0], l[1], l[2], l[3]) : make_uint4(h[0], h[1], h[2], h[3]);
 }
 
 // S -> fp16 hi / lo planes, scaled by the power of two of absmax_kernel, in the layout
@@ -834,6 +821,13 @@ static bool ptc_fill_maps(lcf_plan* p, const void* iq, PtcMaps& maps) {
     return true;
 }
 
+static void ptc_launch_pack(lcf_plan* p, const int* order, cudaStream_t st) {
+    if (p->ptc_G == 2)
+        proj_tc_pack_kernel<true><<<p->K * ((p->ptc_NB + 1) / 2) * (p->ptc_Kp / 8), 256, 0, st>>>(p->B_d, order, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
+    else
+        proj_tc_pack_kernel<false><<<p->K * p->ptc_NB * (p->ptc_Kp / 8), 256, 0, st>>>(p->B_d, order, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
+}
+
 static void ptc_fill_args(lcf_plan* p, PtcArgs& a) {
     a.N = p->N; a.Kp = p->ptc_Kp; a.Nz = p->Nz; a.Nx = p->Nx;
     a.gz = p->gz_d; a.gx = p->gx_d; a.box = p->box_d; a.segs = p->ptc_segs_d; a.cta_first = p->ptc_cta_first_d;
@@ -845,7 +839,7 @@ cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     if (p->ptc_nseg == 0 || p->n_pitems == 0) return cudaSuccess;
     PtcMaps maps;
     if (!ptc_fill_maps(p, iq, maps)) return cudaErrorInvalidValue;
-    proj_tc_pack_kernel<<<p->K * p->ptc_NB * (p->ptc_Kp / 8), 256, 0, st>>>(p->B_d, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
+    ptc_launch_pack(p, nullptr, st);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     PtcArgs a;
@@ -864,7 +858,7 @@ cudaError_t launch_project_tc_mag(lcf_plan* p, const float2* iq, cudaStream_t st
     if (p->ptc_nseg == 0 || p->n_pitems == 0) return cudaSuccess;
     PtcMaps maps;
     if (!ptc_fill_maps(p, iq, maps)) return cudaErrorInvalidValue;
-    proj_tc_pack_rank_kernel<<<p->K * p->ptc_NB * (p->ptc_Kp / 8), 256, 0, st>>>(p->B_d, p->order_d, p->N, p->Ns, p->ptc_Kp, p->ptc_NB, p->ptc_bpack_d);
+    ptc_launch_pack(p, p->order_d, st);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     PtcArgs a;
