@@ -490,10 +490,13 @@ __device__ __forceinline__ int ecb_round_tracked(EcbCol& X, EcbCol& Y, EcbCol& Z
     const float nhi = fmaxf(app, aqq), nlo = fminf(app, aqq);
     const bool exempt = nhi >= 2.f * ECB_RHO * nlo && nhi >= cr.tc2;   // separated pair with a dominant column: the clean-up finishes it
     const bool strict = cr.strict_all || absa2 > cr.eabs2;
-    // (the clean-up is a first-order update: an exempt pair must be inside its range, cos^2 <= ECB_EXEMPT2, before the last sweep)
-    int flags = rot ? (exempt ? (absa2 > ECB_EXEMPT2 * pq ? 3 : 0)
-                              : (1 | (((strict && absa2 > big2 * pq) || absa2 > ECB_LOOSE2 * pq) ? 2 : 0))) : 0;
-    if (app - d < 0.25f * app || aqq + d < 0.25f * aqq) flags |= 4;
+    // One threshold on cos^2 says whether the pair still counts as big: exempt pairs only have to be inside the
+    // range of the first-order clean-up (ECB_EXEMPT2), strict pairs below 2 tol, the others below ECB_LOOSE2.
+    const float thr = exempt ? ECB_EXEMPT2 : (strict ? big2 : ECB_LOOSE2);
+    const bool isbig = rot && absa2 > thr * pq;
+    int flags = ((rot && !exempt) || isbig ? 1 : 0) | (isbig ? 2 : 0);
+    // sign(d) = sign(|g_q|^2 - |g_p|^2): the update takes |d| off the smaller norm; refresh if that cancels 3/4 of it
+    if (fabsf(d) > 0.75f * nlo) flags |= 4;
     // each half computed one rotation; swap so that every lane has both
     const float ocs = __shfl_xor_sync(0xffffffffu, cs, 16), ogr = __shfl_xor_sync(0xffffffffu, gr, 16);
     const float ogi = __shfl_xor_sync(0xffffffffu, gi, 16), od = __shfl_xor_sync(0xffffffffu, d, 16);
