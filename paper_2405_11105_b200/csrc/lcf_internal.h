@@ -175,7 +175,6 @@ struct lcf_plan {
     int* ptc_cta_first_d = nullptr;
     float* ptc_bpack_d = nullptr;           // [K][NB][Kp/4][256][4]
     float* ptc_part_d = nullptr;            // [NB][sum_k P_k]
-    lcf::TmapCache ptc_tmaps;
     bool ptc_pre = false, ptc_premaps_ready = false;   // pre-split fp16 planes of the ensemble (lcf_project_tc.cu, PRE variant)
     void *ptc_sh_d = nullptr, *ptc_sl_d = nullptr;     // [Kp/8][Nx][Nz][2][8] fp16 hi / lo
     alignas(64) unsigned char ptc_premaps[256];

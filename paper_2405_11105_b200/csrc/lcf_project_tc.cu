@@ -7,7 +7,7 @@
 // Real formulation.  Rows m of the A operand are the interleaved re/im samples of 64 pixels
 // (m = 2p: Re S, m = 2p+1: Im S), K = frames, and one CTA works on a block of 64 eigen-columns u
 // whose operand tile stays resident in shared memory for a whole segment:
-//   B tile rows  [0,64) Re B hi   [64,128) Im B hi   [128,192) Re B lo   [192,256) Im B lo
+//   B tile rows  [0,64) Re B hi   [64,128) Im B hi   [128,192) Re B lo   [192,256) Im B lo        (project_tc_kernel)
 //   D[:, 0:256] += A_hi * B[0:256]^T        D[:, 0:128] += A_lo * B[0:128]^T        (two MMAs / 16 frames)
 //   P_r[m][u] = D[m][u] + D[m][128+u] = X_m . Re B_u      P_i[m][u] = D[m][64+u] + D[m][192+u]
 //   U_r = P_r[2p] - P_i[2p+1]      U_i = P_i[2p] + P_r[2p+1]
@@ -19,18 +19,21 @@
 // normal fp16 number down to 2^-9 of the maximum and an absolute 2^-25 of it below.  Stacking B hi
 // over B lo makes one N = 256 MMA do two of the three products.
 //
-// Persistent CTAs walk a static slice of the list of (window, column block, 64-pixel tile) jobs,
-// cut into segments at (window, block) changes.  Roles (512 threads):
-//   warp 0      producer: the segment's packed B block (one bulk copy), then per 16 frames one TMA
-//               box [16 frames][4 x][16 z] complex64 -> raw stage (no swizzle: rows of 512 bytes);
+// The ensemble is split ONCE per call into fp16 hi / lo planes (presplit_kernel) laid out so that a TMA box is a
+// K-major A operand tile: the projection has no window weight inside its contraction, so the conversion is not
+// repeated for each of the ~15 windows and 2-4 column blocks that read a pixel, and no converter warps exist.
+//
+// Persistent CTAs walk a static slice of the list of (window, column block group, 64-pixel tile) jobs,
+// cut into segments at (window, group) changes.  Roles:
+//   warp 0      producer: the segment's packed B tile (one bulk copy), then per 16 frames two TMA boxes
+//               {16 z x 16 halves, 4 x, 2 chunks} of the hi and lo planes -> A_hi / A_lo of an operand stage;
 //   warp 1      MMA issuer (uniform control flow, one elected lane);
-//   warps 4-11  converters: raw [t][m] -> K-major fp16 A_hi / A_lo tiles (the transposition happens in
-//               registers: 8 frames of one row = one 16-byte core-matrix row);
-//   warps 12-15 epilogue: TMEM -> registers, pair exchange by shuffle, |U|^2 summed over the 64
-//               columns, times w^2, one float per (block, pixel); two accumulator buffers so the
-//               epilogue of a tile overlaps the MMAs of the next.
-// proj_tc_pack_kernel builds the B blocks from B_k; proj_tc_finish_kernel adds the column blocks
-// into the per-window PD tiles and the per-chunk sums that the alpha / combine kernels use.
+//   epilogue    TMEM -> registers, pair exchange by shuffle, |U|^2 summed over the 64 columns, times w^2, one float
+//               per (block, pixel); two accumulator buffers so the epilogue of a tile overlaps the MMAs of the next.
+// project_tc2_kernel (two resident column blocks as one N = 256 operand, N <= 152) and project_tc_kernel (one block, its hi
+// and lo rows as one N = 256 operand) differ in the resident tile and the TMEM layout only.  proj_tc_pack_kernel builds the
+// B tiles from B_k; proj_tc_finish_kernel adds the column blocks into the per-window PD tiles and the per-chunk sums that
+// the alpha / combine kernels use.
 #include <cuda.h>
 #include <cuda_fp16.h>
 #include <cstring>
@@ -46,19 +49,15 @@ constexpr int PTC_TZ = 16, PTC_TX = 4;                     // pixel tile: 16 z x
 constexpr int PTC_ROWS = 128;
 constexpr int PTC_KC = 16;                                 // frames per A stage
 constexpr int PTC_UB = 64;                                 // eigen-columns per block
-constexpr int PTC_RAW_STAGES = 8, PTC_OP_STAGES = 8;
-constexpr int PTC_RAW_BYTES = PTC_KC * PTC_ROWS * 4;       // 8 KB of fp32
+constexpr int PTC_OP_STAGES = 8;
 constexpr int PTC_A_BYTES = PTC_KC * PTC_ROWS * 2;         // one of A_hi / A_lo per stage: 4 KB of fp16
 constexpr int PTC_OP_BYTES = 2 * PTC_A_BYTES;
 constexpr int PTC_A_LBO = PTC_ROWS * 16;                   // 2048: next 8-frame chunk of A
 constexpr int PTC_B_LBO = 256 * 16;                        // 4096: next 8-frame chunk of B
 constexpr int PTC_SBO = 128;
 constexpr float PTC_B_SCALE = 256.f;
-constexpr int PTC_CONV_WARPS = 8, PTC_EPI_WARPS = 4;
-constexpr int PTC_CONV_GROUPS = 4;                         // converter groups working on alternate stages
-// a group must see every use of the stages it touches (an mbarrier waiter may not skip a phase)
-static_assert(PTC_RAW_STAGES % PTC_CONV_GROUPS == 0 && PTC_OP_STAGES % PTC_CONV_GROUPS == 0 && 4 % PTC_CONV_GROUPS == 0, "stages per group");
-constexpr int PTC_FIRST_CONV = 4, PTC_FIRST_EPI = PTC_FIRST_CONV + PTC_CONV_WARPS;
+constexpr int PTC_EPI_WARPS = 4;
+constexpr int PTC_FIRST_EPI = 12;                           // project_tc_kernel: warps 12-15 (warps 2-11 idle)
 constexpr int PTC_THREADS = 32 * (PTC_FIRST_EPI + PTC_EPI_WARPS);
 
 struct PtcArgs {
@@ -73,7 +72,7 @@ struct PtcArgs {
     int NB;
     float* part;                   // [NB][sum_k P_k]
     long long sumPk;
-    int nstg;                      // raw / operand stages in use: PTC_RAW_STAGES, or 4 when the B block needs the room
+    int nstg;                      // operand stages in use
     // MAG variant (method 4, lcf_ncc.cu): B = V in rank order; instead of the power sum the epilogue writes
     // |u_i(p)| = w(p) |U[p][i]| / sigma_i  to  mag[(tile_off + q) * magN + rank]
     float* mag;
@@ -82,7 +81,6 @@ struct PtcArgs {
 };
 
 struct PtcBars {
-    uint64_t full[PTC_RAW_STAGES], empty[PTC_RAW_STAGES];
     uint64_t opfull[PTC_OP_STAGES], opempty[PTC_OP_STAGES];
     uint64_t accfull[2], accempty[2];
     uint64_t bfull, bfree;
@@ -100,22 +98,16 @@ __device__ __forceinline__ void ptc_sts128(uint32_t addr, float x, float y, floa
 __device__ __forceinline__ void ptc_sts128u(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
-// PRE: the ensemble was split once into fp16 hi / lo planes laid out so that a TMA box IS a K-major operand tile
-// (presplit_kernel below): the producer loads A_hi / A_lo straight into the operand stages and the converter
-// warps have nothing to do -- the projection has no window weight inside its contraction, so the conversion
-// need not be repeated for each of the ~15 windows and 2-4 column blocks that read a pixel.
-struct PtcMaps { CUtensorMap m[2]; };    // !PRE: m[0] = fp32 cube.  PRE: hi plane, lo plane
+struct PtcMaps { CUtensorMap m[2]; };    // hi plane, lo plane
 
-template <bool MAG, bool PRE>
+template <bool MAG>
 __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid_constant__ PtcMaps maps, PtcArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     unsigned char* sbase = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
-    const int NSTG = a.nstg;                                                  // stages in use (raw and operand alike): 8 or 4
-    const uint32_t SMSK = (uint32_t)NSTG - 1u, SSH = NSTG == 8 ? 3u : 2u;
+    const uint32_t SMSK = (uint32_t)a.nstg - 1u, SSH = a.nstg == 8 ? 3u : 2u;           // operand stages in use: 8 (or 4)
     unsigned char* bsm = sbase;                                               // resident B block: Kp / 8 chunks of 4 KB
-    unsigned char* raw = sbase + (size_t)(a.Kp / 8) * PTC_B_LBO;              // [NSTG][8 KB]   (none with PRE)
-    unsigned char* ops = raw + (PRE ? 0 : NSTG * PTC_RAW_BYTES);              // [NSTG][A_hi 4 KB | A_lo 4 KB]
-    PtcBars* bars = reinterpret_cast<PtcBars*>(ops + NSTG * PTC_OP_BYTES);
+    unsigned char* ops = sbase + (size_t)(a.Kp / 8) * PTC_B_LBO;              // [stages][A_hi 4 KB | A_lo 4 KB]
+    PtcBars* bars = reinterpret_cast<PtcBars*>(ops + a.nstg * PTC_OP_BYTES);
     double* gzs = reinterpret_cast<double*>(bars + 1);                        // [Nz] window table rows (epilogue only)
     double* gxs = gzs + a.Nz;                                                 // [Nx]
     float* isig_s = reinterpret_cast<float*>(gxs + a.Nx);                     // [64] (MAG) 1 / sigma of the segment's column block
@@ -126,8 +118,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
     const uint32_t bbytes = (uint32_t)(a.Kp / 8) * 4096u;
 
     if (tid == 0) {
-        for (int s = 0; s < PTC_RAW_STAGES; ++s) { mbar_init(&bars->full[s], 1); mbar_init(&bars->empty[s], PTC_CONV_WARPS / PTC_CONV_GROUPS); }
-        for (int s = 0; s < PTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], PRE ? 1 : PTC_CONV_WARPS / PTC_CONV_GROUPS); mbar_init(&bars->opempty[s], 1); }
+        for (int s = 0; s < PTC_OP_STAGES; ++s) { mbar_init(&bars->opfull[s], 1); mbar_init(&bars->opempty[s], 1); }
         for (int b = 0; b < 2; ++b) { mbar_init(&bars->accfull[b], 1); mbar_init(&bars->accempty[b], PTC_EPI_WARPS); }
         mbar_init(&bars->bfull, 1);
         mbar_init(&bars->bfree, 1);
@@ -141,7 +132,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
 
     if (warp == 0) {
         // =========================== producer ===========================
-        if (lane == 0) { tma_prefetch_desc(&maps.m[0]); if (PRE) tma_prefetch_desc(&maps.m[1]); }
+        if (lane == 0) { tma_prefetch_desc(&maps.m[0]); tma_prefetch_desc(&maps.m[1]); }
         uint32_t it = 0;
         for (int sg = seg0; sg < seg1; ++sg) {
             const PtcSeg seg = a.segs[sg];
@@ -159,19 +150,11 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                 const int z = ze + tzi * PTC_TZ, x = bx.x0 + txi * PTC_TX;
                 for (int st = 0; st < nst; ++st, ++it) {
                     const int s = (it & SMSK);
-                    if (PRE) {                             // operand tiles straight from the pre-split planes
-                        mbar_wait(&bars->opempty[s], ((it >> SSH) & 1) ^ 1);
-                        if (lane == 0) {
-                            mbar_arrive_expect_tx(&bars->opfull[s], PTC_OP_BYTES);
-                            tma_load_3d(ops + (size_t)s * PTC_OP_BYTES, &maps.m[0], 16 * z, x, 2 * st, &bars->opfull[s]);
-                            tma_load_3d(ops + (size_t)s * PTC_OP_BYTES + PTC_A_BYTES, &maps.m[1], 16 * z, x, 2 * st, &bars->opfull[s]);
-                        }
-                    } else {
-                        mbar_wait(&bars->empty[s], ((it >> SSH) & 1) ^ 1);
-                        if (lane == 0) {
-                            mbar_arrive_expect_tx(&bars->full[s], PTC_RAW_BYTES);
-                            tma_load_3d(raw + (size_t)s * PTC_RAW_BYTES, &maps.m[0], 2 * z, x, st * PTC_KC, &bars->full[s]);
-                        }
+                    mbar_wait(&bars->opempty[s], ((it >> SSH) & 1) ^ 1);     // operand tiles straight from the pre-split planes
+                    if (lane == 0) {
+                        mbar_arrive_expect_tx(&bars->opfull[s], PTC_OP_BYTES);
+                        tma_load_3d(ops + (size_t)s * PTC_OP_BYTES, &maps.m[0], 16 * z, x, 2 * st, &bars->opfull[s]);
+                        tma_load_3d(ops + (size_t)s * PTC_OP_BYTES + PTC_A_BYTES, &maps.m[1], 16 * z, x, 2 * st, &bars->opfull[s]);
                     }
                 }
             }
@@ -208,56 +191,6 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
             }
             if (elect_one()) mma_commit(&bars->bfree);     // every MMA that reads this B block has completed
             __syncwarp();
-        }
-    } else if (!PRE && warp >= PTC_FIRST_CONV && warp < PTC_FIRST_EPI) {
-        // =========================== converters ===========================
-        const int cw = warp - PTC_FIRST_CONV;
-        const uint32_t raw_u32 = smem_u32(raw), ops_u32 = smem_u32(ops);
-        // 8 warp tasks per stage: (8-frame chunk c8, 32-row block).  The converter warps form
-        // PTC_CONV_GROUPS groups that take alternate stages (a warp does 8 / warps-per-group tasks of its
-        // stage), so the load -> convert -> store -> fence latency of one stage overlaps the next.
-        constexpr int WPG = PTC_CONV_WARPS / PTC_CONV_GROUPS, TPW = 8 / WPG;    // warps per group, tasks per warp
-        const int grp = cw / WPG, gw = cw % WPG;
-        uint32_t trd[TPW], tdst[TPW];
-#pragma unroll
-        for (int j = 0; j < TPW; ++j) {
-            const int wt = gw + j * WPG;
-            const int c8 = wt & 1, m = (wt >> 1) * 32 + lane;
-            trd[j] = (uint32_t)(8 * c8) * (PTC_ROWS * 4) + (uint32_t)m * 4u;
-            tdst[j] = (uint32_t)c8 * PTC_A_LBO + (uint32_t)m * 16u;
-        }
-        const float scale = pow2f(pow2_scale_exp(*a.amax));
-        uint32_t it = 0;
-        for (int sg = seg0; sg < seg1; ++sg) {
-            const int nstages = a.segs[sg].ntile * nst;
-            for (int q = 0; q < nstages; ++q, ++it) {
-                if ((int)(it % PTC_CONV_GROUPS) != grp) continue;
-                const int s = (it & SMSK), o = (it & SMSK);
-                const uint32_t rs = raw_u32 + (uint32_t)s * PTC_RAW_BYTES, os = ops_u32 + (uint32_t)o * PTC_OP_BYTES;
-                mbar_wait(&bars->full[s], (it >> SSH) & 1);
-                float v[TPW][8];
-#pragma unroll
-                for (int j = 0; j < TPW; ++j)
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) v[j][i] = ptc_lds32(rs + trd[j] + (uint32_t)i * (PTC_ROWS * 4)) * scale;
-                uint32_t h[TPW][4], l[TPW][4];
-#pragma unroll
-                for (int j = 0; j < TPW; ++j)
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) f16_split2(v[j][2 * i], v[j][2 * i + 1], h[j][i], l[j][i]);
-                mbar_wait(&bars->opempty[o], ((it >> SSH) & 1) ^ 1);
-#pragma unroll
-                for (int j = 0; j < TPW; ++j) {
-                    ptc_sts128u(os + tdst[j], h[j][0], h[j][1], h[j][2], h[j][3]);
-                    ptc_sts128u(os + PTC_A_BYTES + tdst[j], l[j][0], l[j][1], l[j][2], l[j][3]);
-                }
-                fence_proxy_async_smem();
-                __syncwarp();
-                if (lane == 0) {
-                    mbar_arrive(&bars->empty[s]);
-                    mbar_arrive(&bars->opfull[o]);
-                }
-            }
         }
     } else if (warp >= PTC_FIRST_EPI) {
         // =========================== epilogue ===========================
@@ -688,23 +621,6 @@ static PtcEncodeFn ptc_encode_fn() {
     return fn;
 }
 
-// [N][Nx][Nz] complex64 seen as float [N][Nx][2 Nz]; box = 16 z x 4 x x 16 frames, no swizzle
-static const CUtensorMap* ptc_encode_map(lcf_plan* p, const void* iq) {
-    if (const unsigned char* m = p->ptc_tmaps.find(iq)) return reinterpret_cast<const CUtensorMap*>(m);
-    PtcEncodeFn fn = ptc_encode_fn();
-    if (!fn) return nullptr;
-    unsigned char* slot = p->ptc_tmaps.slot(iq);
-    cuuint64_t dims[3] = {(cuuint64_t)2 * p->Nz, (cuuint64_t)p->Nx, (cuuint64_t)p->N};
-    cuuint64_t strides[2] = {(cuuint64_t)p->Nz * 8, (cuuint64_t)p->P * 8};
-    cuuint32_t box[3] = {2 * PTC_TZ, PTC_TX, PTC_KC};
-    cuuint32_t es[3] = {1, 1, 1};
-    CUresult r = fn(reinterpret_cast<CUtensorMap*>(slot), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(iq), dims,
-                    strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) { p->ptc_tmaps.drop_last(iq); return nullptr; }
-    return reinterpret_cast<const CUtensorMap*>(slot);
-}
-
 // fp16 planes [T8][Nx][Nz * 16 halves]; box = {256 halves (16 z), 4 x, 2 chunks}, no swizzle
 static bool ptc_encode_premaps(lcf_plan* p) {
     if (p->ptc_premaps_ready) return true;
@@ -804,20 +720,14 @@ cudaError_t configure_project_tc(lcf_plan* p, std::vector<PtcSeg>& segs, std::ve
     p->ptc_nseg = (int)segs.size();
     cudaError_t e = set_max_dyn_smem(project_tc2_kernel<false>, p->smem_optin);
     if (e == cudaSuccess) e = set_max_dyn_smem(project_tc2_kernel<true>, p->smem_optin);
-    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<false, true>, p->smem_optin);
-    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<true, true>, p->smem_optin);
+    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<false>, p->smem_optin);
+    if (e == cudaSuccess) e = set_max_dyn_smem(project_tc_kernel<true>, p->smem_optin);
     return e;
 }
 
-static bool ptc_fill_maps(lcf_plan* p, const void* iq, PtcMaps& maps) {
-    if (p->ptc_pre) {
-        if (!ptc_encode_premaps(p)) return false;
-        memcpy(&maps, p->ptc_premaps, sizeof(maps));
-        return true;
-    }
-    const CUtensorMap* tmap = ptc_encode_map(p, iq);
-    if (!tmap) return false;
-    maps.m[0] = *tmap; maps.m[1] = *tmap;
+static bool ptc_fill_maps(lcf_plan* p, const void*, PtcMaps& maps) {
+    if (!ptc_encode_premaps(p)) return false;
+    memcpy(&maps, p->ptc_premaps, sizeof(maps));
     return true;
 }
 
@@ -845,7 +755,7 @@ cudaError_t launch_project_tc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     PtcArgs a;
     ptc_fill_args(p, a);
     if (p->ptc_G == 2) project_tc2_kernel<false><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a, 2);
-    else project_tc_kernel<false, true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
+    else project_tc_kernel<false><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     proj_tc_finish_kernel<<<p->n_pitems, PROJ_TPIX, 0, st>>>(p->ptc_part_d, p->sumPk, p->ptc_NB, p->box_d, p->pitems_d, p->tiles_d, p->tsum_d);
@@ -865,7 +775,7 @@ cudaError_t launch_project_tc_mag(lcf_plan* p, const float2* iq, cudaStream_t st
     ptc_fill_args(p, a);
     a.mag = p->ncc_mag_d; a.magN = p->ncc_magN; a.isig = p->ncc_isig_d;
     if (p->ptc_G == 2) project_tc2_kernel<true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a, 2);
-    else project_tc_kernel<true, true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
+    else project_tc_kernel<true><<<p->ptc_grid, PTC_THREADS, p->ptc_smem, st>>>(maps, a);
     return cudaGetLastError();
 }
 
