@@ -145,7 +145,7 @@ lcf_status lcf_filter_batch(lcf_plan* plan, const void* const* iq_devs, float* c
 lcf_status lcf_filter_host(lcf_plan* plan, const void* iq_host, float* pd_host, cudaStream_t stream);
 
 /* `count` ensembles from HOST buffers, pipelined: the host->device copy of ensemble i+1 (on a
- * plan-owned copy stream, two staging buffers) overlaps the kernels of ensemble i, which run on two of the
+ * plan-owned copy stream, three staging buffers) overlaps the kernels of ensembles i and i-1, which run on the
  * lanes of lcf_filter_batch; each image is copied back as soon as it is done.  `stream` is synchronised
  * at entry.  iq_hosts / pd_hosts: HOST arrays of `count` HOST
  * pointers (pinned memory for the copies to be asynchronous).  Returns after everything has

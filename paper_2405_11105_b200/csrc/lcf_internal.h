@@ -211,10 +211,10 @@ struct lcf_plan {
     void* iq_stage_d = nullptr;
     float* pd_stage_d = nullptr;
     // second staging set, copy stream and events of lcf_filter_host_batch
-    void* iq_stage2_d = nullptr;
-    float* pd_stage2_d = nullptr;
+    void *iq_stage2_d = nullptr, *iq_stage3_d = nullptr;
+    float *pd_stage2_d = nullptr, *pd_stage3_d = nullptr;
     cudaStream_t copy_stream = nullptr;
-    cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
+    cudaEvent_t ev_copied[3] = {nullptr, nullptr, nullptr}, ev_done[3] = {nullptr, nullptr, nullptr};
 
     // lane pipelining of lcf_filter_batch (three lanes) / lcf_filter_host_batch (two): twin plans (same parameters,
     // their own workspace) and one internal stream per lane, created on first use
