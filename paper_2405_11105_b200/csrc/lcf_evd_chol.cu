@@ -55,6 +55,7 @@ struct EcArgs {
     int chol_only;                // 1: stop after the Cholesky factor and write it to gfac / shift (cluster Jacobi follows)
     float* gfac;                  // [K][2][Ns][LD] real plane, imaginary plane of G, column-major
     float* shift;                 // [K] delta, or -1 for an all-zero matrix
+    int glob;                     // 1: the matrix does not fit shared memory (N > 128): factor it in place in gfac (global memory, L2-resident)
     int* nexp;                    // [K] power-of-two exponent this kernel scaled R_k by (0 when R carries the tensor-core data scale)
 };
 
@@ -100,9 +101,9 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int k = blockIdx.x;
     // planar storage: real and imaginary parts of column u at Gr/Gi + u*LD (LD floats, multiple of 4)
-    float* Gr = reinterpret_cast<float*>(smem_raw);                  // [Ns][LD]
+    float* Gr = a.glob ? a.gfac + (size_t)k * 2 * Ns * LD : reinterpret_cast<float*>(smem_raw);   // [Ns][LD]
     float* Gi = Gr + (size_t)Ns * LD;                                // [Ns][LD]
-    float* lam_s = Gi + (size_t)Ns * LD;                             // [Ns] eigenvalue of slot u
+    float* lam_s = a.glob ? reinterpret_cast<float*>(smem_raw) : Gi + (size_t)Ns * LD;            // [Ns] eigenvalue of slot u
     float* inv_s = lam_s + Ns;                                       // [Ns] 1 / |g_u|
     float* wsl = inv_s + Ns;                                         // [Ns] eigen-weight of slot u
     float* red = wsl + Ns;                                           // [32]
@@ -162,6 +163,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         // lowest row): each warp reduces its rows when it downdates them, and after the step's barrier
         // every warp reduces the 16 warp keys.
         const int nchc = (N + 3) >> 2;                               // 4-row chunks per column
+        const unsigned KM = N > 128 ? 255u : 127u;                   // row index bits of a pivot key
         float* dgs = lam_s;                                          // [N] current diagonal of the Schur complement, -1 once eliminated
         unsigned* wkey = reinterpret_cast<unsigned*>(red);           // [16] per-warp pivot keys
         int* elist = alist;                                          // [N] pivot of step t = slot of Cholesky column t
@@ -170,7 +172,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
             if (tid < N) {
                 const float d = fmaxf(Gr[(size_t)tid * LD + tid], 0.f);
                 dgs[tid] = d;
-                key = (__float_as_uint(d) & ~127u) | (unsigned)(127 - tid);
+                key = (__float_as_uint(d) & ~KM) | (KM - (unsigned)tid);
             }
             key = __reduce_max_sync(0xffffffffu, key);
             if (lane == 0) wkey[warp] = key;
@@ -181,7 +183,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
             for (int j = jb; j < je; ++j) {
                 unsigned kk = lane < EC_THREADS / 32 ? wkey[lane] : 0u;
                 kk = __reduce_max_sync(0xffffffffu, kk);
-                const int pv = 127 - (int)(kk & 127u);
+                const int pv = (int)(KM - (kk & KM));
                 unsigned key = 0u;
                 if (tid < N) {
                     // a non-positive pivot can only come from rounding: clamp (the column is then ~0)
@@ -204,7 +206,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
                         vi = (Gi[(size_t)pv * LD + i] - si) * sc;
                         const float nd = fmaxf(d - (vr * vr + vi * vi), 0.f);
                         dgs[i] = nd;
-                        key = (__float_as_uint(nd) & ~127u) | (unsigned)(127 - i);
+                        key = (__float_as_uint(nd) & ~KM) | (KM - (unsigned)i);
                     }
                     Gr[(size_t)pv * LD + i] = vr;
                     Gi[(size_t)pv * LD + i] = vi;
@@ -215,35 +217,39 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
                 __syncthreads();
             }
             if (je < N) {
-                // rank-(je - jb) update of the columns still to be eliminated
-                float4 gbr[EC_NB], gbi[EC_NB];
+                // rank-(je - jb) update of the columns still to be eliminated (row chunks lane, lane + 32, ...)
                 const float* gcol[EC_NB];
 #pragma unroll
-                for (int t = 0; t < EC_NB; ++t) {
-                    gcol[t] = Gr + (size_t)elist[jb + t < je ? jb + t : jb] * LD;
-                    gbr[t] = gbi[t] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (jb + t < je && lane < nchc) {
-                        gbr[t] = *reinterpret_cast<const float4*>(&gcol[t][4 * lane]);
-                        gbi[t] = *reinterpret_cast<const float4*>(&gcol[t][(size_t)Ns * LD + 4 * lane]);
-                    }
-                }
-                for (int l = warp; l < N; l += EC_THREADS / 32) {
-                    if (dgs[l] < 0.f) continue;                      // already a Cholesky column
-                    if (lane < nchc) {
-                        float* cr = Gr + (size_t)l * LD + 4 * lane;
-                        float* ci = Gi + (size_t)l * LD + 4 * lane;
-                        float4 xr = *reinterpret_cast<float4*>(cr), xi = *reinterpret_cast<float4*>(ci);
+                for (int t = 0; t < EC_NB; ++t) gcol[t] = Gr + (size_t)elist[jb + t < je ? jb + t : jb] * LD;
+                for (int c0 = 0; c0 < nchc; c0 += 32) {
+                    const int ch = c0 + lane;
+                    float4 gbr[EC_NB], gbi[EC_NB];
 #pragma unroll
-                        for (int t = 0; t < EC_NB; ++t) {
-                            // x -= g_t conj(G[l, e_t]):  re -= gr lr + gi li,  im -= gi lr - gr li  (zero columns for t >= je - jb)
-                            const float lr = gcol[t][l], li = gcol[t][(size_t)Ns * LD + l];
-                            xr.x -= gbr[t].x * lr + gbi[t].x * li;  xi.x -= gbi[t].x * lr - gbr[t].x * li;
-                            xr.y -= gbr[t].y * lr + gbi[t].y * li;  xi.y -= gbi[t].y * lr - gbr[t].y * li;
-                            xr.z -= gbr[t].z * lr + gbi[t].z * li;  xi.z -= gbi[t].z * lr - gbr[t].z * li;
-                            xr.w -= gbr[t].w * lr + gbi[t].w * li;  xi.w -= gbi[t].w * lr - gbr[t].w * li;
+                    for (int t = 0; t < EC_NB; ++t) {
+                        gbr[t] = gbi[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (jb + t < je && ch < nchc) {
+                            gbr[t] = *reinterpret_cast<const float4*>(&gcol[t][4 * ch]);
+                            gbi[t] = *reinterpret_cast<const float4*>(&gcol[t][(size_t)Ns * LD + 4 * ch]);
                         }
-                        *reinterpret_cast<float4*>(cr) = xr;
-                        *reinterpret_cast<float4*>(ci) = xi;
+                    }
+                    for (int l = warp; l < N; l += EC_THREADS / 32) {
+                        if (dgs[l] < 0.f) continue;                  // already a Cholesky column
+                        if (ch < nchc) {
+                            float* cr = Gr + (size_t)l * LD + 4 * ch;
+                            float* ci = Gi + (size_t)l * LD + 4 * ch;
+                            float4 xr = *reinterpret_cast<float4*>(cr), xi = *reinterpret_cast<float4*>(ci);
+#pragma unroll
+                            for (int t = 0; t < EC_NB; ++t) {
+                                // x -= g_t conj(G[l, e_t]):  re -= gr lr + gi li,  im -= gi lr - gr li  (zero columns for t >= je - jb)
+                                const float lr = gcol[t][l], li = gcol[t][(size_t)Ns * LD + l];
+                                xr.x -= gbr[t].x * lr + gbi[t].x * li;  xi.x -= gbi[t].x * lr - gbr[t].x * li;
+                                xr.y -= gbr[t].y * lr + gbi[t].y * li;  xi.y -= gbi[t].y * lr - gbr[t].y * li;
+                                xr.z -= gbr[t].z * lr + gbi[t].z * li;  xi.z -= gbi[t].z * lr - gbr[t].z * li;
+                                xr.w -= gbr[t].w * lr + gbi[t].w * li;  xi.w -= gbi[t].w * lr - gbr[t].w * li;
+                            }
+                            *reinterpret_cast<float4*>(cr) = xr;
+                            *reinterpret_cast<float4*>(ci) = xi;
+                        }
                     }
                 }
                 __syncthreads();
@@ -251,7 +257,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         }
         if (a.chol_only) {
             float* gout = a.gfac + (size_t)k * 2 * Ns * LD;
-            for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) gout[e] = Gr[e];
+            if (!a.glob) for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) gout[e] = Gr[e];
             if (tid == 0) a.shift[k] = delta;
             return;
         }
@@ -345,7 +351,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         __syncthreads();
         if (a.chol_only) {
             float* gout = a.gfac + (size_t)k * 2 * Ns * LD;
-            for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) gout[e] = Gr[e];
+            if (!a.glob) for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) gout[e] = Gr[e];
             if (tid == 0) a.shift[k] = -1.f;
             return;
         }
@@ -427,15 +433,19 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     }
 }
 
-static size_t ec_smem_bytes(int Ns, int LD) {
-    return (size_t)Ns * LD * 8 + 3 * (size_t)Ns * 4 + 32 * 4 + (size_t)Ns * 8 + 3 * (size_t)Ns * 4 + 16 + 16 + 64;
+static size_t ec_smem_bytes(int Ns, int LD, bool glob) {
+    return (glob ? 0 : (size_t)Ns * LD * 8) + 3 * (size_t)Ns * 4 + 32 * 4 + (size_t)Ns * 8 + 3 * (size_t)Ns * 4 + 16 + 16 + 64;
 }
 
-bool evd_chol_eligible(const lcf_plan* p) { return p->prec == 0 && p->N <= 128 && p->N >= 2; }
+// N <= 128: the matrix lives in shared memory.  128 < N <= ECL8_MAXN (even): only the Cholesky factor is taken here,
+// in place in global memory, and the Jacobi sweeps run on 8-CTA clusters (lcf_evd_cluster.cu).
+bool evd_chol_eligible(const lcf_plan* p) {
+    return p->prec == 0 && p->N >= 2 && (p->N <= 128 || (p->N <= ECL8_MAXN && p->N % 2 == 0));
+}
 
 cudaError_t configure_evd_chol(lcf_plan* p) {
     p->ec_LD = ((p->N + 3) & ~3) + 4;   // floats per column plane: whole float4 chunks, +4 shifts the banks column to column
-    p->ec_smem = ec_smem_bytes(p->Ns, p->ec_LD);
+    p->ec_smem = ec_smem_bytes(p->Ns, p->ec_LD, p->N > 128);
     if (p->ec_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaSuccess;
 #define EC_SET(NC, FULL) if (e == cudaSuccess) e = set_max_dyn_smem(evd_chol_kernel<NC, FULL>, p->smem_optin)
@@ -454,6 +464,12 @@ cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only) {
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
     a.mode = evd_mode(p); a.k_fixed = evd_kfixed(p); a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
+    a.glob = p->N > 128 ? 1 : 0;
+    if (a.glob) {                                                    // factor only (chol_only is implied: see evd_chol_eligible)
+        if (!chol_only) return cudaErrorInvalidConfiguration;
+        evd_chol_kernel<1, false><<<p->K, EC_THREADS, p->ec_smem, st>>>(a);
+        return cudaGetLastError();
+    }
     const int nch = (p->N + 3) / 4, nc = (nch + 7) / 8;
     const bool full = (p->N % 32) == 0;
 #define EC_RUN(NC) do { if (full) evd_chol_kernel<NC, true><<<p->K, EC_THREADS, p->ec_smem, st>>>(a); \

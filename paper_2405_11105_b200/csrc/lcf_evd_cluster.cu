@@ -1,5 +1,5 @@
 // lcf_evd_cluster.cu -- kernel 2+3, one-sided Jacobi spread over a 2-CTA thread-block cluster
-// (precision 0, even N, 32 <= N <= 128).  The single-CTA kernel of lcf_evd_chol.cu is bound by
+// (precision 0, even N, 32 <= N <= 128; above that, up to ECL8_MAXN frames, over an 8-CTA cluster: jacobi_cluster8_kernel).  The single-CTA kernel of lcf_evd_chol.cu is bound by
 // shared-memory bandwidth (the whole N x N matrix crosses the 128 B/clk crossbar twice per
 // rotation step) and uses 64 of 148 SMs at 64 windows; here each matrix gets two SMs.
 //
@@ -140,9 +140,9 @@ __device__ __forceinline__ int ecl_slot(int b, int t, int j, int LD) { return ((
 
 // Shared tail of the cluster kernels: eigenvalues (|g|^2 - delta) and 1/|g| of this CTA's ncl columns
 // (local column cl = global slot u0 + cl, real plane at colptr(cl), imaginary plane LD floats on),
-// published to both CTAs; ranking, cut-off rule, eigen-weights; V_k and B_k = V_k diag(wt).
+// published to all csz CTAs of the cluster; ranking, cut-off rule, eigen-weights; V_k and B_k = V_k diag(wt).
 template <class ColPtr>
-__device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t rank, uint32_t peer, int u0, int ncl, ColPtr colptr,
+__device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t rank, uint32_t csz, int u0, int ncl, ColPtr colptr,
                                              float* lam_s, float* inv_s, float* wsl, double* lsort, int* ish,
                                              float shiftv, float delta, int sweep, int converged) {
     const int N = a.N, Ns = a.N, LD = a.LD;
@@ -169,8 +169,10 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
             const float lamv = shiftv < 0.f ? 0.f : nn - delta;
             const float invv = nn > 0.f ? rsqrtf(nn) : 0.f;
             const uint32_t la = ecl_smem(&lam_s[u]), ia = ecl_smem(&inv_s[u]);
-            ecl_st_cluster_f32(la, lamv); ecl_st_cluster_f32(ecl_mapa(la, peer), lamv);
-            ecl_st_cluster_f32(ia, invv); ecl_st_cluster_f32(ecl_mapa(ia, peer), invv);
+            for (uint32_t c = 0; c < csz; ++c) {
+                ecl_st_cluster_f32(ecl_mapa(la, c), lamv);
+                ecl_st_cluster_f32(ecl_mapa(ia, c), invv);
+            }
         }
     }
     ecl_cluster_sync();
@@ -218,7 +220,7 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
     // ---- V[row][u] = G[row][u] / |g_u|, B = V diag(wt) for this CTA's slots u in [u0, u0 + ncl)
     float2* Vk = a.V + (size_t)k * N * Ns;
     float2* Bk = a.B + (size_t)k * N * Ns;
-    for (int e = tid; e < N * ncl; e += ECL_THREADS) {
+    for (int e = tid; e < N * ncl; e += (int)blockDim.x) {
         const int row = e / ncl, cl = e - row * ncl;
         const int u = u0 + cl;
         const float* cr = colptr(cl);
@@ -388,8 +390,189 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
         last = small;
     }
 
-    ecl_epilogue(a, k, rank, peer, 2 * p0, 2 * npl,
+    ecl_epilogue(a, k, rank, 2u, 2 * p0, 2 * npl,
                  [&](int cl) { return (const float*)(buf + ecl_slot(b, cl & 1, cl >> 1, LD)); },
+                 lam_s, inv_s, wsl, lsort, ish, shiftv, delta, sweep, converged);
+}
+
+// ------------------------------------------------------------------------------------------------
+// 128 < N <= ECL8_MAXN (even): the same pair-systolic array over an 8-CTA cluster.  A 200 x 200 complex
+// factor is 320 KB, more than one SM's shared memory, so CTA c owns pairs [n c / 8, n (c + 1) / 8)
+// (<= ECL8_PL = 13 pairs, double-buffered: <= 88 KB, so two CTAs of different windows share an SM and
+// fill each other's barrier and latency gaps); the columns that cross a CTA boundary go to the
+// neighbour over DSMEM, one cluster barrier per step.  16 threads per pair, 4-row chunks r + 16 c.
+// Measured on config 3 (192 windows of 200 frames, 6.6 sweeps): 15.9 ms, against 17.2 ms for 4-CTA
+// clusters of 26 pairs (one CTA per SM) and 17.4 ms for the two-sided CUDA-core kernel it replaces.
+constexpr int ECL8_PL = 13;                     // pair slots per CTA
+constexpr uint32_t ECL8_CS = 8;                // CTAs per cluster
+constexpr int ECL8_THREADS = 256;              // 16 threads per pair; two CTAs (of different windows) share an SM
+__device__ __forceinline__ int ecl8_slot(int b, int t, int j, int LD) { return (((b * 2 + t) * ECL8_PL + j) * 2) * LD; }
+__device__ __forceinline__ int ecl8_first(int n, int c) { return (n * c) / (int)ECL8_CS; }
+
+template <int NC>
+__global__ void __cluster_dims__(8, 1, 1) __launch_bounds__(ECL8_THREADS, 2) jacobi_cluster8_kernel(EclArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = a.N, n = a.n, LD = a.LD, Ns = N;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const uint32_t rank = ecl_cluster_rank();
+    const int k = blockIdx.x / (int)ECL8_CS;
+    const int p0 = ecl8_first(n, (int)rank), npl = ecl8_first(n, (int)rank + 1) - p0;   // this CTA's pairs [p0, p0 + npl)
+    float* buf = reinterpret_cast<float*>(smem_raw);                 // [2 buffers][2 rows][ECL8_PL][2 planes][LD]
+    float* lam_s = buf + (size_t)2 * 2 * ECL8_PL * 2 * LD;           // [Ns] eigenvalue of slot u (all slots, every CTA)
+    float* inv_s = lam_s + Ns;                                       // [Ns]
+    float* wsl = inv_s + Ns;                                         // [Ns]
+    float* flg = wsl + Ns;                                           // [2 parities][ECL8_CS ranks] "rotated in this sweep"
+    double* lsort = reinterpret_cast<double*>(flg + 2 * ECL8_CS);              // [Ns]
+    int* ish = reinterpret_cast<int*>(lsort + Ns);                   // [4]
+    const uint32_t buf_u32 = ecl_smem(buf);
+
+    // ---- initial placement: top[i] = column 2i, bot[i] = column 2i+1
+    const float* gk = a.gfac + (size_t)k * 2 * N * a.LDg;
+    const int nch = (N + 3) >> 2;                                    // 4-row chunks per column
+    for (int e = tid; e < npl * 2 * 2 * nch; e += ECL8_THREADS) {
+        const int ch = e % nch; int q = e / nch;
+        const int pl = q & 1; q >>= 1;
+        const int t = q & 1, j = q >> 1;
+        const int col = 2 * (p0 + j) + t;
+        const float4 v = *reinterpret_cast<const float4*>(gk + ((size_t)pl * N + col) * a.LDg + 4 * ch);
+        *reinterpret_cast<float4*>(buf + ecl8_slot(0, t, j, LD) + pl * LD + 4 * ch) = v;
+    }
+    // the padding chunk behind row N of every plane stays zero: lanes whose chunk r + 16 c is past the last row read it
+    // instead (no branch around the loads, nothing added to the sums) and skip their stores
+    for (int e = tid; e < 2 * 2 * ECL8_PL * 2; e += ECL8_THREADS)
+        *reinterpret_cast<float4*>(buf + (size_t)e * LD + 4 * nch) = make_float4(0.f, 0.f, 0.f, 0.f);
+    const float shiftv = a.shift[k];
+    const float delta = shiftv < 0.f ? 0.f : shiftv;
+
+    // ---- one-sided Jacobi sweeps
+    // Rotate whenever the cosine is above 4 eps (not the 4 sqrt(N) eps of the kernels for N <= 128): the
+    // normalised columns are the eigenvectors, so what is left of a (tissue, blood) pair's cosine is tissue leaking
+    // into the filtered signal at that amplitude -- with tissue 60 dB up (config 3) 7e-6 is a 4e-3 image error,
+    // 5e-7 is 5e-4 (measured).  The stop rule keeps the 2 * 4 sqrt(N) eps bound on the squared cosine.
+    const float tol = 4.f * FLT_EPSILON;
+    const float tol2 = tol * tol;
+    const float bigt = 2.f * 4.f * sqrtf((float)N) * FLT_EPSILON;
+    const int j = tid >> 4, r = tid & 15;                            // local pair, lane within the pair
+    const int gi = p0 + j;                                           // global pair index
+    const unsigned hmask = (lane < 16) ? 0x0000ffffu : 0xffff0000u;  // j < npl is uniform per half warp
+    // destinations of this pair's columns after the step (row, global pair): see the header
+    int dPt, dPi, dQt, dQi;
+    if (gi == 0) { dPt = 0; dPi = 0; dQt = 0; dQi = 1; }
+    else { dQt = 1; dQi = gi - 1; if (gi == n - 1) { dPt = 1; dPi = n - 1; } else { dPt = 0; dPi = gi + 1; } }
+    if (j >= npl) { dPi = dQi = p0; }                                // idle threads: any valid pair
+    int rP = 0, rQ = 0;                                              // owning CTAs of the destinations
+    while (dPi >= ecl8_first(n, rP + 1)) ++rP;
+    while (dQi >= ecl8_first(n, rQ + 1)) ++rQ;
+    const int dPj = dPi - ecl8_first(n, rP), dQj = dQi - ecl8_first(n, rQ);
+    const uint32_t baseP = ecl_mapa(buf_u32, (uint32_t)rP), baseQ = ecl_mapa(buf_u32, (uint32_t)rQ);
+    // One cluster barrier per step covers the local and the remote hazard.  (Measured on config 3 with 4-CTA clusters: per-pair mbarrier
+    // dataflow as in jacobi_cluster_block_kernel, with 16-thread pairs spinning inside shared warps, runs at 6.0 ms
+    // per sweep over the 192 windows; __syncthreads plus one st.async mbarrier per CTA for the boundary columns at
+    // 3.0 ms; this plain barrier at 2.5 ms -- the step is bound by its FMA2 and shared-memory phases, not by the barrier.)
+    ecl_cluster_sync();                                              // all CTAs of the cluster resident, buffers filled
+    const int M = 2 * n - 1;
+    uint32_t cho[NC];                                                // byte offset of this lane's chunk c in a plane (the zero chunk when past the end)
+#pragma unroll
+    for (int c = 0; c < NC; ++c) cho[c] = 16u * (uint32_t)(r + 16 * c < nch ? r + 16 * c : nch);
+    const uint32_t L4 = 4u * (uint32_t)LD;
+    int b = 0, sweep = 0, converged = 0;
+    bool last = false;
+    for (;;) {
+        int any = 0, big = 0;
+        for (int s = 0; s < M; ++s) {
+            if (j < npl) {
+                const uint32_t sP = buf_u32 + (uint32_t)ecl8_slot(b, 0, j, LD) * 4u, sQ = buf_u32 + (uint32_t)ecl8_slot(b, 1, j, LD) * 4u;
+                ulonglong2 PR[NC], PI[NC], QR[NC], QI[NC];
+                unsigned long long app2 = 0ull, aqq2 = 0ull, re2 = 0ull, ima2 = 0ull, imb2 = 0ull;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    PR[c] = ecl_ld_local(sP + cho[c]); PI[c] = ecl_ld_local(sP + L4 + cho[c]);
+                    QR[c] = ecl_ld_local(sQ + cho[c]); QI[c] = ecl_ld_local(sQ + L4 + cho[c]);
+                }
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    app2 = ecl_fma2(PR[c].x, PR[c].x, app2); app2 = ecl_fma2(PI[c].x, PI[c].x, app2);
+                    app2 = ecl_fma2(PR[c].y, PR[c].y, app2); app2 = ecl_fma2(PI[c].y, PI[c].y, app2);
+                    aqq2 = ecl_fma2(QR[c].x, QR[c].x, aqq2); aqq2 = ecl_fma2(QI[c].x, QI[c].x, aqq2);
+                    aqq2 = ecl_fma2(QR[c].y, QR[c].y, aqq2); aqq2 = ecl_fma2(QI[c].y, QI[c].y, aqq2);
+                    re2 = ecl_fma2(PR[c].x, QR[c].x, re2);   re2 = ecl_fma2(PI[c].x, QI[c].x, re2);
+                    re2 = ecl_fma2(PR[c].y, QR[c].y, re2);   re2 = ecl_fma2(PI[c].y, QI[c].y, re2);
+                    ima2 = ecl_fma2(PR[c].x, QI[c].x, ima2); imb2 = ecl_fma2(PI[c].x, QR[c].x, imb2);
+                    ima2 = ecl_fma2(PR[c].y, QI[c].y, ima2); imb2 = ecl_fma2(PI[c].y, QR[c].y, imb2);
+                }
+                float app = ecl_hsum(app2), aqq = ecl_hsum(aqq2), xr = ecl_hsum(re2), xi = ecl_hsum(ima2) - ecl_hsum(imb2);
+#pragma unroll
+                for (int o = 8; o > 0; o >>= 1) {
+                    app += __shfl_xor_sync(hmask, app, o);
+                    aqq += __shfl_xor_sync(hmask, aqq, o);
+                    xr += __shfl_xor_sync(hmask, xr, o);
+                    xi += __shfl_xor_sync(hmask, xi, o);
+                }
+                const float absa2 = xr * xr + xi * xi;
+                const bool rot = absa2 > tol2 * app * aqq && absa2 > 0.f;
+                float cs = 1.f, gr = 0.f, gim = 0.f;
+                if (rot) {
+                    any = 1;
+                    if (absa2 > bigt * app * aqq) big = 1;        // cos^2 > 2 tol: not yet in the final quadratic phase
+                    const float inv = rsqrtf(absa2);
+                    const float tau = (aqq - app) * (0.5f * inv);
+                    const float at = fminf(fabsf(tau), 1e18f);
+                    const float w1 = fmaf(at, at, 1.f);
+                    const float t0 = __fdividef(1.f, at + w1 * rsqrtf(w1));
+                    const float t = copysignf(t0, tau);
+                    const float x1 = fmaf(t, t, 1.f);
+                    float c0 = rsqrtf(x1);
+                    c0 = c0 * fmaf(-0.5f * x1, c0 * c0, 1.5f);
+                    cs = c0;
+                    const float sn = t * cs;
+                    gr = sn * xr * inv; gim = sn * xi * inv;
+                }
+                const unsigned long long c2 = ecl_pack(cs, cs), gr2 = ecl_pack(gr, gr), gi2 = ecl_pack(gim, gim);
+                const unsigned long long ngr2 = ecl_pack(-gr, -gr), ngi2 = ecl_pack(-gim, -gim);
+                const uint32_t aP = baseP + (uint32_t)ecl8_slot(b ^ 1, dPt, dPj, LD) * 4u;
+                const uint32_t aQ = baseQ + (uint32_t)ecl8_slot(b ^ 1, dQt, dQj, LD) * 4u;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const int ch = r + 16 * c;
+                    {
+                        ulonglong2 npr, npi, nqr, nqi;
+                        // g_p' = c g_p - conj(g) g_q,   g_q' = g g_p + c g_q   (identity when not rotating)
+                        npr.x = ecl_fma2(ngi2, QI[c].x, ecl_fma2(ngr2, QR[c].x, ecl_mul2(c2, PR[c].x)));
+                        npr.y = ecl_fma2(ngi2, QI[c].y, ecl_fma2(ngr2, QR[c].y, ecl_mul2(c2, PR[c].y)));
+                        npi.x = ecl_fma2(gi2, QR[c].x, ecl_fma2(ngr2, QI[c].x, ecl_mul2(c2, PI[c].x)));
+                        npi.y = ecl_fma2(gi2, QR[c].y, ecl_fma2(ngr2, QI[c].y, ecl_mul2(c2, PI[c].y)));
+                        nqr.x = ecl_fma2(c2, QR[c].x, ecl_fma2(ngi2, PI[c].x, ecl_mul2(gr2, PR[c].x)));
+                        nqr.y = ecl_fma2(c2, QR[c].y, ecl_fma2(ngi2, PI[c].y, ecl_mul2(gr2, PR[c].y)));
+                        nqi.x = ecl_fma2(c2, QI[c].x, ecl_fma2(gi2, PR[c].x, ecl_mul2(gr2, PI[c].x)));
+                        nqi.y = ecl_fma2(c2, QI[c].y, ecl_fma2(gi2, PR[c].y, ecl_mul2(gr2, PI[c].y)));
+                        if (ch < nch) {                              // shared::cluster addresses (mapa of the own rank for local slots)
+                            ecl_st_cluster(aP + cho[c], npr); ecl_st_cluster(aP + L4 + cho[c], npi);
+                            ecl_st_cluster(aQ + cho[c], nqr); ecl_st_cluster(aQ + L4 + cho[c], nqi);
+                        }
+                    }
+                }
+            }
+            ecl_cluster_sync();
+            b ^= 1;
+        }
+        ++sweep;
+        // stop rule of jacobi_cluster_kernel, over the cluster's CTAs
+        const int mine = __syncthreads_or(any) + __syncthreads_or(big);
+        if (tid == 0) {
+            const uint32_t fa = ecl_smem(&flg[(sweep & 1) * ECL8_CS + rank]);
+            for (uint32_t c = 0; c < ECL8_CS; ++c) ecl_st_cluster_f32(ecl_mapa(fa, c), (float)mine);
+        }
+        ecl_cluster_sync();
+        float fmx = 0.f;
+        for (int c = 0; c < (int)ECL8_CS; ++c) fmx = fmaxf(fmx, flg[(sweep & 1) * ECL8_CS + c]);
+        const bool small = fmx < 2.f;
+        if ((last && small) || fmx == 0.f) { converged = 1; break; }
+        if (sweep == a.max_sweeps) break;
+        last = small;
+    }
+
+    ecl_epilogue(a, k, rank, ECL8_CS, 2 * p0, 2 * npl,
+                 [&](int cl) { return (const float*)(buf + ecl8_slot(b, cl & 1, cl >> 1, LD)); },
                  lam_s, inv_s, wsl, lsort, ish, shiftv, delta, sweep, converged);
 }
 
@@ -920,7 +1103,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
         ecb_cleanup(N, LD, rank, peer, 4 * p0, npl,
                     [&](int cl) { return buf + ecb_slot(b, (cl >> 1) & 1, cl >> 2, cl & 1, LD); },
                     nrm_all, care, Pb, Gm, dP);
-    ecl_epilogue(a, k, rank, peer, 4 * p0, 4 * npl,
+    ecl_epilogue(a, k, rank, 2u, 4 * p0, 4 * npl,
                  [&](int cl) { return (const float*)(buf + ecb_slot(b, (cl >> 1) & 1, cl >> 2, cl & 1, LD)); },
                  lam_s, inv_s, wsl, lsort, ish, shiftv, delta, sweep, converged);
 }
@@ -930,9 +1113,19 @@ static size_t ecl_smem_bytes(int N, int LD) {
            (128 + 4) * 4 + ECB_KC * 4 + (size_t)ECB_KC * 2 * LD * 4 + ECB_KC * 64 * 8 + (size_t)2 * ECB_KC * 2 * LD * 4;   // clean-up workspace
 }
 
-bool evd_cluster_eligible(const lcf_plan* p) { return p->prec == 0 && (p->N % 2) == 0 && p->N >= 32 && p->N <= 128; }
+static size_t ecl8_smem_bytes(int N, int LD) {
+    return (size_t)2 * 2 * ECL8_PL * 2 * LD * 4 + 3 * (size_t)N * 4 + 2 * ECL8_CS * 4 + (size_t)N * 8 + 16 + 64;
+}
+
+bool evd_cluster_eligible(const lcf_plan* p) { return p->prec == 0 && (p->N % 2) == 0 && p->N >= 32 && p->N <= ECL8_MAXN; }
 
 cudaError_t configure_evd_cluster(lcf_plan* p) {
+    if (p->N > 128) {
+        static_assert(ECL8_MAXN <= 2 * (int)ECL8_CS * ECL8_PL, "ECL8_CS CTAs of ECL8_PL pairs");
+        p->ecl_smem = ecl8_smem_bytes(p->N, p->ec_LD);
+        if (p->ecl_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
+        return set_max_dyn_smem(jacobi_cluster8_kernel<4>, p->smem_optin);
+    }
     p->ecl_smem = ecl_smem_bytes(p->N, p->ec_LD);
     if (p->ecl_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaSuccess;
@@ -951,6 +1144,10 @@ cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st) {
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
     a.mode = evd_mode(p); a.k_fixed = evd_kfixed(p); a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
+    if (p->N > 128) {
+        jacobi_cluster8_kernel<4><<<(int)ECL8_CS * p->K, ECL8_THREADS, p->ecl_smem, st>>>(a);
+        return cudaGetLastError();
+    }
     if (p->N % 4 == 0) {
         jacobi_cluster_block_kernel<<<2 * p->K, ECL_THREADS, p->ecl_smem, st>>>(a);
         return cudaGetLastError();

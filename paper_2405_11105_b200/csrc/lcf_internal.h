@@ -269,6 +269,7 @@ cudaError_t launch_gram_stream(lcf_plan* p, const float2* iq, int stride, cudaSt
 bool evd_chol_eligible(const lcf_plan* p);
 cudaError_t configure_evd_chol(lcf_plan* p);
 cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only);
+constexpr int ECL8_MAXN = 208;                // most frames of the 8-CTA cluster EVD (13 column pairs per CTA)
 bool evd_cluster_eligible(const lcf_plan* p);
 cudaError_t configure_evd_cluster(lcf_plan* p);
 cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st);

@@ -253,6 +253,7 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
         cudaGetLastError();
         p->evd_cluster = false;
     }
+    if (p->N > 128 && !p->evd_cluster) p->evd_chol = false;   // above 128 frames the Cholesky kernel only factors (the cluster kernel sweeps)
     std::vector<PtcSeg> ptc_segs;
     std::vector<int> ptc_cta_first;
     p->proj_tc = project_tc_eligible(p);

@@ -173,7 +173,9 @@ SMALL = [
     (40, 40, 16, 1, 1, 0.0, 0.0, synth.HARD_FIXED, 3, 1),         # all-ones window
     (40, 24, 24, 2, 2, 30.0, 0.0, synth.HARD_FIXED, 2, 0),        # Gaussian, no truncation
     (33, 65, 2, 2, 2, 8.0, 3.0, synth.HARD_FIXED, 1, 1),          # N = 2: one rotation, no blocks
-    (96, 80, 140, 2, 2, 20.0, 3.0, synth.HARD_ENERGY, 0, 0),      # N > 128: 3 pivots per lane, 2 Gram batches
+    (96, 80, 140, 2, 2, 20.0, 3.0, synth.HARD_ENERGY, 0, 0),      # N > 128, even: block-form tcgen05 Gram, global-memory Cholesky, Jacobi on 8-CTA clusters
+    (64, 48, 206, 1, 2, 20.0, 3.0, synth.SOFT_ENERGY, 0, 0),      # N = 206: 103 column pairs over eight CTAs (12 + 7 x 13), ragged row chunks
+    (64, 48, 131, 1, 2, 20.0, 3.0, synth.HARD_ENERGY, 0, 0),      # N > 128, odd: two-sided fp32 Jacobi (3 pivots per lane), 2 Gram batches
     (64, 48, 64, 2, 2, 14.0, 3.0, synth.SOFT_MEDIAN, 0, 0),       # method 3 (median rule) + sigmoid, cluster EVD path
     (64, 48, 40, 2, 2, 14.0, 3.0, synth.HARD_MEDIAN, 0, 1),       # hard median cut (fp64: a hard cut 40 dB down needs it)
     (50, 37, 24, 1, 2, 12.0, 3.0, synth.HARD_MEDIAN, 0, 1),       # median rule in the fp64 path
@@ -383,7 +385,7 @@ def test_deterministic_and_stream_and_host_path(lcf):
 
 def test_b200_kernels_are_selected(lcf):
     """The metric workloads must run on the tcgen05 / cluster kernels, not on the CUDA-core fallback."""
-    for ci, want in ((2, (1, 1, 1)), (4, (1, 1, 1)), (0, (0, 0, 1)), (3, (1, 0, 1))):
+    for ci, want in ((2, (1, 1, 1)), (4, (1, 1, 1)), (0, (0, 0, 1)), (3, (1, 1, 1))):
         cfg = synth.baseline_configs()[ci]
         d = cfg.data
         with lcf.Plan.from_spec(d.Nz, d.Nx, d.N, cfg.filt) as plan:
@@ -535,10 +537,10 @@ def test_plans_of_different_sizes_alive_together(lcf, oracle):
         check_pd(pd_d.cpu().numpy().astype(np.float64), o["PD"])
 
 
-@pytest.mark.parametrize("N,Nz,prec", [(64, 48, 0), (128, 32, 0), (50, 37, 0), (24, 32, 0), (140, 32, 0), (24, 32, 1)])
+@pytest.mark.parametrize("N,Nz,prec", [(64, 48, 0), (128, 32, 0), (50, 37, 0), (24, 32, 0), (140, 32, 0), (131, 32, 0), (24, 32, 1)])
 def test_non_convergence_is_reported(lcf, N, Nz, prec):
     """A sweep cap too small for the input must surface as LCF_ERR_NOT_CONVERGED from the host entry
-    points, the getters and lcf_get_converged -- on every EVD kernel (cluster block / pair kernels,
+    points, the getters and lcf_get_converged -- on every EVD kernel (cluster block / pair / 8-CTA kernels,
     single-CTA Cholesky kernel for odd shapes, two-sided fp32 / fp64 Jacobi) -- and must clear again."""
     import torch
     iq = synth.random_cube(Nz, 24, N, seed=31)
