@@ -80,29 +80,67 @@ __global__ void __launch_bounds__(256) ncc_mag_kernel(const float2* iq, int N, i
 }
 
 // Step 3.  CTA (chunk c, window k), thread k' = candidate cut (1-based k' = threadIdx.x + 1).  The chunk's pixels
-// stream through shared memory eight rows at a time; thread k' adds its I_T I_B, I_T^2, I_B^2.
+// stream through shared memory NCC_ROWS rows at a time (cp.async, two buffers); a row sits between NCC_FN zeros on
+// either side, so the clipping of I_T / I_B to 1..N is the padding and every thread adds ten taps with fixed bounds.
+constexpr int NCC_ROWS = 32;
+constexpr int NCC_PADL = 8;                // floats of zeros before a row (>= NCC_FN - 1, keeps rows 16-byte aligned)
+__device__ __forceinline__ void ncc_cp16(float* dst, const float* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void ncc_cp4(float* dst, const float* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
 __global__ void __launch_bounds__(256) ncc_sums_kernel(const float* mag, int N, int ncol, const WinBox* box, float* part /* [K][CHUNKS][3][N] */) {
-    extern __shared__ float ncc_rows[];                // [8][ncol]
+    extern __shared__ __align__(16) float ncc_rows[];  // [2][NCC_ROWS][RS]
     const int k = blockIdx.y, c = blockIdx.x, kk = threadIdx.x + 1;
+    const int RS = NCC_PADL + ((ncol + 3) & ~3) + 8;   // row stride: zeros, the row, zeros (>= NCC_FN)
     const WinBox bx = box[k];
     const long long q0 = (long long)bx.Pk * c / NCC_CHUNKS, q1 = (long long)bx.Pk * (c + 1) / NCC_CHUNKS;
-    const int t0 = kk - NCC_FN + 1 < 1 ? 1 : kk - NCC_FN + 1, b1 = kk + NCC_FN > N ? N : kk + NCC_FN;
+    for (int e = threadIdx.x; e < 2 * NCC_ROWS * RS; e += blockDim.x) ncc_rows[e] = 0.f;
+    __syncthreads();
+    const bool vec = (ncol & 3) == 0;
+    auto issue = [&](long long q, int buf) {
+        const int nr = q1 - q < NCC_ROWS ? (int)(q1 - q) : NCC_ROWS;
+        const float* src = mag + ((size_t)bx.tile_off + q) * ncol;
+        float* dst = ncc_rows + (size_t)buf * NCC_ROWS * RS + NCC_PADL;
+        if (vec) {
+            const int cpr = ncol >> 2;
+            for (int e = threadIdx.x; e < nr * cpr; e += blockDim.x) {
+                const int r = e / cpr, j = e - r * cpr;
+                ncc_cp16(dst + r * RS + 4 * j, src + (size_t)r * ncol + 4 * j);
+            }
+        } else {
+            for (int e = threadIdx.x; e < nr * ncol; e += blockDim.x) {
+                const int r = e / ncol, j = e - r * ncol;
+                ncc_cp4(dst + r * RS + j, src + (size_t)r * ncol + j);
+            }
+        }
+        asm volatile("cp.async.commit_group;\n" ::: "memory");
+    };
     float stb = 0.f, stt = 0.f, sbb = 0.f;
-    for (long long q = q0; q < q1; q += 8) {
-        const int nr = q1 - q < 8 ? (int)(q1 - q) : 8;
-        __syncthreads();
-        for (int e = threadIdx.x; e < nr * ncol; e += blockDim.x)
-            ncc_rows[e] = mag[((size_t)bx.tile_off + q) * ncol + e];      // rows are contiguous: one coalesced copy
+    int buf = 0;
+    if (q0 < q1) issue(q0, 0);
+    for (long long q = q0; q < q1; q += NCC_ROWS, buf ^= 1) {
+        const int nr = q1 - q < NCC_ROWS ? (int)(q1 - q) : NCC_ROWS;
+        if (q + NCC_ROWS < q1) {
+            issue(q + NCC_ROWS, buf ^ 1);
+            asm volatile("cp.async.wait_group 1;\n" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+        }
         __syncthreads();
         if (kk <= N - 1) {
-            for (int r = 0; r < nr; ++r) {
-                const float* row = ncc_rows + r * ncol;
+            const float* row = ncc_rows + (size_t)buf * NCC_ROWS * RS + NCC_PADL + (kk - 1);
+            for (int r = 0; r < nr; ++r, row += RS) {
                 float it = 0.f, ib = 0.f;
-                for (int i = t0; i <= kk; ++i) it += row[i - 1];
-                for (int i = kk + 1; i <= b1; ++i) ib += row[i - 1];
+#pragma unroll
+                for (int i = NCC_FN - 1; i >= 0; --i) it += row[-i];            // i = k - fn + 1 .. k, ascending
+#pragma unroll
+                for (int i = 1; i <= NCC_FN; ++i) ib += row[i];                 // i = k + 1 .. k + fn
                 stb = fmaf(it, ib, stb); stt = fmaf(it, it, stt); sbb = fmaf(ib, ib, sbb);
             }
         }
+        __syncthreads();                               // the buffer is refilled two iterations on
     }
     if (threadIdx.x < N) {
         float* o = part + ((size_t)k * NCC_CHUNKS + c) * 3 * N + threadIdx.x;
@@ -181,7 +219,16 @@ cudaError_t launch_ncc(lcf_plan* p, const float2* iq, cudaStream_t st) {
         e = cudaGetLastError();
     }
     if (e != cudaSuccess) return e;
-    ncc_sums_kernel<<<dim3(NCC_CHUNKS, p->K), 256, (size_t)8 * ncol * sizeof(float), st>>>(p->ncc_mag_d, N, ncol, p->box_d, p->ncc_part_d);
+    {
+        const int RS = NCC_PADL + ((ncol + 3) & ~3) + 8;
+        const size_t sm = (size_t)2 * NCC_ROWS * RS * sizeof(float);          // <= 70 KB at ncol = 256
+        const int thr = N <= 128 ? 128 : 256;
+        if (sm > 48 * 1024) {
+            e = set_max_dyn_smem(ncc_sums_kernel, p->smem_optin);
+            if (e != cudaSuccess) return e;
+        }
+        ncc_sums_kernel<<<dim3(NCC_CHUNKS, p->K), thr, sm, st>>>(p->ncc_mag_d, N, ncol, p->box_d, p->ncc_part_d);
+    }
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     ncc_argmin_kernel<<<p->K, 256, 0, st>>>(p->ncc_part_d, N, p->ncc_curve_d, p->cut_d);

@@ -100,6 +100,18 @@ __device__ __forceinline__ void ptc_sts128u(uint32_t addr, uint32_t x, uint32_t 
 }
 struct PtcMaps { CUtensorMap m[2]; };    // hi plane, lo plane
 
+// MAG epilogue helper: val = Re U (even lane) / Im U (odd lane) of the pair's pixel for 16 eigen-columns.  The even lane
+// returns |U| isig w of columns 0-7, the odd lane of columns 8-15 (each squares what it has, hands the partner the half it
+// needs: 8 shuffles and 8 square roots per lane instead of 16 and 16); sqrt as v * rsqrt(v), 2 ulp.
+__device__ __forceinline__ void ptc_mag8(const float (&val)[16], bool odd, const float* isg, float wpix, float (&s8)[8]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float lo2 = val[i] * val[i], hi2 = val[8 + i] * val[8 + i];
+        const float v = (odd ? hi2 : lo2) + __shfl_xor_sync(0xffffffffu, odd ? lo2 : hi2, 1);
+        s8[i] = (v > 1e-36f ? v * rsqrtf(v) : 0.f) * isg[(odd ? 8 : 0) + i] * wpix;
+    }
+}
+
 template <bool MAG>
 __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid_constant__ PtcMaps maps, PtcArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
@@ -246,28 +258,24 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc_kernel(const __grid
                     tmem_ld16(tlane + col + 128, vc);
                     tmem_ld16(tlane + col + 192, vd);
                     tmem_ld_wait();
-                    float mg[16];
+                    float val[16];
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
                         const float pr = __uint_as_float(va[i]) + __uint_as_float(vc[i]);
                         const float pi = __uint_as_float(vb[i]) + __uint_as_float(vd[i]);
                         const float po = __shfl_xor_sync(0xffffffffu, pi, 1);
-                        const float val = ((lane & 1) ? pr + po : pr - po) * unscale;   // odd row: Im U, even row: Re U
-                        if (MAG) {
-                            const float v2 = val * val;
-                            mg[i] = sqrtf(v2 + __shfl_xor_sync(0xffffffffu, v2, 1)) * isig_s[j * 16 + i] * wpix;
-                        } else {
-                            acc = fmaf(val, val, acc);
-                        }
+                        val[i] = ((lane & 1) ? pr + po : pr - po) * unscale;   // odd row: Im U, even row: Re U
+                        if (!MAG) acc = fmaf(val[i], val[i], acc);
                     }
-                    if (MAG && valid) {                      // the pair's even lane stores ranks 0-7 of the 16, the odd lane 8-15
+                    if (MAG) {                               // the pair's even lane stores ranks 0-7 of the 16, the odd lane 8-15
                         const bool odd = (lane & 1) != 0;
                         float s8[8];
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) s8[i] = odd ? mg[8 + i] : mg[i];
-                        float4* o4 = reinterpret_cast<float4*>(mrow + j * 16 + (odd ? 8 : 0));
-                        o4[0] = make_float4(s8[0], s8[1], s8[2], s8[3]);
-                        o4[1] = make_float4(s8[4], s8[5], s8[6], s8[7]);
+                        ptc_mag8(val, odd, isig_s + j * 16, wpix, s8);
+                        if (valid) {
+                            float4* o4 = reinterpret_cast<float4*>(mrow + j * 16 + (odd ? 8 : 0));
+                            o4[0] = make_float4(s8[0], s8[1], s8[2], s8[3]);
+                            o4[1] = make_float4(s8[4], s8[5], s8[6], s8[7]);
+                        }
                     }
                 }
                 tc_fence_before_sync();
@@ -454,27 +462,23 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) project_tc2_kernel(const __gri
                         tmem_ld16(tlane + col, va);
                         tmem_ld16(tlane + col + 64, vb);
                         tmem_ld_wait();
-                        float mg[16];
+                        float val[16];
 #pragma unroll
                         for (int i = 0; i < 16; ++i) {
                             const float pr = __uint_as_float(va[i]), pi = __uint_as_float(vb[i]);
                             const float po = __shfl_xor_sync(0xffffffffu, pi, 1);
-                            const float val = ((lane & 1) ? pr + po : pr - po) * unscale;   // odd row: Im U, even row: Re U
-                            if (MAG) {
-                                const float v2 = val * val;
-                                mg[i] = sqrtf(v2 + __shfl_xor_sync(0xffffffffu, v2, 1)) * isig_s[jb * 64 + j * 16 + i] * wpix;
-                            } else {
-                                acc = fmaf(val, val, acc);
-                            }
+                            val[i] = ((lane & 1) ? pr + po : pr - po) * unscale;   // odd row: Im U, even row: Re U
+                            if (!MAG) acc = fmaf(val[i], val[i], acc);
                         }
-                        if (MAG && valid) {
+                        if (MAG) {
                             const bool odd = (lane & 1) != 0;
                             float s8[8];
-#pragma unroll
-                            for (int i = 0; i < 8; ++i) s8[i] = odd ? mg[8 + i] : mg[i];
-                            float4* o4 = reinterpret_cast<float4*>(mrow + j * 16 + (odd ? 8 : 0));
-                            o4[0] = make_float4(s8[0], s8[1], s8[2], s8[3]);
-                            o4[1] = make_float4(s8[4], s8[5], s8[6], s8[7]);
+                            ptc_mag8(val, odd, isig_s + jb * 64 + j * 16, wpix, s8);
+                            if (valid) {
+                                float4* o4 = reinterpret_cast<float4*>(mrow + j * 16 + (odd ? 8 : 0));
+                                o4[0] = make_float4(s8[0], s8[1], s8[2], s8[3]);
+                                o4[1] = make_float4(s8[4], s8[5], s8[6], s8[7]);
+                            }
                         }
                     }
                 }
