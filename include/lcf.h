@@ -79,14 +79,25 @@ typedef enum {
                             sum_{i=k+1..k+5} |u_i| (clipped to 1..N), u_i = C_w v_i / sigma_i the left singular
                             vectors of the windowed data (fn = 5, w_i = 1; lowest k on ties;
                             DESIGN.md "Readings" 19).  Costs a third pass over the data                 */
-    LCF_SOFT_NCC = 14       /* sigmoid (Eq. 9) centred on the NCC c: methods 4 + 5 as the paper pairs them
+    LCF_SOFT_NCC = 14,      /* sigmoid (Eq. 9) centred on the NCC c: methods 4 + 5 as the paper pairs them
                                                                                        */
+    LCF_HARD_FIXED_TOP = 15,  /* the filter of LCF_HARD_FIXED, F = I - sum_{i<=k_fixed} v_i v_i^H, from the leading
+                            eigenpairs only (block subspace iteration on M = 16 vectors, or 32 where the cut needs
+                            them: DESIGN.md section 10, "partial EVD"; a departure from the paper's full-spectrum
+                            EVD).  Getters: the first M eigenvalues / eigenvectors are Ritz pairs,
+                            the other eigenvalues are reported as their mean (trace(R) - sum of the M) / (N - M),
+                            the other eigenvectors as zero columns; lcf_get_sweeps counts rounds of the iteration.
+                            Runs for precision 0, 40 <= N <= 224, k_fixed <= 26; other plans in this mode compute
+                            the same filter with the full EVD (lcf_get_work: evd_chol = 2 when it runs)   */
+    LCF_HARD_ENERGY_TOP = 16  /* the same for LCF_HARD_ENERGY: c from the leading eigenvalues and trace(R_k).  A
+                            window whose cut is not reached within 26 eigenvalues is reported like an
+                            unconverged EVD (LCF_ERR_NOT_CONVERGED: use LCF_HARD_ENERGY)                  */
 } lcf_thresh_mode;
 
 typedef struct {
     lcf_thresh_mode mode;
-    int k_fixed;        /* 0 <= k_fixed <= N (FIXED modes)                                      */
-    double energy_frac; /* in (0, 1) (ENERGY modes)                                             */
+    int k_fixed;        /* 0 <= k_fixed <= N (FIXED modes, FIXED_TOP)                           */
+    double energy_frac; /* in (0, 1) (ENERGY modes, ENERGY_TOP)                                 */
     double beta;        /* > 0 (SOFT modes: sigmoid sharpness; ADAPTIVE: the exponent of Eq. 10)  */
     int precision;      /* 0: fp32-grade Gram + fp32 EVD.  1: exact-product fp64 Gram + fp64 EVD
                            (single precision can hamper the EVD).  The projection
@@ -197,7 +208,7 @@ lcf_status lcf_get_stage_ms(lcf_plan* plan, float ms[5] /* HOST */);
 typedef struct {
     double gram_flops, proj_flops, hbm_bytes, sum_Pk;
     int launches;
-    int gram_tc, evd_chol, proj_tc;
+    int gram_tc, evd_chol, proj_tc;   /* kernels chosen: evd_chol 0 two-sided Jacobi, 1 Cholesky + one-sided Jacobi, 2 leading eigenpairs (the *_TOP modes) */
     double gram_tensor_flops, proj_tensor_flops;
 } lcf_work;
 lcf_status lcf_get_work(const lcf_plan* plan, lcf_work* out /* HOST */);

@@ -51,7 +51,10 @@
 enum { LCFO_HARD_FIXED = 0, LCFO_HARD_ENERGY = 1, LCFO_SOFT_FIXED = 2, LCFO_SOFT_ENERGY = 3,
        LCFO_HARD_MEDIAN = 4, LCFO_SOFT_MEDIAN = 5, LCFO_HARD_CURVATURE = 6, LCFO_SOFT_CURVATURE = 7,
        LCFO_SOFT_ADAPTIVE = 8, LCFO_HARD_SLOPE = 9, LCFO_SOFT_SLOPE = 10, LCFO_HARD_SLOPE_DB = 11, LCFO_SOFT_SLOPE_DB = 12,
-       LCFO_HARD_NCC = 13, LCFO_SOFT_NCC = 14 };
+       LCFO_HARD_NCC = 13, LCFO_SOFT_NCC = 14,
+       /* include/lcf.h's *_TOP modes name a way of computing (leading eigenpairs only), not another filter: here they
+        * ARE the definition, F = V diag(wt) V^H from the full decomposition with the hard weights of mode 0 / 1 */
+       LCFO_HARD_FIXED_TOP = 15, LCFO_HARD_ENERGY_TOP = 16 };
 
 int lcf_oracle_num_threads(void) {
 #ifdef _OPENMP
@@ -452,7 +455,7 @@ int lcf_oracle_window(const float *iq, int N, int Nx, int Nz, const double *gz, 
     lcf_oracle_gram(iq, N, Nx, Nz, gz, gx, R);
     int sweeps = lcf_oracle_jacobi(R, N, lam, V);
     int c = k_fixed;
-    if (mode == LCFO_HARD_ENERGY || mode == LCFO_SOFT_ENERGY) c = lcf_oracle_cutoff_energy(lam, N, frac);
+    if (mode == LCFO_HARD_ENERGY || mode == LCFO_SOFT_ENERGY || mode == LCFO_HARD_ENERGY_TOP) c = lcf_oracle_cutoff_energy(lam, N, frac);
     if (mode == LCFO_HARD_MEDIAN || mode == LCFO_SOFT_MEDIAN) c = lcf_oracle_cutoff_median(lam, N, cut_scale);
     if (mode == LCFO_HARD_CURVATURE || mode == LCFO_SOFT_CURVATURE) c = lcf_oracle_cutoff_curvature(lam, N, cut_scale);
     if (mode == LCFO_HARD_SLOPE || mode == LCFO_SOFT_SLOPE) c = lcf_oracle_cutoff_slope(lam, N, cut_scale);

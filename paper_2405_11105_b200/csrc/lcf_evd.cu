@@ -390,9 +390,10 @@ __global__ void __launch_bounds__(VB_WARPS * 32) vbuild_kernel(VbArgs a) {
     }
 }
 
-// diagnostic: F_k = V diag(wt) V^H (Eq. 4), double accumulation
+// diagnostic: F_k = V diag(wt) V^H (Eq. 4), double accumulation.  complement: the same filter written as
+// I - V diag(1 - wt) V^H, for the plans whose V holds only the leading eigenvectors (lcf_evd_top.cu: the others have wt = 1)
 template <typename T>
-__global__ void build_filters_kernel(const void* Vv, const double* wdd, double* F, int N, int Ns) {
+__global__ void build_filters_kernel(const void* Vv, const double* wdd, double* F, int N, int Ns, int complement) {
     using C = typename Cx2<T>::type;
     const int k = blockIdx.z;
     const C* V = reinterpret_cast<const C*>(Vv) + (size_t)k * N * Ns;
@@ -403,9 +404,11 @@ __global__ void build_filters_kernel(const void* Vv, const double* wdd, double* 
     for (int u = 0; u < N; ++u) {
         C va = V[(size_t)a_ * Ns + u], vb = V[(size_t)b_ * Ns + u];
         double ar = va.x, ai = va.y, br = vb.x, bi = vb.y;
-        fr += w[u] * (ar * br + ai * bi);
-        fi += w[u] * (ai * br - ar * bi);
+        const double wu = complement ? 1.0 - w[u] : w[u];
+        fr += wu * (ar * br + ai * bi);
+        fi += wu * (ai * br - ar * bi);
     }
+    if (complement) { fr = (a_ == b_ ? 1.0 : 0.0) - fr; fi = -fi; }
     double* o = F + ((size_t)k * N * N + (size_t)a_ * N + b_) * 2;
     o[0] = fr; o[1] = fi;
 }
@@ -473,8 +476,8 @@ cudaError_t launch_vbuild(lcf_plan* p, cudaStream_t st) {
 
 cudaError_t launch_build_filters(lcf_plan* p, cudaStream_t st) {
     dim3 blk(16, 16), grid((p->N + 15) / 16, (p->N + 15) / 16, p->K);
-    if (p->prec == 1) build_filters_kernel<double><<<grid, blk, 0, st>>>(p->V_d, p->wslot_dd_d, p->F_d, p->N, p->Ns);
-    else build_filters_kernel<float><<<grid, blk, 0, st>>>(p->V_d, p->wslot_dd_d, p->F_d, p->N, p->Ns);
+    if (p->prec == 1) build_filters_kernel<double><<<grid, blk, 0, st>>>(p->V_d, p->wslot_dd_d, p->F_d, p->N, p->Ns, p->evd_top ? 1 : 0);
+    else build_filters_kernel<float><<<grid, blk, 0, st>>>(p->V_d, p->wslot_dd_d, p->F_d, p->N, p->Ns, p->evd_top ? 1 : 0);
     return cudaGetLastError();
 }
 

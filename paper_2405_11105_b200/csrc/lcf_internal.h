@@ -164,6 +164,8 @@ struct lcf_plan {
     bool evd_chol = false, evd_cluster = false;   // cluster: Cholesky kernel, then one-sided Jacobi on 2-CTA clusters
     int ec_LD = 0;
     size_t ec_smem = 0, ecl_smem = 0;
+    bool evd_top = false;                         // LCF_HARD_*_TOP: block subspace iteration instead of a full EVD (lcf_evd_top.cu)
+    size_t et_smem = 0, et_smem_small = 0;
     float* ec_gfac_d = nullptr;             // [K][2][Ns][LD] Cholesky factor planes
     float* ec_shift_d = nullptr;            // [K]
     int* ec_nexp_d = nullptr;               // [K]
@@ -269,6 +271,10 @@ cudaError_t launch_gram_stream(lcf_plan* p, const float2* iq, int stride, cudaSt
 bool evd_chol_eligible(const lcf_plan* p);
 cudaError_t configure_evd_chol(lcf_plan* p);
 cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only);
+bool evd_top_mode(int mode);
+bool evd_top_eligible(const lcf_plan* p);
+cudaError_t configure_evd_top(lcf_plan* p);
+cudaError_t launch_evd_top(lcf_plan* p, cudaStream_t st);
 constexpr int ECL8_MAXN = 208;                // most frames of the 8-CTA cluster EVD (13 column pairs per CTA)
 bool evd_cluster_eligible(const lcf_plan* p);
 cudaError_t configure_evd_cluster(lcf_plan* p);
@@ -282,6 +288,10 @@ bool ncc_mode(int mode);
 cudaError_t launch_ncc(lcf_plan* p, const float2* iq, cudaStream_t st);
 // what the EVD kernels are told: under the NCC modes they run with every eigen-weight 1 (hard cut at 0), so that
 // B_k = V_k for the left singular vectors; lcf_ncc.cu then sets the cut-off, the weights and B_k
-inline int evd_mode(const lcf_plan* p) { return (p->thr.mode == LCF_HARD_NCC || p->thr.mode == LCF_SOFT_NCC) ? (int)LCF_HARD_FIXED : (int)p->thr.mode; }
+inline int evd_mode(const lcf_plan* p) {   // the rule the full-spectrum EVD kernels apply
+    if (p->thr.mode == LCF_HARD_NCC || p->thr.mode == LCF_SOFT_NCC || p->thr.mode == LCF_HARD_FIXED_TOP) return (int)LCF_HARD_FIXED;
+    if (p->thr.mode == LCF_HARD_ENERGY_TOP) return (int)LCF_HARD_ENERGY;
+    return (int)p->thr.mode;
+}
 inline int evd_kfixed(const lcf_plan* p) { return (p->thr.mode == LCF_HARD_NCC || p->thr.mode == LCF_SOFT_NCC) ? 0 : p->thr.k_fixed; }
 }  // namespace lcf

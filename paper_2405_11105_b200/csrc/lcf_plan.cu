@@ -154,11 +154,11 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
     if (!win || !thr) return LCF_ERR_INVALID_ARG;
     if (Nz < 1 || Nx < 1 || N < 2 || win->Kz < 1 || win->Kx < 1) return LCF_ERR_INVALID_ARG;
     if ((long long)Nz * Nx > (1LL << 30) || (long long)win->Kz * win->Kx > 65535) return LCF_ERR_INVALID_ARG;
-    if ((int)thr->mode < 0 || (int)thr->mode > 14 || (thr->precision != 0 && thr->precision != 1)) return LCF_ERR_INVALID_ARG;
-    const bool fixed = thr->mode == LCF_HARD_FIXED || thr->mode == LCF_SOFT_FIXED;
+    if ((int)thr->mode < 0 || (int)thr->mode > 16 || (thr->precision != 0 && thr->precision != 1)) return LCF_ERR_INVALID_ARG;
+    const bool fixed = thr->mode == LCF_HARD_FIXED || thr->mode == LCF_SOFT_FIXED || thr->mode == LCF_HARD_FIXED_TOP;
     const bool soft = thresh_is_soft(thr->mode);
     if (fixed && (thr->k_fixed < 0 || thr->k_fixed > N)) return LCF_ERR_INVALID_ARG;
-    const bool energy = thr->mode == LCF_HARD_ENERGY || thr->mode == LCF_SOFT_ENERGY;
+    const bool energy = thr->mode == LCF_HARD_ENERGY || thr->mode == LCF_SOFT_ENERGY || thr->mode == LCF_HARD_ENERGY_TOP;
     const bool median = thr->mode == LCF_HARD_MEDIAN || thr->mode == LCF_SOFT_MEDIAN ||
                         thr->mode == LCF_HARD_CURVATURE || thr->mode == LCF_SOFT_CURVATURE ||
                         thr->mode == LCF_HARD_SLOPE || thr->mode == LCF_SOFT_SLOPE ||
@@ -240,7 +240,12 @@ extern "C" lcf_status lcf_plan_create(lcf_plan** out, int Nz, int Nx, int N, con
         cudaGetLastError();
         p->evd_chol = false;
     }
-    if (!p->evd_chol) p->gram_tc = false;   // the tensor-core Gram leaves R in its data scale, which only these EVD kernels undo
+    p->evd_top = evd_top_eligible(p);
+    if (p->evd_top && configure_evd_top(p) != cudaSuccess) {
+        cudaGetLastError();
+        p->evd_top = false;
+    }
+    if (!p->evd_chol && !p->evd_top) p->gram_tc = false;   // the tensor-core Gram leaves R in its data scale, which only these EVD kernels undo
     std::vector<G2Seg> g2_segs;
     std::vector<int> g2_cta_first, g2_seg_first;
     p->gram_tc2 = gram_tc2_eligible(p);     // block form above 128 frames; its reduction undoes the data scale itself
@@ -398,10 +403,14 @@ static lcf_status filter_impl(lcf_plan* p, const void* iq_dev, float* pd_dev, cu
         if (e == cudaSuccess) run(1, cudaMemcpyAsync(p->amax_prev_d, p->amax_d, sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
     }
     mark(1);
-    if (e == cudaSuccess) run(2, p->evd_chol ? launch_evd_chol(p, st, p->evd_cluster) : launch_jacobi(p, st));
-    if (e == cudaSuccess && p->evd_cluster) run(2, launch_evd_cluster(p, st));
+    if (p->evd_top) {
+        if (e == cudaSuccess) run(2, launch_evd_top(p, st));
+    } else {
+        if (e == cudaSuccess) run(2, p->evd_chol ? launch_evd_chol(p, st, p->evd_cluster) : launch_jacobi(p, st));
+        if (e == cudaSuccess && p->evd_cluster) run(2, launch_evd_cluster(p, st));
+    }
     mark(2);
-    if (e == cudaSuccess && !p->evd_chol) run(3, launch_vbuild(p, st));
+    if (e == cudaSuccess && !p->evd_chol && !p->evd_top) run(3, launch_vbuild(p, st));
     if (e == cudaSuccess && ncc_mode(p->thr.mode)) run(3, launch_ncc(p, iq, st));
     mark(3);
     if (e == cudaSuccess) run(4, p->proj_tc ? launch_project_tc(p, iq, st) : launch_project(p, iq, st));
@@ -697,7 +706,7 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
     w->proj_flops = 8.0 * S * N * N;                 // dense N x N projector factor
     w->hbm_bytes = 8.0 * N * (double)p->P + 4.0 * (double)p->P;
     w->launches = ((p->gram_tc || p->gram_tc2 || p->proj_tc) ? 1 : 0) + ((p->proj_tc && p->ptc_pre) ? 1 : 0) + 2 + (p->evd_chol ? (p->evd_cluster ? 2 : 1) : 2) + (p->proj_tc ? 3 : 1) + 2;   // absmax, gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
-    w->gram_tc = (p->gram_tc || p->gram_tc2) ? 1 : 0; w->evd_chol = p->evd_chol ? 1 : 0; w->proj_tc = p->proj_tc ? 1 : 0;
+    w->gram_tc = (p->gram_tc || p->gram_tc2) ? 1 : 0; w->evd_chol = p->evd_top ? 2 : (p->evd_chol ? 1 : 0); w->proj_tc = p->proj_tc ? 1 : 0;
     w->gram_tensor_flops = 0.0; w->proj_tensor_flops = 0.0;
     for (int k = 0; k < p->K; ++k) {
         const WinBox& b = p->box_h[k];

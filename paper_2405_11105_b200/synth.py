@@ -20,7 +20,7 @@ from typing import Optional
 import numpy as np
 
 # threshold modes (values match include/lcf.h lcf_thresh_mode)
-HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE, HARD_SLOPE_DB, SOFT_SLOPE_DB, HARD_NCC, SOFT_NCC = range(15)
+HARD_FIXED, HARD_ENERGY, SOFT_FIXED, SOFT_ENERGY, HARD_MEDIAN, SOFT_MEDIAN, HARD_CURVATURE, SOFT_CURVATURE, SOFT_ADAPTIVE, HARD_SLOPE, SOFT_SLOPE, HARD_SLOPE_DB, SOFT_SLOPE_DB, HARD_NCC, SOFT_NCC, HARD_FIXED_TOP, HARD_ENERGY_TOP = range(17)
 
 
 @dataclass(frozen=True)
@@ -172,6 +172,18 @@ def rank_r_clutter(Nz: int, Nx: int, N: int, r: int, seed: int) -> np.ndarray:
     A = _cn(rng, (Nx * Nz, r))
     B = _cn(rng, (N, r))
     S = A @ B.conj().T                       # [P][N]
+    return np.ascontiguousarray(S.T.reshape(N, Nx, Nz)).astype(np.complex64)
+
+
+def graded_rank_cube(Nz: int, Nx: int, N: int, r: int, step_db: float, noise_db: float, seed: int) -> np.ndarray:
+    """r clutter components whose powers fall by step_db from one to the next, over white noise noise_db below the
+    strongest: a spectrum with r well separated leading eigenvalues and a flat floor (test input for the cut-off
+    rules that work on the leading eigenpairs).  complex64 [N][Nx][Nz]."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    A = _cn(rng, (Nx * Nz, r))
+    B, _ = np.linalg.qr(_cn(rng, (N, r)))
+    amp = 10.0 ** (-step_db * np.arange(r) / 20.0)
+    S = (A * amp) @ B.conj().T + 10.0 ** (noise_db / 20.0) * _cn(rng, (Nx * Nz, N))
     return np.ascontiguousarray(S.T.reshape(N, Nx, Nz)).astype(np.complex64)
 
 

@@ -50,7 +50,7 @@ def _create(lcf, Nz=8, Nx=8, N=4, Kz=1, Kx=1, sz=0.0, sx=0.0, tr=0.0, mode=0, k=
 
 
 @pytest.mark.parametrize("kw", [
-    dict(Nz=0), dict(Nx=-1), dict(N=1), dict(Kz=0), dict(Kx=0), dict(mode=15), dict(mode=-1), dict(mode=14, beta=0.0), dict(mode=11, cs=0.0), dict(mode=12, beta=0.0), dict(mode=8, beta=0.0), dict(mode=9, cs=0.0), dict(mode=10, cs=-2.0), dict(mode=10, beta=0.0), dict(mode=4, cs=0.0), dict(mode=5, cs=-1.0), dict(mode=6, cs=0.0),
+    dict(Nz=0), dict(Nx=-1), dict(N=1), dict(Kz=0), dict(Kx=0), dict(mode=17), dict(mode=-1), dict(mode=15, k=-1), dict(mode=16, frac=1.5), dict(mode=14, beta=0.0), dict(mode=11, cs=0.0), dict(mode=12, beta=0.0), dict(mode=8, beta=0.0), dict(mode=9, cs=0.0), dict(mode=10, cs=-2.0), dict(mode=10, beta=0.0), dict(mode=4, cs=0.0), dict(mode=5, cs=-1.0), dict(mode=6, cs=0.0),
     dict(k=-1), dict(k=5), dict(mode=1, frac=1.0), dict(mode=3, frac=0.0), dict(mode=2, beta=0.0),
     dict(prec=2), dict(sz=float("nan")), dict(tr=float("inf")),
 ])

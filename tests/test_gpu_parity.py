@@ -286,6 +286,104 @@ def test_ncc_cutoff_method4(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, mode, prec):
         check_pd(g["PD"], o["PD"])
 
 
+# ------------------------------------------------------------------ leading-eigenpair modes (partial EVD)
+# (synthetic spectra here keep the weakest rejected component within ~30 dB of the strongest: beyond that the fp32 Gram,
+# not the eigen-solver, sets the projector error -- the full-spectrum kernels fail the same gate on such inputs)
+def check_top(lcf, oracle, iq, filt, label, want_top=True, nblock=16):
+    """LCF_HARD_*_TOP against the oracle's full decomposition: the cut, the leading eigenvalues (the others are
+    reported as their mean: sum and order are checked), the clutter projector and the filter matrix on every
+    window, the image."""
+    import torch
+    N, Nx, Nz = iq.shape
+    o = oracle.run_config(iq, filt, want_V=True, want_F=True)
+    iq_d = torch.from_numpy(np.ascontiguousarray(iq)).cuda()
+    pd_d = torch.full((Nx, Nz), float("nan"), dtype=torch.float32, device="cuda")
+    with lcf.Plan.from_spec(Nz, Nx, N, filt) as plan:
+        assert (plan.work()["evd_chol"] == 2) == want_top, plan.work()
+        plan.filter(iq_d, pd_d)
+        torch.cuda.synchronize()
+        lam, c, V, F = plan.eigenvalues(), plan.cutoffs(), plan.eigenvectors(), plan.filters()
+        rounds = plan.sweeps()
+    assert np.array_equal(c, o["c"]), (c, o["c"])
+    lmax = o["lam"][:, :1]
+    nb = nblock if want_top else N
+    assert (np.abs(lam[:, :nb] - o["lam"][:, :nb]) / lmax).max() <= LAM_TOL
+    assert (np.diff(lam, axis=1) <= 0).all() and (lam >= 0).all()
+    assert (np.abs(lam.sum(axis=1) - o["lam"].sum(axis=1)) / lmax[:, 0]).max() <= LAM_TOL      # the trace
+    worst = 0.0
+    for k in range(lam.shape[0]):
+        ck = int(o["c"][k])
+        if 0 < ck < N:
+            e = projector_err(V[k], o["V"][k], ck)
+            assert e <= PROJ_TOL, f"{label} window {k}: projector err {e:.3e}"
+            worst = max(worst, e)
+        ef = float(np.linalg.norm(F[k] - o["F"][k]))            # hard weights: F = I - Pi_c, so this one is gated too
+        assert ef <= PROJ_TOL, f"{label} window {k}: filter err {ef:.3e}"
+    err = check_pd(pd_d.cpu().numpy().astype(np.float64), o["PD"])
+    print(f"[{label}] cuts {int(c.min())}..{int(c.max())}, rounds {int(rounds.min())}..{int(rounds.max())}, "
+          f"max projector err {worst:.2e}, PD err {err:.2e}")
+
+
+def test_top_modes_on_the_configs(lcf, oracle):
+    """Config 3 (200 frames, 192 windows, hard energy cut) and config 2 / 4 shapes through the leading-eigenpair modes."""
+    for ci in (3, 2, 4):
+        cfg = synth.baseline_configs()[ci]
+        iq = np.ascontiguousarray(synth.ensemble(synth.generate(cfg), cfg, 0))
+        check_top(lcf, oracle, iq, replace(cfg.filt, mode=synth.HARD_ENERGY_TOP, precision=0), f"{cfg.name} energy_top")
+
+
+TOP_CASES = [
+    # Nz, Nx, N, Kz, Kx, sigma, r, step_db, noise_db, mode, k_fixed, frac, block that settles it
+    (64, 48, 64, 2, 2, 14.0, 4, 10.0, -70.0, "fixed", 4, 0.0, 16),     # fixed count inside the small block
+    (64, 48, 100, 2, 1, 14.0, 12, 2.5, -60.0, "fixed", 12, 0.0, 32),   # fixed count 12 > 10: the block of 32
+    (64, 48, 64, 2, 2, 14.0, 5, 10.0, -70.0, "energy", 0, 0.9999, 16),  # energy rule, small block
+    (48, 40, 140, 1, 2, 14.0, 14, 1.0, -60.0, "energy", 0, 0.97, 32),  # 14 nearly equal components: the small block gives up, the second pass settles it; block-form Gram
+    (45, 40, 72, 1, 2, 12.0, 3, 15.0, -60.0, "energy", 0, 0.999, 16),  # odd Nz: FP32 Gram in raw units, FP32 projection
+    (64, 48, 131, 2, 1, 14.0, 3, 12.0, -60.0, "fixed", 2, 0.0, 16),    # odd N above 128 (padded slot count)
+    (64, 48, 206, 1, 2, 20.0, 6, 5.0, -60.0, "energy", 0, 0.999, 16),   # N = 206
+]
+
+
+@pytest.mark.parametrize("Nz,Nx,N,Kz,Kx,sigma,r,step_db,noise_db,rule,k,frac,nblock", TOP_CASES)
+def test_top_modes_shapes_and_blocks(lcf, oracle, Nz, Nx, N, Kz, Kx, sigma, r, step_db, noise_db, rule, k, frac, nblock):
+    iq = synth.graded_rank_cube(Nz, Nx, N, r, step_db, noise_db, seed=300 + N + r)
+    mode = synth.HARD_FIXED_TOP if rule == "fixed" else synth.HARD_ENERGY_TOP
+    f = synth.FilterSpec(Kz, Kx, sigma, sigma, 3.0, mode, k_fixed=k, energy_frac=frac if frac else 0.995, precision=0)
+    check_top(lcf, oracle, iq, f, f"top {rule} N={N} r={r}", nblock=nblock)
+
+
+def test_top_modes_fall_back_to_the_full_evd(lcf, oracle):
+    """Plans the subspace iteration does not take (fp64, short ensembles, a fixed count beyond the block) compute the
+    same filter with the full-spectrum kernels."""
+    for (N, prec, k) in ((64, 1, 3), (24, 0, 3), (64, 0, 30)):
+        iq = synth.graded_rank_cube(48, 40, N, max(k, 3), 6.0 if k < 10 else 1.0, -50.0 if k < 10 else -45.0, seed=400 + N + k)
+        f = synth.FilterSpec(2, 1, 12.0, 12.0, 3.0, synth.HARD_FIXED_TOP, k_fixed=k, precision=prec)
+        check_top(lcf, oracle, iq, f, f"top fallback N={N} prec={prec} k={k}", want_top=False)
+
+
+def test_top_modes_report_what_they_cannot_settle(lcf):
+    """White noise has no leading subspace: the energy cut lies far beyond the block of 32 and a fixed cut inside the
+    flat spectrum does not separate -- both surface as LCF_ERR_NOT_CONVERGED, and a zero ensemble is fine."""
+    import torch
+    iq = synth.random_cube(32, 24, 64, seed=77)
+    iq_d = torch.from_numpy(iq).cuda()
+    pd_d = torch.empty((24, 32), dtype=torch.float32, device="cuda")
+    for mode, k in ((synth.HARD_ENERGY_TOP, 0), (synth.HARD_FIXED_TOP, 5)):
+        f = synth.FilterSpec(1, 2, 10.0, 10.0, 3.0, mode, k_fixed=k, energy_frac=0.9, precision=0)
+        with lcf.Plan.from_spec(32, 24, 64, f) as plan:
+            plan.filter(iq_d, pd_d)
+            assert plan.unconverged() == 2
+            with pytest.raises(lcf.LcfError) as ei:
+                plan.eigenvalues()
+            assert ei.value.status == lcf.ERR_NOT_CONVERGED
+            plan.filter(torch.zeros_like(iq_d), pd_d)       # all-zero data: nothing to iterate on, no error
+            assert plan.unconverged() == 0
+            assert float(pd_d.abs().max()) == 0.0
+            plan.set_max_sweeps(1)                          # a round cap too small for any input
+            plan.filter(iq_d, pd_d)
+            assert plan.unconverged() == 2
+
+
 def test_allpass_and_allstop(lcf, oracle):
     iq = synth.random_cube(32, 24, 12, seed=5)
     f0 = synth.FilterSpec(2, 2, 8.0, 8.0, 3.0, synth.HARD_FIXED, k_fixed=0)

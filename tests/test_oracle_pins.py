@@ -593,3 +593,24 @@ def test_ncc_mode_runs_like_fixed_cut(oracle):
             w = oracle.window(iq, gz[kz], gx[0], mode_fix, k_fixed=k, beta=0.7)
             PD += w["PDk"] / w["mean"]
         assert np.allclose(a["PD"], PD, rtol=1e-12)
+
+
+def test_top_modes_are_the_hard_modes_on_the_oracle_side(oracle):
+    """LCF_HARD_FIXED_TOP / LCF_HARD_ENERGY_TOP name a way of computing (leading eigenpairs only, include/lcf.h), not
+    another filter: the oracle's answer for them is its answer for LCF_HARD_FIXED / LCF_HARD_ENERGY, from the full
+    decomposition (Eq. 4).  Pinned independently of the mode plumbing: the image of a hard cut is the
+    slow-time power of (I - Pi_c) applied to the windowed data, Pi_c from numpy.linalg.eigh of the oracle's own R."""
+    cfg = synth.scaled_config(synth.baseline_configs()[0], Nz=24, Nx=20, N=16, n_frames=16)
+    iq = synth.generate(cfg)
+    for top, base, k in ((oracle.HARD_FIXED_TOP, oracle.HARD_FIXED, 3), (oracle.HARD_ENERGY_TOP, oracle.HARD_ENERGY, 0)):
+        a = oracle.run(iq, 2, 1, 8.0, 8.0, 3.0, top, k_fixed=k, frac=0.99, want_R=True, want_F=True)
+        b = oracle.run(iq, 2, 1, 8.0, 8.0, 3.0, base, k_fixed=k, frac=0.99, want_F=True)
+        assert np.array_equal(a["c"], b["c"]) and np.array_equal(a["PD"], b["PD"]) and np.array_equal(a["F"], b["F"])
+        for kz in range(2):
+            lam, U = np.linalg.eigh(a["R"][kz])
+            lam, U = lam[::-1], U[:, ::-1]
+            c = int(a["c"][kz])
+            if top == oracle.HARD_ENERGY_TOP:
+                assert c == int(np.searchsorted(np.cumsum(lam), 0.99 * lam.sum(), side="right") + 1)
+            F = np.eye(16) - U[:, :c] @ U[:, :c].conj().T
+            assert np.abs(a["F"][kz] - F).max() <= 1e-10
