@@ -55,7 +55,6 @@ struct EcArgs {
     int chol_only;                // 1: stop after the Cholesky factor and write it to gfac / shift (cluster Jacobi follows)
     float* gfac;                  // [K][2][Ns][LD] real plane, imaginary plane of G, column-major
     float* shift;                 // [K] delta, or -1 for an all-zero matrix
-    int glob;                     // 1: the matrix does not fit shared memory (N > 128): factor it in place in gfac (global memory, L2-resident)
     int* nexp;                    // [K] power-of-two exponent this kernel scaled R_k by (0 when R carries the tensor-core data scale)
 };
 
@@ -93,7 +92,7 @@ __device__ __forceinline__ float ec_hsum(unsigned long long v) {
     return x + y;
 }
 
-template <int NC, bool FULL>
+template <int NC, bool FULL, bool GLOB>
 __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double wnorm_sh;                                      // normalisation of the adaptive weights (method 6)
@@ -101,9 +100,11 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int k = blockIdx.x;
     // planar storage: real and imaginary parts of column u at Gr/Gi + u*LD (LD floats, multiple of 4)
-    float* Gr = a.glob ? a.gfac + (size_t)k * 2 * Ns * LD : reinterpret_cast<float*>(smem_raw);   // [Ns][LD]
+    // (GLOB: the factor does not fit shared memory -- N > 128 -- and is built in place in gfac, global memory, L2-resident;
+    // a template parameter, so that the shared-memory variant keeps shared-space loads and stores)
+    float* Gr = GLOB ? a.gfac + (size_t)k * 2 * Ns * LD : reinterpret_cast<float*>(smem_raw);   // [Ns][LD]
     float* Gi = Gr + (size_t)Ns * LD;                                // [Ns][LD]
-    float* lam_s = a.glob ? reinterpret_cast<float*>(smem_raw) : Gi + (size_t)Ns * LD;            // [Ns] eigenvalue of slot u
+    float* lam_s = GLOB ? reinterpret_cast<float*>(smem_raw) : Gi + (size_t)Ns * LD;            // [Ns] eigenvalue of slot u
     float* inv_s = lam_s + Ns;                                       // [Ns] 1 / |g_u|
     float* wsl = inv_s + Ns;                                         // [Ns] eigen-weight of slot u
     float* red = wsl + Ns;                                           // [32]
@@ -164,14 +165,20 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         // every warp reduces the 16 warp keys.
         const int nchc = (N + 3) >> 2;                               // 4-row chunks per column
         const unsigned KM = N > 128 ? 255u : 127u;                   // row index bits of a pivot key
-        float* dgs = lam_s;                                          // [N] current diagonal of the Schur complement, -1 once eliminated
-        unsigned* wkey = reinterpret_cast<unsigned*>(red);           // [16] per-warp pivot keys
+        // Between two barriers a warp both reads what the step needs from the others (the 16 warp keys, the pivot's
+        // diagonal entry) and writes what the next step needs; a warp that runs a whole step ahead of a slow one must
+        // not change what the slow one still has to read.  So the warp keys alternate between two sets by step
+        // parity, and the diagonal of an eliminated row is left in place (its flag elim[] is what marks it).
+        float* dgs = lam_s;                                          // [N] current diagonal of the Schur complement
+        int* elim = reinterpret_cast<int*>(wsl);                     // [N] 1 once the row is a pivot (wsl is free until the epilogue)
+        unsigned* wkey = reinterpret_cast<unsigned*>(red);           // [2][16] per-warp pivot keys, set (j & 1) read at step j
         int* elist = alist;                                          // [N] pivot of step t = slot of Cholesky column t
         {
             unsigned key = 0u;
             if (tid < N) {
                 const float d = fmaxf(Gr[(size_t)tid * LD + tid], 0.f);
                 dgs[tid] = d;
+                elim[tid] = 0;
                 key = (__float_as_uint(d) & ~KM) | (KM - (unsigned)tid);
             }
             key = __reduce_max_sync(0xffffffffu, key);
@@ -181,7 +188,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         for (int jb = 0; jb < N; jb += EC_NB) {
             const int je = jb + EC_NB < N ? jb + EC_NB : N;
             for (int j = jb; j < je; ++j) {
-                unsigned kk = lane < EC_THREADS / 32 ? wkey[lane] : 0u;
+                unsigned kk = lane < EC_THREADS / 32 ? wkey[(j & 1) * 16 + lane] : 0u;
                 kk = __reduce_max_sync(0xffffffffu, kk);
                 const int pv = (int)(KM - (kk & KM));
                 unsigned key = 0u;
@@ -200,8 +207,8 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
                     }
                     const float d = dgs[i];
                     float vr = 0.f, vi = 0.f;                        // Cholesky column pi_j is zero in eliminated rows
-                    if (i == pv) { vr = dsq; dgs[i] = -1.f; }
-                    else if (d >= 0.f) {
+                    if (i == pv) { vr = dsq; elim[i] = 1; }
+                    else if (!elim[i]) {
                         vr = (Gr[(size_t)pv * LD + i] - sr) * sc;
                         vi = (Gi[(size_t)pv * LD + i] - si) * sc;
                         const float nd = fmaxf(d - (vr * vr + vi * vi), 0.f);
@@ -213,7 +220,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
                     if (tid == 0) elist[j] = pv;
                 }
                 key = __reduce_max_sync(0xffffffffu, key);
-                if (lane == 0) wkey[warp] = key;
+                if (lane == 0) wkey[((j + 1) & 1) * 16 + warp] = key;
                 __syncthreads();
             }
             if (je < N) {
@@ -233,7 +240,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
                         }
                     }
                     for (int l = warp; l < N; l += EC_THREADS / 32) {
-                        if (dgs[l] < 0.f) continue;                  // already a Cholesky column
+                        if (elim[l]) continue;                       // already a Cholesky column
                         if (ch < nchc) {
                             float* cr = Gr + (size_t)l * LD + 4 * ch;
                             float* ci = Gi + (size_t)l * LD + 4 * ch;
@@ -257,7 +264,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         }
         if (a.chol_only) {
             float* gout = a.gfac + (size_t)k * 2 * Ns * LD;
-            if (!a.glob) for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) gout[e] = Gr[e];
+            if (!GLOB) for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) gout[e] = Gr[e];
             if (tid == 0) a.shift[k] = delta;
             return;
         }
@@ -351,7 +358,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         __syncthreads();
         if (a.chol_only) {
             float* gout = a.gfac + (size_t)k * 2 * Ns * LD;
-            if (!a.glob) for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) gout[e] = Gr[e];
+            if (!GLOB) for (int e = tid; e < 2 * Ns * LD; e += EC_THREADS) gout[e] = Gr[e];
             if (tid == 0) a.shift[k] = -1.f;
             return;
         }
@@ -448,7 +455,7 @@ cudaError_t configure_evd_chol(lcf_plan* p) {
     p->ec_smem = ec_smem_bytes(p->Ns, p->ec_LD, p->N > 128);
     if (p->ec_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaSuccess;
-#define EC_SET(NC, FULL) if (e == cudaSuccess) e = set_max_dyn_smem(evd_chol_kernel<NC, FULL>, p->smem_optin)
+#define EC_SET(NC, FULL) if (e == cudaSuccess) e = set_max_dyn_smem(evd_chol_kernel<NC, FULL, false>, p->smem_optin)
     EC_SET(1, false); EC_SET(2, false); EC_SET(3, false); EC_SET(4, false);
     EC_SET(1, true); EC_SET(2, true); EC_SET(3, true); EC_SET(4, true);
 #undef EC_SET
@@ -464,16 +471,15 @@ cudaError_t launch_evd_chol(lcf_plan* p, cudaStream_t st, bool chol_only) {
     a.wslot = p->wslot_d; a.wslot_dd = p->wslot_dd_d; a.wt = p->wt_d;
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
     a.mode = evd_mode(p); a.k_fixed = evd_kfixed(p); a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
-    a.glob = p->N > 128 ? 1 : 0;
-    if (a.glob) {                                                    // factor only (chol_only is implied: see evd_chol_eligible)
+    if (p->N > 128) {                                                // factor only (chol_only is implied: see evd_chol_eligible)
         if (!chol_only) return cudaErrorInvalidConfiguration;
-        evd_chol_kernel<1, false><<<p->K, EC_THREADS, p->ec_smem, st>>>(a);
+        evd_chol_kernel<1, false, true><<<p->K, EC_THREADS, p->ec_smem, st>>>(a);
         return cudaGetLastError();
     }
     const int nch = (p->N + 3) / 4, nc = (nch + 7) / 8;
     const bool full = (p->N % 32) == 0;
-#define EC_RUN(NC) do { if (full) evd_chol_kernel<NC, true><<<p->K, EC_THREADS, p->ec_smem, st>>>(a); \
-                        else evd_chol_kernel<NC, false><<<p->K, EC_THREADS, p->ec_smem, st>>>(a); } while (0)
+#define EC_RUN(NC) do { if (full) evd_chol_kernel<NC, true, false><<<p->K, EC_THREADS, p->ec_smem, st>>>(a); \
+                        else evd_chol_kernel<NC, false, false><<<p->K, EC_THREADS, p->ec_smem, st>>>(a); } while (0)
     switch (nc) { case 1: EC_RUN(1); break; case 2: EC_RUN(2); break; case 3: EC_RUN(3); break; default: EC_RUN(4); break; }
 #undef EC_RUN
     return cudaGetLastError();

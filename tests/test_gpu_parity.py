@@ -571,6 +571,34 @@ def test_filter_batch_two_lanes_matches_single_calls(lcf):
         plan.filter_batch([], [])
 
 
+@pytest.mark.parametrize("ci", [4, 2])
+def test_filter_batch_three_lanes_at_full_size(lcf, ci):
+    """The configuration bench.py times: lcf_filter_batch over many ensembles at the full size of config 4 (100 windows of
+    100 frames: 200 cluster CTAs per EVD, more than the SMs) and config 2, with the kernels of three ensembles in
+    flight -- bit for bit the images of single calls, no error, twice in a row."""
+    import torch
+    cfg = synth.baseline_configs()[ci]
+    d = cfg.data
+    seq_d = torch.from_numpy(synth.generate(cfg)).cuda()
+    n_e = max(cfg.n_ensembles, 1)
+    views = [seq_d[e * cfg.stride:e * cfg.stride + d.N] for e in range(n_e)] if n_e > 1 else [seq_d[:d.N]]
+    n_run = 32 if n_e > 1 else 8
+    with lcf.Plan.from_spec(d.Nz, d.Nx, d.N, cfg.filt) as plan:
+        single = []
+        for v in views:
+            pd = torch.empty((d.Nx, d.Nz), dtype=torch.float32, device="cuda")
+            plan.filter(v, pd)
+            single.append(pd)
+        torch.cuda.synchronize()
+        for _ in range(2):
+            outs = [torch.full((d.Nx, d.Nz), float("nan"), dtype=torch.float32, device="cuda") for _ in range(n_run)]
+            plan.filter_batch([views[i % len(views)] for i in range(n_run)], outs)
+            torch.cuda.synchronize()
+            for i, o in enumerate(outs):
+                assert torch.equal(o, single[i % len(views)]), i
+        assert plan.unconverged() == 0
+
+
 @pytest.mark.parametrize("N,stride,Nz,Nx", [(100, 50, 96, 64), (64, 5, 64, 48), (128, 16, 64, 48), (48, 40, 64, 48)])
 def test_sliding_window_stream_reuses_the_gram(lcf, oracle, N, stride, Nz, Nx):
     """lcf_filter_stream (sliding packets): ensemble e+1 = ensemble e advanced by `stride` frames; only the
