@@ -63,7 +63,7 @@ def parse_args():
 
 def workload_name(cfg) -> str:
     d, f = cfg.data, cfg.filt
-    mode = {0: "hard_fixed", 1: "hard_energy", 2: "soft_fixed", 3: "soft_energy", 4: "hard_median", 5: "soft_median", 6: "hard_curvature", 7: "soft_curvature", 8: "soft_adaptive", 9: "hard_slope", 10: "soft_slope", 11: "hard_slope_db", 12: "soft_slope_db", 13: "hard_ncc", 14: "soft_ncc"}[f.mode]
+    mode = {0: "hard_fixed", 1: "hard_energy", 2: "soft_fixed", 3: "soft_energy", 4: "hard_median", 5: "soft_median", 6: "hard_curvature", 7: "soft_curvature", 8: "soft_adaptive", 9: "hard_slope", 10: "soft_slope", 11: "hard_slope_db", 12: "soft_slope_db", 13: "hard_ncc", 14: "soft_ncc", 15: "hard_fixed_top", 16: "hard_energy_top"}[f.mode]
     return (f"{cfg.name}: IQ {d.Nz}x{d.Nx}x{d.N} complex64, {f.Kz}x{f.Kx} windows sigma={f.sigma_z:g} "
             f"trunc={f.trunc:g}, {mode}, precision={f.precision}")
 
@@ -544,7 +544,7 @@ def run_ours(args, cfg):
         context = {"note": "synthetic IQ of the paper's shapes, hard fixed cut k = 5, windows over the full field of view (trunc = 0), "
                            "sigma = 0.75 x window spacing; paper (RTX A6000 + Xeon W-2265, MATLAB, PAPER.md:198,212,224): "
                            "global 2.4-2.6 ms, 2x2 15.6-16.6 ms, 3x3 35.2-39.8 ms per packet of 50",
-                   "ms_per_packet": {}, "ms_per_packet_leading_eigenpairs": {}}
+                   "ms_per_packet": {}}
         base = synth.baseline_configs()[1]
         for (name, Nz, Nx) in (("phantom_196x180", 196, 180), ("kidney_180x180", 180, 180), ("liver_177x173", 177, 173)):
             for Np_ in (50, 70, 90):
@@ -559,9 +559,6 @@ def run_ours(args, cfg):
                         c = synth.Config(f"{name}_N{Np_}_K{Kg}x{Kg}", dsp, f)
                         r = quick_latency(lcf, torch, c, seq, steps=5, warmup=2)
                         context["ms_per_packet"][c.name] = round(r["ms"], 4)
-                        ct = _rep(c, filt=_rep(f, mode=synth.HARD_FIXED_TOP))       # the same cut from the leading eigenpairs only
-                        rt = quick_latency(lcf, torch, ct, seq, steps=5, warmup=2)
-                        context["ms_per_packet_leading_eigenpairs"][c.name] = round(rt["ms"], 4) if rt["unconverged_windows"] == 0 else "not settled (cut inside a flat spectrum)"
                 except Exception as ex:
                     context["ms_per_packet"][f"{name}_N{Np_}"] = repr(ex)
 
