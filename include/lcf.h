@@ -99,9 +99,10 @@ typedef struct {
     int k_fixed;        /* 0 <= k_fixed <= N (FIXED modes, FIXED_TOP)                           */
     double energy_frac; /* in (0, 1) (ENERGY modes, ENERGY_TOP)                                 */
     double beta;        /* > 0 (SOFT modes: sigmoid sharpness; ADAPTIVE: the exponent of Eq. 10)  */
-    int precision;      /* 0: fp32-grade Gram + fp32 EVD.  1: exact-product fp64 Gram + fp64 EVD
-                           (single precision can hamper the EVD).  The projection
-                           is fp32-grade in both.  "fp32-grade": on the tensor-core kernels
+    int precision;      /* 0: fp32-grade Gram, EVD and projection.  1: double precision throughout -- exact-product
+                           fp64 Gram, fp64 EVD, fp64 projection (single precision can hamper the
+                           EVD of long packets; "a double precision may be essential"); the image is still
+                           returned as float.  "fp32-grade": on the tensor-core kernels
                            (even Nz) each fp32 operand, scaled by a power of two taken
                            from the ensemble's largest sample, is the sum of two fp16 numbers (22
                            significant bits) and products accumulate in fp32 (DESIGN.md section

@@ -256,6 +256,7 @@ cudaError_t launch_vbuild(lcf_plan* p, cudaStream_t st);
 cudaError_t launch_project(lcf_plan* p, const float2* iq, cudaStream_t st);
 cudaError_t launch_combine(lcf_plan* p, float* pd, cudaStream_t st);
 cudaError_t launch_build_filters(lcf_plan* p, cudaStream_t st);
+cudaError_t launch_project_dd(lcf_plan* p, const float2* iq, cudaStream_t st);
 cudaError_t configure_gram(lcf_plan* p);     // each: opt-in shared memory size, launch geometry
 cudaError_t configure_evd(lcf_plan* p);
 cudaError_t configure_project(lcf_plan* p);

@@ -413,7 +413,7 @@ static lcf_status filter_impl(lcf_plan* p, const void* iq_dev, float* pd_dev, cu
     if (e == cudaSuccess && !p->evd_chol && !p->evd_top) run(3, launch_vbuild(p, st));
     if (e == cudaSuccess && ncc_mode(p->thr.mode)) run(3, launch_ncc(p, iq, st));
     mark(3);
-    if (e == cudaSuccess) run(4, p->proj_tc ? launch_project_tc(p, iq, st) : launch_project(p, iq, st));
+    if (e == cudaSuccess) run(4, p->prec == 1 ? launch_project_dd(p, iq, st) : (p->proj_tc ? launch_project_tc(p, iq, st) : launch_project(p, iq, st)));
     mark(4);
     if (e == cudaSuccess) run(5, launch_combine(p, pd_dev, st));
     mark(5);
@@ -706,7 +706,7 @@ extern "C" lcf_status lcf_get_work(const lcf_plan* p, lcf_work* w) {
     w->proj_flops = 8.0 * S * N * N;                 // dense N x N projector factor
     w->hbm_bytes = 8.0 * N * (double)p->P + 4.0 * (double)p->P;
     w->launches = ((p->gram_tc || p->gram_tc2 || p->proj_tc) ? 1 : 0) + ((p->proj_tc && p->ptc_pre) ? 1 : 0) + 2 + (p->evd_chol ? (p->evd_cluster ? 2 : 1) : 2) + (p->proj_tc ? 3 : 1) + 2;   // absmax, gram+reduce, evd(+V build), projection(+pack, finish), alpha, combine
-    w->gram_tc = (p->gram_tc || p->gram_tc2) ? 1 : 0; w->evd_chol = p->evd_top ? 2 : (p->evd_chol ? 1 : 0); w->proj_tc = p->proj_tc ? 1 : 0;
+    w->gram_tc = (p->gram_tc || p->gram_tc2) ? 1 : 0; w->evd_chol = p->evd_top ? 2 : (p->evd_chol ? 1 : 0); w->proj_tc = (p->proj_tc && p->prec == 0) ? 1 : 0;
     w->gram_tensor_flops = 0.0; w->proj_tensor_flops = 0.0;
     for (int k = 0; k < p->K; ++k) {
         const WinBox& b = p->box_h[k];

@@ -182,6 +182,93 @@ __global__ void __launch_bounds__(256, 1) project_kernel(ProjArgs a) {
     }
 }
 
+// 4a in double (precision = 1: "a double precision may be essential"): the same contraction on the FP64
+// pipe, B_k = V_k diag(wt) formed on the fly from the fp64 eigenvectors and weights.  CTA = one ProjItem (<= 64 pixels);
+// thread (tp, tc) of a 16 x 16 grid keeps pixels tp + 16 i and columns tc + 16 j (i, j < 4) of a 64-column tile in
+// registers; frames stream through shared memory PDD_KT at a time (converted to double on the way in); the squared
+// magnitudes are summed over the columns of a tile in the thread, over tiles in the thread, over tc in shared memory.
+constexpr int PDD_KT = 8;
+__global__ void __launch_bounds__(256) project_dd_kernel(const float2* iq, int N, int Ns, int Nz, int Nx, long long P, const double2* V,
+                                                        const double* wdd, const WinBox* box, const ProjItem* items, const double* gz,
+                                                        const double* gx, float* tiles, float* tsum) {
+    __shared__ double2 Ss[PDD_KT][64], Bs[PDD_KT][64];
+    __shared__ double red[16][64];
+    __shared__ long long poff[64];
+    const int tid = threadIdx.x, tp = tid & 15, tc = tid >> 4;
+    const ProjItem it = items[blockIdx.x];
+    const WinBox bx = box[it.k];
+    if (tid < 64) {
+        const int q = it.q0 + tid;
+        long long off = -1;
+        if (q < it.q1) { const int xr = q / bx.Lz, zr = q - xr * bx.Lz; off = (long long)(bx.x0 + xr) * Nz + (bx.z0 + zr); }
+        poff[tid] = off;
+    }
+    __syncthreads();
+    const double2* Vk = V + (size_t)it.k * N * Ns;
+    const double* wk = wdd + (size_t)it.k * Ns;
+    double psum[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int c0 = 0; c0 < Ns; c0 += 64) {
+        double ar[4][4], ai[4][4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) ar[i][j] = ai[i][j] = 0.0;
+        for (int t0 = 0; t0 < N; t0 += PDD_KT) {
+            for (int e = tid; e < PDD_KT * 64; e += 256) {
+                const int tt = e >> 6, x = e & 63, t = t0 + tt;
+                double2 sv = make_double2(0.0, 0.0), bv = make_double2(0.0, 0.0);
+                if (t < N) {
+                    if (poff[x] >= 0) { const float2 f = iq[(size_t)t * P + poff[x]]; sv = make_double2(f.x, f.y); }
+                    const int u = c0 + x;
+                    if (u < Ns) { const double2 v = Vk[(size_t)t * Ns + u]; const double w = wk[u]; bv = make_double2(v.x * w, v.y * w); }
+                }
+                Ss[tt][x] = sv; Bs[tt][x] = bv;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int tt = 0; tt < PDD_KT; ++tt) {
+                double2 s[4], b[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) { s[i] = Ss[tt][tp + 16 * i]; b[i] = Bs[tt][tc + 16 * i]; }
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        ar[i][j] = fma(s[i].x, b[j].x, fma(-s[i].y, b[j].y, ar[i][j]));
+                        ai[i][j] = fma(s[i].x, b[j].y, fma(s[i].y, b[j].x, ai[i][j]));
+                    }
+            }
+            __syncthreads();
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) psum[i] += ar[i][j] * ar[i][j] + ai[i][j] * ai[i][j];
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) red[tc][tp + 16 * i] = psum[i];
+    __syncthreads();
+    if (tid < 64) {
+        double s = 0.0;
+        for (int c = 0; c < 16; ++c) s += red[c][tid];
+        const int q = it.q0 + tid;
+        float val = 0.f;
+        if (q < it.q1) {
+            const int xr = q / bx.Lz, zr = q - xr * bx.Lz;
+            const double w = gz[(size_t)bx.kz * Nz + bx.z0 + zr] * gx[(size_t)bx.kx * Nx + bx.x0 + xr];
+            val = (float)(w * w * s);
+            tiles[bx.tile_off + q] = val;
+        }
+        // the CTA's sum of its (rounded) pixel values, fixed order, as project_kernel forms it
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xffffffffu, val, o);
+        __shared__ float wsum[2];
+        if ((tid & 31) == 0) wsum[tid >> 5] = val;
+        asm volatile("bar.sync 1, 64;\n" ::: "memory");
+        if (tid == 0) tsum[blockIdx.x] = wsum[0] + wsum[1];
+    }
+}
+
 __global__ void alpha_kernel(const float* tsum, const int* pfirst, long long P, double* mean, float* alpha) {
     const int k = blockIdx.x, tid = threadIdx.x;
     __shared__ double sh[128];
@@ -246,6 +333,13 @@ cudaError_t launch_project(lcf_plan* p, const float2* iq, cudaStream_t st) {
     a.iq = iq; a.N = p->N; a.Ns = p->Ns; a.Nz = p->Nz; a.Nx = p->Nx; a.P = p->P; a.B = p->B_d; a.box = p->box_d;
     a.items = p->pitems_d; a.gz = p->gz_d; a.gx = p->gx_d; a.tiles = p->tiles_d; a.tsum = p->tsum_d; a.nct = p->proj_nct;
     project_kernel<<<p->n_pitems, p->proj_threads, p->proj_smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_project_dd(lcf_plan* p, const float2* iq, cudaStream_t st) {
+    if (p->n_pitems == 0) return cudaSuccess;
+    project_dd_kernel<<<p->n_pitems, 256, 0, st>>>(iq, p->N, p->Ns, p->Nz, p->Nx, p->P, reinterpret_cast<const double2*>(p->V_d), p->wslot_dd_d,
+                                                   p->box_d, p->pitems_d, p->gz_d, p->gx_d, p->tiles_d, p->tsum_d);
     return cudaGetLastError();
 }
 

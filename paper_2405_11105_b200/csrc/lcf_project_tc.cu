@@ -654,7 +654,9 @@ cudaError_t launch_presplit(lcf_plan* p, const float2* iq, cudaStream_t st) {
     return cudaGetLastError();
 }
 
+// precision 1 projects in double (project_dd_kernel); its NCC modes still take the magnitude pass of method 4 from here
 bool project_tc_eligible(const lcf_plan* p) {
+    if (p->prec == 1 && !ncc_mode(p->thr.mode)) return false;
     return p->N <= 256 && p->N >= PTC_KC && (p->Nz % 2) == 0 && p->Nz >= PTC_TZ && p->Nx >= PTC_TX && ptc_encode_fn() != nullptr;
 }
 
