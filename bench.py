@@ -55,6 +55,9 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (metric: 2)")
+    ap.add_argument("--thresh-mode", type=int, default=None,
+                    help="override the threshold mode of the chosen config (include/lcf.h lcf_thresh_mode; e.g. 16 = "
+                         "LCF_HARD_ENERGY_TOP); the workload string says so.  For profiling the other kernels.")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-streaming", action="store_true", help="skip the config 4 streaming section")
     ap.add_argument("--no-context", action="store_true", help="skip the per-config latencies and the paper-shaped context runs")
@@ -384,7 +387,14 @@ def run_ours(args, cfg):
     # EVD algorithmic flops: one-sided Jacobi = 36 flops per row per column pair (three dot products,
     # two rotated columns), N rows, N(N-1)/2 pairs per sweep; two-sided = 30 N^3 per sweep
     # (DESIGN.md "Rooflines"); sweeps as measured on this input
-    evd_flops = float(sweeps.sum()) * (36.0 * N * N * (N - 1) / 2 if work["evd_chol"] else 30.0 * N ** 3)
+    if work["evd_chol"] == 2:
+        # leading-eigenpair modes: a round of the block iteration on M = 16 vectors is the product R Q (8 N^2 M), the
+        # small Gram H (8 N M^2), classical Gram-Schmidt twice (16 N M^2 / 2 x 2) and the rotation of Q and Y
+        # (16 N M^2): 8 N M (N + 5 M) flops in double; rounds as measured on this input
+        Mb = 16
+        evd_flops = float(sweeps.sum()) * 8.0 * N * Mb * (N + 5 * Mb)
+    else:
+        evd_flops = float(sweeps.sum()) * (36.0 * N * N * (N - 1) / 2 if work["evd_chol"] else 30.0 * N ** 3)
     # the contractions run on the FP16 tensor path (.kind::f16, fp32 accumulate).  Denominator: the bare
     # tcgen05 kind::f16 loop measured in this run (lcf_measure_peak(3)); MEASURED_PEAKS.json's bf16 matmul
     # figure (same nominal rate) is carried beside it
@@ -402,9 +412,9 @@ def run_ours(args, cfg):
     kern = {
         "gram": {"kernel": "gram_tc_kernel" if work["gram_tc"] else "gram_kernel", "flops": work["gram_flops"],
                  "bound": "tensor" if work["gram_tc"] else "alu", "executed_flops": work["gram_tensor_flops"] or None},
-        "evd": {"kernel": "evd_chol_kernel (Cholesky) + jacobi_cluster_*_kernel | evd_chol_kernel" if work["evd_chol"] else "jacobi_kernel + vbuild_kernel", "flops": evd_flops, "bound": "alu",
+        "evd": {"kernel": "evd_top_kernel (block subspace iteration, fp64)" if work["evd_chol"] == 2 else ("evd_chol_kernel (Cholesky) + jacobi_cluster_*_kernel | evd_chol_kernel" if work["evd_chol"] else "jacobi_kernel + vbuild_kernel"), "flops": evd_flops, "bound": "alu",
                 "executed_flops": None},
-        "projection": {"kernel": "project_tc_kernel" if work["proj_tc"] else "project_kernel", "flops": work["proj_flops"],
+        "projection": {"kernel": "project_tc_kernel" if work["proj_tc"] else ("project_dd_kernel" if cfg.filt.precision == 1 else "project_kernel"), "flops": work["proj_flops"],
                        "bound": "tensor" if work["proj_tc"] else "alu", "executed_flops": work["proj_tensor_flops"] or None},
     }
     per_kernel = {}
@@ -412,11 +422,12 @@ def run_ours(args, cfg):
         ms = stages.get(sname)
         if not ms:
             continue
-        peak = tensor_peak if kd["bound"] == "tensor" else (fp64_peak if cfg.filt.precision == 1 and sname != "projection" else fp32_peak)
+        dbl = cfg.filt.precision == 1 or (sname == "evd" and work["evd_chol"] == 2)       # kernels on the FP64 pipe
+        peak = tensor_peak if kd["bound"] == "tensor" else (fp64_peak if dbl else fp32_peak)
         ach = kd["flops"] / (ms * 1e-3) / 1e12
         per_kernel[sname] = {"kernel": kd["kernel"], "ms": ms, "bound": kd["bound"], "achieved": ach, "peak": peak,
                              "unit": "TFLOP/s", "frac": ach / peak, "algorithmic_flops_per_launch": kd["flops"],
-                             "peak_source": tensor_src if kd["bound"] == "tensor" else fp32_src}
+                             "peak_source": tensor_src if kd["bound"] == "tensor" else ("lcf_measure_peak(2): DFMA register loop, this run" if dbl else fp32_src)}
         if kd["executed_flops"]:
             ex = kd["executed_flops"] / (ms * 1e-3) / 1e12
             per_kernel[sname].update({"executed_tflops": ex, "executed_frac": ex / peak,
@@ -630,6 +641,9 @@ def run_ours(args, cfg):
 def main():
     args = parse_args()
     cfg = synth.baseline_configs()[args.config]
+    if args.thresh_mode is not None:
+        from dataclasses import replace as _rep
+        cfg = _rep(cfg, filt=_rep(cfg.filt, mode=args.thresh_mode))
     if args.impl == "reference":
         run_reference(args, cfg)
     else:
