@@ -5,9 +5,10 @@
 // LCF_HARD_ENERGY_TOP compute exactly that filter by block subspace iteration with Rayleigh-Ritz (a departure from the
 // paper's full-spectrum EVD; the full-spectrum modes stay the default):
 //     Q <- orth(Y);  Y <- R Q;  H = Q^H Y;  H = J Theta J^H;  Q <- Q J, Y <- Y J        (one round)
-// on a block of ET_M = 32 vectors.  Tissue dominates R_k by 20-60 dB, so lambda_{33} / lambda_c is tiny and the block
-// converges in 3-4 rounds whatever N is: O(N^2 M) per round instead of the O(N^3) per sweep of a Jacobi EVD (config 3,
-// 192 windows of 200 frames: 17 ms of cluster Jacobi).
+// on a block of M = 16 vectors (cuts up to 10), or 32 (cuts up to 26) for the windows the small block cannot settle.
+// Tissue dominates R_k by 20-60 dB, so lambda_{M+1} / lambda_c is tiny and the block converges in 2-3 rounds whatever N
+// is: O(N^2 M) per round instead of the O(N^3) per sweep of a Jacobi EVD (config 3, 192 windows of 200 frames: 1.1 ms
+// against 17 ms of cluster Jacobi).
 //
 // One CTA (256 threads) per window.  Q lives in shared memory in double, Y in float; every inner product and the
 // products with R accumulate in double (R_k itself is the fp32 Gram).  Steps of a round:
@@ -19,8 +20,8 @@
 //           R q_j outside the span of the leading c Ritz vectors; converged when every rho_j, j <= c, is below
 //           2e-6 (theta_j - theta_{c+1}) (the sine of the angle by which it tilts that span), or at the rounding floor
 //           of the fp32 column it is computed from.
-// Outputs: lambda (the M Ritz values; the N - M others are reported as their mean, (trace - sum theta) / (N - M), which
-// keeps the array descending and its sum equal to the trace), c_k, weights, V_k = [q_1 .. q_M, 0 ...], and
+// Outputs: lambda (the M Ritz values, a rounding-negative one as 0; the N - M others are reported as their mean,
+// (trace - sum theta) / (N - M), capped by the last Ritz value so that the array stays descending), c_k, weights, V_k = [q_1 .. q_M, 0 ...], and
 // B_k = F_k itself (Hermitian, idempotent: |F^T s|^2 = |F conj(s)|^2 is the filtered power, so the projection kernels
 // take it unchanged).
 #include <cfloat>
