@@ -166,13 +166,20 @@ __global__ void __launch_bounds__(ET_THREADS, 1) evd_top_kernel(EtArgs a) {
 #pragma unroll
                 for (int cc = 0; cc < CPT; ++cc) ar[cc] = ai[cc] = 0.0;
                 const double2* q0 = Q + (size_t)(cs * CPT) * LQ;
-                for (int j = 0; j < N; ++j) {
-                    const float2 rf = Rk[(size_t)j * N + row];
-                    const double rr = rf.x, ri = -(double)rf.y;
+                constexpr int PF = 8;                                // loads of R in flight per thread (L2 latency, 8 warps per SM)
+                for (int j0 = 0; j0 < N; j0 += PF) {
+                    float2 rf[PF];
 #pragma unroll
-                    for (int cc = 0; cc < CPT; ++cc) {
-                        const double2 q = q0[(size_t)cc * LQ + j];
-                        ar[cc] += rr * q.x - ri * q.y; ai[cc] += rr * q.y + ri * q.x;
+                    for (int u = 0; u < PF; ++u) rf[u] = j0 + u < N ? Rk[(size_t)(j0 + u) * N + row] : make_float2(0.f, 0.f);
+#pragma unroll
+                    for (int u = 0; u < PF; ++u) {
+                        const int j = j0 + u < N ? j0 + u : N - 1;   // (a zero R entry past the end adds nothing)
+                        const double rr = rf[u].x, ri = -(double)rf[u].y;
+#pragma unroll
+                        for (int cc = 0; cc < CPT; ++cc) {
+                            const double2 q = q0[(size_t)cc * LQ + j];
+                            ar[cc] += rr * q.x - ri * q.y; ai[cc] += rr * q.y + ri * q.x;
+                        }
                     }
                 }
 #pragma unroll
