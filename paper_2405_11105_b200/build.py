@@ -14,7 +14,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "liblcf.so"
-SOURCES = ["lcf_plan.cu", "lcf_gram.cu", "lcf_gram_tc.cu", "lcf_gram_tc2.cu", "lcf_evd.cu", "lcf_evd_chol.cu", "lcf_evd_cluster.cu", "lcf_evd_top.cu", "lcf_project.cu", "lcf_project_tc.cu", "lcf_ncc.cu", "lcf_peaks.cu"]
+SOURCES = ["lcf_plan.cu", "lcf_gram.cu", "lcf_gram_tc.cu", "lcf_gram_tc2.cu", "lcf_evd.cu", "lcf_evd_chol.cu", "lcf_evd_cluster.cu", "lcf_evd_top.cu", "lcf_project.cu", "lcf_project_tc.cu", "lcf_ncc.cu", "lcf_peaks.cu", "lcf_noalloc.cu"]
 # no --use_fast_math: the EVD needs IEEE division and square roots
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
@@ -31,7 +31,7 @@ def needs_build() -> bool:
     if not LIB.exists():
         return True
     t = LIB.stat().st_mtime
-    deps = [CSRC / s for s in SOURCES] + [CSRC / "lcf_internal.h", CSRC / "lcf_sm100.cuh", CSRC / "lcf_thresh.cuh", HERE.parent / "include" / "lcf.h"]
+    deps = [CSRC / s for s in SOURCES] + [CSRC / "lcf_internal.h", CSRC / "lcf_sm100.cuh", CSRC / "lcf_thresh.cuh", HERE.parent / "include" / "lcf.h", HERE.parent / "include" / "lcf_noalloc.h"]
     return any(d.stat().st_mtime > t for d in deps)
 
 
