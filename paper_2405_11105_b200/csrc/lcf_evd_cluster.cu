@@ -624,6 +624,7 @@ struct EcbCrit { float tol2, big2, eabs2, tc2; bool strict_all; };
 constexpr float ECB_RHO = 100.f;               // squared-norm ratio from which a pair is "separated" (clean-up)
 constexpr float ECB_LOOSE2 = 0.09f;            // squared cosine every counted pair must reach before the last sweep
 constexpr float ECB_EXEMPT2 = 0.01f;           // squared cosine up to which the first-order clean-up is trusted with a separated pair
+constexpr float ECB_FLOOR = 1e-7f;             // median / largest eigenvalue above which a window is swept with the strict rule whatever the mode
 constexpr float ECB_EABS = 1e-6f;              // |g_p^H g_q| / largest eigenvalue below which a pair may stay at the loose cosine
 __device__ __forceinline__ int ecb_round_tracked(EcbCol& X, EcbCol& Y, EcbCol& Z, EcbCol& W, float& nX, float& nY, float& nZ, float& nW,
                                                  int lane, const EcbCrit& cr) {
@@ -975,7 +976,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
     EcbCrit crit;
     crit.tol2 = tol2; crit.big2 = 2.f * tol;
     crit.eabs2 = 0.f; crit.tc2 = 3.0e38f;                            // first sweep: nothing known yet, everything strict
-    crit.strict_all = !(a.mode == LCF_SOFT_FIXED || a.mode == LCF_SOFT_ENERGY);
+    const bool strict_mode = !(a.mode == LCF_SOFT_FIXED || a.mode == LCF_SOFT_ENERGY);
+    crit.strict_all = strict_mode;
     const bool rowok = lane < nch;                                   // this lane's 4 rows exist
     int dPt, dPi, dQt, dQi;                                          // destinations of the top / bottom block (row, block pair)
     if (gi == 0) { dPt = 0; dPi = 0; dQt = 0; dQi = 1; }
@@ -1084,10 +1086,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                 }
                 if (rnk == 0) thr_sh[0] = my;
                 if (rnk == ECB_KC - 1) thr_sh[1] = my;
+                if (rnk == N / 2) thr_sh[2] = my;
             }
             __syncthreads();
             const float e1 = ECB_EABS * thr_sh[0];
             crit.eabs2 = e1 * e1; crit.tc2 = 2.f * thr_sh[1];
+            // the loose rule is for spectra whose noise floor lies deep below the clutter: with the median eigenvalue
+            // (column norm minus the Cholesky shift) above ECB_FLOOR of the largest, the residual couplings it leaves
+            // inside the floor show in the image (random shapes and noise levels against the oracle: image errors up
+            // to 2e-3 for floors above 1e-7, below 5e-4 under it; the strict rule: 1e-4 .. 4e-4), so such a window sweeps strictly
+            crit.strict_all = strict_mode || (thr_sh[2] - delta) > ECB_FLOOR * thr_sh[0];
         }
         const float f0 = flg[(sweep & 1) * 2], f1 = flg[(sweep & 1) * 2 + 1];
         // the sweep after an all-small sweep is the last one -- unless it still made a big rotation

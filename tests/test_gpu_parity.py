@@ -388,6 +388,24 @@ def test_top_modes_report_what_they_cannot_settle(lcf):
             assert plan.unconverged() == 2
 
 
+@pytest.mark.parametrize("Nz", [35, 36])
+def test_high_noise_floor_is_swept_with_the_strict_rule(lcf, oracle, Nz):
+    """The loose stop rule of the cluster Jacobi (sigmoid weights) is for spectra whose noise floor lies deep
+    below the clutter.  Found by random shapes against the oracle: with noise 40 dB under the tissue (median eigenvalue
+    1e-6 of the largest) it left an image error of 1.0e-3 on this input; such windows now take the strict rule
+    (7+ sweeps instead of 5-6) and reach 1e-5."""
+    cfg = synth.baseline_configs()[2]
+    d = replace(cfg.data, Nz=Nz, Nx=77, N=128, n_frames=128, seed=227180, n_vessels=3, tissue_db=40.0, noise_db=-40.0)
+    f = synth.FilterSpec(3, 1, 40.0, 40.0, 2.5, synth.SOFT_ENERGY, precision=0)
+    iq = synth.generate_sequence(d)
+    o = oracle.run_config(iq, f)
+    assert 3e-7 < (o["lam"][:, 64] / o["lam"][:, 0]).min()          # the floor this test is about
+    g = gpu_run(lcf, iq, f)
+    check_spectrum(g, o)
+    assert g["sweeps"].min() >= 7, g["sweeps"]
+    assert check_pd(g["PD"], o["PD"], tol=1e-4) <= 1e-4
+
+
 def test_allpass_and_allstop(lcf, oracle):
     iq = synth.random_cube(32, 24, 12, seed=5)
     f0 = synth.FilterSpec(2, 2, 8.0, 8.0, 3.0, synth.HARD_FIXED, k_fixed=0)
