@@ -287,6 +287,9 @@ __global__ void __launch_bounds__(1024, 1) jacobi_kernel(JacArgs a) {
         const int c = thresh_is_adaptive(a.mode) ? 0 : thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
         if (thresh_is_adaptive(a.mode)) wnorm_sh = thresh_adaptive_norm(lsort, N, a.beta);
         *csh = c;
+        bool finite = true;                                // a NaN or Inf anywhere in the spectrum is reported, not passed on as a result
+        for (int i = 0; i < N; ++i) finite = finite && isfinite(lsort[i]);
+        if (!finite) converged = 0;
         a.cut[k] = c;
         a.sweeps[k] = sweep;
         a.conv[k] = converged;

@@ -185,6 +185,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
             if (lane == 0) wkey[warp] = key;
         }
         __syncthreads();
+        bool exhausted = false;                                      // (every thread decides it from the same dgs[pv]: uniform)
         for (int jb = 0; jb < N; jb += EC_NB) {
             const int je = jb + EC_NB < N ? jb + EC_NB : N;
             for (int j = jb; j < je; ++j) {
@@ -193,8 +194,15 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
                 const int pv = (int)(KM - (kk & KM));
                 unsigned key = 0u;
                 if (tid < N) {
-                    // a non-positive pivot can only come from rounding: clamp (the column is then ~0)
-                    const float piv = fmaxf(dgs[pv], 1e-30f * maxdiag + 1e-37f);
+                    // R + delta I >= delta I, so every Schur complement has its diagonal >= delta.  R comes out of fp32-grade
+                    // arithmetic, though: its smallest eigenvalues are off by a few ulp of the LARGEST one (a rank-deficient
+                    // window of 208 coherent frames: down to -3.7e-5 maxdiag, beyond the shift), the matrix is then indefinite
+                    // and going on would amplify rounding noise step by step (1e20 and NaN, found by random shapes).  A pivot
+                    // below delta / 2 says what is left is that noise: from there on the remaining columns keep their
+                    // diagonal only (G G^H then differs from R + delta I by off-diagonal noise of the order of delta).
+                    const float praw = dgs[pv];
+                    if (praw < 0.5f * delta) exhausted = true;
+                    const float piv = fmaxf(praw, 0.25f * delta);
                     const float sc = rsqrtf(piv), dsq = piv * sc;
                     const int i = tid;
                     float sr = 0.f, si = 0.f;
@@ -209,8 +217,10 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
                     float vr = 0.f, vi = 0.f;                        // Cholesky column pi_j is zero in eliminated rows
                     if (i == pv) { vr = dsq; elim[i] = 1; }
                     else if (!elim[i]) {
-                        vr = (Gr[(size_t)pv * LD + i] - sr) * sc;
-                        vi = (Gi[(size_t)pv * LD + i] - si) * sc;
+                        if (!exhausted) {
+                            vr = (Gr[(size_t)pv * LD + i] - sr) * sc;
+                            vi = (Gi[(size_t)pv * LD + i] - si) * sc;
+                        }
                         const float nd = fmaxf(d - (vr * vr + vi * vi), 0.f);
                         dgs[i] = nd;
                         key = (__float_as_uint(nd) & ~KM) | (KM - (unsigned)i);
@@ -405,6 +415,9 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
         const int c = thresh_is_adaptive(a.mode) ? 0 : thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
         if (thresh_is_adaptive(a.mode)) wnorm_sh = thresh_adaptive_norm(lsort, N, a.beta);
         ish[1] = c;
+        bool finite = true;                                          // a NaN or Inf anywhere in the spectrum is reported, not passed on as a result
+        for (int i = 0; i < N; ++i) finite = finite && isfinite(lsort[i]);
+        if (!finite) converged = 0;
         a.cut[k] = c;
         a.sweeps[k] = sweep;
         a.conv[k] = converged;

@@ -197,6 +197,9 @@ __device__ __forceinline__ void ecl_epilogue(const EclArgs& a, int k, uint32_t r
         const int c = thresh_is_adaptive(a.mode) ? 0 : thresh_cutoff(a.mode, a.k_fixed, a.energy_frac, a.cut_scale, lsort, N);
         if (thresh_is_adaptive(a.mode)) wnorm_sh = thresh_adaptive_norm(lsort, N, a.beta);
         ish[1] = c;
+        bool finite = true;                                          // a NaN or Inf anywhere in the spectrum is reported, not passed on as a result
+        for (int i = 0; i < N; ++i) finite = finite && isfinite(lsort[i]);
+        if (!finite) converged = 0;
         if (rank == 0) { a.cut[k] = c; a.sweeps[k] = sweep; a.conv[k] = converged; if (!converged) atomicAdd(a.nunconv, 1); }
     }
     __syncthreads();

@@ -393,7 +393,9 @@ __global__ void __launch_bounds__(ET_THREADS, 1) evd_top_kernel(EtArgs a) {
     if (tid == 0) {
         a.cut[k] = found ? c : 0;
         a.sweeps[k] = rounds;
-        const int cv = converged && found;
+        bool finite = isfinite(trace);
+        for (int i = 0; i < M; ++i) finite = finite && isfinite(theta[i]);
+        const int cv = converged && found && finite;
         a.conv[k] = cv;
         if (!cv) atomicAdd(a.nunconv, 1);
     }
