@@ -214,6 +214,10 @@ cudaError_t launch_ncc(lcf_plan* p, const float2* iq, cudaStream_t st) {
     if (p->proj_tc) {
         e = launch_project_tc_mag(p, iq, st);
     } else {
+        if ((size_t)32 * N * sizeof(float2) > 48 * 1024) {           // above 192 frames the chunk needs the opt-in shared-memory size
+            e = set_max_dyn_smem(ncc_mag_kernel, p->smem_optin);
+            if (e != cudaSuccess) return e;
+        }
         ncc_mag_kernel<<<p->n_pitems, 256, (size_t)32 * N * sizeof(float2), st>>>(iq, N, p->Ns, p->Nz, p->Nx, p->P, p->B_d, p->order_d, p->box_d,
                                                                                   p->pitems_d, p->gz_d, p->gx_d, p->ncc_isig_d, ncol, p->ncc_mag_d);
         e = cudaGetLastError();

@@ -242,6 +242,8 @@ NCC_CASES = [
     (48, 40, 100, 2, 1, 12.0, synth.SOFT_NCC, 0),    # N = 100: padded column block
     (45, 40, 32, 1, 2, 12.0, synth.HARD_NCC, 1),     # odd Nz: FP32 magnitude fallback
     (40, 24, 12, 2, 1, 10.0, synth.SOFT_NCC, 1),     # N < 16: fallback, fn windows clipped at both ends
+    (45, 40, 208, 1, 2, 12.0, synth.HARD_NCC, 0),    # long ensemble, odd Nz: the FP32 magnitude pass with 52 KB of shared memory (opt-in size; found by random shapes)
+    (48, 40, 160, 2, 1, 12.0, synth.HARD_NCC, 1),    # above 152 frames: the wide-form tcgen05 magnitude pass (one resident column block), fp64 EVD
 ]
 
 
