@@ -324,14 +324,16 @@ __global__ void __launch_bounds__(EC_THREADS, 1) evd_chol_kernel(EcArgs a) {
                     const float absa2 = xr * xr + xi * xi;
                     if (absa2 > tol2 * app * aqq && absa2 > 0.f) {
                         any = 1;
-                        const float inv = rsqrtf(absa2);
-                        const float tau = (aqq - app) * (0.5f * inv);
-                        const float at = fabsf(tau);
-                        float t = (at > 1e8f) ? 0.5f / at : 1.f / (at + sqrtf(1.f + tau * tau));
-                        if (tau < 0.f) t = -t;
-                        const float cs = rsqrtf(1.f + t * t);
-                        const float sn = t * cs;
-                        const float gr = sn * xr * inv, gi = sn * xi * inv;
+                        // rotation parameters as in lcf_evd_cluster.cu (ecb_round_tracked): unitary to rounding without bias
+                        const float alpha = 0.5f * (aqq - app);
+                        const float rinv = rsqrtf(fmaxf(fmaf(alpha, alpha, absa2), 1e-37f));
+                        const float c2h = fmaf(0.5f * fabsf(alpha), rinv, 0.5f);
+                        const float rc = rsqrtf(c2h);
+                        const float cs0 = c2h * rc;
+                        const float kk = copysignf(0.5f * rinv * rc, alpha);
+                        const float gr = kk * xr, gi = kk * xi;
+                        const float resid = fmaf(-cs0, cs0, 1.f) - fmaf(gr, gr, gi * gi);
+                        const float cs = fmaf(0.5f * rc, resid, cs0);
                         const unsigned long long c2 = ec_pack(cs, cs), gr2 = ec_pack(gr, gr), gi2 = ec_pack(gi, gi);
                         const unsigned long long ngr2 = ec_pack(-gr, -gr), ngi2 = ec_pack(-gi, -gi);
 #pragma unroll
