@@ -87,6 +87,9 @@ typedef enum {
                             EVD).  Getters: the first M eigenvalues / eigenvectors are Ritz pairs,
                             the other eigenvalues are reported as their mean (trace(R) - sum of the M) / (N - M),
                             the other eigenvectors as zero columns; lcf_get_sweeps counts rounds of the iteration.
+                            Only the k_fixed (or c_k) leading pairs are iterated to the accuracy of the full EVD;
+                            the Ritz values behind them are lower bounds of their eigenvalues, as converged as the
+                            cut needed (typically within 1e-4 of the largest; with k_fixed = 0 nothing is iterated).
                             Runs for precision 0, 40 <= N <= 224, k_fixed <= 26; other plans in this mode compute
                             the same filter with the full EVD (lcf_get_work: evd_chol = 2 when it runs)   */
     LCF_HARD_ENERGY_TOP = 16  /* the same for LCF_HARD_ENERGY: c from the leading eigenvalues and trace(R_k).  A
