@@ -139,7 +139,7 @@ extern "C" const char* lcf_status_string(lcf_status s) {
     switch (s) {
         case LCF_OK: return "ok";
         case LCF_ERR_INVALID_ARG: return "invalid argument";
-        case LCF_ERR_UNSUPPORTED: return "unsupported size (EVD matrix does not fit shared memory)";
+        case LCF_ERR_UNSUPPORTED: return "unsupported size or configuration (plan: the EVD matrix does not fit shared memory; other calls: lcf_last_error)";
         case LCF_ERR_ALLOC: return "allocation failed";
         case LCF_ERR_CUDA: return "CUDA error";
         case LCF_ERR_NOT_CONVERGED: return "EVD did not converge";
@@ -435,7 +435,10 @@ extern "C" lcf_status lcf_filter(lcf_plan* p, const void* iq_dev, float* pd_dev,
 
 extern "C" lcf_status lcf_filter_stream(lcf_plan* p, const void* iq_dev, float* pd_dev, int stride, cudaStream_t stream) {
     if (!p || !iq_dev || !pd_dev || stride < 0 || stride > p->N) return LCF_ERR_INVALID_ARG;
-    if (!gram_stream_eligible(p)) return LCF_ERR_UNSUPPORTED;
+    if (!gram_stream_eligible(p)) {
+        snprintf(p->last_error, sizeof(p->last_error), "lcf_filter_stream needs the tensor-core Gram of 32 .. 128 frames (precision 0, even Nz); use lcf_filter with this plan");
+        return LCF_ERR_UNSUPPORTED;
+    }
     if (!p->strm_ready) {                               // first use: segments, partials, the kept R
         std::vector<G2Seg> segs;
         std::vector<int> cta_first, seg_first;
