@@ -614,3 +614,15 @@ def test_top_modes_are_the_hard_modes_on_the_oracle_side(oracle):
                 assert c == int(np.searchsorted(np.cumsum(lam), 0.99 * lam.sum(), side="right") + 1)
             F = np.eye(16) - U[:, :c] @ U[:, :c].conj().T
             assert np.abs(a["F"][kz] - F).max() <= 1e-10
+
+
+def test_fig2f_sigmoid_example(oracle):
+    """The paper's one stated example of Eq. 9 (Fig. 2f: beta = 2, k = 13) against the logistic table values
+    in tests/golden/fig2f_sigmoid_beta2_k13.txt."""
+    from pathlib import Path
+    rows = [l.split() for l in (Path(__file__).parent / "golden" / "fig2f_sigmoid_beta2_k13.txt").read_text().splitlines()
+            if l.strip() and not l.startswith("#")]
+    wt = oracle.weights(50, True, 13, 2.0)
+    assert len(rows) == 7
+    for i, v in rows:
+        assert np.isclose(wt[int(i) - 1], float(v), rtol=1e-14), (i, wt[int(i) - 1], v)
