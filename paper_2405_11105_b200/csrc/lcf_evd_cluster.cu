@@ -1,5 +1,6 @@
 // lcf_evd_cluster.cu -- kernel 2+3, one-sided Jacobi spread over a 2-CTA thread-block cluster
-// (precision 0, even N, 32 <= N <= 128; above that, up to ECL8_MAXN frames, over an 8-CTA cluster: jacobi_cluster8_kernel).  The single-CTA kernel of lcf_evd_chol.cu is bound by
+// (precision 0, even N, 32 <= N <= 128; above that, up to ECL8_MAXN frames, over an 8-CTA cluster: jacobi_cluster8_block_kernel,
+// jacobi_cluster8_kernel).  The single-CTA kernel of lcf_evd_chol.cu is bound by
 // shared-memory bandwidth (the whole N x N matrix crosses the 128 B/clk crossbar twice per
 // rotation step) and uses 64 of 148 SMs at 64 windows; here each matrix gets two SMs.
 //
@@ -1118,9 +1119,298 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(ECL_THREADS, 1) jaco
                  lam_s, inv_s, wsl, lsort, ish, shiftv, delta, sweep, converged);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Block form above 128 frames (jacobi_cluster8_block_kernel, N % 4 == 0): the block-systolic sweep of
+// jacobi_cluster_block_kernel over an 8-CTA cluster.  One warp owns a block pair; lane r holds the 4-row chunks r and
+// r + 32 of its four columns (N <= 256); CTA c owns the block pairs [n c / 8, n (c + 1) / 8) (at most ECB8_PL = 8,
+// double-buffered: 107 KB at N = 208, two CTAs of different windows per SM under a 128-register cap); blocks move between
+// pairs by mbarrier dataflow, across CTAs with st.async.  No clean-up pass here: every pair is rotated down to a cosine of
+// 4 eps and the stop rule is the strict one (see jacobi_cluster8_kernel for why long ensembles need that).
+// Measured on config 3 (192 windows of 200 frames, 6.8 sweeps): 11.9 ms, against 15.9 ms for the pair form below it
+// (which stays for N % 4 == 2); with one CTA per SM (168 registers, no spills) 14.6 ms.
+template <int NCH>
+struct EcbNCol { ulonglong2 re[NCH], im[NCH]; };
+
+template <int NCH>
+__device__ __forceinline__ void ecbn_norms4(const EcbNCol<NCH>& X, const EcbNCol<NCH>& Y, const EcbNCol<NCH>& Z, const EcbNCol<NCH>& W, int lane,
+                                            float& nX, float& nY, float& nZ, float& nW) {
+    auto nrm = [](const EcbNCol<NCH>& C) {
+        unsigned long long s2 = 0ull;
+#pragma unroll
+        for (int c = 0; c < NCH; ++c)
+            s2 = ecl_fma2(C.re[c].x, C.re[c].x, ecl_fma2(C.im[c].x, C.im[c].x, ecl_fma2(C.re[c].y, C.re[c].y, ecl_fma2(C.im[c].y, C.im[c].y, s2))));
+        return ecl_hsum(s2);
+    };
+    const float a0 = nrm(X), a1 = nrm(Y), a2 = nrm(Z), a3 = nrm(W);
+    const bool h16 = (lane & 16) != 0, h8 = (lane & 8) != 0;
+    float k0 = (h16 ? a2 : a0) + __shfl_xor_sync(0xffffffffu, h16 ? a0 : a2, 16);
+    float k1 = (h16 ? a3 : a1) + __shfl_xor_sync(0xffffffffu, h16 ? a1 : a3, 16);
+    float v = (h8 ? k1 : k0) + __shfl_xor_sync(0xffffffffu, h8 ? k0 : k1, 8);
+    v += __shfl_xor_sync(0xffffffffu, v, 4);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    nX = __shfl_sync(0xffffffffu, v, 0);  nY = __shfl_sync(0xffffffffu, v, 8);
+    nZ = __shfl_sync(0xffffffffu, v, 16); nW = __shfl_sync(0xffffffffu, v, 24);
+}
+
+// ecb_round_tracked with NCH chunks per lane and the plain strict criteria: rotate above tol2, "big" above big2.
+// Returns bit 0: rotated, bit 1: a rotated pair was big.
+template <int NCH>
+__device__ __forceinline__ int ecbn_round_tracked(EcbNCol<NCH>& X, EcbNCol<NCH>& Y, EcbNCol<NCH>& Z, EcbNCol<NCH>& W, float& nX, float& nY, float& nZ,
+                                                  float& nW, int lane, float tol2, float big2) {
+    float v1[2], v2[2];
+    {
+        unsigned long long re2 = 0ull, ia2 = 0ull, ib2 = 0ull;
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            re2 = ecl_fma2(X.re[c].x, Y.re[c].x, ecl_fma2(X.im[c].x, Y.im[c].x, ecl_fma2(X.re[c].y, Y.re[c].y, ecl_fma2(X.im[c].y, Y.im[c].y, re2))));
+            ia2 = ecl_fma2(X.re[c].x, Y.im[c].x, ecl_fma2(X.re[c].y, Y.im[c].y, ia2));
+            ib2 = ecl_fma2(X.im[c].x, Y.re[c].x, ecl_fma2(X.im[c].y, Y.re[c].y, ib2));
+        }
+        v1[0] = ecl_hsum(re2); v1[1] = ecl_hsum(ia2) - ecl_hsum(ib2);
+    }
+    {
+        unsigned long long re2 = 0ull, ia2 = 0ull, ib2 = 0ull;
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            re2 = ecl_fma2(Z.re[c].x, W.re[c].x, ecl_fma2(Z.im[c].x, W.im[c].x, ecl_fma2(Z.re[c].y, W.re[c].y, ecl_fma2(Z.im[c].y, W.im[c].y, re2))));
+            ia2 = ecl_fma2(Z.re[c].x, W.im[c].x, ecl_fma2(Z.re[c].y, W.im[c].y, ia2));
+            ib2 = ecl_fma2(Z.im[c].x, W.re[c].x, ecl_fma2(Z.im[c].y, W.re[c].y, ib2));
+        }
+        v2[0] = ecl_hsum(re2); v2[1] = ecl_hsum(ia2) - ecl_hsum(ib2);
+    }
+    const bool lo = lane < 16;                                       // lanes 0-15: parameters of (X, Y), lanes 16-31: of (Z, W)
+    float xr = (lo ? v1[0] : v2[0]) + __shfl_xor_sync(0xffffffffu, lo ? v2[0] : v1[0], 16);
+    float xi = (lo ? v1[1] : v2[1]) + __shfl_xor_sync(0xffffffffu, lo ? v2[1] : v1[1], 16);
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) {
+        xr += __shfl_xor_sync(0xffffffffu, xr, o);
+        xi += __shfl_xor_sync(0xffffffffu, xi, o);
+    }
+    const float app = lo ? nX : nZ, aqq = lo ? nY : nW;
+    const float absa2 = xr * xr + xi * xi;
+    const float pq = app * aqq;
+    const bool rot = absa2 > tol2 * pq && absa2 > 0.f;
+    const float alpha = 0.5f * (aqq - app);
+    const float rinv = rsqrtf(fmaxf(fmaf(alpha, alpha, absa2), 1e-37f));
+    const float c2h = fmaf(0.5f * fabsf(alpha), rinv, 0.5f);
+    const float rc = rsqrtf(c2h);
+    const float cs0 = c2h * rc;
+    const float kk = rot ? copysignf(0.5f * rinv * rc, alpha) : 0.f;
+    const float gr = kk * xr, gi = kk * xi;
+    const float resid = fmaf(-cs0, cs0, 1.f) - fmaf(gr, gr, gi * gi);
+    const float cs = rot ? fmaf(0.5f * rc, resid, cs0) : 1.f;
+    const float d = kk * absa2 * rc;
+    int flags = (rot ? 1 : 0) | (rot && absa2 > big2 * pq ? 2 : 0);
+    if (fabsf(d) > 0.75f * fminf(app, aqq)) flags |= 4;              // the update cancels most of the smaller norm: refresh
+    const float ocs = __shfl_xor_sync(0xffffffffu, cs, 16), ogr = __shfl_xor_sync(0xffffffffu, gr, 16);
+    const float ogi = __shfl_xor_sync(0xffffffffu, gi, 16), od = __shfl_xor_sync(0xffffffffu, d, 16);
+    const float c1 = lo ? cs : ocs, r1 = lo ? gr : ogr, i1 = lo ? gi : ogi, d1 = lo ? d : od;
+    const float c2_ = lo ? ocs : cs, r2_ = lo ? ogr : gr, i2_ = lo ? ogi : gi, d2 = lo ? od : d;
+    auto apply = [](EcbNCol<NCH>& P, EcbNCol<NCH>& Q, float c, float gr_, float gi_) {
+        const unsigned long long c2 = ecl_pack(c, c), g2 = ecl_pack(gr_, gr_), h2 = ecl_pack(gi_, gi_);
+        const unsigned long long ng2 = ecl_pack(-gr_, -gr_), nh2 = ecl_pack(-gi_, -gi_);
+#pragma unroll
+        for (int q = 0; q < NCH; ++q) {
+            ulonglong2 pre, pim, qre, qim;                           // g_p' = c g_p - conj(g) g_q,   g_q' = g g_p + c g_q
+            pre.x = ecl_fma2(nh2, Q.im[q].x, ecl_fma2(ng2, Q.re[q].x, ecl_mul2(c2, P.re[q].x)));
+            pre.y = ecl_fma2(nh2, Q.im[q].y, ecl_fma2(ng2, Q.re[q].y, ecl_mul2(c2, P.re[q].y)));
+            pim.x = ecl_fma2(h2, Q.re[q].x, ecl_fma2(ng2, Q.im[q].x, ecl_mul2(c2, P.im[q].x)));
+            pim.y = ecl_fma2(h2, Q.re[q].y, ecl_fma2(ng2, Q.im[q].y, ecl_mul2(c2, P.im[q].y)));
+            qre.x = ecl_fma2(c2, Q.re[q].x, ecl_fma2(nh2, P.im[q].x, ecl_mul2(g2, P.re[q].x)));
+            qre.y = ecl_fma2(c2, Q.re[q].y, ecl_fma2(nh2, P.im[q].y, ecl_mul2(g2, P.re[q].y)));
+            qim.x = ecl_fma2(c2, Q.im[q].x, ecl_fma2(h2, P.re[q].x, ecl_mul2(g2, P.im[q].x)));
+            qim.y = ecl_fma2(c2, Q.im[q].y, ecl_fma2(h2, P.re[q].y, ecl_mul2(g2, P.im[q].y)));
+            P.re[q] = pre; P.im[q] = pim; Q.re[q] = qre; Q.im[q] = qim;
+        }
+    };
+    apply(X, Y, c1, r1, i1);
+    apply(Z, W, c2_, r2_, i2_);
+    nX -= d1; nY += d1; nZ -= d2; nW += d2;
+    if (__any_sync(0xffffffffu, flags & 4)) ecbn_norms4<NCH>(X, Y, Z, W, lane, nX, nY, nZ, nW);
+    return flags & 3;
+}
+
+constexpr int ECB8_PL = 7;                     // block-pair slots per CTA (N <= 208: 52 block pairs over 8 CTAs)
+constexpr int ECB8_THREADS = 256;
+__device__ __forceinline__ int ecb8_slot(int b, int t, int j, int cb, int LD) { return ((((b * 2 + t) * ECB8_PL + j) * 2 + cb) * 2) * LD; }
+
+template <int NCH>
+__global__ void __cluster_dims__(8, 1, 1) __launch_bounds__(ECB8_THREADS, 2) jacobi_cluster8_block_kernel(EclArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = a.N, LD = a.LD, Ns = N;
+    const int n = N / 4;                                             // block pairs
+    const int tid = threadIdx.x, lane = tid & 31;
+    const uint32_t rank = ecl_cluster_rank();
+    const int k = blockIdx.x / (int)ECL8_CS;
+    const int p0 = ecl8_first(n, (int)rank), npl = ecl8_first(n, (int)rank + 1) - p0;
+    float* buf = reinterpret_cast<float*>(smem_raw);                 // [2 buffers][2 rows][ECB8_PL][2 columns][2 planes][LD]
+    float* lam_s = buf + (size_t)2 * 2 * ECB8_PL * 2 * 2 * LD;
+    float* inv_s = lam_s + Ns;
+    float* wsl = inv_s + Ns;
+    float* flg = wsl + Ns;                                           // [2 parities][ECL8_CS ranks]
+    double* lsort = reinterpret_cast<double*>(flg + 2 * ECL8_CS);
+    int* ish = reinterpret_cast<int*>(lsort + Ns);
+    uint64_t* fullb = reinterpret_cast<uint64_t*>(ish + 4);         // [2 buffers][ECB8_PL] "both blocks of this pair have arrived"
+    const uint32_t buf_u32 = ecl_smem(buf), full_u32 = ecl_smem(fullb);
+
+    // ---- initial placement: block pair i = columns 4i .. 4i+3 (top block 4i, 4i+1; bottom block 4i+2, 4i+3)
+    const float* gk = a.gfac + (size_t)k * 2 * N * a.LDg;
+    const int nch = N >> 2;                                          // 4-row chunks per column (<= 32 NCH)
+    for (int e = tid; e < npl * 4 * 2 * nch; e += ECB8_THREADS) {
+        const int ch = e % nch; int q = e / nch;
+        const int pl = q & 1; q >>= 1;
+        const int cb = q & 1; q >>= 1;
+        const int t = q & 1, jj = q >> 1;
+        const int col = 4 * (p0 + jj) + 2 * t + cb;
+        const float4 v = *reinterpret_cast<const float4*>(gk + ((size_t)pl * N + col) * a.LDg + 4 * ch);
+        *reinterpret_cast<float4*>(buf + ecb8_slot(0, t, jj, cb, LD) + pl * LD + 4 * ch) = v;
+    }
+    const float shiftv = a.shift[k];
+    const float delta = shiftv < 0.f ? 0.f : shiftv;
+    const int jraw = tid >> 5;                                       // local block pair = warp
+    const bool act = jraw < npl;
+    const int j = act ? jraw : 0;
+    const int gi = p0 + j;
+    // destinations of the top / bottom block after a step (row, block pair) and the CTAs that own them
+    int dPt, dPi, dQt, dQi;
+    if (gi == 0) { dPt = 0; dPi = 0; dQt = 0; dQi = 1; }
+    else { dQt = 1; dQi = gi - 1; if (gi == n - 1) { dPt = 1; dPi = n - 1; } else { dPt = 0; dPi = gi + 1; } }
+    int rP = 0, rQ = 0;
+    while (dPi >= ecl8_first(n, rP + 1)) ++rP;
+    while (dQi >= ecl8_first(n, rQ + 1)) ++rQ;
+    const bool Prem = rP != (int)rank, Qrem = rQ != (int)rank;
+    const int dPj = dPi - ecl8_first(n, rP), dQj = dQi - ecl8_first(n, rQ);
+    // dataflow between block pairs as in jacobi_cluster_block_kernel: the pair's two blocks of the next step come from its
+    // ring neighbours gi - 1, gi + 1 (itself at the ends); a neighbour in this CTA stores them and arrives on the pair's
+    // mbarrier, a neighbour in another CTA sends them with st.async, whose bytes the mbarrier counts
+    const int glo = gi > 0 ? gi - 1 : 0, ghi = gi < n - 1 ? gi + 1 : n - 1;
+    const int nloc = (int)(glo >= p0 && glo < p0 + npl) + (int)(ghi >= p0 && ghi < p0 + npl);
+    const uint32_t txb = (uint32_t)(2 - nloc) * (64u * (uint32_t)nch + 8u);   // bytes of the blocks (+ two norms each) that arrive by st.async
+    if (act && lane == 0) {
+        ecl_mbar_init(full_u32 + 8u * (uint32_t)j, 1u + (uint32_t)nloc);
+        ecl_mbar_init(full_u32 + 8u * (uint32_t)(ECB8_PL + j), 1u + (uint32_t)nloc);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        ecl_mbar_arrive_tx(full_u32 + 8u * (uint32_t)j, txb);                // buffer 0 is refilled at step 1
+        ecl_mbar_arrive_tx(full_u32 + 8u * (uint32_t)(ECB8_PL + j), txb);    // buffer 1 is filled at step 0
+    }
+    ecl_cluster_sync();
+
+    const float tol = 4.f * FLT_EPSILON;                             // rotate down to a cosine of 4 eps (see jacobi_cluster8_kernel)
+    const float tol2 = tol * tol;
+    const float big2 = 2.f * 4.f * sqrtf((float)N) * FLT_EPSILON;
+    bool chok[NCH];
+    uint32_t cho[NCH];
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) { chok[c] = act && lane + 32 * c < nch; cho[c] = 16u * (uint32_t)(lane + 32 * c); }
+    const int M = 2 * n - 1;
+    const uint32_t BST = (uint32_t)ecb8_slot(1, 0, 0, 0, LD) * 4u, MST = 8u * ECB8_PL, L4 = (uint32_t)LD * 4u;
+    const uint32_t srcT = buf_u32 + (uint32_t)ecb8_slot(0, 0, j, 0, LD) * 4u;
+    const uint32_t srcB = buf_u32 + (uint32_t)ecb8_slot(0, 1, j, 0, LD) * 4u;
+    const uint32_t nrmT = srcT + 4u * (uint32_t)N, nrmB = srcB + 4u * (uint32_t)N;
+    const uint32_t dstP = (Prem ? ecl_mapa(buf_u32, (uint32_t)rP) : buf_u32) + (uint32_t)ecb8_slot(0, dPt, dPj, 0, LD) * 4u;
+    const uint32_t dstQ = (Qrem ? ecl_mapa(buf_u32, (uint32_t)rQ) : buf_u32) + (uint32_t)ecb8_slot(0, dQt, dQj, 0, LD) * 4u;
+    const uint32_t fb0 = full_u32 + 8u * (uint32_t)j;
+    const uint32_t mP0 = (Prem ? ecl_mapa(full_u32, (uint32_t)rP) : full_u32) + 8u * (uint32_t)dPj;
+    const uint32_t mQ0 = (Qrem ? ecl_mapa(full_u32, (uint32_t)rQ) : full_u32) + 8u * (uint32_t)dQj;
+    int b = 0, sweep = 0, converged = 0;
+    unsigned t = 0;                                                  // steps so far, over all sweeps
+    bool last = false;
+    for (;;) {
+        int fl = 0;
+        for (int s = 0; s < M; ++s, ++t) {
+            if (act) {
+                const uint32_t cb_ = b ? BST : 0u, nb_ = BST - cb_;  // byte offsets of the buffer read / written in this step
+                const uint32_t cm_ = b ? MST : 0u, nm_ = MST - cm_;
+                if (t > 0) {
+                    ecl_mbar_wait(fb0 + cm_, ((t - 1) >> 1) & 1u);
+                    if (lane == 0) ecl_mbar_arrive_tx(fb0 + cm_, txb);       // this pair's arrival for the buffer's next use
+                }
+                EcbNCol<NCH> A0, A1, B0, B1;
+                const ulonglong2 z2 = make_ulonglong2(0ull, 0ull);
+#pragma unroll
+                for (int c = 0; c < NCH; ++c) {
+                    A0.re[c] = A0.im[c] = A1.re[c] = A1.im[c] = B0.re[c] = B0.im[c] = B1.re[c] = B1.im[c] = z2;
+                    if (chok[c]) {
+                        const uint32_t t0 = srcT + cb_ + cho[c], b0 = srcB + cb_ + cho[c];
+                        A0.re[c] = ecl_ld_local(t0);          A0.im[c] = ecl_ld_local(t0 + L4);
+                        A1.re[c] = ecl_ld_local(t0 + 2 * L4); A1.im[c] = ecl_ld_local(t0 + 3 * L4);
+                        B0.re[c] = ecl_ld_local(b0);          B0.im[c] = ecl_ld_local(b0 + L4);
+                        B1.re[c] = ecl_ld_local(b0 + 2 * L4); B1.im[c] = ecl_ld_local(b0 + 3 * L4);
+                    }
+                }
+                float nA0, nA1, nB0, nB1;
+                if (s == 0) {
+                    ecbn_norms4<NCH>(A0, A1, B0, B1, lane, nA0, nA1, nB0, nB1);
+                    fl |= ecbn_round_tracked<NCH>(A0, A1, B0, B1, nA0, nA1, nB0, nB1, lane, tol2, big2);   // inner pairs, once per sweep
+                } else {
+                    nA0 = ecl_ld_local_f32(nrmT + cb_); nA1 = ecl_ld_local_f32(nrmT + cb_ + 2 * L4);
+                    nB0 = ecl_ld_local_f32(nrmB + cb_); nB1 = ecl_ld_local_f32(nrmB + cb_ + 2 * L4);
+                }
+                fl |= ecbn_round_tracked<NCH>(A0, B0, A1, B1, nA0, nB0, nA1, nB1, lane, tol2, big2);
+                fl |= ecbn_round_tracked<NCH>(A0, B1, A1, B0, nA0, nB1, nA1, nB0, lane, tol2, big2);
+                const uint32_t mP = mP0 + nm_, mQ = mQ0 + nm_;
+#pragma unroll
+                for (int c = 0; c < NCH; ++c) {
+                    if (chok[c]) {
+                        const uint32_t aP = dstP + nb_ + cho[c], aQ = dstQ + nb_ + cho[c];
+                        if (Prem) {
+                            ecl_st_async(aP, A0.re[c], mP); ecl_st_async(aP + L4, A0.im[c], mP); ecl_st_async(aP + 2 * L4, A1.re[c], mP); ecl_st_async(aP + 3 * L4, A1.im[c], mP);
+                        } else {
+                            ecl_st_local(aP, A0.re[c]); ecl_st_local(aP + L4, A0.im[c]); ecl_st_local(aP + 2 * L4, A1.re[c]); ecl_st_local(aP + 3 * L4, A1.im[c]);
+                        }
+                        if (Qrem) {
+                            ecl_st_async(aQ, B0.re[c], mQ); ecl_st_async(aQ + L4, B0.im[c], mQ); ecl_st_async(aQ + 2 * L4, B1.re[c], mQ); ecl_st_async(aQ + 3 * L4, B1.im[c], mQ);
+                        } else {
+                            ecl_st_local(aQ, B0.re[c]); ecl_st_local(aQ + L4, B0.im[c]); ecl_st_local(aQ + 2 * L4, B1.re[c]); ecl_st_local(aQ + 3 * L4, B1.im[c]);
+                        }
+                    }
+                }
+                if (lane == 0) {                                     // the norms travel with their columns
+                    const uint32_t nP = dstP + nb_ + 4u * (uint32_t)N, nQ = dstQ + nb_ + 4u * (uint32_t)N;
+                    if (Prem) { ecl_st_async_f32(nP, nA0, mP); ecl_st_async_f32(nP + 2 * L4, nA1, mP); }
+                    else { ecl_st_local_f32(nP, nA0); ecl_st_local_f32(nP + 2 * L4, nA1); }
+                    if (Qrem) { ecl_st_async_f32(nQ, nB0, mQ); ecl_st_async_f32(nQ + 2 * L4, nB1, mQ); }
+                    else { ecl_st_local_f32(nQ, nB0); ecl_st_local_f32(nQ + 2 * L4, nB1); }
+                }
+                __syncwarp();
+                if (lane == 0) {                                     // blocks stored in this CTA: arrive for the whole warp
+                    if (!Prem) ecl_mbar_arrive(mP);
+                    if (!Qrem) ecl_mbar_arrive(mQ);
+                }
+            }
+            b ^= 1;
+        }
+        ++sweep;
+        // stop rule of jacobi_cluster8_kernel over the cluster's CTAs
+        const int mine = __syncthreads_or(fl & 1) + __syncthreads_or(fl & 2);
+        if (tid == 0) {
+            const uint32_t fa = ecl_smem(&flg[(sweep & 1) * ECL8_CS + rank]);
+            for (uint32_t c = 0; c < ECL8_CS; ++c) ecl_st_cluster_f32(ecl_mapa(fa, c), (float)mine);
+        }
+        ecl_cluster_sync();
+        float fmx = 0.f;
+        for (int c = 0; c < (int)ECL8_CS; ++c) fmx = fmaxf(fmx, flg[(sweep & 1) * ECL8_CS + c]);
+        const bool small = fmx < 2.f;
+        if ((last && small) || fmx == 0.f) { converged = 1; break; }
+        if (sweep == a.max_sweeps) break;
+        last = small;
+    }
+
+    if (act) ecl_mbar_wait(full_u32 + 8u * (uint32_t)(b * ECB8_PL + j), ((t - 1) >> 1) & 1u);   // the last step's blocks
+    ecl_cluster_sync();
+    ecl_epilogue(a, k, rank, ECL8_CS, 4 * p0, 4 * npl,
+                 [&](int cl) { return (const float*)(buf + ecb8_slot(b, (cl >> 1) & 1, cl >> 2, cl & 1, LD)); },
+                 lam_s, inv_s, wsl, lsort, ish, shiftv, delta, sweep, converged);
+}
+
 static size_t ecl_smem_bytes(int N, int LD) {
     return (size_t)2 * 2 * ECL_PL * 2 * LD * 4 + 3 * (size_t)N * 4 + 16 + (size_t)N * 8 + 16 + 2 * ECB_PL * 8 + 64 +
            (128 + 4) * 4 + ECB_KC * 4 + (size_t)ECB_KC * 2 * LD * 4 + ECB_KC * 64 * 8 + (size_t)2 * ECB_KC * 2 * LD * 4;   // clean-up workspace
+}
+
+static size_t ecb8_smem_bytes(int N, int LD) {
+    return (size_t)2 * 2 * ECB8_PL * 2 * 2 * LD * 4 + 3 * (size_t)N * 4 + 2 * ECL8_CS * 4 + (size_t)N * 8 + 16 + 2 * ECB8_PL * 8 + 64;
 }
 
 static size_t ecl8_smem_bytes(int N, int LD) {
@@ -1132,9 +1422,13 @@ bool evd_cluster_eligible(const lcf_plan* p) { return p->prec == 0 && (p->N % 2)
 cudaError_t configure_evd_cluster(lcf_plan* p) {
     if (p->N > 128) {
         static_assert(ECL8_MAXN <= 2 * (int)ECL8_CS * ECL8_PL, "ECL8_CS CTAs of ECL8_PL pairs");
-        p->ecl_smem = ecl8_smem_bytes(p->N, p->ec_LD);
+        static_assert(ECL8_MAXN <= 4 * (int)ECL8_CS * ECB8_PL, "ECL8_CS CTAs of ECB8_PL block pairs");
+        const size_t sp = ecl8_smem_bytes(p->N, p->ec_LD), sb = ecb8_smem_bytes(p->N, p->ec_LD);
+        p->ecl_smem = p->N % 4 == 0 ? sb : sp;
         if (p->ecl_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
-        return set_max_dyn_smem(jacobi_cluster8_kernel<4>, p->smem_optin);
+        cudaError_t e8 = set_max_dyn_smem(jacobi_cluster8_kernel<4>, p->smem_optin);
+        if (e8 == cudaSuccess) e8 = set_max_dyn_smem(jacobi_cluster8_block_kernel<2>, p->smem_optin);
+        return e8;
     }
     p->ecl_smem = ecl_smem_bytes(p->N, p->ec_LD);
     if (p->ecl_smem > (size_t)p->smem_optin) return cudaErrorInvalidConfiguration;
@@ -1155,7 +1449,8 @@ cudaError_t launch_evd_cluster(lcf_plan* p, cudaStream_t st) {
     a.V = reinterpret_cast<float2*>(p->V_d); a.B = p->B_d;
     a.mode = evd_mode(p); a.k_fixed = evd_kfixed(p); a.energy_frac = p->thr.energy_frac; a.beta = p->thr.beta; a.cut_scale = p->thr.cut_scale;
     if (p->N > 128) {
-        jacobi_cluster8_kernel<4><<<(int)ECL8_CS * p->K, ECL8_THREADS, p->ecl_smem, st>>>(a);
+        if (p->N % 4 == 0) jacobi_cluster8_block_kernel<2><<<(int)ECL8_CS * p->K, ECB8_THREADS, p->ecl_smem, st>>>(a);
+        else jacobi_cluster8_kernel<4><<<(int)ECL8_CS * p->K, ECL8_THREADS, ecl8_smem_bytes(p->N, p->ec_LD), st>>>(a);
         return cudaGetLastError();
     }
     if (p->N % 4 == 0) {

@@ -176,8 +176,8 @@ SMALL = [
     (40, 40, 16, 1, 1, 0.0, 0.0, synth.HARD_FIXED, 3, 1),         # all-ones window
     (40, 24, 24, 2, 2, 30.0, 0.0, synth.HARD_FIXED, 2, 0),        # Gaussian, no truncation
     (33, 65, 2, 2, 2, 8.0, 3.0, synth.HARD_FIXED, 1, 1),          # N = 2: one rotation, no blocks
-    (96, 80, 140, 2, 2, 20.0, 3.0, synth.HARD_ENERGY, 0, 0),      # N > 128, even: block-form tcgen05 Gram, global-memory Cholesky, Jacobi on 8-CTA clusters
-    (64, 48, 206, 1, 2, 20.0, 3.0, synth.SOFT_ENERGY, 0, 0),      # N = 206: 103 column pairs over eight CTAs (12 + 7 x 13), ragged row chunks
+    (96, 80, 140, 2, 2, 20.0, 3.0, synth.HARD_ENERGY, 0, 0),      # N > 128, N % 4 == 0: block-form tcgen05 Gram, global-memory Cholesky, block-form Jacobi on 8-CTA clusters (35 block pairs: 4-5 per CTA)
+    (64, 48, 206, 1, 2, 20.0, 3.0, synth.SOFT_ENERGY, 0, 0),      # N = 206 (N % 4 == 2): the pair form, 103 column pairs over eight CTAs (12 + 7 x 13), ragged row chunks
     (64, 48, 131, 1, 2, 20.0, 3.0, synth.HARD_ENERGY, 0, 0),      # N > 128, odd: two-sided fp32 Jacobi (3 pivots per lane), 2 Gram batches
     (64, 48, 64, 2, 2, 14.0, 3.0, synth.SOFT_MEDIAN, 0, 0),       # method 3 (median rule) + sigmoid, cluster EVD path
     (64, 48, 40, 2, 2, 14.0, 3.0, synth.HARD_MEDIAN, 0, 1),       # hard median cut (fp64: a hard cut 40 dB down needs it)
